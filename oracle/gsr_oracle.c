@@ -1,0 +1,597 @@
+/*
+ * gsr_oracle.c — the CPU ORACLE for the batched counterfactual-state Gaussian renderer.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  It is a plain, slow, obviously-correct CPU
+ * restatement of what the hot path computes.  It shares no code, header, table or constant with
+ * the CUDA path under paper_2606_17212_b200/csrc/.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may build, load or call it.
+ *
+ * What it follows (PAPER.md = /root/reference/PAPER.md; DESIGN.md §3 = the written spec):
+ *   O-0 activation at load ........ DESIGN.md §3.0      (exp / sigmoid / quaternion -> Sigma; double -> fp32 once)
+ *   O-1 dependency closure ........ PAPER.md:64,164,185 ("usable only when all chunks in its
+ *                                   dependency closure are usable"), BASELINE.json configs[0]
+ *   O-2 deformation ............... PAPER.md:46-50, Eq. (1): mu = A_{c,t} mu_bar + sum_r b_{t,r} q_{i,r}
+ *   O-3 EWA projection ............ PAPER.md:140 delegates to a splatting library and prints nothing;
+ *                                   the definition is the standard EWA one fixed by BASELINE.json
+ *                                   north_star (2) and DESIGN.md §3.3 (every constant is a listed reading)
+ *   O-4 order ..................... north_star (3): (state, tile, depth, gaussian-index), keys unique
+ *   O-5 pixel ..................... north_star (4): per-pixel brute force over ALL depth-sorted Gaussians,
+ *                                   front-to-back alpha compositing with early termination
+ *   O-6 distortion ................ north_star (5): MSE / PSNR against the full-state render
+ *   O-7 utility ................... PAPER.md:80-88, Eq. (3) and Eq. (4) (alpha=0.25, beta=0.05, Q_0.1)
+ *
+ * Precision split.  Quantities that feed an INTEGER decision (deformed mean,
+ * camera-space point, 2-D covariance, conic, radius, tile rectangle, depth bits, the quadratic
+ * form q and the test q > tau) are computed in IEEE binary32 with ONE written operation order
+ * (fmaf explicit, build with -ffp-contract=off) so that another implementation can match them bit
+ * for bit.  Continuous quantities (SH colour, exp(-q), alpha, T, C, SSE) are computed in double
+ * from those fp32 values.
+ *
+ * Parity pins: tests/test_oracle_pins.py (P1..P16 of SURVEY.md §8(c)).  Unpinned: parity with the
+ * PAPER's own pixels/utilities (needs its trained scenes + renderer, which are not available) —
+ * "parity unpinned" for that item only; every function below has at least one pin.
+ *
+ * Build: gcc -O2 -ffp-contract=off -fno-fast-math -mfma -fopenmp -shared -fPIC (see oracle/oracle.py).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define TILE 16
+
+/* ------------------------------------------------------------------------------------------ */
+/* types                                                                                       */
+/* ------------------------------------------------------------------------------------------ */
+
+typedef struct {
+  int32_t C, N, K, R; /* K = (sh_degree+1)^2 coefficients per channel */
+  const int32_t* group_off; /* [4C+1]  Gaussians sorted by (cluster, level) */
+  const float* mean;        /* [N,3]   canonical mu_bar                      */
+  const float* cov3d;       /* [N,6]   activated: xx xy xz yy yz zz          */
+  const float* opacity;     /* [N]     activated sigmoid                     */
+  const float* tau;         /* [N]     ln(255 * opacity)                     */
+  const float* sh_base;     /* [N,K,3]                                       */
+  const float* sh_res;      /* [N,K,3] level-3 payload                       */
+  const int8_t* motion_q;   /* [N,R,3] level-1 payload                       */
+  const float* A0;          /* [C,3,4] */
+  const float* A1;          /* [C,3,4] */
+  const float* motion_scale; /* [C]    */
+  float background[3];
+} orc_scene;
+
+typedef struct {
+  float R[9], t[3], fx, fy, cx, cy;
+  int32_t W, H;
+  float znear;
+} orc_camera;
+
+/* one Gaussian of one state after O-2/O-3 */
+typedef struct {
+  int32_t valid;       /* 1 = present in the state and not culled      */
+  float mu[3];         /* deformed world position (O-2)                */
+  float z;             /* camera-space depth                           */
+  float mx, my;        /* 2-D mean in pixels                           */
+  float qa, qb, qc;    /* A = conic_a/2, B = conic_b, Cq = conic_c/2   */
+  float cov2d[3];      /* a, b, c after the +0.3 dilation              */
+  int32_t radius;      /* ceil(3 sqrt(lambda_max))                     */
+  int32_t rect[4];     /* tx0, ty0, tx1, ty1 (half-open, in tiles)     */
+  uint32_t depth_bits; /* raw bits of z                                */
+  int32_t count;       /* tiles touched                                */
+  double rgb[3];       /* SH colour (continuous)                       */
+} orc_proj;
+
+/* ------------------------------------------------------------------------------------------ */
+/* O-1  dependency closure                               */
+/* ------------------------------------------------------------------------------------------ */
+
+/* mask bit l = "level-l completion group of this cluster is usable".  Level l is renderable iff
+ * levels 0..l are all usable, so the delivered depth is (number of trailing one bits) - 1. */
+void orc_close_levels(const uint8_t* mask, int64_t n, int8_t* depth, uint8_t* closure) {
+  for (int64_t i = 0; i < n; ++i) {
+    int d = -1;
+    for (int l = 0; l < 4; ++l) {
+      if ((mask[i] >> l) & 1)
+        d = l;
+      else
+        break;
+    }
+    depth[i] = (int8_t)d;
+    closure[i] = (uint8_t)((1u << (d + 1)) - 1u);
+  }
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* O-0  activation at load — double, rounded to fp32 once                    */
+/* ------------------------------------------------------------------------------------------ */
+
+void orc_activate(int64_t N, const float* log_scale, const float* quat, const float* logit,
+                  float* cov3d, float* opacity, float* tau) {
+  for (int64_t i = 0; i < N; ++i) {
+    double s[3];
+    for (int k = 0; k < 3; ++k) s[k] = exp((double)log_scale[3 * i + k]);
+    double w = quat[4 * i + 0], x = quat[4 * i + 1], y = quat[4 * i + 2], z = quat[4 * i + 3];
+    double n = sqrt(w * w + x * x + y * y + z * z);
+    w /= n; x /= n; y /= n; z /= n;
+    double Rm[9] = {1.0 - 2.0 * (y * y + z * z), 2.0 * (x * y - w * z),       2.0 * (x * z + w * y),
+                    2.0 * (x * y + w * z),       1.0 - 2.0 * (x * x + z * z), 2.0 * (y * z - w * x),
+                    2.0 * (x * z - w * y),       2.0 * (y * z + w * x),       1.0 - 2.0 * (x * x + y * y)};
+    double M[9]; /* M = Rm * diag(s) */
+    for (int a = 0; a < 3; ++a)
+      for (int k = 0; k < 3; ++k) M[3 * a + k] = Rm[3 * a + k] * s[k];
+    /* Sigma = M M^T */
+    int o = 0;
+    for (int a = 0; a < 3; ++a)
+      for (int b = a; b < 3; ++b) {
+        double acc = M[3 * a + 0] * M[3 * b + 0];
+        acc += M[3 * a + 1] * M[3 * b + 1];
+        acc += M[3 * a + 2] * M[3 * b + 2];
+        cov3d[6 * i + o++] = (float)acc;
+      }
+    float of = (float)(1.0 / (1.0 + exp(-(double)logit[i])));
+    opacity[i] = of;
+    tau[i] = (float)log(255.0 * (double)of);
+  }
+}
+
+/* temporal basis b_r(t) = cos(pi r t), r = 1..R  (reading A6), double -> fp32 */
+void orc_basis(float t, int32_t R, float* b) {
+  for (int r = 1; r <= R; ++r) b[r - 1] = (float)cos(M_PI * (double)r * (double)t);
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* real spherical harmonics to degree 3 (textbook orthonormal basis, DESIGN.md §3.3 colour)    */
+/* ------------------------------------------------------------------------------------------ */
+
+static void sh_basis(int K, double x, double y, double z, double* Y) {
+  const double pi = M_PI;
+  Y[0] = 0.5 * sqrt(1.0 / pi);
+  if (K <= 1) return;
+  double c1 = sqrt(3.0 / (4.0 * pi));
+  Y[1] = c1 * y;
+  Y[2] = c1 * z;
+  Y[3] = c1 * x;
+  if (K <= 4) return;
+  Y[4] = 0.5 * sqrt(15.0 / pi) * x * y;
+  Y[5] = 0.5 * sqrt(15.0 / pi) * y * z;
+  Y[6] = 0.25 * sqrt(5.0 / pi) * (3.0 * z * z - 1.0);
+  Y[7] = 0.5 * sqrt(15.0 / pi) * x * z;
+  Y[8] = 0.25 * sqrt(15.0 / pi) * (x * x - y * y);
+  if (K <= 9) return;
+  Y[9] = 0.25 * sqrt(35.0 / (2.0 * pi)) * y * (3.0 * x * x - y * y);
+  Y[10] = 0.5 * sqrt(105.0 / pi) * x * y * z;
+  Y[11] = 0.25 * sqrt(21.0 / (2.0 * pi)) * y * (5.0 * z * z - 1.0);
+  Y[12] = 0.25 * sqrt(7.0 / pi) * (5.0 * z * z * z - 3.0 * z);
+  Y[13] = 0.25 * sqrt(21.0 / (2.0 * pi)) * x * (5.0 * z * z - 1.0);
+  Y[14] = 0.25 * sqrt(105.0 / pi) * (x * x - y * y) * z;
+  Y[15] = 0.25 * sqrt(35.0 / (2.0 * pi)) * x * (x * x - 3.0 * y * y);
+}
+
+/* exported for the orthonormality pin (P9) */
+void orc_sh_basis(int32_t K, double x, double y, double z, double* Y) { sh_basis(K, x, y, z, Y); }
+
+/* ------------------------------------------------------------------------------------------ */
+/* O-2 + O-3  deformation and EWA projection of Gaussian i in a state whose cluster depth is d */
+/* ------------------------------------------------------------------------------------------ */
+
+static int level_of(const orc_scene* s, int c, int i) {
+  int l = 0;
+  while (l < 3 && i >= s->group_off[4 * c + l + 1]) ++l;
+  return l;
+}
+
+static float clampf(float v, float lo, float hi) { return fminf(hi, fmaxf(lo, v)); }
+
+static void project_one(const orc_scene* s, const orc_camera* cam, float t, const float* basis,
+                        int c, int i, int d, orc_proj* o) {
+  memset(o, 0, sizeof(*o));
+  int lvl = level_of(s, c, i);
+  if (d < lvl) return; /* O-1: present iff d >= level(i); d = -1 removes the whole cluster */
+
+  /* ---- O-2 (Eq. 1): A = A0 + t A1 ; p = A [mu_bar;1] ; residual = s_c * sum_r b_r q_r ---- */
+  const float* A0 = s->A0 + 12 * c;
+  const float* A1 = s->A1 + 12 * c;
+  float A[12];
+  for (int k = 0; k < 12; ++k) A[k] = fmaf(t, A1[k], A0[k]);
+  const float* mb = s->mean + 3 * (int64_t)i;
+  float mu[3];
+  for (int k = 0; k < 3; ++k) {
+    float p = fmaf(A[4 * k + 0], mb[0], fmaf(A[4 * k + 1], mb[1], fmaf(A[4 * k + 2], mb[2], A[4 * k + 3])));
+    if (d >= 1) {
+      float acc = 0.0f;
+      for (int r = 0; r < s->R; ++r)
+        acc = fmaf(basis[r], (float)s->motion_q[((int64_t)i * s->R + r) * 3 + k], acc);
+      p = fmaf(s->motion_scale[c], acc, p);
+    }
+    mu[k] = p;
+    o->mu[k] = p;
+  }
+
+  /* ---- O-3: camera transform ---- */
+  const float* Rw = cam->R;
+  float pc[3];
+  for (int k = 0; k < 3; ++k)
+    pc[k] = fmaf(Rw[3 * k + 0], mu[0], fmaf(Rw[3 * k + 1], mu[1], fmaf(Rw[3 * k + 2], mu[2], cam->t[k])));
+  float z = pc[2];
+  o->z = z;
+  if (!(z > cam->znear)) return;
+  float rz = 1.0f / z;
+  float txz = pc[0] * rz;
+  float tyz = pc[1] * rz;
+  float limx = ((0.5f * (float)cam->W) / cam->fx) * 1.3f;
+  float limy = ((0.5f * (float)cam->H) / cam->fy) * 1.3f;
+  float xt = clampf(txz, -limx, limx) * z;
+  float yt = clampf(tyz, -limy, limy) * z;
+  /* Jacobian of the pinhole projection at the (clamped) point */
+  float J00 = cam->fx * rz;
+  float J02 = -(((cam->fx * xt) * rz) * rz);
+  float J11 = cam->fy * rz;
+  float J12 = -(((cam->fy * yt) * rz) * rz);
+  /* M = J * R_wc  (2x3) */
+  float M0[3], M1[3];
+  for (int k = 0; k < 3; ++k) {
+    M0[k] = fmaf(J02, Rw[6 + k], J00 * Rw[0 + k]);
+    M1[k] = fmaf(J12, Rw[6 + k], J11 * Rw[3 + k]);
+  }
+  /* Sigma' = M Sigma M^T */
+  const float* S6 = s->cov3d + 6 * (int64_t)i;
+  float S[9] = {S6[0], S6[1], S6[2], S6[1], S6[3], S6[4], S6[2], S6[4], S6[5]};
+  float v0[3], v1[3];
+  for (int a = 0; a < 3; ++a) {
+    v0[a] = fmaf(S[3 * a + 2], M0[2], fmaf(S[3 * a + 1], M0[1], S[3 * a + 0] * M0[0]));
+    v1[a] = fmaf(S[3 * a + 2], M1[2], fmaf(S[3 * a + 1], M1[1], S[3 * a + 0] * M1[0]));
+  }
+  float s00 = fmaf(M0[2], v0[2], fmaf(M0[1], v0[1], M0[0] * v0[0]));
+  float s01 = fmaf(M0[2], v1[2], fmaf(M0[1], v1[1], M0[0] * v1[0]));
+  float s11 = fmaf(M1[2], v1[2], fmaf(M1[1], v1[1], M1[0] * v1[0]));
+  float a = s00 + 0.3f, b = s01, cc = s11 + 0.3f; /* reading A11: dilation 0.3 */
+  float det = fmaf(a, cc, -(b * b));
+  if (!(det > 0.0f)) return;
+  float rdet = 1.0f / det;
+  float conic_a = cc * rdet, conic_b = -(b * rdet), conic_c = a * rdet;
+  o->cov2d[0] = a; o->cov2d[1] = b; o->cov2d[2] = cc;
+  o->qa = 0.5f * conic_a;
+  o->qb = conic_b;
+  o->qc = 0.5f * conic_c;
+  float mid = 0.5f * (a + cc);
+  float disc = fmaxf(0.1f, fmaf(mid, mid, -det));
+  float lam = mid + sqrtf(disc);
+  float rad = ceilf(3.0f * sqrtf(lam));
+  o->radius = (int32_t)rad;
+  float mx = fmaf(cam->fx, txz, cam->cx);
+  float my = fmaf(cam->fy, tyz, cam->cy);
+  o->mx = mx;
+  o->my = my;
+  /* tile rectangle (half-open), clamped in float before conversion (reading A15) */
+  float TXf = (float)((cam->W + TILE - 1) / TILE), TYf = (float)((cam->H + TILE - 1) / TILE);
+  int tx0 = (int)clampf(floorf((mx - rad) * 0.0625f), 0.0f, TXf);
+  int tx1 = (int)clampf(floorf(((mx + rad) + 15.0f) * 0.0625f), 0.0f, TXf);
+  int ty0 = (int)clampf(floorf((my - rad) * 0.0625f), 0.0f, TYf);
+  int ty1 = (int)clampf(floorf(((my + rad) + 15.0f) * 0.0625f), 0.0f, TYf);
+  if (tx1 <= tx0 || ty1 <= ty0) return;
+  o->rect[0] = tx0; o->rect[1] = ty0; o->rect[2] = tx1; o->rect[3] = ty1;
+  o->count = (tx1 - tx0) * (ty1 - ty0);
+  memcpy(&o->depth_bits, &z, 4);
+
+  /* ---- colour: degree-L real SH of the view direction, + level-3 residual iff d >= 3 ---- */
+  double cc3[3]; /* camera centre = -R^T t */
+  for (int k = 0; k < 3; ++k)
+    cc3[k] = -((double)Rw[0 + k] * cam->t[0] + (double)Rw[3 + k] * cam->t[1] + (double)Rw[6 + k] * cam->t[2]);
+  double dx = (double)mu[0] - cc3[0], dy = (double)mu[1] - cc3[1], dz = (double)mu[2] - cc3[2];
+  double nrm = sqrt(dx * dx + dy * dy + dz * dz);
+  dx /= nrm; dy /= nrm; dz /= nrm;
+  double Y[16];
+  sh_basis(s->K, dx, dy, dz, Y);
+  for (int ch = 0; ch < 3; ++ch) {
+    double acc = 0.5;
+    for (int j = 0; j < s->K; ++j) {
+      double coef = (double)s->sh_base[((int64_t)i * s->K + j) * 3 + ch];
+      if (d >= 3) coef += (double)s->sh_res[((int64_t)i * s->K + j) * 3 + ch];
+      acc += Y[j] * coef;
+    }
+    o->rgb[ch] = acc > 0.0 ? acc : 0.0;
+  }
+  o->valid = 1;
+}
+
+/* Project every Gaussian of one state.  depth: int8 [C].  out: orc_proj [N]. */
+void orc_project_state(const orc_scene* s, const orc_camera* cam, float t, const int8_t* depth,
+                       orc_proj* out) {
+  float basis[64];
+  orc_basis(t, s->R, basis);
+  for (int c = 0; c < s->C; ++c)
+    for (int i = s->group_off[4 * c]; i < s->group_off[4 * c + 4]; ++i)
+      project_one(s, cam, t, basis, c, i, (int)depth[c], &out[i]);
+}
+
+int32_t orc_sizeof_proj(void) { return (int32_t)sizeof(orc_proj); }
+
+/* ------------------------------------------------------------------------------------------ */
+/* O-4  order: survivors sorted by (depth bits, Gaussian index)                                */
+/* ------------------------------------------------------------------------------------------ */
+
+typedef struct { uint32_t depth_bits; int32_t idx; } order_key;
+
+static int cmp_order(const void* pa, const void* pb) {
+  const order_key* a = (const order_key*)pa;
+  const order_key* b = (const order_key*)pb;
+  if (a->depth_bits != b->depth_bits) return a->depth_bits < b->depth_bits ? -1 : 1;
+  return (a->idx > b->idx) - (a->idx < b->idx);
+}
+
+static int64_t build_order(const orc_proj* p, int32_t N, order_key* ord) {
+  int64_t n = 0;
+  for (int32_t i = 0; i < N; ++i)
+    if (p[i].valid) {
+      ord[n].depth_bits = p[i].depth_bits;
+      ord[n].idx = i;
+      ++n;
+    }
+  qsort(ord, (size_t)n, sizeof(order_key), cmp_order);
+  return n;
+}
+
+/* canonical key list of one state: all (tile, depth bits, index) triples, lexicographic.
+ * Returns the number of keys; writes at most cap of them. tile = ty*TX + tx. */
+typedef struct { uint32_t tile, depth_bits; int32_t idx; } tile_key;
+
+static int cmp_tile_key(const void* pa, const void* pb) {
+  const tile_key* a = (const tile_key*)pa;
+  const tile_key* b = (const tile_key*)pb;
+  if (a->tile != b->tile) return a->tile < b->tile ? -1 : 1;
+  if (a->depth_bits != b->depth_bits) return a->depth_bits < b->depth_bits ? -1 : 1;
+  return (a->idx > b->idx) - (a->idx < b->idx);
+}
+
+int64_t orc_keys_state(const orc_proj* p, int32_t N, int32_t TX, int64_t cap, uint32_t* tile,
+                       uint32_t* depth_bits, int32_t* idx) {
+  int64_t total = 0;
+  for (int32_t i = 0; i < N; ++i)
+    if (p[i].valid) total += p[i].count;
+  if (total > cap) return total;
+  tile_key* keys = (tile_key*)malloc(sizeof(tile_key) * (size_t)(total > 0 ? total : 1));
+  int64_t n = 0;
+  for (int32_t i = 0; i < N; ++i)
+    if (p[i].valid)
+      for (int ty = p[i].rect[1]; ty < p[i].rect[3]; ++ty)
+        for (int tx = p[i].rect[0]; tx < p[i].rect[2]; ++tx) {
+          keys[n].tile = (uint32_t)(ty * TX + tx);
+          keys[n].depth_bits = p[i].depth_bits;
+          keys[n].idx = i;
+          ++n;
+        }
+  qsort(keys, (size_t)n, sizeof(tile_key), cmp_tile_key);
+  for (int64_t k = 0; k < n; ++k) {
+    tile[k] = keys[k].tile;
+    depth_bits[k] = keys[k].depth_bits;
+    idx[k] = keys[k].idx;
+  }
+  free(keys);
+  return n;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* O-5  pixel                                                                                  */
+/* ------------------------------------------------------------------------------------------ */
+
+/* One (pixel, Gaussian) step.  Returns 1 if the pixel terminated at this Gaussian.
+ * px, py = pixel centre.  T, Cacc = the pixel's running transmittance / colour (double). */
+static inline int pixel_step(const orc_proj* g, float opac, float tau, float px, float py, double t_stop,
+                             double* T, double* Cacc, int64_t* evaluated, double* alpha_out) {
+  /* spec-exact fp32 quadratic form: u=A dx; s=fma(B,dy,u); q=s dx; v=Cq dy; q=fma(v,dy,q) */
+  float dx = g->mx - px;
+  float dy = g->my - py;
+  float u = g->qa * dx;
+  float sacc = fmaf(g->qb, dy, u);
+  float q = sacc * dx;
+  float v = g->qc * dy;
+  q = fmaf(v, dy, q);
+  ++*evaluated;
+  if (alpha_out) *alpha_out = 0.0;
+  if (q > tau) return 0; /* alpha < 1/255: skipped (bit-exact decision) */
+  double e = exp(-(double)q);
+  double alpha = (double)opac * e;
+  if (alpha > 0.99) alpha = 0.99;
+  double Tn = *T * (1.0 - alpha);
+  if (Tn < t_stop) return 1; /* stop; this Gaussian is NOT added */
+  if (alpha_out) *alpha_out = alpha;
+  double w = alpha * *T;
+  Cacc[0] += w * g->rgb[0];
+  Cacc[1] += w * g->rgb[1];
+  Cacc[2] += w * g->rgb[2];
+  *T = Tn;
+  return 0;
+}
+
+/* O1: brute force.  For every pixel, walk ALL survivors in depth order; a Gaussian takes part iff
+ * its tile rectangle contains the pixel's tile.  img: double [H,W,3].  stats: [0]=I_b (tile
+ * intersections), [1]=E_b (pairs evaluated).  Tfinal (optional): double [H,W]. */
+void orc_render_O1(const orc_scene* s, const orc_camera* cam, const orc_proj* p, double t_stop, double* img,
+                   int64_t* stats, double* Tfinal) {
+  order_key* ord = (order_key*)malloc(sizeof(order_key) * (size_t)(s->N > 0 ? s->N : 1));
+  int64_t n = build_order(p, s->N, ord);
+  int64_t inter = 0, evaluated = 0;
+  for (int64_t k = 0; k < n; ++k) inter += p[ord[k].idx].count;
+  for (int y = 0; y < cam->H; ++y)
+    for (int x = 0; x < cam->W; ++x) {
+      int tx = x / TILE, ty = y / TILE;
+      float px = (float)x + 0.5f, py = (float)y + 0.5f;
+      double T = 1.0, Cc[3] = {0.0, 0.0, 0.0};
+      for (int64_t k = 0; k < n; ++k) {
+        const orc_proj* g = &p[ord[k].idx];
+        if (tx < g->rect[0] || tx >= g->rect[2] || ty < g->rect[1] || ty >= g->rect[3]) continue;
+        if (pixel_step(g, s->opacity[ord[k].idx], s->tau[ord[k].idx], px, py, t_stop, &T, Cc, &evaluated, NULL))
+          break;
+      }
+      double* o = img + 3 * ((int64_t)y * cam->W + x);
+      for (int ch = 0; ch < 3; ++ch) o[ch] = Cc[ch] + T * (double)s->background[ch];
+      if (Tfinal) Tfinal[(int64_t)y * cam->W + x] = T;
+    }
+  if (stats) { stats[0] = inter; stats[1] = evaluated; }
+  free(ord);
+}
+
+/* O2: the same per-pixel arithmetic sequence, Gaussian-major: walk survivors in depth order and
+ * scatter each into the pixels of its tile rectangle.  Must equal O1 bitwise (pin P11). */
+void orc_render_O2(const orc_scene* s, const orc_camera* cam, const orc_proj* p, double t_stop, double* img,
+                   int64_t* stats, double* Tfinal) {
+  order_key* ord = (order_key*)malloc(sizeof(order_key) * (size_t)(s->N > 0 ? s->N : 1));
+  int64_t n = build_order(p, s->N, ord);
+  int64_t P = (int64_t)cam->W * cam->H;
+  double* T = (double*)malloc(sizeof(double) * (size_t)P);
+  uint8_t* done = (uint8_t*)calloc((size_t)P, 1);
+  for (int64_t k = 0; k < P; ++k) T[k] = 1.0;
+  memset(img, 0, sizeof(double) * 3 * (size_t)P);
+  int64_t inter = 0, evaluated = 0;
+  for (int64_t k = 0; k < n; ++k) {
+    int gi = ord[k].idx;
+    const orc_proj* g = &p[gi];
+    inter += g->count;
+    int x0 = g->rect[0] * TILE, x1 = g->rect[2] * TILE, y0 = g->rect[1] * TILE, y1 = g->rect[3] * TILE;
+    if (x1 > cam->W) x1 = cam->W;
+    if (y1 > cam->H) y1 = cam->H;
+    for (int y = y0; y < y1; ++y)
+      for (int x = x0; x < x1; ++x) {
+        int64_t pix = (int64_t)y * cam->W + x;
+        if (done[pix]) continue;
+        if (pixel_step(g, s->opacity[gi], s->tau[gi], (float)x + 0.5f, (float)y + 0.5f, t_stop, &T[pix],
+                       img + 3 * pix, &evaluated, NULL))
+          done[pix] = 1;
+      }
+  }
+  for (int64_t pix = 0; pix < P; ++pix) {
+    for (int ch = 0; ch < 3; ++ch) img[3 * pix + ch] += T[pix] * (double)s->background[ch];
+    if (Tfinal) Tfinal[pix] = T[pix];
+  }
+  if (stats) { stats[0] = inter; stats[1] = evaluated; }
+  free(ord); free(T); free(done);
+}
+
+/* Per-pixel trace for pins P4/P5/P16: the sequence of Gaussians the pixel meets, with alpha
+ * (0 if skipped) and T after each.  Returns the number of entries (terminating one included,
+ * flagged by alpha = -1). */
+int64_t orc_trace_pixel(const orc_scene* s, const orc_camera* cam, const orc_proj* p, double t_stop, int32_t x,
+                        int32_t y, int64_t cap, int32_t* gidx, double* alpha, double* Tafter) {
+  order_key* ord = (order_key*)malloc(sizeof(order_key) * (size_t)(s->N > 0 ? s->N : 1));
+  int64_t n = build_order(p, s->N, ord);
+  int tx = x / TILE, ty = y / TILE;
+  double T = 1.0, Cc[3] = {0, 0, 0};
+  int64_t m = 0, evaluated = 0;
+  for (int64_t k = 0; k < n; ++k) {
+    const orc_proj* g = &p[ord[k].idx];
+    if (tx < g->rect[0] || tx >= g->rect[2] || ty < g->rect[1] || ty >= g->rect[3]) continue;
+    double a = 0.0;
+    int stop = pixel_step(g, s->opacity[ord[k].idx], s->tau[ord[k].idx], (float)x + 0.5f, (float)y + 0.5f,
+                          t_stop, &T, Cc, &evaluated, &a);
+    if (m < cap) { gidx[m] = ord[k].idx; alpha[m] = stop ? -1.0 : a; Tafter[m] = T; }
+    ++m;
+    if (stop) break;
+  }
+  free(ord);
+  return m;
+}
+
+/* Batch driver (O2 per state, OpenMP over states: states are independent).  levels int8 [B,C];
+ * img double [B,H,W,3]; stats int64 [B,2]. Used for parity tests and as the timed CPU baseline. */
+void orc_render_batch(const orc_scene* s, const orc_camera* cam, float t, const int8_t* levels, int32_t B,
+                      double t_stop, double* img, int64_t* stats, int32_t brute_force) {
+  int64_t P3 = 3 * (int64_t)cam->W * cam->H;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int b = 0; b < B; ++b) {
+    orc_proj* p = (orc_proj*)malloc(sizeof(orc_proj) * (size_t)(s->N > 0 ? s->N : 1));
+    orc_project_state(s, cam, t, levels + (int64_t)b * s->C, p);
+    if (brute_force)
+      orc_render_O1(s, cam, p, t_stop, img + b * P3, stats ? stats + 2 * b : NULL, NULL);
+    else
+      orc_render_O2(s, cam, p, t_stop, img + b * P3, stats ? stats + 2 * b : NULL, NULL);
+    free(p);
+  }
+}
+
+int32_t orc_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* O-6  distortion                                                                             */
+/* ------------------------------------------------------------------------------------------ */
+
+/* imgs: double [B, n] (n = 3*W*H), ref: double [n].  MSE in double; PSNR = -10 log10(max(MSE,1e-10)). */
+void orc_distortion(const double* imgs, const double* ref, int32_t B, int64_t n, double* mse, double* psnr_db) {
+  for (int b = 0; b < B; ++b) {
+    double sse = 0.0;
+    for (int64_t k = 0; k < n; ++k) {
+      double d = imgs[(int64_t)b * n + k] - ref[k];
+      sse += d * d;
+    }
+    mse[b] = sse / (double)n;
+    double m = mse[b] > 1e-10 ? mse[b] : 1e-10;
+    psnr_db[b] = -10.0 * log10(m);
+  }
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* O-7  counterfactual utility: Eq. (3) per pair, Eq. (4) per group          */
+/* ------------------------------------------------------------------------------------------ */
+
+static int cmp_double(const void* a, const void* b) {
+  double x = *(const double*)a, y = *(const double*)b;
+  return (x > y) - (x < y);
+}
+
+/* mean, Q_0.1 (linear interpolation at position 0.1 (n-1) of the sorted samples), population std,
+ * and the risk-adjusted utility of Eq. (4) with alpha = 0.25, beta = 0.05. */
+static void aggregate(double* v, int64_t n, double* out4) {
+  if (n == 0) { out4[0] = out4[1] = out4[2] = out4[3] = 0.0; return; }
+  double mean = 0.0;
+  for (int64_t k = 0; k < n; ++k) mean += v[k];
+  mean /= (double)n;
+  double var = 0.0;
+  for (int64_t k = 0; k < n; ++k) var += (v[k] - mean) * (v[k] - mean);
+  var /= (double)n;
+  double sd = sqrt(var);
+  qsort(v, (size_t)n, sizeof(double), cmp_double);
+  double pos = 0.1 * (double)(n - 1);
+  int64_t lo = (int64_t)floor(pos);
+  int64_t hi = lo + 1 < n ? lo + 1 : n - 1;
+  double fr = pos - (double)lo;
+  double q10 = v[lo] + fr * (v[hi] - v[lo]);
+  const double alpha = 0.25, beta = 0.05;
+  out4[0] = mean;
+  out4[1] = q10;
+  out4[2] = sd;
+  out4[3] = ((1.0 - alpha) * mean + alpha * q10) / (1.0 + beta * sd);
+}
+
+/* mse, psnr: [B].  Pairs: idx_without[p], idx_with[p], group_id[p] in [0,G).
+ * delta_mse[p] = MSE(m) - MSE(m u g) (Eq. 3 with D = MSE); delta_db[p] = PSNR(m u g) - PSNR(m).
+ * util: double [G, 9] = {mean,q10,std,risk}_mse, {mean,q10,std,risk}_dB, count. */
+void orc_group_utility(const double* mse, const double* psnr_db, const int32_t* idx_without,
+                       const int32_t* idx_with, const int32_t* group_id, int64_t n_pairs, int32_t G,
+                       double* delta_mse, double* delta_db, double* util) {
+  for (int64_t p = 0; p < n_pairs; ++p) {
+    delta_mse[p] = mse[idx_without[p]] - mse[idx_with[p]];
+    delta_db[p] = psnr_db[idx_with[p]] - psnr_db[idx_without[p]];
+  }
+  double* buf = (double*)malloc(sizeof(double) * (size_t)(n_pairs > 0 ? n_pairs : 1));
+  for (int g = 0; g < G; ++g) {
+    int64_t n = 0;
+    for (int64_t p = 0; p < n_pairs; ++p)
+      if (group_id[p] == g) buf[n++] = delta_mse[p];
+    aggregate(buf, n, util + 9 * g);
+    n = 0;
+    for (int64_t p = 0; p < n_pairs; ++p)
+      if (group_id[p] == g) buf[n++] = delta_db[p];
+    aggregate(buf, n, util + 9 * g + 4);
+    util[9 * g + 8] = (double)n;
+  }
+  free(buf);
+}

@@ -1,0 +1,221 @@
+"""ctypes front-end of the CPU oracle (oracle/gsr_oracle.c).
+
+TEST INFRASTRUCTURE ONLY.  Importable from tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs — never from the product package.  It does not import the
+product package either; scenes and cameras are duck-typed objects carrying numpy arrays (see
+paper_2606_17212_b200/synth.py for the attribute names).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_SRC = _HERE / "gsr_oracle.c"
+_LIB = _HERE / "libgsr_oracle.so"
+
+CFLAGS = ["-O2", "-ffp-contract=off", "-fno-fast-math", "-mfma", "-fopenmp", "-shared", "-fPIC", "-std=c11",
+          "-D_GNU_SOURCE", "-Wall"]
+
+
+def build(force: bool = False) -> Path:
+    """Compile the oracle with gcc (no CUDA involved)."""
+    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
+        tmp = _LIB.with_suffix(f".tmp{os.getpid()}.so")
+        subprocess.check_call(["gcc", *CFLAGS, str(_SRC), "-o", str(tmp), "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class _Scene(C.Structure):
+    _fields_ = [("C", C.c_int32), ("N", C.c_int32), ("K", C.c_int32), ("R", C.c_int32),
+                ("group_off", C.c_void_p), ("mean", C.c_void_p), ("cov3d", C.c_void_p),
+                ("opacity", C.c_void_p), ("tau", C.c_void_p), ("sh_base", C.c_void_p),
+                ("sh_res", C.c_void_p), ("motion_q", C.c_void_p), ("A0", C.c_void_p), ("A1", C.c_void_p),
+                ("motion_scale", C.c_void_p), ("background", C.c_float * 3)]
+
+
+class _Camera(C.Structure):
+    _fields_ = [("R", C.c_float * 9), ("t", C.c_float * 3), ("fx", C.c_float), ("fy", C.c_float),
+                ("cx", C.c_float), ("cy", C.c_float), ("W", C.c_int32), ("H", C.c_int32),
+                ("znear", C.c_float)]
+
+
+PROJ_DTYPE = np.dtype([("valid", np.int32), ("mu", np.float32, 3), ("z", np.float32), ("mx", np.float32),
+                       ("my", np.float32), ("qa", np.float32), ("qb", np.float32), ("qc", np.float32),
+                       ("cov2d", np.float32, 3), ("radius", np.int32), ("rect", np.int32, 4),
+                       ("depth_bits", np.uint32), ("count", np.int32), ("rgb", np.float64, 3)], align=True)
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = C.CDLL(str(_LIB))
+        _lib.orc_keys_state.restype = C.c_int64
+        _lib.orc_trace_pixel.restype = C.c_int64
+        _lib.orc_sizeof_proj.restype = C.c_int32
+        _lib.orc_num_threads.restype = C.c_int32
+        assert _lib.orc_sizeof_proj() == PROJ_DTYPE.itemsize, (_lib.orc_sizeof_proj(), PROJ_DTYPE.itemsize)
+    return _lib
+
+
+def _p(a: np.ndarray):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _c(a, dtype):
+    return np.ascontiguousarray(a, dtype=dtype)
+
+
+# ------------------------------------------------------------------------------------------------
+def close_levels(mask) -> tuple[np.ndarray, np.ndarray]:
+    """O-1: raw 4-bit delivery masks -> (delivered depth int8 in -1..3, closure bitmask uint8)."""
+    m = _c(mask, np.uint8)
+    depth = np.empty(m.shape, np.int8)
+    closure = np.empty(m.shape, np.uint8)
+    lib().orc_close_levels(_p(m), C.c_int64(m.size), _p(depth), _p(closure))
+    return depth, closure
+
+
+def basis(t: float, R: int) -> np.ndarray:
+    b = np.empty(R, np.float32)
+    lib().orc_basis(C.c_float(t), C.c_int32(R), _p(b))
+    return b
+
+
+def sh_basis(K: int, d) -> np.ndarray:
+    Y = np.zeros(16, np.float64)
+    lib().orc_sh_basis(C.c_int32(K), C.c_double(d[0]), C.c_double(d[1]), C.c_double(d[2]), _p(Y))
+    return Y[:K]
+
+
+def make_camera(cam) -> _Camera:
+    c = _Camera()
+    c.R[:] = [float(v) for v in np.asarray(cam.R_wc, np.float32).reshape(9)]
+    c.t[:] = [float(v) for v in np.asarray(cam.t_wc, np.float32).reshape(3)]
+    c.fx, c.fy, c.cx, c.cy = float(cam.fx), float(cam.fy), float(cam.cx), float(cam.cy)
+    c.W, c.H, c.znear = int(cam.W), int(cam.H), float(cam.znear)
+    return c
+
+
+class OracleScene:
+    """Activated scene (O-0) + the per-state / per-batch oracle calls."""
+
+    def __init__(self, sc):
+        L = lib()
+        self.C, self.N, self.R = int(sc.C), int(sc.N), int(sc.R)
+        self.K = (int(sc.sh_degree) + 1) ** 2
+        self.group_off = _c(sc.group_off, np.int32)
+        self.mean = _c(sc.mean, np.float32)
+        self.sh_base = _c(sc.sh_base, np.float32)
+        self.sh_res = _c(sc.sh_res, np.float32)
+        self.motion_q = _c(sc.motion_q, np.int8)
+        self.A0 = _c(sc.A0, np.float32)
+        self.A1 = _c(sc.A1, np.float32)
+        self.motion_scale = _c(sc.motion_scale, np.float32)
+        self.cov3d = np.empty((self.N, 6), np.float32)
+        self.opacity = np.empty(self.N, np.float32)
+        self.tau = np.empty(self.N, np.float32)
+        ls, qt, lg = _c(sc.log_scale, np.float32), _c(sc.quat, np.float32), _c(sc.opacity_logit, np.float32)
+        L.orc_activate(C.c_int64(self.N), _p(ls), _p(qt), _p(lg), _p(self.cov3d), _p(self.opacity),
+                       _p(self.tau))
+        s = _Scene()
+        s.C, s.N, s.K, s.R = self.C, self.N, self.K, self.R
+        for name in ("group_off", "mean", "cov3d", "opacity", "tau", "sh_base", "sh_res", "motion_q", "A0",
+                     "A1", "motion_scale"):
+            setattr(s, name, getattr(self, name).ctypes.data)
+        s.background[:] = [float(v) for v in np.asarray(sc.background, np.float32)]
+        self._s = s
+
+    # -- O-2/O-3
+    def project(self, cam, t: float, depth) -> np.ndarray:
+        d = _c(depth, np.int8)
+        assert d.shape == (self.C,)
+        out = np.zeros(self.N, PROJ_DTYPE)
+        lib().orc_project_state(C.byref(self._s), C.byref(make_camera(cam)), C.c_float(t), _p(d), _p(out))
+        return out
+
+    # -- O-4
+    def keys(self, proj: np.ndarray, cam) -> tuple[np.ndarray, np.ndarray, np.ndarray]:
+        TX = (int(cam.W) + 15) // 16
+        total = int(proj["count"][proj["valid"] == 1].sum())
+        tile = np.empty(max(total, 1), np.uint32)
+        dbits = np.empty(max(total, 1), np.uint32)
+        idx = np.empty(max(total, 1), np.int32)
+        n = lib().orc_keys_state(_p(proj), C.c_int32(self.N), C.c_int32(TX), C.c_int64(total), _p(tile),
+                                 _p(dbits), _p(idx))
+        assert n == total
+        return tile[:n], dbits[:n], idx[:n]
+
+    # -- O-5
+    def render(self, cam, t: float, depth, brute_force: bool = False, t_stop: float = 1e-4,
+               want_T: bool = False, proj: np.ndarray | None = None):
+        if proj is None:
+            proj = self.project(cam, t, depth)
+        img = np.zeros((cam.H, cam.W, 3), np.float64)
+        stats = np.zeros(2, np.int64)
+        Tf = np.zeros((cam.H, cam.W), np.float64) if want_T else None
+        fn = lib().orc_render_O1 if brute_force else lib().orc_render_O2
+        fn(C.byref(self._s), C.byref(make_camera(cam)), _p(proj), C.c_double(t_stop), _p(img), _p(stats),
+           _p(Tf) if want_T else None)
+        return (img, stats, Tf) if want_T else (img, stats)
+
+    def trace_pixel(self, cam, t: float, depth, x: int, y: int, t_stop: float = 1e-4, cap: int = 4096):
+        proj = self.project(cam, t, depth)
+        g = np.zeros(cap, np.int32)
+        a = np.zeros(cap, np.float64)
+        T = np.zeros(cap, np.float64)
+        n = lib().orc_trace_pixel(C.byref(self._s), C.byref(make_camera(cam)), _p(proj), C.c_double(t_stop),
+                                  C.c_int32(x), C.c_int32(y), C.c_int64(cap), _p(g), _p(a), _p(T))
+        n = min(int(n), cap)
+        return g[:n], a[:n], T[:n]
+
+    def render_batch(self, cam, t: float, levels, brute_force: bool = False, t_stop: float = 1e-4):
+        lv = _c(levels, np.int8)
+        B = lv.shape[0]
+        assert lv.shape == (B, self.C)
+        img = np.zeros((B, cam.H, cam.W, 3), np.float64)
+        stats = np.zeros((B, 2), np.int64)
+        lib().orc_render_batch(C.byref(self._s), C.byref(make_camera(cam)), C.c_float(t), _p(lv), C.c_int32(B),
+                               C.c_double(t_stop), _p(img), _p(stats), C.c_int32(1 if brute_force else 0))
+        return img, stats
+
+
+# -- O-6
+def distortion(imgs, ref) -> tuple[np.ndarray, np.ndarray]:
+    im = _c(imgs, np.float64)
+    B = im.shape[0]
+    rf = _c(ref, np.float64).reshape(-1)
+    im = im.reshape(B, -1)
+    assert im.shape[1] == rf.size
+    mse = np.empty(B, np.float64)
+    psnr = np.empty(B, np.float64)
+    lib().orc_distortion(_p(im), _p(rf), C.c_int32(B), C.c_int64(rf.size), _p(mse), _p(psnr))
+    return mse, psnr
+
+
+# -- O-7
+UTIL_FIELDS = ("mean_mse", "q10_mse", "std_mse", "risk_mse", "mean_db", "q10_db", "std_db", "risk_db", "count")
+
+
+def group_utility(mse, psnr_db, idx_without, idx_with, group_id, G: int):
+    m, p = _c(mse, np.float64), _c(psnr_db, np.float64)
+    a, b, g = _c(idx_without, np.int32), _c(idx_with, np.int32), _c(group_id, np.int32)
+    n = a.size
+    dm = np.empty(max(n, 1), np.float64)
+    dd = np.empty(max(n, 1), np.float64)
+    util = np.zeros((G, 9), np.float64)
+    lib().orc_group_utility(_p(m), _p(p), _p(a), _p(b), _p(g), C.c_int64(n), C.c_int32(G), _p(dm), _p(dd),
+                            _p(util))
+    return dm[:n], dd[:n], util
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
