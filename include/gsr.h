@@ -1,0 +1,216 @@
+/*
+ * gsr.h — C ABI of libgsr: batched counterfactual-state rendering of a clustered dynamic Gaussian
+ * scene on one B200 (sm_100a), per-state distortion and per-group marginal render utility.
+ *
+ * Citations: PAPER.md = the text of arxiv/paper_2606_17212; DESIGN.md §3 = the written spec of every
+ * step (the paper delegates image formation to a splatting library and prints no rasteriser maths,
+ * PAPER.md:140, so each constant is a listed reading there).
+ *
+ * The four calls named by the problem statement ("the same learned scene is evaluated under many
+ * delivery masks ... states are rasterised in one call"; "render paired states with
+ * and without g") are gsr_load_scene, gsr_render_states, gsr_distortion and
+ * gsr_group_utility.  Everything else is a helper around them.
+ *
+ * Conventions
+ *   - Every function returns GSR_OK (0) or a negative GSR_E_* code; gsr_last_error() gives the text
+ *     of the last failure on the calling thread.  Nothing throws, nothing aborts.
+ *   - "dev" pointers are CUDA device pointers owned by the caller (e.g. torch tensors' data_ptr());
+ *     "host" pointers are ordinary host memory.  The library never frees caller memory.
+ *   - Calls that take a `cuda_stream` (a cudaStream_t passed as void*, NULL = the legacy default
+ *     stream) only ENQUEUE work on that stream and return; they allocate nothing.  Errors that can
+ *     only be seen on the device (an out-of-range level, key capacity exceeded) are latched in the
+ *     workspace and read back with gsr_workspace_status().
+ *   - A gsr_scene is immutable after load and may be used from several streams at once; a workspace
+ *     may be used by one call at a time.
+ *   - All images are fp32, layout [B, H, W, 3] (row-major, RGB interleaved), colour range [0,1]
+ *     (not clamped, reading A13).
+ */
+#ifndef GSR_H_
+#define GSR_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GSR_OK 0
+#define GSR_E_INVALID_ARG (-1)         /* NULL pointer, negative size, unsupported R / sh_degree ...   */
+#define GSR_E_INVALID_LEVEL (-2)       /* a levels[] entry outside -1..3 (latched, see status)         */
+#define GSR_E_WORKSPACE_TOO_SMALL (-3) /* ws_bytes below gsr_workspace_bytes, or key capacity exceeded */
+#define GSR_E_CUDA (-4)                /* a CUDA runtime call failed; text in gsr_last_error()         */
+
+#define GSR_TILE 16    /* tile edge in pixels (BASELINE.json north_star (3))   */
+#define GSR_MAX_R 32   /* temporal-basis terms supported                        */
+#define GSR_MAX_SH_DEGREE 3
+
+typedef struct gsr_scene gsr_scene; /* opaque; owns the device copy of the scene */
+
+/* Scene description: host pointers, caller-owned, copied (and activated) by gsr_load_scene.
+ * Gaussians are sorted by (cluster, level): group g = 4*c + l owns [group_off[g], group_off[g+1]).
+ * "Every cluster produces one base completion group and three refinement groups". */
+typedef struct {
+  int32_t C;                  /* clusters                                                      */
+  int32_t N;                  /* Gaussians                                                     */
+  int32_t sh_degree;          /* 0..3; K = (sh_degree+1)^2 coefficients per channel            */
+  int32_t R;                  /* temporal-basis terms of Eq. (1), 1..GSR_MAX_R                  */
+  const int32_t* group_off;   /* [4C+1]                                                        */
+  const float* mean;          /* [N,3]   canonical position mu_bar of Eq. (1)                  */
+  const float* log_scale;     /* [N,3]                                                         */
+  const float* quat;          /* [N,4]   w,x,y,z (need not be normalised)                      */
+  const float* opacity_logit; /* [N]                                                           */
+  const float* sh_base;       /* [N,K,3] base colour coefficients                              */
+  const float* sh_res;        /* [N,K,3] level-3 payload: added iff the cluster's depth is 3   */
+  const int8_t* motion_q;     /* [N,R,3] level-1 payload: q_{i,r} of Eq. (1), int8             */
+  const float* A0;            /* [C,3,4] row-major; A_c(t) = A0 + t*A1 (Eq. (1), reading A6)   */
+  const float* A1;            /* [C,3,4]                                                       */
+  const float* motion_scale;  /* [C]     dequantisation step s_c of the motion residual        */
+  float background[3];
+} gsr_scene_desc;
+
+/* Pinhole camera, OpenCV axes (x right, y down, z forward), pixel centres at +0.5 (reading A9).
+ * p_cam = R_wc * p_world + t_wc. */
+typedef struct {
+  float R_wc[9]; /* row-major */
+  float t_wc[3];
+  float fx, fy, cx, cy;
+  int32_t W, H;
+  float znear; /* Gaussians with z <= znear are culled (0.2 in every config) */
+} gsr_camera;
+
+/* Per-group aggregates of Eq. (3)/(4): mean, 0.10 lower-tail quantile (linear
+ * interpolation), population std and risk-adjusted utility ((1-a)mean + a q10)/(1 + b std) with
+ * a = 0.25, b = 0.05 — once with D = MSE (delta = MSE(m) - MSE(m u g)) and once in dB
+ * (delta = PSNR(m u g) - PSNR(m)). */
+typedef struct {
+  double mean_mse, q10_mse, std_mse, risk_mse;
+  double mean_db, q10_db, std_db, risk_db;
+  double count; /* number of pairs of this group */
+} gsr_utility;
+
+/* ------------------------------------------------------------------------------------------------
+ * gsr_load_scene — DESIGN.md §3.0.  Activates the scene once on the host in double precision
+ * (scale = exp(log_scale); unit quaternion -> rotation; Sigma = R diag(scale^2) R^T;
+ * opacity = sigmoid(logit); tau = ln(255 * opacity)), rounds to fp32, and uploads it in the device
+ * layout of DESIGN.md §5.  Synchronous (cudaMalloc + cudaMemcpy).  *out is NULL on failure.
+ * gsr_free_scene releases it (NULL is allowed). */
+int gsr_load_scene(const gsr_scene_desc* desc, gsr_scene** out);
+void gsr_free_scene(gsr_scene* scene);
+
+/* Bytes of workspace gsr_render_states needs for this scene / camera / batch.  The tile-key
+ * capacity defaults to 12 keys per projected record (+1Mi); gsr_workspace_bytes_ex takes an explicit
+ * capacity (0 = default).  Returns 0 on invalid arguments. */
+size_t gsr_workspace_bytes(const gsr_scene* scene, const gsr_camera* cam, int32_t B);
+size_t gsr_workspace_bytes_ex(const gsr_scene* scene, const gsr_camera* cam, int32_t B, int64_t key_capacity);
+
+/* ------------------------------------------------------------------------------------------------
+ * gsr_render_states — the hot path, BASELINE.json north_star (1)-(4); DESIGN.md §3.1-§3.5.
+ * Renders B partial states of `scene` seen from `cam` at time `t` in one call.
+ *   levels  dev int8 [B, C]  delivered depth of cluster c in state b, -1..3 (reading A3): Gaussian i of
+ *                            cluster c with level l is present iff depth >= l; the motion residual
+ *                            of Eq. (1) is applied iff depth >= 1, the SH residual iff depth == 3.
+ *   out     dev fp32 [B, H, W, 3], or NULL (then only the fused distortion is produced).
+ *   ref     dev fp32 [H, W, 3] or NULL; when given, mse/psnr_db (dev [B]) receive the per-state
+ *           distortion against it, reduced inside the compositing kernel with the same tree as
+ *           gsr_distortion (bitwise equal results).  mse/psnr_db may be NULL iff ref is NULL.
+ *   workspace dev, >= gsr_workspace_bytes(...) bytes, 256-byte aligned.
+ * The result for a state depends only on its row of `levels`: rendering a batch is bitwise equal to
+ * rendering its states one at a time ("CUDA batched/serial equivalence").
+ * Asynchronous on `cuda_stream`.  Device-side failures: see gsr_workspace_status. */
+int gsr_render_states(const gsr_scene* scene, const gsr_camera* cam, float t, const int8_t* levels, int32_t B,
+                      float* out, void* workspace, size_t ws_bytes, void* cuda_stream);
+int gsr_render_states_ex(const gsr_scene* scene, const gsr_camera* cam, float t, const int8_t* levels,
+                         int32_t B, float* out, const float* ref, double* mse, float* psnr_db,
+                         void* workspace, size_t ws_bytes, void* cuda_stream);
+
+/* Synchronises `cuda_stream` and reads the status latched by the last render into `workspace`:
+ * returns GSR_OK, GSR_E_INVALID_LEVEL or GSR_E_WORKSPACE_TOO_SMALL.  keys_needed (host, may be NULL)
+ * receives the number of (tile, depth, record) keys the frame produced. */
+int gsr_workspace_status(const void* workspace, int64_t* keys_needed, void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * gsr_distortion — north_star (5), DESIGN.md §3.6.  Per state b: MSE_b = sum((img_b - ref)^2)/(3HW)
+ * accumulated in double with a fixed reduction tree; PSNR_b = -10 log10(max(MSE_b, 1e-10)).
+ *   imgs dev fp32 [B,H,W,3]; ref dev fp32 [H,W,3]; mse dev double [B]; psnr_db dev fp32 [B].
+ *   workspace dev, >= gsr_distortion_workspace_bytes(B,H,W) bytes.  Asynchronous. */
+size_t gsr_distortion_workspace_bytes(int32_t B, int32_t H, int32_t W);
+int gsr_distortion(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, double* mse,
+                   float* psnr_db, void* workspace, size_t ws_bytes, void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * gsr_group_utility — Eq. (3) and Eq. (4); DESIGN.md §3.7.
+ *   mse dev double [B], psnr_db dev fp32 [B]: distortions of a batch.
+ *   idx_without[p], idx_with[p] (dev int32 [n_pairs]): the states m and m u g of pair p;
+ *   group_id[p] in [0, G).  out dev gsr_utility [G].  delta_mse / delta_db: dev double [n_pairs] or NULL.
+ * Asynchronous; one CTA per group, fixed summation order (deterministic). */
+int gsr_group_utility(const double* mse, const float* psnr_db, const int32_t* idx_without,
+                      const int32_t* idx_with, const int32_t* group_id, int32_t n_pairs, int32_t G,
+                      gsr_utility* out, double* delta_mse, double* delta_db, void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * gsr_close_levels — dependency closure, PAPER.md:185 ("A cluster-layer is usable only when all
+ * chunks in its dependency closure are usable"), chain 0 <- 1 <- 2 <- 3 (reading A8).
+ *   delivered_mask dev uint8 [n], bit l = level-l group usable.
+ *   depth_out dev int8 [n] = (number of trailing one bits) - 1;  closure_out dev uint8 [n] or NULL
+ *   = (1 << (depth+1)) - 1.  Asynchronous. */
+int gsr_close_levels(const uint8_t* delivered_mask, int64_t n, int8_t* depth_out, uint8_t* closure_out,
+                     void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * One-call convenience with HOST buffers (used for the end-to-end measurement): uploads `levels`
+ * and the pair lists, renders the full state (all depths 3) as the reference, renders the batch with
+ * fused distortion, aggregates utilities, and copies mse / psnr_db / util back.  Synchronous.
+ *   levels host int8 [B,C]; idx_without, idx_with, group_id host int32 [n_pairs] (n_pairs may be 0);
+ *   mse host double [B]; psnr_db host float [B]; util host gsr_utility [G] (may be NULL if G == 0);
+ *   out_host: host fp32 [B,H,W,3] or NULL.  workspace dev >= gsr_frame_workspace_bytes(...). */
+size_t gsr_frame_workspace_bytes(const gsr_scene* scene, const gsr_camera* cam, int32_t B, int32_t n_pairs,
+                                 int32_t G, int32_t want_images);
+int gsr_utility_frame_host(const gsr_scene* scene, const gsr_camera* cam, float t, const int8_t* levels,
+                           int32_t B, const int32_t* idx_without, const int32_t* idx_with,
+                           const int32_t* group_id, int32_t n_pairs, int32_t G, double* mse, float* psnr_db,
+                           gsr_utility* util, float* out_host, void* workspace, size_t ws_bytes,
+                           void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * Debug / parity exports (tests only; synchronous unless noted).  They read what the last
+ * gsr_render_states left in `workspace`.
+ *
+ * gsr_debug_projection: per projected record r = 2*i + v (v = 0: geometry without the motion
+ * residual, used when the cluster's depth is 0 — only level-0 Gaussians have it; v = 1: with the
+ * residual, used when depth >= 1).  All host arrays of length 2N (any may be NULL):
+ *   valid u8, radius i32, rect i32 [2N,4] (tx0,ty0,tx1,ty1), depth_bits u32, count i32,
+ *   mean2d f32 [2N,2], conic f32 [2N,3] (A=conic_a/2, B=conic_b, Cq=conic_c/2),
+ *   rgb_base f32 [2N,3], rgb_res f32 [2N,3]. */
+int gsr_debug_projection(const gsr_scene* scene, const void* workspace, uint8_t* valid, int32_t* radius,
+                         int32_t* rect, uint32_t* depth_bits, int32_t* count, float* mean2d, float* conic,
+                         float* rgb_base, float* rgb_res, void* cuda_stream);
+
+/* gsr_debug_keys: the canonical sorted key list (state, tile, depth bits, Gaussian index) of state
+ * `b` of the last rendered batch (north_star (3)).  Writes at most `cap` entries to the host arrays
+ * and returns the list length in *n_keys. */
+int gsr_debug_keys(const gsr_scene* scene, const void* workspace, int32_t b, int64_t cap, uint32_t* tile,
+                   uint32_t* depth_bits, int32_t* gaussian, int64_t* n_keys, void* cuda_stream);
+
+/* gsr_debug_state_counts: per state of the last batch, the number of tile intersections I_b
+ * (= its key-list length).  counts: host int64 [B]. */
+int gsr_debug_state_counts(const gsr_scene* scene, const void* workspace, int64_t* counts, void* cuda_stream);
+
+/* gsr_debug_closure: closed depth / presence predicates the renderer derived from the last `levels`.
+ * depth host int8 [B,C] (as validated). */
+int gsr_debug_closure(const gsr_scene* scene, const void* workspace, int8_t* depth, void* cuda_stream);
+
+/* Tuning knob for experiments: "state_block" = states composited per CTA (1, 4, 8 or 16; default 8).
+ * Results do not depend on it (bitwise). */
+int gsr_set_option(const char* name, int32_t value);
+
+/* Text of the last error on this thread ("" if none). */
+const char* gsr_last_error(void);
+
+/* Library build tag, e.g. "gsr 0.1 sm_100a". */
+const char* gsr_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GSR_H_ */

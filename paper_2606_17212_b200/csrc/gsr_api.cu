@@ -1,0 +1,570 @@
+// gsr_api.cu — the C ABI of include/gsr.h: argument checks, scene activation + upload, workspace
+// carving and the launch sequence of the hot path.  No arithmetic of the method lives here except the
+// load-time activation and the per-call temporal basis / camera centre, which the spec
+// fixes to be evaluated once on the host in double precision and rounded to fp32.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <vector>
+
+#include "gsr_internal.h"
+
+namespace gsr {
+
+static thread_local char g_err[512] = "";
+
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+
+#define GSR_CUDA(call)                                                                      \
+  do {                                                                                      \
+    cudaError_t e_ = (call);                                                                \
+    if (e_ != cudaSuccess) {                                                                \
+      set_error("%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+      return GSR_E_CUDA;                                                                    \
+    }                                                                                       \
+  } while (0)
+
+extern int g_state_block;
+
+long long default_key_capacity(int32_t N) { return 12ll * 2ll * (long long)N + (1ll << 20); }
+
+static size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+
+// Lays the workspace out; with base == nullptr only computes the size.
+size_t carve_workspace(Workspace* ws, void* base, int32_t N, int32_t C, int32_t B, int32_t tiles, long long cap) {
+  char* p = (char*)base;
+  size_t off = 0;
+  auto take = [&](size_t bytes) -> void* {
+    void* r = base ? (void*)(p + off) : nullptr;
+    off += align_up(bytes);
+    return r;
+  };
+  const size_t n_rec = 2 * (size_t)N;
+  Workspace w;
+  w.hdr = (WsHeader*)take(sizeof(WsHeader));
+  w.depth = (int8_t*)take((size_t)B * C);
+  w.r0 = (float4*)take(sizeof(float4) * n_rec);
+  w.r1 = (float4*)take(sizeof(float4) * n_rec);
+  w.rc0 = (float4*)take(sizeof(float4) * n_rec);
+  w.rc1 = (float4*)take(sizeof(float4) * n_rec);
+  w.radius = (int32_t*)take(sizeof(int32_t) * n_rec);
+  w.rect = (uint2*)take(sizeof(uint2) * n_rec);
+  w.depth_bits = (uint32_t*)take(sizeof(uint32_t) * n_rec);
+  w.count = (uint32_t*)take(sizeof(uint32_t) * n_rec);
+  w.offset = (uint32_t*)take(sizeof(uint32_t) * (n_rec + 1));
+  w.scan_blk = (uint32_t*)take(sizeof(uint32_t) * (n_rec / 2048 + 2));
+  for (int k = 0; k < 2; ++k) {
+    w.keys[k] = (unsigned long long*)take(sizeof(unsigned long long) * (size_t)cap);
+    w.vals[k] = (uint32_t*)take(sizeof(uint32_t) * (size_t)cap);
+  }
+  w.hist = (uint32_t*)take(sizeof(uint32_t) * 256 * ((size_t)cap / kSortTileKeys + 2));
+  w.tile_range = (uint2*)take(sizeof(uint2) * (size_t)tiles);
+  w.state_counts = (long long*)take(sizeof(long long) * (size_t)(B > 0 ? B : 1));
+  w.sse_part = (double*)take(sizeof(double) * (size_t)(B > 0 ? B : 1) * tiles);
+  w.bytes = off;
+  if (ws) *ws = w;
+  return off;
+}
+
+struct SceneImpl {
+  DeviceScene d;
+  void* blob = nullptr;  // one device allocation holding every array
+};
+
+static bool camera_ok(const gsr_camera* cam) {
+  return cam && cam->W > 0 && cam->H > 0 && cam->W <= 65535 * kTile && cam->H <= 65535 * kTile && cam->fx > 0 &&
+         cam->fy > 0;
+}
+
+static void make_frame(const SceneImpl* s, const gsr_camera* cam, float t, FrameParams* fp) {
+  memcpy(fp->R, cam->R_wc, sizeof(fp->R));
+  memcpy(fp->t, cam->t_wc, sizeof(fp->t));
+  fp->fx = cam->fx; fp->fy = cam->fy; fp->cx = cam->cx; fp->cy = cam->cy;
+  fp->W = cam->W; fp->H = cam->H;
+  fp->TX = (cam->W + kTile - 1) / kTile;
+  fp->TY = (cam->H + kTile - 1) / kTile;
+  fp->znear = cam->znear;
+  fp->time = t;
+  // temporal basis b_r(t) = cos(pi r t), r = 1..R (reading A6): double -> fp32 once per call
+  for (int r = 0; r < GSR_MAX_R; ++r)
+    fp->basis[r] = r < s->d.R ? (float)cos(M_PI * (double)(r + 1) * (double)t) : 0.0f;
+  // camera centre -R^T t in double -> fp32 (colour only)
+  for (int k = 0; k < 3; ++k) {
+    double c = -((double)cam->R_wc[0 + k] * cam->t_wc[0] + (double)cam->R_wc[3 + k] * cam->t_wc[1] +
+                 (double)cam->R_wc[6 + k] * cam->t_wc[2]);
+    fp->cam_centre[k] = (float)c;
+  }
+  for (int k = 0; k < 3; ++k) fp->bg[k] = s->d.bg[k];
+}
+
+}  // namespace gsr
+
+using namespace gsr;
+
+extern "C" {
+
+struct gsr_scene {
+  SceneImpl impl;
+};
+
+const char* gsr_last_error(void) { return g_err; }
+const char* gsr_version(void) { return "gsr 0.1 sm_100a"; }
+
+int gsr_set_option(const char* name, int value) {
+  if (name && strcmp(name, "state_block") == 0 && (value == 1 || value == 4 || value == 8 || value == 16)) {
+    g_state_block = value;
+    return GSR_OK;
+  }
+  set_error("gsr_set_option: unknown option or value");
+  return GSR_E_INVALID_ARG;
+}
+
+int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
+  if (out) *out = nullptr;
+  if (!d || !out) { set_error("gsr_load_scene: NULL argument"); return GSR_E_INVALID_ARG; }
+  if (d->C <= 0 || d->C > kMaxC || d->N < 0 || d->sh_degree < 0 || d->sh_degree > GSR_MAX_SH_DEGREE || d->R < 1 ||
+      d->R > GSR_MAX_R || d->N > (1 << 28)) {
+    set_error("gsr_load_scene: unsupported sizes C=%d N=%d sh_degree=%d R=%d", d->C, d->N, d->sh_degree, d->R);
+    return GSR_E_INVALID_ARG;
+  }
+  if (!d->group_off || !d->A0 || !d->A1 || !d->motion_scale ||
+      (d->N > 0 && (!d->mean || !d->log_scale || !d->quat || !d->opacity_logit || !d->sh_base || !d->sh_res ||
+                    !d->motion_q))) {
+    set_error("gsr_load_scene: NULL array");
+    return GSR_E_INVALID_ARG;
+  }
+  const int C = d->C, N = d->N, K = (d->sh_degree + 1) * (d->sh_degree + 1), R = d->R;
+  if (d->group_off[0] != 0 || d->group_off[4 * C] != N) {
+    set_error("gsr_load_scene: group_off must start at 0 and end at N");
+    return GSR_E_INVALID_ARG;
+  }
+  for (int g = 0; g < 4 * C; ++g)
+    if (d->group_off[g + 1] < d->group_off[g]) {
+      set_error("gsr_load_scene: group_off not monotone at %d", g);
+      return GSR_E_INVALID_ARG;
+    }
+  const int n_sh4 = (3 * K + 3) / 4, n_qw = (3 * R + 3) / 4;
+  const size_t Np = (size_t)(N > 0 ? N : 1);
+
+  // ---- host staging in the device layout
+  std::vector<float4> g0(Np), g1(Np), g2(Np), shb((size_t)n_sh4 * Np), shr((size_t)n_sh4 * Np);
+  std::vector<uint32_t> qw((size_t)n_qw * Np, 0u);
+  for (int c = 0; c < C; ++c)
+    for (int l = 0; l < 4; ++l)
+      for (int i = d->group_off[4 * c + l]; i < d->group_off[4 * c + l + 1]; ++i) {
+        // DESIGN.md §3.0 activation, double precision, this operation order
+        double s[3];
+        for (int k = 0; k < 3; ++k) s[k] = exp((double)d->log_scale[3 * (size_t)i + k]);
+        double qw_ = d->quat[4 * (size_t)i + 0], qx = d->quat[4 * (size_t)i + 1], qy = d->quat[4 * (size_t)i + 2],
+               qz = d->quat[4 * (size_t)i + 3];
+        const double nrm = sqrt(qw_ * qw_ + qx * qx + qy * qy + qz * qz);
+        qw_ /= nrm; qx /= nrm; qy /= nrm; qz /= nrm;
+        const double Rm[9] = {1.0 - 2.0 * (qy * qy + qz * qz), 2.0 * (qx * qy - qw_ * qz), 2.0 * (qx * qz + qw_ * qy),
+                              2.0 * (qx * qy + qw_ * qz), 1.0 - 2.0 * (qx * qx + qz * qz), 2.0 * (qy * qz - qw_ * qx),
+                              2.0 * (qx * qz - qw_ * qy), 2.0 * (qy * qz + qw_ * qx), 1.0 - 2.0 * (qx * qx + qy * qy)};
+        double M[9];
+        for (int a = 0; a < 3; ++a)
+          for (int k = 0; k < 3; ++k) M[3 * a + k] = Rm[3 * a + k] * s[k];
+        float cov[6];
+        int o = 0;
+        for (int a = 0; a < 3; ++a)
+          for (int b = a; b < 3; ++b) {
+            double acc = M[3 * a + 0] * M[3 * b + 0];
+            acc += M[3 * a + 1] * M[3 * b + 1];
+            acc += M[3 * a + 2] * M[3 * b + 2];
+            cov[o++] = (float)acc;
+          }
+        const float opac = (float)(1.0 / (1.0 + exp(-(double)d->opacity_logit[i])));
+        const float tau = (float)log(255.0 * (double)opac);
+        const uint32_t bits = ((uint32_t)c << 2) | (uint32_t)l;
+        float bitsf;
+        memcpy(&bitsf, &bits, 4);
+        g0[i] = make_float4(d->mean[3 * (size_t)i], d->mean[3 * (size_t)i + 1], d->mean[3 * (size_t)i + 2], opac);
+        g1[i] = make_float4(cov[0], cov[1], cov[2], tau);
+        g2[i] = make_float4(cov[3], cov[4], cov[5], bitsf);
+        for (int w4 = 0; w4 < n_sh4; ++w4) {
+          float vb[4] = {0, 0, 0, 0}, vr[4] = {0, 0, 0, 0};
+          for (int e = 0; e < 4; ++e) {
+            const int flat = 4 * w4 + e;
+            if (flat < 3 * K) {
+              vb[e] = d->sh_base[(size_t)i * 3 * K + flat];
+              vr[e] = d->sh_res[(size_t)i * 3 * K + flat];
+            }
+          }
+          shb[(size_t)w4 * Np + i] = make_float4(vb[0], vb[1], vb[2], vb[3]);
+          shr[(size_t)w4 * Np + i] = make_float4(vr[0], vr[1], vr[2], vr[3]);
+        }
+        for (int byte = 0; byte < 3 * R; ++byte) {
+          const uint32_t v = (uint8_t)d->motion_q[(size_t)i * 3 * R + byte];
+          qw[(size_t)(byte >> 2) * Np + i] |= v << ((byte & 3) * 8);
+        }
+      }
+
+  // ---- one device blob
+  gsr_scene* sc = new (std::nothrow) gsr_scene();
+  if (!sc) { set_error("gsr_load_scene: out of host memory"); return GSR_E_INVALID_ARG; }
+  DeviceScene& D = sc->impl.d;
+  D.C = C; D.N = N; D.K = K; D.R = R; D.sh_degree = d->sh_degree; D.n_sh4 = n_sh4; D.n_qw = n_qw;
+  for (int k = 0; k < 3; ++k) D.bg[k] = d->background[k];
+  size_t off = 0;
+  auto reserve = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
+  const size_t o_g0 = reserve(sizeof(float4) * Np), o_g1 = reserve(sizeof(float4) * Np),
+               o_g2 = reserve(sizeof(float4) * Np), o_shb = reserve(sizeof(float4) * n_sh4 * Np),
+               o_shr = reserve(sizeof(float4) * n_sh4 * Np), o_qw = reserve(sizeof(uint32_t) * n_qw * Np),
+               o_A0 = reserve(sizeof(float) * 12 * C), o_A1 = reserve(sizeof(float) * 12 * C),
+               o_ms = reserve(sizeof(float) * C), o_go = reserve(sizeof(int32_t) * (4 * C + 1));
+  cudaError_t e = cudaMalloc(&sc->impl.blob, off);
+  if (e != cudaSuccess) {
+    set_error("gsr_load_scene: cudaMalloc(%zu) failed: %s", off, cudaGetErrorString(e));
+    delete sc;
+    return GSR_E_CUDA;
+  }
+  char* base = (char*)sc->impl.blob;
+  D.g0 = (float4*)(base + o_g0); D.g1 = (float4*)(base + o_g1); D.g2 = (float4*)(base + o_g2);
+  D.sh_base = (float4*)(base + o_shb); D.sh_res = (float4*)(base + o_shr); D.qw = (uint32_t*)(base + o_qw);
+  D.A0 = (float*)(base + o_A0); D.A1 = (float*)(base + o_A1); D.mscale = (float*)(base + o_ms);
+  D.group_off = (int32_t*)(base + o_go);
+  bool ok = true;
+  auto up = [&](void* dst, const void* src, size_t bytes) {
+    if (bytes && cudaMemcpy(dst, src, bytes, cudaMemcpyHostToDevice) != cudaSuccess) ok = false;
+  };
+  up(D.g0, g0.data(), sizeof(float4) * Np); up(D.g1, g1.data(), sizeof(float4) * Np);
+  up(D.g2, g2.data(), sizeof(float4) * Np);
+  up(D.sh_base, shb.data(), sizeof(float4) * n_sh4 * Np); up(D.sh_res, shr.data(), sizeof(float4) * n_sh4 * Np);
+  up(D.qw, qw.data(), sizeof(uint32_t) * n_qw * Np);
+  up(D.A0, d->A0, sizeof(float) * 12 * C); up(D.A1, d->A1, sizeof(float) * 12 * C);
+  up(D.mscale, d->motion_scale, sizeof(float) * C); up(D.group_off, d->group_off, sizeof(int32_t) * (4 * C + 1));
+  if (!ok) {
+    set_error("gsr_load_scene: upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+    cudaFree(sc->impl.blob);
+    delete sc;
+    return GSR_E_CUDA;
+  }
+  *out = sc;
+  return GSR_OK;
+}
+
+void gsr_free_scene(gsr_scene* scene) {
+  if (!scene) return;
+  if (scene->impl.blob) cudaFree(scene->impl.blob);
+  delete scene;
+}
+
+size_t gsr_workspace_bytes_ex(const gsr_scene* scene, const gsr_camera* cam, int32_t B, int64_t key_capacity) {
+  if (!scene || !camera_ok(cam) || B < 0) return 0;
+  const int tiles = ((cam->W + kTile - 1) / kTile) * ((cam->H + kTile - 1) / kTile);
+  const long long cap = key_capacity > 0 ? key_capacity : default_key_capacity(scene->impl.d.N);
+  if (cap >= (1ll << 31)) return 0;
+  return carve_workspace(nullptr, nullptr, scene->impl.d.N, scene->impl.d.C, B, tiles, cap);
+}
+
+size_t gsr_workspace_bytes(const gsr_scene* scene, const gsr_camera* cam, int32_t B) {
+  return gsr_workspace_bytes_ex(scene, cam, B, 0);
+}
+
+// Recovers the key capacity a workspace of ws_bytes can hold (largest cap whose layout fits).
+static long long capacity_for(const gsr_scene* scene, int tiles, int32_t B, size_t ws_bytes) {
+  const int N = scene->impl.d.N, C = scene->impl.d.C;
+  const long long dflt = default_key_capacity(N);
+  if (carve_workspace(nullptr, nullptr, N, C, B, tiles, dflt) <= ws_bytes) {
+    // grow while it fits (callers that passed gsr_workspace_bytes_ex with a larger capacity)
+    long long lo = dflt, hi = (1ll << 31) - 1;
+    while (lo < hi) {
+      long long mid = lo + (hi - lo + 1) / 2;
+      if (carve_workspace(nullptr, nullptr, N, C, B, tiles, mid) <= ws_bytes) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+  }
+  long long lo = 0, hi = dflt;
+  while (lo < hi) {
+    long long mid = lo + (hi - lo + 1) / 2;
+    if (carve_workspace(nullptr, nullptr, N, C, B, tiles, mid) <= ws_bytes) lo = mid; else hi = mid - 1;
+  }
+  return lo;
+}
+
+int gsr_render_states_ex(const gsr_scene* scene, const gsr_camera* cam, float t, const int8_t* levels, int32_t B,
+                         float* out, const float* ref, double* mse, float* psnr_db, void* workspace,
+                         size_t ws_bytes, void* cuda_stream) {
+  if (!scene || !camera_ok(cam) || B < 0 || (B > 0 && !levels) || !workspace) {
+    set_error("gsr_render_states: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  if (ref && !mse) { set_error("gsr_render_states: ref given without mse"); return GSR_E_INVALID_ARG; }
+  if (((uintptr_t)workspace & 255u) != 0) { set_error("gsr_render_states: workspace must be 256-byte aligned"); return GSR_E_INVALID_ARG; }
+  const SceneImpl* s = &scene->impl;
+  FrameParams fp;
+  make_frame(s, cam, t, &fp);
+  const int tiles = fp.TX * fp.TY;
+  if (carve_workspace(nullptr, nullptr, s->d.N, s->d.C, B, tiles, 1) > ws_bytes) {
+    set_error("gsr_render_states: workspace of %zu bytes is too small", ws_bytes);
+    return GSR_E_WORKSPACE_TOO_SMALL;
+  }
+  const long long cap = capacity_for(scene, tiles, B, ws_bytes);
+  if (cap < 1) { set_error("gsr_render_states: workspace too small"); return GSR_E_WORKSPACE_TOO_SMALL; }
+  Workspace ws;
+  carve_workspace(&ws, workspace, s->d.N, s->d.C, B, tiles, cap);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  launch_init_header(ws, B, s->d.C, s->d.N, fp, cap, st);
+  launch_validate_levels(levels, B, s->d.C, ws, st);                  // a0
+  launch_project(s->d, fp, ws, st);                                   // a1 + a2
+  launch_bin_and_sort(s->d, fp, ws, cap, st);                         // a3
+  launch_composite(s->d, fp, ws, B, out, ref, mse, psnr_db, st);      // a4 (+ fused a5)
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
+int gsr_render_states(const gsr_scene* scene, const gsr_camera* cam, float t, const int8_t* levels, int32_t B,
+                      float* out, void* workspace, size_t ws_bytes, void* cuda_stream) {
+  if (!out) { set_error("gsr_render_states: out is NULL (use gsr_render_states_ex for distortion only)"); return GSR_E_INVALID_ARG; }
+  return gsr_render_states_ex(scene, cam, t, levels, B, out, nullptr, nullptr, nullptr, workspace, ws_bytes,
+                              cuda_stream);
+}
+
+int gsr_workspace_status(const void* workspace, int64_t* keys_needed, void* cuda_stream) {
+  if (!workspace) { set_error("gsr_workspace_status: NULL workspace"); return GSR_E_INVALID_ARG; }
+  WsHeader h;
+  GSR_CUDA(cudaMemcpyAsync(&h, workspace, sizeof(h), cudaMemcpyDeviceToHost, (cudaStream_t)cuda_stream));
+  GSR_CUDA(cudaStreamSynchronize((cudaStream_t)cuda_stream));
+  if (keys_needed) *keys_needed = (int64_t)h.total_keys;
+  if (h.status == GSR_E_WORKSPACE_TOO_SMALL)
+    set_error("key capacity %lld exceeded: the frame produced %llu keys", h.key_capacity, h.total_keys);
+  else if (h.status == GSR_E_INVALID_LEVEL)
+    set_error("levels contains a value outside -1..3");
+  return h.status;
+}
+
+size_t gsr_distortion_workspace_bytes(int32_t B, int32_t H, int32_t W) {
+  if (B < 0 || H <= 0 || W <= 0) return 0;
+  const size_t tiles = (size_t)((W + kTile - 1) / kTile) * ((H + kTile - 1) / kTile);
+  return align_up(sizeof(double) * (size_t)(B > 0 ? B : 1) * tiles);
+}
+
+int gsr_distortion(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, double* mse,
+                   float* psnr_db, void* workspace, size_t ws_bytes, void* cuda_stream) {
+  if (B < 0 || H <= 0 || W <= 0 || (B > 0 && (!imgs || !ref || !mse)) || !workspace) {
+    set_error("gsr_distortion: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  if (ws_bytes < gsr_distortion_workspace_bytes(B, H, W)) {
+    set_error("gsr_distortion: workspace too small");
+    return GSR_E_WORKSPACE_TOO_SMALL;
+  }
+  launch_distortion(imgs, ref, B, H, W, (double*)workspace, mse, psnr_db, (cudaStream_t)cuda_stream);
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
+int gsr_group_utility(const double* mse, const float* psnr_db, const int32_t* idx_without, const int32_t* idx_with,
+                      const int32_t* group_id, int32_t n_pairs, int32_t G, gsr_utility* out, double* delta_mse,
+                      double* delta_db, void* cuda_stream) {
+  if (n_pairs < 0 || G < 0 || (n_pairs > 0 && (!mse || !psnr_db || !idx_without || !idx_with || !group_id)) ||
+      (G > 0 && !out)) {
+    set_error("gsr_group_utility: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  launch_group_utility(mse, psnr_db, idx_without, idx_with, group_id, n_pairs, G, out, delta_mse, delta_db,
+                       (cudaStream_t)cuda_stream);
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
+int gsr_close_levels(const uint8_t* delivered_mask, int64_t n, int8_t* depth_out, uint8_t* closure_out,
+                     void* cuda_stream) {
+  if (n < 0 || (n > 0 && (!delivered_mask || !depth_out))) {
+    set_error("gsr_close_levels: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  launch_close_levels(delivered_mask, n, depth_out, closure_out, (cudaStream_t)cuda_stream);
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// host-buffer convenience call (end-to-end measurement)
+struct FrameCarve {
+  size_t o_render, o_levels, o_full, o_ref, o_mse, o_psnr, o_pairs, o_util, o_out, o_refmse, total;
+};
+
+static FrameCarve carve_frame(const gsr_scene* scene, const gsr_camera* cam, int32_t B, int32_t n_pairs, int32_t G,
+                              int want_images) {
+  FrameCarve f;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
+  const size_t P3 = (size_t)cam->W * cam->H * 3;
+  f.o_render = take(gsr_workspace_bytes(scene, cam, B > 1 ? B : 1));
+  f.o_levels = take((size_t)B * scene->impl.d.C);
+  f.o_full = take((size_t)scene->impl.d.C);
+  f.o_ref = take(sizeof(float) * P3);
+  f.o_mse = take(sizeof(double) * (size_t)(B + 1));
+  f.o_psnr = take(sizeof(float) * (size_t)(B + 1));
+  f.o_pairs = take(sizeof(int32_t) * 3 * (size_t)(n_pairs > 0 ? n_pairs : 1));
+  f.o_util = take(sizeof(gsr_utility) * (size_t)(G > 0 ? G : 1));
+  f.o_out = take(want_images ? sizeof(float) * P3 * (size_t)B : 0);
+  f.o_refmse = take(64);
+  f.total = off;
+  return f;
+}
+
+size_t gsr_frame_workspace_bytes(const gsr_scene* scene, const gsr_camera* cam, int32_t B, int32_t n_pairs,
+                                 int32_t G, int32_t want_images) {
+  if (!scene || !camera_ok(cam) || B < 0 || n_pairs < 0 || G < 0) return 0;
+  return carve_frame(scene, cam, B, n_pairs, G, want_images).total;
+}
+
+int gsr_utility_frame_host(const gsr_scene* scene, const gsr_camera* cam, float t, const int8_t* levels, int32_t B,
+                           const int32_t* idx_without, const int32_t* idx_with, const int32_t* group_id,
+                           int32_t n_pairs, int32_t G, double* mse, float* psnr_db, gsr_utility* util,
+                           float* out_host, void* workspace, size_t ws_bytes, void* cuda_stream) {
+  if (!scene || !camera_ok(cam) || B <= 0 || !levels || !mse || !psnr_db || !workspace || n_pairs < 0 || G < 0 ||
+      (n_pairs > 0 && (!idx_without || !idx_with || !group_id)) || (G > 0 && !util)) {
+    set_error("gsr_utility_frame_host: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  const FrameCarve f = carve_frame(scene, cam, B, n_pairs, G, out_host != nullptr);
+  if (ws_bytes < f.total) { set_error("gsr_utility_frame_host: workspace too small"); return GSR_E_WORKSPACE_TOO_SMALL; }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  char* base = (char*)workspace;
+  const int C = scene->impl.d.C;
+  int8_t* d_levels = (int8_t*)(base + f.o_levels);
+  int8_t* d_full = (int8_t*)(base + f.o_full);
+  float* d_ref = (float*)(base + f.o_ref);
+  double* d_mse = (double*)(base + f.o_mse);
+  float* d_psnr = (float*)(base + f.o_psnr);
+  int32_t* d_pairs = (int32_t*)(base + f.o_pairs);
+  gsr_utility* d_util = (gsr_utility*)(base + f.o_util);
+  float* d_out = out_host ? (float*)(base + f.o_out) : nullptr;
+  void* rws = base + f.o_render;
+  const size_t rws_bytes = gsr_workspace_bytes(scene, cam, B > 1 ? B : 1);
+  GSR_CUDA(cudaMemcpyAsync(d_levels, levels, (size_t)B * C, cudaMemcpyHostToDevice, st));
+  GSR_CUDA(cudaMemsetAsync(d_full, 3, (size_t)C, st));
+  if (n_pairs > 0) {
+    GSR_CUDA(cudaMemcpyAsync(d_pairs, idx_without, sizeof(int32_t) * n_pairs, cudaMemcpyHostToDevice, st));
+    GSR_CUDA(cudaMemcpyAsync(d_pairs + n_pairs, idx_with, sizeof(int32_t) * n_pairs, cudaMemcpyHostToDevice, st));
+    GSR_CUDA(cudaMemcpyAsync(d_pairs + 2 * (size_t)n_pairs, group_id, sizeof(int32_t) * n_pairs, cudaMemcpyHostToDevice, st));
+  }
+  // reference = the full state (reading A16), then the batch with fused distortion
+  int rc = gsr_render_states(scene, cam, t, d_full, 1, d_ref, rws, rws_bytes, st);
+  if (rc != GSR_OK) return rc;
+  rc = gsr_render_states_ex(scene, cam, t, d_levels, B, d_out, d_ref, d_mse, d_psnr, rws, rws_bytes, st);
+  if (rc != GSR_OK) return rc;
+  if (G > 0) {
+    rc = gsr_group_utility(d_mse, d_psnr, d_pairs, d_pairs + n_pairs, d_pairs + 2 * (size_t)n_pairs, n_pairs, G,
+                           d_util, nullptr, nullptr, st);
+    if (rc != GSR_OK) return rc;
+  }
+  GSR_CUDA(cudaMemcpyAsync(mse, d_mse, sizeof(double) * B, cudaMemcpyDeviceToHost, st));
+  GSR_CUDA(cudaMemcpyAsync(psnr_db, d_psnr, sizeof(float) * B, cudaMemcpyDeviceToHost, st));
+  if (G > 0) GSR_CUDA(cudaMemcpyAsync(util, d_util, sizeof(gsr_utility) * G, cudaMemcpyDeviceToHost, st));
+  if (out_host)
+    GSR_CUDA(cudaMemcpyAsync(out_host, d_out, sizeof(float) * 3 * (size_t)cam->W * cam->H * B, cudaMemcpyDeviceToHost, st));
+  return gsr_workspace_status(rws, nullptr, st);
+}
+
+// ------------------------------------------------------------------------------------------------
+// debug / parity exports
+static int ws_from(const gsr_scene* scene, const void* workspace, Workspace* ws, WsHeader* h, cudaStream_t st) {
+  if (!scene || !workspace) { set_error("debug: NULL argument"); return GSR_E_INVALID_ARG; }
+  GSR_CUDA(cudaMemcpyAsync(h, workspace, sizeof(*h), cudaMemcpyDeviceToHost, st));
+  GSR_CUDA(cudaStreamSynchronize(st));
+  if (h->N != scene->impl.d.N || h->C != scene->impl.d.C) { set_error("debug: workspace does not belong to this scene"); return GSR_E_INVALID_ARG; }
+  carve_workspace(ws, const_cast<void*>(workspace), h->N, h->C, h->B, h->TX * h->TY, h->key_capacity);
+  return GSR_OK;
+}
+
+int gsr_debug_projection(const gsr_scene* scene, const void* workspace, uint8_t* valid, int32_t* radius,
+                         int32_t* rect, uint32_t* depth_bits, int32_t* count, float* mean2d, float* conic,
+                         float* rgb_base, float* rgb_res, void* cuda_stream) {
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  Workspace ws; WsHeader h;
+  int rc = ws_from(scene, workspace, &ws, &h, st);
+  if (rc != GSR_OK) return rc;
+  const size_t n = 2 * (size_t)h.N;
+  std::vector<float4> r0(n), r1(n), c0(n), c1(n);
+  std::vector<int32_t> rad(n);
+  std::vector<uint2> rc4(n);
+  std::vector<uint32_t> db(n), cnt(n);
+  GSR_CUDA(cudaMemcpy(r0.data(), ws.r0, sizeof(float4) * n, cudaMemcpyDeviceToHost));
+  GSR_CUDA(cudaMemcpy(r1.data(), ws.r1, sizeof(float4) * n, cudaMemcpyDeviceToHost));
+  GSR_CUDA(cudaMemcpy(c0.data(), ws.rc0, sizeof(float4) * n, cudaMemcpyDeviceToHost));
+  GSR_CUDA(cudaMemcpy(c1.data(), ws.rc1, sizeof(float4) * n, cudaMemcpyDeviceToHost));
+  GSR_CUDA(cudaMemcpy(rad.data(), ws.radius, sizeof(int32_t) * n, cudaMemcpyDeviceToHost));
+  GSR_CUDA(cudaMemcpy(rc4.data(), ws.rect, sizeof(uint2) * n, cudaMemcpyDeviceToHost));
+  GSR_CUDA(cudaMemcpy(db.data(), ws.depth_bits, sizeof(uint32_t) * n, cudaMemcpyDeviceToHost));
+  GSR_CUDA(cudaMemcpy(cnt.data(), ws.count, sizeof(uint32_t) * n, cudaMemcpyDeviceToHost));
+  for (size_t r = 0; r < n; ++r) {
+    if (valid) valid[r] = cnt[r] > 0;
+    if (radius) radius[r] = rad[r];
+    if (rect) {
+      rect[4 * r + 0] = rc4[r].x & 0xFFFF; rect[4 * r + 1] = rc4[r].x >> 16;
+      rect[4 * r + 2] = rc4[r].y & 0xFFFF; rect[4 * r + 3] = rc4[r].y >> 16;
+    }
+    if (depth_bits) depth_bits[r] = db[r];
+    if (count) count[r] = (int32_t)cnt[r];
+    if (mean2d) { mean2d[2 * r] = r0[r].x; mean2d[2 * r + 1] = r0[r].y; }
+    if (conic) { conic[3 * r] = r0[r].z; conic[3 * r + 1] = r0[r].w; conic[3 * r + 2] = r1[r].x; }
+    if (rgb_base) { rgb_base[3 * r] = c0[r].x; rgb_base[3 * r + 1] = c0[r].y; rgb_base[3 * r + 2] = c0[r].z; }
+    if (rgb_res) { rgb_res[3 * r] = c1[r].x; rgb_res[3 * r + 1] = c1[r].y; rgb_res[3 * r + 2] = c1[r].z; }
+  }
+  return GSR_OK;
+}
+
+int gsr_debug_keys(const gsr_scene* scene, const void* workspace, int32_t b, int64_t cap, uint32_t* tile,
+                   uint32_t* depth_bits, int32_t* gaussian, int64_t* n_keys, void* cuda_stream) {
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  Workspace ws; WsHeader h;
+  int rc = ws_from(scene, workspace, &ws, &h, st);
+  if (rc != GSR_OK) return rc;
+  if (b < 0 || b >= h.B || cap < 0 || !n_keys) { set_error("gsr_debug_keys: invalid argument"); return GSR_E_INVALID_ARG; }
+  const size_t m = (size_t)(cap > 0 ? cap : 1);
+  uint32_t *d_tile = nullptr, *d_db = nullptr;
+  int32_t* d_gi = nullptr;
+  unsigned long long* d_n = nullptr;
+  GSR_CUDA(cudaMalloc(&d_tile, 4 * m)); GSR_CUDA(cudaMalloc(&d_db, 4 * m)); GSR_CUDA(cudaMalloc(&d_gi, 4 * m));
+  GSR_CUDA(cudaMalloc(&d_n, 8));
+  launch_filter_keys(scene->impl.d, ws, b, d_tile, d_db, d_gi, d_n, cap, st);
+  unsigned long long n = 0;
+  GSR_CUDA(cudaMemcpyAsync(&n, d_n, 8, cudaMemcpyDeviceToHost, st));
+  GSR_CUDA(cudaStreamSynchronize(st));
+  const size_t ncopy = (size_t)((long long)n < cap ? (long long)n : cap);
+  if (ncopy) {
+    if (tile) GSR_CUDA(cudaMemcpy(tile, d_tile, 4 * ncopy, cudaMemcpyDeviceToHost));
+    if (depth_bits) GSR_CUDA(cudaMemcpy(depth_bits, d_db, 4 * ncopy, cudaMemcpyDeviceToHost));
+    if (gaussian) GSR_CUDA(cudaMemcpy(gaussian, d_gi, 4 * ncopy, cudaMemcpyDeviceToHost));
+  }
+  cudaFree(d_tile); cudaFree(d_db); cudaFree(d_gi); cudaFree(d_n);
+  *n_keys = (int64_t)n;
+  return GSR_OK;
+}
+
+int gsr_debug_state_counts(const gsr_scene* scene, const void* workspace, int64_t* counts, void* cuda_stream) {
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  Workspace ws; WsHeader h;
+  int rc = ws_from(scene, workspace, &ws, &h, st);
+  if (rc != GSR_OK) return rc;
+  if (!counts) { set_error("gsr_debug_state_counts: NULL counts"); return GSR_E_INVALID_ARG; }
+  launch_state_counts(scene->impl.d, ws, h.B, st);
+  GSR_CUDA(cudaMemcpyAsync(counts, ws.state_counts, sizeof(long long) * (size_t)h.B, cudaMemcpyDeviceToHost, st));
+  GSR_CUDA(cudaStreamSynchronize(st));
+  return GSR_OK;
+}
+
+int gsr_debug_closure(const gsr_scene* scene, const void* workspace, int8_t* depth, void* cuda_stream) {
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  Workspace ws; WsHeader h;
+  int rc = ws_from(scene, workspace, &ws, &h, st);
+  if (rc != GSR_OK) return rc;
+  if (!depth) { set_error("gsr_debug_closure: NULL depth"); return GSR_E_INVALID_ARG; }
+  GSR_CUDA(cudaMemcpyAsync(depth, ws.depth, (size_t)h.B * h.C, cudaMemcpyDeviceToHost, st));
+  GSR_CUDA(cudaStreamSynchronize(st));
+  return GSR_OK;
+}
+
+}  // extern "C"

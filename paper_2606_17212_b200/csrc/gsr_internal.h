@@ -1,0 +1,105 @@
+// gsr_internal.h — shared declarations of the CUDA path (NOT shared with oracle/).
+// Spec references: DESIGN.md §3 (written spec), §5 (device layout), §6 (kernels).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "gsr.h"
+
+namespace gsr {
+
+constexpr int kTile = GSR_TILE;
+constexpr int kTilePix = kTile * kTile;  // 256 threads per compositing CTA, one per pixel
+constexpr int kMaxC = 4096;              // clusters (mask table lives in shared memory)
+
+// ---- device scene: SoA of 16-byte words so that every warp load is 512 B contiguous
+struct DeviceScene {
+  int32_t C, N, K, R, sh_degree;
+  int32_t n_sh4;  // float4 words of SH coefficients per Gaussian = ceil(3K/4)
+  int32_t n_qw;   // 32-bit words of int8 motion coefficients per Gaussian = ceil(3R/4)
+  float4* g0;     // [N] mean.xyz, opacity
+  float4* g1;     // [N] Sxx Sxy Sxz, tau
+  float4* g2;     // [N] Syy Syz Szz, bits(cluster<<2 | level)
+  float4* sh_base;  // [n_sh4][N]  flat coefficient index j*3+ch, zero padded
+  float4* sh_res;   // [n_sh4][N]
+  uint32_t* qw;     // [n_qw][N]   int8 q_{i,r,k} at byte (r*3+k)
+  float* A0;        // [C,12]
+  float* A1;        // [C,12]
+  float* mscale;    // [C]
+  int32_t* group_off;  // [4C+1]
+  float bg[3];
+};
+
+// ---- per-call constants passed by value to the kernels
+struct FrameParams {
+  float R[9], t[3];
+  float fx, fy, cx, cy;
+  int32_t W, H, TX, TY;
+  float znear;
+  float time;
+  float basis[GSR_MAX_R];  // b_r(t) = cos(pi r t), r = 1..R, double -> fp32 on the host
+  float cam_centre[3];     // -R^T t, double -> fp32 on the host
+  float bg[3];
+};
+
+// ---- workspace
+struct WsHeader {
+  int32_t status;        // GSR_OK / GSR_E_INVALID_LEVEL / GSR_E_WORKSPACE_TOO_SMALL (latched by kernels)
+  int32_t B, C, N;
+  int32_t W, H, TX, TY;
+  unsigned long long total_keys;  // keys the frame produced (before clamping to capacity)
+  unsigned long long n_keys;      // keys actually sorted (0 if over capacity)
+  long long key_capacity;
+  int32_t pad[16];
+};
+
+struct Workspace {
+  WsHeader* hdr;
+  int8_t* depth;          // [B,C] validated copy of levels
+  float4 *r0, *r1, *rc0, *rc1;  // [2N] projected records
+  int32_t* radius;        // [2N]
+  uint2* rect;            // [2N] 4 x u16: tx0,ty0,tx1,ty1
+  uint32_t* depth_bits;   // [2N]
+  uint32_t* count;        // [2N]
+  uint32_t* offset;       // [2N+1] exclusive scan of count
+  uint32_t* scan_blk;     // block sums of the scan
+  unsigned long long* keys[2];  // [cap] (tile<<32 | depth bits)
+  uint32_t* vals[2];            // [cap] record id
+  uint32_t* hist;         // [256 * n_sort_blocks]
+  uint2* tile_range;      // [tiles] start,end into the sorted list
+  long long* state_counts;  // [B]
+  double* sse_part;       // [B * tiles] per-(state,tile) squared-error partials (fused distortion)
+  size_t bytes;           // total
+};
+
+constexpr int kSortThreads = 256;
+constexpr int kSortItems = 16;
+constexpr int kSortTileKeys = kSortThreads * kSortItems;  // keys per block per pass
+
+size_t carve_workspace(Workspace* ws, void* base, int32_t N, int32_t C, int32_t B, int32_t tiles, long long cap);
+long long default_key_capacity(int32_t N);
+
+// ---- kernel launchers (each only enqueues on `st`)
+void launch_init_header(Workspace& ws, int32_t B, int32_t C, int32_t N, const FrameParams& fp, long long cap,
+                        cudaStream_t st);
+void launch_validate_levels(const int8_t* levels, int32_t B, int32_t C, Workspace& ws, cudaStream_t st);
+void launch_project(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, cudaStream_t st);
+void launch_bin_and_sort(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, long long cap, cudaStream_t st);
+void launch_state_counts(const DeviceScene& sc, Workspace& ws, int32_t B, cudaStream_t st);
+void launch_composite(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, int32_t B, float* out,
+                      const float* ref, double* mse, float* psnr, cudaStream_t st);
+void launch_distortion(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, double* part,
+                       double* mse, float* psnr, cudaStream_t st);
+void launch_distortion_finalize(const double* part, int32_t B, int32_t tiles, int64_t n_values, double* mse,
+                                float* psnr, cudaStream_t st);
+void launch_group_utility(const double* mse, const float* psnr, const int32_t* iwo, const int32_t* iw,
+                          const int32_t* gid, int32_t n_pairs, int32_t G, gsr_utility* out, double* dmse,
+                          double* ddb, cudaStream_t st);
+void launch_close_levels(const uint8_t* mask, int64_t n, int8_t* depth, uint8_t* closure, cudaStream_t st);
+void launch_filter_keys(const DeviceScene& sc, Workspace& ws, int32_t b, uint32_t* tile, uint32_t* dbits,
+                        int32_t* gi, unsigned long long* n_out, long long cap, cudaStream_t st);
+
+void set_error(const char* fmt, ...);
+
+}  // namespace gsr

@@ -1,0 +1,307 @@
+// k_composite.cu — stage a4 (+ fused a5) of the hot path:
+// per-tile front-to-back alpha compositing with early termination, state-blocked.
+//
+// One CTA = one 16x16 tile x S states of the batch; thread = pixel; each thread keeps (T, r, g, b)
+// of its pixel for the S states in registers.  For a record of the tile's depth-sorted superset
+// list, alpha of a (pixel, record) pair does NOT depend on the state — only whether the record is
+// present does, and that is uniform over the CTA (it depends on the cluster's delivered depth in
+// that state).  So alpha is evaluated once and applied to the states in which the record is present:
+//     shared by S states : dx, dy, q (spec-exact fp32), the cut q > tau, exp, alpha, 1-alpha
+//     per present state  : T' = T(1-alpha); stop if T' < 1e-4; C += alpha T c; T = T'
+//
+// Staging: the tile's records are gathered 256 at a time into shared memory; records present in none
+// of the S states are dropped on the way with a warp-ballot ordered compaction.  Warp ballots also
+// (i) skip a record when no pixel of the warp passes the cut and (ii) retire (warp, state) pairs
+// whose 32 pixels have all terminated; the CTA leaves the list when every (pixel, state) is done.
+//
+// Determinism: the arithmetic applied to one (pixel, state) is a fixed sequence of explicitly
+// rounded fp32 operations that depends only on that state's row of `levels`; skipped work is
+// exactly the work that would have been a no-op.  Hence batched == serial bitwise (tests).
+#include "gsr_internal.h"
+#include "reduce.cuh"
+
+namespace gsr {
+
+struct CompositeArgs {
+  const uint2* tile_range;
+  const uint32_t* vals;
+  const float4 *r0, *r1, *rc0, *rc1;
+  const int8_t* depth;
+  int32_t B, C, nsb;
+  int32_t W, H, TX, tiles;
+  float bg[3];
+  float* out;          // [B,H,W,3] or nullptr
+  const float* ref;    // [H,W,3] or nullptr
+  double* sse_part;    // [B, tiles]
+};
+
+constexpr float kTStop = 1e-4f;     // reading A11
+constexpr float kAlphaCap = 0.99f;  // reading A11
+
+template <int S>
+__global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const CompositeArgs a) {
+  extern __shared__ uint16_t s_tab[];  // [C][4]: states (bit s) with depth ==0, >=1, >=2, >=3
+  __shared__ float4 s_r0[kTilePix], s_r1[kTilePix], s_c0[kTilePix], s_c1[kTilePix];
+  __shared__ uint32_t s_wcnt[8];
+  __shared__ double s_red[8][S];
+
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  const int tile = blockIdx.x / a.nsb, sb = blockIdx.x - tile * a.nsb;
+  const int b0 = sb * S;
+
+  // ---- presence masks of this state block (a0: closure predicates)
+  for (int c = tid; c < a.C; c += kTilePix) {
+    uint32_t eq0 = 0, ge1 = 0, ge2 = 0, ge3 = 0;
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+      if (b0 + s < a.B) {
+        const int d = a.depth[(size_t)(b0 + s) * a.C + c];
+        eq0 |= (uint32_t)(d == 0) << s;
+        ge1 |= (uint32_t)(d >= 1) << s;
+        ge2 |= (uint32_t)(d >= 2) << s;
+        ge3 |= (uint32_t)(d >= 3) << s;
+      }
+    }
+    s_tab[4 * c + 0] = (uint16_t)eq0;
+    s_tab[4 * c + 1] = (uint16_t)ge1;
+    s_tab[4 * c + 2] = (uint16_t)ge2;
+    s_tab[4 * c + 3] = (uint16_t)ge3;
+  }
+
+  const int tx = tile % a.TX, ty = tile / a.TX;
+  const int x = tx * kTile + (tid & 15), y = ty * kTile + (tid >> 4);
+  const bool inside = x < a.W && y < a.H;
+  const float px = (float)x + 0.5f, py = (float)y + 0.5f;
+  const float bg0 = a.bg[0], bg1 = a.bg[1], bg2 = a.bg[2];
+
+  float T[S], Cr[S], Cg[S], Cb[S];
+#pragma unroll
+  for (int s = 0; s < S; ++s) {
+    T[s] = (inside && b0 + s < a.B) ? 1.0f : 0.0f;  // T == 0 marks a finished (pixel, state)
+    Cr[s] = Cg[s] = Cb[s] = 0.0f;
+  }
+
+  const uint2 rg = a.tile_range[tile];
+  __syncthreads();
+
+  for (uint32_t base = rg.x; base < rg.y; base += kTilePix) {
+    // ---- stage up to 256 records, dropping those present in no state of the block
+    const uint32_t idx = base + tid;
+    const bool have = idx < rg.y;
+    uint32_t act = 0, res = 0;
+    float4 g0 = make_float4(0, 0, 0, 0), g1 = g0, c0 = g0, c1 = g0;
+    if (have) {
+      const uint32_t rid = __ldg(a.vals + idx);
+      g1 = __ldg(a.r1 + rid);
+      g0 = __ldg(a.r0 + rid);
+      c0 = __ldg(a.rc0 + rid);
+      c1 = __ldg(a.rc1 + rid);
+      const uint32_t meta = __float_as_uint(g1.w);
+      const uint32_t cls = meta >> 16;
+      const uint16_t* t = s_tab + 4 * (meta & 0xFFFFu);
+      act = cls == 0 ? t[0] : (cls <= 2 ? t[1] : (cls == 3 ? t[2] : t[3]));
+      res = cls == 0 ? 0u : t[3];
+    }
+    const bool keep = act != 0;
+    const uint32_t bal = __ballot_sync(0xffffffffu, keep);
+    if (lane == 0) s_wcnt[w] = __popc(bal);
+    __syncthreads();
+    uint32_t woff = 0, nb = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      const uint32_t cnt = s_wcnt[k];
+      if (k < w) woff += cnt;
+      nb += cnt;
+    }
+    if (keep) {
+      const uint32_t pos = woff + __popc(bal & ((1u << lane) - 1u));
+      s_r0[pos] = g0;
+      s_r1[pos] = make_float4(g1.x, g1.y, g1.z, __uint_as_float(act | (res << 16)));
+      s_c0[pos] = c0;
+      s_c1[pos] = c1;
+    }
+    __syncthreads();
+
+    // ---- composite the staged records in order
+    uint32_t walive = 0;
+    for (uint32_t j = 0; j < nb; ++j) {
+      if ((j & 31u) == 0) {  // refresh the (warp, state) liveness mask
+        walive = 0;
+#pragma unroll
+        for (int s = 0; s < S; ++s) walive |= (uint32_t)(__any_sync(0xffffffffu, T[s] > 0.0f) != 0) << s;
+        if (walive == 0) break;
+      }
+      const float4 h1 = s_r1[j];
+      const uint32_t mk = __float_as_uint(h1.w);
+      const uint32_t actw = mk & walive;
+      if (actw == 0) continue;
+      const float4 h0 = s_r0[j];
+      // spec-exact quadratic form: u = A dx; s = fma(B,dy,u); q = s dx; v = Cq dy; q = fma(v,dy,q)
+      const float dx = __fsub_rn(h0.x, px);
+      const float dy = __fsub_rn(h0.y, py);
+      const float u = __fmul_rn(h0.z, dx);
+      const float sacc = __fmaf_rn(h0.w, dy, u);
+      float q = __fmul_rn(sacc, dx);
+      const float v = __fmul_rn(h1.x, dy);
+      q = __fmaf_rn(v, dy, q);
+      const bool pass = !(q > h1.z);  // skip iff q > tau  (alpha < 1/255)
+      if (!__any_sync(0xffffffffu, pass)) continue;
+      float alpha = fminf(kAlphaCap, __fmul_rn(h1.y, __expf(-q)));
+      alpha = pass ? alpha : 0.0f;
+      const float om = __fsub_rn(1.0f, alpha);
+      const float4 k0 = s_c0[j], k1 = s_c1[j];
+      const uint32_t resw = mk >> 16;
+#pragma unroll
+      for (int s = 0; s < S; ++s) {
+        if ((actw >> s) & 1u) {
+          const float Tn = __fmul_rn(T[s], om);
+          if (Tn < kTStop) {
+            if (T[s] > 0.0f) {  // early termination: this record is NOT added; fold the background in
+              Cr[s] = __fmaf_rn(T[s], bg0, Cr[s]);
+              Cg[s] = __fmaf_rn(T[s], bg1, Cg[s]);
+              Cb[s] = __fmaf_rn(T[s], bg2, Cb[s]);
+              T[s] = 0.0f;
+            }
+          } else {
+            const float wgt = __fmul_rn(alpha, T[s]);
+            const bool rs = (resw >> s) & 1u;
+            Cr[s] = __fmaf_rn(wgt, rs ? k1.x : k0.x, Cr[s]);
+            Cg[s] = __fmaf_rn(wgt, rs ? k1.y : k0.y, Cg[s]);
+            Cb[s] = __fmaf_rn(wgt, rs ? k1.z : k0.z, Cb[s]);
+            T[s] = Tn;
+          }
+        }
+      }
+    }
+    bool any_alive = false;
+#pragma unroll
+    for (int s = 0; s < S; ++s) any_alive |= T[s] > 0.0f;
+    if (!__syncthreads_or(any_alive)) break;
+  }
+
+  // ---- pixel = C + T * background; optional fused squared error against the reference
+  float rr0 = 0.f, rr1 = 0.f, rr2 = 0.f;
+  if (a.ref && inside) {
+    const float* rp = a.ref + ((size_t)y * a.W + x) * 3;
+    rr0 = __ldg(rp); rr1 = __ldg(rp + 1); rr2 = __ldg(rp + 2);
+  }
+#pragma unroll
+  for (int s = 0; s < S; ++s) {
+    const float o0 = __fmaf_rn(T[s], bg0, Cr[s]);
+    const float o1 = __fmaf_rn(T[s], bg1, Cg[s]);
+    const float o2 = __fmaf_rn(T[s], bg2, Cb[s]);
+    if (a.out && inside && b0 + s < a.B) {
+      float* op = a.out + (((size_t)(b0 + s) * a.H + y) * a.W + x) * 3;
+      op[0] = o0; op[1] = o1; op[2] = o2;
+    }
+    if (a.ref) {
+      const float e = inside ? pixel_sq_err(o0, o1, o2, rr0, rr1, rr2) : 0.0f;
+      const double ws = warp_sum_butterfly((double)e);
+      if (lane == 0) s_red[w][s] = ws;
+    }
+  }
+  if (a.ref) {
+    __syncthreads();
+    if (tid < S && b0 + tid < a.B) {
+      double acc = s_red[0][tid];
+#pragma unroll
+      for (int k = 1; k < 8; ++k) acc += s_red[k][tid];
+      a.sse_part[(size_t)(b0 + tid) * a.tiles + tile] = acc;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// gsr_distortion (unfused): same pixel->thread mapping and the same tree as the fused path
+__global__ void __launch_bounds__(kTilePix) k_distortion_tiles(const float* __restrict__ imgs,
+                                                               const float* __restrict__ ref, int W, int H,
+                                                               int TX, int tiles, double* __restrict__ part) {
+  __shared__ double s_red[8];
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  const int tile = blockIdx.x, b = blockIdx.y;
+  const int x = (tile % TX) * kTile + (tid & 15), y = (tile / TX) * kTile + (tid >> 4);
+  float e = 0.0f;
+  if (x < W && y < H) {
+    const size_t p = ((size_t)y * W + x) * 3;
+    const float* ip = imgs + (size_t)b * H * W * 3 + p;
+    e = pixel_sq_err(ip[0], ip[1], ip[2], __ldg(ref + p), __ldg(ref + p + 1), __ldg(ref + p + 2));
+  }
+  const double ws = warp_sum_butterfly((double)e);
+  if (lane == 0) s_red[w] = ws;
+  __syncthreads();
+  if (tid == 0) {
+    double acc = s_red[0];
+#pragma unroll
+    for (int k = 1; k < 8; ++k) acc += s_red[k];
+    part[(size_t)b * tiles + tile] = acc;
+  }
+}
+
+// one warp per state: tiles in index order (lane-strided), then the butterfly; MSE and PSNR
+__global__ void __launch_bounds__(128) k_distortion_finalize(const double* __restrict__ part, int B, int tiles,
+                                                             double inv_n, double* __restrict__ mse,
+                                                             float* __restrict__ psnr) {
+  const int b = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (b >= B) return;
+  double acc = 0.0;
+  for (int k = lane; k < tiles; k += 32) acc += part[(size_t)b * tiles + k];
+  acc = warp_sum_butterfly(acc);
+  if (lane == 0) {
+    const double m = acc * inv_n;
+    mse[b] = m;
+    if (psnr) psnr[b] = (float)(-10.0 * log10(m > 1e-10 ? m : 1e-10));
+  }
+}
+
+void launch_distortion_finalize(const double* part, int32_t B, int32_t tiles, int64_t n_values, double* mse,
+                                float* psnr, cudaStream_t st) {
+  if (B == 0) return;
+  k_distortion_finalize<<<(B + 3) / 4, 128, 0, st>>>(part, B, tiles, 1.0 / (double)n_values, mse, psnr);
+}
+
+void launch_distortion(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, double* part,
+                       double* mse, float* psnr, cudaStream_t st) {
+  if (B == 0) return;
+  const int TX = (W + kTile - 1) / kTile, TY = (H + kTile - 1) / kTile, tiles = TX * TY;
+  for (int b0 = 0; b0 < B; b0 += 65535) {  // gridDim.y limit
+    const int nb = B - b0 < 65535 ? B - b0 : 65535;
+    k_distortion_tiles<<<dim3(tiles, nb), kTilePix, 0, st>>>(imgs + (size_t)b0 * H * W * 3, ref, W, H, TX, tiles,
+                                                            part + (size_t)b0 * tiles);
+  }
+  launch_distortion_finalize(part, B, tiles, (int64_t)3 * W * H, mse, psnr, st);
+}
+
+template <int S>
+static void launch_composite_S(const CompositeArgs& a, cudaStream_t st) {
+  const size_t smem = sizeof(uint16_t) * 4 * (size_t)a.C;
+  const long long grid = (long long)a.tiles * a.nsb;
+  k_composite<S><<<(unsigned)grid, kTilePix, smem, st>>>(a);
+}
+
+int g_state_block = 8;  // S; set through gsr_set_option for experiments (1, 4, 8, 16)
+
+void launch_composite(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, int32_t B, float* out,
+                      const float* ref, double* mse, float* psnr, cudaStream_t st) {
+  if (B == 0) return;
+  CompositeArgs a;
+  a.tile_range = ws.tile_range;
+  a.vals = ws.vals[0];
+  a.r0 = ws.r0; a.r1 = ws.r1; a.rc0 = ws.rc0; a.rc1 = ws.rc1;
+  a.depth = ws.depth;
+  a.B = B; a.C = sc.C;
+  a.W = fp.W; a.H = fp.H; a.TX = fp.TX; a.tiles = fp.TX * fp.TY;
+  a.bg[0] = fp.bg[0]; a.bg[1] = fp.bg[1]; a.bg[2] = fp.bg[2];
+  a.out = out; a.ref = ref; a.sse_part = ws.sse_part;
+  int S = g_state_block;
+  if (B == 1) S = 1;
+  a.nsb = (B + S - 1) / S;
+  switch (S) {
+    case 1: launch_composite_S<1>(a, st); break;
+    case 4: launch_composite_S<4>(a, st); break;
+    case 16: launch_composite_S<16>(a, st); break;
+    default: launch_composite_S<8>(a, st); break;
+  }
+  if (ref) launch_distortion_finalize(ws.sse_part, B, a.tiles, (int64_t)3 * fp.W * fp.H, mse, psnr, st);
+}
+
+}  // namespace gsr

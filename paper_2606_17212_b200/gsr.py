@@ -1,0 +1,286 @@
+"""Thin ctypes binding of libgsr.so (include/gsr.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C ABI.  PyTorch is used for device
+memory and streams only.  There is NO CPU fallback: importing this module without the built
+extension, or calling it without a CUDA device, raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+
+_PKG = Path(__file__).resolve().parent
+LIB_PATH = _PKG / "libgsr.so"
+
+GSR_OK, GSR_E_INVALID_ARG, GSR_E_INVALID_LEVEL, GSR_E_WORKSPACE_TOO_SMALL, GSR_E_CUDA = 0, -1, -2, -3, -4
+
+
+class GsrError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"gsr error {code}: {msg}")
+        self.code = code
+
+
+class SceneDesc(C.Structure):
+    _fields_ = [("C", C.c_int32), ("N", C.c_int32), ("sh_degree", C.c_int32), ("R", C.c_int32),
+                ("group_off", C.c_void_p), ("mean", C.c_void_p), ("log_scale", C.c_void_p), ("quat", C.c_void_p),
+                ("opacity_logit", C.c_void_p), ("sh_base", C.c_void_p), ("sh_res", C.c_void_p),
+                ("motion_q", C.c_void_p), ("A0", C.c_void_p), ("A1", C.c_void_p), ("motion_scale", C.c_void_p),
+                ("background", C.c_float * 3)]
+
+
+class CameraC(C.Structure):
+    _fields_ = [("R_wc", C.c_float * 9), ("t_wc", C.c_float * 3), ("fx", C.c_float), ("fy", C.c_float),
+                ("cx", C.c_float), ("cy", C.c_float), ("W", C.c_int32), ("H", C.c_int32), ("znear", C.c_float)]
+
+
+UTILITY_DTYPE = np.dtype([(n, np.float64) for n in
+                          ("mean_mse", "q10_mse", "std_mse", "risk_mse", "mean_db", "q10_db", "std_db", "risk_db",
+                           "count")])
+
+_lib = None
+
+
+def lib():
+    """Loads libgsr.so; fails loudly if it has not been built (python -m paper_2606_17212_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not LIB_PATH.exists():
+            raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2606_17212_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(str(LIB_PATH))
+        vp, i32, i64, sz, f32 = C.c_void_p, C.c_int32, C.c_int64, C.c_size_t, C.c_float
+        L.gsr_last_error.restype = C.c_char_p
+        L.gsr_version.restype = C.c_char_p
+        L.gsr_load_scene.argtypes = [C.POINTER(SceneDesc), C.POINTER(vp)]
+        L.gsr_free_scene.argtypes = [vp]
+        L.gsr_free_scene.restype = None
+        L.gsr_workspace_bytes.argtypes = [vp, C.POINTER(CameraC), i32]
+        L.gsr_workspace_bytes.restype = sz
+        L.gsr_workspace_bytes_ex.argtypes = [vp, C.POINTER(CameraC), i32, i64]
+        L.gsr_workspace_bytes_ex.restype = sz
+        L.gsr_render_states.argtypes = [vp, C.POINTER(CameraC), f32, vp, i32, vp, vp, sz, vp]
+        L.gsr_render_states_ex.argtypes = [vp, C.POINTER(CameraC), f32, vp, i32, vp, vp, vp, vp, vp, sz, vp]
+        L.gsr_workspace_status.argtypes = [vp, C.POINTER(i64), vp]
+        L.gsr_distortion_workspace_bytes.argtypes = [i32, i32, i32]
+        L.gsr_distortion_workspace_bytes.restype = sz
+        L.gsr_distortion.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp, sz, vp]
+        L.gsr_group_utility.argtypes = [vp, vp, vp, vp, vp, i32, i32, vp, vp, vp, vp]
+        L.gsr_close_levels.argtypes = [vp, i64, vp, vp, vp]
+        L.gsr_frame_workspace_bytes.argtypes = [vp, C.POINTER(CameraC), i32, i32, i32, i32]
+        L.gsr_frame_workspace_bytes.restype = sz
+        L.gsr_utility_frame_host.argtypes = [vp, C.POINTER(CameraC), f32, vp, i32, vp, vp, vp, i32, i32, vp, vp, vp,
+                                             vp, vp, sz, vp]
+        L.gsr_debug_projection.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+        L.gsr_debug_keys.argtypes = [vp, vp, i32, i64, vp, vp, vp, C.POINTER(i64), vp]
+        L.gsr_debug_state_counts.argtypes = [vp, vp, vp, vp]
+        L.gsr_debug_closure.argtypes = [vp, vp, vp, vp]
+        L.gsr_set_option.argtypes = [C.c_char_p, i32]
+        _lib = L
+    return _lib
+
+
+def _check(rc: int):
+    if rc != GSR_OK:
+        raise GsrError(rc, lib().gsr_last_error().decode())
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("gsr needs a CUDA device (no CPU fallback)")
+    return torch
+
+
+def _stream():
+    return C.c_void_p(_torch().cuda.current_stream().cuda_stream)
+
+
+def _np(a, dtype):
+    return np.ascontiguousarray(a, dtype=dtype)
+
+
+def _hp(a: np.ndarray):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _dp(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else None
+
+
+def camera_struct(cam) -> CameraC:
+    c = CameraC()
+    c.R_wc[:] = [float(v) for v in np.asarray(cam.R_wc, np.float32).reshape(9)]
+    c.t_wc[:] = [float(v) for v in np.asarray(cam.t_wc, np.float32).reshape(3)]
+    c.fx, c.fy, c.cx, c.cy = float(cam.fx), float(cam.fy), float(cam.cx), float(cam.cy)
+    c.W, c.H, c.znear = int(cam.W), int(cam.H), float(cam.znear)
+    return c
+
+
+def set_option(name: str, value: int):
+    _check(lib().gsr_set_option(name.encode(), int(value)))
+
+
+class Scene:
+    """gsr_load_scene / gsr_free_scene.  `sc` carries the arrays of gsr_scene_desc as numpy attributes."""
+
+    def __init__(self, sc):
+        _torch().cuda.init()
+        self.C, self.N, self.R, self.sh_degree = int(sc.C), int(sc.N), int(sc.R), int(sc.sh_degree)
+        keep = dict(group_off=_np(sc.group_off, np.int32), mean=_np(sc.mean, np.float32),
+                    log_scale=_np(sc.log_scale, np.float32), quat=_np(sc.quat, np.float32),
+                    opacity_logit=_np(sc.opacity_logit, np.float32), sh_base=_np(sc.sh_base, np.float32),
+                    sh_res=_np(sc.sh_res, np.float32), motion_q=_np(sc.motion_q, np.int8),
+                    A0=_np(sc.A0, np.float32), A1=_np(sc.A1, np.float32),
+                    motion_scale=_np(sc.motion_scale, np.float32))
+        d = SceneDesc()
+        d.C, d.N, d.sh_degree, d.R = self.C, self.N, self.sh_degree, self.R
+        for k, v in keep.items():
+            setattr(d, k, v.ctypes.data)
+        d.background[:] = [float(v) for v in np.asarray(sc.background, np.float32)]
+        h = C.c_void_p()
+        _check(lib().gsr_load_scene(C.byref(d), C.byref(h)))
+        self.handle = h
+
+    def close(self):
+        if getattr(self, "handle", None):
+            lib().gsr_free_scene(self.handle)
+            self.handle = None
+
+    __del__ = close
+
+    # ---- workspace
+    def workspace_bytes(self, cam, B: int, key_capacity: int = 0) -> int:
+        n = lib().gsr_workspace_bytes_ex(self.handle, C.byref(camera_struct(cam)), int(B), int(key_capacity))
+        if n == 0:
+            raise GsrError(GSR_E_INVALID_ARG, "gsr_workspace_bytes: invalid arguments")
+        return int(n)
+
+    def new_workspace(self, cam, B: int, key_capacity: int = 0):
+        torch = _torch()
+        return torch.empty(self.workspace_bytes(cam, B, key_capacity), dtype=torch.uint8, device="cuda")
+
+    # ---- hot path
+    def render_states(self, cam, t: float, levels, out=None, workspace=None, ref=None, mse=None, psnr=None,
+                      want_images: bool = True):
+        """gsr_render_states(_ex).  levels: cuda int8 [B,C].  Returns (out, mse, psnr) (entries may be None)."""
+        torch = _torch()
+        B = int(levels.shape[0])
+        assert levels.dtype == torch.int8 and levels.is_cuda and levels.is_contiguous()
+        assert levels.shape[1] == self.C
+        if workspace is None:
+            workspace = self.new_workspace(cam, B)
+        if out is None and want_images:
+            out = torch.empty((B, cam.H, cam.W, 3), dtype=torch.float32, device="cuda")
+        if ref is not None:
+            assert ref.dtype == torch.float32 and ref.is_cuda and ref.is_contiguous()
+            if mse is None:
+                mse = torch.empty(B, dtype=torch.float64, device="cuda")
+            if psnr is None:
+                psnr = torch.empty(B, dtype=torch.float32, device="cuda")
+        _check(lib().gsr_render_states_ex(self.handle, C.byref(camera_struct(cam)), C.c_float(t), _dp(levels), B,
+                                          _dp(out), _dp(ref), _dp(mse), _dp(psnr), _dp(workspace),
+                                          workspace.numel(), _stream()))
+        return out, mse, psnr
+
+    def status(self, workspace) -> int:
+        """gsr_workspace_status: synchronises; raises on a latched device-side error; returns #keys."""
+        n = C.c_int64(0)
+        _check(lib().gsr_workspace_status(_dp(workspace), C.byref(n), _stream()))
+        return int(n.value)
+
+    # ---- host-buffer convenience call
+    def utility_frame_host(self, cam, t: float, levels_host: np.ndarray, idx_without, idx_with, group_id, G: int,
+                           workspace=None, want_images: bool = False):
+        torch = _torch()
+        lv = _np(levels_host, np.int8)
+        B = lv.shape[0]
+        iwo, iw, gid = _np(idx_without, np.int32), _np(idx_with, np.int32), _np(group_id, np.int32)
+        n_pairs = int(iwo.size)
+        camc = camera_struct(cam)
+        need = lib().gsr_frame_workspace_bytes(self.handle, C.byref(camc), B, n_pairs, G, int(want_images))
+        if workspace is None or workspace.numel() < need:
+            workspace = torch.empty(need, dtype=torch.uint8, device="cuda")
+        mse = np.empty(B, np.float64)
+        psnr = np.empty(B, np.float32)
+        util = np.zeros(max(G, 1), UTILITY_DTYPE)
+        out = np.empty((B, cam.H, cam.W, 3), np.float32) if want_images else None
+        _check(lib().gsr_utility_frame_host(self.handle, C.byref(camc), C.c_float(t), _hp(lv), B, _hp(iwo), _hp(iw),
+                                            _hp(gid), n_pairs, G, _hp(mse), _hp(psnr), _hp(util),
+                                            _hp(out) if out is not None else None, _dp(workspace),
+                                            workspace.numel(), _stream()))
+        return mse, psnr, util[:G], out, workspace
+
+    # ---- debug / parity exports
+    def debug_projection(self, workspace) -> dict:
+        n = 2 * self.N
+        o = dict(valid=np.zeros(n, np.uint8), radius=np.zeros(n, np.int32), rect=np.zeros((n, 4), np.int32),
+                 depth_bits=np.zeros(n, np.uint32), count=np.zeros(n, np.int32), mean2d=np.zeros((n, 2), np.float32),
+                 conic=np.zeros((n, 3), np.float32), rgb_base=np.zeros((n, 3), np.float32),
+                 rgb_res=np.zeros((n, 3), np.float32))
+        _check(lib().gsr_debug_projection(self.handle, _dp(workspace), _hp(o["valid"]), _hp(o["radius"]),
+                                          _hp(o["rect"]), _hp(o["depth_bits"]), _hp(o["count"]), _hp(o["mean2d"]),
+                                          _hp(o["conic"]), _hp(o["rgb_base"]), _hp(o["rgb_res"]), _stream()))
+        return o
+
+    def debug_keys(self, workspace, b: int, cap: int):
+        tile = np.zeros(max(cap, 1), np.uint32)
+        dbits = np.zeros(max(cap, 1), np.uint32)
+        gi = np.zeros(max(cap, 1), np.int32)
+        n = C.c_int64(0)
+        _check(lib().gsr_debug_keys(self.handle, _dp(workspace), int(b), int(cap), _hp(tile), _hp(dbits), _hp(gi),
+                                    C.byref(n), _stream()))
+        m = min(int(n.value), cap)
+        return tile[:m], dbits[:m], gi[:m], int(n.value)
+
+    def debug_state_counts(self, workspace, B: int) -> np.ndarray:
+        c = np.zeros(B, np.int64)
+        _check(lib().gsr_debug_state_counts(self.handle, _dp(workspace), _hp(c), _stream()))
+        return c
+
+    def debug_closure(self, workspace, B: int) -> np.ndarray:
+        d = np.zeros((B, self.C), np.int8)
+        _check(lib().gsr_debug_closure(self.handle, _dp(workspace), _hp(d), _stream()))
+        return d
+
+
+def distortion(imgs, ref, workspace=None):
+    """gsr_distortion: imgs cuda f32 [B,H,W,3], ref cuda f32 [H,W,3] -> (mse f64 [B], psnr f32 [B]) on device."""
+    torch = _torch()
+    B, H, W = int(imgs.shape[0]), int(imgs.shape[1]), int(imgs.shape[2])
+    assert imgs.dtype == torch.float32 and imgs.is_contiguous() and ref.is_contiguous()
+    need = lib().gsr_distortion_workspace_bytes(B, H, W)
+    if workspace is None or workspace.numel() < need:
+        workspace = torch.empty(need, dtype=torch.uint8, device="cuda")
+    mse = torch.empty(B, dtype=torch.float64, device="cuda")
+    psnr = torch.empty(B, dtype=torch.float32, device="cuda")
+    _check(lib().gsr_distortion(_dp(imgs), _dp(ref), B, H, W, _dp(mse), _dp(psnr), _dp(workspace),
+                                workspace.numel(), _stream()))
+    return mse, psnr
+
+
+def group_utility(mse, psnr, idx_without, idx_with, group_id, G: int, want_deltas: bool = True):
+    """gsr_group_utility on device tensors.  Returns (util structured array [G], delta_mse, delta_db)."""
+    torch = _torch()
+    n_pairs = int(idx_without.numel())
+    util = torch.zeros((max(G, 1), 9), dtype=torch.float64, device="cuda")
+    dm = torch.empty(max(n_pairs, 1), dtype=torch.float64, device="cuda") if want_deltas else None
+    dd = torch.empty(max(n_pairs, 1), dtype=torch.float64, device="cuda") if want_deltas else None
+    for t in (idx_without, idx_with, group_id):
+        assert t.dtype == torch.int32 and t.is_cuda and t.is_contiguous()
+    _check(lib().gsr_group_utility(_dp(mse), _dp(psnr), _dp(idx_without), _dp(idx_with), _dp(group_id), n_pairs, G,
+                                   _dp(util), _dp(dm), _dp(dd), _stream()))
+    u = util[:G].cpu().numpy().view(UTILITY_DTYPE).reshape(G)
+    return u, (dm[:n_pairs] if dm is not None else None), (dd[:n_pairs] if dd is not None else None)
+
+
+def close_levels(mask):
+    """gsr_close_levels: cuda uint8 masks -> (depth int8, closure uint8) on device."""
+    torch = _torch()
+    assert mask.dtype == torch.uint8 and mask.is_cuda and mask.is_contiguous()
+    depth = torch.empty(mask.shape, dtype=torch.int8, device="cuda")
+    closure = torch.empty(mask.shape, dtype=torch.uint8, device="cuda")
+    _check(lib().gsr_close_levels(_dp(mask), mask.numel(), _dp(depth), _dp(closure), _stream()))
+    return depth, closure

@@ -1,0 +1,80 @@
+"""CPU-only checks of the boundary: libgsr.so builds, loads and exports every symbol include/gsr.h
+declares; argument errors are reported without touching a GPU; the binding has no CPU fallback."""
+import ctypes
+import re
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+@pytest.fixture(scope="module")
+def libgsr():
+    from paper_2606_17212_b200 import build
+    path = build.build()
+    return ctypes.CDLL(str(path))
+
+
+def declared_symbols():
+    text = (ROOT / "include" / "gsr.h").read_text()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(gsr_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_header_declares_the_four_named_calls():
+    syms = declared_symbols()
+    for name in ("gsr_load_scene", "gsr_render_states", "gsr_distortion", "gsr_group_utility"):
+        assert name in syms
+
+
+def test_library_exports_every_declared_symbol(libgsr):
+    syms = declared_symbols()
+    assert len(syms) >= 15
+    for name in syms:
+        assert hasattr(libgsr, name), f"libgsr.so does not export {name}"
+
+
+def test_library_targets_sm_100a():
+    import subprocess
+    from paper_2606_17212_b200 import build
+    out = subprocess.run(["cuobjdump", "-lelf", str(build.build())], capture_output=True, text=True).stdout
+    assert "sm_100a" in out, out
+
+
+def test_argument_errors_without_gpu(libgsr):
+    libgsr.gsr_last_error.restype = ctypes.c_char_p
+    libgsr.gsr_version.restype = ctypes.c_char_p
+    assert b"sm_100a" in libgsr.gsr_version()
+    out = ctypes.c_void_p()
+    assert libgsr.gsr_load_scene(None, ctypes.byref(out)) == -1
+    assert b"NULL" in libgsr.gsr_last_error()
+    assert libgsr.gsr_render_states(None, None, ctypes.c_float(0), None, 1, None, None, 0, None) == -1
+    assert libgsr.gsr_distortion(None, None, -1, 4, 4, None, None, None, 0, None) == -1
+    assert libgsr.gsr_group_utility(None, None, None, None, None, -1, 0, None, None, None, None) == -1
+    libgsr.gsr_workspace_bytes.restype = ctypes.c_size_t
+    assert libgsr.gsr_workspace_bytes(None, None, 4) == 0
+    libgsr.gsr_distortion_workspace_bytes.restype = ctypes.c_size_t
+    assert libgsr.gsr_distortion_workspace_bytes(2, 17, 33) == 256  # 2 states x (3x2 tiles) doubles, 256-aligned
+
+
+def test_binding_has_no_cpu_fallback():
+    import torch
+    from paper_2606_17212_b200 import gsr, synth
+    if torch.cuda.is_available():
+        pytest.skip("this check is for the CPU-only box")
+    with pytest.raises(RuntimeError):
+        gsr.Scene(synth.scene_cfg0())
+    with pytest.raises(RuntimeError):
+        gsr.close_levels(torch.zeros(4, dtype=torch.uint8))
+
+
+def test_product_does_not_import_oracle():
+    """The product path may not import, include, link or execute anything under oracle/."""
+    pat = re.compile(r"^\s*(from\s+oracle|import\s+oracle|from\s+\.\.?oracle|#\s*include\s*[\"<].*oracle)", re.M)
+    for p in (ROOT / "paper_2606_17212_b200").rglob("*"):
+        if p.suffix in (".py", ".cu", ".cuh", ".h") and p.is_file():
+            text = p.read_text()
+            assert not pat.search(text), p
+            assert "libgsr_oracle" not in text and "gsr_oracle.c" not in text, p

@@ -1,0 +1,372 @@
+"""GPU parity tests: the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle
+on the same seeded inputs.  Run on a B200 with `pytest -m gpu`.
+
+Bars (BASELINE.json north_star): closure masks, radii / rectangles / depth bits / tile-intersection
+counts and sorted key lists BIT-EXACT; pixels max-abs <= 2e-4; utilities <= 1e-3 dB; batched GPU render
+bitwise equal to one-state-at-a-time GPU render.
+"""
+import numpy as np
+import pytest
+
+from paper_2606_17212_b200 import synth
+from tests.helpers import axis_camera, tiny_scene
+
+pytestmark = pytest.mark.gpu
+
+PIX_TOL = 2e-4
+DB_TOL = 1e-3
+
+
+@pytest.fixture(scope="module")
+def torch_mod():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def gsr(torch_mod):
+    from paper_2606_17212_b200 import gsr as G
+    G.lib()
+    return G
+
+
+def _dev_levels(torch, lv):
+    return torch.from_numpy(np.ascontiguousarray(lv, np.int8)).cuda()
+
+
+def _render(torch, scene, cam, t, lv, **kw):
+    ws = scene.new_workspace(cam, lv.shape[0])
+    out, mse, psnr = scene.render_states(cam, t, _dev_levels(torch, lv), workspace=ws, **kw)
+    scene.status(ws)
+    return out, mse, psnr, ws
+
+
+# ------------------------------------------------------------------------------------------ closure
+def test_closure_bit_exact(gsr, torch_mod, oracle_mod):
+    rng = np.random.default_rng(5)
+    mask = np.concatenate([np.arange(16, dtype=np.uint8), synth.sample_masks(rng, 4099)])
+    d_ref, c_ref = oracle_mod.close_levels(mask)
+    d, c = gsr.close_levels(torch_mod.from_numpy(mask).cuda())
+    assert np.array_equal(d.cpu().numpy(), d_ref)
+    assert np.array_equal(c.cpu().numpy(), c_ref)
+
+
+# ------------------------------------------------------------------------------------------ projection
+def _check_projection(gsr, torch, oracle_mod, sc_np, cam, t):
+    """Every (Gaussian, cluster depth) combination of the oracle must equal the GPU record that the
+    state semantics select: variant 0 for depth 0, variant 1 for depth >= 1, absent if depth < level."""
+    scene = gsr.Scene(sc_np)
+    osc = oracle_mod.OracleScene(sc_np)
+    lv = np.stack([np.full(sc_np.C, d, np.int8) for d in range(-1, 4)])
+    _, _, _, ws = _render(torch, scene, cam, t, lv)
+    assert np.array_equal(scene.debug_closure(ws, lv.shape[0]), lv)
+    P = scene.debug_projection(ws)
+    level = sc_np.level_of()
+    n_checked = 0
+    for d in range(-1, 4):
+        op = osc.project(cam, t, np.full(sc_np.C, d, np.int8))
+        v = 0 if d == 0 else 1
+        rid = 2 * np.arange(sc_np.N) + v
+        present = level <= d
+        ovalid = op["valid"] == 1
+        assert not np.any(ovalid & ~present)
+        gvalid = (P["valid"][rid] == 1) & present
+        assert np.array_equal(gvalid, ovalid), f"valid mismatch at depth {d}"
+        m = ovalid
+        n_checked += int(m.sum())
+        assert np.array_equal(P["radius"][rid][m], op["radius"][m])
+        assert np.array_equal(P["rect"][rid][m], op["rect"][m])
+        assert np.array_equal(P["depth_bits"][rid][m], op["depth_bits"][m])
+        assert np.array_equal(P["count"][rid][m], op["count"][m])
+        # decision-feeding fp32 quantities: bit-exact
+        assert np.array_equal(P["mean2d"][rid][m].view(np.uint32), np.stack([op["mx"], op["my"]], 1)[m].view(np.uint32))
+        assert np.array_equal(P["conic"][rid][m].view(np.uint32),
+                              np.stack([op["qa"], op["qb"], op["qc"]], 1)[m].view(np.uint32))
+        # colour is continuous (fp32 on the GPU, double in the oracle)
+        col = P["rgb_res"][rid] if d == 3 else P["rgb_base"][rid]
+        assert np.max(np.abs(col[m] - op["rgb"][m])) < 2e-6 if m.any() else True
+    assert n_checked > 0
+    scene.close()
+
+
+def test_projection_bit_exact_cfg0(gsr, torch_mod, oracle_mod):
+    wl = synth.workload_cfg0()
+    cam, t = wl.frames[0]
+    _check_projection(gsr, torch_mod, oracle_mod, wl.scene, cam, t)
+
+
+def test_projection_bit_exact_scaled_cfg1_sh3(gsr, torch_mod, oracle_mod):
+    wl = synth.scaled_object_workload(11, C=6, per_cluster=900.0, W=200, H=136, fov=40.0, n_frames=2, B=8)
+    for cam, t in wl.frames:
+        _check_projection(gsr, torch_mod, oracle_mod, wl.scene, cam, t)
+
+
+def test_projection_forward_facing_near_plane_and_offscreen(gsr, torch_mod, oracle_mod):
+    # cfg2-like geometry at reduced size: Gaussians behind / near the camera and outside the frustum
+    full = synth.scene_cfg2()
+    keep = np.zeros(full.N, bool)
+    off = full.group_off
+    new_off = [0]
+    idx = []
+    for g in range(4 * full.C):
+        take = np.arange(off[g], off[g + 1])[:: 40]
+        idx.append(take)
+        new_off.append(new_off[-1] + take.size)
+    idx = np.concatenate(idx)
+    sc = synth.Scene(full.C, idx.size, full.sh_degree, full.R, np.asarray(new_off, np.int32), full.mean[idx],
+                     full.log_scale[idx], full.quat[idx], full.opacity_logit[idx], full.sh_base[idx],
+                     full.sh_res[idx], full.motion_q[idx], full.A0, full.A1, full.motion_scale, full.background)
+    cam = synth.jitter_cameras(2, 1, 134, 240, synth.focal_from_fov(240, 50.0))[0]
+    _check_projection(gsr, torch_mod, oracle_mod, sc, cam, 0.375)
+
+
+# ------------------------------------------------------------------------------------------ keys
+def test_sorted_key_lists_and_counts_bit_exact_cfg0(gsr, torch_mod, oracle_mod):
+    wl = synth.workload_cfg0()
+    cam, t = wl.frames[0]
+    lv = wl.levels[0]
+    scene = gsr.Scene(wl.scene)
+    osc = oracle_mod.OracleScene(wl.scene)
+    _, _, _, ws = _render(torch_mod, scene, cam, t, lv)
+    counts = scene.debug_state_counts(ws, lv.shape[0])
+    rng = np.random.default_rng(1)
+    picks = [0, 1, 312, 624] + rng.integers(0, 625, 12).tolist()
+    for b in range(lv.shape[0]):
+        if b in picks:
+            op = osc.project(cam, t, lv[b])
+            tile, dbits, idx = osc.keys(op, cam)
+            g_tile, g_db, g_idx, n = scene.debug_keys(ws, b, cap=max(tile.size, 1) + 16)
+            assert n == tile.size == counts[b]
+            assert np.array_equal(g_tile, tile) and np.array_equal(g_db, dbits) and np.array_equal(g_idx, idx)
+    # I_b for ALL states against the oracle's own count
+    _, stats = osc.render_batch(cam, t, lv)
+    assert np.array_equal(counts, stats[:, 0])
+    scene.close()
+
+
+def test_sorted_key_lists_scaled_cfg1(gsr, torch_mod, oracle_mod):
+    wl = synth.scaled_object_workload(12, C=8, per_cluster=1500.0, W=328, H=200, fov=40.0, n_frames=1, B=24)
+    cam, t = wl.frames[0]
+    lv = wl.levels[0]
+    scene = gsr.Scene(wl.scene)
+    osc = oracle_mod.OracleScene(wl.scene)
+    _, _, _, ws = _render(torch_mod, scene, cam, t, lv)
+    counts = scene.debug_state_counts(ws, lv.shape[0])
+    for b in (0, 5, 13, 23):
+        op = osc.project(cam, t, lv[b])
+        tile, dbits, idx = osc.keys(op, cam)
+        g_tile, g_db, g_idx, n = scene.debug_keys(ws, b, cap=tile.size + 16)
+        assert n == tile.size == counts[b]
+        assert np.array_equal(g_tile, tile) and np.array_equal(g_db, dbits) and np.array_equal(g_idx, idx)
+        # strictly increasing (tile, depth, index): the list is the unique sorted order
+        a, b_, c = g_tile.astype(np.int64), g_db.astype(np.int64), g_idx.astype(np.int64)
+        da, db_, dc = np.diff(a), np.diff(b_), np.diff(c)
+        assert np.all((da > 0) | ((da == 0) & ((db_ > 0) | ((db_ == 0) & (dc > 0)))))
+    scene.close()
+
+
+# ------------------------------------------------------------------------------------------ pixels
+def test_pixels_cfg0_all_625_states(gsr, torch_mod, oracle_mod):
+    wl = synth.workload_cfg0()
+    cam, t = wl.frames[0]
+    lv = wl.levels[0]
+    scene = gsr.Scene(wl.scene)
+    osc = oracle_mod.OracleScene(wl.scene)
+    out, _, _, _ = _render(torch_mod, scene, cam, t, lv)
+    ref, _ = osc.render_batch(cam, t, lv)
+    err = np.abs(out.cpu().numpy().astype(np.float64) - ref)
+    assert err.max() <= PIX_TOL, err.max()
+    # the all-absent state is exactly the background
+    assert np.array_equal(out[0].cpu().numpy(), np.broadcast_to(wl.scene.background, (cam.H, cam.W, 3)))
+    scene.close()
+
+
+@pytest.mark.parametrize("S", [1, 4, 8, 16])
+def test_pixels_scaled_cfg1_ragged_tiles_white_background(gsr, torch_mod, oracle_mod, S):
+    # 200x136: 13x9 tiles with ragged right and bottom edges; B = 21 is not a multiple of any state block
+    wl = synth.scaled_object_workload(13, C=8, per_cluster=1200.0, W=200, H=136, fov=40.0, n_frames=1, B=42)
+    cam, t = wl.frames[0]
+    lv = wl.levels[0][:21]
+    scene = gsr.Scene(wl.scene)
+    osc = oracle_mod.OracleScene(wl.scene)
+    gsr.set_option("state_block", S)
+    try:
+        out, _, _, _ = _render(torch_mod, scene, cam, t, lv)
+    finally:
+        gsr.set_option("state_block", 8)
+    ref, _ = osc.render_batch(cam, t, lv)
+    err = np.abs(out.cpu().numpy().astype(np.float64) - ref)
+    assert err.max() <= PIX_TOL, err.max()
+    scene.close()
+
+
+def test_pixels_dense_stack_early_termination(gsr, torch_mod, oracle_mod):
+    # many opaque wide Gaussians stacked over the image: every pixel terminates early
+    rng = np.random.default_rng(3)
+    n = 400
+    means = np.stack([rng.uniform(-0.5, 0.5, n), rng.uniform(-0.5, 0.5, n), rng.uniform(-0.5, 0.5, n)], 1)
+    lev = rng.integers(0, 4, n)
+    clu = rng.integers(0, 3, n)
+    sc, _ = tiny_scene(means, 0.25, logits=3.0, colors=rng.uniform(0, 1, (n, 3)), levels=lev, clusters=clu, C=3,
+                       background=(0.2, 0.4, 0.6))
+    cam = axis_camera(W=96, H=80, f=90.0)
+    lv = synth.all_closed_states(3)
+    scene = gsr.Scene(sc)
+    osc = oracle_mod.OracleScene(sc)
+    out, _, _, _ = _render(torch_mod, scene, cam, 0.3, lv)
+    ref, stats = osc.render_batch(cam, 0.3, lv)
+    assert np.abs(out.cpu().numpy() - ref).max() <= PIX_TOL
+    scene.close()
+
+
+# ------------------------------------------------------------------------------------------ batched == serial
+def test_batched_equals_serial_bitwise(gsr, torch_mod):
+    wl = synth.workload_cfg0()
+    cam, t = wl.frames[0]
+    lv = wl.levels[0]
+    scene = gsr.Scene(wl.scene)
+    out, _, _, _ = _render(torch_mod, scene, cam, t, lv)
+    rng = np.random.default_rng(2)
+    for b in [0, 624] + rng.integers(0, 625, 30).tolist():
+        one, _, _, _ = _render(torch_mod, scene, cam, t, lv[b:b + 1])
+        assert torch_mod.equal(one[0], out[b]), f"state {b} differs between batched and serial rendering"
+    # and the result does not depend on the state-block size or on batch composition
+    perm = rng.permutation(625)
+    for S in (4, 16):
+        gsr.set_option("state_block", S)
+        try:
+            o2, _, _, _ = _render(torch_mod, scene, cam, t, lv[perm])
+        finally:
+            gsr.set_option("state_block", 8)
+        assert torch_mod.equal(o2, out[torch_mod.from_numpy(perm).cuda()])
+    scene.close()
+
+
+def test_batched_equals_serial_scaled_cfg1(gsr, torch_mod):
+    wl = synth.scaled_object_workload(14, C=8, per_cluster=1500.0, W=328, H=200, fov=40.0, n_frames=1, B=32)
+    cam, t = wl.frames[0]
+    lv = wl.levels[0]
+    scene = gsr.Scene(wl.scene)
+    out, _, _, _ = _render(torch_mod, scene, cam, t, lv)
+    for b in (0, 7, 16, 31):
+        one, _, _, _ = _render(torch_mod, scene, cam, t, lv[b:b + 1])
+        assert torch_mod.equal(one[0], out[b])
+    scene.close()
+
+
+# ------------------------------------------------------------------------------------------ distortion / utility
+def test_distortion_and_utility_against_oracle(gsr, torch_mod, oracle_mod):
+    wl = synth.scaled_object_workload(15, C=8, per_cluster=1200.0, W=200, H=136, fov=40.0, n_frames=1, B=64)
+    cam, t = wl.frames[0]
+    lv = wl.levels[0]
+    scene = gsr.Scene(wl.scene)
+    osc = oracle_mod.OracleScene(wl.scene)
+    full = np.full((1, wl.scene.C), 3, np.int8)
+    ref_img, _, _, _ = _render(torch_mod, scene, cam, t, full)
+    out, _, _, _ = _render(torch_mod, scene, cam, t, lv)
+    mse, psnr = gsr.distortion(out, ref_img[0].contiguous())
+    # fused path: bitwise the same distortions, with and without materialising the images
+    _, mse_f, psnr_f, _ = _render(torch_mod, scene, cam, t, lv, ref=ref_img[0].contiguous(), want_images=False)
+    assert torch_mod.equal(mse, mse_f) and torch_mod.equal(psnr, psnr_f)
+    out2, mse_f2, _, _ = _render(torch_mod, scene, cam, t, lv, ref=ref_img[0].contiguous())
+    assert torch_mod.equal(mse, mse_f2) and torch_mod.equal(out, out2)
+    # oracle
+    o_imgs, _ = osc.render_batch(cam, t, lv)
+    o_ref, _ = osc.render(cam, t, full[0])
+    o_mse, o_psnr = oracle_mod.distortion(o_imgs, o_ref)
+    assert np.max(np.abs(psnr.cpu().numpy() - o_psnr)) <= DB_TOL
+    assert np.allclose(mse.cpu().numpy(), o_mse, rtol=2e-4, atol=1e-12)
+    # utilities
+    G = wl.G
+    iwo, iw, gid = wl.idx_without[0], wl.idx_with[0], wl.group_id[0]
+    u, dm, dd = gsr.group_utility(mse, psnr, torch_mod.from_numpy(iwo).cuda(), torch_mod.from_numpy(iw).cuda(),
+                                  torch_mod.from_numpy(gid).cuda(), G)
+    o_dm, o_dd, o_u = oracle_mod.group_utility(o_mse, o_psnr, iwo, iw, gid, G)
+    assert np.max(np.abs(dd.cpu().numpy() - o_dd)) <= DB_TOL
+    for k, name in enumerate(oracle_mod.UTIL_FIELDS):
+        tol = DB_TOL if name.endswith("_db") else (0 if name == "count" else 1e-6)
+        assert np.max(np.abs(u[name] - o_u[:, k])) <= tol + 2e-4 * np.max(np.abs(o_u[:, k])), name
+    scene.close()
+
+
+def test_group_utility_matches_oracle_on_random_tables(gsr, torch_mod, oracle_mod):
+    # the aggregation alone, on random distortion tables, incl. empty groups, singletons and a group
+    # larger than the shared-memory cache (radix select from global memory)
+    rng = np.random.default_rng(9)
+    B = 9000
+    mse = rng.uniform(1e-5, 1e-2, B)
+    psnr = (-10 * np.log10(mse)).astype(np.float32)
+    n_pairs = 4500
+    iwo = rng.integers(0, B, n_pairs).astype(np.int32)
+    iw = rng.integers(0, B, n_pairs).astype(np.int32)
+    gid = rng.integers(0, 5, n_pairs).astype(np.int32)
+    gid[:3000] = 6            # one big group (> 2048 members)
+    gid[3000] = 7             # a singleton; groups 5 and 8 stay empty
+    G = 9
+    u, dm, dd = gsr.group_utility(torch_mod.from_numpy(mse).cuda(), torch_mod.from_numpy(psnr).cuda(),
+                                  torch_mod.from_numpy(iwo).cuda(), torch_mod.from_numpy(iw).cuda(),
+                                  torch_mod.from_numpy(gid).cuda(), G)
+    o_dm, o_dd, o_u = oracle_mod.group_utility(mse, psnr.astype(np.float64), iwo, iw, gid, G)
+    assert np.allclose(dm.cpu().numpy(), o_dm, rtol=0, atol=1e-15)
+    assert np.allclose(dd.cpu().numpy(), o_dd, rtol=0, atol=1e-9)
+    for k, name in enumerate(oracle_mod.UTIL_FIELDS):
+        assert np.allclose(u[name], o_u[:, k], rtol=1e-9, atol=1e-12), name
+
+
+# ------------------------------------------------------------------------------------------ edge cases / errors
+def test_empty_batch_and_empty_scene(gsr, torch_mod):
+    wl = synth.workload_cfg0()
+    cam, t = wl.frames[0]
+    scene = gsr.Scene(wl.scene)
+    out, _, _, ws = _render(torch_mod, scene, cam, t, np.zeros((0, 4), np.int8))
+    assert out.shape[0] == 0
+    scene.close()
+    sc, _ = tiny_scene(np.zeros((0, 3)), 0.1, C=2, background=(0.1, 0.2, 0.3))
+    scene = gsr.Scene(sc)
+    lv = synth.all_closed_states(2)
+    out, _, _, _ = _render(torch_mod, scene, axis_camera(W=40, H=24), 0.0, lv)
+    assert np.array_equal(out.cpu().numpy(), np.broadcast_to(np.float32([0.1, 0.2, 0.3]), out.shape))
+    scene.close()
+
+
+def test_invalid_level_and_key_capacity_are_reported(gsr, torch_mod):
+    wl = synth.workload_cfg0()
+    cam, t = wl.frames[0]
+    scene = gsr.Scene(wl.scene)
+    lv = wl.levels[0][:8].copy()
+    lv[3, 2] = 4
+    ws = scene.new_workspace(cam, 8)
+    scene.render_states(cam, t, _dev_levels(torch_mod, lv), workspace=ws)
+    with pytest.raises(gsr.GsrError) as e:
+        scene.status(ws)
+    assert e.value.code == gsr.GSR_E_INVALID_LEVEL
+    ws = scene.new_workspace(cam, 8, key_capacity=100)       # far too few keys for this frame
+    out, _, _ = scene.render_states(cam, t, _dev_levels(torch_mod, wl.levels[0][:8]), workspace=ws)
+    with pytest.raises(gsr.GsrError) as e:
+        scene.status(ws)
+    assert e.value.code == gsr.GSR_E_WORKSPACE_TOO_SMALL
+    with pytest.raises(gsr.GsrError):
+        scene.render_states(cam, t, _dev_levels(torch_mod, wl.levels[0][:8]),
+                            workspace=torch_mod.empty(1024, dtype=torch_mod.uint8, device="cuda"))
+    scene.close()
+
+
+def test_host_buffer_frame_call_matches_device_calls(gsr, torch_mod):
+    wl = synth.scaled_object_workload(16, C=8, per_cluster=800.0, W=200, H=136, fov=40.0, n_frames=1, B=32)
+    cam, t = wl.frames[0]
+    lv = wl.levels[0]
+    scene = gsr.Scene(wl.scene)
+    mse_h, psnr_h, util_h, out_h, _ = scene.utility_frame_host(cam, t, lv, wl.idx_without[0], wl.idx_with[0],
+                                                               wl.group_id[0], wl.G, want_images=True)
+    full = np.full((1, wl.scene.C), 3, np.int8)
+    ref_img, _, _, _ = _render(torch_mod, scene, cam, t, full)
+    out, mse, psnr, _ = _render(torch_mod, scene, cam, t, lv, ref=ref_img[0].contiguous())
+    assert np.array_equal(out.cpu().numpy(), out_h)
+    assert np.array_equal(mse.cpu().numpy(), mse_h) and np.array_equal(psnr.cpu().numpy(), psnr_h)
+    u, _, _ = gsr.group_utility(mse, psnr, torch_mod.from_numpy(wl.idx_without[0]).cuda(),
+                                torch_mod.from_numpy(wl.idx_with[0]).cuda(),
+                                torch_mod.from_numpy(wl.group_id[0]).cuda(), wl.G)
+    for name in u.dtype.names:
+        assert np.array_equal(u[name], util_h[name])
+    scene.close()
