@@ -1,0 +1,340 @@
+#!/usr/bin/env python
+"""bench.py — counterfactual state-renders/s of the whole hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg1|cfg2|cfg4|cfg0]
+
+A step = one frame of the workload through every stage of the path:
+closure, per-variant deformation + EWA projection, tile binning + radix sort, state-blocked
+compositing of B states (images materialised in HBM) with the fused per-state distortion against the
+full-state render of the same frame, and the per-group utility aggregation.
+
+N > 1 (torchrun): frames are independent units; rank r renders frames r, r+N, ... — no data-path
+collective ("weak" scaling: every rank does K steps).  Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+from paper_2606_17212_b200 import synth  # noqa: E402
+
+# FLOP accounting of the compositing kernel, FMA = 2 flop:
+#   per (pixel, record) alpha evaluation : dx, dy (2) + u (1) + s (2) + q (1) + v (1) + q (2) + o*e (1) + 1-alpha (1) = 11
+#   per (pixel, record, state) update    : T' (1) + alpha*T (1) + 3 FMA (6) + the T' < 1e-4 compare (1)          =  9
+#   literal per-state model: 20 flop per logical (pixel, Gaussian, state) pair
+FLOP_SHARED, FLOP_STATE, FLOP_LITERAL = 11.0, 9.0, 20.0
+NOMINAL_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # 74.4: SMs x FP32 lanes x 2 x max SM clock
+
+
+def build_workload(name: str, n_frames: int):
+    if name == "cfg0":
+        wl = synth.workload_cfg0()
+        wl.frames = wl.frames * n_frames
+        wl.levels = wl.levels * n_frames
+        e = np.zeros(0, np.int32)
+        wl.idx_without, wl.idx_with, wl.group_id, wl.G = [e] * n_frames, [e] * n_frames, [e] * n_frames, 0
+        return wl
+    if name == "cfg1":
+        return synth.workload_cfg1(n_frames=n_frames)
+    if name == "cfg2":
+        return synth.workload_cfg2(n_frames=n_frames)
+    if name == "cfg4":
+        wl = synth.workload_cfg4()
+        return wl
+    raise SystemExit(f"unknown workload {name}")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------ reference arm
+def oracle_sample(wl, frame: int, n_states: int):
+    """Times the CPU oracle, as it stands, on the first n_states states of a frame (+ the full-state
+    reference and the distortion).  Returns seconds."""
+    from oracle import oracle as O
+    cam, t = wl.frames[frame]
+    osc = oracle_sample.cache.get("scene")
+    if osc is None:
+        osc = oracle_sample.cache["scene"] = O.OracleScene(wl.scene)
+    lv = np.ascontiguousarray(wl.levels[frame][:n_states])
+    t0 = time.perf_counter()
+    full = np.full((1, wl.scene.C), 3, np.int8)
+    both = np.concatenate([lv, full], axis=0)
+    imgs, _ = osc.render_batch(cam, t, both)
+    O.distortion(imgs[:-1], imgs[-1])
+    return time.perf_counter() - t0, O.num_threads()
+
+
+oracle_sample.cache = {}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    wl = build_workload(args.workload, max(1, min(args.steps + args.warmup, 8)))
+    cam0, _ = wl.frames[0]
+    B = wl.levels[0].shape[0]
+    n_s = min(args.ref_states, B)
+    for k in range(args.warmup):
+        oracle_sample(wl, k % len(wl.frames), n_s)
+    tot, cores = 0.0, 1
+    for k in range(args.steps):
+        dt, cores = oracle_sample(wl, k % len(wl.frames), n_s)
+        tot += dt
+    value = n_s * args.steps / tot
+    sample = f"{n_s} of {B} states per frame (+1 full-state reference render and the MSE/PSNR reduction), {args.steps} frames"
+    line = {"impl": "reference", "metric": "counterfactual_state_renders_per_s", "value": value, "unit": "states/s",
+            "mpix_states_per_s": value * cam0.W * cam0.H / 1e6, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64 (decisions in f32)", "data": "synthetic",
+            "config": {"workload": wl.name, "states_per_frame": B, "resolution": [cam0.W, cam0.H],
+                       "gaussians": wl.scene.N, "clusters": wl.scene.C},
+            "cpu_baseline": {"value": value, "unit": "states/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": "states/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------ our arm
+def run_ours(args):
+    import torch
+    from paper_2606_17212_b200 import build as gbuild
+    gbuild.build()
+    from paper_2606_17212_b200 import gsr
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    total_steps = args.steps + args.warmup
+    n_frames = min(150, max(1, total_steps * world)) if args.workload == "cfg1" else min(8, max(1, total_steps))
+    wl = build_workload(args.workload, n_frames)
+    n_frames = len(wl.frames)
+    scene = gsr.Scene(wl.scene)
+    cam0, _ = wl.frames[0]
+    B, Cn, G = wl.levels[0].shape[0], wl.scene.C, wl.G
+    W, H = cam0.W, cam0.H
+    cams = [gsr.camera_struct(c) for c, _ in wl.frames]
+    ts = [float(t) for _, t in wl.frames]
+    dev = torch.device("cuda", local)
+    lv_dev = [torch.from_numpy(np.ascontiguousarray(l)).to(dev) for l in wl.levels]
+    iwo = [torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in wl.idx_without]
+    iw = [torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in wl.idx_with]
+    gid = [torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in wl.group_id]
+    ws = scene.new_workspace(cam0, B)
+    out = torch.empty((B, H, W, 3), dtype=torch.float32, device=dev)
+    ref = torch.empty((H, W, 3), dtype=torch.float32, device=dev)
+    mse = torch.empty(B, dtype=torch.float64, device=dev)
+    psnr = torch.empty(B, dtype=torch.float32, device=dev)
+    util = torch.zeros((max(G, 1), 9), dtype=torch.float64, device=dev)
+
+    def frame_of(step):
+        return (step * world + rank) % n_frames
+
+    def step(k, images=True):
+        f = frame_of(k)
+        scene.render_states_vs_full(cams[f], ts[f], lv_dev[f], ws, ref, mse, psnr, out=out if images else None)
+        if G > 0:
+            gsr.group_utility_into(mse, psnr, iwo[f], iw[f], gid[f], G, util)
+
+    def timed(fn, k0, K):
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for k in range(k0, k0 + K):
+            fn(k)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        if dist is not None:
+            tms = torch.tensor([ms], dtype=torch.float64, device=dev)
+            dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+            ms = float(tms.item())
+        return ms
+
+    # ---- warm-up, then the timed region (device-resident inputs), clocks sampled during it
+    for k in range(args.warmup):
+        step(k)
+    scene.status(ws)
+    gsr.set_option("profile", 1)
+    l0 = gsr.launch_count()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ms = timed(step, args.warmup, args.steps)
+    clocks = sampler.stop() if rank == 0 else None
+    launches = gsr.launch_count() - l0
+    comp_ms, comp_n = gsr.profile_read()
+    gsr.set_option("profile", 0)
+    keys = scene.status(ws)
+    value = B * args.steps * world / (ms * 1e-3)
+
+    # ---- the same path without materialising the images (distortion/utility only), reported beside it
+    ms_noimg = timed(lambda k: step(k, images=False), args.warmup, args.steps)
+
+    # ---- end to end through the host-buffer C-ABI call: pinned host inputs, H2D + D2H inside the timed region
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    h_lv = [pin(l) for l in wl.levels]
+    h_iwo, h_iw, h_gid = [pin(a) for a in wl.idx_without], [pin(a) for a in wl.idx_with], [pin(a) for a in wl.group_id]
+    h_mse = torch.empty(B, dtype=torch.float64).pin_memory()
+    h_psnr = torch.empty(B, dtype=torch.float32).pin_memory()
+    h_util = torch.zeros((max(G, 1), 9), dtype=torch.float64).pin_memory()
+    bufs = (h_mse.numpy(), h_psnr.numpy(), h_util.numpy().view(gsr.UTILITY_DTYPE).reshape(-1))
+    fws = [None]
+
+    def step_e2e(k):
+        f = frame_of(k)
+        r = scene.utility_frame_host(cams[f], ts[f], h_lv[f].numpy(), h_iwo[f].numpy(), h_iw[f].numpy(),
+                                     h_gid[f].numpy(), G, workspace=fws[0], materialise=True, bufs=bufs)
+        fws[0] = r[4]
+
+    del out
+    torch.cuda.empty_cache()
+    for k in range(min(args.warmup, 3)):
+        step_e2e(k)
+    ms_e2e = timed(step_e2e, args.warmup, args.steps)
+    n_pairs = int(wl.idx_without[0].size)
+    e2e = {"value": B * args.steps * world / (ms_e2e * 1e-3), "unit": "states/s",
+           "h2d_bytes_per_step": int(B * Cn + 3 * 4 * n_pairs), "d2h_bytes_per_step": int(B * 8 + B * 4 + G * 72),
+           "ms_per_step": ms_e2e / args.steps,
+           "note": "gsr_utility_frame_host: pinned host levels/pairs in, mse/psnr/utilities out; images materialised on device"}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (k_composite): counted work / CUDA-event time / FP32 peak
+    out = torch.empty((B, H, W, 3), dtype=torch.float32, device=dev)
+    n_cnt = min(args.steps, 6)
+    cnt = np.zeros(3, np.float64)
+    for k in range(args.warmup, args.warmup + n_cnt):
+        step(k)
+        cnt += scene.debug_pair_counts(ws)
+    cnt *= args.steps / n_cnt                       # scaled to the timed region (frames are statistically alike)
+    comp_s = comp_ms * 1e-3
+    flop_alg = cnt[0] * FLOP_SHARED + cnt[1] * FLOP_STATE
+    peak_meas = gsr.measure_fp32_peak()
+    achieved = flop_alg / comp_s / 1e12 if comp_s > 0 else 0.0
+    roofline = {"kernel": "k_composite", "bound": "alu", "achieved": achieved, "peak": peak_meas, "unit": "TFLOP/s",
+                "frac": achieved / peak_meas if peak_meas else None, "traffic": None,
+                "peak_kind": "measured here: FFMA-chain kernel (gsr_measure_fp32_peak); nominal %.1f" % NOMINAL_FP32_TFLOPS,
+                "kernel_ms_per_launch": comp_ms / max(comp_n, 1), "kernel_launches": comp_n,
+                "kernel_share_of_step": comp_ms / ms,
+                "alpha_evals_per_step": cnt[0] / args.steps, "state_updates_per_step": cnt[1] / args.steps,
+                "logical_pairs_per_step": cnt[2] / args.steps,
+                "literal_equiv_tflops": cnt[2] * FLOP_LITERAL / comp_s / 1e12 if comp_s > 0 else 0.0,
+                "image_write_gbs": B * H * W * 12 * args.steps / comp_s / 1e9 if comp_s > 0 else None}
+    tp = Path(ROOT / "profiles" / "traffic.json")
+    if tp.exists():
+        try:
+            roofline["traffic"] = json.loads(tp.read_text()).get(wl.name)
+        except Exception:
+            pass
+
+    # ---- CPU oracle on this box's cores, bounded sample of the same workload
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        n_s = min(args.ref_states, B)
+        dt, cores = oracle_sample(wl, frame_of(args.warmup), n_s)
+        cpu = {"value": n_s / dt, "unit": "states/s", "cores": cores, "kind": "oracle",
+               "sample": f"first {n_s} of {B} states of frame {frame_of(args.warmup)} (+ full-state reference render and MSE/PSNR), {dt:.1f} s"}
+
+    line = {"metric": "counterfactual_state_renders_per_s", "value": value, "unit": "states/s",
+            "mpix_states_per_s": value * W * H / 1e6, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": wl.name, "states_per_frame": B, "resolution": [W, H], "gaussians": wl.scene.N,
+                       "clusters": Cn, "sh_degree": wl.scene.sh_degree, "R": wl.scene.R, "frames": n_frames,
+                       "images_materialised": True, "state_block": 8, "keys_per_frame": keys,
+                       "l2": "per-step working set (%.2f GB of images written) exceeds the 126 MB L2; every step is a different frame" % (B * H * W * 12 / 1e9),
+                       "parallelism": "frames sharded over ranks, no collective" if world > 1 else "1 GPU"},
+            "value_without_images": B * args.steps * world / (ms_noimg * 1e-3),
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+            "context": {"paper_h100_pcie_utility_states_per_s": 1889.7,
+                        "note": "PAPER.md:150, other hardware, unstated resolution/scene: context only"}}
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg1", choices=["cfg0", "cfg1", "cfg2", "cfg4"])
+    ap.add_argument("--ref-states", type=int, default=64, help="states per frame the CPU oracle renders")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -124,6 +124,15 @@ int gsr_render_states_ex(const gsr_scene* scene, const gsr_camera* cam, float t,
                          int32_t B, float* out, const float* ref, double* mse, float* psnr_db,
                          void* workspace, size_t ws_bytes, void* cuda_stream);
 
+/* gsr_render_states_vs_full — the utility workload's frame call (north_star (5), reading A16): like
+ * gsr_render_states_ex, but the reference is the FULL state (every cluster at depth 3) of the same
+ * (camera, t), composited from the same projected records and sorted lists (one projection and one
+ * sort per frame) into ref_out (dev fp32 [H,W,3], required).  mse (required) / psnr_db (dev [B])
+ * receive each state's distortion against it; out may be NULL. */
+int gsr_render_states_vs_full(const gsr_scene* scene, const gsr_camera* cam, float t, const int8_t* levels,
+                              int32_t B, float* out, float* ref_out, double* mse, float* psnr_db,
+                              void* workspace, size_t ws_bytes, void* cuda_stream);
+
 /* Synchronises `cuda_stream` and reads the status latched by the last render into `workspace`:
  * returns GSR_OK, GSR_E_INVALID_LEVEL or GSR_E_WORKSPACE_TOO_SMALL.  keys_needed (host, may be NULL)
  * receives the number of (tile, depth, record) keys the frame produced. */
@@ -163,13 +172,16 @@ int gsr_close_levels(const uint8_t* delivered_mask, int64_t n, int8_t* depth_out
  * fused distortion, aggregates utilities, and copies mse / psnr_db / util back.  Synchronous.
  *   levels host int8 [B,C]; idx_without, idx_with, group_id host int32 [n_pairs] (n_pairs may be 0);
  *   mse host double [B]; psnr_db host float [B]; util host gsr_utility [G] (may be NULL if G == 0);
- *   out_host: host fp32 [B,H,W,3] or NULL.  workspace dev >= gsr_frame_workspace_bytes(...). */
+ *   materialise_images != 0: the [B,H,W,3] images are written to device memory inside the workspace
+ *   (as gsr_render_states does); out_host (host fp32 [B,H,W,3] or NULL) additionally copies them back.
+ *   workspace dev >= gsr_frame_workspace_bytes(..., want_images = materialise_images). */
 size_t gsr_frame_workspace_bytes(const gsr_scene* scene, const gsr_camera* cam, int32_t B, int32_t n_pairs,
                                  int32_t G, int32_t want_images);
 int gsr_utility_frame_host(const gsr_scene* scene, const gsr_camera* cam, float t, const int8_t* levels,
                            int32_t B, const int32_t* idx_without, const int32_t* idx_with,
                            const int32_t* group_id, int32_t n_pairs, int32_t G, double* mse, float* psnr_db,
-                           gsr_utility* util, float* out_host, void* workspace, size_t ws_bytes,
+                           gsr_utility* util, int32_t materialise_images, float* out_host, void* workspace,
+                           size_t ws_bytes,
                            void* cuda_stream);
 
 /* ------------------------------------------------------------------------------------------------
@@ -200,9 +212,27 @@ int gsr_debug_state_counts(const gsr_scene* scene, const void* workspace, int64_
  * depth host int8 [B,C] (as validated). */
 int gsr_debug_closure(const gsr_scene* scene, const void* workspace, int8_t* depth, void* cuda_stream);
 
-/* Tuning knob for experiments: "state_block" = states composited per CTA (1, 4, 8 or 16; default 8).
- * Results do not depend on it (bitwise). */
+/* gsr_debug_pair_counts: instrumented re-run of the compositing kernel over the last batch (same
+ * lists, same arithmetic, nothing written).  counts3 (host int64 [3]):
+ *   [0] (pixel, record) pairs whose alpha was evaluated with at least one live present state,
+ *   [1] (pixel, record, state) colour/transmittance updates on live present states,
+ *   [2] logical (pixel, Gaussian, state) pairs E = sum_b E_b in the sense of the oracle. */
+int gsr_debug_pair_counts(const gsr_scene* scene, const void* workspace, int64_t* counts3, void* cuda_stream);
+
+/* Options: "state_block" = states composited per CTA (1, 4, 8 or 16; default 8) — results do not
+ * depend on it (bitwise); "profile" = 1 records CUDA events around every compositing-kernel launch. */
 int gsr_set_option(const char* name, int32_t value);
+
+/* Sum of the compositing kernel's durations (ms, CUDA events on its launch stream) and the number
+ * of launches recorded since "profile" was set or last read.  Synchronises those events. */
+int gsr_profile_read(double* composite_ms, int32_t* composite_launches);
+
+/* Kernels launched by this library since load (the caller's evidence for "gpu_launches"). */
+int64_t gsr_launch_count(void);
+
+/* Measures this device's FP32 FMA throughput (TFLOP/s, FMA = 2 flop) with a register-resident FFMA
+ * chain kernel: the denominator of the compositing roofline.  Synchronous. */
+int gsr_measure_fp32_peak(double* tflops, void* cuda_stream);
 
 /* Text of the last error on this thread ("" if none). */
 const char* gsr_last_error(void);

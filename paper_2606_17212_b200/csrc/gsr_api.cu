@@ -31,7 +31,11 @@ void set_error(const char* fmt, ...) {
     }                                                                                       \
   } while (0)
 
-extern int g_state_block;
+extern int g_state_block, g_profile;
+void profile_reset();
+int profile_read(double* ms, int* n);
+unsigned long long launches_total();
+int measure_ffma_peak(int num_sms, double* tflops, cudaStream_t st);
 
 long long default_key_capacity(int32_t N) { return 12ll * 2ll * (long long)N + (1ll << 20); }
 
@@ -49,7 +53,7 @@ size_t carve_workspace(Workspace* ws, void* base, int32_t N, int32_t C, int32_t 
   const size_t n_rec = 2 * (size_t)N;
   Workspace w;
   w.hdr = (WsHeader*)take(sizeof(WsHeader));
-  w.depth = (int8_t*)take((size_t)B * C);
+  w.depth = (int8_t*)take((size_t)(B + 1) * C);
   w.r0 = (float4*)take(sizeof(float4) * n_rec);
   w.r1 = (float4*)take(sizeof(float4) * n_rec);
   w.rc0 = (float4*)take(sizeof(float4) * n_rec);
@@ -122,8 +126,36 @@ int gsr_set_option(const char* name, int value) {
     g_state_block = value;
     return GSR_OK;
   }
+  if (name && strcmp(name, "profile") == 0) {
+    g_profile = value != 0;
+    profile_reset();
+    return GSR_OK;
+  }
   set_error("gsr_set_option: unknown option or value");
   return GSR_E_INVALID_ARG;
+}
+
+int gsr_profile_read(double* composite_ms, int32_t* composite_launches) {
+  if (!composite_ms || !composite_launches) { set_error("gsr_profile_read: NULL argument"); return GSR_E_INVALID_ARG; }
+  int n = 0;
+  if (profile_read(composite_ms, &n) != 0) { set_error("gsr_profile_read: event query failed"); return GSR_E_CUDA; }
+  *composite_launches = n;
+  profile_reset();
+  return GSR_OK;
+}
+
+int64_t gsr_launch_count(void) { return (int64_t)launches_total(); }
+
+int gsr_measure_fp32_peak(double* tflops, void* cuda_stream) {
+  if (!tflops) { set_error("gsr_measure_fp32_peak: NULL argument"); return GSR_E_INVALID_ARG; }
+  int dev = 0, sms = 0;
+  GSR_CUDA(cudaGetDevice(&dev));
+  GSR_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  if (measure_ffma_peak(sms, tflops, (cudaStream_t)cuda_stream) != 0) {
+    set_error("gsr_measure_fp32_peak: kernel failed: %s", cudaGetErrorString(cudaGetLastError()));
+    return GSR_E_CUDA;
+  }
+  return GSR_OK;
 }
 
 int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
@@ -290,33 +322,59 @@ static long long capacity_for(const gsr_scene* scene, int tiles, int32_t B, size
   return lo;
 }
 
-int gsr_render_states_ex(const gsr_scene* scene, const gsr_camera* cam, float t, const int8_t* levels, int32_t B,
-                         float* out, const float* ref, double* mse, float* psnr_db, void* workspace,
-                         size_t ws_bytes, void* cuda_stream) {
+// a0..a3 for one frame: validates levels, projects every variant once, bins and sorts.  On success
+// *ws_out / *fp_out describe the prepared frame.
+static int prepare_frame(const gsr_scene* scene, const gsr_camera* cam, float t, const int8_t* levels, int32_t B,
+                         void* workspace, size_t ws_bytes, cudaStream_t st, Workspace* ws_out, FrameParams* fp_out) {
   if (!scene || !camera_ok(cam) || B < 0 || (B > 0 && !levels) || !workspace) {
     set_error("gsr_render_states: invalid argument");
     return GSR_E_INVALID_ARG;
   }
-  if (ref && !mse) { set_error("gsr_render_states: ref given without mse"); return GSR_E_INVALID_ARG; }
   if (((uintptr_t)workspace & 255u) != 0) { set_error("gsr_render_states: workspace must be 256-byte aligned"); return GSR_E_INVALID_ARG; }
   const SceneImpl* s = &scene->impl;
-  FrameParams fp;
-  make_frame(s, cam, t, &fp);
-  const int tiles = fp.TX * fp.TY;
+  make_frame(s, cam, t, fp_out);
+  const int tiles = fp_out->TX * fp_out->TY;
   if (carve_workspace(nullptr, nullptr, s->d.N, s->d.C, B, tiles, 1) > ws_bytes) {
     set_error("gsr_render_states: workspace of %zu bytes is too small", ws_bytes);
     return GSR_E_WORKSPACE_TOO_SMALL;
   }
   const long long cap = capacity_for(scene, tiles, B, ws_bytes);
   if (cap < 1) { set_error("gsr_render_states: workspace too small"); return GSR_E_WORKSPACE_TOO_SMALL; }
-  Workspace ws;
-  carve_workspace(&ws, workspace, s->d.N, s->d.C, B, tiles, cap);
+  carve_workspace(ws_out, workspace, s->d.N, s->d.C, B, tiles, cap);
+  launch_init_header(*ws_out, B, s->d.C, s->d.N, *fp_out, cap, st);
+  launch_validate_levels(levels, B, s->d.C, *ws_out, st);   // a0
+  launch_project(s->d, *fp_out, *ws_out, st);                // a1 + a2
+  launch_bin_and_sort(s->d, *fp_out, *ws_out, cap, st);      // a3
+  return GSR_OK;
+}
+
+int gsr_render_states_ex(const gsr_scene* scene, const gsr_camera* cam, float t, const int8_t* levels, int32_t B,
+                         float* out, const float* ref, double* mse, float* psnr_db, void* workspace,
+                         size_t ws_bytes, void* cuda_stream) {
+  if (ref && !mse) { set_error("gsr_render_states: ref given without mse"); return GSR_E_INVALID_ARG; }
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  launch_init_header(ws, B, s->d.C, s->d.N, fp, cap, st);
-  launch_validate_levels(levels, B, s->d.C, ws, st);                  // a0
-  launch_project(s->d, fp, ws, st);                                   // a1 + a2
-  launch_bin_and_sort(s->d, fp, ws, cap, st);                         // a3
-  launch_composite(s->d, fp, ws, B, out, ref, mse, psnr_db, st);      // a4 (+ fused a5)
+  Workspace ws;
+  FrameParams fp;
+  int rc = prepare_frame(scene, cam, t, levels, B, workspace, ws_bytes, st, &ws, &fp);
+  if (rc != GSR_OK) return rc;
+  launch_composite(scene->impl.d, fp, ws, ws.depth, B, out, ref, mse, psnr_db, st);  // a4 (+ fused a5)
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
+int gsr_render_states_vs_full(const gsr_scene* scene, const gsr_camera* cam, float t, const int8_t* levels,
+                              int32_t B, float* out, float* ref_out, double* mse, float* psnr_db, void* workspace,
+                              size_t ws_bytes, void* cuda_stream) {
+  if (!ref_out || !mse) { set_error("gsr_render_states_vs_full: ref_out and mse are required"); return GSR_E_INVALID_ARG; }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  Workspace ws;
+  FrameParams fp;
+  int rc = prepare_frame(scene, cam, t, levels, B, workspace, ws_bytes, st, &ws, &fp);
+  if (rc != GSR_OK) return rc;
+  const DeviceScene& d = scene->impl.d;
+  // the reference: the full state (row B of ws.depth), composited from the same sorted lists
+  launch_composite(d, fp, ws, ws.depth + (size_t)B * d.C, 1, ref_out, nullptr, nullptr, nullptr, st);
+  launch_composite(d, fp, ws, ws.depth, B, out, ref_out, mse, psnr_db, st);
   GSR_CUDA(cudaGetLastError());
   return GSR_OK;
 }
@@ -422,13 +480,15 @@ size_t gsr_frame_workspace_bytes(const gsr_scene* scene, const gsr_camera* cam, 
 int gsr_utility_frame_host(const gsr_scene* scene, const gsr_camera* cam, float t, const int8_t* levels, int32_t B,
                            const int32_t* idx_without, const int32_t* idx_with, const int32_t* group_id,
                            int32_t n_pairs, int32_t G, double* mse, float* psnr_db, gsr_utility* util,
-                           float* out_host, void* workspace, size_t ws_bytes, void* cuda_stream) {
+                           int32_t materialise_images, float* out_host, void* workspace, size_t ws_bytes,
+                           void* cuda_stream) {
   if (!scene || !camera_ok(cam) || B <= 0 || !levels || !mse || !psnr_db || !workspace || n_pairs < 0 || G < 0 ||
       (n_pairs > 0 && (!idx_without || !idx_with || !group_id)) || (G > 0 && !util)) {
     set_error("gsr_utility_frame_host: invalid argument");
     return GSR_E_INVALID_ARG;
   }
-  const FrameCarve f = carve_frame(scene, cam, B, n_pairs, G, out_host != nullptr);
+  if (out_host) materialise_images = 1;
+  const FrameCarve f = carve_frame(scene, cam, B, n_pairs, G, materialise_images);
   if (ws_bytes < f.total) { set_error("gsr_utility_frame_host: workspace too small"); return GSR_E_WORKSPACE_TOO_SMALL; }
   cudaStream_t st = (cudaStream_t)cuda_stream;
   char* base = (char*)workspace;
@@ -440,7 +500,7 @@ int gsr_utility_frame_host(const gsr_scene* scene, const gsr_camera* cam, float 
   float* d_psnr = (float*)(base + f.o_psnr);
   int32_t* d_pairs = (int32_t*)(base + f.o_pairs);
   gsr_utility* d_util = (gsr_utility*)(base + f.o_util);
-  float* d_out = out_host ? (float*)(base + f.o_out) : nullptr;
+  float* d_out = materialise_images ? (float*)(base + f.o_out) : nullptr;
   void* rws = base + f.o_render;
   const size_t rws_bytes = gsr_workspace_bytes(scene, cam, B > 1 ? B : 1);
   GSR_CUDA(cudaMemcpyAsync(d_levels, levels, (size_t)B * C, cudaMemcpyHostToDevice, st));
@@ -450,10 +510,8 @@ int gsr_utility_frame_host(const gsr_scene* scene, const gsr_camera* cam, float 
     GSR_CUDA(cudaMemcpyAsync(d_pairs + n_pairs, idx_with, sizeof(int32_t) * n_pairs, cudaMemcpyHostToDevice, st));
     GSR_CUDA(cudaMemcpyAsync(d_pairs + 2 * (size_t)n_pairs, group_id, sizeof(int32_t) * n_pairs, cudaMemcpyHostToDevice, st));
   }
-  // reference = the full state (reading A16), then the batch with fused distortion
-  int rc = gsr_render_states(scene, cam, t, d_full, 1, d_ref, rws, rws_bytes, st);
-  if (rc != GSR_OK) return rc;
-  rc = gsr_render_states_ex(scene, cam, t, d_levels, B, d_out, d_ref, d_mse, d_psnr, rws, rws_bytes, st);
+  // reference = the full state (reading A16) and the batch with fused distortion, one projection + sort
+  int rc = gsr_render_states_vs_full(scene, cam, t, d_levels, B, d_out, d_ref, d_mse, d_psnr, rws, rws_bytes, st);
   if (rc != GSR_OK) return rc;
   if (G > 0) {
     rc = gsr_group_utility(d_mse, d_psnr, d_pairs, d_pairs + n_pairs, d_pairs + 2 * (size_t)n_pairs, n_pairs, G,
@@ -553,6 +611,27 @@ int gsr_debug_state_counts(const gsr_scene* scene, const void* workspace, int64_
   launch_state_counts(scene->impl.d, ws, h.B, st);
   GSR_CUDA(cudaMemcpyAsync(counts, ws.state_counts, sizeof(long long) * (size_t)h.B, cudaMemcpyDeviceToHost, st));
   GSR_CUDA(cudaStreamSynchronize(st));
+  return GSR_OK;
+}
+
+int gsr_debug_pair_counts(const gsr_scene* scene, const void* workspace, int64_t* counts3, void* cuda_stream) {
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  Workspace ws; WsHeader h;
+  int rc = ws_from(scene, workspace, &ws, &h, st);
+  if (rc != GSR_OK) return rc;
+  if (!counts3) { set_error("gsr_debug_pair_counts: NULL counts"); return GSR_E_INVALID_ARG; }
+  unsigned long long* d_c = nullptr;
+  GSR_CUDA(cudaMalloc(&d_c, 24));
+  GSR_CUDA(cudaMemsetAsync(d_c, 0, 24, st));
+  FrameParams fp;
+  memset(&fp, 0, sizeof(fp));
+  fp.W = h.W; fp.H = h.H; fp.TX = h.TX; fp.TY = h.TY;
+  launch_composite_count(scene->impl.d, fp, ws, ws.depth, h.B, d_c, st);
+  unsigned long long c[3];
+  GSR_CUDA(cudaMemcpyAsync(c, d_c, 24, cudaMemcpyDeviceToHost, st));
+  GSR_CUDA(cudaStreamSynchronize(st));
+  cudaFree(d_c);
+  for (int k = 0; k < 3; ++k) counts3[k] = (int64_t)c[k];
   return GSR_OK;
 }
 

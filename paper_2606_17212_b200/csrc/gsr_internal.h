@@ -56,7 +56,7 @@ struct WsHeader {
 
 struct Workspace {
   WsHeader* hdr;
-  int8_t* depth;          // [B,C] validated copy of levels
+  int8_t* depth;          // [B+1,C] validated copy of levels; row B = the full state (all 3)
   float4 *r0, *r1, *rc0, *rc1;  // [2N] projected records
   int32_t* radius;        // [2N]
   uint2* rect;            // [2N] 4 x u16: tx0,ty0,tx1,ty1
@@ -87,8 +87,14 @@ void launch_validate_levels(const int8_t* levels, int32_t B, int32_t C, Workspac
 void launch_project(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, cudaStream_t st);
 void launch_bin_and_sort(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, long long cap, cudaStream_t st);
 void launch_state_counts(const DeviceScene& sc, Workspace& ws, int32_t B, cudaStream_t st);
-void launch_composite(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, int32_t B, float* out,
-                      const float* ref, double* mse, float* psnr, cudaStream_t st);
+// composites B states whose depth rows start at `depth_rows` (ws.depth, or ws.depth + B*C for the full state)
+void launch_composite(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, const int8_t* depth_rows,
+                      int32_t B, float* out, const float* ref, double* mse, float* psnr, cudaStream_t st);
+// instrumented run of the same kernel: counts[0] = (pixel, record) pairs evaluated with >= 1 live present
+// state, counts[1] = (pixel, record, state) updates on live present states, counts[2] = logical pairs E
+void launch_composite_count(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, const int8_t* depth_rows,
+                            int32_t B, unsigned long long* counts, cudaStream_t st);
+void count_launches(int n);
 void launch_distortion(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, double* part,
                        double* mse, float* psnr, cudaStream_t st);
 void launch_distortion_finalize(const double* part, int32_t B, int32_t tiles, int64_t n_values, double* mse,

@@ -33,12 +33,13 @@ struct CompositeArgs {
   float* out;          // [B,H,W,3] or nullptr
   const float* ref;    // [H,W,3] or nullptr
   double* sse_part;    // [B, tiles]
+  unsigned long long* counts;  // instrumented run only: [3] (see launch_composite_count)
 };
 
 constexpr float kTStop = 1e-4f;     // reading A11
 constexpr float kAlphaCap = 0.99f;  // reading A11
 
-template <int S>
+template <int S, bool COUNT>
 __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const CompositeArgs a) {
   extern __shared__ uint16_t s_tab[];  // [C][4]: states (bit s) with depth ==0, >=1, >=2, >=3
   __shared__ float4 s_r0[kTilePix], s_r1[kTilePix], s_c0[kTilePix], s_c1[kTilePix];
@@ -82,6 +83,7 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
   }
 
   const uint2 rg = a.tile_range[tile];
+  unsigned long long n_shared = 0, n_state = 0, n_logical = 0;  // COUNT only
   __syncthreads();
 
   for (uint32_t base = rg.x; base < rg.y; base += kTilePix) {
@@ -145,6 +147,14 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
       const float v = __fmul_rn(h1.x, dy);
       q = __fmaf_rn(v, dy, q);
       const bool pass = !(q > h1.z);  // skip iff q > tau  (alpha < 1/255)
+      if (COUNT) {
+        int live = 0;
+#pragma unroll
+        for (int s = 0; s < S; ++s) live += ((mk >> s) & 1u) && T[s] > 0.0f;
+        n_shared += live > 0;
+        n_logical += live;
+        n_state += pass ? live : 0;
+      }
       if (!__any_sync(0xffffffffu, pass)) continue;
       float alpha = fminf(kAlphaCap, __fmul_rn(h1.y, __expf(-q)));
       alpha = pass ? alpha : 0.0f;
@@ -179,6 +189,17 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
     if (!__syncthreads_or(any_alive)) break;
   }
 
+  if (COUNT) {
+    n_shared = (unsigned long long)warp_sum_butterfly((double)n_shared);
+    n_state = (unsigned long long)warp_sum_butterfly((double)n_state);
+    n_logical = (unsigned long long)warp_sum_butterfly((double)n_logical);
+    if (lane == 0) {
+      atomicAdd(a.counts + 0, n_shared);
+      atomicAdd(a.counts + 1, n_state);
+      atomicAdd(a.counts + 2, n_logical);
+    }
+    return;
+  }
   // ---- pixel = C + T * background; optional fused squared error against the reference
   float rr0 = 0.f, rr1 = 0.f, rr2 = 0.f;
   if (a.ref && inside) {
@@ -271,37 +292,135 @@ void launch_distortion(const float* imgs, const float* ref, int32_t B, int32_t H
   launch_distortion_finalize(part, B, tiles, (int64_t)3 * W * H, mse, psnr, st);
 }
 
-template <int S>
+// ------------------------------------------------------------------------------------------------
+// launch bookkeeping: kernel-launch counter and optional CUDA-event timing of the compositing kernel
+static unsigned long long g_launches = 0;
+void count_launches(int n) { g_launches += (unsigned long long)n; }
+unsigned long long launches_total() { return g_launches; }
+
+int g_state_block = 8;  // S; set through gsr_set_option for experiments (1, 4, 8, 16)
+int g_profile = 0;      // gsr_set_option("profile", 1): record events around every k_composite launch
+constexpr int kMaxProfEvents = 8192;
+static cudaEvent_t g_ev[kMaxProfEvents][2];
+static int g_ev_created = 0, g_ev_used = 0;
+
+void profile_reset() { g_ev_used = 0; }
+// sum of k_composite durations (ms) and launches recorded since the last reset; synchronises the events
+int profile_read(double* ms, int* n) {
+  double tot = 0;
+  for (int k = 0; k < g_ev_used; ++k) {
+    float e = 0;
+    if (cudaEventSynchronize(g_ev[k][1]) != cudaSuccess) return -1;
+    if (cudaEventElapsedTime(&e, g_ev[k][0], g_ev[k][1]) != cudaSuccess) return -1;
+    tot += e;
+  }
+  *ms = tot;
+  *n = g_ev_used;
+  return 0;
+}
+
+template <int S, bool COUNT>
 static void launch_composite_S(const CompositeArgs& a, cudaStream_t st) {
   const size_t smem = sizeof(uint16_t) * 4 * (size_t)a.C;
   const long long grid = (long long)a.tiles * a.nsb;
-  k_composite<S><<<(unsigned)grid, kTilePix, smem, st>>>(a);
+  int slot = -1;
+  if (!COUNT && g_profile && g_ev_used < kMaxProfEvents) {
+    slot = g_ev_used++;
+    while (g_ev_created <= slot) {
+      cudaEventCreate(&g_ev[g_ev_created][0]);
+      cudaEventCreate(&g_ev[g_ev_created][1]);
+      ++g_ev_created;
+    }
+    cudaEventRecord(g_ev[slot][0], st);
+  }
+  k_composite<S, COUNT><<<(unsigned)grid, kTilePix, smem, st>>>(a);
+  if (slot >= 0) cudaEventRecord(g_ev[slot][1], st);
+  count_launches(1);
 }
 
-int g_state_block = 8;  // S; set through gsr_set_option for experiments (1, 4, 8, 16)
-
-void launch_composite(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, int32_t B, float* out,
-                      const float* ref, double* mse, float* psnr, cudaStream_t st) {
-  if (B == 0) return;
+static CompositeArgs make_args(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, const int8_t* depth_rows,
+                               int32_t B) {
   CompositeArgs a;
   a.tile_range = ws.tile_range;
   a.vals = ws.vals[0];
   a.r0 = ws.r0; a.r1 = ws.r1; a.rc0 = ws.rc0; a.rc1 = ws.rc1;
-  a.depth = ws.depth;
+  a.depth = depth_rows;
   a.B = B; a.C = sc.C;
   a.W = fp.W; a.H = fp.H; a.TX = fp.TX; a.tiles = fp.TX * fp.TY;
   a.bg[0] = fp.bg[0]; a.bg[1] = fp.bg[1]; a.bg[2] = fp.bg[2];
-  a.out = out; a.ref = ref; a.sse_part = ws.sse_part;
+  a.out = nullptr; a.ref = nullptr; a.sse_part = ws.sse_part; a.counts = nullptr;
+  return a;
+}
+
+template <bool COUNT>
+static void dispatch_composite(CompositeArgs& a, cudaStream_t st) {
   int S = g_state_block;
-  if (B == 1) S = 1;
-  a.nsb = (B + S - 1) / S;
+  if (a.B == 1) S = 1;
+  a.nsb = (a.B + S - 1) / S;
   switch (S) {
-    case 1: launch_composite_S<1>(a, st); break;
-    case 4: launch_composite_S<4>(a, st); break;
-    case 16: launch_composite_S<16>(a, st); break;
-    default: launch_composite_S<8>(a, st); break;
+    case 1: launch_composite_S<1, COUNT>(a, st); break;
+    case 4: launch_composite_S<4, COUNT>(a, st); break;
+    case 16: launch_composite_S<16, COUNT>(a, st); break;
+    default: launch_composite_S<8, COUNT>(a, st); break;
   }
+}
+
+void launch_composite(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, const int8_t* depth_rows,
+                      int32_t B, float* out, const float* ref, double* mse, float* psnr, cudaStream_t st) {
+  if (B == 0) return;
+  CompositeArgs a = make_args(sc, fp, ws, depth_rows, B);
+  a.out = out; a.ref = ref;
+  dispatch_composite<false>(a, st);
   if (ref) launch_distortion_finalize(ws.sse_part, B, a.tiles, (int64_t)3 * fp.W * fp.H, mse, psnr, st);
+}
+
+void launch_composite_count(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, const int8_t* depth_rows,
+                            int32_t B, unsigned long long* counts, cudaStream_t st) {
+  if (B == 0) return;
+  CompositeArgs a = make_args(sc, fp, ws, depth_rows, B);
+  a.counts = counts;
+  dispatch_composite<true>(a, st);
+}
+
+// ------------------------------------------------------------------------------------------------
+// FP32 FMA-pipe peak of this device, measured: 8 independent FFMA chains per thread, 2 x 512-thread
+// CTAs per SM.  Denominator of the compositing kernel's roofline.
+__global__ void __launch_bounds__(512) k_ffma_peak(float* sink, int iters, float a, float b) {
+  float x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < 16; ++u) {
+      x0 = fmaf(x0, a, b); x1 = fmaf(x1, a, b); x2 = fmaf(x2, a, b); x3 = fmaf(x3, a, b);
+      x4 = fmaf(x4, a, b); x5 = fmaf(x5, a, b); x6 = fmaf(x6, a, b); x7 = fmaf(x7, a, b);
+    }
+  }
+  float s = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
+  if (s == 12345.678f) sink[0] = s;
+}
+
+int measure_ffma_peak(int num_sms, double* tflops, cudaStream_t st) {
+  float* sink = nullptr;
+  if (cudaMalloc(&sink, 4) != cudaSuccess) return -1;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int iters = 4096, grid = num_sms * 4;
+  k_ffma_peak<<<grid, 512, 0, st>>>(sink, 64, 0.999f, 0.001f);  // warm-up
+  double best = 0;
+  for (int rep = 0; rep < 5; ++rep) {
+    cudaEventRecord(e0, st);
+    k_ffma_peak<<<grid, 512, 0, st>>>(sink, iters, 0.999f, 0.001f);
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(sink); return -1; }
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double flop = 2.0 * 8 * 16 * (double)iters * 512.0 * grid;
+    const double tf = flop / (ms * 1e-3) / 1e12;
+    if (tf > best) best = tf;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(sink);
+  *tflops = best;
+  return 0;
 }
 
 }  // namespace gsr

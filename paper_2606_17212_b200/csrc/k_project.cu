@@ -29,8 +29,11 @@ __global__ void k_validate_levels(const int8_t* __restrict__ levels, int64_t n, 
   depth[i] = (int8_t)d;
 }
 
-__global__ void k_init_header(WsHeader* hdr, int32_t B, int32_t C, int32_t N, int32_t W, int32_t H, int32_t TX,
-                              int32_t TY, long long cap) {
+// also writes row B of ws.depth: the full state (every cluster at depth 3), the reference of §3.6
+__global__ void k_init_header(WsHeader* hdr, int8_t* full_row, int32_t B, int32_t C, int32_t N, int32_t W,
+                              int32_t H, int32_t TX, int32_t TY, long long cap) {
+  for (int c = threadIdx.x; c < C; c += blockDim.x) full_row[c] = 3;
+  if (threadIdx.x != 0) return;
   hdr->status = GSR_OK;
   hdr->B = B; hdr->C = C; hdr->N = N; hdr->W = W; hdr->H = H; hdr->TX = TX; hdr->TY = TY;
   hdr->total_keys = 0; hdr->n_keys = 0; hdr->key_capacity = cap;
@@ -40,6 +43,7 @@ void launch_validate_levels(const int8_t* levels, int32_t B, int32_t C, Workspac
   int64_t n = (int64_t)B * C;
   if (n == 0) return;
   k_validate_levels<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(levels, n, ws.depth, ws.hdr);
+  count_launches(1);
 }
 
 // dependency closure of raw 4-bit delivery masks: depth = (#trailing one bits) - 1
@@ -56,6 +60,7 @@ __global__ void k_close_levels(const uint8_t* __restrict__ mask, int64_t n, int8
 void launch_close_levels(const uint8_t* mask, int64_t n, int8_t* depth, uint8_t* closure, cudaStream_t st) {
   if (n == 0) return;
   k_close_levels<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(mask, n, depth, closure);
+  count_launches(1);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -274,11 +279,13 @@ void launch_project(const DeviceScene& sc, const FrameParams& fp, Workspace& ws,
     case 9: k_project<9><<<grid, block, 0, st>>>(sc, fp, ws); break;
     default: k_project<16><<<grid, block, 0, st>>>(sc, fp, ws); break;
   }
+  count_launches(1);
 }
 
 void launch_init_header(Workspace& ws, int32_t B, int32_t C, int32_t N, const FrameParams& fp, long long cap,
                         cudaStream_t st) {
-  k_init_header<<<1, 1, 0, st>>>(ws.hdr, B, C, N, fp.W, fp.H, fp.TX, fp.TY, cap);
+  k_init_header<<<1, 256, 0, st>>>(ws.hdr, ws.depth + (size_t)B * C, B, C, N, fp.W, fp.H, fp.TX, fp.TY, cap);
+  count_launches(1);
 }
 
 }  // namespace gsr

@@ -305,6 +305,7 @@ void launch_bin_and_sort(const DeviceScene& sc, const FrameParams& fp, Workspace
                                                           ws.hdr, shift, ws.hist);
   }
   k_tile_ranges<<<148 * 8, 256, 0, st>>>(ws.keys[0], ws.hdr, ws.tile_range);
+  count_launches(4 + 3 * passes + 1);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -341,6 +342,7 @@ __global__ void __launch_bounds__(256) k_state_counts(int n_rec, const uint32_t*
 void launch_state_counts(const DeviceScene& sc, Workspace& ws, int32_t B, cudaStream_t st) {
   if (B == 0) return;
   k_state_counts<<<B, 256, 0, st>>>(2 * sc.N, ws.count, ws.r1, ws.depth, sc.C, ws.state_counts);
+  count_launches(1);
 }
 
 // Debug: the literal (tile, depth bits, Gaussian) list of state b = ordered filter of the superset list.

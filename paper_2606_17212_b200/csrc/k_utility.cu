@@ -162,8 +162,14 @@ void launch_group_utility(const double* mse, const float* psnr, const int32_t* i
                           double* ddb, cudaStream_t st) {
   PairView pv{mse, psnr, iwo, iw, gid, n_pairs};
   if (n_pairs > 0 && (dmse || ddb))
+  {
     k_pair_delta<<<(n_pairs + kUtilThreads - 1) / kUtilThreads, kUtilThreads, 0, st>>>(pv, dmse, ddb);
-  if (G > 0) k_group_utility<<<G, kUtilThreads, 0, st>>>(pv, G, out);
+    count_launches(1);
+  }
+  if (G > 0) {
+    k_group_utility<<<G, kUtilThreads, 0, st>>>(pv, G, out);
+    count_launches(1);
+  }
 }
 
 }  // namespace gsr

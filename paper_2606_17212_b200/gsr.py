@@ -72,12 +72,17 @@ def lib():
         L.gsr_frame_workspace_bytes.argtypes = [vp, C.POINTER(CameraC), i32, i32, i32, i32]
         L.gsr_frame_workspace_bytes.restype = sz
         L.gsr_utility_frame_host.argtypes = [vp, C.POINTER(CameraC), f32, vp, i32, vp, vp, vp, i32, i32, vp, vp, vp,
-                                             vp, vp, sz, vp]
+                                             i32, vp, vp, sz, vp]
         L.gsr_debug_projection.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.gsr_debug_keys.argtypes = [vp, vp, i32, i64, vp, vp, vp, C.POINTER(i64), vp]
         L.gsr_debug_state_counts.argtypes = [vp, vp, vp, vp]
         L.gsr_debug_closure.argtypes = [vp, vp, vp, vp]
         L.gsr_set_option.argtypes = [C.c_char_p, i32]
+        L.gsr_render_states_vs_full.argtypes = [vp, C.POINTER(CameraC), f32, vp, i32, vp, vp, vp, vp, vp, sz, vp]
+        L.gsr_debug_pair_counts.argtypes = [vp, vp, vp, vp]
+        L.gsr_profile_read.argtypes = [C.POINTER(C.c_double), C.POINTER(i32)]
+        L.gsr_launch_count.restype = i64
+        L.gsr_measure_fp32_peak.argtypes = [C.POINTER(C.c_double), vp]
         _lib = L
     return _lib
 
@@ -111,6 +116,8 @@ def _dp(t):
 
 
 def camera_struct(cam) -> CameraC:
+    if isinstance(cam, CameraC):
+        return cam
     c = CameraC()
     c.R_wc[:] = [float(v) for v in np.asarray(cam.R_wc, np.float32).reshape(9)]
     c.t_wc[:] = [float(v) for v in np.asarray(cam.t_wc, np.float32).reshape(3)]
@@ -121,6 +128,24 @@ def camera_struct(cam) -> CameraC:
 
 def set_option(name: str, value: int):
     _check(lib().gsr_set_option(name.encode(), int(value)))
+
+
+def profile_read():
+    """gsr_profile_read -> (sum of compositing-kernel ms, launches) since the last read."""
+    ms, n = C.c_double(0), C.c_int32(0)
+    _check(lib().gsr_profile_read(C.byref(ms), C.byref(n)))
+    return float(ms.value), int(n.value)
+
+
+def launch_count() -> int:
+    return int(lib().gsr_launch_count())
+
+
+def measure_fp32_peak() -> float:
+    _torch()
+    tf = C.c_double(0)
+    _check(lib().gsr_measure_fp32_peak(C.byref(tf), _stream()))
+    return float(tf.value)
 
 
 class Scene:
@@ -185,6 +210,18 @@ class Scene:
                                           workspace.numel(), _stream()))
         return out, mse, psnr
 
+    def render_states_vs_full(self, cam, t: float, levels, workspace, ref_out, mse, psnr, out=None):
+        """gsr_render_states_vs_full: all buffers are caller-provided device tensors (nothing allocated)."""
+        B = int(levels.shape[0])
+        _check(lib().gsr_render_states_vs_full(self.handle, C.byref(camera_struct(cam)), C.c_float(t), _dp(levels),
+                                               B, _dp(out), _dp(ref_out), _dp(mse), _dp(psnr), _dp(workspace),
+                                               workspace.numel(), _stream()))
+
+    def debug_pair_counts(self, workspace) -> np.ndarray:
+        c = np.zeros(3, np.int64)
+        _check(lib().gsr_debug_pair_counts(self.handle, _dp(workspace), _hp(c), _stream()))
+        return c
+
     def status(self, workspace) -> int:
         """gsr_workspace_status: synchronises; raises on a latched device-side error; returns #keys."""
         n = C.c_int64(0)
@@ -193,22 +230,27 @@ class Scene:
 
     # ---- host-buffer convenience call
     def utility_frame_host(self, cam, t: float, levels_host: np.ndarray, idx_without, idx_with, group_id, G: int,
-                           workspace=None, want_images: bool = False):
+                           workspace=None, want_images: bool = False, materialise: bool = False, bufs=None):
+        """gsr_utility_frame_host.  want_images copies the [B,H,W,3] images back to the host; materialise
+        only writes them on the device (what gsr_render_states does).  `bufs` = (mse, psnr, util) host
+        arrays to reuse (e.g. views of pinned memory)."""
         torch = _torch()
         lv = _np(levels_host, np.int8)
         B = lv.shape[0]
         iwo, iw, gid = _np(idx_without, np.int32), _np(idx_with, np.int32), _np(group_id, np.int32)
         n_pairs = int(iwo.size)
         camc = camera_struct(cam)
-        need = lib().gsr_frame_workspace_bytes(self.handle, C.byref(camc), B, n_pairs, G, int(want_images))
+        mat = int(bool(want_images or materialise))
+        need = lib().gsr_frame_workspace_bytes(self.handle, C.byref(camc), B, n_pairs, G, mat)
         if workspace is None or workspace.numel() < need:
             workspace = torch.empty(need, dtype=torch.uint8, device="cuda")
-        mse = np.empty(B, np.float64)
-        psnr = np.empty(B, np.float32)
-        util = np.zeros(max(G, 1), UTILITY_DTYPE)
+        if bufs is None:
+            mse, psnr, util = np.empty(B, np.float64), np.empty(B, np.float32), np.zeros(max(G, 1), UTILITY_DTYPE)
+        else:
+            mse, psnr, util = bufs
         out = np.empty((B, cam.H, cam.W, 3), np.float32) if want_images else None
         _check(lib().gsr_utility_frame_host(self.handle, C.byref(camc), C.c_float(t), _hp(lv), B, _hp(iwo), _hp(iw),
-                                            _hp(gid), n_pairs, G, _hp(mse), _hp(psnr), _hp(util),
+                                            _hp(gid), n_pairs, G, _hp(mse), _hp(psnr), _hp(util), mat,
                                             _hp(out) if out is not None else None, _dp(workspace),
                                             workspace.numel(), _stream()))
         return mse, psnr, util[:G], out, workspace
@@ -274,6 +316,12 @@ def group_utility(mse, psnr, idx_without, idx_with, group_id, G: int, want_delta
                                    _dp(util), _dp(dm), _dp(dd), _stream()))
     u = util[:G].cpu().numpy().view(UTILITY_DTYPE).reshape(G)
     return u, (dm[:n_pairs] if dm is not None else None), (dd[:n_pairs] if dd is not None else None)
+
+
+def group_utility_into(mse, psnr, idx_without, idx_with, group_id, G: int, util_out):
+    """gsr_group_utility with a caller-provided cuda float64 [G,9] output (no allocation, no sync)."""
+    _check(lib().gsr_group_utility(_dp(mse), _dp(psnr), _dp(idx_without), _dp(idx_with), _dp(group_id),
+                                   int(idx_without.numel()), G, _dp(util_out), None, None, _stream()))
 
 
 def close_levels(mask):
