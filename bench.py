@@ -171,6 +171,8 @@ def run_ours(args):
     wl = build_workload(args.workload, n_frames)
     n_frames = len(wl.frames)
     scene = gsr.Scene(wl.scene)
+    if args.state_block:
+        gsr.set_option("state_block", args.state_block)
     cam0, _ = wl.frames[0]
     B, Cn, G = wl.levels[0].shape[0], wl.scene.C, wl.G
     W, H = cam0.W, cam0.H
@@ -308,7 +310,7 @@ def run_ours(args):
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": wl.name, "states_per_frame": B, "resolution": [W, H], "gaussians": wl.scene.N,
                        "clusters": Cn, "sh_degree": wl.scene.sh_degree, "R": wl.scene.R, "frames": n_frames,
-                       "images_materialised": True, "state_block": 8, "keys_per_frame": keys,
+                       "images_materialised": True, "state_block": args.state_block or "default", "keys_per_frame": keys,
                        "l2": "per-step working set (%.2f GB of images written) exceeds the 126 MB L2; every step is a different frame" % (B * H * W * 12 / 1e9),
                        "parallelism": "frames sharded over ranks, no collective" if world > 1 else "1 GPU"},
             "value_without_images": B * args.steps * world / (ms_noimg * 1e-3),
@@ -329,6 +331,7 @@ def main():
     ap.add_argument("--workload", default="cfg1", choices=["cfg0", "cfg1", "cfg2", "cfg4"])
     ap.add_argument("--ref-states", type=int, default=64, help="states per frame the CPU oracle renders")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--state-block", type=int, default=0, help="states per compositing CTA (0 = library default)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -36,13 +36,20 @@ struct CompositeArgs {
   unsigned long long* counts;  // instrumented run only: [3] (see launch_composite_count)
 };
 
+__device__ __forceinline__ float4 lds128(uint32_t addr) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+  return v;
+}
+
 constexpr float kTStop = 1e-4f;     // reading A11
 constexpr float kAlphaCap = 0.99f;  // reading A11
 
 template <int S, bool COUNT>
 __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const CompositeArgs a) {
   extern __shared__ uint16_t s_tab[];  // [C][4]: states (bit s) with depth ==0, >=1, >=2, >=3
-  __shared__ float4 s_r0[kTilePix], s_r1[kTilePix], s_c0[kTilePix], s_c1[kTilePix];
+  // staged records, 64 B each: {m_x, m_y, A, B} {Cq, o, tau, act | res << 16} {rgb} {rgb + SH residual}
+  __shared__ __align__(16) float4 s_rec[kTilePix * 4];
   __shared__ uint32_t s_wcnt[8];
   __shared__ double s_red[8][S];
 
@@ -72,13 +79,15 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
   const int tx = tile % a.TX, ty = tile / a.TX;
   const int x = tx * kTile + (tid & 15), y = ty * kTile + (tid >> 4);
   const bool inside = x < a.W && y < a.H;
-  const float px = (float)x + 0.5f, py = (float)y + 0.5f;
+  float px = (float)x + 0.5f, py = (float)y + 0.5f;
+  asm volatile("" : "+f"(px), "+f"(py));  // keep them in registers (the compiler would rebuild them per record)
+  const uint32_t rec_base = (uint32_t)__cvta_generic_to_shared(s_rec);
   const float bg0 = a.bg[0], bg1 = a.bg[1], bg2 = a.bg[2];
 
   float T[S], Cr[S], Cg[S], Cb[S];
 #pragma unroll
   for (int s = 0; s < S; ++s) {
-    T[s] = (inside && b0 + s < a.B) ? 1.0f : 0.0f;  // T == 0 marks a finished (pixel, state)
+    T[s] = (inside && b0 + s < a.B) ? 1.0f : -1.0f;  // T < 0 marks a finished (pixel, state): -(frozen T)
     Cr[s] = Cg[s] = Cb[s] = 0.0f;
   }
 
@@ -117,27 +126,28 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
     }
     if (keep) {
       const uint32_t pos = woff + __popc(bal & ((1u << lane) - 1u));
-      s_r0[pos] = g0;
-      s_r1[pos] = make_float4(g1.x, g1.y, g1.z, __uint_as_float(act | (res << 16)));
-      s_c0[pos] = c0;
-      s_c1[pos] = c1;
+      s_rec[4 * pos + 0] = g0;
+      s_rec[4 * pos + 1] = make_float4(g1.x, g1.y, g1.z, __uint_as_float(act | (res << 16)));
+      s_rec[4 * pos + 2] = c0;
+      s_rec[4 * pos + 3] = c1;
     }
     __syncthreads();
 
     // ---- composite the staged records in order
     uint32_t walive = 0;
-    for (uint32_t j = 0; j < nb; ++j) {
+    uint32_t addr = rec_base;
+    for (uint32_t j = 0; j < nb; ++j, addr += 64u) {
       if ((j & 31u) == 0) {  // refresh the (warp, state) liveness mask
         walive = 0;
 #pragma unroll
         for (int s = 0; s < S; ++s) walive |= (uint32_t)(__any_sync(0xffffffffu, T[s] > 0.0f) != 0) << s;
         if (walive == 0) break;
       }
-      const float4 h1 = s_r1[j];
+      const float4 h1 = lds128(addr + 16u);
       const uint32_t mk = __float_as_uint(h1.w);
       const uint32_t actw = mk & walive;
       if (actw == 0) continue;
-      const float4 h0 = s_r0[j];
+      const float4 h0 = lds128(addr);
       // spec-exact quadratic form: u = A dx; s = fma(B,dy,u); q = s dx; v = Cq dy; q = fma(v,dy,q)
       const float dx = __fsub_rn(h0.x, px);
       const float dy = __fsub_rn(h0.y, py);
@@ -159,26 +169,24 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
       float alpha = fminf(kAlphaCap, __fmul_rn(h1.y, __expf(-q)));
       alpha = pass ? alpha : 0.0f;
       const float om = __fsub_rn(1.0f, alpha);
-      const float4 k0 = s_c0[j], k1 = s_c1[j];
+      const float4 k0 = lds128(addr + 32u), k1 = lds128(addr + 48u);
       const uint32_t resw = mk >> 16;
 #pragma unroll
       for (int s = 0; s < S; ++s) {
-        if ((actw >> s) & 1u) {
+        if ((actw >> s) & 1u) {  // warp-uniform: the record is present in state s
+          // T' = T(1-alpha); T' < 1e-4 stops the pixel BEFORE this record (a finished pixel has T < 0,
+          // so T' <= 0 and it stays finished); lanes that fail the cut have alpha = 0: a no-op.
           const float Tn = __fmul_rn(T[s], om);
-          if (Tn < kTStop) {
-            if (T[s] > 0.0f) {  // early termination: this record is NOT added; fold the background in
-              Cr[s] = __fmaf_rn(T[s], bg0, Cr[s]);
-              Cg[s] = __fmaf_rn(T[s], bg1, Cg[s]);
-              Cb[s] = __fmaf_rn(T[s], bg2, Cb[s]);
-              T[s] = 0.0f;
-            }
-          } else {
-            const float wgt = __fmul_rn(alpha, T[s]);
-            const bool rs = (resw >> s) & 1u;
-            Cr[s] = __fmaf_rn(wgt, rs ? k1.x : k0.x, Cr[s]);
-            Cg[s] = __fmaf_rn(wgt, rs ? k1.y : k0.y, Cg[s]);
-            Cb[s] = __fmaf_rn(wgt, rs ? k1.z : k0.z, Cb[s]);
+          const float wgt = __fmul_rn(alpha, T[s]);
+          const bool rs = (resw >> s) & 1u;
+          const float cr = rs ? k1.x : k0.x, cg = rs ? k1.y : k0.y, cb = rs ? k1.z : k0.z;
+          if (!(Tn < kTStop)) {
+            Cr[s] = __fmaf_rn(wgt, cr, Cr[s]);
+            Cg[s] = __fmaf_rn(wgt, cg, Cg[s]);
+            Cb[s] = __fmaf_rn(wgt, cb, Cb[s]);
             T[s] = Tn;
+          } else {
+            T[s] = __uint_as_float(__float_as_uint(T[s]) | 0x80000000u);
           }
         }
       }
@@ -208,9 +216,10 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
   }
 #pragma unroll
   for (int s = 0; s < S; ++s) {
-    const float o0 = __fmaf_rn(T[s], bg0, Cr[s]);
-    const float o1 = __fmaf_rn(T[s], bg1, Cg[s]);
-    const float o2 = __fmaf_rn(T[s], bg2, Cb[s]);
+    const float Tf = fabsf(T[s]);  // the transmittance the pixel ended with (frozen at termination)
+    const float o0 = __fmaf_rn(Tf, bg0, Cr[s]);
+    const float o1 = __fmaf_rn(Tf, bg1, Cg[s]);
+    const float o2 = __fmaf_rn(Tf, bg2, Cb[s]);
     if (a.out && inside && b0 + s < a.B) {
       float* op = a.out + (((size_t)(b0 + s) * a.H + y) * a.W + x) * 3;
       op[0] = o0; op[1] = o1; op[2] = o2;
