@@ -42,6 +42,40 @@ __device__ __forceinline__ float4 lds128(uint32_t addr) {
   return v;
 }
 
+__device__ __forceinline__ uint2 lds64(uint32_t addr) {
+  uint2 v;
+  asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ float2 lds64f(uint32_t addr) {
+  float2 v;
+  asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+  return v;
+}
+
+// One (pixel, state) step of DESIGN.md §3.5, branch-free:  T' = T (1 - alpha);  if T' >= 1e-4 { C += (alpha T) c;
+// T = T' } else { T = -|T| }.  T < 0 marks a finished pixel (-(frozen transmittance)): then T' <= 0 and it
+// stays finished.  A lane that failed the cut has alpha = 0, for which the step is exactly a no-op.
+// Explicitly rounded (mul.rn / fma.rn, never contracted) and predicated, so that every instantiation of
+// the kernel applies bit-identical arithmetic to a state: batched == serial.
+__device__ __forceinline__ void state_update(float& T, float& Cr, float& Cg, float& Cb, float om, float alpha,
+                                             float cr, float cg, float cb) {
+  asm("{\n\t"
+      ".reg .pred p;\n\t"
+      ".reg .f32 tn, wg;\n\t"
+      "mul.rn.f32 tn, %0, %4;\n\t"
+      "setp.geu.f32 p, tn, 0f38D1B717;\n\t"  // 1e-4f
+      "mul.rn.f32 wg, %5, %0;\n\t"
+      "@p fma.rn.f32 %1, wg, %6, %1;\n\t"
+      "@p fma.rn.f32 %2, wg, %7, %2;\n\t"
+      "@p fma.rn.f32 %3, wg, %8, %3;\n\t"
+      "@!p or.b32 %0, %0, 0x80000000;\n\t"
+      "@p mov.f32 %0, tn;\n\t"
+      "}"
+      : "+f"(T), "+f"(Cr), "+f"(Cg), "+f"(Cb)
+      : "f"(om), "f"(alpha), "f"(cr), "f"(cg), "f"(cb));
+}
+
 constexpr float kTStop = 1e-4f;     // reading A11
 constexpr float kAlphaCap = 0.99f;  // reading A11
 
@@ -53,7 +87,8 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
   __shared__ uint32_t s_wcnt[8];
   __shared__ double s_red[8][S];
 
-  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int w = __shfl_sync(0xffffffffu, tid >> 5, 0);  // broadcast: lets the compiler treat the warp index as warp-uniform
   const int tile = blockIdx.x / a.nsb, sb = blockIdx.x - tile * a.nsb;
   const int b0 = sb * S;
 
@@ -77,7 +112,9 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
   }
 
   const int tx = tile % a.TX, ty = tile / a.TX;
-  const int x = tx * kTile + (tid & 15), y = ty * kTile + (tid >> 4);
+  // warp w owns the 8x4 pixel block (w & 1, w >> 1) of the tile: compact footprints make the warp-level
+  // culls below sharper than 16x2 strips
+  const int x = tx * kTile + 8 * (w & 1) + (lane & 7), y = ty * kTile + 4 * (w >> 1) + (lane >> 3);
   const bool inside = x < a.W && y < a.H;
   float px = (float)x + 0.5f, py = (float)y + 0.5f;
   asm volatile("" : "+f"(px), "+f"(py));  // keep them in registers (the compiler would rebuild them per record)
@@ -96,10 +133,11 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
   __syncthreads();
 
   for (uint32_t base = rg.x; base < rg.y; base += kTilePix) {
-    // ---- stage up to 256 records, dropping those present in no state of the block
+    // ---- stage up to 256 records; drop those present in no state of the block and those whose
+    //      q <= tau region (conservative box from k_project) misses the tile
     const uint32_t idx = base + tid;
     const bool have = idx < rg.y;
-    uint32_t act = 0, res = 0;
+    uint32_t act = 0, res = 0, wmask = 0;
     float4 g0 = make_float4(0, 0, 0, 0), g1 = g0, c0 = g0, c1 = g0;
     if (have) {
       const uint32_t rid = __ldg(a.vals + idx);
@@ -112,8 +150,18 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
       const uint16_t* t = s_tab + 4 * (meta & 0xFFFFu);
       act = cls == 0 ? t[0] : (cls <= 2 ? t[1] : (cls == 3 ? t[2] : t[3]));
       res = cls == 0 ? 0u : t[3];
+      // pixel-centre box of the record vs the eight 8x4 pixel blocks of the tile
+      const float xlo = g0.x - c0.w, xhi = g0.x + c0.w, ylo = g0.y - c1.w, yhi = g0.y + c1.w;
+      const float X0 = (float)(tx * kTile) + 0.5f, Y0 = (float)(ty * kTile) + 0.5f;
+      uint32_t ox = 0, oy = 0;
+#pragma unroll
+      for (int k = 0; k < 2; ++k) ox |= (uint32_t)(xlo <= X0 + 8.0f * k + 7.0f && xhi >= X0 + 8.0f * k) << k;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) oy |= (uint32_t)(ylo <= Y0 + 4.0f * k + 3.0f && yhi >= Y0 + 4.0f * k) << k;
+#pragma unroll
+      for (int k = 0; k < 8; ++k) wmask |= (((ox >> (k & 1)) & (oy >> (k >> 1))) & 1u) << k;
     }
-    const bool keep = act != 0;
+    const bool keep = act != 0 && wmask != 0;
     const uint32_t bal = __ballot_sync(0xffffffffu, keep);
     if (lane == 0) s_wcnt[w] = __popc(bal);
     __syncthreads();
@@ -127,8 +175,8 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
     if (keep) {
       const uint32_t pos = woff + __popc(bal & ((1u << lane) - 1u));
       s_rec[4 * pos + 0] = g0;
-      s_rec[4 * pos + 1] = make_float4(g1.x, g1.y, g1.z, __uint_as_float(act | (res << 16)));
-      s_rec[4 * pos + 2] = c0;
+      s_rec[4 * pos + 1] = make_float4(g1.x, g1.z, __uint_as_float(wmask), __uint_as_float(act | (res << 16)));
+      s_rec[4 * pos + 2] = make_float4(c0.x, c0.y, c0.z, g1.y);
       s_rec[4 * pos + 3] = c1;
     }
     __syncthreads();
@@ -136,6 +184,7 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
     // ---- composite the staged records in order
     uint32_t walive = 0;
     uint32_t addr = rec_base;
+    const uint32_t wbit = 1u << w;
     for (uint32_t j = 0; j < nb; ++j, addr += 64u) {
       if ((j & 31u) == 0) {  // refresh the (warp, state) liveness mask
         walive = 0;
@@ -143,11 +192,11 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
         for (int s = 0; s < S; ++s) walive |= (uint32_t)(__any_sync(0xffffffffu, T[s] > 0.0f) != 0) << s;
         if (walive == 0) break;
       }
-      const float4 h1 = lds128(addr + 16u);
-      const uint32_t mk = __float_as_uint(h1.w);
-      const uint32_t actw = mk & walive;
-      if (actw == 0) continue;
+      const uint2 tag = lds64(addr + 24u);  // {8x4-block mask, act | res << 16}
+      const uint32_t actw = tag.y & walive;
+      if ((tag.x & wbit) == 0 || actw == 0) continue;
       const float4 h0 = lds128(addr);
+      const float2 h1 = lds64f(addr + 16u);  // {Cq, tau}
       // spec-exact quadratic form: u = A dx; s = fma(B,dy,u); q = s dx; v = Cq dy; q = fma(v,dy,q)
       const float dx = __fsub_rn(h0.x, px);
       const float dy = __fsub_rn(h0.y, py);
@@ -156,38 +205,26 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
       float q = __fmul_rn(sacc, dx);
       const float v = __fmul_rn(h1.x, dy);
       q = __fmaf_rn(v, dy, q);
-      const bool pass = !(q > h1.z);  // skip iff q > tau  (alpha < 1/255)
+      const bool pass = !(q > h1.y);  // skip iff q > tau  (alpha < 1/255)
       if (COUNT) {
         int live = 0;
 #pragma unroll
-        for (int s = 0; s < S; ++s) live += ((mk >> s) & 1u) && T[s] > 0.0f;
+        for (int s = 0; s < S; ++s) live += ((tag.y >> s) & 1u) && T[s] > 0.0f;
         n_shared += live > 0;
         n_logical += live;
         n_state += pass ? live : 0;
       }
       if (!__any_sync(0xffffffffu, pass)) continue;
-      float alpha = fminf(kAlphaCap, __fmul_rn(h1.y, __expf(-q)));
+      const float4 k0 = lds128(addr + 32u), k1 = lds128(addr + 48u);
+      float alpha = fminf(kAlphaCap, __fmul_rn(k0.w, __expf(-q)));
       alpha = pass ? alpha : 0.0f;
       const float om = __fsub_rn(1.0f, alpha);
-      const float4 k0 = lds128(addr + 32u), k1 = lds128(addr + 48u);
-      const uint32_t resw = mk >> 16;
+      const uint32_t resw = tag.y >> 16;
 #pragma unroll
       for (int s = 0; s < S; ++s) {
         if ((actw >> s) & 1u) {  // warp-uniform: the record is present in state s
-          // T' = T(1-alpha); T' < 1e-4 stops the pixel BEFORE this record (a finished pixel has T < 0,
-          // so T' <= 0 and it stays finished); lanes that fail the cut have alpha = 0: a no-op.
-          const float Tn = __fmul_rn(T[s], om);
-          const float wgt = __fmul_rn(alpha, T[s]);
           const bool rs = (resw >> s) & 1u;
-          const float cr = rs ? k1.x : k0.x, cg = rs ? k1.y : k0.y, cb = rs ? k1.z : k0.z;
-          if (!(Tn < kTStop)) {
-            Cr[s] = __fmaf_rn(wgt, cr, Cr[s]);
-            Cg[s] = __fmaf_rn(wgt, cg, Cg[s]);
-            Cb[s] = __fmaf_rn(wgt, cb, Cb[s]);
-            T[s] = Tn;
-          } else {
-            T[s] = __uint_as_float(__float_as_uint(T[s]) | 0x80000000u);
-          }
+          state_update(T[s], Cr[s], Cg[s], Cb[s], om, alpha, rs ? k1.x : k0.x, rs ? k1.y : k0.y, rs ? k1.z : k0.z);
         }
       }
     }
@@ -249,7 +286,7 @@ __global__ void __launch_bounds__(kTilePix) k_distortion_tiles(const float* __re
   __shared__ double s_red[8];
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   const int tile = blockIdx.x, b = blockIdx.y;
-  const int x = (tile % TX) * kTile + (tid & 15), y = (tile / TX) * kTile + (tid >> 4);
+  const int x = (tile % TX) * kTile + 8 * (w & 1) + (lane & 7), y = (tile / TX) * kTile + 4 * (w >> 1) + (lane >> 3);
   float e = 0.0f;
   if (x < W && y < H) {
     const size_t p = ((size_t)y * W + x) * 3;

@@ -67,6 +67,7 @@ void launch_close_levels(const uint8_t* mask, int64_t n, int8_t* depth, uint8_t*
 // K1 helpers
 struct Proj {
   float mx, my, qa, qb, qc;
+  float hx, hy;  // conservative half-extents (pixels) of the region where the cut q <= tau can pass
   int radius;
   int tx0, ty0, tx1, ty1;
   uint32_t depth_bits;
@@ -76,10 +77,12 @@ struct Proj {
 __device__ __forceinline__ float clampf_rn(float v, float lo, float hi) { return fminf(hi, fmaxf(lo, v)); }
 
 // EWA projection of a world-space mean `mu` with 3-D covariance S (xx xy xz yy yz zz).
-__device__ __forceinline__ Proj project_variant(const FrameParams& fp, const float mu[3], const float S6[6]) {
+__device__ __forceinline__ Proj project_variant(const FrameParams& fp, const float mu[3], const float S6[6],
+                                                const float tau) {
   Proj o;
   o.count = 0; o.radius = 0; o.tx0 = o.ty0 = o.tx1 = o.ty1 = 0; o.depth_bits = 0;
   o.mx = o.my = o.qa = o.qb = o.qc = 0.f;
+  o.hx = o.hy = 0.f;
   const float* Rw = fp.R;
   float pc[3];
 #pragma unroll
@@ -132,6 +135,18 @@ __device__ __forceinline__ Proj project_variant(const FrameParams& fp, const flo
   int ty1 = (int)clampf_rn(floorf(__fmul_rn(__fadd_rn(__fadd_rn(my, rad), 15.0f), 0.0625f)), 0.0f, TYf);
   o.mx = mx; o.my = my;
   o.qa = __fmul_rn(0.5f, conic_a); o.qb = conic_b; o.qc = __fmul_rn(0.5f, conic_c);
+  {
+    // Sub-tile culling bound: {q <= tau} is the ellipse x^T Sigma'^-1 x <= 2 tau, whose
+    // half-extents are sqrt(2 tau a), sqrt(2 tau c).  The kernel evaluates q in fp32 from the ROUNDED
+    // conic, so the bound is inflated by m = 8e-6 kappa + 1e-3, kappa = a c / det >= 1 (conditioning of
+    // the form: bounds both the conic rounding and the cancellation in q, each < 3e-6 kappa), and tau by
+    // +1e-2 (covers tau <= 0 and q rounding to a tiny negative).  Continuous, never feeds a list decision.
+    const float kappa = a * c * rdet;
+    const float m = 1.0f + fminf(1.0f, 8e-6f * kappa + 1e-3f);
+    const float t2 = 2.0f * (fmaxf(tau, 0.0f) + 1e-2f);
+    o.hx = sqrtf(t2 * a) * m + 1e-3f;
+    o.hy = sqrtf(t2 * c) * m + 1e-3f;
+  }
   o.radius = (int)rad;
   if (tx1 <= tx0 || ty1 <= ty0) return o;
   o.tx0 = tx0; o.ty0 = ty0; o.tx1 = tx1; o.ty1 = ty1;
@@ -180,8 +195,8 @@ __device__ __forceinline__ void store_record(Workspace& ws, uint32_t rid, const 
                                              uint32_t meta, const float* c0, const float* c1) {
   ws.r0[rid] = make_float4(p.mx, p.my, p.qa, p.qb);
   ws.r1[rid] = make_float4(p.qc, opac, tau, __uint_as_float(meta));
-  ws.rc0[rid] = make_float4(c0[0], c0[1], c0[2], 0.f);
-  ws.rc1[rid] = make_float4(c1[0], c1[1], c1[2], 0.f);
+  ws.rc0[rid] = make_float4(c0[0], c0[1], c0[2], p.hx);
+  ws.rc1[rid] = make_float4(c1[0], c1[1], c1[2], p.hy);
   ws.radius[rid] = p.radius;
   ws.rect[rid] = make_uint2((uint32_t)p.tx0 | ((uint32_t)p.ty0 << 16), (uint32_t)p.tx1 | ((uint32_t)p.ty1 << 16));
   ws.depth_bits[rid] = p.depth_bits;
@@ -230,8 +245,8 @@ __global__ void __launch_bounds__(128) k_project(DeviceScene sc, FrameParams fp,
   // ---- EWA projection of both geometries
   Proj pa;
   pa.count = 0;
-  if (lvl == 0) pa = project_variant(fp, p, S6);
-  Proj pb = project_variant(fp, muB, S6);
+  if (lvl == 0) pa = project_variant(fp, p, S6, tau);
+  Proj pb = project_variant(fp, muB, S6, tau);
 
   // ---- colour (continuous; fp32): rgb = max(0, 0.5 + sum_j Y_j(dir) * coef_j)
   float cA[3] = {0.f, 0.f, 0.f}, cB0[3] = {0.f, 0.f, 0.f}, cB1[3] = {0.f, 0.f, 0.f};
