@@ -31,7 +31,7 @@ void set_error(const char* fmt, ...) {
     }                                                                                       \
   } while (0)
 
-extern int g_state_block, g_profile;
+extern int g_state_block, g_profile, g_dedup;
 void profile_reset();
 int profile_read(double* ms, int* n);
 unsigned long long launches_total();
@@ -72,6 +72,9 @@ size_t carve_workspace(Workspace* ws, void* base, int32_t N, int32_t C, int32_t 
   w.tile_range = (uint2*)take(sizeof(uint2) * (size_t)tiles);
   w.state_counts = (long long*)take(sizeof(long long) * (size_t)(B > 0 ? B : 1));
   w.sse_part = (double*)take(sizeof(double) * (size_t)(B > 0 ? B : 1) * tiles);
+  w.uorder = (uint32_t*)take(sizeof(uint32_t) * (size_t)(B > 0 ? B : 1) * tiles);
+  w.upos = (uint32_t*)take(sizeof(uint32_t) * (size_t)(B > 0 ? B : 1) * tiles);
+  w.n_unique = (uint32_t*)take(sizeof(uint32_t) * (size_t)tiles);
   w.bytes = off;
   if (ws) *ws = w;
   return off;
@@ -124,6 +127,10 @@ const char* gsr_version(void) { return "gsr 0.1 sm_100a"; }
 int gsr_set_option(const char* name, int value) {
   if (name && strcmp(name, "state_block") == 0 && (value == 1 || value == 4 || value == 8 || value == 16)) {
     g_state_block = value;
+    return GSR_OK;
+  }
+  if (name && strcmp(name, "dedup") == 0) {
+    g_dedup = value != 0;
     return GSR_OK;
   }
   if (name && strcmp(name, "profile") == 0) {

@@ -70,6 +70,9 @@ struct Workspace {
   uint2* tile_range;      // [tiles] start,end into the sorted list
   long long* state_counts;  // [B]
   double* sse_part;       // [B * tiles] per-(state,tile) squared-error partials (fused distortion)
+  uint32_t* uorder;       // [tiles * B] states sorted by their tile-restricted signature (k_tile_dedup)
+  uint32_t* upos;         // [tiles * B] upos[tile*B + u] = index in uorder of the first member of class u
+  uint32_t* n_unique;     // [tiles] number of distinct signatures
   size_t bytes;           // total
 };
 
@@ -95,6 +98,8 @@ void launch_composite(const DeviceScene& sc, const FrameParams& fp, Workspace& w
 void launch_composite_count(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, const int8_t* depth_rows,
                             int32_t B, unsigned long long* counts, cudaStream_t st);
 void count_launches(int n);
+bool launch_tile_dedup(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, const int8_t* depth_rows,
+                       int32_t B, cudaStream_t st);
 void launch_distortion(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, double* part,
                        double* mse, float* psnr, cudaStream_t st);
 void launch_distortion_finalize(const double* part, int32_t B, int32_t tiles, int64_t n_values, double* mse,

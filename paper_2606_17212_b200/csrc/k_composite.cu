@@ -34,6 +34,7 @@ struct CompositeArgs {
   const float* ref;    // [H,W,3] or nullptr
   double* sse_part;    // [B, tiles]
   unsigned long long* counts;  // instrumented run only: [3] (see launch_composite_count)
+  const uint32_t *uorder, *upos, *n_unique;  // tile-level state dedup (k_tile_dedup); n_unique == nullptr: off
 };
 
 __device__ __forceinline__ float4 lds128(uint32_t addr) {
@@ -90,15 +91,38 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
   const int tid = threadIdx.x, lane = tid & 31;
   const int w = __shfl_sync(0xffffffffu, tid >> 5, 0);  // broadcast: lets the compiler treat the warp index as warp-uniform
   const int tile = blockIdx.x / a.nsb, sb = blockIdx.x - tile * a.nsb;
-  const int b0 = sb * S;
+  const int b0 = sb * S;  // first slot of this block: a state index, or a class index when dedup is on
+
+  // ---- which states this CTA composites.  With tile-level dedup (k_tile_dedup) slot s is the s-th
+  //      distinct signature class of this tile from b0 on; its first member stands for the class.
+  __shared__ int s_rep[S];        // representative state of slot s, -1 = empty slot
+  __shared__ uint32_t s_mlo[S], s_mhi[S];  // members of the class: uorder[tile*B + [mlo, mhi))
+  const int n_slots = a.n_unique ? (int)a.n_unique[tile] : a.B;
+  if (b0 >= n_slots) return;
+  if (tid < S) {
+    const int u = b0 + tid;
+    int rep = -1;
+    uint32_t lo = 0, hi = 0;
+    if (u < n_slots) {
+      if (a.n_unique) {
+        lo = a.upos[(size_t)tile * a.B + u];
+        hi = u + 1 < n_slots ? a.upos[(size_t)tile * a.B + u + 1] : (uint32_t)a.B;
+        rep = (int)a.uorder[(size_t)tile * a.B + lo];
+      } else {
+        rep = u;
+      }
+    }
+    s_rep[tid] = rep; s_mlo[tid] = lo; s_mhi[tid] = hi;
+  }
+  __syncthreads();
 
   // ---- presence masks of this state block (a0: closure predicates)
   for (int c = tid; c < a.C; c += kTilePix) {
     uint32_t eq0 = 0, ge1 = 0, ge2 = 0, ge3 = 0;
 #pragma unroll
     for (int s = 0; s < S; ++s) {
-      if (b0 + s < a.B) {
-        const int d = a.depth[(size_t)(b0 + s) * a.C + c];
+      if (s_rep[s] >= 0) {
+        const int d = a.depth[(size_t)s_rep[s] * a.C + c];
         eq0 |= (uint32_t)(d == 0) << s;
         ge1 |= (uint32_t)(d >= 1) << s;
         ge2 |= (uint32_t)(d >= 2) << s;
@@ -124,7 +148,7 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
   float T[S], Cr[S], Cg[S], Cb[S];
 #pragma unroll
   for (int s = 0; s < S; ++s) {
-    T[s] = (inside && b0 + s < a.B) ? 1.0f : -1.0f;  // T < 0 marks a finished (pixel, state): -(frozen T)
+    T[s] = (inside && s_rep[s] >= 0) ? 1.0f : -1.0f;  // T < 0 marks a finished (pixel, state): -(frozen T)
     Cr[s] = Cg[s] = Cb[s] = 0.0f;
   }
 
@@ -207,11 +231,15 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
       q = __fmaf_rn(v, dy, q);
       const bool pass = !(q > h1.y);  // skip iff q > tau  (alpha < 1/255)
       if (COUNT) {
-        int live = 0;
+        int live = 0, logical = 0;
 #pragma unroll
-        for (int s = 0; s < S; ++s) live += ((tag.y >> s) & 1u) && T[s] > 0.0f;
+        for (int s = 0; s < S; ++s) {
+          const bool l = ((tag.y >> s) & 1u) && T[s] > 0.0f;
+          live += l;
+          logical += l ? (a.n_unique ? (int)(s_mhi[s] - s_mlo[s]) : 1) : 0;  // every member of the class
+        }
         n_shared += live > 0;
-        n_logical += live;
+        n_logical += logical;
         n_state += pass ? live : 0;
       }
       if (!__any_sync(0xffffffffu, pass)) continue;
@@ -257,9 +285,19 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
     const float o0 = __fmaf_rn(Tf, bg0, Cr[s]);
     const float o1 = __fmaf_rn(Tf, bg1, Cg[s]);
     const float o2 = __fmaf_rn(Tf, bg2, Cb[s]);
-    if (a.out && inside && b0 + s < a.B) {
-      float* op = a.out + (((size_t)(b0 + s) * a.H + y) * a.W + x) * 3;
-      op[0] = o0; op[1] = o1; op[2] = o2;
+    if (a.out && inside && s_rep[s] >= 0) {
+      const size_t pix = ((size_t)y * a.W + x) * 3;
+      const size_t img = (size_t)a.H * a.W * 3;
+      if (a.n_unique) {  // every state of the class receives the (identical) tile
+        const uint32_t* mem = a.uorder + (size_t)tile * a.B;
+        for (uint32_t i = s_mlo[s]; i < s_mhi[s]; ++i) {
+          float* op = a.out + (size_t)mem[i] * img + pix;
+          op[0] = o0; op[1] = o1; op[2] = o2;
+        }
+      } else {
+        float* op = a.out + (size_t)s_rep[s] * img + pix;
+        op[0] = o0; op[1] = o1; op[2] = o2;
+      }
     }
     if (a.ref) {
       const float e = inside ? pixel_sq_err(o0, o1, o2, rr0, rr1, rr2) : 0.0f;
@@ -269,11 +307,16 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
   }
   if (a.ref) {
     __syncthreads();
-    if (tid < S && b0 + tid < a.B) {
+    if (tid < S && s_rep[tid] >= 0) {
       double acc = s_red[0][tid];
 #pragma unroll
       for (int k = 1; k < 8; ++k) acc += s_red[k][tid];
-      a.sse_part[(size_t)(b0 + tid) * a.tiles + tile] = acc;
+      if (a.n_unique) {
+        const uint32_t* mem = a.uorder + (size_t)tile * a.B;
+        for (uint32_t i = s_mlo[tid]; i < s_mhi[tid]; ++i) a.sse_part[(size_t)mem[i] * a.tiles + tile] = acc;
+      } else {
+        a.sse_part[(size_t)s_rep[tid] * a.tiles + tile] = acc;
+      }
     }
   }
 }
@@ -345,6 +388,7 @@ void count_launches(int n) { g_launches += (unsigned long long)n; }
 unsigned long long launches_total() { return g_launches; }
 
 int g_state_block = 8;  // S; set through gsr_set_option for experiments (1, 4, 8, 16)
+int g_dedup = 1;        // gsr_set_option("dedup", 0/1): tile-level state dedup
 int g_profile = 0;      // gsr_set_option("profile", 1): record events around every k_composite launch
 constexpr int kMaxProfEvents = 8192;
 static cudaEvent_t g_ev[kMaxProfEvents][2];
@@ -395,6 +439,7 @@ static CompositeArgs make_args(const DeviceScene& sc, const FrameParams& fp, Wor
   a.W = fp.W; a.H = fp.H; a.TX = fp.TX; a.tiles = fp.TX * fp.TY;
   a.bg[0] = fp.bg[0]; a.bg[1] = fp.bg[1]; a.bg[2] = fp.bg[2];
   a.out = nullptr; a.ref = nullptr; a.sse_part = ws.sse_part; a.counts = nullptr;
+  a.uorder = nullptr; a.upos = nullptr; a.n_unique = nullptr;
   return a;
 }
 
@@ -416,6 +461,9 @@ void launch_composite(const DeviceScene& sc, const FrameParams& fp, Workspace& w
   if (B == 0) return;
   CompositeArgs a = make_args(sc, fp, ws, depth_rows, B);
   a.out = out; a.ref = ref;
+  if (g_dedup && launch_tile_dedup(sc, fp, ws, depth_rows, B, st)) {
+    a.uorder = ws.uorder; a.upos = ws.upos; a.n_unique = ws.n_unique;
+  }
   dispatch_composite<false>(a, st);
   if (ref) launch_distortion_finalize(ws.sse_part, B, a.tiles, (int64_t)3 * fp.W * fp.H, mse, psnr, st);
 }
@@ -425,6 +473,9 @@ void launch_composite_count(const DeviceScene& sc, const FrameParams& fp, Worksp
   if (B == 0) return;
   CompositeArgs a = make_args(sc, fp, ws, depth_rows, B);
   a.counts = counts;
+  if (g_dedup && launch_tile_dedup(sc, fp, ws, depth_rows, B, st)) {
+    a.uorder = ws.uorder; a.upos = ws.upos; a.n_unique = ws.n_unique;
+  }
   dispatch_composite<true>(a, st);
 }
 
