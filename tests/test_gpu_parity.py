@@ -370,3 +370,93 @@ def test_host_buffer_frame_call_matches_device_calls(gsr, torch_mod):
     for name in u.dtype.names:
         assert np.array_equal(u[name], util_h[name])
     scene.close()
+
+
+# ------------------------------------------------------------------------------------------ dedup / culling
+def test_tile_dedup_is_bitwise_neutral_and_hash_mode(gsr, torch_mod, oracle_mod):
+    """24 clusters piled on the same screen area: more than 21 clusters per tile, so the dedup keys are
+    hashes (exactly verified); plus duplicated states.  Dedup on/off must give identical bits."""
+    rng = np.random.default_rng(21)
+    C, per = 24, 40
+    n = C * per
+    clu = np.repeat(np.arange(C), per)
+    lev = rng.integers(0, 4, n)
+    means = rng.uniform(-0.25, 0.25, (n, 3))
+    sc, _ = tiny_scene(means, rng.uniform(0.03, 0.08, (n, 3)), quats=rng.standard_normal((n, 4)),
+                       logits=rng.normal(0.5, 1.0, n), colors=rng.uniform(0, 1, (n, 3)), levels=lev, clusters=clu,
+                       C=C, sh_degree=1, R=2, background=(0.3, 0.3, 0.3),
+                       motion_q=rng.integers(-100, 100, (n, 2, 3)).astype(np.int8),
+                       motion_scale=np.full(C, 2e-4), sh_res=0.05 * rng.standard_normal((n, 4, 3)))
+    cam = axis_camera(W=72, H=56, f=120.0)
+    lv = synth.sample_levels(rng, 96, C)
+    lv[40:60] = lv[0:20]                      # exact duplicates
+    lv[60:80] = lv[0:20]
+    lv[60:80, 5] = np.where(lv[60:80, 5] < 3, lv[60:80, 5] + 1, 2)   # pairs differing in one cluster
+    scene = gsr.Scene(sc)
+    osc = oracle_mod.OracleScene(sc)
+    out, _, _, _ = _render(torch_mod, scene, cam, 0.4, lv)
+    gsr.set_option("dedup", 0)
+    try:
+        out_nd, _, _, _ = _render(torch_mod, scene, cam, 0.4, lv)
+    finally:
+        gsr.set_option("dedup", 1)
+    assert torch_mod.equal(out, out_nd)
+    assert torch_mod.equal(out[40:60], out[0:20])
+    ref, _ = osc.render_batch(cam, 0.4, lv)
+    assert np.abs(out.cpu().numpy() - ref).max() <= PIX_TOL
+    for b in (0, 47, 95):
+        one, _, _, _ = _render(torch_mod, scene, cam, 0.4, lv[b:b + 1])
+        assert torch_mod.equal(one[0], out[b])
+    scene.close()
+
+
+def test_subtile_culling_never_drops_a_contribution(gsr, torch_mod, oracle_mod):
+    """Needle-like, strongly rotated, nearly opaque Gaussians (ill-conditioned conics) and faint ones
+    (tau near 0): the conservative culling boxes must keep every pixel that passes the cut."""
+    rng = np.random.default_rng(22)
+    n = 300
+    means = np.stack([rng.uniform(-1.2, 1.2, n), rng.uniform(-0.9, 0.9, n), rng.uniform(-0.5, 0.5, n)], 1)
+    scales = np.stack([rng.uniform(0.2, 0.6, n), rng.uniform(0.002, 0.01, n), rng.uniform(0.002, 0.01, n)], 1)
+    logits = np.where(rng.uniform(size=n) < 0.5, 6.0, -5.2)        # o ~ 0.9975 or ~ 0.0055 (tau ~ 0.34)
+    sc, _ = tiny_scene(means, scales, quats=rng.standard_normal((n, 4)), logits=logits,
+                       colors=rng.uniform(0, 1, (n, 3)), levels=rng.integers(0, 4, n),
+                       clusters=rng.integers(0, 3, n), C=3, background=(1.0, 1.0, 1.0))
+    cam = axis_camera(W=160, H=120, f=110.0)
+    lv = synth.all_closed_states(3)[::5]
+    scene = gsr.Scene(sc)
+    osc = oracle_mod.OracleScene(sc)
+    out, _, _, _ = _render(torch_mod, scene, cam, 0.0, lv)
+    ref, _ = osc.render_batch(cam, 0.0, lv)
+    assert np.abs(out.cpu().numpy() - ref).max() <= PIX_TOL
+    scene.close()
+
+
+def test_full_size_cfg1_frame_sampled_states(gsr, torch_mod, oracle_mod):
+    """configs[1] at full size in the launch configuration bench.py times (B = 256, default state block,
+    dedup on, fused distortion): sampled states element by element against the oracle, I_b for all."""
+    wl = synth.workload_cfg1(n_frames=2)
+    cam, t = wl.frames[1]
+    lv = wl.levels[1]
+    scene = gsr.Scene(wl.scene)
+    osc = oracle_mod.OracleScene(wl.scene)
+    B = lv.shape[0]
+    ws = scene.new_workspace(cam, B)
+    out = torch_mod.empty((B, cam.H, cam.W, 3), dtype=torch_mod.float32, device="cuda")
+    ref = torch_mod.empty((cam.H, cam.W, 3), dtype=torch_mod.float32, device="cuda")
+    mse = torch_mod.empty(B, dtype=torch_mod.float64, device="cuda")
+    psnr = torch_mod.empty(B, dtype=torch_mod.float32, device="cuda")
+    scene.render_states_vs_full(cam, t, _dev_levels(torch_mod, lv), ws, ref, mse, psnr, out=out)
+    scene.status(ws)
+    pick = [0, 37, 128, 255]
+    o_img, o_stats = osc.render_batch(cam, t, np.concatenate([lv[pick], np.full((1, wl.scene.C), 3, np.int8)]))
+    for k, b in enumerate(pick):
+        assert np.abs(out[b].cpu().numpy() - o_img[k]).max() <= PIX_TOL, b
+    assert np.abs(ref.cpu().numpy() - o_img[-1]).max() <= PIX_TOL
+    o_mse, o_psnr = oracle_mod.distortion(o_img[:-1], o_img[-1])
+    assert np.max(np.abs(psnr.cpu().numpy()[pick] - o_psnr)) <= DB_TOL
+    counts = scene.debug_state_counts(ws, B)
+    assert np.array_equal(counts[pick], o_stats[:-1, 0])
+    # the unfused reduction over the materialised images gives the same bits as the fused one
+    mse_u, psnr_u = gsr.distortion(out, ref)
+    assert torch_mod.equal(mse_u, mse) and torch_mod.equal(psnr_u, psnr)
+    scene.close()
