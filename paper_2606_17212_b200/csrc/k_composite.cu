@@ -48,6 +48,16 @@ __device__ __forceinline__ uint2 lds64(uint32_t addr) {
   asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
   return v;
 }
+__device__ __forceinline__ uint32_t lds32(uint32_t addr) {
+  uint32_t v;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ uint32_t lds8(uint32_t addr) {
+  uint32_t v;
+  asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(addr));
+  return v;
+}
 __device__ __forceinline__ float2 lds64f(uint32_t addr) {
   float2 v;
   asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
@@ -85,7 +95,8 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
   extern __shared__ uint16_t s_tab[];  // [C][4]: states (bit s) with depth ==0, >=1, >=2, >=3
   // staged records, 64 B each: {m_x, m_y, A, B} {Cq, o, tau, act | res << 16} {rgb} {rgb + SH residual}
   __shared__ __align__(16) float4 s_rec[kTilePix * 4];
-  __shared__ uint32_t s_wcnt[8];
+  __shared__ uint32_t s_lcnt[8][8];            // [list k][source warp]
+  __shared__ __align__(16) uint8_t s_list[8][kTilePix];  // per 8x4 block: ordered staging slots that touch it
   __shared__ double s_red[8][S];
 
   const int tid = threadIdx.x, lane = tid & 31;
@@ -185,40 +196,50 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
 #pragma unroll
       for (int k = 0; k < 8; ++k) wmask |= (((ox >> (k & 1)) & (oy >> (k >> 1))) & 1u) << k;
     }
-    const bool keep = act != 0 && wmask != 0;
-    const uint32_t bal = __ballot_sync(0xffffffffu, keep);
-    if (lane == 0) s_wcnt[w] = __popc(bal);
-    __syncthreads();
-    uint32_t woff = 0, nb = 0;
+    // ordered compaction: the record keeps slot `tid` of the staging buffer; each 8x4 pixel block k gets
+    // the ordered list s_list[k] of the slots whose box touches it (warp ballots + an 8x8 count table)
+    if (!(act != 0)) wmask = 0;
+    uint32_t balk[8];
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
-      const uint32_t cnt = s_wcnt[k];
-      if (k < w) woff += cnt;
-      nb += cnt;
+      balk[k] = __ballot_sync(0xffffffffu, (wmask >> k) & 1u);
+      if (lane == k) s_lcnt[k][w] = __popc(balk[k]);  // lane k publishes the count of list k
     }
-    if (keep) {
-      const uint32_t pos = woff + __popc(bal & ((1u << lane) - 1u));
-      s_rec[4 * pos + 0] = g0;
-      s_rec[4 * pos + 1] = make_float4(g1.x, g1.z, __uint_as_float(wmask), __uint_as_float(act | (res << 16)));
-      s_rec[4 * pos + 2] = make_float4(c0.x, c0.y, c0.z, g1.y);
-      s_rec[4 * pos + 3] = c1;
+    if (wmask != 0) {
+      s_rec[4 * tid + 0] = g0;
+      s_rec[4 * tid + 1] = make_float4(g1.x, g1.z, 0.0f, __uint_as_float(act | (res << 16)));
+      s_rec[4 * tid + 2] = make_float4(c0.x, c0.y, c0.z, g1.y);
+      s_rec[4 * tid + 3] = c1;
+    }
+    __syncthreads();
+    uint32_t nb = 0;  // length of this warp's list
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      uint32_t off = 0;
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+        const uint32_t cnt = s_lcnt[k][q];
+        if (q < w) off += cnt;
+        if (k == w) nb += cnt;
+      }
+      if ((wmask >> k) & 1u) s_list[k][off + __popc(balk[k] & ((1u << lane) - 1u))] = (uint8_t)tid;
     }
     __syncthreads();
 
-    // ---- composite the staged records in order
+    // ---- composite this warp's records in order
     uint32_t walive = 0;
-    uint32_t addr = rec_base;
-    const uint32_t wbit = 1u << w;
-    for (uint32_t j = 0; j < nb; ++j, addr += 64u) {
+    const uint32_t lbase = (uint32_t)__cvta_generic_to_shared(&s_list[w][0]);
+    for (uint32_t j = 0; j < nb; ++j) {
       if ((j & 31u) == 0) {  // refresh the (warp, state) liveness mask
         walive = 0;
 #pragma unroll
         for (int s = 0; s < S; ++s) walive |= (uint32_t)(__any_sync(0xffffffffu, T[s] > 0.0f) != 0) << s;
         if (walive == 0) break;
       }
-      const uint2 tag = lds64(addr + 24u);  // {8x4-block mask, act | res << 16}
+      const uint32_t addr = rec_base + 64u * lds8(lbase + j);
+      const uint2 tag = make_uint2(0u, lds32(addr + 28u));  // act | res << 16
       const uint32_t actw = tag.y & walive;
-      if ((tag.x & wbit) == 0 || actw == 0) continue;
+      if (actw == 0) continue;
       const float4 h0 = lds128(addr);
       const float2 h1 = lds64f(addr + 16u);  // {Cq, tau}
       // spec-exact quadratic form: u = A dx; s = fma(B,dy,u); q = s dx; v = Cq dy; q = fma(v,dy,q)
