@@ -28,7 +28,7 @@ ROOT = Path(__file__).resolve().parent
 if str(ROOT) not in sys.path:
     sys.path.insert(0, str(ROOT))
 
-from paper_2606_17212_b200 import synth  # noqa: E402
+from paper_2606_17212_b200 import shard, synth  # noqa: E402
 
 # FLOP accounting of the compositing kernel, FMA = 2 flop:
 #   per (pixel, record) alpha evaluation : dx, dy (2) + u (1) + s (2) + q (1) + v (1) + q (2) + o*e (1) + 1-alpha (1) = 11
@@ -191,7 +191,7 @@ def run_ours(args):
     util = torch.zeros((max(G, 1), 9), dtype=torch.float64, device=dev)
 
     def frame_of(step):
-        return (step * world + rank) % n_frames
+        return shard.frame_for_step(step, rank, world, n_frames)
 
     def step(k, images=True):
         f = frame_of(k)
@@ -210,11 +210,7 @@ def run_ours(args):
         e1.record()
         torch.cuda.synchronize()
         ms = e0.elapsed_time(e1)
-        if dist is not None:
-            tms = torch.tensor([ms], dtype=torch.float64, device=dev)
-            dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-            ms = float(tms.item())
-        return ms
+        return shard.max_over_ranks(ms, device=dev)
 
     # ---- warm-up, then the timed region (device-resident inputs), clocks sampled during it
     for k in range(args.warmup):

@@ -164,44 +164,23 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_hist(const unsigned long
   hist[(size_t)threadIdx.x * nblk + blockIdx.x] = h[threadIdx.x];
 }
 
-__global__ void __launch_bounds__(1024) k_radix_scan(uint32_t* __restrict__ hist, const WsHeader* __restrict__ hdr) {
+// one warp per digit: exclusive prefix of that digit's per-block counts (in place) and the digit total,
+// stored behind the table at hist[256 * nblk + digit]; the scatter kernel scans the 256 totals itself
+__global__ void __launch_bounds__(256) k_radix_scan(uint32_t* __restrict__ hist, const WsHeader* __restrict__ hdr) {
   const unsigned long long n = hdr->n_keys;
   const uint32_t nblk = (uint32_t)((n + kSortTileKeys - 1) / kSortTileKeys);
-  const uint32_t total = 256u * nblk;
-  __shared__ uint32_t wsum[32];
-  __shared__ uint32_t carry_s;
-  if (threadIdx.x == 0) carry_s = 0;
-  __syncthreads();
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  // each thread owns 4 consecutive entries per round -> 4096 entries per round
-  for (uint32_t base = 0; base < total; base += 4096u) {
-    uint32_t i0 = base + threadIdx.x * 4u;
-    uint32_t v[4], s = 0;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      v[k] = (i0 + k < total) ? hist[i0 + k] : 0u;
-      s += v[k];
-    }
-    uint32_t inc = warp_incl_scan(s);
-    if (lane == 31) wsum[w] = inc;
-    __syncthreads();
-    if (w == 0) {
-      uint32_t x = wsum[lane];
-      uint32_t xi = warp_incl_scan(x);
-      wsum[lane] = xi - x;  // exclusive prefix of warp sums
-    }
-    __syncthreads();
-    uint32_t carry = carry_s;
-    uint32_t ex = carry + wsum[w] + inc - s;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      if (i0 + k < total) hist[i0 + k] = ex;
-      ex += v[k];
-    }
-    __syncthreads();
-    if (threadIdx.x == 1023) carry_s = ex;  // last thread's running end = carry + round total
-    __syncthreads();
+  const int lane = threadIdx.x & 31;
+  const uint32_t d = blockIdx.x * 8 + (threadIdx.x >> 5);
+  uint32_t* row = hist + (size_t)d * nblk;
+  uint32_t carry = 0;
+  for (uint32_t base = 0; base < nblk; base += 32) {
+    const uint32_t b = base + lane;
+    const uint32_t v = b < nblk ? row[b] : 0u;
+    const uint32_t inc = warp_incl_scan(v);
+    if (b < nblk) row[b] = carry + inc - v;
+    carry += __shfl_sync(0xffffffffu, inc, 31);
   }
+  if (lane == 0) hist[(size_t)256 * nblk + d] = carry;
 }
 
 __global__ void __launch_bounds__(kSortThreads) k_radix_scatter(const unsigned long long* __restrict__ keys_in,
@@ -245,8 +224,16 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_scatter(const unsigned l
   }
   __syncthreads();
   {  // per digit: exclusive prefix over warps + the block's global base
+    //   base(d) = sum of the totals of digits < d  +  this digit's count in earlier blocks
     const int d = threadIdx.x;
-    uint32_t acc = hist[(size_t)d * nblk + blockIdx.x];
+    __shared__ uint32_t s_w8[8];
+    const uint32_t tot = hist[(size_t)256 * nblk + d];
+    const uint32_t inc = warp_incl_scan(tot);
+    if (lane == 31) s_w8[w] = inc;
+    __syncthreads();
+    uint32_t dbase = inc - tot;
+    for (int ww = 0; ww < w; ++ww) dbase += s_w8[ww];
+    uint32_t acc = hist[(size_t)d * nblk + blockIdx.x] + dbase;
 #pragma unroll
     for (int ww = 0; ww < kSortThreads / 32; ++ww) {
       uint32_t c = cnt[ww][d];
@@ -300,7 +287,7 @@ void launch_bin_and_sort(const DeviceScene& sc, const FrameParams& fp, Workspace
   for (int p = 0; p < passes; ++p) {
     const int in = p & 1, out = in ^ 1, shift = 8 * p;
     k_radix_hist<<<sort_blocks, kSortThreads, 0, st>>>(ws.keys[in], ws.hdr, shift, ws.hist);
-    k_radix_scan<<<1, 1024, 0, st>>>(ws.hist, ws.hdr);
+    k_radix_scan<<<32, 256, 0, st>>>(ws.hist, ws.hdr);
     k_radix_scatter<<<sort_blocks, kSortThreads, 0, st>>>(ws.keys[in], ws.vals[in], ws.keys[out], ws.vals[out],
                                                           ws.hdr, shift, ws.hist);
   }

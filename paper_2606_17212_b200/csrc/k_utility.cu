@@ -138,8 +138,28 @@ __global__ void __launch_bounds__(kUtilThreads) k_group_utility(PairView pv, int
     const int lo = (int)floor(posq);
     const int hi = lo + 1 < n_g ? lo + 1 : n_g - 1;
     const double fr = posq - (double)lo;
-    const double vlo = select_kth(pv, g, metric, n_g, cached ? cache : nullptr, lo, sm_c);
-    const double vhi = hi == lo ? vlo : select_kth(pv, g, metric, n_g, cached ? cache : nullptr, hi, sm_c);
+    double vlo, vhi;
+    if (cached) {
+      // rank by counting (ties broken by position: ranks are a permutation) — one pass, no sort
+      __shared__ double s_sel[2];
+      for (int i = threadIdx.x; i < n_g; i += kUtilThreads) {
+        const double v = cache[i];
+        int r = 0;
+        for (int j = 0; j < n_g; ++j) {
+          const double c = cache[j];
+          r += (c < v) || (c == v && j < i);
+        }
+        if (r == lo) s_sel[0] = v;
+        if (r == hi) s_sel[1] = v;
+      }
+      __syncthreads();
+      vlo = s_sel[0];
+      vhi = s_sel[1];
+      __syncthreads();
+    } else {
+      vlo = select_kth(pv, g, metric, n_g, nullptr, lo, sm_c);
+      vhi = hi == lo ? vlo : select_kth(pv, g, metric, n_g, nullptr, hi, sm_c);
+    }
     const double q10 = vlo + fr * (vhi - vlo);
     const double alpha = 0.25, beta = 0.05;
     res[metric][0] = mean;
