@@ -50,6 +50,8 @@ def build_workload(name: str, n_frames: int):
         return synth.workload_cfg1(n_frames=n_frames)
     if name == "cfg2":
         return synth.workload_cfg2(n_frames=n_frames)
+    if name == "cfg3":
+        return synth.workload_cfg3(n_views=max(1, min(8, n_frames)))
     if name == "cfg4":
         wl = synth.workload_cfg4()
         return wl
@@ -324,7 +326,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg1", choices=["cfg0", "cfg1", "cfg2", "cfg4"])
+    ap.add_argument("--workload", default="cfg1", choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"])
     ap.add_argument("--ref-states", type=int, default=64, help="states per frame the CPU oracle renders")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--state-block", type=int, default=0, help="states per compositing CTA (0 = library default)")

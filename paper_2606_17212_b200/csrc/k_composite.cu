@@ -9,8 +9,13 @@
 //     shared by S states : dx, dy, q (spec-exact fp32), the cut q > tau, exp, alpha, 1-alpha
 //     per present state  : T' = T(1-alpha); stop if T' < 1e-4; C += alpha T c; T = T'
 //
-// Staging: the tile's records are gathered 256 at a time into shared memory; records present in none
-// of the S states are dropped on the way with a warp-ballot ordered compaction.  Warp ballots also
+// With tile-level dedup (k_dedup.cu) the S "states" of a CTA are S distinct signature classes of the
+// tile; the result is written to every member state of each class.
+//
+// Staging: the tile's records are gathered 256 at a time into shared memory (64 B each).  A warp owns
+// an 8x4 pixel block; per block an ordered list of the staged records whose conservative q <= tau box
+// (k_project) touches it and that are present in at least one of the S states is built with warp
+// ballots, so the hot loop only visits records that can matter to the warp.  Warp ballots also
 // (i) skip a record when no pixel of the warp passes the cut and (ii) retire (warp, state) pairs
 // whose 32 pixels have all terminated; the CTA leaves the list when every (pixel, state) is done.
 //
@@ -93,7 +98,7 @@ constexpr float kAlphaCap = 0.99f;  // reading A11
 template <int S, bool COUNT>
 __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const CompositeArgs a) {
   extern __shared__ uint16_t s_tab[];  // [C][4]: states (bit s) with depth ==0, >=1, >=2, >=3
-  // staged records, 64 B each: {m_x, m_y, A, B} {Cq, o, tau, act | res << 16} {rgb} {rgb + SH residual}
+  // staged records, 64 B each: {m_x, m_y, A, B} {Cq, tau, -, act | res << 16} {rgb, o} {rgb + SH residual, -}
   __shared__ __align__(16) float4 s_rec[kTilePix * 4];
   __shared__ uint32_t s_lcnt[8][8];            // [list k][source warp]
   __shared__ __align__(16) uint8_t s_list[8][kTilePix];  // per 8x4 block: ordered staging slots that touch it
