@@ -58,9 +58,9 @@ __device__ __forceinline__ uint32_t lds32(uint32_t addr) {
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
   return v;
 }
-__device__ __forceinline__ uint32_t lds8(uint32_t addr) {
+__device__ __forceinline__ uint32_t lds16(uint32_t addr) {
   uint32_t v;
-  asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(addr));
+  asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(addr));
   return v;
 }
 __device__ __forceinline__ float2 lds64f(uint32_t addr) {
@@ -69,39 +69,48 @@ __device__ __forceinline__ float2 lds64f(uint32_t addr) {
   return v;
 }
 
-// One (pixel, state) step of DESIGN.md §3.5, branch-free:  T' = T (1 - alpha);  if T' >= 1e-4 { C += (alpha T) c;
-// T = T' } else { T = -|T| }.  T < 0 marks a finished pixel (-(frozen transmittance)): then T' <= 0 and it
-// stays finished.  A lane that failed the cut has alpha = 0, for which the step is exactly a no-op.
+// One (pixel, state) step of DESIGN.md §3.5:  T' = T (1 - alpha);  if T' >= 1e-4 { C += (alpha T) c; T = T' }
+// else { T = -|T| }.  T < 0 marks a finished pixel (-(frozen transmittance)): then T' <= 0 and it stays
+// finished.  A lane that failed the cut has alpha = 0, for which the step is exactly a no-op.
 // Explicitly rounded (mul.rn / fma.rn, never contracted) and predicated, so that every instantiation of
 // the kernel applies bit-identical arithmetic to a state: batched == serial.
+// Pipe balance (profiles/r1b): the half-rate ALU pipe (FSETP/FSEL/LOP3) was the binding unit, so the step
+// keeps ONE compare and ONE select (with the -|T| folded into its operand) there; the rest is FMA-pipe work.
 __device__ __forceinline__ void state_update(float& T, float& Cr, float& Cg, float& Cb, float om, float alpha,
                                              float cr, float cg, float cb) {
   asm("{\n\t"
       ".reg .pred p;\n\t"
-      ".reg .f32 tn, wg;\n\t"
+      ".reg .f32 tn, wg, tm;\n\t"
       "mul.rn.f32 tn, %0, %4;\n\t"
       "setp.geu.f32 p, tn, 0f38D1B717;\n\t"  // 1e-4f
       "mul.rn.f32 wg, %5, %0;\n\t"
       "@p fma.rn.f32 %1, wg, %6, %1;\n\t"
       "@p fma.rn.f32 %2, wg, %7, %2;\n\t"
       "@p fma.rn.f32 %3, wg, %8, %3;\n\t"
-      "@!p or.b32 %0, %0, 0x80000000;\n\t"
-      "@p mov.f32 %0, tn;\n\t"
+      "abs.f32 tm, %0;\n\t"
+      "neg.f32 tm, tm;\n\t"
+      "selp.f32 %0, tn, tm, p;\n\t"
       "}"
       : "+f"(T), "+f"(Cr), "+f"(Cg), "+f"(Cb)
       : "f"(om), "f"(alpha), "f"(cr), "f"(cg), "f"(cb));
+}
+
+__device__ __forceinline__ float ex2_approx_ftz(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
 }
 
 constexpr float kTStop = 1e-4f;     // reading A11
 constexpr float kAlphaCap = 0.99f;  // reading A11
 
 template <int S, bool COUNT>
-__global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const CompositeArgs a) {
+__global__ void __launch_bounds__(kTilePix, (S <= 8 ? 4 : 2)) k_composite(const CompositeArgs a) {
   extern __shared__ uint16_t s_tab[];  // [C][4]: states (bit s) with depth ==0, >=1, >=2, >=3
   // staged records, 64 B each: {m_x, m_y, A, B} {Cq, tau, -, act | res << 16} {rgb, o} {rgb + SH residual, -}
   __shared__ __align__(16) float4 s_rec[kTilePix * 4];
   __shared__ uint32_t s_lcnt[8][8];            // [list k][source warp]
-  __shared__ __align__(16) uint8_t s_list[8][kTilePix];  // per 8x4 block: ordered staging slots that touch it
+  __shared__ __align__(16) uint16_t s_list[8][kTilePix];  // per 8x4 block: ordered shared-window addresses of the staged records that touch it
   __shared__ double s_red[8][S];
 
   const int tid = threadIdx.x, lane = tid & 31;
@@ -158,7 +167,9 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
   const bool inside = x < a.W && y < a.H;
   float px = (float)x + 0.5f, py = (float)y + 0.5f;
   asm volatile("" : "+f"(px), "+f"(py));  // keep them in registers (the compiler would rebuild them per record)
-  const uint32_t rec_base = (uint32_t)__cvta_generic_to_shared(s_rec);
+  uint32_t rec_base = (uint32_t)__cvta_generic_to_shared(s_rec);
+  uint32_t lbase = (uint32_t)__cvta_generic_to_shared(&s_list[w][0]);
+  asm volatile("" : "+r"(rec_base), "+r"(lbase));  // loop-invariant: keep them in registers
   const float bg0 = a.bg[0], bg1 = a.bg[1], bg2 = a.bg[2];
 
   float T[S], Cr[S], Cg[S], Cb[S];
@@ -227,64 +238,71 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 3 : 2)) k_composite(const 
         if (q < w) off += cnt;
         if (k == w) nb += cnt;
       }
-      if ((wmask >> k) & 1u) s_list[k][off + __popc(balk[k] & ((1u << lane) - 1u))] = (uint8_t)tid;
+      if ((wmask >> k) & 1u) s_list[k][off + __popc(balk[k] & ((1u << lane) - 1u))] = (uint16_t)(rec_base + 64u * tid);
     }
     __syncthreads();
 
     // ---- composite this warp's records in order
-    uint32_t walive = 0;
-    const uint32_t lbase = (uint32_t)__cvta_generic_to_shared(&s_list[w][0]);
-    for (uint32_t j = 0; j < nb; ++j) {
-      if ((j & 31u) == 0) {  // refresh the (warp, state) liveness mask
-        walive = 0;
+    for (uint32_t j0 = 0; j0 < nb; j0 += 32u) {
+      // refresh the (warp, slot) liveness mask every 32 records
+      uint32_t walive = 0;
 #pragma unroll
-        for (int s = 0; s < S; ++s) walive |= (uint32_t)(__any_sync(0xffffffffu, T[s] > 0.0f) != 0) << s;
-        if (walive == 0) break;
-      }
-      const uint32_t addr = rec_base + 64u * lds8(lbase + j);
-      const uint2 tag = make_uint2(0u, lds32(addr + 28u));  // act | res << 16
-      const uint32_t actw = tag.y & walive;
-      if (actw == 0) continue;
-      const float4 h0 = lds128(addr);
-      const float2 h1 = lds64f(addr + 16u);  // {Cq, tau}
-      // spec-exact quadratic form: u = A dx; s = fma(B,dy,u); q = s dx; v = Cq dy; q = fma(v,dy,q)
-      const float dx = __fsub_rn(h0.x, px);
-      const float dy = __fsub_rn(h0.y, py);
-      const float u = __fmul_rn(h0.z, dx);
-      const float sacc = __fmaf_rn(h0.w, dy, u);
-      float q = __fmul_rn(sacc, dx);
-      const float v = __fmul_rn(h1.x, dy);
-      q = __fmaf_rn(v, dy, q);
-      const bool pass = !(q > h1.y);  // skip iff q > tau  (alpha < 1/255)
-      if (COUNT) {
-        int live = 0, logical = 0;
+      for (int s = 0; s < S; ++s) walive |= (uint32_t)(__any_sync(0xffffffffu, T[s] > 0.0f) != 0) << s;
+      if (walive == 0) break;
+      walive |= 0xFFFF0000u;  // keep the residual bits of the tag
+      const uint32_t j1 = min(nb, j0 + 32u);
+      for (uint32_t j = j0; j < j1; ++j) {
+        const uint32_t addr = lds16(lbase + 2u * j);
+        const uint32_t tagw = lds32(addr + 28u) & walive;  // act | res << 16, dead slots masked out
+        if ((tagw & 0xFFFFu) == 0) continue;
+        const float4 h0 = lds128(addr);
+        const float2 h1 = lds64f(addr + 16u);  // {Cq, tau}
+        // spec-exact quadratic form: u = A dx; s = fma(B,dy,u); q = s dx; v = Cq dy; q = fma(v,dy,q)
+        const float dx = __fsub_rn(h0.x, px);
+        const float dy = __fsub_rn(h0.y, py);
+        const float u = __fmul_rn(h0.z, dx);
+        const float sacc = __fmaf_rn(h0.w, dy, u);
+        float q = __fmul_rn(sacc, dx);
+        const float v = __fmul_rn(h1.x, dy);
+        q = __fmaf_rn(v, dy, q);
+        const bool pass = !(q > h1.y);  // skip iff q > tau  (alpha < 1/255)
+        if (COUNT) {
+          int live = 0, logical = 0;
 #pragma unroll
-        for (int s = 0; s < S; ++s) {
-          const bool l = ((tag.y >> s) & 1u) && T[s] > 0.0f;
-          live += l;
-          logical += l ? (a.n_unique ? (int)(s_mhi[s] - s_mlo[s]) : 1) : 0;  // every member of the class
+          for (int s = 0; s < S; ++s) {
+            const bool l = ((tagw >> s) & 1u) && T[s] > 0.0f;
+            live += l;
+            logical += l ? (a.n_unique ? (int)(s_mhi[s] - s_mlo[s]) : 1) : 0;  // every member of the class
+          }
+          n_shared += live > 0;
+          n_logical += logical;
+          n_state += pass ? live : 0;
         }
-        n_shared += live > 0;
-        n_logical += logical;
-        n_state += pass ? live : 0;
-      }
-      if (!__any_sync(0xffffffffu, pass)) continue;
-      const float4 k0 = lds128(addr + 32u), k1 = lds128(addr + 48u);
-      float alpha = fminf(kAlphaCap, __fmul_rn(k0.w, __expf(-q)));
-      alpha = pass ? alpha : 0.0f;
-      const float om = __fsub_rn(1.0f, alpha);
-      const uint32_t resw = tag.y >> 16;
+        if (!__any_sync(0xffffffffu, pass)) continue;
+        const float4 k0 = lds128(addr + 32u), k1 = lds128(addr + 48u);
+        // q <= tau <= ln 255 on every lane that passes: no denormal range to guard, ex2.approx.ftz is enough
+        float alpha = fminf(kAlphaCap, __fmul_rn(k0.w, ex2_approx_ftz(__fmul_rn(q, -1.4426950408889634f))));
+        alpha = pass ? alpha : 0.0f;
+        const float om = __fsub_rn(1.0f, alpha);
+        // The tag is the same on every lane; the warp reduction only tells the compiler so (it lands in a
+        // uniform register), which turns every slot test below into a plain skip without reconvergence
+        // barriers.  Slots taking the plain colour first, then those taking the colour with the SH residual.
+        const uint32_t tagu = __reduce_or_sync(0xffffffffu, tagw);
+        const uint32_t act1 = tagu & (tagu >> 16), act0 = (tagu & 0xFFFFu) ^ act1;
 #pragma unroll
-      for (int s = 0; s < S; ++s) {
-        if ((actw >> s) & 1u) {  // warp-uniform: the record is present in state s
-          const bool rs = (resw >> s) & 1u;
-          state_update(T[s], Cr[s], Cg[s], Cb[s], om, alpha, rs ? k1.x : k0.x, rs ? k1.y : k0.y, rs ? k1.z : k0.z);
+        for (int s = 0; s < S; ++s)
+          if ((act0 >> s) & 1u) state_update(T[s], Cr[s], Cg[s], Cb[s], om, alpha, k0.x, k0.y, k0.z);
+        if (act1 != 0) {
+#pragma unroll
+          for (int s = 0; s < S; ++s)
+            if ((act1 >> s) & 1u) state_update(T[s], Cr[s], Cg[s], Cb[s], om, alpha, k1.x, k1.y, k1.z);
         }
       }
     }
     bool any_alive = false;
 #pragma unroll
     for (int s = 0; s < S; ++s) any_alive |= T[s] > 0.0f;
+    if (base + kTilePix >= rg.y) break;  // last chunk: nothing left to stage, no need to meet the other warps
     if (!__syncthreads_or(any_alive)) break;
   }
 

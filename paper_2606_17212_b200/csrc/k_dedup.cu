@@ -9,8 +9,12 @@
 //
 // One CTA per tile:
 //   1. class presence bits per cluster from the tile's record list
-//   2. per present cluster, the canonical code (0..4) of each depth -1..3 (equal code <=> same signature)
-//   3. per state a 64-bit key: the packed codes if they fit (3 bits x <= 21 clusters), else a hash
+//   2. per present cluster, the canonical code (0..4) of each depth -1..3 (equal code <=> same signature);
+//      the present clusters are ordered by DESCENDING record count in the tile, so that the sort below makes
+//      consecutive classes agree on the clusters that carry most of the tile's records: a compositing CTA
+//      takes S consecutive classes, and a record it stages is then present in (nearly) all or none of them
+//   3. per state a 64-bit key: the packed codes if they fit (3 bits x <= 21 clusters), else the packed codes
+//      of the 13 heaviest clusters followed by a 24-bit hash of all of them
 //   4. in-CTA bitonic sort of (key, state); a state starts a new class unless its restricted code vector
 //      EQUALS its predecessor's (verified exactly, so a hash collision can only cost dedup, never
 //      correctness)
@@ -41,14 +45,18 @@ __global__ void __launch_bounds__(kDedupThreads) k_tile_dedup(const uint2* __res
                                                               uint32_t* __restrict__ upos,
                                                               uint32_t* __restrict__ n_unique) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  // layout: keys u64[Bp] | idx u32[Bp] | head u32[Bp] | cbits u32[ceil(C/4)] | klist u16[C] | codes u8[5*C]
+  // layout: keys u64[Bp] | idx u32[Bp] | head u32[Bp] | cbits u32[ceil(C/4)] | ccnt u32[C] | klist0 u16[C] |
+  //         klist u16[C] | codes0 u8[5*C] | codes u8[5*C]
   unsigned long long* keys = (unsigned long long*)smem_raw;
   uint32_t* idx = (uint32_t*)(keys + Bp);
   uint32_t* head = idx + Bp;
   uint32_t* cbits = head + Bp;
   const int cwords = (C + 3) / 4;
-  uint16_t* klist = (uint16_t*)(cbits + cwords);
-  uint8_t* codes = (uint8_t*)(klist + ((C + 1) & ~1));
+  uint32_t* ccnt = cbits + cwords;
+  uint16_t* klist0 = (uint16_t*)(ccnt + C);
+  uint16_t* klist = klist0 + ((C + 1) & ~1);
+  uint8_t* codes0 = (uint8_t*)(klist + ((C + 1) & ~1));
+  uint8_t* codes = codes0 + 5 * (size_t)C;
   __shared__ uint32_t s_cnt[8];
   __shared__ uint32_t s_run;
 
@@ -58,12 +66,14 @@ __global__ void __launch_bounds__(kDedupThreads) k_tile_dedup(const uint2* __res
 
   // 1. class presence bits
   for (int k = tid; k < cwords; k += kDedupThreads) cbits[k] = 0;
+  for (int k = tid; k < C; k += kDedupThreads) ccnt[k] = 0;
   __syncthreads();
   for (uint32_t i = rg.x + tid; i < rg.y; i += kDedupThreads) {
     const uint32_t meta = __float_as_uint(r1[vals[i]].w);
     const uint32_t c = meta & 0xFFFFu, cls = meta >> 16;
     const uint32_t bit = cls == 0 ? 1u : (cls <= 2 ? 2u : (cls == 3 ? 4u : 8u));
     atomicOr(&cbits[c >> 2], bit << (8 * (c & 3)));
+    atomicAdd(&ccnt[c], 1u);
   }
   if (tid == 0) s_run = 0;
   __syncthreads();
@@ -82,14 +92,14 @@ __global__ void __launch_bounds__(kDedupThreads) k_tile_dedup(const uint2* __res
     }
     if (present) {
       const uint32_t pos = s_run + woff + __popc(bal & ((1u << lane) - 1u));
-      klist[pos] = (uint16_t)c;
+      klist0[pos] = (uint16_t)c;
       uint32_t sig[5];
       for (int d = -1; d <= 3; ++d) sig[d + 1] = class_sig(bits, d);
       for (int d = 0; d < 5; ++d) {
         int code = d;
         for (int e = d - 1; e >= 0; --e)
           if (sig[e] == sig[d]) code = e;
-        codes[5 * pos + d] = (uint8_t)code;
+        codes0[5 * pos + d] = (uint8_t)code;
       }
     }
     __syncthreads();
@@ -98,18 +108,35 @@ __global__ void __launch_bounds__(kDedupThreads) k_tile_dedup(const uint2* __res
   }
   const int k = (int)s_run;
   const bool packed = 3 * k <= 63;
+  // order the present clusters by descending record count (rank sort; index order beyond 512 clusters)
+  for (int j = tid; j < k; j += kDedupThreads) {
+    int rank = j;
+    if (k <= 512) {
+      const uint32_t mine = ccnt[klist0[j]];
+      rank = 0;
+      for (int i = 0; i < k; ++i) {
+        const uint32_t other = ccnt[klist0[i]];
+        rank += (other > mine) || (other == mine && i < j);
+      }
+    }
+    klist[rank] = klist0[j];
+    for (int d = 0; d < 5; ++d) codes[5 * rank + d] = codes0[5 * j + d];
+  }
+  __syncthreads();
 
   // 3. keys
   for (int b = tid; b < Bp; b += kDedupThreads) {
     unsigned long long key = ~0ull;
     if (b < B) {
       key = 0ull;
+      unsigned long long h = 0ull;
       const int8_t* row = depth + (size_t)b * C;
       for (int j = 0; j < k; ++j) {
         const unsigned long long code = codes[5 * j + row[klist[j]] + 1];
-        key = packed ? ((key << 3) | code) : ((key ^ code) * 0x9E3779B97F4A7C15ull + 0x632BE59BD9B4E019ull);
+        if (packed || j < 13) key = (key << 3) | code;
+        if (!packed) h = (h ^ code) * 0x9E3779B97F4A7C15ull + 0x632BE59BD9B4E019ull;
       }
-      if (!packed) key &= 0x7FFFFFFFFFFFFFFFull;  // keep real keys below the padding key
+      if (!packed) key = (key << 24) | (h >> 40);  // 39 + 24 bits: real keys stay below the padding key
     }
     keys[b] = key;
     idx[b] = b < B ? (uint32_t)b : 0xFFFFFFFFu;
@@ -177,7 +204,7 @@ size_t dedup_smem_bytes(int B, int C, int* Bp_out) {
   int Bp = 2;
   while (Bp < B) Bp <<= 1;
   *Bp_out = Bp;
-  return (size_t)Bp * 16 + (size_t)((C + 3) / 4) * 4 + (size_t)((C + 1) & ~1) * 2 + (size_t)5 * C + 16;
+  return (size_t)Bp * 16 + (size_t)((C + 3) / 4) * 4 + (size_t)C * 4 + 2 * (size_t)((C + 1) & ~1) * 2 + (size_t)10 * C + 16;
 }
 
 // Returns false (and launches nothing) if the batch is too large for the in-CTA sort.
