@@ -167,6 +167,42 @@ int gsr_close_levels(const uint8_t* delivered_mask, int64_t n, int8_t* depth_out
                      void* cuda_stream);
 
 /* ------------------------------------------------------------------------------------------------
+ * Scheduling frontier and partial-state atlas (Fig. 2, Fig. 6; DESIGN.md
+ * §11, readings F1-F4).  Integer / comparison helpers around the renderer: all results are bit-exact and
+ * independent of thread scheduling (ties are broken by the written keys).  Group g = 4*c + l.  All
+ * pointers are dev; all calls are asynchronous on `cuda_stream`.
+ *
+ * gsr_group_wire_bytes: "raw stream bytes plus one 48-byte chunk header and 4 bytes per dependency word
+ *   for each 1200-byte payload chunk": wire[g] = raw[g] + ceil(raw[g]/1200) * (48 + 4 l).
+ *   raw_bytes, wire: int64 [4C].
+ * gsr_frontier_order: greedy dependency-closed total order of the 4C groups.  At every step the eligible
+ *   groups are (c, l) whose prerequisites (c, 0..l-1) are already in the order; the policy takes the one
+ *   with the smallest key: GSR_POLICY_UTILITY (-score[g], l, c) — "render-utility order";
+ *   GSR_POLICY_NOMINAL (l, c) — "nominal layer order"; GSR_POLICY_BYTE_GREEDY (wire[g], l, c) —
+ *   "dependency byte-greedy order".  A flat score table reproduces the nominal order
+ *   (PAPER.md:90).  score: double [4C] (only read for GSR_POLICY_UTILITY, e.g. the risk_db column of
+ *   gsr_group_utility; must be finite); order: int32 [4C]; cum_bytes: int64 [4C] or NULL (running wire sum).
+ * gsr_frontier_states: the state of an order at budget j = its longest prefix whose cumulative wire bytes
+ *   are <= budgets[j]; levels int8 [nb, C] receives each cluster's delivered depth (-1..3), used int64 [nb]
+ *   (or NULL) the bytes of that prefix, n_groups int32 [nb] (or NULL) its length.
+ * gsr_state_bytes: wire cost of dependency-closed states: bytes[b] = sum_c sum_{l <= levels[b,c]} wire[4c+l].
+ *   levels int8 [B, C] (values outside -1..3 are clamped to that range); bytes int64 [B].
+ * gsr_best_state_under_budget: the "empirical oracle" of the atlas: best[j] = the state of highest
+ *   psnr_db among those with state_bytes <= budgets[j]; ties -> lowest index; -1 if none.  best int32 [nb]. */
+#define GSR_POLICY_UTILITY 0
+#define GSR_POLICY_NOMINAL 1
+#define GSR_POLICY_BYTE_GREEDY 2
+int gsr_group_wire_bytes(const int64_t* raw_bytes, int32_t C, int64_t* wire, void* cuda_stream);
+int gsr_frontier_order(const double* score, const int64_t* wire, int32_t C, int32_t policy, int32_t* order,
+                       int64_t* cum_bytes, void* cuda_stream);
+int gsr_frontier_states(const int32_t* order, const int64_t* wire, int32_t C, const int64_t* budgets, int32_t nb,
+                        int8_t* levels, int64_t* used, int32_t* n_groups, void* cuda_stream);
+int gsr_state_bytes(const int8_t* levels, int32_t B, int32_t C, const int64_t* wire, int64_t* bytes,
+                    void* cuda_stream);
+int gsr_best_state_under_budget(const float* psnr_db, const int64_t* state_bytes, int32_t B,
+                                const int64_t* budgets, int32_t nb, int32_t* best, void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------------------
  * One-call convenience with HOST buffers (used for the end-to-end measurement): uploads `levels`
  * and the pair lists, renders the full state (all depths 3) as the reference, renders the batch with
  * fused distortion, aggregates utilities, and copies mse / psnr_db / util back.  Synchronous.

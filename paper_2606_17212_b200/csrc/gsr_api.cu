@@ -453,6 +453,63 @@ int gsr_close_levels(const uint8_t* delivered_mask, int64_t n, int8_t* depth_out
 }
 
 // ------------------------------------------------------------------------------------------------
+// scheduling frontier / partial-state atlas
+int gsr_group_wire_bytes(const int64_t* raw_bytes, int32_t C, int64_t* wire, void* cuda_stream) {
+  if (C <= 0 || C > kMaxC || !raw_bytes || !wire) { set_error("gsr_group_wire_bytes: invalid argument"); return GSR_E_INVALID_ARG; }
+  launch_wire_bytes((const long long*)raw_bytes, C, (long long*)wire, (cudaStream_t)cuda_stream);
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
+int gsr_frontier_order(const double* score, const int64_t* wire, int32_t C, int32_t policy, int32_t* order,
+                       int64_t* cum_bytes, void* cuda_stream) {
+  if (C <= 0 || C > kMaxC || !wire || !order || policy < GSR_POLICY_UTILITY || policy > GSR_POLICY_BYTE_GREEDY ||
+      (policy == GSR_POLICY_UTILITY && !score)) {
+    set_error("gsr_frontier_order: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  launch_frontier_order(score, (const long long*)wire, C, policy, order, (long long*)cum_bytes,
+                        (cudaStream_t)cuda_stream);
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
+int gsr_frontier_states(const int32_t* order, const int64_t* wire, int32_t C, const int64_t* budgets, int32_t nb,
+                        int8_t* levels, int64_t* used, int32_t* n_groups, void* cuda_stream) {
+  if (C <= 0 || C > kMaxC || nb < 0 || !order || !wire || (nb > 0 && (!budgets || !levels))) {
+    set_error("gsr_frontier_states: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  launch_frontier_states(order, (const long long*)wire, C, (const long long*)budgets, nb, levels, (long long*)used,
+                         n_groups, (cudaStream_t)cuda_stream);
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
+int gsr_state_bytes(const int8_t* levels, int32_t B, int32_t C, const int64_t* wire, int64_t* bytes,
+                    void* cuda_stream) {
+  if (C <= 0 || C > kMaxC || B < 0 || !wire || (B > 0 && (!levels || !bytes))) {
+    set_error("gsr_state_bytes: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  launch_state_bytes(levels, B, C, (const long long*)wire, (long long*)bytes, (cudaStream_t)cuda_stream);
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
+int gsr_best_state_under_budget(const float* psnr_db, const int64_t* state_bytes, int32_t B,
+                                const int64_t* budgets, int32_t nb, int32_t* best, void* cuda_stream) {
+  if (B < 0 || nb < 0 || (nb > 0 && (!budgets || !best)) || (B > 0 && (!psnr_db || !state_bytes))) {
+    set_error("gsr_best_state_under_budget: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  launch_best_under_budget(psnr_db, (const long long*)state_bytes, B, (const long long*)budgets, nb, best,
+                           (cudaStream_t)cuda_stream);
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
 // host-buffer convenience call (end-to-end measurement)
 struct FrameCarve {
   size_t o_render, o_levels, o_full, o_ref, o_mse, o_psnr, o_pairs, o_util, o_out, o_refmse, total;

@@ -111,6 +111,17 @@ void launch_close_levels(const uint8_t* mask, int64_t n, int8_t* depth, uint8_t*
 void launch_filter_keys(const DeviceScene& sc, Workspace& ws, int32_t b, uint32_t* tile, uint32_t* dbits,
                         int32_t* gi, unsigned long long* n_out, long long cap, cudaStream_t st);
 
+// scheduling frontier / atlas (k_policy.cu)
+void launch_wire_bytes(const long long* raw, int32_t C, long long* wire, cudaStream_t st);
+void launch_frontier_order(const double* score, const long long* wire, int32_t C, int32_t policy, int32_t* order,
+                           long long* cum, cudaStream_t st);
+void launch_frontier_states(const int32_t* order, const long long* wire, int32_t C, const long long* budgets,
+                            int32_t nb, int8_t* levels, long long* used, int32_t* n_groups, cudaStream_t st);
+void launch_state_bytes(const int8_t* levels, int32_t B, int32_t C, const long long* wire, long long* out,
+                        cudaStream_t st);
+void launch_best_under_budget(const float* psnr, const long long* bytes, int32_t B, const long long* budgets,
+                              int32_t nb, int32_t* best, cudaStream_t st);
+
 void set_error(const char* fmt, ...);
 
 }  // namespace gsr

@@ -500,27 +500,51 @@ static void dispatch_composite(CompositeArgs& a, cudaStream_t st) {
   }
 }
 
+// Batches larger than the in-CTA signature sort of k_tile_dedup can hold (kDedupMaxStates) are composited in
+// equal chunks of states; a state's pixels do not depend on what it is batched with, so this is invisible.
+constexpr int kDedupMaxStates = 8192;
+
+static int chunk_states(int32_t B) {
+  if (!g_dedup || B <= kDedupMaxStates) return B;
+  const int n_chunks = (B + kDedupMaxStates - 1) / kDedupMaxStates;
+  return (B + n_chunks - 1) / n_chunks;
+}
+
 void launch_composite(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, const int8_t* depth_rows,
                       int32_t B, float* out, const float* ref, double* mse, float* psnr, cudaStream_t st) {
   if (B == 0) return;
-  CompositeArgs a = make_args(sc, fp, ws, depth_rows, B);
-  a.out = out; a.ref = ref;
-  if (g_dedup && launch_tile_dedup(sc, fp, ws, depth_rows, B, st)) {
-    a.uorder = ws.uorder; a.upos = ws.upos; a.n_unique = ws.n_unique;
+  const int tiles = fp.TX * fp.TY;
+  const size_t img = (size_t)fp.H * fp.W * 3;
+  const int step = chunk_states(B);
+  for (int b0 = 0; b0 < B; b0 += step) {
+    const int nb = B - b0 < step ? B - b0 : step;
+    const int8_t* rows = depth_rows + (size_t)b0 * sc.C;
+    CompositeArgs a = make_args(sc, fp, ws, rows, nb);
+    a.out = out ? out + (size_t)b0 * img : nullptr;
+    a.ref = ref;
+    a.sse_part = ws.sse_part + (size_t)b0 * tiles;
+    if (g_dedup && launch_tile_dedup(sc, fp, ws, rows, nb, st)) {
+      a.uorder = ws.uorder; a.upos = ws.upos; a.n_unique = ws.n_unique;
+    }
+    dispatch_composite<false>(a, st);
   }
-  dispatch_composite<false>(a, st);
-  if (ref) launch_distortion_finalize(ws.sse_part, B, a.tiles, (int64_t)3 * fp.W * fp.H, mse, psnr, st);
+  if (ref) launch_distortion_finalize(ws.sse_part, B, tiles, (int64_t)3 * fp.W * fp.H, mse, psnr, st);
 }
 
 void launch_composite_count(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, const int8_t* depth_rows,
                             int32_t B, unsigned long long* counts, cudaStream_t st) {
   if (B == 0) return;
-  CompositeArgs a = make_args(sc, fp, ws, depth_rows, B);
-  a.counts = counts;
-  if (g_dedup && launch_tile_dedup(sc, fp, ws, depth_rows, B, st)) {
-    a.uorder = ws.uorder; a.upos = ws.upos; a.n_unique = ws.n_unique;
+  const int step = chunk_states(B);
+  for (int b0 = 0; b0 < B; b0 += step) {
+    const int nb = B - b0 < step ? B - b0 : step;
+    const int8_t* rows = depth_rows + (size_t)b0 * sc.C;
+    CompositeArgs a = make_args(sc, fp, ws, rows, nb);
+    a.counts = counts;
+    if (g_dedup && launch_tile_dedup(sc, fp, ws, rows, nb, st)) {
+      a.uorder = ws.uorder; a.upos = ws.upos; a.n_unique = ws.n_unique;
+    }
+    dispatch_composite<true>(a, st);
   }
-  dispatch_composite<true>(a, st);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -83,6 +83,11 @@ def lib():
         L.gsr_profile_read.argtypes = [C.POINTER(C.c_double), C.POINTER(i32)]
         L.gsr_launch_count.restype = i64
         L.gsr_measure_fp32_peak.argtypes = [C.POINTER(C.c_double), vp]
+        L.gsr_group_wire_bytes.argtypes = [vp, i32, vp, vp]
+        L.gsr_frontier_order.argtypes = [vp, vp, i32, i32, vp, vp, vp]
+        L.gsr_frontier_states.argtypes = [vp, vp, i32, vp, i32, vp, vp, vp, vp]
+        L.gsr_state_bytes.argtypes = [vp, i32, i32, vp, vp, vp]
+        L.gsr_best_state_under_budget.argtypes = [vp, vp, i32, vp, i32, vp, vp]
         _lib = L
     return _lib
 
@@ -332,3 +337,64 @@ def close_levels(mask):
     closure = torch.empty(mask.shape, dtype=torch.uint8, device="cuda")
     _check(lib().gsr_close_levels(_dp(mask), mask.numel(), _dp(depth), _dp(closure), _stream()))
     return depth, closure
+
+
+# ---- scheduling frontier / partial-state atlas (include/gsr.h): marshalling only
+POLICY_UTILITY, POLICY_NOMINAL, POLICY_BYTE_GREEDY = 0, 1, 2
+
+
+def group_wire_bytes(raw_bytes):
+    """gsr_group_wire_bytes: cuda int64 [4C] -> cuda int64 [4C]."""
+    torch = _torch()
+    assert raw_bytes.dtype == torch.int64 and raw_bytes.is_cuda and raw_bytes.is_contiguous()
+    wire = torch.empty_like(raw_bytes)
+    _check(lib().gsr_group_wire_bytes(_dp(raw_bytes), raw_bytes.numel() // 4, _dp(wire), _stream()))
+    return wire
+
+
+def frontier_order(score, wire, policy: int):
+    """gsr_frontier_order -> (order int32 [4C], cum_bytes int64 [4C]) on device."""
+    torch = _torch()
+    n = wire.numel()
+    assert wire.dtype == torch.int64 and wire.is_cuda and wire.is_contiguous()
+    if score is not None:
+        assert score.dtype == torch.float64 and score.is_cuda and score.is_contiguous() and score.numel() == n
+    order = torch.empty(n, dtype=torch.int32, device="cuda")
+    cum = torch.empty(n, dtype=torch.int64, device="cuda")
+    _check(lib().gsr_frontier_order(_dp(score), _dp(wire), n // 4, int(policy), _dp(order), _dp(cum), _stream()))
+    return order, cum
+
+
+def frontier_states(order, wire, budgets, levels_out=None):
+    """gsr_frontier_states -> (levels int8 [nb, C], used int64 [nb], n_groups int32 [nb]) on device."""
+    torch = _torch()
+    Cn, nb = wire.numel() // 4, budgets.numel()
+    assert budgets.dtype == torch.int64 and budgets.is_cuda and order.dtype == torch.int32
+    levels = levels_out if levels_out is not None else torch.empty((nb, Cn), dtype=torch.int8, device="cuda")
+    used = torch.empty(nb, dtype=torch.int64, device="cuda")
+    ng = torch.empty(nb, dtype=torch.int32, device="cuda")
+    _check(lib().gsr_frontier_states(_dp(order), _dp(wire), Cn, _dp(budgets), nb, _dp(levels), _dp(used), _dp(ng),
+                                     _stream()))
+    return levels, used, ng
+
+
+def state_bytes(levels, wire, out=None):
+    """gsr_state_bytes: cuda int8 [B, C] -> cuda int64 [B]."""
+    torch = _torch()
+    B, Cn = int(levels.shape[0]), int(levels.shape[1])
+    assert levels.dtype == torch.int8 and levels.is_cuda and levels.is_contiguous() and wire.numel() == 4 * Cn
+    if out is None:
+        out = torch.empty(B, dtype=torch.int64, device="cuda")
+    _check(lib().gsr_state_bytes(_dp(levels), B, Cn, _dp(wire), _dp(out), _stream()))
+    return out
+
+
+def best_state_under_budget(psnr, bytes_per_state, budgets, out=None):
+    """gsr_best_state_under_budget -> cuda int32 [nb]."""
+    torch = _torch()
+    assert psnr.dtype == torch.float32 and bytes_per_state.dtype == torch.int64 and budgets.dtype == torch.int64
+    if out is None:
+        out = torch.empty(budgets.numel(), dtype=torch.int32, device="cuda")
+    _check(lib().gsr_best_state_under_budget(_dp(psnr), _dp(bytes_per_state), psnr.numel(), _dp(budgets),
+                                             budgets.numel(), _dp(out), _stream()))
+    return out

@@ -384,3 +384,72 @@ def scaled_object_workload(seed_cfg: int, C: int, per_cluster: float, W: int, H:
     frames = [(cams[n], float(np.float32((n + 0.5) / max(n_frames, 1)))) for n in range(n_frames)]
     levels, iw, iwith, gid = _paired_frame_batches(seed_cfg, sc, n_frames, B)
     return Workload(f"scaled_cfg{seed_cfg}_{W}x{H}_B{B}", sc, frames, levels, iw, iwith, gid, 4 * sc.C)
+
+
+# ----------------------------------------------------------------------------- scheduling frontier / atlas inputs
+def group_raw_bytes(sc: Scene) -> np.ndarray:
+    """Synthetic raw stream bytes of the 4C completion groups (input recipe): a Gaussian of
+    a group costs its fp32 attributes (mean 3, log-scale 3, quaternion 4, opacity 1, base SH 3K); the
+    level-1 group also carries the int8 motion coefficients (3R) of the level-0 and level-1 Gaussians,
+    levels 2 and 3 those of their own Gaussians; the level-3 group also carries the fp32 SH residuals (3K)
+    of every Gaussian of the cluster."""
+    K = (sc.sh_degree + 1) ** 2
+    attr = 4 * (11 + 3 * K)
+    n = np.diff(np.asarray(sc.group_off, np.int64)).reshape(sc.C, 4)
+    raw = np.zeros((sc.C, 4), np.int64)
+    raw[:, 0] = n[:, 0] * attr
+    raw[:, 1] = n[:, 1] * attr + (n[:, 0] + n[:, 1]) * 3 * sc.R
+    raw[:, 2] = n[:, 2] * (attr + 3 * sc.R)
+    raw[:, 3] = n[:, 3] * (attr + 3 * sc.R) + n.sum(axis=1) * 12 * K
+    return raw.reshape(-1)
+
+
+@dataclass
+class AtlasWorkload:
+    """Partial-state atlas + scheduling frontier on one scene.
+    Per view: a utility sweep (all 4 groups of every cluster x n_ctx contexts, with / without), then
+    n_atlas sampled closed states + the 5 complete prefixes, then 3 policies x len(budget_fracs) frontier
+    states (built on the device from the measured utilities)."""
+    name: str
+    scene: Scene
+    frames: List[Tuple[Camera, float]]
+    sweep_levels: List[np.ndarray]       # per view int8 [2*n_pairs, C]
+    idx_without: List[np.ndarray]
+    idx_with: List[np.ndarray]
+    group_id: List[np.ndarray]
+    G: int
+    atlas_levels: List[np.ndarray]       # per view int8 [n_atlas + 5, C]
+    raw_bytes: np.ndarray                # int64 [4C]
+    budget_fracs: Tuple[float, ...]      # budgets = floor(frac * total wire bytes)
+
+
+def workload_atlas(n_views: int = 2, n_ctx: int = 8, n_atlas: int = 8192, scene: Scene | None = None,
+                   W: int = 800, H: int = 800, fov: float = 40.0, seed_cfg: int = 5,
+                   budget_fracs=(0.2, 0.4, 0.6, 0.8)) -> AtlasWorkload:
+    """The paper samples 8,197 dependency-closed states per scene: here n_atlas = 8192
+    sampled with the per-level law plus the 5 complete prefixes (all clusters at depth -1, 0, 1, 2, 3)."""
+    sc = scene if scene is not None else scene_cfg1()
+    rng = _rng(seed_cfg, 2)
+    cams = sphere_cameras(seed_cfg, n_views, W, H, fov)
+    frames = [(cams[v], float(np.float32((v + 0.5) / n_views))) for v in range(n_views)]
+    sweep, iw, iwith, gid, atlas = [], [], [], [], []
+    for _ in range(n_views):
+        n_pairs = sc.C * 4 * n_ctx
+        ctx = sample_levels(rng, n_pairs, sc.C)
+        wo, wi = ctx.copy(), ctx.copy()
+        g = np.empty(n_pairs, np.int32)
+        k = 0
+        for c in range(sc.C):
+            for l in range(4):
+                wo[k:k + n_ctx, c] = l - 1
+                wi[k:k + n_ctx, c] = l
+                g[k:k + n_ctx] = 4 * c + l
+                k += n_ctx
+        sweep.append(np.concatenate([wo, wi], axis=0))
+        iw.append(np.arange(n_pairs, dtype=np.int32))
+        iwith.append(np.arange(n_pairs, 2 * n_pairs, dtype=np.int32))
+        gid.append(g)
+        prefixes = np.stack([np.full(sc.C, d, np.int8) for d in range(-1, 4)])
+        atlas.append(np.concatenate([sample_levels(rng, n_atlas, sc.C), prefixes], axis=0))
+    return AtlasWorkload(f"atlas_{W}x{H}_B{n_atlas + 5}", sc, frames, sweep, iw, iwith, gid, 4 * sc.C, atlas,
+                         group_raw_bytes(sc), tuple(budget_fracs))
