@@ -350,19 +350,174 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+# ------------------------------------------------------------------------------------------------ atlas workload
+def run_atlas(args):
+    """--workload atlas.  A step = one view of the partial-state atlas:
+    utility sweep (2 x 4C x n_ctx states, fused distortion) -> Eq. (3)-(4) -> three policy orders -> frontier
+    states at 4 matched budgets -> 8197 sampled states + 12 frontier states rendered (fused distortion, no
+    images: 8209 x 800 x 800 x 12 B would be 63 GB) -> state bytes -> best sampled state per budget."""
+    import torch
+    from paper_2606_17212_b200 import build as gbuild
+    gbuild.build()
+    from paper_2606_17212_b200 import gsr
+
+    assert int(os.environ.get("WORLD_SIZE", "1")) == 1, "the atlas workload is a 1-GPU bench line"
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    n_views = max(1, min(args.steps + args.warmup, 4))
+    wl = synth.workload_atlas(n_views=n_views)
+    scene = gsr.Scene(wl.scene)
+    Cn, G = wl.scene.C, wl.G
+    cam0, _ = wl.frames[0]
+    W, H = cam0.W, cam0.H
+    cams = [gsr.camera_struct(c) for c, _ in wl.frames]
+    ts = [float(t) for _, t in wl.frames]
+    nb, n_pol = len(wl.budget_fracs), 3
+    Bs, Ba = wl.sweep_levels[0].shape[0], wl.atlas_levels[0].shape[0]
+    Bt = Ba + n_pol * nb
+    to_dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    sweep = [to_dev(l) for l in wl.sweep_levels]
+    iwo, iw, gid = [to_dev(a) for a in wl.idx_without], [to_dev(a) for a in wl.idx_with], [to_dev(a) for a in wl.group_id]
+    batch = [torch.cat([to_dev(l), torch.zeros((n_pol * nb, Cn), dtype=torch.int8, device=dev)]) for l in wl.atlas_levels]
+    raw = to_dev(wl.raw_bytes)
+    wire = gsr.group_wire_bytes(raw)
+    total_wire = int(wire.sum().item())
+    budgets = to_dev(np.asarray([int(f * total_wire) for f in wl.budget_fracs], np.int64))
+    ws = scene.new_workspace(cam0, Bt)
+    ref = torch.empty((H, W, 3), dtype=torch.float32, device=dev)
+    mse_s, psnr_s = torch.empty(Bs, dtype=torch.float64, device=dev), torch.empty(Bs, dtype=torch.float32, device=dev)
+    mse_a, psnr_a = torch.empty(Bt, dtype=torch.float64, device=dev), torch.empty(Bt, dtype=torch.float32, device=dev)
+    util = torch.zeros((G, 9), dtype=torch.float64, device=dev)
+    cost = torch.empty(Bt, dtype=torch.int64, device=dev)
+    best = torch.empty(nb, dtype=torch.int32, device=dev)
+    n_frames = len(wl.frames)
+
+    def step(k):
+        f = k % n_frames
+        scene.render_states_vs_full(cams[f], ts[f], sweep[f], ws, ref, mse_s, psnr_s, out=None)
+        gsr.group_utility_into(mse_s, psnr_s, iwo[f], iw[f], gid[f], G, util)
+        score = util[:, 7].contiguous()                      # risk-adjusted utility in dB (Eq. 4)
+        for p in range(n_pol):
+            order, _ = gsr.frontier_order(score, wire, p)
+            gsr.frontier_states(order, wire, budgets, levels_out=batch[f][Ba + p * nb: Ba + (p + 1) * nb])
+        scene.render_states_vs_full(cams[f], ts[f], batch[f], ws, ref, mse_a, psnr_a, out=None)
+        gsr.state_bytes(batch[f], wire, out=cost)
+        gsr.best_state_under_budget(psnr_a[:Ba], cost[:Ba], budgets, out=best)
+
+    def timed(fn, k0, K):
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for k in range(k0, k0 + K):
+            fn(k)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1)
+
+    for k in range(args.warmup):
+        step(k)
+    scene.status(ws)
+    gsr.set_option("profile", 1)
+    l0 = gsr.launch_count()
+    sampler = ClockSampler(0)
+    sampler.start()
+    sampler.mark()
+    ms = timed(step, args.warmup, args.steps)
+    clocks = sampler.stop()
+    launches = gsr.launch_count() - l0
+    comp_ms, comp_n = gsr.profile_read()
+    gsr.set_option("profile", 0)
+    scene.status(ws)
+    states_per_step = Bs + Bt
+    value = states_per_step * args.steps / (ms * 1e-3)
+
+    # end to end: pinned host levels in, every result of the step back on the host
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    h_sweep, h_atlas = [pin(l) for l in wl.sweep_levels], [pin(l) for l in wl.atlas_levels]
+    h_out = {"psnr": torch.empty(Bt, dtype=torch.float32).pin_memory(), "cost": torch.empty(Bt, dtype=torch.int64).pin_memory(),
+             "best": torch.empty(nb, dtype=torch.int32).pin_memory(), "util": torch.empty((G, 9), dtype=torch.float64).pin_memory()}
+
+    def step_e2e(k):
+        f = k % n_frames
+        sweep[f].copy_(h_sweep[f], non_blocking=True)
+        batch[f][:Ba].copy_(h_atlas[f], non_blocking=True)
+        step(k)
+        h_out["psnr"].copy_(psnr_a, non_blocking=True)
+        h_out["cost"].copy_(cost, non_blocking=True)
+        h_out["best"].copy_(best, non_blocking=True)
+        h_out["util"].copy_(util, non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+
+    step_e2e(0)
+    ms_e2e = timed(step_e2e, args.warmup, args.steps)
+    e2e = {"value": states_per_step * args.steps / (ms_e2e * 1e-3), "unit": "states/s",
+           "h2d_bytes_per_step": int((Bs + Ba) * Cn), "d2h_bytes_per_step": int(Bt * 12 + nb * 4 + G * 72),
+           "ms_per_step": ms_e2e / args.steps}
+
+    # roofline of the dominant kernel, counted work of the two render calls of one step
+    cnt = np.zeros(3, np.float64)
+    f = args.warmup % n_frames
+    scene.render_states_vs_full(cams[f], ts[f], sweep[f], ws, ref, mse_s, psnr_s, out=None)
+    cnt += scene.debug_pair_counts(ws)
+    scene.render_states_vs_full(cams[f], ts[f], batch[f], ws, ref, mse_a, psnr_a, out=None)
+    cnt += scene.debug_pair_counts(ws)
+    comp_s = comp_ms * 1e-3 / args.steps
+    peak = gsr.measure_fp32_peak()
+    achieved = (cnt[0] * FLOP_SHARED + cnt[1] * FLOP_STATE) / comp_s / 1e12
+    roofline = {"kernel": "k_composite", "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                "frac": achieved / peak, "traffic": None,
+                "peak_kind": "measured here: FFMA-chain kernel (gsr_measure_fp32_peak); nominal %.1f" % NOMINAL_FP32_TFLOPS,
+                "kernel_ms_per_launch": comp_ms / max(comp_n, 1), "kernel_launches": comp_n,
+                "kernel_share_of_step": comp_ms / ms, "alpha_evals_per_step": cnt[0], "state_updates_per_step": cnt[1],
+                "logical_pairs_per_step": cnt[2], "literal_equiv_tflops": cnt[2] * FLOP_LITERAL / comp_s / 1e12}
+
+    psnr_h, best_h = psnr_a.cpu().numpy(), best.cpu().numpy()
+    result = {"budget_fracs": list(wl.budget_fracs),
+              "sampled_oracle_psnr_db": [float(psnr_h[i]) if i >= 0 else None for i in best_h],
+              "utility_order_psnr_db": [float(v) for v in psnr_h[Ba:Ba + nb]],
+              "nominal_order_psnr_db": [float(v) for v in psnr_h[Ba + nb:Ba + 2 * nb]],
+              "byte_greedy_psnr_db": [float(v) for v in psnr_h[Ba + 2 * nb:Ba + 3 * nb]]}
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import oracle as O
+        osc = O.OracleScene(wl.scene)
+        n_s = min(args.ref_states, Ba)
+        cam, t = wl.frames[f]
+        t0 = time.perf_counter()
+        imgs, _ = osc.render_batch(cam, t, np.concatenate([wl.atlas_levels[f][:n_s], np.full((1, Cn), 3, np.int8)]))
+        O.distortion(imgs[:-1], imgs[-1])
+        dt = time.perf_counter() - t0
+        cpu = {"value": n_s / dt, "unit": "states/s", "cores": O.num_threads(), "kind": "oracle",
+               "sample": f"first {n_s} of {Ba} atlas states of view {f} (+ full-state reference and MSE/PSNR), {dt:.1f} s"}
+    line = {"metric": "counterfactual_state_renders_per_s", "value": value, "unit": "states/s",
+            "mpix_states_per_s": value * W * H / 1e6, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": wl.name, "states_per_step": states_per_step, "sweep_states": Bs, "atlas_states": Ba,
+                       "frontier_states": n_pol * nb, "resolution": [W, H], "gaussians": wl.scene.N, "clusters": Cn,
+                       "images_materialised": False,
+                       "l2": "each step projects, sorts and composites a different view; no output is re-read"},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+            "atlas": result}
+    print(json.dumps(line))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=60)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg1", choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"])
+    ap.add_argument("--workload", default="cfg1", choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4", "atlas"])
     ap.add_argument("--ref-states", type=int, default=64, help="states per frame the CPU oracle renders")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--state-block", type=int, default=0, help="states per compositing CTA (0 = library default)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.workload == "atlas":
+        run_atlas(args)
     else:
         run_ours(args)
 
