@@ -203,6 +203,40 @@ int gsr_best_state_under_budget(const float* psnr_db, const int64_t* state_bytes
                                 const int64_t* budgets, int32_t nb, int32_t* best, void* cuda_stream);
 
 /* ------------------------------------------------------------------------------------------------
+ * Richer distortion and risk reductions (Eq. (2) and the text below it; DESIGN.md §12,
+ * readings G1-G4).  All pointers dev; asynchronous on `cuda_stream`; deterministic (fixed reduction trees).
+ *
+ * gsr_distortion_ssim: "D = MSE + 0.20(1 - SSIM)".  SSIM per state against `ref`: per
+ *   channel, 11x11 Gaussian window (sigma 1.5, normalised, separable), zero padding, C1 = 0.01^2,
+ *   C2 = 0.03^2, mean of the SSIM map over H x W x 3 (reading G1); fp32 pixels, double moments and sums.
+ *   imgs fp32 [B,H,W,3]; ref fp32 [H,W,3]; ssim double [B] (or NULL); mse double [B] (or NULL: e.g. from
+ *   gsr_distortion / the fused path); d_mix double [B] (or NULL; needs mse) = mse + 0.20 (1 - ssim).
+ *   workspace >= gsr_distortion_workspace_bytes(B,H,W).
+ * gsr_flicker: temporal-change error ("F penalizes temporal-change error"; reading G3):
+ *   out[b] = mean(((imgs_t2[b] - imgs_t1[b]) - (ref_t2 - ref_t1))^2), fp32 differences, double sum.
+ *   imgs_t1, imgs_t2 fp32 [B,H,W,3] (the same states at two times); ref_t1, ref_t2 fp32 [H,W,3];
+ *   out double [B]; workspace >= gsr_distortion_workspace_bytes(B,H,W).
+ * gsr_risk_reduce: mean, CVaR_alpha, alpha-quantile and worst value of n per-state values (PAPER.md:68
+ *   "CVaR_0.05(D)", "p10 PSNR"; reading G2): k = max(1, ceil(alpha n)); cvar = mean of the k
+ *   worst values (upper_tail != 0: the largest, for a distortion; 0: the smallest, for a PSNR); quantile =
+ *   linear interpolation at position (1 - alpha)(n-1) resp. alpha (n-1) of the ascending order.
+ *   values: double [n] (dtype 0) or float [n] (dtype 1); out: gsr_risk [1].
+ * gsr_prefix_monotonicity: "M penalizes quality regressions as a prefix grows" (reading G4):
+ *   M = sum_p max(0, d[idx_next[p]] - d[idx_prev[p]]), violations = #{p : d[next] > d[prev]}.
+ *   d double [.]; idx_prev, idx_next int32 [n_pairs]; m_out double [1]; violations int32 [1] (either may be NULL). */
+typedef struct {
+  double mean, cvar, quantile, worst, count;
+} gsr_risk;
+int gsr_distortion_ssim(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, const double* mse,
+                        double* ssim, double* d_mix, void* workspace, size_t ws_bytes, void* cuda_stream);
+int gsr_flicker(const float* imgs_t1, const float* imgs_t2, const float* ref_t1, const float* ref_t2, int32_t B,
+                int32_t H, int32_t W, double* out, void* workspace, size_t ws_bytes, void* cuda_stream);
+int gsr_risk_reduce(const void* values, int32_t dtype, int32_t n, double alpha, int32_t upper_tail, gsr_risk* out,
+                    void* cuda_stream);
+int gsr_prefix_monotonicity(const double* d, const int32_t* idx_prev, const int32_t* idx_next, int32_t n_pairs,
+                            double* m_out, int32_t* violations, void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------------------
  * One-call convenience with HOST buffers (used for the end-to-end measurement): uploads `levels`
  * and the pair lists, renders the full state (all depths 3) as the reference, renders the batch with
  * fused distortion, aggregates utilities, and copies mse / psnr_db / util back.  Synchronous.

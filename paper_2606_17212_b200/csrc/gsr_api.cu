@@ -510,6 +510,60 @@ int gsr_best_state_under_budget(const float* psnr_db, const int64_t* state_bytes
 }
 
 // ------------------------------------------------------------------------------------------------
+// richer distortion / risk reductions
+int gsr_distortion_ssim(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, const double* mse,
+                        double* ssim, double* d_mix, void* workspace, size_t ws_bytes, void* cuda_stream) {
+  if (B < 0 || H <= 0 || W <= 0 || (B > 0 && (!imgs || !ref || (!ssim && !d_mix))) || (d_mix && !mse) || !workspace) {
+    set_error("gsr_distortion_ssim: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  if (ws_bytes < gsr_distortion_workspace_bytes(B, H, W)) {
+    set_error("gsr_distortion_ssim: workspace too small");
+    return GSR_E_WORKSPACE_TOO_SMALL;
+  }
+  launch_ssim(imgs, ref, B, H, W, mse, (double*)workspace, ssim, d_mix, (cudaStream_t)cuda_stream);
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
+int gsr_flicker(const float* imgs_t1, const float* imgs_t2, const float* ref_t1, const float* ref_t2, int32_t B,
+                int32_t H, int32_t W, double* out, void* workspace, size_t ws_bytes, void* cuda_stream) {
+  if (B < 0 || H <= 0 || W <= 0 || (B > 0 && (!imgs_t1 || !imgs_t2 || !ref_t1 || !ref_t2 || !out)) || !workspace) {
+    set_error("gsr_flicker: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  if (ws_bytes < gsr_distortion_workspace_bytes(B, H, W)) {
+    set_error("gsr_flicker: workspace too small");
+    return GSR_E_WORKSPACE_TOO_SMALL;
+  }
+  launch_flicker(imgs_t1, imgs_t2, ref_t1, ref_t2, B, H, W, (double*)workspace, out, (cudaStream_t)cuda_stream);
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
+int gsr_risk_reduce(const void* values, int32_t dtype, int32_t n, double alpha, int32_t upper_tail, gsr_risk* out,
+                    void* cuda_stream) {
+  if (n < 0 || (n > 0 && !values) || !out || (dtype != 0 && dtype != 1) || !(alpha > 0.0) || alpha > 1.0) {
+    set_error("gsr_risk_reduce: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  launch_risk_reduce(values, dtype, n, alpha, upper_tail != 0, out, (cudaStream_t)cuda_stream);
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
+int gsr_prefix_monotonicity(const double* d, const int32_t* idx_prev, const int32_t* idx_next, int32_t n_pairs,
+                            double* m_out, int32_t* violations, void* cuda_stream) {
+  if (n_pairs < 0 || (n_pairs > 0 && (!d || !idx_prev || !idx_next)) || (!m_out && !violations)) {
+    set_error("gsr_prefix_monotonicity: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  launch_prefix_monotonicity(d, idx_prev, idx_next, n_pairs, m_out, violations, (cudaStream_t)cuda_stream);
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
 // host-buffer convenience call (end-to-end measurement)
 struct FrameCarve {
   size_t o_render, o_levels, o_full, o_ref, o_mse, o_psnr, o_pairs, o_util, o_out, o_refmse, total;

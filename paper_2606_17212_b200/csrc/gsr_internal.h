@@ -122,6 +122,16 @@ void launch_state_bytes(const int8_t* levels, int32_t B, int32_t C, const long l
 void launch_best_under_budget(const float* psnr, const long long* bytes, int32_t B, const long long* budgets,
                               int32_t nb, int32_t* best, cudaStream_t st);
 
+// richer distortion / risk reductions (k_metrics.cu)
+void launch_ssim(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, const double* mse, double* part,
+                 double* ssim, double* dmix, cudaStream_t st);
+void launch_flicker(const float* a1, const float* a2, const float* r1, const float* r2, int32_t B, int32_t H, int32_t W,
+                    double* part, double* out, cudaStream_t st);
+void launch_risk_reduce(const void* values, int32_t is_f32, int32_t n, double alpha, int32_t upper, gsr_risk* out,
+                        cudaStream_t st);
+void launch_prefix_monotonicity(const double* d, const int32_t* prev, const int32_t* next, int32_t n_pairs, double* m_out,
+                                int32_t* viol, cudaStream_t st);
+
 void set_error(const char* fmt, ...);
 
 }  // namespace gsr

@@ -1,0 +1,286 @@
+// k_metrics.cu — richer distortion and risk reductions:
+//   SSIM and D = MSE + 0.20 (1 - SSIM)        PAPER.md:72   (reading G1)
+//   mean / CVaR / quantile / worst over states PAPER.md:68-76 (reading G2)
+//   temporal flicker F                          PAPER.md:70   (reading G3)
+//   prefix monotonicity M                       PAPER.md:70   (reading G4)
+// SSIM and flicker read materialised images ([B,H,W,3] fp32) and are reduced with the canonical tree of
+// reduce.cuh (warp butterfly in double, warps in index order, tiles in index order), so they are
+// deterministic.  The reductions over states are single-CTA, latency-bound helpers.
+#include "gsr_internal.h"
+#include "reduce.cuh"
+
+namespace gsr {
+
+constexpr int kSsimR = 5;                      // window radius (11 x 11)
+constexpr int kSsimHalo = kTile + 2 * kSsimR;  // 26
+constexpr double kSsimC1 = 0.01 * 0.01, kSsimC2 = 0.03 * 0.03;
+
+struct SsimWindow { double g[2 * kSsimR + 1]; };  // normalised weights, evaluated on the host
+
+// One CTA = one 16x16 tile of one state.  Per channel: stage the 26x26 halo of img and ref (zero outside
+// the image: reading G1's zero padding), blur the five moments x, y, xx, yy, xy horizontally into 26 rows x
+// 16 columns, then vertically at the thread's pixel.  The moments are accumulated in DOUBLE: the variance
+// terms E[x^2] - mu^2 cancel against C2 = 9e-4, and fp32 moments leave a systematic 4e-5 error on flat
+// regions (measured); B200's FP64 pipe makes this a ~10 % cost on a kernel that is not on the hot path.
+__global__ void __launch_bounds__(kTilePix) k_ssim_tiles(const float* __restrict__ imgs, const float* __restrict__ ref,
+                                                         int W, int H, int TX, int tiles, SsimWindow win,
+                                                         double* __restrict__ part) {
+  __shared__ float s_x[kSsimHalo][kSsimHalo + 1], s_y[kSsimHalo][kSsimHalo + 1];
+  __shared__ double s_h[5][kSsimHalo][kTile + 1];
+  __shared__ double s_red[8];
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  const int tile = blockIdx.x, b = blockIdx.y;
+  const int x0 = (tile % TX) * kTile, y0 = (tile / TX) * kTile;
+  const int lx = tid & 15, ly = tid >> 4;
+  const int px = x0 + lx, py = y0 + ly;
+  const bool inside = px < W && py < H;
+  const float* img = imgs + (size_t)b * H * W * 3;
+  double acc = 0.0;
+  for (int ch = 0; ch < 3; ++ch) {
+    for (int i = tid; i < kSsimHalo * kSsimHalo; i += kTilePix) {
+      const int hy = i / kSsimHalo, hx = i - hy * kSsimHalo;
+      const int gx = x0 + hx - kSsimR, gy = y0 + hy - kSsimR;
+      float vx = 0.0f, vy = 0.0f;
+      if (gx >= 0 && gx < W && gy >= 0 && gy < H) {
+        const size_t p = ((size_t)gy * W + gx) * 3 + ch;
+        vx = img[p];
+        vy = __ldg(ref + p);
+      }
+      s_x[hy][hx] = vx;
+      s_y[hy][hx] = vy;
+    }
+    __syncthreads();
+    for (int i = tid; i < kSsimHalo * kTile; i += kTilePix) {
+      const int hy = i >> 4, cx = i & 15;
+      double m0 = 0., m1 = 0., m2 = 0., m3 = 0., m4 = 0.;
+#pragma unroll
+      for (int k = 0; k <= 2 * kSsimR; ++k) {
+        const double a = (double)s_x[hy][cx + k], c = (double)s_y[hy][cx + k], g = win.g[k];
+        m0 = fma(g, a, m0);
+        m1 = fma(g, c, m1);
+        m2 = fma(g, a * a, m2);
+        m3 = fma(g, c * c, m3);
+        m4 = fma(g, a * c, m4);
+      }
+      s_h[0][hy][cx] = m0; s_h[1][hy][cx] = m1; s_h[2][hy][cx] = m2; s_h[3][hy][cx] = m3; s_h[4][hy][cx] = m4;
+    }
+    __syncthreads();
+    double mx = 0., my = 0., xx = 0., yy = 0., xy = 0.;
+#pragma unroll
+    for (int k = 0; k <= 2 * kSsimR; ++k) {
+      const double g = win.g[k];
+      mx = fma(g, s_h[0][ly + k][lx], mx);
+      my = fma(g, s_h[1][ly + k][lx], my);
+      xx = fma(g, s_h[2][ly + k][lx], xx);
+      yy = fma(g, s_h[3][ly + k][lx], yy);
+      xy = fma(g, s_h[4][ly + k][lx], xy);
+    }
+    const double sxx = xx - mx * mx, syy = yy - my * my, sxy = xy - mx * my;
+    const double num = (2.0 * mx * my + kSsimC1) * (2.0 * sxy + kSsimC2);
+    const double den = (mx * mx + my * my + kSsimC1) * (sxx + syy + kSsimC2);
+    if (inside) acc += num / den;
+    __syncthreads();
+  }
+  const double ws = warp_sum_butterfly(acc);
+  if (lane == 0) s_red[w] = ws;
+  __syncthreads();
+  if (tid == 0) {
+    double t = s_red[0];
+#pragma unroll
+    for (int k = 1; k < 8; ++k) t += s_red[k];
+    part[(size_t)b * tiles + tile] = t;
+  }
+}
+
+// one warp per state: tiles in index order (lane-strided), then the butterfly; SSIM and the mixed distortion
+__global__ void __launch_bounds__(128) k_ssim_finalize(const double* __restrict__ part, int B, int tiles, double inv_n,
+                                                       const double* __restrict__ mse, double* __restrict__ ssim,
+                                                       double* __restrict__ dmix) {
+  const int b = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (b >= B) return;
+  double acc = 0.0;
+  for (int k = lane; k < tiles; k += 32) acc += part[(size_t)b * tiles + k];
+  acc = warp_sum_butterfly(acc);
+  if (lane == 0) {
+    const double s = acc * inv_n;
+    if (ssim) ssim[b] = s;
+    if (dmix && mse) dmix[b] = mse[b] + 0.20 * (1.0 - s);
+  }
+}
+
+// ---- flicker (reading G3): same pixel->thread mapping and tree as gsr_distortion
+__global__ void __launch_bounds__(kTilePix) k_flicker_tiles(const float* __restrict__ a1, const float* __restrict__ a2,
+                                                            const float* __restrict__ r1, const float* __restrict__ r2,
+                                                            int W, int H, int TX, int tiles, double* __restrict__ part) {
+  __shared__ double s_red[8];
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  const int tile = blockIdx.x, b = blockIdx.y;
+  const int x = (tile % TX) * kTile + 8 * (w & 1) + (lane & 7), y = (tile / TX) * kTile + 4 * (w >> 1) + (lane >> 3);
+  float e = 0.0f;
+  if (x < W && y < H) {
+    const size_t p = ((size_t)y * W + x) * 3;
+    const size_t o = (size_t)b * H * W * 3 + p;
+    float d[3];
+#pragma unroll
+    for (int ch = 0; ch < 3; ++ch)
+      d[ch] = __fsub_rn(__fsub_rn(a2[o + ch], a1[o + ch]), __fsub_rn(__ldg(r2 + p + ch), __ldg(r1 + p + ch)));
+    e = __fmaf_rn(d[2], d[2], __fmaf_rn(d[1], d[1], __fmul_rn(d[0], d[0])));
+  }
+  const double ws = warp_sum_butterfly((double)e);
+  if (lane == 0) s_red[w] = ws;
+  __syncthreads();
+  if (tid == 0) {
+    double acc = s_red[0];
+#pragma unroll
+    for (int k = 1; k < 8; ++k) acc += s_red[k];
+    part[(size_t)b * tiles + tile] = acc;
+  }
+}
+
+// ---- reductions over states (reading G2): one CTA, any n; order statistics by exact MSB-first radix select
+constexpr int kRiskThreads = 256;
+
+__device__ __forceinline__ unsigned long long risk_key(double v) {
+  unsigned long long u = (unsigned long long)__double_as_longlong(v);
+  return (u & 0x8000000000000000ull) ? ~u : (u | 0x8000000000000000ull);
+}
+__device__ __forceinline__ double risk_unkey(unsigned long long k) {
+  unsigned long long u = (k & 0x8000000000000000ull) ? (k & 0x7FFFFFFFFFFFFFFFull) : ~k;
+  return __longlong_as_double((long long)u);
+}
+__device__ __forceinline__ double risk_load(const void* v, int is_f32, int i) {
+  return is_f32 ? (double)((const float*)v)[i] : ((const double*)v)[i];
+}
+
+template <typename T>
+__device__ __forceinline__ T risk_block_sum(T v, T* sm) {
+  sm[threadIdx.x] = v;
+  __syncthreads();
+  for (int k = kRiskThreads / 2; k > 0; k >>= 1) {
+    if (threadIdx.x < k) sm[threadIdx.x] += sm[threadIdx.x + k];
+    __syncthreads();
+  }
+  T r = sm[0];
+  __syncthreads();
+  return r;
+}
+
+// k-th smallest (0-based) value
+__device__ double risk_select(const void* v, int is_f32, int n, int k, unsigned long long* sm) {
+  unsigned long long ans = 0ull;
+  for (int bit = 63; bit >= 0; --bit) {
+    const unsigned long long cand = ans | (1ull << bit);
+    unsigned long long c = 0;
+    for (int i = threadIdx.x; i < n; i += kRiskThreads) c += risk_key(risk_load(v, is_f32, i)) < cand;
+    c = risk_block_sum<unsigned long long>(c, sm);
+    if (c <= (unsigned long long)k) ans = cand;  // at most k keys below cand => the k-th key is >= cand
+  }
+  return risk_unkey(ans);
+}
+
+__global__ void __launch_bounds__(kRiskThreads) k_risk_reduce(const void* __restrict__ v, int is_f32, int n, double alpha,
+                                                              int upper, gsr_risk* __restrict__ out) {
+  __shared__ double sm_d[kRiskThreads];
+  __shared__ unsigned long long sm_c[kRiskThreads];
+  gsr_risk r;
+  r.mean = r.cvar = r.quantile = r.worst = 0.0;
+  r.count = (double)n;
+  if (n > 0) {
+    double s = 0.0;
+    for (int i = threadIdx.x; i < n; i += kRiskThreads) s += risk_load(v, is_f32, i);
+    r.mean = risk_block_sum<double>(s, sm_d) / (double)n;
+    int k = (int)ceil(alpha * (double)n);
+    k = k < 1 ? 1 : (k > n ? n : k);
+    // threshold = the mildest of the k worst values; the tail sum takes everything strictly worse plus the
+    // right number of copies of the threshold (ties)
+    const double thr = risk_select(v, is_f32, n, upper ? n - k : k - 1, sm_c);
+    double ts = 0.0;
+    unsigned long long tc = 0;
+    for (int i = threadIdx.x; i < n; i += kRiskThreads) {
+      const double x = risk_load(v, is_f32, i);
+      if (upper ? x > thr : x < thr) { ts += x; ++tc; }
+    }
+    ts = risk_block_sum<double>(ts, sm_d);
+    tc = risk_block_sum<unsigned long long>(tc, sm_c);
+    r.cvar = (ts + (double)(k - (int)tc) * thr) / (double)k;
+    const double pos = (upper ? 1.0 - alpha : alpha) * (double)(n - 1);
+    const int lo = (int)floor(pos);
+    const int hi = lo + 1 < n ? lo + 1 : n - 1;
+    const double vlo = risk_select(v, is_f32, n, lo, sm_c);
+    const double vhi = hi == lo ? vlo : risk_select(v, is_f32, n, hi, sm_c);
+    r.quantile = vlo + (pos - (double)lo) * (vhi - vlo);
+    r.worst = risk_select(v, is_f32, n, upper ? n - 1 : 0, sm_c);
+  }
+  if (threadIdx.x == 0) *out = r;
+}
+
+// ---- prefix monotonicity (reading G4)
+__global__ void __launch_bounds__(kRiskThreads) k_prefix_monotonicity(const double* __restrict__ d,
+                                                                      const int* __restrict__ prev,
+                                                                      const int* __restrict__ next, int n_pairs,
+                                                                      double* __restrict__ m_out, int* __restrict__ viol) {
+  __shared__ double sm_d[kRiskThreads];
+  __shared__ unsigned long long sm_c[kRiskThreads];
+  double s = 0.0;
+  unsigned long long c = 0;
+  for (int p = threadIdx.x; p < n_pairs; p += kRiskThreads) {
+    const double inc = d[next[p]] - d[prev[p]];
+    if (inc > 0.0) { s += inc; ++c; }
+  }
+  s = risk_block_sum<double>(s, sm_d);
+  c = risk_block_sum<unsigned long long>(c, sm_c);
+  if (threadIdx.x == 0) {
+    if (m_out) *m_out = s;
+    if (viol) *viol = (int)c;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ launchers
+void launch_ssim(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, const double* mse, double* part,
+                 double* ssim, double* dmix, cudaStream_t st) {
+  if (B == 0) return;
+  const int TX = (W + kTile - 1) / kTile, TY = (H + kTile - 1) / kTile, tiles = TX * TY;
+  SsimWindow win;
+  double g[2 * kSsimR + 1], sum = 0.0;
+  for (int k = 0; k <= 2 * kSsimR; ++k) {  // exp(-(k-5)^2 / (2 * 1.5^2)), normalised
+    g[k] = exp(-(double)((k - kSsimR) * (k - kSsimR)) / (2.0 * 1.5 * 1.5));
+    sum += g[k];
+  }
+  for (int k = 0; k <= 2 * kSsimR; ++k) win.g[k] = g[k] / sum;
+  for (int b0 = 0; b0 < B; b0 += 65535) {  // gridDim.y limit
+    const int nb = B - b0 < 65535 ? B - b0 : 65535;
+    k_ssim_tiles<<<dim3(tiles, nb), kTilePix, 0, st>>>(imgs + (size_t)b0 * H * W * 3, ref, W, H, TX, tiles, win,
+                                                      part + (size_t)b0 * tiles);
+    count_launches(1);
+  }
+  k_ssim_finalize<<<(B + 3) / 4, 128, 0, st>>>(part, B, tiles, 1.0 / (3.0 * (double)W * (double)H), mse, ssim, dmix);
+  count_launches(1);
+}
+
+void launch_flicker(const float* a1, const float* a2, const float* r1, const float* r2, int32_t B, int32_t H, int32_t W,
+                    double* part, double* out, cudaStream_t st) {
+  if (B == 0) return;
+  const int TX = (W + kTile - 1) / kTile, TY = (H + kTile - 1) / kTile, tiles = TX * TY;
+  for (int b0 = 0; b0 < B; b0 += 65535) {
+    const int nb = B - b0 < 65535 ? B - b0 : 65535;
+    const size_t off = (size_t)b0 * H * W * 3;
+    k_flicker_tiles<<<dim3(tiles, nb), kTilePix, 0, st>>>(a1 + off, a2 + off, r1, r2, W, H, TX, tiles,
+                                                         part + (size_t)b0 * tiles);
+    count_launches(1);
+  }
+  launch_distortion_finalize(part, B, tiles, (int64_t)3 * W * H, out, nullptr, st);
+}
+
+void launch_risk_reduce(const void* values, int32_t is_f32, int32_t n, double alpha, int32_t upper, gsr_risk* out,
+                        cudaStream_t st) {
+  k_risk_reduce<<<1, kRiskThreads, 0, st>>>(values, is_f32, n, alpha, upper, out);
+  count_launches(1);
+}
+
+void launch_prefix_monotonicity(const double* d, const int32_t* prev, const int32_t* next, int32_t n_pairs, double* m_out,
+                                int32_t* viol, cudaStream_t st) {
+  k_prefix_monotonicity<<<1, kRiskThreads, 0, st>>>(d, prev, next, n_pairs, m_out, viol);
+  count_launches(1);
+}
+
+}  // namespace gsr

@@ -88,6 +88,10 @@ def lib():
         L.gsr_frontier_states.argtypes = [vp, vp, i32, vp, i32, vp, vp, vp, vp]
         L.gsr_state_bytes.argtypes = [vp, i32, i32, vp, vp, vp]
         L.gsr_best_state_under_budget.argtypes = [vp, vp, i32, vp, i32, vp, vp]
+        L.gsr_distortion_ssim.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp, vp, sz, vp]
+        L.gsr_flicker.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp, sz, vp]
+        L.gsr_risk_reduce.argtypes = [vp, i32, i32, C.c_double, i32, vp, vp]
+        L.gsr_prefix_monotonicity.argtypes = [vp, vp, vp, i32, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -398,3 +402,62 @@ def best_state_under_budget(psnr, bytes_per_state, budgets, out=None):
     _check(lib().gsr_best_state_under_budget(_dp(psnr), _dp(bytes_per_state), psnr.numel(), _dp(budgets),
                                              budgets.numel(), _dp(out), _stream()))
     return out
+
+
+# ---- richer distortion / risk reductions (include/gsr.h): marshalling only
+RISK_DTYPE = np.dtype([(n, np.float64) for n in ("mean", "cvar", "quantile", "worst", "count")])
+
+
+def _tile_workspace(B, H, W, workspace):
+    torch = _torch()
+    need = lib().gsr_distortion_workspace_bytes(B, H, W)
+    if workspace is None or workspace.numel() < need:
+        workspace = torch.empty(need, dtype=torch.uint8, device="cuda")
+    return workspace
+
+
+def distortion_ssim(imgs, ref, mse=None, workspace=None):
+    """gsr_distortion_ssim -> (ssim f64 [B], d_mix f64 [B] or None) on device."""
+    torch = _torch()
+    B, H, W = int(imgs.shape[0]), int(imgs.shape[1]), int(imgs.shape[2])
+    assert imgs.dtype == torch.float32 and imgs.is_contiguous() and ref.is_contiguous()
+    workspace = _tile_workspace(B, H, W, workspace)
+    ssim = torch.empty(B, dtype=torch.float64, device="cuda")
+    dmix = torch.empty(B, dtype=torch.float64, device="cuda") if mse is not None else None
+    _check(lib().gsr_distortion_ssim(_dp(imgs), _dp(ref), B, H, W, _dp(mse), _dp(ssim), _dp(dmix), _dp(workspace),
+                                     workspace.numel(), _stream()))
+    return ssim, dmix
+
+
+def flicker(imgs_t1, imgs_t2, ref_t1, ref_t2, workspace=None):
+    """gsr_flicker -> f64 [B] on device."""
+    torch = _torch()
+    B, H, W = int(imgs_t1.shape[0]), int(imgs_t1.shape[1]), int(imgs_t1.shape[2])
+    for t in (imgs_t1, imgs_t2, ref_t1, ref_t2):
+        assert t.dtype == torch.float32 and t.is_cuda and t.is_contiguous()
+    workspace = _tile_workspace(B, H, W, workspace)
+    out = torch.empty(B, dtype=torch.float64, device="cuda")
+    _check(lib().gsr_flicker(_dp(imgs_t1), _dp(imgs_t2), _dp(ref_t1), _dp(ref_t2), B, H, W, _dp(out), _dp(workspace),
+                             workspace.numel(), _stream()))
+    return out
+
+
+def risk_reduce(values, alpha: float, upper_tail: bool):
+    """gsr_risk_reduce on a cuda float64 / float32 vector -> structured numpy record (synchronises)."""
+    torch = _torch()
+    assert values.is_cuda and values.is_contiguous() and values.dtype in (torch.float64, torch.float32)
+    out = torch.zeros(5, dtype=torch.float64, device="cuda")
+    _check(lib().gsr_risk_reduce(_dp(values), 1 if values.dtype == torch.float32 else 0, values.numel(),
+                                 C.c_double(alpha), int(bool(upper_tail)), _dp(out), _stream()))
+    return out.cpu().numpy().view(RISK_DTYPE)[0]
+
+
+def prefix_monotonicity(d, idx_prev, idx_next):
+    """gsr_prefix_monotonicity -> (M, violations) (synchronises)."""
+    torch = _torch()
+    assert d.dtype == torch.float64 and idx_prev.dtype == torch.int32 and idx_next.dtype == torch.int32
+    m = torch.zeros(1, dtype=torch.float64, device="cuda")
+    v = torch.zeros(1, dtype=torch.int32, device="cuda")
+    _check(lib().gsr_prefix_monotonicity(_dp(d), _dp(idx_prev), _dp(idx_next), idx_prev.numel(), _dp(m), _dp(v),
+                                         _stream()))
+    return float(m.item()), int(v.item())
