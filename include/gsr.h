@@ -237,6 +237,33 @@ int gsr_prefix_monotonicity(const double* d, const int32_t* idx_prev, const int3
                             double* m_out, int32_t* violations, void* cuda_stream);
 
 /* ------------------------------------------------------------------------------------------------
+ * gsr_sample_delivery — the step before the hot path: "A training world samples capacity, RTT, display
+ * deadline, IID erasure, and a Gilbert-Elliott burst process.  Packet dependencies are enforced after
+ * delivery, then converted to cluster-layer masks".  DESIGN.md §13, readings H1-H6:
+ *   - group g = 4c + l is cut into ceil(raw_bytes[g] / 1200) packets (an empty group is always usable);
+ *   - the packets of a world are sent group by group in `order` (e.g. a gsr_frontier_order result);
+ *     packet_budget[w] (or NULL = no limit) packets are sent before the display deadline, the rest never arrive;
+ *   - a sent packet is lost if the IID process drops it (p_iid) OR the Gilbert-Elliott channel does: state of
+ *     packet 0 = Bad with the stationary probability p_gb/(p_gb+p_bg) (0 if both are 0), then P(G->B) = p_gb,
+ *     P(B->G) = p_bg; drop probability e_good in Good, e_bad in Bad;
+ *   - a group is usable iff all its packets arrived; mask[w,c] bit l; levels[w,c] = dependency closure.
+ * Randomness: Philox4x32-10, key = seed, counter = (packet index, world0 + w, 0, 0); words x0..x3 drive the
+ * IID drop, the GE transition, the GE drop and (packet 0) the initial state; an event of probability p happens
+ * iff x < floor(p * 2^32).  The result for a world depends only on (seed, world0 + w): sampling a batch in
+ * pieces gives the same masks.  Bit-exact against the oracle.
+ *   raw_bytes dev int64 [4C]; order dev int32 [4C] (a permutation); model: host; packet_budget dev int32 [W] or
+ *   NULL; mask dev uint8 [W,C]; levels dev int8 [W,C] or NULL (feeds gsr_render_states directly);
+ *   workspace dev >= gsr_delivery_workspace_bytes(C).  Asynchronous. */
+typedef struct {
+  double p_iid, p_gb, p_bg, e_good, e_bad;
+  uint64_t seed;
+} gsr_loss_model;
+size_t gsr_delivery_workspace_bytes(int32_t C);
+int gsr_sample_delivery(const int64_t* raw_bytes, const int32_t* order, int32_t C, const gsr_loss_model* model,
+                        const int32_t* packet_budget, int32_t W, int32_t world0, uint8_t* mask, int8_t* levels,
+                        void* workspace, size_t ws_bytes, void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------------------
  * One-call convenience with HOST buffers (used for the end-to-end measurement): uploads `levels`
  * and the pair lists, renders the full state (all depths 3) as the reference, renders the batch with
  * fused distortion, aggregates utilities, and copies mse / psnr_db / util back.  Synchronous.

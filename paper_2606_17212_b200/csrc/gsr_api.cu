@@ -564,6 +564,28 @@ int gsr_prefix_monotonicity(const double* d, const int32_t* idx_prev, const int3
 }
 
 // ------------------------------------------------------------------------------------------------
+// delivery-mask sampler
+size_t gsr_delivery_workspace_bytes(int32_t C) { return C > 0 ? align_up(delivery_workspace_bytes(C)) : 0; }
+
+int gsr_sample_delivery(const int64_t* raw_bytes, const int32_t* order, int32_t C, const gsr_loss_model* model,
+                        const int32_t* packet_budget, int32_t W, int32_t world0, uint8_t* mask, int8_t* levels,
+                        void* workspace, size_t ws_bytes, void* cuda_stream) {
+  if (C <= 0 || C > kMaxC || W < 0 || world0 < 0 || !raw_bytes || !order || !model || !workspace ||
+      (W > 0 && !mask)) {
+    set_error("gsr_sample_delivery: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  const double ps[5] = {model->p_iid, model->p_gb, model->p_bg, model->e_good, model->e_bad};
+  for (double p : ps)
+    if (!(p >= 0.0 && p <= 1.0)) { set_error("gsr_sample_delivery: probabilities must be in [0, 1]"); return GSR_E_INVALID_ARG; }
+  if (ws_bytes < delivery_workspace_bytes(C)) { set_error("gsr_sample_delivery: workspace too small"); return GSR_E_WORKSPACE_TOO_SMALL; }
+  launch_sample_delivery((const long long*)raw_bytes, order, C, *model, packet_budget, W, world0, mask, levels,
+                         (long long*)workspace, (cudaStream_t)cuda_stream);
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
 // host-buffer convenience call (end-to-end measurement)
 struct FrameCarve {
   size_t o_render, o_levels, o_full, o_ref, o_mse, o_psnr, o_pairs, o_util, o_out, o_refmse, total;

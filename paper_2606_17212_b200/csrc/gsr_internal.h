@@ -132,6 +132,12 @@ void launch_risk_reduce(const void* values, int32_t is_f32, int32_t n, double al
 void launch_prefix_monotonicity(const double* d, const int32_t* prev, const int32_t* next, int32_t n_pairs, double* m_out,
                                 int32_t* viol, cudaStream_t st);
 
+// delivery-mask sampler (k_delivery.cu)
+size_t delivery_workspace_bytes(int32_t C);
+void launch_sample_delivery(const long long* raw, const int32_t* order, int32_t C, const gsr_loss_model& m,
+                            const int32_t* budget, int32_t W, int32_t world0, uint8_t* mask, int8_t* levels,
+                            long long* pk_start, cudaStream_t st);
+
 void set_error(const char* fmt, ...);
 
 }  // namespace gsr

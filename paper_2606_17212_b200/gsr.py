@@ -36,6 +36,11 @@ class CameraC(C.Structure):
                 ("cx", C.c_float), ("cy", C.c_float), ("W", C.c_int32), ("H", C.c_int32), ("znear", C.c_float)]
 
 
+class LossModel(C.Structure):
+    _fields_ = [("p_iid", C.c_double), ("p_gb", C.c_double), ("p_bg", C.c_double), ("e_good", C.c_double),
+                ("e_bad", C.c_double), ("seed", C.c_uint64)]
+
+
 UTILITY_DTYPE = np.dtype([(n, np.float64) for n in
                           ("mean_mse", "q10_mse", "std_mse", "risk_mse", "mean_db", "q10_db", "std_db", "risk_db",
                            "count")])
@@ -92,6 +97,9 @@ def lib():
         L.gsr_flicker.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp, sz, vp]
         L.gsr_risk_reduce.argtypes = [vp, i32, i32, C.c_double, i32, vp, vp]
         L.gsr_prefix_monotonicity.argtypes = [vp, vp, vp, i32, vp, vp, vp]
+        L.gsr_delivery_workspace_bytes.argtypes = [i32]
+        L.gsr_delivery_workspace_bytes.restype = sz
+        L.gsr_sample_delivery.argtypes = [vp, vp, i32, C.POINTER(LossModel), vp, i32, i32, vp, vp, vp, sz, vp]
         _lib = L
     return _lib
 
@@ -461,3 +469,22 @@ def prefix_monotonicity(d, idx_prev, idx_next):
     _check(lib().gsr_prefix_monotonicity(_dp(d), _dp(idx_prev), _dp(idx_next), idx_prev.numel(), _dp(m), _dp(v),
                                          _stream()))
     return float(m.item()), int(v.item())
+
+
+# ---- delivery-mask sampler (include/gsr.h): marshalling only
+def sample_delivery(raw_bytes, order, model: dict, W: int, packet_budget=None, world0: int = 0, want_levels=True):
+    """gsr_sample_delivery -> (mask uint8 [W, C], levels int8 [W, C] or None) on device.
+    model: dict(p_iid, p_gb, p_bg, e_good, e_bad, seed)."""
+    torch = _torch()
+    Cn = raw_bytes.numel() // 4
+    assert raw_bytes.dtype == torch.int64 and order.dtype == torch.int32 and raw_bytes.is_cuda and order.is_cuda
+    if packet_budget is not None:
+        assert packet_budget.dtype == torch.int32 and packet_budget.is_cuda and packet_budget.numel() == W
+    m = LossModel(float(model["p_iid"]), float(model["p_gb"]), float(model["p_bg"]), float(model["e_good"]),
+                  float(model["e_bad"]), int(model["seed"]))
+    mask = torch.empty((W, Cn), dtype=torch.uint8, device="cuda")
+    levels = torch.empty((W, Cn), dtype=torch.int8, device="cuda") if want_levels else None
+    ws = torch.empty(lib().gsr_delivery_workspace_bytes(Cn), dtype=torch.uint8, device="cuda")
+    _check(lib().gsr_sample_delivery(_dp(raw_bytes), _dp(order), Cn, C.byref(m), _dp(packet_budget), int(W),
+                                     int(world0), _dp(mask), _dp(levels), _dp(ws), ws.numel(), _stream()))
+    return mask, levels
