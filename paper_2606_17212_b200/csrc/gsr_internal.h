@@ -77,7 +77,7 @@ struct Workspace {
 };
 
 constexpr int kSortThreads = 256;
-constexpr int kSortItems = 16;
+constexpr int kSortItems = 4;
 constexpr int kSortTileKeys = kSortThreads * kSortItems;  // keys per block per pass
 
 size_t carve_workspace(Workspace* ws, void* base, int32_t N, int32_t C, int32_t B, int32_t tiles, long long cap);
