@@ -10,7 +10,7 @@
  *   O-0 activation at load ........ DESIGN.md §3.0      (exp / sigmoid / quaternion -> Sigma; double -> fp32 once)
  *   O-1 dependency closure ........ PAPER.md:64,164,185 ("usable only when all chunks in its
  *                                   dependency closure are usable"), BASELINE.json configs[0]
- *   O-2 deformation ............... PAPER.md:46-50, Eq. (1): mu = A_{c,t} mu_bar + sum_r b_{t,r} q_{i,r}
+ *   O-2 deformation ............... PAPER.md:46-50, Eq. (1): mu = A_{c,t} mu_bar + sum_r b_{t,r} q_{i,r} + delta^(2) + delta^(3)
  *   O-3 EWA projection ............ PAPER.md:140 delegates to a splatting library and prints nothing;
  *                                   the definition is the standard EWA one fixed by BASELINE.json
  *                                   north_star (2) and DESIGN.md §3.3 (every constant is a listed reading)
@@ -61,6 +61,8 @@ typedef struct {
   const float* A0;          /* [C,3,4] */
   const float* A1;          /* [C,3,4] */
   const float* motion_scale; /* [C]    */
+  const float* delta2;      /* [N,3] level-2 position residual delta^(2) of Eq. (1), or NULL (= 0) */
+  const float* delta3;      /* [N,3] level-3 position residual delta^(3) of Eq. (1), or NULL (= 0) */
   float background[3];
 } orc_scene;
 
@@ -207,6 +209,10 @@ static void project_one(const orc_scene* s, const orc_camera* cam, float t, cons
         acc = fmaf(basis[r], (float)s->motion_q[((int64_t)i * s->R + r) * 3 + k], acc);
       p = fmaf(s->motion_scale[c], acc, p);
     }
+    /* Eq. (1) "+ delta^(2) + delta^(3)" (reading I1): the level-l position
+     * residual is applied iff the cluster's depth is >= l, added in this order in binary32 */
+    if (d >= 2 && s->delta2) p = p + s->delta2[3 * (int64_t)i + k];
+    if (d >= 3 && s->delta3) p = p + s->delta3[3 * (int64_t)i + k];
     mu[k] = p;
     o->mu[k] = p;
   }

@@ -36,7 +36,8 @@ class _Scene(C.Structure):
                 ("group_off", C.c_void_p), ("mean", C.c_void_p), ("cov3d", C.c_void_p),
                 ("opacity", C.c_void_p), ("tau", C.c_void_p), ("sh_base", C.c_void_p),
                 ("sh_res", C.c_void_p), ("motion_q", C.c_void_p), ("A0", C.c_void_p), ("A1", C.c_void_p),
-                ("motion_scale", C.c_void_p), ("background", C.c_float * 3)]
+                ("motion_scale", C.c_void_p), ("delta2", C.c_void_p), ("delta3", C.c_void_p),
+                ("background", C.c_float * 3)]
 
 
 class _Camera(C.Structure):
@@ -131,6 +132,11 @@ class OracleScene:
         for name in ("group_off", "mean", "cov3d", "opacity", "tau", "sh_base", "sh_res", "motion_q", "A0",
                      "A1", "motion_scale"):
             setattr(s, name, getattr(self, name).ctypes.data)
+        # optional level-2 / level-3 position residuals of Eq. (1) (None = zero)
+        self.delta2 = _c(sc.delta2, np.float32) if getattr(sc, "delta2", None) is not None else None
+        self.delta3 = _c(sc.delta3, np.float32) if getattr(sc, "delta3", None) is not None else None
+        s.delta2 = self.delta2.ctypes.data if self.delta2 is not None else None
+        s.delta3 = self.delta3.ctypes.data if self.delta3 is not None else None
         s.background[:] = [float(v) for v in np.asarray(sc.background, np.float32)]
         self._s = s
 

@@ -45,6 +45,8 @@ class Scene:
     A1: np.ndarray             # f32 [C,3,4]
     motion_scale: np.ndarray   # f32 [C]
     background: np.ndarray     # f32 [3]
+    delta2: np.ndarray | None = None   # f32 [N,3] level-2 position residual of Eq. (1) (None = zero)
+    delta3: np.ndarray | None = None   # f32 [N,3] level-3 position residual of Eq. (1) (None = zero)
 
     @property
     def K(self) -> int:
@@ -453,3 +455,13 @@ def workload_atlas(n_views: int = 2, n_ctx: int = 8, n_atlas: int = 8192, scene:
         atlas.append(np.concatenate([sample_levels(rng, n_atlas, sc.C), prefixes], axis=0))
     return AtlasWorkload(f"atlas_{W}x{H}_B{n_atlas + 5}", sc, frames, sweep, iw, iwith, gid, 4 * sc.C, atlas,
                          group_raw_bytes(sc), tuple(budget_fracs))
+
+
+def with_position_residuals(sc: Scene, seed_cfg: int = 6, sigma2: float = 0.006, sigma3: float = 0.003) -> Scene:
+    """The same scene with level-2 / level-3 position residuals delta^(2), delta^(3) of Eq. (1):
+    N(0, sigma^2) per coordinate, finer at level 3 (input recipe; no config of BASELINE.json defines them)."""
+    import dataclasses
+    rng = _rng(seed_cfg, 7)
+    d2 = rng.normal(0.0, sigma2, (sc.N, 3)).astype(np.float32)
+    d3 = rng.normal(0.0, sigma3, (sc.N, 3)).astype(np.float32)
+    return dataclasses.replace(sc, delta2=d2, delta3=d3)

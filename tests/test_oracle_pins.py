@@ -534,3 +534,42 @@ def test_p8_multi_term_basis_residual(oracle_mod):
     exp = means[order].astype(np.float32).astype(np.float64) + 0.003 * np.einsum("r,nrk->nk", b, q[order].astype(np.float64))
     assert np.abs(p["mu"] - exp).max() < 1e-6
     assert np.abs(exp - means[order]).max() > 0.05          # the residual is not negligible
+
+
+# ------------------------------------------------------------------------------------------ P18: Eq. (1) residual levels
+def test_p18_position_residual_levels(oracle_mod):
+    """Eq. (1): mu = A mu_bar + sum_r b_r q_r + delta^(2) + delta^(3); reading I1: the level-l
+    residual applies iff the cluster's depth is >= l.  Special cases: no residual arrays == zero arrays ==
+    the old result; depth 0/1 ignore them; depth 2 shifts the deformed mean by exactly delta2 (one fp32 add),
+    depth 3 by delta2 then delta3; an on-axis Gaussian shifted sideways by delta lands f*delta/z pixels away."""
+    import dataclasses
+    wl = synth.workload_cfg0()
+    sc = wl.scene
+    cam, t = wl.frames[0]
+    base = oracle_mod.OracleScene(sc)
+    zero = oracle_mod.OracleScene(dataclasses.replace(sc, delta2=np.zeros((sc.N, 3), np.float32),
+                                                      delta3=np.zeros((sc.N, 3), np.float32)))
+    scd = synth.with_position_residuals(sc)
+    res = oracle_mod.OracleScene(scd)
+    for d in range(-1, 4):
+        depth = np.full(sc.C, d, np.int8)
+        p0, pz, pr = base.project(cam, t, depth), zero.project(cam, t, depth), res.project(cam, t, depth)
+        assert p0.tobytes() == pz.tobytes()
+        if d <= 1:
+            assert p0.tobytes() == pr.tobytes()
+        present = sc.level_of() <= d
+        if d == 2:
+            want = p0["mu"] + scd.delta2
+            assert np.array_equal(pr["mu"][present], want.astype(np.float32)[present])
+        if d == 3:
+            want = (p0["mu"] + scd.delta2).astype(np.float32) + scd.delta3
+            assert np.array_equal(pr["mu"][present], want.astype(np.float32)[present])
+    # closed form: one Gaussian on the optical axis, delta2 = (dx, 0, 0): the 2-D mean moves by f dx / z
+    f, z0, dx = 100.0, 4.0, 0.25
+    one, _ = tiny_scene([[0.0, 0.0, 0.0]], 0.05, levels=[0])
+    one = dataclasses.replace(one, delta2=np.array([[dx, 0.0, 0.0]], np.float32))
+    camx = axis_camera(W=128, H=128, f=f, z0=z0)
+    o = oracle_mod.OracleScene(one)
+    m1 = o.project(camx, 0.0, np.array([1], np.int8))
+    m2 = o.project(camx, 0.0, np.array([2], np.int8))
+    assert m2["mx"][0] - m1["mx"][0] == pytest.approx(f * dx / z0, abs=1e-4) and m2["my"][0] == m1["my"][0]
