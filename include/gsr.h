@@ -67,6 +67,11 @@ typedef struct {
   const float* A1;            /* [C,3,4]                                                       */
   const float* motion_scale;  /* [C]     dequantisation step s_c of the motion residual        */
   float background[3];
+  /* Optional level-2 / level-3 position residuals delta^(2), delta^(3) of Eq. (1) (DESIGN.md
+   * reading I1): [N,3] each, applied iff the cluster's depth is >= 2 / >= 3; NULL = zero.  When both are NULL
+   * a Gaussian has 2 projected records per frame, otherwise 4 (one per delivered depth). */
+  const float* delta2;
+  const float* delta3;
 } gsr_scene_desc;
 
 /* Pinhole camera, OpenCV axes (x right, y down, z forward), pixel centres at +0.5 (reading A9).

@@ -251,6 +251,9 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
   if (!sc) { set_error("gsr_load_scene: out of host memory"); return GSR_E_INVALID_ARG; }
   DeviceScene& D = sc->impl.d;
   D.C = C; D.N = N; D.K = K; D.R = R; D.sh_degree = d->sh_degree; D.n_sh4 = n_sh4; D.n_qw = n_qw;
+  const bool has_delta = d->delta2 || d->delta3;
+  D.V = has_delta ? 4 : 2;
+  D.delta = nullptr;
   for (int k = 0; k < 3; ++k) D.bg[k] = d->background[k];
   size_t off = 0;
   auto reserve = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
@@ -258,7 +261,8 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
                o_g2 = reserve(sizeof(float4) * Np), o_shb = reserve(sizeof(float4) * n_sh4 * Np),
                o_shr = reserve(sizeof(float4) * n_sh4 * Np), o_qw = reserve(sizeof(uint32_t) * n_qw * Np),
                o_A0 = reserve(sizeof(float) * 12 * C), o_A1 = reserve(sizeof(float) * 12 * C),
-               o_ms = reserve(sizeof(float) * C), o_go = reserve(sizeof(int32_t) * (4 * C + 1));
+               o_ms = reserve(sizeof(float) * C), o_go = reserve(sizeof(int32_t) * (4 * C + 1)),
+               o_dl = reserve(has_delta ? sizeof(float) * 6 * Np : 0);
   cudaError_t e = cudaMalloc(&sc->impl.blob, off);
   if (e != cudaSuccess) {
     set_error("gsr_load_scene: cudaMalloc(%zu) failed: %s", off, cudaGetErrorString(e));
@@ -270,6 +274,7 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
   D.sh_base = (float4*)(base + o_shb); D.sh_res = (float4*)(base + o_shr); D.qw = (uint32_t*)(base + o_qw);
   D.A0 = (float*)(base + o_A0); D.A1 = (float*)(base + o_A1); D.mscale = (float*)(base + o_ms);
   D.group_off = (int32_t*)(base + o_go);
+  if (has_delta) D.delta = (float*)(base + o_dl);
   bool ok = true;
   auto up = [&](void* dst, const void* src, size_t bytes) {
     if (bytes && cudaMemcpy(dst, src, bytes, cudaMemcpyHostToDevice) != cudaSuccess) ok = false;
@@ -280,6 +285,15 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
   up(D.qw, qw.data(), sizeof(uint32_t) * n_qw * Np);
   up(D.A0, d->A0, sizeof(float) * 12 * C); up(D.A1, d->A1, sizeof(float) * 12 * C);
   up(D.mscale, d->motion_scale, sizeof(float) * C); up(D.group_off, d->group_off, sizeof(int32_t) * (4 * C + 1));
+  if (has_delta) {  // SoA [6][N]: delta2.xyz, delta3.xyz; a missing array is zero (reading I1)
+    std::vector<float> dl(6 * Np, 0.0f);
+    for (int i = 0; i < N; ++i)
+      for (int k = 0; k < 3; ++k) {
+        if (d->delta2) dl[(size_t)k * Np + i] = d->delta2[3 * (size_t)i + k];
+        if (d->delta3) dl[(size_t)(3 + k) * Np + i] = d->delta3[3 * (size_t)i + k];
+      }
+    up(D.delta, dl.data(), sizeof(float) * 6 * Np);
+  }
   if (!ok) {
     set_error("gsr_load_scene: upload failed: %s", cudaGetErrorString(cudaGetLastError()));
     cudaFree(sc->impl.blob);
@@ -299,9 +313,9 @@ void gsr_free_scene(gsr_scene* scene) {
 size_t gsr_workspace_bytes_ex(const gsr_scene* scene, const gsr_camera* cam, int32_t B, int64_t key_capacity) {
   if (!scene || !camera_ok(cam) || B < 0) return 0;
   const int tiles = ((cam->W + kTile - 1) / kTile) * ((cam->H + kTile - 1) / kTile);
-  const long long cap = key_capacity > 0 ? key_capacity : default_key_capacity(scene->impl.d.N);
+  const long long cap = key_capacity > 0 ? key_capacity : default_key_capacity(rec_half(scene->impl.d));
   if (cap >= (1ll << 31)) return 0;
-  return carve_workspace(nullptr, nullptr, scene->impl.d.N, scene->impl.d.C, B, tiles, cap);
+  return carve_workspace(nullptr, nullptr, rec_half(scene->impl.d), scene->impl.d.C, B, tiles, cap);
 }
 
 size_t gsr_workspace_bytes(const gsr_scene* scene, const gsr_camera* cam, int32_t B) {
@@ -310,7 +324,7 @@ size_t gsr_workspace_bytes(const gsr_scene* scene, const gsr_camera* cam, int32_
 
 // Recovers the key capacity a workspace of ws_bytes can hold (largest cap whose layout fits).
 static long long capacity_for(const gsr_scene* scene, int tiles, int32_t B, size_t ws_bytes) {
-  const int N = scene->impl.d.N, C = scene->impl.d.C;
+  const int N = rec_half(scene->impl.d), C = scene->impl.d.C;
   const long long dflt = default_key_capacity(N);
   if (carve_workspace(nullptr, nullptr, N, C, B, tiles, dflt) <= ws_bytes) {
     // grow while it fits (callers that passed gsr_workspace_bytes_ex with a larger capacity)
@@ -341,13 +355,13 @@ static int prepare_frame(const gsr_scene* scene, const gsr_camera* cam, float t,
   const SceneImpl* s = &scene->impl;
   make_frame(s, cam, t, fp_out);
   const int tiles = fp_out->TX * fp_out->TY;
-  if (carve_workspace(nullptr, nullptr, s->d.N, s->d.C, B, tiles, 1) > ws_bytes) {
+  if (carve_workspace(nullptr, nullptr, rec_half(s->d), s->d.C, B, tiles, 1) > ws_bytes) {
     set_error("gsr_render_states: workspace of %zu bytes is too small", ws_bytes);
     return GSR_E_WORKSPACE_TOO_SMALL;
   }
   const long long cap = capacity_for(scene, tiles, B, ws_bytes);
   if (cap < 1) { set_error("gsr_render_states: workspace too small"); return GSR_E_WORKSPACE_TOO_SMALL; }
-  carve_workspace(ws_out, workspace, s->d.N, s->d.C, B, tiles, cap);
+  carve_workspace(ws_out, workspace, rec_half(s->d), s->d.C, B, tiles, cap);
   launch_init_header(*ws_out, B, s->d.C, s->d.N, *fp_out, cap, st);
   launch_validate_levels(levels, B, s->d.C, *ws_out, st);   // a0
   launch_project(s->d, *fp_out, *ws_out, st);                // a1 + a2
@@ -673,7 +687,7 @@ static int ws_from(const gsr_scene* scene, const void* workspace, Workspace* ws,
   GSR_CUDA(cudaMemcpyAsync(h, workspace, sizeof(*h), cudaMemcpyDeviceToHost, st));
   GSR_CUDA(cudaStreamSynchronize(st));
   if (h->N != scene->impl.d.N || h->C != scene->impl.d.C) { set_error("debug: workspace does not belong to this scene"); return GSR_E_INVALID_ARG; }
-  carve_workspace(ws, const_cast<void*>(workspace), h->N, h->C, h->B, h->TX * h->TY, h->key_capacity);
+  carve_workspace(ws, const_cast<void*>(workspace), rec_half(scene->impl.d), h->C, h->B, h->TX * h->TY, h->key_capacity);
   return GSR_OK;
 }
 
@@ -684,7 +698,7 @@ int gsr_debug_projection(const gsr_scene* scene, const void* workspace, uint8_t*
   Workspace ws; WsHeader h;
   int rc = ws_from(scene, workspace, &ws, &h, st);
   if (rc != GSR_OK) return rc;
-  const size_t n = 2 * (size_t)h.N;
+  const size_t n = (size_t)scene->impl.d.V * (size_t)h.N;
   std::vector<float4> r0(n), r1(n), c0(n), c1(n);
   std::vector<int32_t> rad(n);
   std::vector<uint2> rc4(n);

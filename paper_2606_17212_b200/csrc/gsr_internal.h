@@ -16,6 +16,7 @@ constexpr int kMaxC = 4096;              // clusters (mask table lives in shared
 // ---- device scene: SoA of 16-byte words so that every warp load is 512 B contiguous
 struct DeviceScene {
   int32_t C, N, K, R, sh_degree;
+  int32_t V;      // projected records per Gaussian: 2 (no position residual levels) or 4 (delta2 / delta3 given)
   int32_t n_sh4;  // float4 words of SH coefficients per Gaussian = ceil(3K/4)
   int32_t n_qw;   // 32-bit words of int8 motion coefficients per Gaussian = ceil(3R/4)
   float4* g0;     // [N] mean.xyz, opacity
@@ -27,6 +28,7 @@ struct DeviceScene {
   float* A0;        // [C,12]
   float* A1;        // [C,12]
   float* mscale;    // [C]
+  float* delta;     // [6][N] delta2.xyz, delta3.xyz (V == 4 only), else nullptr
   int32_t* group_off;  // [4C+1]
   float bg[3];
 };
@@ -82,6 +84,8 @@ constexpr int kSortTileKeys = kSortThreads * kSortItems;  // keys per block per 
 
 size_t carve_workspace(Workspace* ws, void* base, int32_t N, int32_t C, int32_t B, int32_t tiles, long long cap);
 long long default_key_capacity(int32_t N);
+// carve_workspace / default_key_capacity take HALF the number of projected records (= N when V == 2)
+inline int32_t rec_half(const DeviceScene& d) { return (int32_t)((long long)d.N * d.V / 2); }
 
 // ---- kernel launchers (each only enqueues on `st`)
 void launch_init_header(Workspace& ws, int32_t B, int32_t C, int32_t N, const FrameParams& fp, long long cap,

@@ -199,8 +199,16 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 4 : 2)) k_composite(const 
       const uint32_t meta = __float_as_uint(g1.w);
       const uint32_t cls = meta >> 16;
       const uint16_t* t = s_tab + 4 * (meta & 0xFFFFu);
-      act = cls == 0 ? t[0] : (cls <= 2 ? t[1] : (cls == 3 ? t[2] : t[3]));
-      res = cls == 0 ? 0u : t[3];
+      if (cls >= 16) {
+        // 4-variant scene (reading I1): variant v = cls - 16 is present exactly at depth v; only v = 3 has the
+        // SH residual colour (stored in both colour slots, so `res` is irrelevant: keep it 0)
+        const uint32_t v = cls - 16;
+        act = v == 0 ? t[0] : (v == 1 ? (t[1] & ~t[2]) : (v == 2 ? (t[2] & ~t[3]) : t[3]));
+        res = 0u;
+      } else {
+        act = cls == 0 ? t[0] : (cls <= 2 ? t[1] : (cls == 3 ? t[2] : t[3]));
+        res = cls == 0 ? 0u : t[3];
+      }
       // pixel-centre box of the record vs the eight 8x4 pixel blocks of the tile
       const float xlo = g0.x - c0.w, xhi = g0.x + c0.w, ylo = g0.y - c1.w, yhi = g0.y + c1.w;
       const float X0 = (float)(tx * kTile) + 0.5f, Y0 = (float)(ty * kTile) + 0.5f;

@@ -28,12 +28,14 @@ constexpr int kDedupThreads = 256;
 __device__ __forceinline__ uint32_t class_sig(uint32_t bits, int d) {
   // bits: 1 = variant-A records (present iff d == 0), 2 = variant-B level 0/1 (d >= 1),
   //       4 = variant-B level 2 (d >= 2), 8 = variant-B level 3 (d >= 3); SH residual iff d == 3 (any B)
+  //       16 << v = records of variant v of a 4-variant scene (present iff d == v)
   uint32_t s = 0;
   if ((bits & 1u) && d == 0) s |= 1u;
   if ((bits & 2u) && d >= 1) s |= 2u;
   if ((bits & 4u) && d >= 2) s |= 4u;
   if ((bits & 8u) && d >= 3) s |= 8u;
-  if (s >= 2u && d == 3) s |= 16u;  // a present B record takes the residual colour
+  if (s >= 2u && d == 3) s |= 256u;  // a present B record takes the residual colour
+  if (d >= 0 && ((bits >> (4 + d)) & 1u)) s |= 16u << d;
   return s;
 }
 
@@ -71,7 +73,7 @@ __global__ void __launch_bounds__(kDedupThreads) k_tile_dedup(const uint2* __res
   for (uint32_t i = rg.x + tid; i < rg.y; i += kDedupThreads) {
     const uint32_t meta = __float_as_uint(r1[vals[i]].w);
     const uint32_t c = meta & 0xFFFFu, cls = meta >> 16;
-    const uint32_t bit = cls == 0 ? 1u : (cls <= 2 ? 2u : (cls == 3 ? 4u : 8u));
+    const uint32_t bit = cls >= 16 ? (16u << (cls - 16)) : (cls == 0 ? 1u : (cls <= 2 ? 2u : (cls == 3 ? 4u : 8u)));
     atomicOr(&cbits[c >> 2], bit << (8 * (c & 3)));
     atomicAdd(&ccnt[c], 1u);
   }

@@ -285,9 +285,102 @@ __global__ void __launch_bounds__(128) k_project(DeviceScene sc, FrameParams fp,
   store_record(ws, 2u * i + 1u, pb, opac, tau, (uint32_t)c | ((uint32_t)(1 + lvl) << 16), cB0, cB1);
 }
 
+// K1 with the position residual levels of Eq. (1) (reading I1): a Gaussian has one geometry per
+// delivered depth d = 0..3 — p (affine only), p + motion residual, + delta2, + delta3 — and variant v is present
+// exactly in the states whose cluster depth is v (v = 3: depth 3, with the SH residual colour).  A level-l
+// Gaussian only has the variants v >= l.  Record id = 4*i + v, record class 16 + v.
+template <int K>
+__global__ void __launch_bounds__(128) k_project4(DeviceScene sc, FrameParams fp, Workspace ws) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= sc.N) return;
+  const float4 g0 = __ldg(sc.g0 + i), g1 = __ldg(sc.g1 + i), g2 = __ldg(sc.g2 + i);
+  const uint32_t bits = __float_as_uint(g2.w);
+  const int c = (int)(bits >> 2), lvl = (int)(bits & 3u);
+  const float S6[6] = {g1.x, g1.y, g1.z, g2.x, g2.y, g2.z};
+  const float opac = g0.w, tau = g1.w;
+  const float* A0 = sc.A0 + 12 * c;
+  const float* A1 = sc.A1 + 12 * c;
+  float A[12];
+#pragma unroll
+  for (int k = 0; k < 12; ++k) A[k] = __fmaf_rn(fp.time, __ldg(A1 + k), __ldg(A0 + k));
+  float mu[4][3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k)
+    mu[0][k] = __fmaf_rn(A[4 * k + 0], g0.x, __fmaf_rn(A[4 * k + 1], g0.y, __fmaf_rn(A[4 * k + 2], g0.z, A[4 * k + 3])));
+  float acc[3] = {0.f, 0.f, 0.f};
+  {
+    uint32_t w = 0;
+    for (int r = 0; r < sc.R; ++r) {
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        int byte = r * 3 + k;
+        if ((byte & 3) == 0) w = __ldg(sc.qw + (size_t)(byte >> 2) * sc.N + i);
+        int q = (int)(int8_t)((w >> ((byte & 3) * 8)) & 0xFFu);
+        acc[k] = __fmaf_rn(fp.basis[r], (float)q, acc[k]);
+      }
+    }
+  }
+  const float s_c = __ldg(sc.mscale + c);
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    mu[1][k] = __fmaf_rn(s_c, acc[k], mu[0][k]);
+    mu[2][k] = __fadd_rn(mu[1][k], __ldg(sc.delta + (size_t)k * sc.N + i));
+    mu[3][k] = __fadd_rn(mu[2][k], __ldg(sc.delta + (size_t)(3 + k) * sc.N + i));
+  }
+  Proj pr[4];
+  bool any = false;
+#pragma unroll
+  for (int v = 0; v < 4; ++v) {
+    pr[v].count = 0;
+    if (v >= lvl) pr[v] = project_variant(fp, mu[v], S6, tau);
+    any |= pr[v].count > 0;
+  }
+  float col[4][3] = {{0.f, 0.f, 0.f}, {0.f, 0.f, 0.f}, {0.f, 0.f, 0.f}, {0.f, 0.f, 0.f}};
+  if (any) {
+    constexpr int n4 = (3 * K + 3) / 4;
+#pragma unroll
+    for (int v = 0; v < 4; ++v) {
+      if (pr[v].count == 0) continue;
+      float Y[K];
+      sh_dir<K>(fp, mu[v], Y);
+      float sb[3] = {0.5f, 0.5f, 0.5f}, sr[3] = {0.f, 0.f, 0.f};
+#pragma unroll
+      for (int w4 = 0; w4 < n4; ++w4) {
+        const float4 cb = __ldg(sc.sh_base + (size_t)w4 * sc.N + i);
+        const float4 cr = __ldg(sc.sh_res + (size_t)w4 * sc.N + i);
+        const float vb[4] = {cb.x, cb.y, cb.z, cb.w}, vr[4] = {cr.x, cr.y, cr.z, cr.w};
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const int flat = w4 * 4 + e;
+          if (flat < 3 * K) {
+            const int j = flat / 3, ch = flat % 3;
+            sb[ch] = fmaf(Y[j], vb[e], sb[ch]);
+            sr[ch] = fmaf(Y[j], vr[e], sr[ch]);
+          }
+        }
+      }
+#pragma unroll
+      for (int ch = 0; ch < 3; ++ch) col[v][ch] = fmaxf(0.f, v == 3 ? sb[ch] + sr[ch] : sb[ch]);
+    }
+  }
+#pragma unroll
+  for (int v = 0; v < 4; ++v)
+    store_record(ws, 4u * i + (uint32_t)v, pr[v], opac, tau, (uint32_t)c | ((uint32_t)(16 + v) << 16), col[v], col[v]);
+}
+
 void launch_project(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, cudaStream_t st) {
   if (sc.N == 0) return;
   dim3 grid((sc.N + 127) / 128), block(128);
+  if (sc.V == 4) {
+    switch (sc.K) {
+      case 1: k_project4<1><<<grid, block, 0, st>>>(sc, fp, ws); break;
+      case 4: k_project4<4><<<grid, block, 0, st>>>(sc, fp, ws); break;
+      case 9: k_project4<9><<<grid, block, 0, st>>>(sc, fp, ws); break;
+      default: k_project4<16><<<grid, block, 0, st>>>(sc, fp, ws); break;
+    }
+    count_launches(1);
+    return;
+  }
   switch (sc.K) {
     case 1: k_project<1><<<grid, block, 0, st>>>(sc, fp, ws); break;
     case 4: k_project<4><<<grid, block, 0, st>>>(sc, fp, ws); break;

@@ -268,7 +268,7 @@ __global__ void __launch_bounds__(256) k_tile_ranges(const unsigned long long* _
 
 void launch_bin_and_sort(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, long long cap,
                          cudaStream_t st) {
-  const int n_rec = 2 * sc.N;
+  const int n_rec = sc.V * sc.N;
   const int tiles = fp.TX * fp.TY;
   cudaMemsetAsync(ws.tile_range, 0, sizeof(uint2) * (size_t)tiles, st);
   if (n_rec == 0) return;
@@ -299,6 +299,7 @@ void launch_bin_and_sort(const DeviceScene& sc, const FrameParams& fp, Workspace
 // presence of record r (class cls of cluster c) in a state whose cluster depth is d:
 //   cls 0 (variant A, level-0 Gaussian): d == 0 ; cls 1+l (variant B, level l): d >= max(1, l)
 __device__ __forceinline__ bool record_present(uint32_t cls, int d) {
+  if (cls >= 16) return d == (int)cls - 16;  // 4-variant scenes (reading I1): variant v lives in depth v only
   return cls == 0 ? (d == 0) : (d >= 1 && d >= (int)cls - 1);
 }
 
@@ -328,7 +329,7 @@ __global__ void __launch_bounds__(256) k_state_counts(int n_rec, const uint32_t*
 
 void launch_state_counts(const DeviceScene& sc, Workspace& ws, int32_t B, cudaStream_t st) {
   if (B == 0) return;
-  k_state_counts<<<B, 256, 0, st>>>(2 * sc.N, ws.count, ws.r1, ws.depth, sc.C, ws.state_counts);
+  k_state_counts<<<B, 256, 0, st>>>(sc.V * sc.N, ws.count, ws.r1, ws.depth, sc.C, ws.state_counts);
   count_launches(1);
 }
 
@@ -338,7 +339,7 @@ __global__ void __launch_bounds__(256) k_filter_keys(const unsigned long long* _
                                                      const uint32_t* __restrict__ vals,
                                                      const WsHeader* __restrict__ hdr,
                                                      const float4* __restrict__ r1,
-                                                     const int8_t* __restrict__ depth, int C, int b,
+                                                     const int8_t* __restrict__ depth, int C, int V, int b,
                                                      uint32_t* __restrict__ tile, uint32_t* __restrict__ dbits,
                                                      int32_t* __restrict__ gi, unsigned long long* n_out,
                                                      long long cap) {
@@ -372,7 +373,7 @@ __global__ void __launch_bounds__(256) k_filter_keys(const unsigned long long* _
     if (keep && (long long)pos < cap) {
       tile[pos] = (uint32_t)(k >> 32);
       dbits[pos] = (uint32_t)k;
-      gi[pos] = (int32_t)(rid >> 1);
+      gi[pos] = (int32_t)(rid / (uint32_t)V);
     }
     __syncthreads();
     if (threadIdx.x == 0) run_s += tot;
@@ -383,7 +384,7 @@ __global__ void __launch_bounds__(256) k_filter_keys(const unsigned long long* _
 
 void launch_filter_keys(const DeviceScene& sc, Workspace& ws, int32_t b, uint32_t* tile, uint32_t* dbits,
                         int32_t* gi, unsigned long long* n_out, long long cap, cudaStream_t st) {
-  k_filter_keys<<<1, 256, 0, st>>>(ws.keys[0], ws.vals[0], ws.hdr, ws.r1, ws.depth, sc.C, b, tile, dbits, gi,
+  k_filter_keys<<<1, 256, 0, st>>>(ws.keys[0], ws.vals[0], ws.hdr, ws.r1, ws.depth, sc.C, sc.V, b, tile, dbits, gi,
                                    n_out, cap);
 }
 

@@ -28,7 +28,7 @@ class SceneDesc(C.Structure):
                 ("group_off", C.c_void_p), ("mean", C.c_void_p), ("log_scale", C.c_void_p), ("quat", C.c_void_p),
                 ("opacity_logit", C.c_void_p), ("sh_base", C.c_void_p), ("sh_res", C.c_void_p),
                 ("motion_q", C.c_void_p), ("A0", C.c_void_p), ("A1", C.c_void_p), ("motion_scale", C.c_void_p),
-                ("background", C.c_float * 3)]
+                ("background", C.c_float * 3), ("delta2", C.c_void_p), ("delta3", C.c_void_p)]
 
 
 class CameraC(C.Structure):
@@ -182,6 +182,13 @@ class Scene:
         for k, v in keep.items():
             setattr(d, k, v.ctypes.data)
         d.background[:] = [float(v) for v in np.asarray(sc.background, np.float32)]
+        self.V = 2                                   # projected records per Gaussian
+        for name in ("delta2", "delta3"):            # optional position residual levels of Eq. (1)
+            a = getattr(sc, name, None)
+            if a is not None:
+                keep[name] = _np(a, np.float32)
+                setattr(d, name, keep[name].ctypes.data)
+                self.V = 4
         h = C.c_void_p()
         _check(lib().gsr_load_scene(C.byref(d), C.byref(h)))
         self.handle = h
@@ -274,7 +281,7 @@ class Scene:
 
     # ---- debug / parity exports
     def debug_projection(self, workspace) -> dict:
-        n = 2 * self.N
+        n = self.V * self.N
         o = dict(valid=np.zeros(n, np.uint8), radius=np.zeros(n, np.int32), rect=np.zeros((n, 4), np.int32),
                  depth_bits=np.zeros(n, np.uint32), count=np.zeros(n, np.int32), mean2d=np.zeros((n, 2), np.float32),
                  conic=np.zeros((n, 3), np.float32), rgb_base=np.zeros((n, 3), np.float32),
