@@ -236,17 +236,27 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 4 : 2)) k_composite(const 
       s_rec[4 * tid + 3] = c1;
     }
     __syncthreads();
-    uint32_t nb = 0;  // length of this warp's list
+    // exclusive offsets of the 8 source warps inside each of the 8 lists: lane l scans list k = l >> 2, source
+    // warps 2 (l & 3) and 2 (l & 3) + 1 (a 4-lane segmented scan), then every lane fetches the offset of ITS
+    // warp in list k from lane 4 k + (w >> 1) — 2 shared loads and 10 shuffles instead of an 8 x 8 table walk
+    uint32_t nb;  // length of this warp's list
+    {
+      const uint32_t lk = (uint32_t)lane >> 2, lq = 2u * ((uint32_t)lane & 3u);
+      const uint32_t v0 = s_lcnt[lk][lq], v1 = s_lcnt[lk][lq + 1];
+      uint32_t incl = v0 + v1;
 #pragma unroll
-    for (int k = 0; k < 8; ++k) {
-      uint32_t off = 0;
-#pragma unroll
-      for (int q = 0; q < 8; ++q) {
-        const uint32_t cnt = s_lcnt[k][q];
-        if (q < w) off += cnt;
-        if (k == w) nb += cnt;
+      for (int o = 1; o < 4; o <<= 1) {
+        const uint32_t up = __shfl_up_sync(0xffffffffu, incl, o, 4);
+        if ((lane & 3) >= o) incl += up;
       }
-      if ((wmask >> k) & 1u) s_list[k][off + __popc(balk[k] & ((1u << lane) - 1u))] = (uint16_t)(rec_base + 64u * tid);
+      const uint32_t off0 = incl - (v0 + v1), off1 = off0 + v0;
+      const uint32_t mine = (w & 1) ? off1 : off0;
+      nb = __shfl_sync(0xffffffffu, incl, 4 * w + 3);
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const uint32_t off = __shfl_sync(0xffffffffu, mine, 4 * k + (w >> 1));
+        if ((wmask >> k) & 1u) s_list[k][off + __popc(balk[k] & ((1u << lane) - 1u))] = (uint16_t)(rec_base + 64u * tid);
+      }
     }
     __syncthreads();
 
