@@ -341,8 +341,10 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 4 : 2)) k_composite(const 
     const float* rp = a.ref + ((size_t)y * a.W + x) * 3;
     rr0 = __ldg(rp); rr1 = __ldg(rp + 1); rr2 = __ldg(rp + 2);
   }
+  double err[S];
 #pragma unroll
   for (int s = 0; s < S; ++s) {
+    err[s] = 0.0;
     const float Tf = fabsf(T[s]);  // the transmittance the pixel ended with (frozen at termination)
     const float o0 = __fmaf_rn(Tf, bg0, Cr[s]);
     const float o1 = __fmaf_rn(Tf, bg1, Cg[s]);
@@ -361,13 +363,12 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 4 : 2)) k_composite(const 
         op[0] = o0; op[1] = o1; op[2] = o2;
       }
     }
-    if (a.ref) {
-      const float e = inside ? pixel_sq_err(o0, o1, o2, rr0, rr1, rr2) : 0.0f;
-      const double ws = warp_sum_butterfly((double)e);
-      if (lane == 0) s_red[w][s] = ws;
-    }
+    if (a.ref) err[s] = inside ? (double)pixel_sq_err(o0, o1, o2, rr0, rr1, rr2) : 0.0;
   }
   if (a.ref) {
+    int slot;
+    const double tot = warp_sum_slots<S>(err, lane, slot);  // same bits as S plain butterflies (reduce.cuh)
+    if ((lane & (32 / S - 1)) == 0) s_red[w][slot] = tot;
     __syncthreads();
     if (tid < S && s_rep[tid] >= 0) {
       double acc = s_red[0][tid];

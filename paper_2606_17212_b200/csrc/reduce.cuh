@@ -21,4 +21,31 @@ __device__ __forceinline__ double warp_sum_butterfly(double v) {
   return v;
 }
 
+// The same butterfly for S values per lane at once (S a power of two <= 32), at a fraction of the shuffles:
+// at the first steps the two lanes of a pair split the slots between them (each sends the half it gives up
+// and adds what it receives to the half it keeps), then the usual butterfly runs on the one slot left.
+// For every slot the additions are the pairings lane ^ 16, ^ 8, ... of warp_sum_butterfly, and a + b == b + a
+// bitwise, so each slot's total has exactly the bits the plain butterfly gives.  On return every lane holds
+// the total of slot `slot`; lanes with (lane & (32 / S - 1)) == 0 are one representative per slot.
+template <int S>
+__device__ __forceinline__ double warp_sum_slots(double (&v)[S], int lane, int& slot) {
+  int off = 16;
+  slot = 0;
+#pragma unroll
+  for (int n = S; n > 1; n >>= 1) {
+    const int half = n >> 1;
+    const bool upper = (lane & off) != 0;
+#pragma unroll
+    for (int j = 0; j < half; ++j) {
+      const double send = upper ? v[j] : v[j + half];
+      const double keep = upper ? v[j + half] : v[j];
+      v[j] = keep + __shfl_xor_sync(0xffffffffu, send, off);
+    }
+    slot = 2 * slot + (upper ? 1 : 0);
+    off >>= 1;
+  }
+  for (; off > 0; off >>= 1) v[0] += __shfl_xor_sync(0xffffffffu, v[0], off);
+  return v[0];
+}
+
 }  // namespace gsr
