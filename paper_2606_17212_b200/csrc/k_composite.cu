@@ -69,30 +69,31 @@ __device__ __forceinline__ float2 lds64f(uint32_t addr) {
   return v;
 }
 
-// One (pixel, state) step of DESIGN.md §3.5:  T' = T (1 - alpha);  if T' >= 1e-4 { C += (alpha T) c; T = T' }
-// else { T = -|T| }.  T < 0 marks a finished pixel (-(frozen transmittance)): then T' <= 0 and it stays
-// finished.  A lane that failed the cut has alpha = 0, for which the step is exactly a no-op.
-// Explicitly rounded (mul.rn / fma.rn, never contracted) and predicated, so that every instantiation of
-// the kernel applies bit-identical arithmetic to a state: batched == serial.
+// One (pixel, state) step of DESIGN.md §3.5:  w = alpha T;  T' = T - w  (= T (1 - alpha));  if T' >= 1e-4
+// { C += w c; T = T' } else { T = -|T| }.  T < 0 marks a finished pixel (-(frozen transmittance)): then T' <= 0
+// and it stays finished.  A lane that failed the cut has alpha = 0, for which the step is exactly a no-op.
+// Explicitly rounded (mul.rn / sub.rn / fma.rn, never contracted) and predicated, so that every instantiation
+// of the kernel applies bit-identical arithmetic to a state: batched == serial.
 // Pipe balance (profiles/r1b): the half-rate ALU pipe (FSETP/FSEL/LOP3) was the binding unit, so the step
 // keeps ONE compare and ONE select (with the -|T| folded into its operand) there; the rest is FMA-pipe work.
-__device__ __forceinline__ void state_update(float& T, float& Cr, float& Cg, float& Cb, float om, float alpha,
-                                             float cr, float cg, float cb) {
+// T' is formed from the w the colour needs anyway: 7 instructions per state and no 1 - alpha register.
+__device__ __forceinline__ void state_update(float& T, float& Cr, float& Cg, float& Cb, float alpha, float cr,
+                                             float cg, float cb) {
   asm("{\n\t"
       ".reg .pred p;\n\t"
       ".reg .f32 tn, wg, tm;\n\t"
-      "mul.rn.f32 tn, %0, %4;\n\t"
+      "mul.rn.f32 wg, %4, %0;\n\t"
+      "sub.rn.f32 tn, %0, wg;\n\t"
       "setp.geu.f32 p, tn, 0f38D1B717;\n\t"  // 1e-4f
-      "mul.rn.f32 wg, %5, %0;\n\t"
-      "@p fma.rn.f32 %1, wg, %6, %1;\n\t"
-      "@p fma.rn.f32 %2, wg, %7, %2;\n\t"
-      "@p fma.rn.f32 %3, wg, %8, %3;\n\t"
+      "@p fma.rn.f32 %1, wg, %5, %1;\n\t"
+      "@p fma.rn.f32 %2, wg, %6, %2;\n\t"
+      "@p fma.rn.f32 %3, wg, %7, %3;\n\t"
       "abs.f32 tm, %0;\n\t"
       "neg.f32 tm, tm;\n\t"
       "selp.f32 %0, tn, tm, p;\n\t"
       "}"
       : "+f"(T), "+f"(Cr), "+f"(Cg), "+f"(Cb)
-      : "f"(om), "f"(alpha), "f"(cr), "f"(cg), "f"(cb));
+      : "f"(alpha), "f"(cr), "f"(cg), "f"(cb));
 }
 
 __device__ __forceinline__ float ex2_approx_ftz(float x) {
@@ -301,19 +302,18 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 4 : 2)) k_composite(const 
         // q <= tau <= ln 255 on every lane that passes: no denormal range to guard, ex2.approx.ftz is enough
         float alpha = fminf(kAlphaCap, __fmul_rn(k0.w, ex2_approx_ftz(__fmul_rn(q, -1.4426950408889634f))));
         alpha = pass ? alpha : 0.0f;
-        const float om = __fsub_rn(1.0f, alpha);
-        // The tag is the same on every lane; the warp reduction only tells the compiler so (it lands in a
+          // The tag is the same on every lane; the warp reduction only tells the compiler so (it lands in a
         // uniform register), which turns every slot test below into a plain skip without reconvergence
         // barriers.  Slots taking the plain colour first, then those taking the colour with the SH residual.
         const uint32_t tagu = __reduce_or_sync(0xffffffffu, tagw);
         const uint32_t act1 = tagu & (tagu >> 16), act0 = (tagu & 0xFFFFu) ^ act1;
 #pragma unroll
         for (int s = 0; s < S; ++s)
-          if ((act0 >> s) & 1u) state_update(T[s], Cr[s], Cg[s], Cb[s], om, alpha, k0.x, k0.y, k0.z);
+          if ((act0 >> s) & 1u) state_update(T[s], Cr[s], Cg[s], Cb[s], alpha, k0.x, k0.y, k0.z);
         if (act1 != 0) {
 #pragma unroll
           for (int s = 0; s < S; ++s)
-            if ((act1 >> s) & 1u) state_update(T[s], Cr[s], Cg[s], Cb[s], om, alpha, k1.x, k1.y, k1.z);
+            if ((act1 >> s) & 1u) state_update(T[s], Cr[s], Cg[s], Cb[s], alpha, k1.x, k1.y, k1.z);
         }
       }
     }
