@@ -257,6 +257,7 @@ def run_ours(args):
     clocks = sampler.stop() if rank == 0 else None
     launches = gsr.launch_count() - l0
     comp_ms, comp_n = gsr.profile_read()
+    proj_ms, sort_ms, ph_n = gsr.profile_read_phases()
     gsr.set_option("profile", 0)
     keys = scene.status(ws)
     value = B * args.steps * world / (ms * 1e-3)
@@ -317,6 +318,34 @@ def run_ours(args):
                 "logical_pairs_per_step": cnt[2] / args.steps,
                 "literal_equiv_tflops": cnt[2] * FLOP_LITERAL / comp_s / 1e12 if comp_s > 0 else 0.0,
                 "image_write_gbs": B * H * W * 12 * args.steps / comp_s / 1e9 if comp_s > 0 else None}
+    # ---- the memory-bound phases a1-a3 against the HBM roofline (algorithmic bytes per unit)
+    K = (wl.scene.sh_degree + 1) ** 2
+    n_rec = scene.V * wl.scene.N
+    b_gauss = 48 + 2 * 16 * ((3 * K + 3) // 4) + 4 * ((3 * wl.scene.R + 3) // 4) + (24 if scene.V == 4 else 0)
+    proj_bytes = wl.scene.N * b_gauss + n_rec * 88
+    tiles = ((W + 15) // 16) * ((H + 15) // 16)
+    tile_bits = max(1, int(np.ceil(np.log2(tiles))))
+    passes = (32 + tile_bits + 7) // 8
+    passes += passes & 1
+    sort_bytes = n_rec * 16 + keys * 12 + passes * keys * 32 + keys * 8
+    hbm_peak, hbm_kind = 6650.0, "fallback (B200_PROFILING.md)"
+    mp = ROOT / "MEASURED_PEAKS.json"
+    if mp.exists():
+        try:
+            hbm_peak, hbm_kind = float(json.loads(mp.read_text())["hbm_gbs"]), "MEASURED_PEAKS.json"
+        except Exception:
+            pass
+    phases = None
+    if ph_n > 0:
+        pg = proj_bytes * ph_n / (proj_ms * 1e-3) / 1e9
+        sg = sort_bytes * ph_n / (sort_ms * 1e-3) / 1e9
+        phases = {"bound": "hbm", "peak": hbm_peak, "peak_kind": hbm_kind, "unit": "GB/s", "frames": ph_n,
+                  "project": {"ms_per_frame": proj_ms / ph_n, "algorithmic_bytes": int(proj_bytes), "achieved": pg,
+                              "frac": pg / hbm_peak},
+                  "bin_sort": {"ms_per_frame": sort_ms / ph_n, "algorithmic_bytes": int(sort_bytes), "achieved": sg,
+                               "frac": sg / hbm_peak, "radix_passes": passes, "launches_per_frame": 5 + 3 * passes,
+                               "note": "latency-bound at this key count (%d keys): many small dependent launches" % keys},
+                  "share_of_step": (proj_ms + sort_ms) / ms}
     tp = Path(ROOT / "profiles" / "traffic.json")
     if tp.exists():
         try:
@@ -342,7 +371,8 @@ def run_ours(args):
                        "l2": "per-step working set (%.2f GB of images written) exceeds the 126 MB L2; every step is a different frame" % (B * H * W * 12 / 1e9),
                        "parallelism": "frames sharded over ranks, no collective" if world > 1 else "1 GPU"},
             "value_without_images": B * args.steps * world / (ms_noimg * 1e-3),
-            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "memory_phases": phases,
+            "cpu_baseline": cpu,
             "context": {"paper_h100_pcie_utility_states_per_s": 1889.7,
                         "note": "PAPER.md:150, other hardware, unstated resolution/scene: context only"}}
     print(json.dumps(line))

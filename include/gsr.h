@@ -329,6 +329,11 @@ int gsr_set_option(const char* name, int32_t value);
  * of launches recorded since "profile" was set or last read.  Synchronises those events. */
 int gsr_profile_read(double* composite_ms, int32_t* composite_launches);
 
+/* Sums of the projection phase (a1 + a2: k_project) and of the binning + sort phase (a3: scans, key emission, radix
+ * passes, tile ranges) over the frames prepared since "profile" was set or last read (CUDA events on the launch
+ * stream), and the number of those frames.  Synchronises those events. */
+int gsr_profile_read_phases(double* project_ms, double* sort_ms, int32_t* frames);
+
 /* Kernels launched by this library since load (the caller's evidence for "gpu_launches"). */
 int64_t gsr_launch_count(void);
 

@@ -37,6 +37,20 @@ int profile_read(double* ms, int* n);
 unsigned long long launches_total();
 int measure_ffma_peak(int num_sms, double* tflops, cudaStream_t st);
 
+// ---- optional CUDA-event timing of the memory-bound phases a1-a3 (gsr_set_option("profile", 1))
+constexpr int kMaxPhaseFrames = 4096;
+static cudaEvent_t g_ph[kMaxPhaseFrames][3];
+static int g_ph_created = 0, g_ph_used = 0;
+static int phase_slot() {
+  if (!g_profile || g_ph_used >= kMaxPhaseFrames) return -1;
+  const int slot = g_ph_used++;
+  while (g_ph_created <= slot) {
+    for (int k = 0; k < 3; ++k) cudaEventCreate(&g_ph[g_ph_created][k]);
+    ++g_ph_created;
+  }
+  return slot;
+}
+
 long long default_key_capacity(int32_t N) { return 12ll * 2ll * (long long)N + (1ll << 20); }
 
 static size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
@@ -136,6 +150,7 @@ int gsr_set_option(const char* name, int value) {
   if (name && strcmp(name, "profile") == 0) {
     g_profile = value != 0;
     profile_reset();
+    g_ph_used = 0;
     return GSR_OK;
   }
   set_error("gsr_set_option: unknown option or value");
@@ -148,6 +163,21 @@ int gsr_profile_read(double* composite_ms, int32_t* composite_launches) {
   if (profile_read(composite_ms, &n) != 0) { set_error("gsr_profile_read: event query failed"); return GSR_E_CUDA; }
   *composite_launches = n;
   profile_reset();
+  return GSR_OK;
+}
+
+int gsr_profile_read_phases(double* project_ms, double* sort_ms, int32_t* frames) {
+  if (!project_ms || !sort_ms || !frames) { set_error("gsr_profile_read_phases: NULL argument"); return GSR_E_INVALID_ARG; }
+  double p = 0, q = 0;
+  for (int k = 0; k < g_ph_used; ++k) {
+    float a = 0, b = 0;
+    GSR_CUDA(cudaEventSynchronize(g_ph[k][2]));
+    GSR_CUDA(cudaEventElapsedTime(&a, g_ph[k][0], g_ph[k][1]));
+    GSR_CUDA(cudaEventElapsedTime(&b, g_ph[k][1], g_ph[k][2]));
+    p += a; q += b;
+  }
+  *project_ms = p; *sort_ms = q; *frames = g_ph_used;
+  g_ph_used = 0;
   return GSR_OK;
 }
 
@@ -364,8 +394,12 @@ static int prepare_frame(const gsr_scene* scene, const gsr_camera* cam, float t,
   carve_workspace(ws_out, workspace, rec_half(s->d), s->d.C, B, tiles, cap);
   launch_init_header(*ws_out, B, s->d.C, s->d.N, *fp_out, cap, st);
   launch_validate_levels(levels, B, s->d.C, *ws_out, st);   // a0
+  const int ph = phase_slot();
+  if (ph >= 0) cudaEventRecord(g_ph[ph][0], st);
   launch_project(s->d, *fp_out, *ws_out, st);                // a1 + a2
+  if (ph >= 0) cudaEventRecord(g_ph[ph][1], st);
   launch_bin_and_sort(s->d, *fp_out, *ws_out, cap, st);      // a3
+  if (ph >= 0) cudaEventRecord(g_ph[ph][2], st);
   return GSR_OK;
 }
 

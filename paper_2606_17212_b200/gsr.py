@@ -87,6 +87,7 @@ def lib():
         L.gsr_debug_pair_counts.argtypes = [vp, vp, vp, vp]
         L.gsr_profile_read.argtypes = [C.POINTER(C.c_double), C.POINTER(i32)]
         L.gsr_launch_count.restype = i64
+        L.gsr_profile_read_phases.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(i32)]
         L.gsr_measure_fp32_peak.argtypes = [C.POINTER(C.c_double), vp]
         L.gsr_group_wire_bytes.argtypes = [vp, i32, vp, vp]
         L.gsr_frontier_order.argtypes = [vp, vp, i32, i32, vp, vp, vp]
@@ -152,6 +153,13 @@ def profile_read():
     ms, n = C.c_double(0), C.c_int32(0)
     _check(lib().gsr_profile_read(C.byref(ms), C.byref(n)))
     return float(ms.value), int(n.value)
+
+
+def profile_read_phases():
+    """gsr_profile_read_phases -> (projection ms, binning + sort ms, frames) since the last read."""
+    a, b, n = C.c_double(0), C.c_double(0), C.c_int32(0)
+    _check(lib().gsr_profile_read_phases(C.byref(a), C.byref(b), C.byref(n)))
+    return float(a.value), float(b.value), int(n.value)
 
 
 def launch_count() -> int:
