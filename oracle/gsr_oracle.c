@@ -63,6 +63,11 @@ typedef struct {
   const float* motion_scale; /* [C]    */
   const float* delta2;      /* [N,3] level-2 position residual delta^(2) of Eq. (1), or NULL (= 0) */
   const float* delta3;      /* [N,3] level-3 position residual delta^(3) of Eq. (1), or NULL (= 0) */
+  /* per-depth activated attributes of scenes with scale / rotation / opacity refinements (PAPER.md:50,
+   * DESIGN.md reading I2), or NULL: [4][N,6], [4][N], [4][N] for delivered depth 0..3 */
+  const float* cov3d_lv;
+  const float* opacity_lv;
+  const float* tau_lv;
   float background[3];
 } orc_scene;
 
@@ -85,6 +90,8 @@ typedef struct {
   uint32_t depth_bits; /* raw bits of z                                */
   int32_t count;       /* tiles touched                                */
   double rgb[3];       /* SH colour (continuous)                       */
+  float opacity, tau;  /* activated opacity and ln(255 opacity) at this state's depth */
+  float pad_[2];
 } orc_proj;
 
 /* ------------------------------------------------------------------------------------------ */
@@ -193,6 +200,8 @@ static void project_one(const orc_scene* s, const orc_camera* cam, float t, cons
   memset(o, 0, sizeof(*o));
   int lvl = level_of(s, c, i);
   if (d < lvl) return; /* O-1: present iff d >= level(i); d = -1 removes the whole cluster */
+  o->opacity = s->opacity_lv ? s->opacity_lv[(int64_t)d * s->N + i] : s->opacity[i];
+  o->tau = s->tau_lv ? s->tau_lv[(int64_t)d * s->N + i] : s->tau[i];
 
   /* ---- O-2 (Eq. 1): A = A0 + t A1 ; p = A [mu_bar;1] ; residual = s_c * sum_r b_r q_r ---- */
   const float* A0 = s->A0 + 12 * c;
@@ -244,7 +253,7 @@ static void project_one(const orc_scene* s, const orc_camera* cam, float t, cons
     M1[k] = fmaf(J12, Rw[6 + k], J11 * Rw[3 + k]);
   }
   /* Sigma' = M Sigma M^T */
-  const float* S6 = s->cov3d + 6 * (int64_t)i;
+  const float* S6 = s->cov3d_lv ? s->cov3d_lv + 6 * ((int64_t)d * s->N + i) : s->cov3d + 6 * (int64_t)i;
   float S[9] = {S6[0], S6[1], S6[2], S6[1], S6[3], S6[4], S6[2], S6[4], S6[5]};
   float v0[3], v1[3];
   for (int a = 0; a < 3; ++a) {
@@ -430,7 +439,7 @@ void orc_render_O1(const orc_scene* s, const orc_camera* cam, const orc_proj* p,
       for (int64_t k = 0; k < n; ++k) {
         const orc_proj* g = &p[ord[k].idx];
         if (tx < g->rect[0] || tx >= g->rect[2] || ty < g->rect[1] || ty >= g->rect[3]) continue;
-        if (pixel_step(g, s->opacity[ord[k].idx], s->tau[ord[k].idx], px, py, t_stop, &T, Cc, &evaluated, NULL))
+        if (pixel_step(g, g->opacity, g->tau, px, py, t_stop, &T, Cc, &evaluated, NULL))
           break;
       }
       double* o = img + 3 * ((int64_t)y * cam->W + x);
@@ -464,7 +473,7 @@ void orc_render_O2(const orc_scene* s, const orc_camera* cam, const orc_proj* p,
       for (int x = x0; x < x1; ++x) {
         int64_t pix = (int64_t)y * cam->W + x;
         if (done[pix]) continue;
-        if (pixel_step(g, s->opacity[gi], s->tau[gi], (float)x + 0.5f, (float)y + 0.5f, t_stop, &T[pix],
+        if (pixel_step(g, g->opacity, g->tau, (float)x + 0.5f, (float)y + 0.5f, t_stop, &T[pix],
                        img + 3 * pix, &evaluated, NULL))
           done[pix] = 1;
       }
@@ -491,7 +500,7 @@ int64_t orc_trace_pixel(const orc_scene* s, const orc_camera* cam, const orc_pro
     const orc_proj* g = &p[ord[k].idx];
     if (tx < g->rect[0] || tx >= g->rect[2] || ty < g->rect[1] || ty >= g->rect[3]) continue;
     double a = 0.0;
-    int stop = pixel_step(g, s->opacity[ord[k].idx], s->tau[ord[k].idx], (float)x + 0.5f, (float)y + 0.5f,
+    int stop = pixel_step(g, g->opacity, g->tau, (float)x + 0.5f, (float)y + 0.5f,
                           t_stop, &T, Cc, &evaluated, &a);
     if (m < cap) { gidx[m] = ord[k].idx; alpha[m] = stop ? -1.0 : a; Tafter[m] = T; }
     ++m;

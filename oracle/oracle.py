@@ -37,6 +37,7 @@ class _Scene(C.Structure):
                 ("opacity", C.c_void_p), ("tau", C.c_void_p), ("sh_base", C.c_void_p),
                 ("sh_res", C.c_void_p), ("motion_q", C.c_void_p), ("A0", C.c_void_p), ("A1", C.c_void_p),
                 ("motion_scale", C.c_void_p), ("delta2", C.c_void_p), ("delta3", C.c_void_p),
+                ("cov3d_lv", C.c_void_p), ("opacity_lv", C.c_void_p), ("tau_lv", C.c_void_p),
                 ("background", C.c_float * 3)]
 
 
@@ -49,7 +50,8 @@ class _Camera(C.Structure):
 PROJ_DTYPE = np.dtype([("valid", np.int32), ("mu", np.float32, 3), ("z", np.float32), ("mx", np.float32),
                        ("my", np.float32), ("qa", np.float32), ("qb", np.float32), ("qc", np.float32),
                        ("cov2d", np.float32, 3), ("radius", np.int32), ("rect", np.int32, 4),
-                       ("depth_bits", np.uint32), ("count", np.int32), ("rgb", np.float64, 3)], align=True)
+                       ("depth_bits", np.uint32), ("count", np.int32), ("rgb", np.float64, 3),
+                       ("opacity", np.float32), ("tau", np.float32), ("pad_", np.float32, 2)], align=True)
 
 _lib = None
 
@@ -137,6 +139,26 @@ class OracleScene:
         self.delta3 = _c(sc.delta3, np.float32) if getattr(sc, "delta3", None) is not None else None
         s.delta2 = self.delta2.ctypes.data if self.delta2 is not None else None
         s.delta3 = self.delta3.ctypes.data if self.delta3 is not None else None
+        # optional per-level refinements of log-scale / quaternion / opacity logit (reading I2):
+        # the attributes at delivered depth v are the base plus the residuals of levels 1..v, summed in level
+        # order in binary32, then activated exactly like the base (O-0)
+        refs = [getattr(sc, n, None) for n in ("d_log_scale", "d_quat", "d_opacity_logit")]
+        s.cov3d_lv = s.opacity_lv = s.tau_lv = None
+        if any(r is not None for r in refs):
+            cur = [ls.copy(), qt.copy(), lg.copy()]
+            self.cov3d_lv = np.empty((4, self.N, 6), np.float32)
+            self.opacity_lv = np.empty((4, self.N), np.float32)
+            self.tau_lv = np.empty((4, self.N), np.float32)
+            for v in range(4):
+                if v >= 1:
+                    for k, r in enumerate(refs):
+                        if r is not None:
+                            cur[k] = (cur[k] + _c(r[v - 1], np.float32).reshape(cur[k].shape)).astype(np.float32)
+                L.orc_activate(C.c_int64(self.N), _p(_c(cur[0], np.float32)), _p(_c(cur[1], np.float32)),
+                               _p(_c(cur[2], np.float32)), _p(self.cov3d_lv[v]), _p(self.opacity_lv[v]),
+                               _p(self.tau_lv[v]))
+            s.cov3d_lv, s.opacity_lv, s.tau_lv = (self.cov3d_lv.ctypes.data, self.opacity_lv.ctypes.data,
+                                                   self.tau_lv.ctypes.data)
         s.background[:] = [float(v) for v in np.asarray(sc.background, np.float32)]
         self._s = s
 

@@ -47,6 +47,10 @@ class Scene:
     background: np.ndarray     # f32 [3]
     delta2: np.ndarray | None = None   # f32 [N,3] level-2 position residual of Eq. (1) (None = zero)
     delta3: np.ndarray | None = None   # f32 [N,3] level-3 position residual of Eq. (1) (None = zero)
+    # per-level refinements (levels 1..3) of log-scale / raw quaternion / opacity logit, or None
+    d_log_scale: np.ndarray | None = None      # f32 [3,N,3]
+    d_quat: np.ndarray | None = None           # f32 [3,N,4]
+    d_opacity_logit: np.ndarray | None = None  # f32 [3,N]
 
     @property
     def K(self) -> int:
@@ -465,3 +469,17 @@ def with_position_residuals(sc: Scene, seed_cfg: int = 6, sigma2: float = 0.006,
     d2 = rng.normal(0.0, sigma2, (sc.N, 3)).astype(np.float32)
     d3 = rng.normal(0.0, sigma3, (sc.N, 3)).astype(np.float32)
     return dataclasses.replace(sc, delta2=d2, delta3=d3)
+
+
+def with_attribute_refinements(sc: Scene, seed_cfg: int = 6, s_scale: float = 0.08, s_quat: float = 0.05,
+                               s_logit: float = 0.3) -> Scene:
+    """The same scene with per-level refinements of scale, rotation and opacity ("Scale, rotation,
+    opacity, and colour use a base plus three learned refinements"): additive residuals on log-scale, raw
+    quaternion and opacity logit, N(0, (s / 2^(l-1))^2) at level l = 1..3 (finer planes at later levels)."""
+    import dataclasses
+    rng = _rng(seed_cfg, 8)
+    f = np.array([1.0, 0.5, 0.25])[:, None, None]
+    dls = (rng.normal(0.0, 1.0, (3, sc.N, 3)) * s_scale * f).astype(np.float32)
+    dq = (rng.normal(0.0, 1.0, (3, sc.N, 4)) * s_quat * f).astype(np.float32)
+    dlg = (rng.normal(0.0, 1.0, (3, sc.N)) * s_logit * f[:, :, 0]).astype(np.float32)
+    return dataclasses.replace(sc, d_log_scale=dls, d_quat=dq, d_opacity_logit=dlg)

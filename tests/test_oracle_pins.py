@@ -573,3 +573,50 @@ def test_p18_position_residual_levels(oracle_mod):
     m1 = o.project(camx, 0.0, np.array([1], np.int8))
     m2 = o.project(camx, 0.0, np.array([2], np.int8))
     assert m2["mx"][0] - m1["mx"][0] == pytest.approx(f * dx / z0, abs=1e-4) and m2["my"][0] == m1["my"][0]
+
+
+# ------------------------------------------------------------------------------------------ P19: attribute refinements
+def test_p19_attribute_refinement_levels(oracle_mod):
+    """"Scale, rotation, opacity, and colour use a base plus three learned refinements"; reading I2:
+    additive residuals on log-scale / raw quaternion / opacity logit, level l applied iff depth >= l.
+    Pins: zero refinements == none; depth 0 ignores them; a single on-axis isotropic Gaussian follows the P3
+    closed form with s_v = s exp(sum dls), o_v = sigmoid(logit + sum dlogit); a quaternion refinement that only
+    rescales the quaternion changes nothing (normalisation)."""
+    import dataclasses
+    wl = synth.workload_cfg0()
+    sc, (cam, t) = wl.scene, wl.frames[0]
+    base = oracle_mod.OracleScene(sc)
+    z3 = lambda *shape: np.zeros((3, sc.N) + shape, np.float32)
+    zero = oracle_mod.OracleScene(dataclasses.replace(sc, d_log_scale=z3(3), d_quat=z3(4), d_opacity_logit=z3()))
+    ref = oracle_mod.OracleScene(synth.with_attribute_refinements(sc))
+    # scaling the quaternion by a positive factor per level: same rotation
+    dq = np.stack([0.25 * sc.quat, 0.5 * sc.quat, 1.0 * sc.quat]).astype(np.float32)
+    qonly = oracle_mod.OracleScene(dataclasses.replace(sc, d_quat=dq))
+    for d in range(-1, 4):
+        depth = np.full(sc.C, d, np.int8)
+        p0, pz, pr, pq = (o.project(cam, t, depth) for o in (base, zero, ref, qonly))
+        assert p0.tobytes() == pz.tobytes()
+        if d <= 0:
+            assert p0.tobytes() == pr.tobytes()
+        else:
+            m = p0["valid"] == 1
+            assert np.any(pr["cov2d"][m] != p0["cov2d"][m]) and np.any(pr["opacity"][m] != p0["opacity"][m])
+        m = (p0["valid"] == 1) & (pq["valid"] == 1)
+        assert np.allclose(pq["cov2d"][m], p0["cov2d"][m], rtol=2e-5, atol=1e-6)
+    # closed form (P3) per depth for one isotropic Gaussian on the axis
+    f, z0, s0, logit = 100.0, 4.0, 0.05, 0.3
+    one, _ = tiny_scene([[0.0, 0.0, 0.0]], s0, logits=logit, colors=[0.8, 0.6, 0.4], levels=[0])
+    dls = np.array([0.2, -0.1, 0.05], np.float32).reshape(3, 1, 1) * np.ones((3, 1, 3), np.float32)
+    dlg = np.array([0.5, -0.25, 1.0], np.float32).reshape(3, 1)
+    one = dataclasses.replace(one, d_log_scale=dls, d_opacity_logit=dlg)
+    camx = axis_camera(W=64, H=64, f=f, z0=z0, cx=32.5, cy=32.5)   # pixel (32, 32) centre on the axis
+    o = oracle_mod.OracleScene(one)
+    for d in range(4):
+        s_v = s0 * np.exp(float(dls[:d, 0, 0].astype(np.float64).sum())) if d else s0
+        o_v = 1.0 / (1.0 + np.exp(-(logit + float(dlg[:d, 0].astype(np.float64).sum()))))
+        img, _ = o.render(camx, 0.0, np.array([d], np.int8))
+        sig2 = (f * s_v / z0) ** 2 + 0.3
+        pr = o.project(camx, 0.0, np.array([d], np.int8))
+        assert pr["cov2d"][0][0] == pytest.approx(sig2, rel=1e-5)
+        alpha = min(0.99, o_v)                                       # at the centre exp(0) = 1
+        assert img[32, 32, 0] == pytest.approx(0.8 * alpha, rel=1e-5)
