@@ -72,6 +72,14 @@ typedef struct {
    * a Gaussian has 2 projected records per frame, otherwise 4 (one per delivered depth). */
   const float* delta2;
   const float* delta3;
+  /* Optional per-level refinements of scale, rotation and opacity ("Scale, rotation, opacity, and colour use a
+   * base plus three learned refinements"; reading I2): additive residuals on log_scale
+   * [3,N,3], quat [3,N,4] and opacity_logit [3,N] for levels 1..3; level l applies iff the cluster's depth is
+   * >= l; the attributes at depth v are the base plus levels 1..v summed in level order in binary32, then
+   * activated like the base.  NULL = zero.  Any of them (like delta2 / delta3) gives 4 records per Gaussian. */
+  const float* d_log_scale;
+  const float* d_quat;
+  const float* d_opacity_logit;
 } gsr_scene_desc;
 
 /* Pinhole camera, OpenCV axes (x right, y down, z forward), pixel centres at +0.5 (reading A9).

@@ -125,6 +125,31 @@ static void make_frame(const SceneImpl* s, const gsr_camera* cam, float t, Frame
   for (int k = 0; k < 3; ++k) fp->bg[k] = s->d.bg[k];
 }
 
+// DESIGN.md §3.0 activation of one Gaussian, double precision, this operation order
+static void activate_one(const float ls[3], const float q[4], float logit, float cov[6], float* opac, float* tau) {
+  double s[3];
+  for (int k = 0; k < 3; ++k) s[k] = exp((double)ls[k]);
+  double qw_ = q[0], qx = q[1], qy = q[2], qz = q[3];
+  const double nrm = sqrt(qw_ * qw_ + qx * qx + qy * qy + qz * qz);
+  qw_ /= nrm; qx /= nrm; qy /= nrm; qz /= nrm;
+  const double Rm[9] = {1.0 - 2.0 * (qy * qy + qz * qz), 2.0 * (qx * qy - qw_ * qz), 2.0 * (qx * qz + qw_ * qy),
+                        2.0 * (qx * qy + qw_ * qz), 1.0 - 2.0 * (qx * qx + qz * qz), 2.0 * (qy * qz - qw_ * qx),
+                        2.0 * (qx * qz - qw_ * qy), 2.0 * (qy * qz + qw_ * qx), 1.0 - 2.0 * (qx * qx + qy * qy)};
+  double M[9];
+  for (int a = 0; a < 3; ++a)
+    for (int k = 0; k < 3; ++k) M[3 * a + k] = Rm[3 * a + k] * s[k];
+  int o = 0;
+  for (int a = 0; a < 3; ++a)
+    for (int b = a; b < 3; ++b) {
+      double acc = M[3 * a + 0] * M[3 * b + 0];
+      acc += M[3 * a + 1] * M[3 * b + 1];
+      acc += M[3 * a + 2] * M[3 * b + 2];
+      cov[o++] = (float)acc;
+    }
+  *opac = (float)(1.0 / (1.0 + exp(-(double)logit)));
+  *tau = (float)log(255.0 * (double)*opac);
+}
+
 }  // namespace gsr
 
 using namespace gsr;
@@ -228,30 +253,8 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
   for (int c = 0; c < C; ++c)
     for (int l = 0; l < 4; ++l)
       for (int i = d->group_off[4 * c + l]; i < d->group_off[4 * c + l + 1]; ++i) {
-        // DESIGN.md §3.0 activation, double precision, this operation order
-        double s[3];
-        for (int k = 0; k < 3; ++k) s[k] = exp((double)d->log_scale[3 * (size_t)i + k]);
-        double qw_ = d->quat[4 * (size_t)i + 0], qx = d->quat[4 * (size_t)i + 1], qy = d->quat[4 * (size_t)i + 2],
-               qz = d->quat[4 * (size_t)i + 3];
-        const double nrm = sqrt(qw_ * qw_ + qx * qx + qy * qy + qz * qz);
-        qw_ /= nrm; qx /= nrm; qy /= nrm; qz /= nrm;
-        const double Rm[9] = {1.0 - 2.0 * (qy * qy + qz * qz), 2.0 * (qx * qy - qw_ * qz), 2.0 * (qx * qz + qw_ * qy),
-                              2.0 * (qx * qy + qw_ * qz), 1.0 - 2.0 * (qx * qx + qz * qz), 2.0 * (qy * qz - qw_ * qx),
-                              2.0 * (qx * qz - qw_ * qy), 2.0 * (qy * qz + qw_ * qx), 1.0 - 2.0 * (qx * qx + qy * qy)};
-        double M[9];
-        for (int a = 0; a < 3; ++a)
-          for (int k = 0; k < 3; ++k) M[3 * a + k] = Rm[3 * a + k] * s[k];
-        float cov[6];
-        int o = 0;
-        for (int a = 0; a < 3; ++a)
-          for (int b = a; b < 3; ++b) {
-            double acc = M[3 * a + 0] * M[3 * b + 0];
-            acc += M[3 * a + 1] * M[3 * b + 1];
-            acc += M[3 * a + 2] * M[3 * b + 2];
-            cov[o++] = (float)acc;
-          }
-        const float opac = (float)(1.0 / (1.0 + exp(-(double)d->opacity_logit[i])));
-        const float tau = (float)log(255.0 * (double)opac);
+        float cov[6], opac, tau;
+        activate_one(d->log_scale + 3 * (size_t)i, d->quat + 4 * (size_t)i, d->opacity_logit[i], cov, &opac, &tau);
         const uint32_t bits = ((uint32_t)c << 2) | (uint32_t)l;
         float bitsf;
         memcpy(&bitsf, &bits, 4);
@@ -281,9 +284,10 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
   if (!sc) { set_error("gsr_load_scene: out of host memory"); return GSR_E_INVALID_ARG; }
   DeviceScene& D = sc->impl.d;
   D.C = C; D.N = N; D.K = K; D.R = R; D.sh_degree = d->sh_degree; D.n_sh4 = n_sh4; D.n_qw = n_qw;
-  const bool has_delta = d->delta2 || d->delta3;
+  const bool has_attr = d->d_log_scale || d->d_quat || d->d_opacity_logit;
+  const bool has_delta = d->delta2 || d->delta3 || has_attr;  // 4 records per Gaussian
   D.V = has_delta ? 4 : 2;
-  D.delta = nullptr;
+  D.delta = nullptr; D.g1v = nullptr; D.g2v = nullptr; D.opv = nullptr;
   for (int k = 0; k < 3; ++k) D.bg[k] = d->background[k];
   size_t off = 0;
   auto reserve = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
@@ -292,7 +296,9 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
                o_shr = reserve(sizeof(float4) * n_sh4 * Np), o_qw = reserve(sizeof(uint32_t) * n_qw * Np),
                o_A0 = reserve(sizeof(float) * 12 * C), o_A1 = reserve(sizeof(float) * 12 * C),
                o_ms = reserve(sizeof(float) * C), o_go = reserve(sizeof(int32_t) * (4 * C + 1)),
-               o_dl = reserve(has_delta ? sizeof(float) * 6 * Np : 0);
+               o_dl = reserve(has_delta ? sizeof(float) * 6 * Np : 0),
+               o_g1v = reserve(has_attr ? sizeof(float4) * 4 * Np : 0), o_g2v = reserve(has_attr ? sizeof(float4) * 4 * Np : 0),
+               o_opv = reserve(has_attr ? sizeof(float) * 4 * Np : 0);
   cudaError_t e = cudaMalloc(&sc->impl.blob, off);
   if (e != cudaSuccess) {
     set_error("gsr_load_scene: cudaMalloc(%zu) failed: %s", off, cudaGetErrorString(e));
@@ -305,6 +311,7 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
   D.A0 = (float*)(base + o_A0); D.A1 = (float*)(base + o_A1); D.mscale = (float*)(base + o_ms);
   D.group_off = (int32_t*)(base + o_go);
   if (has_delta) D.delta = (float*)(base + o_dl);
+  if (has_attr) { D.g1v = (float4*)(base + o_g1v); D.g2v = (float4*)(base + o_g2v); D.opv = (float*)(base + o_opv); }
   bool ok = true;
   auto up = [&](void* dst, const void* src, size_t bytes) {
     if (bytes && cudaMemcpy(dst, src, bytes, cudaMemcpyHostToDevice) != cudaSuccess) ok = false;
@@ -323,6 +330,30 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
         if (d->delta3) dl[(size_t)(3 + k) * Np + i] = d->delta3[3 * (size_t)i + k];
       }
     up(D.delta, dl.data(), sizeof(float) * 6 * Np);
+  }
+  if (has_attr) {  // per-depth attributes: base + levels 1..v in binary32 (level order), then §3.0 (reading I2)
+    std::vector<float4> a1(4 * Np), a2(4 * Np);
+    std::vector<float> ao(4 * Np);
+    for (int i = 0; i < N; ++i) {
+      float ls[3] = {d->log_scale[3 * (size_t)i], d->log_scale[3 * (size_t)i + 1], d->log_scale[3 * (size_t)i + 2]};
+      float q[4] = {d->quat[4 * (size_t)i], d->quat[4 * (size_t)i + 1], d->quat[4 * (size_t)i + 2], d->quat[4 * (size_t)i + 3]};
+      float lg = d->opacity_logit[i];
+      for (int v = 0; v < 4; ++v) {
+        if (v >= 1) {
+          const size_t l = (size_t)(v - 1);
+          if (d->d_log_scale) for (int k = 0; k < 3; ++k) ls[k] = ls[k] + d->d_log_scale[(l * N + i) * 3 + k];
+          if (d->d_quat) for (int k = 0; k < 4; ++k) q[k] = q[k] + d->d_quat[(l * N + i) * 4 + k];
+          if (d->d_opacity_logit) lg = lg + d->d_opacity_logit[l * N + i];
+        }
+        float cov[6], opac, tau;
+        activate_one(ls, q, lg, cov, &opac, &tau);
+        a1[(size_t)v * Np + i] = make_float4(cov[0], cov[1], cov[2], tau);
+        a2[(size_t)v * Np + i] = make_float4(cov[3], cov[4], cov[5], 0.0f);
+        ao[(size_t)v * Np + i] = opac;
+      }
+    }
+    up(D.g1v, a1.data(), sizeof(float4) * 4 * Np); up(D.g2v, a2.data(), sizeof(float4) * 4 * Np);
+    up(D.opv, ao.data(), sizeof(float) * 4 * Np);
   }
   if (!ok) {
     set_error("gsr_load_scene: upload failed: %s", cudaGetErrorString(cudaGetLastError()));

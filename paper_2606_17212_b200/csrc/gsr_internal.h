@@ -29,6 +29,9 @@ struct DeviceScene {
   float* A1;        // [C,12]
   float* mscale;    // [C]
   float* delta;     // [6][N] delta2.xyz, delta3.xyz (V == 4 only), else nullptr
+  float4* g1v;      // [4][N] per-depth (Sxx Sxy Sxz, tau) of scenes with attribute refinements, else nullptr
+  float4* g2v;      // [4][N] per-depth (Syy Syz Szz, -)
+  float* opv;       // [4][N] per-depth opacity
   int32_t* group_off;  // [4C+1]
   float bg[3];
 };

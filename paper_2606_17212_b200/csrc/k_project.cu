@@ -328,11 +328,23 @@ __global__ void __launch_bounds__(128) k_project4(DeviceScene sc, FrameParams fp
     mu[3][k] = __fadd_rn(mu[2][k], __ldg(sc.delta + (size_t)(3 + k) * sc.N + i));
   }
   Proj pr[4];
+  float opv[4], tauv[4];
   bool any = false;
 #pragma unroll
   for (int v = 0; v < 4; ++v) {
     pr[v].count = 0;
-    if (v >= lvl) pr[v] = project_variant(fp, mu[v], S6, tau);
+    opv[v] = opac; tauv[v] = tau;
+    if (v >= lvl) {
+      if (sc.g1v) {  // scale / rotation / opacity refinements (reading I2): attributes of delivered depth v
+        const float4 h1 = __ldg(sc.g1v + (size_t)v * sc.N + i), h2 = __ldg(sc.g2v + (size_t)v * sc.N + i);
+        const float Sv[6] = {h1.x, h1.y, h1.z, h2.x, h2.y, h2.z};
+        opv[v] = __ldg(sc.opv + (size_t)v * sc.N + i);
+        tauv[v] = h1.w;
+        pr[v] = project_variant(fp, mu[v], Sv, tauv[v]);
+      } else {
+        pr[v] = project_variant(fp, mu[v], S6, tau);
+      }
+    }
     any |= pr[v].count > 0;
   }
   float col[4][3] = {{0.f, 0.f, 0.f}, {0.f, 0.f, 0.f}, {0.f, 0.f, 0.f}, {0.f, 0.f, 0.f}};
@@ -365,7 +377,7 @@ __global__ void __launch_bounds__(128) k_project4(DeviceScene sc, FrameParams fp
   }
 #pragma unroll
   for (int v = 0; v < 4; ++v)
-    store_record(ws, 4u * i + (uint32_t)v, pr[v], opac, tau, (uint32_t)c | ((uint32_t)(16 + v) << 16), col[v], col[v]);
+    store_record(ws, 4u * i + (uint32_t)v, pr[v], opv[v], tauv[v], (uint32_t)c | ((uint32_t)(16 + v) << 16), col[v], col[v]);
 }
 
 void launch_project(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, cudaStream_t st) {

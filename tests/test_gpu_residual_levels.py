@@ -26,9 +26,11 @@ def gsr(torch_mod):
     return G
 
 
-def _workload(seed, **kw):
+def _workload(seed, attrs=False, **kw):
     wl = synth.scaled_object_workload(seed, **kw)
     wl.scene = synth.with_position_residuals(wl.scene, seed_cfg=seed)
+    if attrs:   # + per-level scale / rotation / opacity refinements (reading I2)
+        wl.scene = synth.with_attribute_refinements(wl.scene, seed_cfg=seed)
     return wl
 
 
@@ -40,8 +42,9 @@ def _render(torch, scene, cam, t, lv, **kw):
     return out, mse, psnr, ws
 
 
-def test_projection_bit_exact_per_depth(gsr, torch_mod, oracle_mod):
-    wl = _workload(21, C=5, per_cluster=700.0, W=168, H=120, fov=40.0, n_frames=2, B=8)
+@pytest.mark.parametrize("attrs", [False, True])
+def test_projection_bit_exact_per_depth(gsr, torch_mod, oracle_mod, attrs):
+    wl = _workload(21, attrs=attrs, C=5, per_cluster=700.0, W=168, H=120, fov=40.0, n_frames=2, B=8)
     sc = wl.scene
     for cam, t in wl.frames:
         scene = gsr.Scene(sc)
@@ -74,9 +77,10 @@ def test_projection_bit_exact_per_depth(gsr, torch_mod, oracle_mod):
         scene.close()
 
 
-def test_keys_pixels_distortion_and_batch_invariance(gsr, torch_mod, oracle_mod):
+@pytest.mark.parametrize("attrs", [False, True])
+def test_keys_pixels_distortion_and_batch_invariance(gsr, torch_mod, oracle_mod, attrs):
     torch = torch_mod
-    wl = _workload(22, C=7, per_cluster=500.0, W=136, H=104, fov=40.0, n_frames=1, B=40)
+    wl = _workload(22, attrs=attrs, C=7, per_cluster=500.0, W=136, H=104, fov=40.0, n_frames=1, B=40)
     cam, t = wl.frames[0]
     lv = wl.levels[0]
     scene = gsr.Scene(wl.scene)
@@ -127,4 +131,24 @@ def test_zero_residuals_equal_the_two_variant_path(gsr, torch_mod):
     assert (s2.V, s4.V) == (2, 4)
     a, _, _, _ = _render(torch, s2, cam, t, lv)
     b, _, _, _ = _render(torch, s4, cam, t, lv)
+    assert torch.equal(a, b)
+
+
+def test_attribute_refinements_alone_and_zero(gsr, torch_mod, oracle_mod):
+    """Attribute refinements without position residuals; zero refinements == the two-record path bitwise."""
+    import dataclasses
+    torch = torch_mod
+    wl = synth.scaled_object_workload(24, C=4, per_cluster=400.0, W=96, H=80, fov=40.0, n_frames=1, B=16)
+    cam, t = wl.frames[0]
+    lv = wl.levels[0]
+    sc = synth.with_attribute_refinements(wl.scene, seed_cfg=24)
+    scene = gsr.Scene(sc)
+    assert scene.V == 4
+    out, _, _, _ = _render(torch, scene, cam, t, lv)
+    o_img, _ = oracle_mod.OracleScene(sc).render_batch(cam, t, lv)
+    assert np.abs(out.cpu().numpy() - o_img).max() <= PIX_TOL
+    z = lambda *shape: np.zeros((3, sc.N) + shape, np.float32)
+    s0 = gsr.Scene(dataclasses.replace(wl.scene, d_log_scale=z(3), d_quat=z(4), d_opacity_logit=z()))
+    a, _, _, _ = _render(torch, gsr.Scene(wl.scene), cam, t, lv)
+    b, _, _, _ = _render(torch, s0, cam, t, lv)
     assert torch.equal(a, b)
