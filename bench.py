@@ -48,6 +48,11 @@ def build_workload(name: str, n_frames: int):
         return wl
     if name == "cfg1":
         return synth.workload_cfg1(n_frames=n_frames)
+    if name == "cfg1r":   # cfg1 with the full representation: delta2/delta3 + scale/rotation/opacity refinements
+        wl = synth.workload_cfg1(n_frames=n_frames)
+        wl.scene = synth.with_attribute_refinements(synth.with_position_residuals(wl.scene))
+        wl.name = "cfg1r_full_representation_800x800_B256"
+        return wl
     if name == "cfg2":
         return synth.workload_cfg2(n_frames=n_frames)
     if name == "cfg3":
@@ -198,7 +203,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     total_steps = args.steps + args.warmup
-    n_frames = min(150, max(1, total_steps * world)) if args.workload == "cfg1" else min(8, max(1, total_steps))
+    n_frames = min(150, max(1, total_steps * world)) if args.workload in ("cfg1", "cfg1r") else min(8, max(1, total_steps))
     wl = build_workload(args.workload, n_frames)
     n_frames = len(wl.frames)
     scene = gsr.Scene(wl.scene)
@@ -539,7 +544,7 @@ def main():
     ap.add_argument("--steps", type=int, default=60)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg1", choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4", "atlas"])
+    ap.add_argument("--workload", default="cfg1", choices=["cfg0", "cfg1", "cfg1r", "cfg2", "cfg3", "cfg4", "atlas"])
     ap.add_argument("--ref-states", type=int, default=64, help="states per frame the CPU oracle renders")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--state-block", type=int, default=0, help="states per compositing CTA (0 = library default)")
