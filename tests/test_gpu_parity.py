@@ -460,3 +460,52 @@ def test_full_size_cfg1_frame_sampled_states(gsr, torch_mod, oracle_mod):
     mse_u, psnr_u = gsr.distortion(out, ref)
     assert torch_mod.equal(mse_u, mse) and torch_mod.equal(psnr_u, psnr)
     scene.close()
+
+
+def _full_size_sampled(gsr, torch, oracle_mod, wl, frame, pick, images):
+    """A bench-sized frame in the launch configuration bench.py times (default state block, dedup on, fused
+    distortion; images materialised or not): PSNR and I_b of sampled states against the oracle, their pixels
+    through a one-state-at-a-time re-render (bitwise equal to the batch by the batched == serial property)."""
+    cam, t = wl.frames[frame]
+    lv = wl.levels[frame]
+    scene = gsr.Scene(wl.scene)
+    osc = oracle_mod.OracleScene(wl.scene)
+    B = lv.shape[0]
+    ws = scene.new_workspace(cam, B)
+    out = torch.empty((B, cam.H, cam.W, 3), dtype=torch.float32, device="cuda") if images else None
+    ref = torch.empty((cam.H, cam.W, 3), dtype=torch.float32, device="cuda")
+    mse = torch.empty(B, dtype=torch.float64, device="cuda")
+    psnr = torch.empty(B, dtype=torch.float32, device="cuda")
+    scene.render_states_vs_full(cam, t, _dev_levels(torch, lv), ws, ref, mse, psnr, out=out)
+    scene.status(ws)
+    counts = scene.debug_state_counts(ws, B)
+    o_img, o_stats = osc.render_batch(cam, t, np.concatenate([lv[pick], np.full((1, wl.scene.C), 3, np.int8)]))
+    assert np.abs(ref.cpu().numpy() - o_img[-1]).max() <= PIX_TOL
+    _, o_psnr = oracle_mod.distortion(o_img[:-1], o_img[-1])
+    assert np.max(np.abs(psnr.cpu().numpy()[pick] - o_psnr)) <= DB_TOL
+    assert np.array_equal(counts[pick], o_stats[:-1, 0])
+    ws1 = scene.new_workspace(cam, 1)
+    for k, b in enumerate(pick):
+        o1, m1, _ = scene.render_states(cam, t, _dev_levels(torch, lv[b:b + 1]), workspace=ws1, ref=ref)
+        scene.status(ws1)
+        assert np.abs(o1[0].cpu().numpy() - o_img[k]).max() <= PIX_TOL, b
+        assert torch.equal(m1[0], mse[b])                          # batched == serial, bitwise
+        if images:
+            assert torch.equal(o1[0], out[b])
+    scene.close()
+
+
+def test_full_size_cfg2_frame_sampled_states(gsr, torch_mod, oracle_mod):
+    """configs[2]: 64 clusters, ~300 k Gaussians, 536 x 960 (ragged tiles), B = 512, images materialised."""
+    _full_size_sampled(gsr, torch_mod, oracle_mod, synth.workload_cfg2(n_frames=1), 0, [0, 255, 511], images=True)
+
+
+def test_full_size_cfg3_view_sampled_states(gsr, torch_mod, oracle_mod):
+    """configs[3]: one view of the utility sweep, B = 6144 paired states, no images (fused distortion only)."""
+    _full_size_sampled(gsr, torch_mod, oracle_mod, synth.workload_cfg3(n_views=1), 0, [0, 3071, 3072, 6143],
+                       images=False)
+
+
+def test_full_size_cfg4_time_step_sampled_states(gsr, torch_mod, oracle_mod):
+    """configs[4]: 128 clusters, ~1 M Gaussians, 1920 x 1080, one time step of 256 states, no images."""
+    _full_size_sampled(gsr, torch_mod, oracle_mod, synth.workload_cfg4(), 2, [0, 100, 255], images=False)
