@@ -68,6 +68,7 @@ typedef struct {
   const float* cov3d_lv;
   const float* opacity_lv;
   const float* tau_lv;
+  const float* d_sh;        /* [3][N,K,3] per-level colour residuals (levels 1..3; reading I3), or NULL */
   float background[3];
 } orc_scene;
 
@@ -306,6 +307,9 @@ static void project_one(const orc_scene* s, const orc_camera* cam, float t, cons
     for (int j = 0; j < s->K; ++j) {
       double coef = (double)s->sh_base[((int64_t)i * s->K + j) * 3 + ch];
       if (d >= 3) coef += (double)s->sh_res[((int64_t)i * s->K + j) * 3 + ch];
+      if (s->d_sh) /* colour: base plus the learned refinements of the delivered levels */
+        for (int l = 1; l <= d && l <= 3; ++l)
+          coef += (double)s->d_sh[(((int64_t)(l - 1) * s->N + i) * s->K + j) * 3 + ch];
       acc += Y[j] * coef;
     }
     o->rgb[ch] = acc > 0.0 ? acc : 0.0;

@@ -37,7 +37,7 @@ class _Scene(C.Structure):
                 ("opacity", C.c_void_p), ("tau", C.c_void_p), ("sh_base", C.c_void_p),
                 ("sh_res", C.c_void_p), ("motion_q", C.c_void_p), ("A0", C.c_void_p), ("A1", C.c_void_p),
                 ("motion_scale", C.c_void_p), ("delta2", C.c_void_p), ("delta3", C.c_void_p),
-                ("cov3d_lv", C.c_void_p), ("opacity_lv", C.c_void_p), ("tau_lv", C.c_void_p),
+                ("cov3d_lv", C.c_void_p), ("opacity_lv", C.c_void_p), ("tau_lv", C.c_void_p), ("d_sh", C.c_void_p),
                 ("background", C.c_float * 3)]
 
 
@@ -159,6 +159,8 @@ class OracleScene:
                                _p(self.tau_lv[v]))
             s.cov3d_lv, s.opacity_lv, s.tau_lv = (self.cov3d_lv.ctypes.data, self.opacity_lv.ctypes.data,
                                                    self.tau_lv.ctypes.data)
+        self.d_sh = _c(sc.d_sh, np.float32) if getattr(sc, "d_sh", None) is not None else None
+        s.d_sh = self.d_sh.ctypes.data if self.d_sh is not None else None
         s.background[:] = [float(v) for v in np.asarray(sc.background, np.float32)]
         self._s = s
 

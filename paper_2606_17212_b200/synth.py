@@ -51,6 +51,7 @@ class Scene:
     d_log_scale: np.ndarray | None = None      # f32 [3,N,3]
     d_quat: np.ndarray | None = None           # f32 [3,N,4]
     d_opacity_logit: np.ndarray | None = None  # f32 [3,N]
+    d_sh: np.ndarray | None = None             # f32 [3,N,K,3] per-level colour residuals
 
     @property
     def K(self) -> int:
@@ -475,11 +476,14 @@ def with_attribute_refinements(sc: Scene, seed_cfg: int = 6, s_scale: float = 0.
                                s_logit: float = 0.3) -> Scene:
     """The same scene with per-level refinements of scale, rotation and opacity ("Scale, rotation,
     opacity, and colour use a base plus three learned refinements"): additive residuals on log-scale, raw
-    quaternion and opacity logit, N(0, (s / 2^(l-1))^2) at level l = 1..3 (finer planes at later levels)."""
+    quaternion and opacity logit, N(0, (s / 2^(l-1))^2) at level l = 1..3 (finer planes at later levels), and
+    per-level SH colour residuals of the same decay."""
     import dataclasses
     rng = _rng(seed_cfg, 8)
     f = np.array([1.0, 0.5, 0.25])[:, None, None]
     dls = (rng.normal(0.0, 1.0, (3, sc.N, 3)) * s_scale * f).astype(np.float32)
     dq = (rng.normal(0.0, 1.0, (3, sc.N, 4)) * s_quat * f).astype(np.float32)
     dlg = (rng.normal(0.0, 1.0, (3, sc.N)) * s_logit * f[:, :, 0]).astype(np.float32)
-    return dataclasses.replace(sc, d_log_scale=dls, d_quat=dq, d_opacity_logit=dlg)
+    K = (sc.sh_degree + 1) ** 2
+    dsh = (rng.normal(0.0, 1.0, (3, sc.N, K, 3)) * 0.03 * f[:, :, :, None]).astype(np.float32)
+    return dataclasses.replace(sc, d_log_scale=dls, d_quat=dq, d_opacity_logit=dlg, d_sh=dsh)

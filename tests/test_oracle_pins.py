@@ -620,3 +620,27 @@ def test_p19_attribute_refinement_levels(oracle_mod):
         assert pr["cov2d"][0][0] == pytest.approx(sig2, rel=1e-5)
         alpha = min(0.99, o_v)                                       # at the centre exp(0) = 1
         assert img[32, 32, 0] == pytest.approx(0.8 * alpha, rel=1e-5)
+
+
+def test_p19b_colour_refinement_levels(oracle_mod):
+    """Reading I3: per-level SH residuals; the colour at depth v uses sh_base + levels 1..v (+ sh_res at 3).
+    Degree-0 closed form: rgb = max(0, 0.5 + Y0 (sh0 + sum_{l<=v} d_l)); zero residuals == none."""
+    import dataclasses
+    one, _ = tiny_scene([[0.0, 0.0, 0.0]], 0.05, colors=[0.5, 0.5, 0.5], levels=[0])
+    dsh = np.zeros((3, 1, 1, 3), np.float32)
+    dsh[0, 0, 0] = [0.3, 0.0, -0.2]
+    dsh[1, 0, 0] = [0.1, 0.2, 0.0]
+    dsh[2, 0, 0] = [-3.0, 0.1, 0.1]                   # drives the red channel below zero: clamped
+    o = oracle_mod.OracleScene(dataclasses.replace(one, d_sh=dsh))
+    cam = axis_camera()
+    for d in range(4):
+        want = np.maximum(0.0, 0.5 + Y0 * dsh[:d, 0, 0].astype(np.float64).sum(axis=0))
+        got = o.project(cam, 0.0, np.array([d], np.int8))["rgb"][0]
+        assert np.allclose(got, want, rtol=0, atol=1e-12), (d, got, want)
+    wl = synth.workload_cfg0()
+    sc, (camw, t) = wl.scene, wl.frames[0]
+    z = oracle_mod.OracleScene(dataclasses.replace(sc, d_sh=np.zeros((3, sc.N, sc.K, 3), np.float32)))
+    b = oracle_mod.OracleScene(sc)
+    for d in range(4):
+        dep = np.full(sc.C, d, np.int8)
+        assert z.project(camw, t, dep).tobytes() == b.project(camw, t, dep).tobytes()
