@@ -80,6 +80,9 @@ typedef struct {
   const float* d_log_scale;
   const float* d_quat;
   const float* d_opacity_logit;
+  /* Optional per-level colour residuals [3,N,K,3] (levels 1..3; reading I3): the SH coefficients at
+   * depth v are sh_base + levels 1..v (+ sh_res at depth 3).  NULL = zero; also selects 4 records per Gaussian. */
+  const float* d_sh;
 } gsr_scene_desc;
 
 /* Pinhole camera, OpenCV axes (x right, y down, z forward), pixel centres at +0.5 (reading A9).

@@ -285,9 +285,10 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
   DeviceScene& D = sc->impl.d;
   D.C = C; D.N = N; D.K = K; D.R = R; D.sh_degree = d->sh_degree; D.n_sh4 = n_sh4; D.n_qw = n_qw;
   const bool has_attr = d->d_log_scale || d->d_quat || d->d_opacity_logit;
-  const bool has_delta = d->delta2 || d->delta3 || has_attr;  // 4 records per Gaussian
+  const bool has_dsh = d->d_sh != nullptr;
+  const bool has_delta = d->delta2 || d->delta3 || has_attr || has_dsh;  // 4 records per Gaussian
   D.V = has_delta ? 4 : 2;
-  D.delta = nullptr; D.g1v = nullptr; D.g2v = nullptr; D.opv = nullptr;
+  D.delta = nullptr; D.g1v = nullptr; D.g2v = nullptr; D.opv = nullptr; D.d_sh = nullptr;
   for (int k = 0; k < 3; ++k) D.bg[k] = d->background[k];
   size_t off = 0;
   auto reserve = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
@@ -298,7 +299,8 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
                o_ms = reserve(sizeof(float) * C), o_go = reserve(sizeof(int32_t) * (4 * C + 1)),
                o_dl = reserve(has_delta ? sizeof(float) * 6 * Np : 0),
                o_g1v = reserve(has_attr ? sizeof(float4) * 4 * Np : 0), o_g2v = reserve(has_attr ? sizeof(float4) * 4 * Np : 0),
-               o_opv = reserve(has_attr ? sizeof(float) * 4 * Np : 0);
+               o_opv = reserve(has_attr ? sizeof(float) * 4 * Np : 0),
+               o_dsh = reserve(has_dsh ? sizeof(float4) * 3 * n_sh4 * Np : 0);
   cudaError_t e = cudaMalloc(&sc->impl.blob, off);
   if (e != cudaSuccess) {
     set_error("gsr_load_scene: cudaMalloc(%zu) failed: %s", off, cudaGetErrorString(e));
@@ -311,6 +313,7 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
   D.A0 = (float*)(base + o_A0); D.A1 = (float*)(base + o_A1); D.mscale = (float*)(base + o_ms);
   D.group_off = (int32_t*)(base + o_go);
   if (has_delta) D.delta = (float*)(base + o_dl);
+  if (has_dsh) D.d_sh = (float4*)(base + o_dsh);
   if (has_attr) { D.g1v = (float4*)(base + o_g1v); D.g2v = (float4*)(base + o_g2v); D.opv = (float*)(base + o_opv); }
   bool ok = true;
   auto up = [&](void* dst, const void* src, size_t bytes) {
@@ -330,6 +333,20 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
         if (d->delta3) dl[(size_t)(3 + k) * Np + i] = d->delta3[3 * (size_t)i + k];
       }
     up(D.delta, dl.data(), sizeof(float) * 6 * Np);
+  }
+  if (has_dsh) {  // [3][n_sh4][N] float4 words of the flat coefficient index j*3+ch, zero padded (as sh_base)
+    std::vector<float4> ds((size_t)3 * n_sh4 * Np, make_float4(0.f, 0.f, 0.f, 0.f));
+    for (int l = 0; l < 3; ++l)
+      for (int i = 0; i < N; ++i)
+        for (int w4 = 0; w4 < n_sh4; ++w4) {
+          float v[4] = {0, 0, 0, 0};
+          for (int e = 0; e < 4; ++e) {
+            const int flat = 4 * w4 + e;
+            if (flat < 3 * K) v[e] = d->d_sh[((size_t)l * N + i) * 3 * K + flat];
+          }
+          ds[((size_t)l * n_sh4 + w4) * Np + i] = make_float4(v[0], v[1], v[2], v[3]);
+        }
+    up(D.d_sh, ds.data(), sizeof(float4) * 3 * n_sh4 * Np);
   }
   if (has_attr) {  // per-depth attributes: base + levels 1..v in binary32 (level order), then §3.0 (reading I2)
     std::vector<float4> a1(4 * Np), a2(4 * Np);

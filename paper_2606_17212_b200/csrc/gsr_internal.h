@@ -32,6 +32,7 @@ struct DeviceScene {
   float4* g1v;      // [4][N] per-depth (Sxx Sxy Sxz, tau) of scenes with attribute refinements, else nullptr
   float4* g2v;      // [4][N] per-depth (Syy Syz Szz, -)
   float* opv;       // [4][N] per-depth opacity
+  float4* d_sh;     // [3][n_sh4][N] per-level colour residuals (layout of sh_base), else nullptr
   int32_t* group_off;  // [4C+1]
   float bg[3];
 };

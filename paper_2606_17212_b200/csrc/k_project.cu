@@ -358,8 +358,14 @@ __global__ void __launch_bounds__(128) k_project4(DeviceScene sc, FrameParams fp
       float sb[3] = {0.5f, 0.5f, 0.5f}, sr[3] = {0.f, 0.f, 0.f};
 #pragma unroll
       for (int w4 = 0; w4 < n4; ++w4) {
-        const float4 cb = __ldg(sc.sh_base + (size_t)w4 * sc.N + i);
+        float4 cb = __ldg(sc.sh_base + (size_t)w4 * sc.N + i);
         const float4 cr = __ldg(sc.sh_res + (size_t)w4 * sc.N + i);
+        if (sc.d_sh) {  // colour refinements of the delivered levels 1..v (reading I3)
+          for (int l = 0; l < v; ++l) {
+            const float4 dl = __ldg(sc.d_sh + ((size_t)l * n4 + w4) * sc.N + i);
+            cb.x += dl.x; cb.y += dl.y; cb.z += dl.z; cb.w += dl.w;
+          }
+        }
         const float vb[4] = {cb.x, cb.y, cb.z, cb.w}, vr[4] = {cr.x, cr.y, cr.z, cr.w};
 #pragma unroll
         for (int e = 0; e < 4; ++e) {

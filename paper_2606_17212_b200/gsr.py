@@ -29,7 +29,8 @@ class SceneDesc(C.Structure):
                 ("opacity_logit", C.c_void_p), ("sh_base", C.c_void_p), ("sh_res", C.c_void_p),
                 ("motion_q", C.c_void_p), ("A0", C.c_void_p), ("A1", C.c_void_p), ("motion_scale", C.c_void_p),
                 ("background", C.c_float * 3), ("delta2", C.c_void_p), ("delta3", C.c_void_p),
-                ("d_log_scale", C.c_void_p), ("d_quat", C.c_void_p), ("d_opacity_logit", C.c_void_p)]
+                ("d_log_scale", C.c_void_p), ("d_quat", C.c_void_p), ("d_opacity_logit", C.c_void_p),
+                ("d_sh", C.c_void_p)]
 
 
 class CameraC(C.Structure):
@@ -193,7 +194,7 @@ class Scene:
         d.background[:] = [float(v) for v in np.asarray(sc.background, np.float32)]
         self.V = 2                                   # projected records per Gaussian
         # optional position residual levels of Eq. (1) and per-level scale / rotation / opacity refinements
-        for name in ("delta2", "delta3", "d_log_scale", "d_quat", "d_opacity_logit"):
+        for name in ("delta2", "delta3", "d_log_scale", "d_quat", "d_opacity_logit", "d_sh"):
             a = getattr(sc, name, None)
             if a is not None:
                 keep[name] = _np(a, np.float32)
