@@ -30,11 +30,11 @@ if str(ROOT) not in sys.path:
 
 from paper_2606_17212_b200 import shard, synth  # noqa: E402
 
-# FLOP accounting of the compositing kernel (DESIGN.md §7.2), FMA = 2 flop:
-#   per (pixel, record) alpha evaluation : dx, dy (2) + u (1) + s (2) + q (1) + v (1) + q (2) + o*e (1) + 1-alpha (1) = 11
-#   per (pixel, record, state) update    : T' (1) + alpha*T (1) + 3 FMA (6) + the T' < 1e-4 compare (1)          =  9
+# FLOP accounting of the compositing kernel (DESIGN.md §6), FMA = 2 flop:
+#   per (pixel, record) alpha evaluation : dx, dy (2) + u (1) + s (2) + q (1) + v (1) + q (2) + o*e (1)               = 10
+#   per (pixel, record, state) update    : w = alpha*T (1) + T' = T - w (1) + 3 FMA (6) + the T' < 1e-4 compare (1) =  9
 #   literal per-state model: 20 flop per logical (pixel, Gaussian, state) pair
-FLOP_SHARED, FLOP_STATE, FLOP_LITERAL = 11.0, 9.0, 20.0
+FLOP_SHARED, FLOP_STATE, FLOP_LITERAL = 10.0, 9.0, 20.0
 NOMINAL_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # 74.4: SMs x FP32 lanes x 2 x max SM clock
 
 

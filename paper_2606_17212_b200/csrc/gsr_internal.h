@@ -13,7 +13,7 @@ constexpr int kTile = GSR_TILE;
 constexpr int kTilePix = kTile * kTile;  // 256 threads per compositing CTA, one per pixel
 constexpr int kMaxC = 4096;              // clusters (mask table lives in shared memory)
 
-// ---- device scene (DESIGN.md §5.1): SoA of 16-byte words so that every warp load is 512 B contiguous
+// ---- device scene (DESIGN.md §5): SoA of 16-byte words so that every warp load is 512 B contiguous
 struct DeviceScene {
   int32_t C, N, K, R, sh_degree;
   int32_t V;      // projected records per Gaussian: 2 (no position residual levels) or 4 (delta2 / delta3 given)
@@ -49,7 +49,7 @@ struct FrameParams {
   float bg[3];
 };
 
-// ---- workspace (DESIGN.md §5.2)
+// ---- workspace (DESIGN.md §5)
 struct WsHeader {
   int32_t status;        // GSR_OK / GSR_E_INVALID_LEVEL / GSR_E_WORKSPACE_TOO_SMALL (latched by kernels)
   int32_t B, C, N;

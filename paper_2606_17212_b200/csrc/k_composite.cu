@@ -1,4 +1,4 @@
-// k_composite.cu — stage a4 (+ fused a5) of the hot path (DESIGN.md §3.5, §4.3, §6.3):
+// k_composite.cu — stage a4 (+ fused a5) of the hot path (DESIGN.md §3.5, §4.3-§4.6, §6):
 // per-tile front-to-back alpha compositing with early termination, state-blocked.
 //
 // One CTA = one 16x16 tile x S states of the batch; thread = pixel; each thread keeps (T, r, g, b)

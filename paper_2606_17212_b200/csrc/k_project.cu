@@ -1,4 +1,4 @@
-// k_project.cu — stages a0..a2 of the hot path (DESIGN.md §3.1-§3.3, §6.1):
+// k_project.cu — stages a0..a2 of the hot path (DESIGN.md §3.1-§3.3, §6):
 //   K0  closure / validation of the delivered-depth matrix (north_star (1))
 //   K1  per-variant deformation (Eq. (1)) + EWA projection + SH colour
 //
@@ -136,7 +136,7 @@ __device__ __forceinline__ Proj project_variant(const FrameParams& fp, const flo
   o.mx = mx; o.my = my;
   o.qa = __fmul_rn(0.5f, conic_a); o.qb = conic_b; o.qc = __fmul_rn(0.5f, conic_c);
   {
-    // Sub-tile culling bound (DESIGN.md §6.3): {q <= tau} is the ellipse x^T Sigma'^-1 x <= 2 tau, whose
+    // Sub-tile culling bound (DESIGN.md §4.6): {q <= tau} is the ellipse x^T Sigma'^-1 x <= 2 tau, whose
     // half-extents are sqrt(2 tau a), sqrt(2 tau c).  The kernel evaluates q in fp32 from the ROUNDED
     // conic, so the bound is inflated by m = 8e-6 kappa + 1e-3, kappa = a c / det >= 1 (conditioning of
     // the form: bounds both the conic rounding and the cancellation in q, each < 3e-6 kappa), and tau by

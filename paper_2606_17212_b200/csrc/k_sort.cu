@@ -1,4 +1,4 @@
-// k_sort.cu — stage a3 of the hot path (DESIGN.md §3.4, §6.2): tile binning and the key sort.
+// k_sort.cu — stage a3 of the hot path (DESIGN.md §3.4, §4.2, §6): tile binning and the key sort.
 //
 //   K2a  exclusive scan of the per-record tile counts (warp-shuffle segmented scan, 3 phases)
 //   K2b  key emission: (tile << 32 | depth bits) with the record id as payload, written at

@@ -1,5 +1,5 @@
 // k_utility.cu — stage a5b: counterfactual utility, Eq. (3) per pair and Eq. (4) per group
-// (DESIGN.md §3.7, §6.5).
+// (DESIGN.md §3.7, §6).
 //
 //   delta_mse[p] = MSE(m) - MSE(m u g)          Eq. (3) with D = MSE
 //   delta_db[p]  = PSNR(m u g) - PSNR(m)        Eq. (3) with D = -PSNR  (unit of the 1e-3 dB tolerance)
