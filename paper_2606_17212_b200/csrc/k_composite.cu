@@ -106,7 +106,7 @@ constexpr float kTStop = 1e-4f;     // reading A11
 constexpr float kAlphaCap = 0.99f;  // reading A11
 
 template <int S, bool COUNT>
-__global__ void __launch_bounds__(kTilePix, (S <= 8 ? 4 : 2)) k_composite(const CompositeArgs a) {
+__global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const CompositeArgs a) {
   extern __shared__ uint16_t s_tab[];  // [C][4]: states (bit s) with depth ==0, >=1, >=2, >=3
   // staged records, 64 B each: {m_x, m_y, A, B} {Cq, tau, -, act | res << 16} {rgb, o} {rgb + SH residual, -}
   __shared__ __align__(16) float4 s_rec[kTilePix * 4];
