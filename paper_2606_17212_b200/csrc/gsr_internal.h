@@ -82,6 +82,23 @@ struct Workspace {
   size_t bytes;           // total
 };
 
+// Which of the eight 8x4 pixel blocks of tile (tx, ty) the conservative q <= tau box of a record touches
+// (DESIGN.md §4.6): centre (mx, my), half-extents (hx, hy) from k_project.  Bit k = block (k & 1, k >> 1).
+// ONE definition, used by the compositor's staging and by the tile dedup (a record with mask 0 contributes
+// to no pixel of the tile in any state, so it must not split signature classes either).
+__device__ __forceinline__ uint32_t record_block_mask(float mx, float my, float hx, float hy, int tx, int ty) {
+  const float xlo = mx - hx, xhi = mx + hx, ylo = my - hy, yhi = my + hy;
+  const float X0 = (float)(tx * kTile) + 0.5f, Y0 = (float)(ty * kTile) + 0.5f;
+  uint32_t ox = 0, oy = 0, m = 0;
+#pragma unroll
+  for (int k = 0; k < 2; ++k) ox |= (uint32_t)(xlo <= X0 + 8.0f * k + 7.0f && xhi >= X0 + 8.0f * k) << k;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) oy |= (uint32_t)(ylo <= Y0 + 4.0f * k + 3.0f && yhi >= Y0 + 4.0f * k) << k;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) m |= (((ox >> (k & 1)) & (oy >> (k >> 1))) & 1u) << k;
+  return m;
+}
+
 constexpr int kSortThreads = 256;
 constexpr int kSortItems = 4;
 constexpr int kSortTileKeys = kSortThreads * kSortItems;  // keys per block per pass

@@ -211,15 +211,7 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const 
         res = cls == 0 ? 0u : t[3];
       }
       // pixel-centre box of the record vs the eight 8x4 pixel blocks of the tile
-      const float xlo = g0.x - c0.w, xhi = g0.x + c0.w, ylo = g0.y - c1.w, yhi = g0.y + c1.w;
-      const float X0 = (float)(tx * kTile) + 0.5f, Y0 = (float)(ty * kTile) + 0.5f;
-      uint32_t ox = 0, oy = 0;
-#pragma unroll
-      for (int k = 0; k < 2; ++k) ox |= (uint32_t)(xlo <= X0 + 8.0f * k + 7.0f && xhi >= X0 + 8.0f * k) << k;
-#pragma unroll
-      for (int k = 0; k < 4; ++k) oy |= (uint32_t)(ylo <= Y0 + 4.0f * k + 3.0f && yhi >= Y0 + 4.0f * k) << k;
-#pragma unroll
-      for (int k = 0; k < 8; ++k) wmask |= (((ox >> (k & 1)) & (oy >> (k >> 1))) & 1u) << k;
+      wmask = record_block_mask(g0.x, g0.y, c0.w, c1.w, tx, ty);
     }
     // ordered compaction: the record keeps slot `tid` of the staging buffer; each 8x4 pixel block k gets
     // the ordered list s_list[k] of the slots whose box touches it (warp ballots + an 8x8 count table)

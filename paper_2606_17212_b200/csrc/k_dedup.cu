@@ -41,7 +41,10 @@ __device__ __forceinline__ uint32_t class_sig(uint32_t bits, int d) {
 
 __global__ void __launch_bounds__(kDedupThreads) k_tile_dedup(const uint2* __restrict__ tile_range,
                                                               const uint32_t* __restrict__ vals,
+                                                              const float4* __restrict__ r0,
                                                               const float4* __restrict__ r1,
+                                                              const float4* __restrict__ rc0,
+                                                              const float4* __restrict__ rc1, int TX,
                                                               const int8_t* __restrict__ depth, int B, int C,
                                                               int Bp, uint32_t* __restrict__ order,
                                                               uint32_t* __restrict__ upos,
@@ -71,7 +74,12 @@ __global__ void __launch_bounds__(kDedupThreads) k_tile_dedup(const uint2* __res
   for (int k = tid; k < C; k += kDedupThreads) ccnt[k] = 0;
   __syncthreads();
   for (uint32_t i = rg.x + tid; i < rg.y; i += kDedupThreads) {
-    const uint32_t meta = __float_as_uint(r1[vals[i]].w);
+    const uint32_t rid = vals[i];
+    // a record whose q <= tau box misses every pixel of the tile is dropped by the compositor's staging in
+    // every state: it must not distinguish signature classes (same predicate: record_block_mask)
+    const float4 g0 = r0[rid];
+    if (record_block_mask(g0.x, g0.y, rc0[rid].w, rc1[rid].w, tile % TX, tile / TX) == 0u) continue;
+    const uint32_t meta = __float_as_uint(r1[rid].w);
     const uint32_t c = meta & 0xFFFFu, cls = meta >> 16;
     const uint32_t bit = cls >= 16 ? (16u << (cls - 16)) : (cls == 0 ? 1u : (cls <= 2 ? 2u : (cls == 3 ? 4u : 8u)));
     atomicOr(&cbits[c >> 2], bit << (8 * (c & 3)));
@@ -220,7 +228,7 @@ bool launch_tile_dedup(const DeviceScene& sc, const FrameParams& fp, Workspace& 
     cudaFuncSetAttribute(k_tile_dedup, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     attr_set = true;
   }
-  k_tile_dedup<<<fp.TX * fp.TY, kDedupThreads, smem, st>>>(ws.tile_range, ws.vals[0], ws.r1, depth_rows, B, sc.C, Bp,
+  k_tile_dedup<<<fp.TX * fp.TY, kDedupThreads, smem, st>>>(ws.tile_range, ws.vals[0], ws.r0, ws.r1, ws.rc0, ws.rc1, fp.TX, depth_rows, B, sc.C, Bp,
                                                           ws.uorder, ws.upos, ws.n_unique);
   count_launches(1);
   return true;
