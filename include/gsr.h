@@ -303,7 +303,9 @@ int gsr_utility_frame_host(const gsr_scene* scene, const gsr_camera* cam, float 
  *
  * gsr_debug_projection: per projected record r = 2*i + v (v = 0: geometry without the motion
  * residual, used when the cluster's depth is 0 — only level-0 Gaussians have it; v = 1: with the
- * residual, used when depth >= 1).  All host arrays of length 2N (any may be NULL):
+ * residual, used when depth >= 1).  Scenes with delta2 / delta3 / d_* arrays have FOUR records per
+ * Gaussian, r = 4*i + v, v = the delivered depth the record belongs to (a level-l Gaussian has v >= l;
+ * rgb_base and rgb_res are then equal).  All host arrays of length 2N resp. 4N (any may be NULL):
  *   valid u8, radius i32, rect i32 [2N,4] (tx0,ty0,tx1,ty1), depth_bits u32, count i32,
  *   mean2d f32 [2N,2], conic f32 [2N,3] (A=conic_a/2, B=conic_b, Cq=conic_c/2),
  *   rgb_base f32 [2N,3], rgb_res f32 [2N,3]. */
@@ -332,8 +334,9 @@ int gsr_debug_closure(const gsr_scene* scene, const void* workspace, int8_t* dep
  *   [2] logical (pixel, Gaussian, state) pairs E = sum_b E_b in the sense of the oracle. */
 int gsr_debug_pair_counts(const gsr_scene* scene, const void* workspace, int64_t* counts3, void* cuda_stream);
 
-/* Options: "state_block" = states composited per CTA (1, 4, 8 or 16; default 8) — results do not
- * depend on it (bitwise); "profile" = 1 records CUDA events around every compositing-kernel launch. */
+/* Options: "state_block" = states composited per CTA (1, 4, 8 or 16; default 8) and "dedup" = 0/1 (tile-level
+ * state dedup, default 1) — results do not depend on either (bitwise); "profile" = 1 records CUDA events around
+ * every compositing-kernel launch and around the projection and binning + sort phases of every frame. */
 int gsr_set_option(const char* name, int32_t value);
 
 /* Sum of the compositing kernel's durations (ms, CUDA events on its launch stream) and the number
