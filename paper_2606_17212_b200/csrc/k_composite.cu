@@ -348,11 +348,11 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const 
         const uint32_t* mem = a.uorder + (size_t)tile * a.B;
         for (uint32_t i = s_mlo[s]; i < s_mhi[s]; ++i) {
           float* op = a.out + (size_t)mem[i] * img + pix;
-          op[0] = o0; op[1] = o1; op[2] = o2;
+          __stcs(op, o0); __stcs(op + 1, o1); __stcs(op + 2, o2);  // write-once stream: evict first
         }
       } else {
         float* op = a.out + (size_t)s_rep[s] * img + pix;
-        op[0] = o0; op[1] = o1; op[2] = o2;
+        __stcs(op, o0); __stcs(op + 1, o1); __stcs(op + 2, o2);  // write-once stream: evict first
       }
     }
     if (a.ref) err[s] = inside ? (double)pixel_sq_err(o0, o1, o2, rr0, rr1, rr2) : 0.0;
