@@ -69,6 +69,8 @@ typedef struct {
   const float* opacity_lv;
   const float* tau_lv;
   const float* d_sh;        /* [3][N,K,3] per-level colour residuals (levels 1..3; reading I3), or NULL */
+  int32_t affine_cov;       /* != 0: the cluster affine also transforms the covariance (reading I4) */
+  int32_t pad_;
   float background[3];
 } orc_scene;
 
@@ -255,6 +257,21 @@ static void project_one(const orc_scene* s, const orc_camera* cam, float t, cons
   }
   /* Sigma' = M Sigma M^T */
   const float* S6 = s->cov3d_lv ? s->cov3d_lv + 6 * ((int64_t)d * s->N + i) : s->cov3d + 6 * (int64_t)i;
+  float S6t[6];
+  if (s->affine_cov) {
+    /* reading I4: Sigma_t = L Sigma L^T with L = the 3x3 part of A_{c,t}; binary32, this order:
+     * Mm = L S (row a, column b), then Sigma_t[a][b] = Mm[a] . L[b] */
+    const float Sf[9] = {S6[0], S6[1], S6[2], S6[1], S6[3], S6[4], S6[2], S6[4], S6[5]};
+    float Mm[9];
+    for (int a = 0; a < 3; ++a)
+      for (int b = 0; b < 3; ++b)
+        Mm[3 * a + b] = fmaf(A[4 * a + 2], Sf[6 + b], fmaf(A[4 * a + 1], Sf[3 + b], A[4 * a + 0] * Sf[b]));
+    int o6 = 0;
+    for (int a = 0; a < 3; ++a)
+      for (int b = a; b < 3; ++b)
+        S6t[o6++] = fmaf(Mm[3 * a + 2], A[4 * b + 2], fmaf(Mm[3 * a + 1], A[4 * b + 1], Mm[3 * a + 0] * A[4 * b + 0]));
+    S6 = S6t;
+  }
   float S[9] = {S6[0], S6[1], S6[2], S6[1], S6[3], S6[4], S6[2], S6[4], S6[5]};
   float v0[3], v1[3];
   for (int a = 0; a < 3; ++a) {

@@ -38,6 +38,7 @@ class _Scene(C.Structure):
                 ("sh_res", C.c_void_p), ("motion_q", C.c_void_p), ("A0", C.c_void_p), ("A1", C.c_void_p),
                 ("motion_scale", C.c_void_p), ("delta2", C.c_void_p), ("delta3", C.c_void_p),
                 ("cov3d_lv", C.c_void_p), ("opacity_lv", C.c_void_p), ("tau_lv", C.c_void_p), ("d_sh", C.c_void_p),
+                ("affine_cov", C.c_int32), ("pad_", C.c_int32),
                 ("background", C.c_float * 3)]
 
 
@@ -161,6 +162,7 @@ class OracleScene:
                                                    self.tau_lv.ctypes.data)
         self.d_sh = _c(sc.d_sh, np.float32) if getattr(sc, "d_sh", None) is not None else None
         s.d_sh = self.d_sh.ctypes.data if self.d_sh is not None else None
+        s.affine_cov = 1 if getattr(sc, "affine_on_covariance", False) else 0
         s.background[:] = [float(v) for v in np.asarray(sc.background, np.float32)]
         self._s = s
 

@@ -52,6 +52,7 @@ class Scene:
     d_quat: np.ndarray | None = None           # f32 [3,N,4]
     d_opacity_logit: np.ndarray | None = None  # f32 [3,N]
     d_sh: np.ndarray | None = None             # f32 [3,N,K,3] per-level colour residuals
+    affine_on_covariance: bool = False         # the cluster affine also transforms Sigma (reading I4)
 
     @property
     def K(self) -> int:

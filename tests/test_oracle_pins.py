@@ -644,3 +644,34 @@ def test_p19b_colour_refinement_levels(oracle_mod):
     for d in range(4):
         dep = np.full(sc.C, d, np.int8)
         assert z.project(camw, t, dep).tobytes() == b.project(camw, t, dep).tobytes()
+
+
+def test_p20_affine_push_forward_of_covariance(oracle_mod):
+    """Reading I4 (optional): Sigma_t = L Sigma L^T with L = the 3x3 part of A_{c,t}.  L = I changes nothing
+    (bitwise); L = s I scales the screen variance by s^2 (closed form of P3); a 90-degree roll about the optical
+    axis swaps the two screen variances of an axis-aligned anisotropic Gaussian (P7)."""
+    import dataclasses
+    wl = synth.workload_cfg0()
+    sc, (cam, t) = wl.scene, wl.frames[0]
+    ident = dataclasses.replace(sc, A1=np.zeros_like(sc.A1), affine_on_covariance=True)
+    plain = dataclasses.replace(sc, A1=np.zeros_like(sc.A1))
+    for d in (0, 3):
+        dep = np.full(sc.C, d, np.int8)
+        assert oracle_mod.OracleScene(ident).project(cam, t, dep).tobytes() == \
+            oracle_mod.OracleScene(plain).project(cam, t, dep).tobytes()
+    f, z0, s0 = 100.0, 4.0, 0.05
+    camx = axis_camera(W=64, H=64, f=f, z0=z0)
+    for scale in (0.5, 2.0):
+        A0 = np.zeros((1, 3, 4)); A0[0, :, :3] = scale * np.eye(3)
+        one, _ = tiny_scene([[0.0, 0.0, 0.0]], s0, levels=[0], A0=A0)
+        one = dataclasses.replace(one, affine_on_covariance=True)
+        pr = oracle_mod.OracleScene(one).project(camx, 0.0, np.array([0], np.int8))
+        assert pr["cov2d"][0][0] == pytest.approx((f * scale * s0 / z0) ** 2 + 0.3, rel=1e-5)
+    # roll by 90 degrees about z: x' = -y, y' = x
+    A0 = np.zeros((1, 3, 4)); A0[0, 0, 1] = -1.0; A0[0, 1, 0] = 1.0; A0[0, 2, 2] = 1.0
+    aniso, _ = tiny_scene([[0.0, 0.0, 0.0]], np.array([[0.08, 0.02, 0.05]]), levels=[0], A0=A0)
+    p_off = oracle_mod.OracleScene(aniso).project(camx, 0.0, np.array([0], np.int8))
+    p_on = oracle_mod.OracleScene(dataclasses.replace(aniso, affine_on_covariance=True)).project(camx, 0.0, np.array([0], np.int8))
+    assert p_on["cov2d"][0][0] == pytest.approx(p_off["cov2d"][0][2], rel=1e-5)
+    assert p_on["cov2d"][0][2] == pytest.approx(p_off["cov2d"][0][0], rel=1e-5)
+    assert abs(p_on["cov2d"][0][1]) < 1e-4
