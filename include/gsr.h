@@ -83,6 +83,9 @@ typedef struct {
   /* Optional per-level colour residuals [3,N,K,3] (levels 1..3; reading I3): the SH coefficients at
    * depth v are sh_base + levels 1..v (+ sh_res at depth 3).  NULL = zero; also selects 4 records per Gaussian. */
   const float* d_sh;
+  /* != 0: the cluster affine also transforms the 3-D covariance, Sigma_t = L Sigma L^T with L = the 3x3 part of
+   * A_c(t) (reading I4; Eq. (1) itself only moves the mean, so the default is 0). */
+  int32_t affine_on_covariance;
 } gsr_scene_desc;
 
 /* Pinhole camera, OpenCV axes (x right, y down, z forward), pixel centres at +0.5 (reading A9).

@@ -288,6 +288,7 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
   const bool has_dsh = d->d_sh != nullptr;
   const bool has_delta = d->delta2 || d->delta3 || has_attr || has_dsh;  // 4 records per Gaussian
   D.V = has_delta ? 4 : 2;
+  D.affine_cov = d->affine_on_covariance != 0;
   D.delta = nullptr; D.g1v = nullptr; D.g2v = nullptr; D.opv = nullptr; D.d_sh = nullptr;
   for (int k = 0; k < 3; ++k) D.bg[k] = d->background[k];
   size_t off = 0;

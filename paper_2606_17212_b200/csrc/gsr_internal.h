@@ -16,6 +16,7 @@ constexpr int kMaxC = 4096;              // clusters (mask table lives in shared
 // ---- device scene: SoA of 16-byte words so that every warp load is 512 B contiguous
 struct DeviceScene {
   int32_t C, N, K, R, sh_degree;
+  int32_t affine_cov;  // != 0: Sigma_t = L Sigma L^T with L = the 3x3 part of A_c(t) (reading I4)
   int32_t V;      // projected records per Gaussian: 2 (no position residual levels) or 4 (delta2 / delta3 given)
   int32_t n_sh4;  // float4 words of SH coefficients per Gaussian = ceil(3K/4)
   int32_t n_qw;   // 32-bit words of int8 motion coefficients per Gaussian = ceil(3R/4)

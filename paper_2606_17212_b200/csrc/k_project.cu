@@ -203,6 +203,24 @@ __device__ __forceinline__ void store_record(Workspace& ws, uint32_t rid, const 
   ws.count[rid] = p.count;
 }
 
+// reading I4 (optional): Sigma_t = L Sigma L^T, L = the 3x3 part of A_c(t); binary32 in the written order of
+// Mm = L S (row a, column b), then Sigma_t[a][b] = Mm[a] . L[b]
+__device__ __forceinline__ void push_forward_cov(const float* A, const float* S6, float* out6) {
+  const float Sf[9] = {S6[0], S6[1], S6[2], S6[1], S6[3], S6[4], S6[2], S6[4], S6[5]};
+  float Mm[9];
+#pragma unroll
+  for (int a = 0; a < 3; ++a)
+#pragma unroll
+    for (int b = 0; b < 3; ++b)
+      Mm[3 * a + b] = __fmaf_rn(A[4 * a + 2], Sf[6 + b], __fmaf_rn(A[4 * a + 1], Sf[3 + b], __fmul_rn(A[4 * a + 0], Sf[b])));
+  int o = 0;
+#pragma unroll
+  for (int a = 0; a < 3; ++a)
+#pragma unroll
+    for (int b = a; b < 3; ++b)
+      out6[o++] = __fmaf_rn(Mm[3 * a + 2], A[4 * b + 2], __fmaf_rn(Mm[3 * a + 1], A[4 * b + 1], __fmul_rn(Mm[3 * a + 0], A[4 * b + 0])));
+}
+
 // K1: one thread per Gaussian; record id = 2*i + v.
 template <int K>
 __global__ void __launch_bounds__(128) k_project(DeviceScene sc, FrameParams fp, Workspace ws) {
@@ -243,10 +261,13 @@ __global__ void __launch_bounds__(128) k_project(DeviceScene sc, FrameParams fp,
   for (int k = 0; k < 3; ++k) muB[k] = __fmaf_rn(s_c, acc[k], p[k]);
 
   // ---- EWA projection of both geometries
+  float St[6];
+  const float* Sp = S6;
+  if (sc.affine_cov) { push_forward_cov(A, S6, St); Sp = St; }
   Proj pa;
   pa.count = 0;
-  if (lvl == 0) pa = project_variant(fp, p, S6, tau);
-  Proj pb = project_variant(fp, muB, S6, tau);
+  if (lvl == 0) pa = project_variant(fp, p, Sp, tau);
+  Proj pb = project_variant(fp, muB, Sp, tau);
 
   // ---- colour (continuous; fp32): rgb = max(0, 0.5 + sum_j Y_j(dir) * coef_j)
   float cA[3] = {0.f, 0.f, 0.f}, cB0[3] = {0.f, 0.f, 0.f}, cB1[3] = {0.f, 0.f, 0.f};
@@ -337,12 +358,16 @@ __global__ void __launch_bounds__(128) k_project4(DeviceScene sc, FrameParams fp
     if (v >= lvl) {
       if (sc.g1v) {  // scale / rotation / opacity refinements (reading I2): attributes of delivered depth v
         const float4 h1 = __ldg(sc.g1v + (size_t)v * sc.N + i), h2 = __ldg(sc.g2v + (size_t)v * sc.N + i);
-        const float Sv[6] = {h1.x, h1.y, h1.z, h2.x, h2.y, h2.z};
+        float Sv[6] = {h1.x, h1.y, h1.z, h2.x, h2.y, h2.z};
+        if (sc.affine_cov) { float Sx[6]; push_forward_cov(A, Sv, Sx); for (int k = 0; k < 6; ++k) Sv[k] = Sx[k]; }
         opv[v] = __ldg(sc.opv + (size_t)v * sc.N + i);
         tauv[v] = h1.w;
         pr[v] = project_variant(fp, mu[v], Sv, tauv[v]);
       } else {
-        pr[v] = project_variant(fp, mu[v], S6, tau);
+        float St[6];
+        const float* Sp = S6;
+        if (sc.affine_cov) { push_forward_cov(A, S6, St); Sp = St; }
+        pr[v] = project_variant(fp, mu[v], Sp, tau);
       }
     }
     any |= pr[v].count > 0;

@@ -30,7 +30,7 @@ class SceneDesc(C.Structure):
                 ("motion_q", C.c_void_p), ("A0", C.c_void_p), ("A1", C.c_void_p), ("motion_scale", C.c_void_p),
                 ("background", C.c_float * 3), ("delta2", C.c_void_p), ("delta3", C.c_void_p),
                 ("d_log_scale", C.c_void_p), ("d_quat", C.c_void_p), ("d_opacity_logit", C.c_void_p),
-                ("d_sh", C.c_void_p)]
+                ("d_sh", C.c_void_p), ("affine_on_covariance", C.c_int32)]
 
 
 class CameraC(C.Structure):
@@ -192,6 +192,7 @@ class Scene:
         for k, v in keep.items():
             setattr(d, k, v.ctypes.data)
         d.background[:] = [float(v) for v in np.asarray(sc.background, np.float32)]
+        d.affine_on_covariance = 1 if getattr(sc, "affine_on_covariance", False) else 0
         self.V = 2                                   # projected records per Gaussian
         # optional position residual levels of Eq. (1) and per-level scale / rotation / opacity refinements
         for name in ("delta2", "delta3", "d_log_scale", "d_quat", "d_opacity_logit", "d_sh"):

@@ -152,3 +152,40 @@ def test_attribute_refinements_alone_and_zero(gsr, torch_mod, oracle_mod):
     a, _, _, _ = _render(torch, gsr.Scene(wl.scene), cam, t, lv)
     b, _, _, _ = _render(torch, s0, cam, t, lv)
     assert torch.equal(a, b)
+
+
+@pytest.mark.parametrize("four", [False, True])
+def test_affine_push_forward_of_covariance(gsr, torch_mod, oracle_mod, four):
+    """Reading I4 (optional flag): projection bit-exact and pixels within tolerance with Sigma_t = L Sigma L^T,
+    on the two-record and on the four-record path; the flag really changes the footprints."""
+    import dataclasses
+    torch = torch_mod
+    wl = synth.scaled_object_workload(25, C=5, per_cluster=400.0, W=112, H=88, fov=40.0, n_frames=1, B=12)
+    cam, t = wl.frames[0]
+    lv = wl.levels[0]
+    sc = wl.scene
+    # a visible shear / scale in the affine, so that the push-forward matters
+    A0 = sc.A0.copy()
+    A0[:, 0, 1] += 0.3
+    A0[:, 1, 1] *= 1.4
+    sc = dataclasses.replace(sc, A0=A0, affine_on_covariance=True)
+    if four:
+        sc = synth.with_attribute_refinements(synth.with_position_residuals(sc, seed_cfg=25), seed_cfg=25)
+    scene = gsr.Scene(sc)
+    osc = oracle_mod.OracleScene(sc)
+    out, _, _, ws = _render(torch, scene, cam, t, lv)
+    P = scene.debug_projection(ws)
+    V = scene.V
+    for d in (0, 1, 3):
+        op = osc.project(cam, t, np.full(sc.C, d, np.int8))
+        v = d if V == 4 else (0 if d == 0 else 1)
+        rid = V * np.arange(sc.N) + v
+        m = op["valid"] == 1
+        assert np.array_equal(P["conic"][rid][m].view(np.uint32),
+                              np.stack([op["qa"], op["qb"], op["qc"]], 1)[m].view(np.uint32))
+        assert np.array_equal(P["radius"][rid][m], op["radius"][m]) and np.array_equal(P["rect"][rid][m], op["rect"][m])
+    o_img, _ = osc.render_batch(cam, t, lv)
+    assert np.abs(out.cpu().numpy() - o_img).max() <= PIX_TOL
+    off = gsr.Scene(dataclasses.replace(sc, affine_on_covariance=False))
+    out_off, _, _, _ = _render(torch, off, cam, t, lv)
+    assert not torch.equal(out_off, out)
