@@ -351,12 +351,12 @@ def run_ours(args):
                                "frac": sg / hbm_peak, "radix_passes": passes, "launches_per_frame": 5 + 3 * passes,
                                "note": "latency-bound at this key count (%d keys): many small dependent launches" % keys},
                   "share_of_step": (proj_ms + sort_ms) / ms}
-    tp = Path(ROOT / "profiles" / "traffic.json")
+    tp = Path(ROOT / "profiles" / "traffic.txt")     # ncu DRAM bytes per launch of this kernel (see the file header)
     if tp.exists():
-        try:
-            roofline["traffic"] = json.loads(tp.read_text()).get(wl.name)
-        except Exception:
-            pass
+        for ln in tp.read_text().splitlines():
+            f = ln.split()
+            if len(f) == 2 and not ln.startswith("#") and f[0] == wl.name:
+                roofline["traffic"] = int(f[1])
 
     # ---- CPU oracle on this box's cores, bounded sample of the same workload
     cpu = None
