@@ -322,6 +322,7 @@ def run_ours(args):
                 "alpha_evals_per_step": cnt[0] / args.steps, "state_updates_per_step": cnt[1] / args.steps,
                 "logical_pairs_per_step": cnt[2] / args.steps,
                 "literal_equiv_tflops": cnt[2] * FLOP_LITERAL / comp_s / 1e12 if comp_s > 0 else 0.0,
+                "literal_equiv_frac": (cnt[2] * FLOP_LITERAL / comp_s / 1e12 / peak_meas) if comp_s > 0 and peak_meas else None,
                 "image_write_gbs": B * H * W * 12 * args.steps / comp_s / 1e9 if comp_s > 0 else None}
     # ---- the memory-bound phases a1-a3 against the HBM roofline (algorithmic bytes per unit)
     K = (wl.scene.sh_degree + 1) ** 2
