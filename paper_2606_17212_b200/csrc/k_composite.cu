@@ -194,9 +194,6 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const 
     if (have) {
       const uint32_t rid = __ldg(a.vals + idx);
       g1 = __ldg(a.r1 + rid);
-      g0 = __ldg(a.r0 + rid);
-      c0 = __ldg(a.rc0 + rid);
-      c1 = __ldg(a.rc1 + rid);
       const uint32_t meta = __float_as_uint(g1.w);
       const uint32_t cls = meta >> 16;
       const uint16_t* t = s_tab + 4 * (meta & 0xFFFFu);
@@ -210,8 +207,14 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const 
         act = cls == 0 ? t[0] : (cls <= 2 ? t[1] : (cls == 3 ? t[2] : t[3]));
         res = cls == 0 ? 0u : t[3];
       }
-      // pixel-centre box of the record vs the eight 8x4 pixel blocks of the tile
-      wmask = record_block_mask(g0.x, g0.y, c0.w, c1.w, tx, ty);
+      // pixel-centre box of the record vs the eight 8x4 pixel blocks of the tile (records present in no slot
+      // of this CTA are not fetched any further)
+      if (act != 0) {
+        g0 = __ldg(a.r0 + rid);
+        c0 = __ldg(a.rc0 + rid);
+        c1 = __ldg(a.rc1 + rid);
+        wmask = record_block_mask(g0.x, g0.y, c0.w, c1.w, tx, ty);
+      }
     }
     // ordered compaction: the record keeps slot `tid` of the staging buffer; each 8x4 pixel block k gets
     // the ordered list s_list[k] of the slots whose box touches it (warp ballots + an 8x8 count table)
