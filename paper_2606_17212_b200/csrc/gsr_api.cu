@@ -84,6 +84,7 @@ size_t carve_workspace(Workspace* ws, void* base, int32_t N, int32_t C, int32_t 
   }
   w.hist = (uint32_t*)take(sizeof(uint32_t) * 256 * ((size_t)cap / kSortTileKeys + 2));
   w.tile_range = (uint2*)take(sizeof(uint2) * (size_t)tiles);
+  w.render_range = (uint2*)take(sizeof(uint2) * (size_t)tiles);
   w.state_counts = (long long*)take(sizeof(long long) * (size_t)(B > 0 ? B : 1));
   w.sse_part = (double*)take(sizeof(double) * (size_t)(B > 0 ? B : 1) * tiles);
   w.uorder = (uint32_t*)take(sizeof(uint32_t) * (size_t)(B > 0 ? B : 1) * tiles);
@@ -448,6 +449,7 @@ static int prepare_frame(const gsr_scene* scene, const gsr_camera* cam, float t,
   launch_project(s->d, *fp_out, *ws_out, st);                // a1 + a2
   if (ph >= 0) cudaEventRecord(g_ph[ph][1], st);
   launch_bin_and_sort(s->d, *fp_out, *ws_out, cap, st);      // a3
+  launch_tile_render_list(*fp_out, *ws_out, st);             // a3: per-tile lists without the sub-tile-culled records
   if (ph >= 0) cudaEventRecord(g_ph[ph][2], st);
   return GSR_OK;
 }

@@ -75,6 +75,8 @@ struct Workspace {
   uint32_t* vals[2];            // [cap] record id
   uint32_t* hist;         // [256 * n_sort_blocks]
   uint2* tile_range;      // [tiles] start,end into the sorted list
+  uint2* render_range;    // [tiles] start,end into the render list (vals[1]): the tile's records whose q <= tau
+                          // box touches a pixel of the tile, in list order (k_tile_render_list)
   long long* state_counts;  // [B]
   double* sse_part;       // [B * tiles] per-(state,tile) squared-error partials (fused distortion)
   uint32_t* uorder;       // [tiles * B] states sorted by their tile-restricted signature (k_tile_dedup)
@@ -124,6 +126,7 @@ void launch_composite(const DeviceScene& sc, const FrameParams& fp, Workspace& w
 void launch_composite_count(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, const int8_t* depth_rows,
                             int32_t B, unsigned long long* counts, cudaStream_t st);
 void count_launches(int n);
+void launch_tile_render_list(const FrameParams& fp, Workspace& ws, cudaStream_t st);
 bool launch_tile_dedup(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, const int8_t* depth_rows,
                        int32_t B, cudaStream_t st);
 void launch_distortion(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, double* part,

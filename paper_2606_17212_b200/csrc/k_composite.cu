@@ -489,8 +489,8 @@ static void launch_composite_S(const CompositeArgs& a, cudaStream_t st) {
 static CompositeArgs make_args(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, const int8_t* depth_rows,
                                int32_t B) {
   CompositeArgs a;
-  a.tile_range = ws.tile_range;
-  a.vals = ws.vals[0];
+  a.tile_range = ws.render_range;  // the render list: sorted superset list minus the sub-tile-culled records
+  a.vals = ws.vals[1];
   a.r0 = ws.r0; a.r1 = ws.r1; a.rc0 = ws.rc0; a.rc1 = ws.rc1;
   a.depth = depth_rows;
   a.B = B; a.C = sc.C;

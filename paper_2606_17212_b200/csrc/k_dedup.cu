@@ -41,10 +41,7 @@ __device__ __forceinline__ uint32_t class_sig(uint32_t bits, int d) {
 
 __global__ void __launch_bounds__(kDedupThreads) k_tile_dedup(const uint2* __restrict__ tile_range,
                                                               const uint32_t* __restrict__ vals,
-                                                              const float4* __restrict__ r0,
                                                               const float4* __restrict__ r1,
-                                                              const float4* __restrict__ rc0,
-                                                              const float4* __restrict__ rc1, int TX,
                                                               const int8_t* __restrict__ depth, int B, int C,
                                                               int Bp, uint32_t* __restrict__ order,
                                                               uint32_t* __restrict__ upos,
@@ -74,11 +71,7 @@ __global__ void __launch_bounds__(kDedupThreads) k_tile_dedup(const uint2* __res
   for (int k = tid; k < C; k += kDedupThreads) ccnt[k] = 0;
   __syncthreads();
   for (uint32_t i = rg.x + tid; i < rg.y; i += kDedupThreads) {
-    const uint32_t rid = vals[i];
-    // a record whose q <= tau box misses every pixel of the tile is dropped by the compositor's staging in
-    // every state: it must not distinguish signature classes (same predicate: record_block_mask)
-    const float4 g0 = r0[rid];
-    if (record_block_mask(g0.x, g0.y, rc0[rid].w, rc1[rid].w, tile % TX, tile / TX) == 0u) continue;
+    const uint32_t rid = vals[i];  // render list: sub-tile-culled records are already gone (k_tile_render_list)
     const uint32_t meta = __float_as_uint(r1[rid].w);
     const uint32_t c = meta & 0xFFFFu, cls = meta >> 16;
     const uint32_t bit = cls >= 16 ? (16u << (cls - 16)) : (cls == 0 ? 1u : (cls <= 2 ? 2u : (cls == 3 ? 4u : 8u)));
@@ -210,6 +203,56 @@ __global__ void __launch_bounds__(kDedupThreads) k_tile_dedup(const uint2* __res
   if (tid == 0) n_unique[tile] = s_run;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Render list: the tile's sorted superset list without the records whose conservative q <= tau box touches
+// no pixel of the tile — they contribute to no pixel in any state, and every one of the
+// ~B/S CTAs that composite the tile would otherwise fetch and drop them again.  Order is kept (ballot
+// compaction); the canonical key lists (vals[0], tile_range) are untouched.  One CTA per tile.
+__global__ void __launch_bounds__(kDedupThreads) k_tile_render_list(const uint2* __restrict__ tile_range,
+                                                                    const uint32_t* __restrict__ vals,
+                                                                    const float4* __restrict__ r0,
+                                                                    const float4* __restrict__ rc0,
+                                                                    const float4* __restrict__ rc1, int TX,
+                                                                    uint32_t* __restrict__ rvals,
+                                                                    uint2* __restrict__ render_range) {
+  __shared__ uint32_t s_cnt[8];
+  __shared__ uint32_t s_run;
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  const int tile = blockIdx.x;
+  const uint2 rg = tile_range[tile];
+  if (tid == 0) s_run = 0;
+  __syncthreads();
+  for (uint32_t base = rg.x; base < rg.y; base += kDedupThreads) {
+    const uint32_t i = base + tid;
+    uint32_t rid = 0;
+    bool keep = false;
+    if (i < rg.y) {
+      rid = vals[i];
+      const float4 g0 = r0[rid];
+      keep = record_block_mask(g0.x, g0.y, rc0[rid].w, rc1[rid].w, tile % TX, tile / TX) != 0u;
+    }
+    const uint32_t bal = __ballot_sync(0xffffffffu, keep);
+    if (lane == 0) s_cnt[w] = __popc(bal);
+    __syncthreads();
+    uint32_t woff = 0, tot = 0;
+    for (int q = 0; q < 8; ++q) {
+      if (q < w) woff += s_cnt[q];
+      tot += s_cnt[q];
+    }
+    if (keep) rvals[rg.x + s_run + woff + __popc(bal & ((1u << lane) - 1u))] = rid;
+    __syncthreads();
+    if (tid == 0) s_run += tot;
+    __syncthreads();
+  }
+  if (tid == 0) render_range[tile] = make_uint2(rg.x, rg.x + s_run);
+}
+
+void launch_tile_render_list(const FrameParams& fp, Workspace& ws, cudaStream_t st) {
+  k_tile_render_list<<<fp.TX * fp.TY, kDedupThreads, 0, st>>>(ws.tile_range, ws.vals[0], ws.r0, ws.rc0, ws.rc1, fp.TX,
+                                                             ws.vals[1], ws.render_range);
+  count_launches(1);
+}
+
 size_t dedup_smem_bytes(int B, int C, int* Bp_out) {
   int Bp = 2;
   while (Bp < B) Bp <<= 1;
@@ -228,7 +271,7 @@ bool launch_tile_dedup(const DeviceScene& sc, const FrameParams& fp, Workspace& 
     cudaFuncSetAttribute(k_tile_dedup, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     attr_set = true;
   }
-  k_tile_dedup<<<fp.TX * fp.TY, kDedupThreads, smem, st>>>(ws.tile_range, ws.vals[0], ws.r0, ws.r1, ws.rc0, ws.rc1, fp.TX, depth_rows, B, sc.C, Bp,
+  k_tile_dedup<<<fp.TX * fp.TY, kDedupThreads, smem, st>>>(ws.render_range, ws.vals[1], ws.r1, depth_rows, B, sc.C, Bp,
                                                           ws.uorder, ws.upos, ws.n_unique);
   count_launches(1);
   return true;
