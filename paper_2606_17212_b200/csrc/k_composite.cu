@@ -263,14 +263,16 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const 
 #pragma unroll
       for (int s = 0; s < S; ++s) walive |= (uint32_t)(__any_sync(0xffffffffu, T[s] > 0.0f) != 0) << s;
       if (walive == 0) break;
-      walive |= 0xFFFF0000u;  // keep the residual bits of the tag
       const uint32_t j1 = min(nb, j0 + 32u);
       for (uint32_t j = j0; j < j1; ++j) {
         const uint32_t addr = lds16(lbase + 2u * j);
-        const uint32_t tagw = lds32(addr + 28u) & walive;  // act | res << 16, dead slots masked out
-        if ((tagw & 0xFFFFu) == 0) continue;
+        const float4 hq = lds128(addr + 16u);  // {Cq, tau, -, act | res << 16}
+        const uint32_t tag = __float_as_uint(hq.w);
+        const uint32_t actl = tag & walive;  // slots that contain the record and are still alive
+        if (actl == 0) continue;
+        const uint32_t tagw = actl | (tag & 0xFFFF0000u);
         const float4 h0 = lds128(addr);
-        const float2 h1 = lds64f(addr + 16u);  // {Cq, tau}
+        const float2 h1 = make_float2(hq.x, hq.y);  // {Cq, tau}
         // spec-exact quadratic form: u = A dx; s = fma(B,dy,u); q = s dx; v = Cq dy; q = fma(v,dy,q)
         const float dx = __fsub_rn(h0.x, px);
         const float dy = __fsub_rn(h0.y, py);
