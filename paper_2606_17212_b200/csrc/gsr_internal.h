@@ -102,6 +102,46 @@ __device__ __forceinline__ uint32_t record_block_mask(float mx, float my, float 
   return m;
 }
 
+// Tighter version, evaluated once per frame per (tile, record) by k_tile_render_list: a block that passes the
+// box test is kept only if the MINIMUM of the quadratic form q over the block's rectangle of pixel centres can
+// pass the cut.  q is convex, so when the centre lies outside the rectangle the minimum sits on one of the four
+// edges, where q is a 1-D quadratic (closed-form minimiser, clamped to the edge).  The block is dropped iff
+// q_min > (max(tau, 0) + 0.01) (1 + m)^2 with the same m = min(1, 8e-6 kappa + 1e-3) as the box (DESIGN.md §4.6:
+// fp32 evaluation of q, here and in the compositor, is within ~3e-6 kappa relative); ill-conditioned forms
+// (kappa > 1e4) keep the box result.  (A, B, Cq) = (conic_a / 2, conic_b, conic_c / 2): q = (A dx + B dy) dx + Cq dy^2.
+__device__ __forceinline__ uint32_t record_block_mask_tight(float mx, float my, float A, float B, float Cq, float tau,
+                                                            float hx, float hy, int tx, int ty) {
+  uint32_t m = record_block_mask(mx, my, hx, hy, tx, ty);
+  const float det4 = 4.0f * A * Cq - B * B;  // 4 det(conic) > 0
+  if (m == 0u || !(det4 > 0.0f)) return m;
+  const float kappa = 4.0f * A * Cq / det4;
+  if (!(kappa <= 1e4f)) return m;
+  const float mm = 1.0f + fminf(1.0f, 8e-6f * kappa + 1e-3f);
+  const float thr = (fmaxf(tau, 0.0f) + 1e-2f) * mm * mm;
+  const float X0 = (float)(tx * kTile) + 0.5f, Y0 = (float)(ty * kTile) + 0.5f;
+  const float iA = 0.5f / A, iC = 0.5f / Cq;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    if (!((m >> k) & 1u)) continue;
+    const float bx = X0 + 8.0f * (k & 1), by = Y0 + 4.0f * (k >> 1);
+    // d = centre - pixel; over the block dx in [dx0, dx1], dy in [dy0, dy1]
+    const float dx0 = mx - (bx + 7.0f), dx1 = mx - bx, dy0 = my - (by + 3.0f), dy1 = my - by;
+    if (dx0 <= 0.0f && dx1 >= 0.0f && dy0 <= 0.0f && dy1 >= 0.0f) continue;  // centre inside: q_min = 0
+    float qmin = 3.4e38f;
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+      const float dx = e ? dx1 : dx0;                       // vertical edges: dx fixed, dy free
+      float dy = fminf(dy1, fmaxf(dy0, -(B * dx) * iC));
+      qmin = fminf(qmin, (A * dx + B * dy) * dx + Cq * dy * dy);
+      const float dyf = e ? dy1 : dy0;                      // horizontal edges: dy fixed, dx free
+      float dxs = fminf(dx1, fmaxf(dx0, -(B * dyf) * iA));
+      qmin = fminf(qmin, (A * dxs + B * dyf) * dxs + Cq * dyf * dyf);
+    }
+    if (qmin > thr) m &= ~(1u << k);
+  }
+  return m;
+}
+
 constexpr int kSortThreads = 256;
 constexpr int kSortItems = 4;
 constexpr int kSortTileKeys = kSortThreads * kSortItems;  // keys per block per pass

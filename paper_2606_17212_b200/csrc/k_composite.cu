@@ -30,6 +30,7 @@ namespace gsr {
 struct CompositeArgs {
   const uint2* tile_range;
   const uint32_t* vals;
+  const uint8_t* vmask;  // per render-list entry: the 8x4 blocks of the tile the record can contribute to
   const float4 *r0, *r1, *rc0, *rc1;
   const int8_t* depth;
   int32_t B, C, nsb;
@@ -207,13 +208,13 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const 
         act = cls == 0 ? t[0] : (cls <= 2 ? t[1] : (cls == 3 ? t[2] : t[3]));
         res = cls == 0 ? 0u : t[3];
       }
-      // pixel-centre box of the record vs the eight 8x4 pixel blocks of the tile (records present in no slot
-      // of this CTA are not fetched any further)
+      // which 8x4 blocks the record can contribute to was decided once per frame (k_tile_render_list: box, then
+      // the minimum of q over the block); records present in no slot of this CTA are not fetched any further
       if (act != 0) {
         g0 = __ldg(a.r0 + rid);
         c0 = __ldg(a.rc0 + rid);
         c1 = __ldg(a.rc1 + rid);
-        wmask = record_block_mask(g0.x, g0.y, c0.w, c1.w, tx, ty);
+        wmask = __ldg(a.vmask + idx);
       }
     }
     // ordered compaction: the record keeps slot `tid` of the staging buffer; each 8x4 pixel block k gets
@@ -493,6 +494,7 @@ static CompositeArgs make_args(const DeviceScene& sc, const FrameParams& fp, Wor
   CompositeArgs a;
   a.tile_range = ws.render_range;  // the render list: sorted superset list minus the sub-tile-culled records
   a.vals = ws.vals[1];
+  a.vmask = (const uint8_t*)ws.keys[1];
   a.r0 = ws.r0; a.r1 = ws.r1; a.rc0 = ws.rc0; a.rc1 = ws.rc1;
   a.depth = depth_rows;
   a.B = B; a.C = sc.C;

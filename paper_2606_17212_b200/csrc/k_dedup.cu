@@ -211,9 +211,11 @@ __global__ void __launch_bounds__(kDedupThreads) k_tile_dedup(const uint2* __res
 __global__ void __launch_bounds__(kDedupThreads) k_tile_render_list(const uint2* __restrict__ tile_range,
                                                                     const uint32_t* __restrict__ vals,
                                                                     const float4* __restrict__ r0,
+                                                                    const float4* __restrict__ r1,
                                                                     const float4* __restrict__ rc0,
                                                                     const float4* __restrict__ rc1, int TX,
                                                                     uint32_t* __restrict__ rvals,
+                                                                    uint8_t* __restrict__ rmask,
                                                                     uint2* __restrict__ render_range) {
   __shared__ uint32_t s_cnt[8];
   __shared__ uint32_t s_run;
@@ -225,12 +227,13 @@ __global__ void __launch_bounds__(kDedupThreads) k_tile_render_list(const uint2*
   for (uint32_t base = rg.x; base < rg.y; base += kDedupThreads) {
     const uint32_t i = base + tid;
     uint32_t rid = 0;
-    bool keep = false;
+    uint32_t bm = 0;
     if (i < rg.y) {
       rid = vals[i];
-      const float4 g0 = r0[rid];
-      keep = record_block_mask(g0.x, g0.y, rc0[rid].w, rc1[rid].w, tile % TX, tile / TX) != 0u;
+      const float4 g0 = r0[rid], g1 = r1[rid];
+      bm = record_block_mask_tight(g0.x, g0.y, g0.z, g0.w, g1.x, g1.z, rc0[rid].w, rc1[rid].w, tile % TX, tile / TX);
     }
+    const bool keep = bm != 0u;
     const uint32_t bal = __ballot_sync(0xffffffffu, keep);
     if (lane == 0) s_cnt[w] = __popc(bal);
     __syncthreads();
@@ -239,7 +242,11 @@ __global__ void __launch_bounds__(kDedupThreads) k_tile_render_list(const uint2*
       if (q < w) woff += s_cnt[q];
       tot += s_cnt[q];
     }
-    if (keep) rvals[rg.x + s_run + woff + __popc(bal & ((1u << lane) - 1u))] = rid;
+    if (keep) {
+      const uint32_t pos = rg.x + s_run + woff + __popc(bal & ((1u << lane) - 1u));
+      rvals[pos] = rid;
+      rmask[pos] = (uint8_t)bm;  // the 8x4 blocks whose pixels can pass the cut: the compositor's staging reads it
+    }
     __syncthreads();
     if (tid == 0) s_run += tot;
     __syncthreads();
@@ -248,8 +255,8 @@ __global__ void __launch_bounds__(kDedupThreads) k_tile_render_list(const uint2*
 }
 
 void launch_tile_render_list(const FrameParams& fp, Workspace& ws, cudaStream_t st) {
-  k_tile_render_list<<<fp.TX * fp.TY, kDedupThreads, 0, st>>>(ws.tile_range, ws.vals[0], ws.r0, ws.rc0, ws.rc1, fp.TX,
-                                                             ws.vals[1], ws.render_range);
+  k_tile_render_list<<<fp.TX * fp.TY, kDedupThreads, 0, st>>>(ws.tile_range, ws.vals[0], ws.r0, ws.r1, ws.rc0, ws.rc1,
+                                                             fp.TX, ws.vals[1], (uint8_t*)ws.keys[1], ws.render_range);
   count_launches(1);
 }
 
