@@ -334,7 +334,9 @@ int gsr_debug_closure(const gsr_scene* scene, const void* workspace, int8_t* dep
  * lists, same arithmetic, nothing written).  counts3 (host int64 [3]):
  *   [0] (pixel, record) pairs whose alpha was evaluated with at least one live present state,
  *   [1] (pixel, record, state) colour/transmittance updates on live present states,
- *   [2] logical (pixel, Gaussian, state) pairs E = sum_b E_b in the sense of the oracle. */
+ *   [2] logical (pixel, record, state) triples: like [1] without the cut and with every member state of a
+ *       dedup class counted — what a per-state rasteriser walking the same sub-tile-culled lists would evaluate
+ *       (a lower bound of the oracle's E = sum_b E_b, whose lists are the unculled 3-sigma tile lists). */
 int gsr_debug_pair_counts(const gsr_scene* scene, const void* workspace, int64_t* counts3, void* cuda_stream);
 
 /* Options: "state_block" = states composited per CTA (1, 4, 8 or 16; default 8) and "dedup" = 0/1 (tile-level
