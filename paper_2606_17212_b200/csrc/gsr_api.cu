@@ -449,8 +449,8 @@ static int prepare_frame(const gsr_scene* scene, const gsr_camera* cam, float t,
   launch_project(s->d, *fp_out, *ws_out, st);                // a1 + a2
   if (ph >= 0) cudaEventRecord(g_ph[ph][1], st);
   launch_bin_and_sort(s->d, *fp_out, *ws_out, cap, st);      // a3
-  launch_tile_render_list(*fp_out, *ws_out, st);             // a3: per-tile lists without the sub-tile-culled records
   if (ph >= 0) cudaEventRecord(g_ph[ph][2], st);
+  launch_tile_render_list(*fp_out, *ws_out, st);             // a4 preparation: sub-tile culling, once per frame
   return GSR_OK;
 }
 
