@@ -431,6 +431,31 @@ def test_subtile_culling_never_drops_a_contribution(gsr, torch_mod, oracle_mod):
     scene.close()
 
 
+@pytest.mark.parametrize("aspect", [1.5, 6.0, 40.0])
+def test_block_culling_by_minimum_of_q_keeps_every_contribution(gsr, torch_mod, oracle_mod, aspect):
+    """The once-per-frame per-block culling (minimum of q over the 8x4 block, k_tile_render_list) on its own
+    ground: moderately elongated, randomly rotated Gaussians (conditioning 2 .. ~2000, below the kappa cut-off of
+    the tight test) a few pixels wide, so that most footprints clip block corners and edges; strong and faint
+    opacities.  The oracle culls nothing: a wrongly dropped block would show as a >= 1/255 pixel error."""
+    rng = np.random.default_rng(int(aspect * 10))
+    n = 1500
+    means = np.stack([rng.uniform(-1.3, 1.3, n), rng.uniform(-1.0, 1.0, n), rng.uniform(-0.3, 0.3, n)], 1)
+    s_small = rng.uniform(0.01, 0.05, n)
+    scales = np.stack([s_small * aspect, s_small, s_small], 1)
+    logits = np.where(rng.uniform(size=n) < 0.5, 3.0, -4.5)        # o ~ 0.95 or ~ 0.011 (tau ~ 1.0)
+    sc, _ = tiny_scene(means, scales, quats=rng.standard_normal((n, 4)), logits=logits,
+                       colors=rng.uniform(0, 1, (n, 3)), levels=rng.integers(0, 4, n),
+                       clusters=rng.integers(0, 4, n), C=4, background=(0.0, 0.0, 0.0))
+    cam = axis_camera(W=176, H=136, f=120.0)
+    lv = synth.all_closed_states(4)[::9]
+    scene = gsr.Scene(sc)
+    osc = oracle_mod.OracleScene(sc)
+    out, _, _, _ = _render(torch_mod, scene, cam, 0.0, lv)
+    ref, _ = osc.render_batch(cam, 0.0, lv)
+    assert np.abs(out.cpu().numpy() - ref).max() <= PIX_TOL
+    scene.close()
+
+
 def test_full_size_cfg1_frame_sampled_states(gsr, torch_mod, oracle_mod):
     """configs[1] at full size in the launch configuration bench.py times (B = 256, default state block,
     dedup on, fused distortion): sampled states element by element against the oracle, I_b for all."""
