@@ -59,6 +59,50 @@ def test_argument_errors_without_gpu(libgsr):
     assert libgsr.gsr_distortion_workspace_bytes(2, 17, 33) == 256  # 2 states x (3x2 tiles) doubles, 256-aligned
 
 
+C_PROGRAM = r"""
+#include <stdio.h>
+#include <string.h>
+#include "gsr.h"
+int main(void) {
+  gsr_scene* scene = NULL;
+  gsr_scene_desc d;
+  memset(&d, 0, sizeof d);
+  if (gsr_load_scene(NULL, &scene) != GSR_E_INVALID_ARG) return 1;
+  if (gsr_load_scene(&d, &scene) != GSR_E_INVALID_ARG) return 2;       /* C = N = 0 */
+  if (strlen(gsr_last_error()) == 0) return 3;
+  if (gsr_workspace_bytes(NULL, NULL, 4) != 0) return 4;
+  if (gsr_render_states(NULL, NULL, 0.0f, NULL, 1, NULL, NULL, 0, NULL) != GSR_E_INVALID_ARG) return 5;
+  printf("%s\n", gsr_version());
+  return 0;
+}
+"""
+
+
+def test_header_is_plain_c99_and_a_c_program_links(tmp_path):
+    """include/gsr.h is the boundary: no C++ in it, usable from a C translation unit, and a plain C program
+    linked against libgsr.so reaches the argument checks (no GPU needed for those)."""
+    import shutil
+    import subprocess
+    from paper_2606_17212_b200 import build
+    if shutil.which("gcc") is None:
+        pytest.skip("no gcc")
+    inc = ROOT / "include"
+    r = subprocess.run(["gcc", "-std=c99", "-Wall", "-Wextra", "-pedantic", "-Werror", "-fsyntax-only", "-x", "c",
+                        str(inc / "gsr.h")], capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
+    lib = Path(build.build())
+    src = tmp_path / "abi.c"
+    src.write_text(C_PROGRAM)
+    exe = tmp_path / "abi"
+    r = subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", str(inc), str(src), "-o", str(exe),
+                        "-L", str(lib.parent), "-l:" + lib.name, "-Wl,-rpath," + str(lib.parent)],
+                       capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
+    r = subprocess.run([str(exe)], capture_output=True, text=True)
+    assert r.returncode == 0, (r.returncode, r.stderr)
+    assert "sm_100a" in r.stdout
+
+
 def test_binding_has_no_cpu_fallback():
     import torch
     from paper_2606_17212_b200 import gsr, synth
