@@ -265,13 +265,14 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const 
       for (int s = 0; s < S; ++s) walive |= (uint32_t)(__any_sync(0xffffffffu, T[s] > 0.0f) != 0) << s;
       if (walive == 0) break;
       const uint32_t j1 = min(nb, j0 + 32u);
+      const uint32_t keep = walive | 0xFFFF0000u;
+#pragma unroll 2
       for (uint32_t j = j0; j < j1; ++j) {
         const uint32_t addr = lds16(lbase + 2u * j);
         const float4 hq = lds128(addr + 16u);  // {Cq, tau, -, act | res << 16}
         const uint32_t tag = __float_as_uint(hq.w);
-        const uint32_t actl = tag & walive;  // slots that contain the record and are still alive
-        if (actl == 0) continue;
-        const uint32_t tagw = actl | (tag & 0xFFFF0000u);
+        const uint32_t tagw = tag & keep;  // slots that contain the record and are still alive | residual slots
+        if ((tagw & 0xFFFFu) == 0) continue;
         const float4 h0 = lds128(addr);
         const float2 h1 = make_float2(hq.x, hq.y);  // {Cq, tau}
         // spec-exact quadratic form: u = A dx; s = fma(B,dy,u); q = s dx; v = Cq dy; q = fma(v,dy,q)
@@ -297,7 +298,7 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const 
         }
         // (no warp vote here: after the per-block q_min culling of k_tile_render_list a record whose cut fails on
         //  all 32 pixels reaches this point in 0.3 % of the iterations; alpha = 0 makes the updates no-ops)
-        const float4 k0 = lds128(addr + 32u), k1 = lds128(addr + 48u);
+        const float4 k0 = lds128(addr + 32u);
         // q <= tau <= ln 255 on every lane that passes: no denormal range to guard, ex2.approx.ftz is enough
         float alpha = fminf(kAlphaCap, __fmul_rn(k0.w, ex2_approx_ftz(__fmul_rn(q, -1.4426950408889634f))));
         alpha = pass ? alpha : 0.0f;
@@ -310,6 +311,7 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const 
         for (int s = 0; s < S; ++s)
           if ((act0 >> s) & 1u) state_update(T[s], Cr[s], Cg[s], Cb[s], alpha, k0.x, k0.y, k0.z);
         if (act1 != 0) {
+          const float4 k1 = lds128(addr + 48u);
 #pragma unroll
           for (int s = 0; s < S; ++s)
             if ((act1 >> s) & 1u) state_update(T[s], Cr[s], Cg[s], Cb[s], alpha, k1.x, k1.y, k1.z);
