@@ -190,14 +190,17 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const 
     //      q <= tau region (conservative box from k_project) misses the tile
     const uint32_t idx = base + tid;
     const bool have = idx < rg.y;
-    uint32_t act = 0, res = 0, wmask = 0;
-    float4 g0 = make_float4(0, 0, 0, 0), g1 = g0, c0 = g0, c1 = g0;
+    // The record keeps slot `tid` of the staging buffer and is written there at once, so that only its block
+    // mask stays live across the ballots (the 32 state registers leave little room: profiles/r1j showed the
+    // staging spilling to local memory when the four float4 were carried through the compaction).
+    uint32_t wmask = 0;
     if (have) {
       const uint32_t rid = __ldg(a.vals + idx);
-      g1 = __ldg(a.r1 + rid);
+      const float4 g1 = __ldg(a.r1 + rid);
       const uint32_t meta = __float_as_uint(g1.w);
       const uint32_t cls = meta >> 16;
       const uint16_t* t = s_tab + 4 * (meta & 0xFFFFu);
+      uint32_t act, res;
       if (cls >= 16) {
         // 4-variant scene (reading I1): variant v = cls - 16 is present exactly at depth v; only v = 3 has the
         // SH residual colour (stored in both colour slots, so `res` is irrelevant: keep it 0)
@@ -210,27 +213,22 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const 
       }
       // which 8x4 blocks the record can contribute to was decided once per frame (k_tile_render_list: box, then
       // the minimum of q over the block); records present in no slot of this CTA are not fetched any further
-      if (act != 0) {
-        g0 = __ldg(a.r0 + rid);
-        c0 = __ldg(a.rc0 + rid);
-        c1 = __ldg(a.rc1 + rid);
-        wmask = __ldg(a.vmask + idx);
+      if (act != 0) wmask = __ldg(a.vmask + idx);
+      if (wmask != 0) {
+        s_rec[4 * tid + 0] = __ldg(a.r0 + rid);
+        s_rec[4 * tid + 1] = make_float4(g1.x, g1.z, 0.0f, __uint_as_float(act | (res << 16)));
+        const float4 c0 = __ldg(a.rc0 + rid);
+        s_rec[4 * tid + 2] = make_float4(c0.x, c0.y, c0.z, g1.y);
+        s_rec[4 * tid + 3] = __ldg(a.rc1 + rid);
       }
     }
-    // ordered compaction: the record keeps slot `tid` of the staging buffer; each 8x4 pixel block k gets
-    // the ordered list s_list[k] of the slots whose box touches it (warp ballots + an 8x8 count table)
-    if (!(act != 0)) wmask = 0;
-    uint32_t balk[8];
+    // ordered compaction: each 8x4 pixel block k gets the ordered list s_list[k] of the slots whose region
+    // touches it (warp ballots + an 8x8 count table); the ballots are re-taken after the barrier rather than
+    // kept in eight registers
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
-      balk[k] = __ballot_sync(0xffffffffu, (wmask >> k) & 1u);
-      if (lane == k) s_lcnt[k][w] = __popc(balk[k]);  // lane k publishes the count of list k
-    }
-    if (wmask != 0) {
-      s_rec[4 * tid + 0] = g0;
-      s_rec[4 * tid + 1] = make_float4(g1.x, g1.z, 0.0f, __uint_as_float(act | (res << 16)));
-      s_rec[4 * tid + 2] = make_float4(c0.x, c0.y, c0.z, g1.y);
-      s_rec[4 * tid + 3] = c1;
+      const uint32_t bal = __ballot_sync(0xffffffffu, (wmask >> k) & 1u);
+      if (lane == k) s_lcnt[k][w] = __popc(bal);  // lane k publishes the count of list k
     }
     __syncthreads();
     // exclusive offsets of the 8 source warps inside each of the 8 lists: lane l scans list k = l >> 2, source
@@ -252,7 +250,8 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const 
 #pragma unroll
       for (int k = 0; k < 8; ++k) {
         const uint32_t off = __shfl_sync(0xffffffffu, mine, 4 * k + (w >> 1));
-        if ((wmask >> k) & 1u) s_list[k][off + __popc(balk[k] & ((1u << lane) - 1u))] = (uint16_t)(rec_base + 64u * tid);
+        const uint32_t bal = __ballot_sync(0xffffffffu, (wmask >> k) & 1u);
+        if ((wmask >> k) & 1u) s_list[k][off + __popc(bal & ((1u << lane) - 1u))] = (uint16_t)(rec_base + 64u * tid);
       }
     }
     __syncthreads();
