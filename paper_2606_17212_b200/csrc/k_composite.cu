@@ -264,14 +264,13 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const 
       for (int s = 0; s < S; ++s) walive |= (uint32_t)(__any_sync(0xffffffffu, T[s] > 0.0f) != 0) << s;
       if (walive == 0) break;
       const uint32_t j1 = min(nb, j0 + 32u);
-      const uint32_t keep = walive | 0xFFFF0000u;
 #pragma unroll 2
       for (uint32_t j = j0; j < j1; ++j) {
         const uint32_t addr = lds16(lbase + 2u * j);
         const float4 hq = lds128(addr + 16u);  // {Cq, tau, -, act | res << 16}
         const uint32_t tag = __float_as_uint(hq.w);
-        const uint32_t tagw = tag & keep;  // slots that contain the record and are still alive | residual slots
-        if ((tagw & 0xFFFFu) == 0) continue;
+        const uint32_t actl = tag & walive;  // slots that contain the record and are still alive
+        if (actl == 0) continue;
         const float4 h0 = lds128(addr);
         const float2 h1 = make_float2(hq.x, hq.y);  // {Cq, tau}
         // spec-exact quadratic form: u = A dx; s = fma(B,dy,u); q = s dx; v = Cq dy; q = fma(v,dy,q)
@@ -287,7 +286,7 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const 
           int live = 0, logical = 0;
 #pragma unroll
           for (int s = 0; s < S; ++s) {
-            const bool l = ((tagw >> s) & 1u) && T[s] > 0.0f;
+            const bool l = ((actl >> s) & 1u) && T[s] > 0.0f;
             live += l;
             logical += l ? (a.n_unique ? (int)(s_mhi[s] - s_mlo[s]) : 1) : 0;  // every member of the class
           }
@@ -301,11 +300,11 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const 
         // q <= tau <= ln 255 on every lane that passes: no denormal range to guard, ex2.approx.ftz is enough
         float alpha = fminf(kAlphaCap, __fmul_rn(k0.w, ex2_approx_ftz(__fmul_rn(q, -1.4426950408889634f))));
         alpha = pass ? alpha : 0.0f;
-          // The tag is the same on every lane; the warp reduction only tells the compiler so (it lands in a
-        // uniform register), which turns every slot test below into a plain skip without reconvergence
-        // barriers.  Slots taking the plain colour first, then those taking the colour with the SH residual.
-        const uint32_t tagu = __reduce_or_sync(0xffffffffu, tagw);
-        const uint32_t act1 = tagu & (tagu >> 16), act0 = (tagu & 0xFFFFu) ^ act1;
+        // The tag is the same on every lane, and ptxas knows it: the list entry and the record are loaded from
+        // warp-uniform shared addresses, so the tag lands in a uniform register (R2UR) and every slot test below
+        // is a plain uniform skip (BRA.U) without reconvergence barriers — no warp reduction needed to say so.
+        // Slots taking the plain colour first, then those taking the colour with the SH residual.
+        const uint32_t act1 = actl & (tag >> 16), act0 = actl ^ act1;
 #pragma unroll
         for (int s = 0; s < S; ++s)
           if ((act0 >> s) & 1u) state_update(T[s], Cr[s], Cg[s], Cb[s], alpha, k0.x, k0.y, k0.z);
