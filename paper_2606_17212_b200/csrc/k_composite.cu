@@ -64,6 +64,12 @@ __device__ __forceinline__ uint32_t lds16(uint32_t addr) {
   asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(addr));
   return v;
 }
+__device__ __forceinline__ void sts32(uint32_t addr, uint32_t v) {
+  asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ void sts16(uint32_t addr, uint32_t v) {
+  asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"((unsigned short)v) : "memory");
+}
 __device__ __forceinline__ float2 lds64f(uint32_t addr) {
   float2 v;
   asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
@@ -172,6 +178,7 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const 
   uint32_t rec_base = (uint32_t)__cvta_generic_to_shared(s_rec);
   uint32_t lbase = (uint32_t)__cvta_generic_to_shared(&s_list[w][0]);
   asm volatile("" : "+r"(rec_base), "+r"(lbase));  // loop-invariant: keep them in registers
+  const uint32_t lcnt_base = (uint32_t)__cvta_generic_to_shared(s_lcnt);
   const float bg0 = a.bg[0], bg1 = a.bg[1], bg2 = a.bg[2];
 
   float T[S], Cr[S], Cg[S], Cb[S];
@@ -225,10 +232,14 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const 
     // ordered compaction: each 8x4 pixel block k gets the ordered list s_list[k] of the slots whose region
     // touches it (warp ballots + an 8x8 count table); the ballots are re-taken after the barrier rather than
     // kept in eight registers
+    {
+      uint32_t cnt = 0;
 #pragma unroll
-    for (int k = 0; k < 8; ++k) {
-      const uint32_t bal = __ballot_sync(0xffffffffu, (wmask >> k) & 1u);
-      if (lane == k) s_lcnt[k][w] = __popc(bal);  // lane k publishes the count of list k
+      for (int k = 0; k < 8; ++k) {
+        const uint32_t bal = __ballot_sync(0xffffffffu, (wmask >> k) & 1u);
+        cnt = lane == k ? __popc(bal) : cnt;
+      }
+      if (lane < 8) sts32(lcnt_base + 4u * (8u * lane + w), cnt);  // lane k publishes the count of list k
     }
     __syncthreads();
     // exclusive offsets of the 8 source warps inside each of the 8 lists: lane l scans list k = l >> 2, source
@@ -247,11 +258,13 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const 
       const uint32_t off0 = incl - (v0 + v1), off1 = off0 + v0;
       const uint32_t mine = (w & 1) ? off1 : off0;
       nb = __shfl_sync(0xffffffffu, incl, 4 * w + 3);
+      const uint32_t lt = (1u << lane) - 1u, mine_addr = rec_base + 64u * tid;
+      const uint32_t list0 = lbase - 2u * kTilePix * w;  // shared address of s_list[0][0]
 #pragma unroll
       for (int k = 0; k < 8; ++k) {
         const uint32_t off = __shfl_sync(0xffffffffu, mine, 4 * k + (w >> 1));
         const uint32_t bal = __ballot_sync(0xffffffffu, (wmask >> k) & 1u);
-        if ((wmask >> k) & 1u) s_list[k][off + __popc(bal & ((1u << lane) - 1u))] = (uint16_t)(rec_base + 64u * tid);
+        if ((wmask >> k) & 1u) sts16(list0 + 2u * (kTilePix * k + off + __popc(bal & lt)), mine_addr);
       }
     }
     __syncthreads();
