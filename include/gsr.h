@@ -94,7 +94,7 @@ typedef struct {
   float R_wc[9]; /* row-major */
   float t_wc[3];
   float fx, fy, cx, cy;
-  int32_t W, H;
+  int32_t W, H;  /* 1 <= W, H <= 65535 * 16 and 3 * W * H < 2^32 (else GSR_E_INVALID_ARG) */
   float znear; /* Gaussians with z <= znear are culled (0.2 in every config) */
 } gsr_camera;
 

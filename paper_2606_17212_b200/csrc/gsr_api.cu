@@ -102,7 +102,7 @@ struct SceneImpl {
 
 static bool camera_ok(const gsr_camera* cam) {
   return cam && cam->W > 0 && cam->H > 0 && cam->W <= 65535 * kTile && cam->H <= 65535 * kTile && cam->fx > 0 &&
-         cam->fy > 0;
+         cam->fy > 0 && 3ull * (unsigned long long)cam->W * (unsigned long long)cam->H < (1ull << 32);  // floats per image fit 32 bits
 }
 
 static void make_frame(const SceneImpl* s, const gsr_camera* cam, float t, FrameParams* fp) {

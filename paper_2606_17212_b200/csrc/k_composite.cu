@@ -353,32 +353,37 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const 
     const float* rp = a.ref + ((size_t)y * a.W + x) * 3;
     rr0 = __ldg(rp); rr1 = __ldg(rp + 1); rr2 = __ldg(rp + 2);
   }
-  double err[S];
+  // the squared errors stay in fp32 registers until the reduction (the widening is exact); the image pointer of
+  // a member state is one 32 x 32 -> 64-bit multiply-add from the pixel's pointer in image 0
+  float errf[S];
+  float* const pixp = a.out ? a.out + ((size_t)y * a.W + x) * 3 : nullptr;
+  const uint32_t img = (uint32_t)a.H * (uint32_t)a.W * 3u;  // floats per image (< 2^32: checked by camera_ok at the API)
+  const uint32_t* const mem = a.n_unique ? a.uorder + (size_t)tile * a.B : nullptr;
 #pragma unroll
   for (int s = 0; s < S; ++s) {
-    err[s] = 0.0;
     const float Tf = fabsf(T[s]);  // the transmittance the pixel ended with (frozen at termination)
     const float o0 = __fmaf_rn(Tf, bg0, Cr[s]);
     const float o1 = __fmaf_rn(Tf, bg1, Cg[s]);
     const float o2 = __fmaf_rn(Tf, bg2, Cb[s]);
     if (a.out && inside && s_rep[s] >= 0) {
-      const size_t pix = ((size_t)y * a.W + x) * 3;
-      const size_t img = (size_t)a.H * a.W * 3;
-      if (a.n_unique) {  // every state of the class receives the (identical) tile
-        const uint32_t* mem = a.uorder + (size_t)tile * a.B;
-        for (uint32_t i = s_mlo[s]; i < s_mhi[s]; ++i) {
-          float* op = a.out + (size_t)mem[i] * img + pix;
+      if (mem) {  // every state of the class receives the (identical) tile
+        const uint32_t hi = s_mhi[s];
+        for (uint32_t i = s_mlo[s]; i < hi; ++i) {
+          float* op = pixp + (size_t)__ldg(mem + i) * img;
           __stcs(op, o0); __stcs(op + 1, o1); __stcs(op + 2, o2);  // write-once stream: evict first
         }
       } else {
-        float* op = a.out + (size_t)s_rep[s] * img + pix;
+        float* op = pixp + (size_t)(uint32_t)s_rep[s] * img;
         __stcs(op, o0); __stcs(op + 1, o1); __stcs(op + 2, o2);  // write-once stream: evict first
       }
     }
-    if (a.ref) err[s] = inside ? (double)pixel_sq_err(o0, o1, o2, rr0, rr1, rr2) : 0.0;
+    errf[s] = (a.ref && inside) ? pixel_sq_err(o0, o1, o2, rr0, rr1, rr2) : 0.0f;
   }
   if (a.ref) {
     int slot;
+    double err[S];
+#pragma unroll
+    for (int s = 0; s < S; ++s) err[s] = (double)errf[s];
     const double tot = warp_sum_slots<S>(err, lane, slot);  // same bits as S plain butterflies (reduce.cuh)
     if ((lane & (32 / S - 1)) == 0) s_red[w][slot] = tot;
     __syncthreads();

@@ -349,6 +349,11 @@ def test_invalid_level_and_key_capacity_are_reported(gsr, torch_mod):
     with pytest.raises(gsr.GsrError):
         scene.render_states(cam, t, _dev_levels(torch_mod, wl.levels[0][:8]),
                             workspace=torch_mod.empty(1024, dtype=torch_mod.uint8, device="cuda"))
+    # an image whose float count does not fit 32 bits is refused up front (include/gsr.h: gsr_camera)
+    import dataclasses
+    huge = dataclasses.replace(cam, W=40000, H=40000)
+    with pytest.raises(gsr.GsrError):
+        scene.workspace_bytes(huge, 1)
     scene.close()
 
 
