@@ -420,7 +420,7 @@ def run_ours(args):
     # ---- CPU oracle on this box's cores, bounded sample of the same workload
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        n_s = min(args.ref_states, B)
+        n_s = min(4 * args.ref_states, B)          # cfg1: all 256 states of one frame, ~10 s of CPU work
         dt, cores = oracle_sample(wl, frame_of(args.warmup), n_s)
         cpu = {"value": n_s / dt, "unit": "states/s", "cores": cores, "kind": "oracle",
                "sample": f"first {n_s} of {B} states of frame {frame_of(args.warmup)} (+ full-state reference render and MSE/PSNR), {dt:.1f} s"}
