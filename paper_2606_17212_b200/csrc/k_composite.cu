@@ -274,7 +274,8 @@ __global__ void __launch_bounds__(kTilePix, (S <= 8 ? 5 : 2)) k_composite(const 
       // refresh the (warp, slot) liveness mask every 32 records
       uint32_t walive = 0;
 #pragma unroll
-      for (int s = 0; s < S; ++s) walive |= (uint32_t)(__any_sync(0xffffffffu, T[s] > 0.0f) != 0) << s;
+      for (int s = 0; s < S; ++s) walive |= (T[s] > 0.0f ? 1u : 0u) << s;
+      walive = __reduce_or_sync(0xffffffffu, walive);  // one warp reduction of the per-lane masks instead of S votes
       if (walive == 0) break;
       const uint32_t j1 = min(nb, j0 + 32u);
 #pragma unroll 2
