@@ -12,12 +12,15 @@
 // With tile-level dedup (k_dedup.cu) the S "states" of a CTA are S distinct signature classes of the
 // tile; the result is written to every member state of each class.
 //
-// Staging: the tile's records are gathered 256 at a time into shared memory (64 B each).  A warp owns
-// an 8x4 pixel block; per block an ordered list of the staged records whose conservative q <= tau box
-// (k_project) touches it and that are present in at least one of the S states is built with warp
-// ballots, so the hot loop only visits records that can matter to the warp.  Warp ballots also
-// (i) skip a record when no pixel of the warp passes the cut and (ii) retire (warp, state) pairs
-// whose 32 pixels have all terminated; the CTA leaves the list when every (pixel, state) is done.
+// Staging: the tile's render list (k_tile_render_list: the sorted superset list minus the records that can
+// reach no pixel of the tile, with an 8-bit mask of the 8x4 pixel blocks each record can contribute to) is
+// gathered 256 entries at a time into shared memory (64 B per record).  A warp owns an 8x4 pixel block; per
+// block an ordered list of the staged records whose mask has the block's bit and that are present in at
+// least one of the S states is built with warp ballots, so the hot loop only visits records that can matter
+// to the warp.  (warp, state) pairs whose 32 pixels have all terminated are retired every 32 records (one
+// warp reduction of per-lane liveness masks); the CTA leaves the list when every (pixel, state) is done.
+// The per-record tag (which slots contain the record, which take the residual colour) is warp-uniform and
+// ptxas knows it (uniform shared addresses), so the slot tests are uniform-datapath skips (ULOP3 + BRA.U).
 //
 // Determinism: the arithmetic applied to one (pixel, state) is a fixed sequence of explicitly
 // rounded fp32 operations that depends only on that state's row of `levels`; skipped work is
