@@ -330,6 +330,38 @@ def test_empty_batch_and_empty_scene(gsr, torch_mod):
     scene.close()
 
 
+@pytest.mark.parametrize("W,H", [(1, 1), (1, 37), (53, 1), (15, 17), (16, 16), (17, 15), (33, 2)])
+def test_degenerate_image_shapes(gsr, torch_mod, oracle_mod, W, H):
+    """One pixel, one-pixel-wide strips, one short of / exactly / one past a tile boundary: pixels, key counts
+    and the fused distortion against the oracle; batched == serial bitwise."""
+    rng = np.random.default_rng(100 * W + H)
+    n = 60
+    means = np.c_[rng.uniform(-0.4, 0.4, n), rng.uniform(-0.4, 0.4, n), rng.uniform(-0.3, 0.3, n)]
+    sc, _ = tiny_scene(means, rng.uniform(0.03, 0.15, (n, 3)), logits=rng.uniform(-1, 3, n),
+                       colors=rng.uniform(0.1, 0.9, (n, 3)), levels=rng.integers(0, 4, n),
+                       clusters=rng.integers(0, 3, n), C=3, background=(0.2, 0.1, 0.3))
+    cam = axis_camera(W=W, H=H, f=0.9 * max(W, H, 8), z0=3.0)
+    lv = synth.all_closed_states(3)[::5]                       # 25 of the 125 closed states
+    scene = gsr.Scene(sc)
+    osc = oracle_mod.OracleScene(sc)
+    full = np.full((1, 3), 3, np.int8)
+    ref, _, _, _ = _render(torch_mod, scene, cam, 0.0, full)
+    ref = ref[0].contiguous()
+    ws = scene.new_workspace(cam, lv.shape[0])
+    out, mse, psnr = scene.render_states(cam, 0.0, _dev_levels(torch_mod, lv), workspace=ws, ref=ref)
+    scene.status(ws)
+    o_img, o_cnt = osc.render_batch(cam, 0.0, lv)
+    o_ref, _ = osc.render(cam, 0.0, full[0])
+    assert np.array_equal(scene.debug_state_counts(ws, lv.shape[0]), o_cnt[:, 0])
+    assert np.abs(out.cpu().numpy() - o_img).max() <= PIX_TOL
+    _, o_psnr = oracle_mod.distortion(o_img, o_ref)
+    assert np.abs(psnr.cpu().numpy() - o_psnr).max() <= 1e-3
+    for b in (0, 7, lv.shape[0] - 1):
+        one, _, _, _ = _render(torch_mod, scene, cam, 0.0, lv[b:b + 1])
+        assert torch_mod.equal(one[0], out[b])
+    scene.close()
+
+
 def test_invalid_level_and_key_capacity_are_reported(gsr, torch_mod):
     wl = synth.workload_cfg0()
     cam, t = wl.frames[0]
