@@ -102,6 +102,26 @@ def test_projection_bit_exact_scaled_cfg1_sh3(gsr, torch_mod, oracle_mod):
         _check_projection(gsr, torch_mod, oracle_mod, wl.scene, cam, t)
 
 
+@pytest.mark.parametrize("sh_degree,R", [(0, 1), (1, 3), (2, 5), (3, 7), (2, 32)])
+def test_projection_every_sh_degree_and_ragged_basis_sizes(gsr, torch_mod, oracle_mod, sh_degree, R):
+    """SH degrees 0..3 and temporal-basis sizes whose 3R int8 coefficients do not fill whole 4-byte words
+    (and the maximum, GSR_MAX_R = 32): projection bit-exact, colours within 2e-6, at t != 0 so that every
+    basis term and the affine's A1 contribute."""
+    rng = np.random.default_rng(1000 * sh_degree + R)
+    n, Cn, K = 240, 4, (sh_degree + 1) ** 2
+    means = rng.uniform(-0.6, 0.6, (n, 3))
+    sh_base = rng.normal(0.0, 0.15, (n, K, 3))
+    sh_base[:, 0, :] += rng.uniform(-0.5, 1.2, (n, 3))
+    A1 = rng.normal(0.0, 0.03, (Cn, 3, 4))
+    sc, _ = tiny_scene(means, rng.uniform(0.02, 0.12, (n, 3)), quats=rng.normal(size=(n, 4)),
+                       logits=rng.uniform(-2, 3, n), levels=rng.integers(0, 4, n), clusters=rng.integers(0, Cn, n),
+                       C=Cn, sh_degree=sh_degree, R=R, A1=A1, motion_q=rng.integers(-127, 128, (n, R, 3)),
+                       motion_scale=rng.uniform(1e-4, 6e-4, Cn), sh_base=sh_base,
+                       sh_res=rng.normal(0.0, 0.05, (n, K, 3)))
+    cam = axis_camera(W=152, H=104, f=130.0, z0=3.5)
+    _check_projection(gsr, torch_mod, oracle_mod, sc, cam, 0.37)
+
+
 def test_projection_forward_facing_near_plane_and_offscreen(gsr, torch_mod, oracle_mod):
     # cfg2-like geometry at reduced size: Gaussians behind / near the camera and outside the frustum
     full = synth.scene_cfg2()
