@@ -51,7 +51,7 @@ typedef struct gsr_scene gsr_scene; /* opaque; owns the device copy of the scene
  * Gaussians are sorted by (cluster, level): group g = 4*c + l owns [group_off[g], group_off[g+1]).
  * "Every cluster produces one base completion group and three refinement groups". */
 typedef struct {
-  int32_t C;                  /* clusters                                                      */
+  int32_t C;                  /* clusters, 1..4096                                             */
   int32_t N;                  /* Gaussians                                                     */
   int32_t sh_degree;          /* 0..3; K = (sh_degree+1)^2 coefficients per channel            */
   int32_t R;                  /* temporal-basis terms of Eq. (1), 1..GSR_MAX_R                  */

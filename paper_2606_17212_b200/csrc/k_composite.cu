@@ -497,6 +497,12 @@ template <int S, bool COUNT>
 static void launch_composite_S(const CompositeArgs& a, cudaStream_t st) {
   const size_t smem = sizeof(uint16_t) * 4 * (size_t)a.C;
   const long long grid = (long long)a.tiles * a.nsb;
+  static bool attr_set = false;  // per instantiation: static + dynamic shared memory passes 48 KB from C ~ 3300 on
+  if (!attr_set) {
+    cudaFuncSetAttribute(k_composite<S, COUNT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                         (int)(sizeof(uint16_t) * 4 * kMaxC));
+    attr_set = true;
+  }
   int slot = -1;
   if (!COUNT && g_profile && g_ev_used < kMaxProfEvents) {
     slot = g_ev_used++;

@@ -382,6 +382,35 @@ def test_degenerate_image_shapes(gsr, torch_mod, oracle_mod, W, H):
     scene.close()
 
 
+def test_maximum_cluster_count(gsr, torch_mod, oracle_mod):
+    """C = 4096, the documented maximum (the per-CTA presence table then needs more than the default 48 KB of
+    shared memory): pixels against the oracle, with and without tile dedup; C = 4097 is refused at load."""
+    import dataclasses
+    rng = np.random.default_rng(4096)
+    Cn, n = 4096, 8192
+    sc, _ = tiny_scene(rng.uniform(-0.8, 0.8, (n, 3)), rng.uniform(0.02, 0.06, (n, 3)), logits=rng.uniform(-1, 3, n),
+                       colors=rng.uniform(0.1, 0.9, (n, 3)), levels=rng.integers(0, 4, n), clusters=np.arange(n) % Cn,
+                       C=Cn, background=(0.1, 0.1, 0.1))
+    cam = axis_camera(W=96, H=64, f=80.0, z0=3.0)
+    lv = synth.sample_levels(rng, 24, Cn)
+    scene = gsr.Scene(sc)
+    o_img, _ = oracle_mod.OracleScene(sc).render_batch(cam, 0.0, lv)
+    for dedup in (1, 0):
+        gsr.set_option("dedup", dedup)
+        try:
+            out, _, _, _ = _render(torch_mod, scene, cam, 0.0, lv)
+        finally:
+            gsr.set_option("dedup", 1)
+        assert np.abs(out.cpu().numpy() - o_img).max() <= PIX_TOL
+    scene.close()
+    off = np.concatenate([sc.group_off, np.full(4, sc.group_off[-1], np.int32)])
+    A = np.zeros((1, 3, 4), np.float32)
+    bad = dataclasses.replace(sc, C=Cn + 1, group_off=off, A0=np.concatenate([sc.A0, A]), A1=np.concatenate([sc.A1, A]),
+                              motion_scale=np.concatenate([sc.motion_scale, np.ones(1, np.float32)]))
+    with pytest.raises(gsr.GsrError):
+        gsr.Scene(bad)
+
+
 def test_invalid_level_and_key_capacity_are_reported(gsr, torch_mod):
     wl = synth.workload_cfg0()
     cam, t = wl.frames[0]
