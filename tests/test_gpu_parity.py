@@ -411,6 +411,46 @@ def test_maximum_cluster_count(gsr, torch_mod, oracle_mod):
         gsr.Scene(bad)
 
 
+def _limit_case(name):
+    rng = np.random.default_rng(17)
+    if name == "large_image_few_gaussians":          # 188 x 119 tiles: 16-bit tile indices, 2-3 radix passes on them
+        n = 50
+        sc, _ = tiny_scene(rng.uniform(-1, 1, (n, 3)), rng.uniform(0.05, 0.3, (n, 3)), logits=rng.uniform(-1, 3, n),
+                           colors=rng.uniform(0.1, 0.9, (n, 3)), levels=rng.integers(0, 4, n),
+                           clusters=rng.integers(0, 2, n), C=2, background=(0.2, 0.2, 0.2))
+        return sc, axis_camera(W=3000, H=1900, f=1800.0, z0=4.0), synth.all_closed_states(2)[[0, 12, 24]]
+    if name == "footprints_covering_every_tile":     # 3-sigma radius far larger than the image
+        n = 40
+        sc, _ = tiny_scene(rng.uniform(-0.5, 0.5, (n, 3)), rng.uniform(3.0, 20.0, (n, 3)), logits=rng.uniform(-3, 0, n),
+                           colors=rng.uniform(0.1, 0.9, (n, 3)), levels=rng.integers(0, 4, n),
+                           clusters=rng.integers(0, 3, n), C=3)
+        return sc, axis_camera(W=320, H=200, f=200.0, z0=30.0), synth.all_closed_states(3)[::9]
+    if name == "extreme_opacity_and_tiny_scales":    # tau = ln(255 o) from -24 to +5.5; Sigma' = dilation only
+        n = 300
+        sc, _ = tiny_scene(rng.uniform(-0.5, 0.5, (n, 3)), rng.choice([1e-6, 1e-3, 0.05], (n, 3)),
+                           logits=rng.choice([-30.0, -6.0, 0.0, 30.0], n), colors=rng.uniform(0.1, 0.9, (n, 3)),
+                           levels=rng.integers(0, 4, n), clusters=rng.integers(0, 3, n), C=3, background=(1, 1, 1))
+        return sc, axis_camera(W=160, H=120, f=150.0, z0=3.0), synth.all_closed_states(3)[::9]
+    n = 100                                          # everything_behind_or_outside: no key at all
+    sc, _ = tiny_scene(np.c_[rng.uniform(-50, 50, n), rng.uniform(-50, 50, n), rng.uniform(-20, -5, n)], 0.1,
+                       levels=rng.integers(0, 4, n), clusters=rng.integers(0, 2, n), C=2, background=(0.3, 0.6, 0.9))
+    return sc, axis_camera(W=64, H=48, f=60.0, z0=3.0), synth.all_closed_states(2)[::5]
+
+
+@pytest.mark.parametrize("name", ["large_image_few_gaussians", "footprints_covering_every_tile",
+                                  "extreme_opacity_and_tiny_scales", "everything_behind_or_outside"])
+def test_limit_cases(gsr, torch_mod, oracle_mod, name):
+    sc, cam, lv = _limit_case(name)
+    scene = gsr.Scene(sc)
+    out, _, _, ws = _render(torch_mod, scene, cam, 0.0, lv)
+    o_img, o_stats = oracle_mod.OracleScene(sc).render_batch(cam, 0.0, lv)
+    assert np.array_equal(scene.debug_state_counts(ws, lv.shape[0]), o_stats[:, 0])
+    assert np.abs(out.cpu().numpy() - o_img).max() <= PIX_TOL
+    if name == "everything_behind_or_outside":
+        assert scene.status(ws) == 0
+    scene.close()
+
+
 def test_invalid_level_and_key_capacity_are_reported(gsr, torch_mod):
     wl = synth.workload_cfg0()
     cam, t = wl.frames[0]
