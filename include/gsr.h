@@ -341,7 +341,9 @@ int gsr_debug_pair_counts(const gsr_scene* scene, const void* workspace, int64_t
 
 /* Options: "state_block" = states composited per CTA (1, 4, 8 or 16; default 8) and "dedup" = 0/1 (tile-level
  * state dedup, default 1) — results do not depend on either (bitwise); "profile" = 1 records CUDA events around
- * every compositing-kernel launch and around the projection and binning + sort phases of every frame. */
+ * every compositing-kernel launch and around the projection and binning + sort phases of every frame (a
+ * measurement aid: call the library from ONE host thread while it is on).  Everything else may be called from
+ * several host threads at once, each with its own stream and workspace (tests/test_gpu_streams.py). */
 int gsr_set_option(const char* name, int32_t value);
 
 /* Sum of the compositing kernel's durations (ms, CUDA events on its launch stream) and the number

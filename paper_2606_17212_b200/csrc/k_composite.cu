@@ -25,6 +25,8 @@
 // Determinism: the arithmetic applied to one (pixel, state) is a fixed sequence of explicitly
 // rounded fp32 operations that depends only on that state's row of `levels`; skipped work is
 // exactly the work that would have been a no-op.  Hence batched == serial bitwise (tests).
+#include <atomic>
+
 #include "gsr_internal.h"
 #include "reduce.cuh"
 
@@ -467,9 +469,9 @@ void launch_distortion(const float* imgs, const float* ref, int32_t B, int32_t H
 
 // ------------------------------------------------------------------------------------------------
 // launch bookkeeping: kernel-launch counter and optional CUDA-event timing of the compositing kernel
-static unsigned long long g_launches = 0;
-void count_launches(int n) { g_launches += (unsigned long long)n; }
-unsigned long long launches_total() { return g_launches; }
+static std::atomic<unsigned long long> g_launches{0};  // calls may come from several host threads (one stream each)
+void count_launches(int n) { g_launches.fetch_add((unsigned long long)n, std::memory_order_relaxed); }
+unsigned long long launches_total() { return g_launches.load(std::memory_order_relaxed); }
 
 int g_state_block = 8;  // S; set through gsr_set_option for experiments (1, 4, 8, 16)
 int g_dedup = 1;        // gsr_set_option("dedup", 0/1): tile-level state dedup
