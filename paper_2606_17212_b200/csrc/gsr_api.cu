@@ -86,7 +86,10 @@ size_t carve_workspace(Workspace* ws, void* base, int32_t N, int32_t C, int32_t 
   w.tile_range = (uint2*)take(sizeof(uint2) * (size_t)tiles);
   w.render_range = (uint2*)take(sizeof(uint2) * (size_t)tiles);
   w.state_counts = (long long*)take(sizeof(long long) * (size_t)(B > 0 ? B : 1));
-  w.sse_part = (double*)take(sizeof(double) * (size_t)(B > 0 ? B : 1) * tiles);
+  w.sse_blk = (double*)take(sizeof(double) * (size_t)(B > 0 ? B : 1) * tiles * 8);
+  w.rec = (float4*)take(sizeof(float4) * 4 * n_rec);
+  w.qlist = (uint2*)take(sizeof(uint2) * 4 * (size_t)cap);
+  w.qrange = (uint2*)take(sizeof(uint2) * 4 * (size_t)tiles);
   w.uorder = (uint32_t*)take(sizeof(uint32_t) * (size_t)(B > 0 ? B : 1) * tiles);
   w.upos = (uint32_t*)take(sizeof(uint32_t) * (size_t)(B > 0 ? B : 1) * tiles);
   w.n_unique = (uint32_t*)take(sizeof(uint32_t) * (size_t)tiles);
@@ -165,7 +168,7 @@ const char* gsr_last_error(void) { return g_err; }
 const char* gsr_version(void) { return "gsr 0.1 sm_100a"; }
 
 int gsr_set_option(const char* name, int value) {
-  if (name && strcmp(name, "state_block") == 0 && (value == 1 || value == 4 || value == 8 || value == 16)) {
+  if (name && strcmp(name, "state_block") == 0 && (value == 0 || value == 1 || (value >= 4 && value <= 8) || value == 16)) {
     g_state_block = value;
     return GSR_OK;
   }
@@ -451,6 +454,7 @@ static int prepare_frame(const gsr_scene* scene, const gsr_camera* cam, float t,
   launch_bin_and_sort(s->d, *fp_out, *ws_out, cap, st);      // a3
   if (ph >= 0) cudaEventRecord(g_ph[ph][2], st);
   launch_tile_render_list(*fp_out, *ws_out, st);             // a4 preparation: sub-tile culling, once per frame
+  launch_pack_records(s->d, *fp_out, *ws_out, st);
   return GSR_OK;
 }
 

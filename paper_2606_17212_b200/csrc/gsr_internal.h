@@ -78,7 +78,10 @@ struct Workspace {
   uint2* render_range;    // [tiles] start,end into the render list (vals[1]): the tile's records whose q <= tau
                           // box touches a pixel of the tile, in list order (k_tile_render_list)
   long long* state_counts;  // [B]
-  double* sse_part;       // [B * tiles] per-(state,tile) squared-error partials (fused distortion)
+  double* sse_blk;        // [B * tiles * 8] per-(state,tile,8x4 block) squared-error partials (fused distortion)
+  float4* rec;            // [4 * 2N] packed 64-byte records for the quadrant compositor (k_pack_records)
+  uint2* qlist;           // [4 * cap] per-(tile, quadrant) render lists of {record id, meta} (k_tile_render_list)
+  uint2* qrange;          // [tiles * 4] start, end into qlist
   uint32_t* uorder;       // [tiles * B] states sorted by their tile-restricted signature (k_tile_dedup)
   uint32_t* upos;         // [tiles * B] upos[tile*B + u] = index in uorder of the first member of class u
   uint32_t* n_unique;     // [tiles] number of distinct signatures
@@ -167,6 +170,11 @@ void launch_composite_count(const DeviceScene& sc, const FrameParams& fp, Worksp
                             int32_t B, unsigned long long* counts, cudaStream_t st);
 void count_launches(int n);
 void launch_tile_render_list(const FrameParams& fp, Workspace& ws, cudaStream_t st);
+void launch_pack_records(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, cudaStream_t st);
+struct CompositeArgs;
+void launch_composite_q(const CompositeArgs& a, int S, bool count, cudaStream_t st);
+void launch_distortion_finalize_blk(const double* blk, int32_t B, int32_t tiles, int64_t n_values, double* mse,
+                                    float* psnr, cudaStream_t st);
 bool launch_tile_dedup(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, const int8_t* depth_rows,
                        int32_t B, cudaStream_t st);
 void launch_distortion(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, double* part,
