@@ -17,6 +17,10 @@ import numpy as np
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "gsr_oracle.c"
 _LIB = _HERE / "libgsr_oracle.so"
+# GSR_ORACLE_SANITIZE=1 (tests/test_oracle_sanitized.py): the same source under -fsanitize=address,undefined, as a
+# separate library; the process must then run with libasan preloaded
+if os.environ.get("GSR_ORACLE_SANITIZE") == "1":
+    _LIB = _HERE / "libgsr_oracle_san.so"
 
 CFLAGS = ["-O2", "-ffp-contract=off", "-fno-fast-math", "-mfma", "-fopenmp", "-shared", "-fPIC", "-std=c11",
           "-D_GNU_SOURCE", "-Wall"]
@@ -26,7 +30,8 @@ def build(force: bool = False) -> Path:
     """Compile the oracle with gcc (no CUDA involved)."""
     if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
         tmp = _LIB.with_suffix(f".tmp{os.getpid()}.so")
-        subprocess.check_call(["gcc", *CFLAGS, str(_SRC), "-o", str(tmp), "-lm"])
+        extra = ["-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-g"] if _LIB.name.endswith("_san.so") else []
+        subprocess.check_call(["gcc", *CFLAGS, *extra, str(_SRC), "-o", str(tmp), "-lm"])
         os.replace(tmp, _LIB)
     return _LIB
 

@@ -675,3 +675,108 @@ def test_p20_affine_push_forward_of_covariance(oracle_mod):
     assert p_on["cov2d"][0][0] == pytest.approx(p_off["cov2d"][0][2], rel=1e-5)
     assert p_on["cov2d"][0][2] == pytest.approx(p_off["cov2d"][0][0], rel=1e-5)
     assert abs(p_on["cov2d"][0][1]) < 1e-4
+
+
+# ------------------------------------------------------------------------------------------ P21-P24
+# Pins of four constants / conventions of readings A9 and A11 that no pin above exercises (each chosen so that the
+# nearest plausible mistake fails it): the SH view direction, the alpha cap, the Jacobian clamp, the lambda floor.
+def pin_scene_sh_view_direction():
+    """One Gaussian off the optical axis, SH degree 1 with one pure degree-1 coefficient per channel (R on the x
+    term, G on the y term, B on the z term), seen by a camera whose R_wc and t_wc are both non-trivial, so that
+    -R^T t (the camera centre) differs from -R t."""
+    eye = np.array([1.5, -2.0, -3.0])
+    R, tw = synth.look_at(eye, target=(0.2, 0.1, 0.3))
+    cam = synth.make_camera(R, tw, 96, 80, 90.0)
+    mu = np.array([0.5, 0.4, 0.6])
+    k = 0.6
+    sh = np.zeros((1, 4, 3))
+    sh[0, 3, 0] = k          # basis order (1; y, z, x): index 3 is the x term
+    sh[0, 1, 1] = k          # index 1 is the y term
+    sh[0, 2, 2] = k          # index 2 is the z term
+    scn, _ = tiny_scene([mu], 0.05, sh_degree=1, sh_base=sh)
+    return scn, cam, eye, mu, k
+
+
+def test_p21_sh_view_direction_is_from_the_camera_centre(oracle_mod):
+    scn, cam, eye, mu, k = pin_scene_sh_view_direction()
+    p = oracle_mod.OracleScene(scn).project(cam, 0.0, np.zeros(1, np.int8))[0]
+    assert p["valid"] == 1
+    d = mu.astype(np.float32).astype(np.float64) - eye        # Gaussian minus the camera position given to look_at
+    d /= np.linalg.norm(d)
+    c1 = np.sqrt(3.0 / (4.0 * np.pi))                         # degree-1 constant of the orthonormal real basis
+    expect = 0.5 + c1 * k * d                                 # channel R <- x, G <- y, B <- z
+    assert np.all(expect > 0.05)                              # away from the clamp at 0
+    assert np.abs(p["rgb"] - expect).max() < 2e-6             # eye is exact only to the fp32 rounding of t_wc
+    # what the two nearest mistakes would give is far away: centre = -R t, and the direction reversed
+    Rd, td = cam.R_wc.astype(np.float64), cam.t_wc.astype(np.float64)
+    wrong = mu - (-(Rd @ td))
+    wrong /= np.linalg.norm(wrong)
+    assert np.abs(0.5 + c1 * k * wrong - expect).max() > 0.05
+    assert np.abs((0.5 - c1 * k * d) - expect).max() > 0.05
+
+
+def pin_scene_alpha_cap(bg):
+    col = (0.8, 0.3, 0.6)
+    scn, _ = tiny_scene([[0, 0, 0]], 0.2, logits=8.0, colors=col, background=bg)      # o = 0.99966 > 0.99
+    cam = axis_camera(64, 64, 100.0, 4.0, cx=32.5, cy=32.5)                           # pixel (32,32) centred on the axis
+    return scn, cam, col
+
+
+@pytest.mark.parametrize("bg", [(0.0, 0.0, 0.0), (1.0, 1.0, 1.0)])
+def test_p22_alpha_is_capped_at_0_99(oracle_mod, bg):
+    scn, cam, col = pin_scene_alpha_cap(bg)
+    sc = oracle_mod.OracleScene(scn)
+    for brute in (False, True):
+        img, _ = sc.render(cam, 0.0, np.zeros(1, np.int8), brute_force=brute)
+        # q = 0 at the centre pixel: alpha = min(0.99, 0.99966) = 0.99; T' = 0.01 >= 1e-4, so it is added
+        expect = 0.99 * np.array(col) + 0.01 * np.array(bg)
+        assert np.abs(img[32, 32] - expect).max() < 1e-6
+        # uncapped (0.99966) or capped at 0.999 the pixel would move by > 3e-3 times |c - bg|
+        assert np.abs((0.999 * np.array(col) + 0.001 * np.array(bg)) - expect).max() > 1e-3
+
+
+def pin_scene_jacobian_clamp():
+    """A large isotropic Gaussian at x/z = 2 lim_x (lim_x = 1.3 (W/2)/fx), in front of the near plane; it is big
+    enough (3 sigma' ~ 59 px) for its footprint to reach the screen, so the record is valid."""
+    W, H, f, z = 64, 64, 50.0, 4.0
+    lim = 1.3 * 0.5 * W / f
+    s = 1.2
+    scn, _ = tiny_scene([[2.0 * lim * z, 0.0, 0.0]], s)
+    return scn, axis_camera(W, H, f, z), lim, s, f, z
+
+
+def test_p23_jacobian_uses_the_clamped_point(oracle_mod):
+    scn, cam, lim, s, f, z = pin_scene_jacobian_clamp()
+    p = oracle_mod.OracleScene(scn).project(cam, 0.0, np.zeros(1, np.int8))[0]
+    assert p["valid"] == 1
+    x = float(np.float32(2.0 * lim * z))
+
+    def cov(xt):       # Sigma' = s^2 J J^T + 0.3 I with J = [[f/z, 0, -f xt/z^2], [0, f/z, 0]]  (R_wc = I, Sigma = s^2 I)
+        J = np.array([[f / z, 0.0, -f * xt / z ** 2], [0.0, f / z, 0.0]])
+        return s * s * J @ J.T + 0.3 * np.eye(2)
+    clamped, unclamped = cov(lim * z), cov(x)
+    assert unclamped[0, 0] > 2.0 * clamped[0, 0]                       # the two readings are far apart
+    assert np.allclose(p["cov2d"], [clamped[0, 0], clamped[0, 1], clamped[1, 1]], rtol=2e-5)
+    # the 2-D mean is NOT clamped: it sits at cx + f x / z
+    assert abs(p["mx"] - (cam.cx + f * x / z)) < 1e-3
+    # a clamp at 1.0 lim instead of 1.3 lim: lim_x = 0.64 gives a visibly different Sigma'_00
+    wrong = cov((lim / 1.3) * z)
+    assert abs(wrong[0, 0] - clamped[0, 0]) > 0.1 * clamped[0, 0]
+
+
+def pin_scene_lambda_floor():
+    f, z0 = 100.0, 4.0
+    s = np.sqrt(1.4) * z0 / f        # sigma'^2 = 1.4 + 0.3 = 1.7, isotropic: mid^2 - det = 0 < 0.1
+    scn, _ = tiny_scene([[0, 0, 0]], s)
+    return scn, axis_camera(128, 128, f, z0)
+
+
+def test_p24_lambda_floor_sets_the_radius(oracle_mod):
+    scn, cam = pin_scene_lambda_floor()
+    p = oracle_mod.OracleScene(scn).project(cam, 0.0, np.zeros(1, np.int8))[0]
+    # by hand: lambda = 1.7 + sqrt(0.1) = 2.0162 ; 3 sqrt(lambda) = 4.2598 -> radius 5
+    # without the floor: 3 sqrt(1.7) = 3.9115 -> radius 4
+    assert np.ceil(3 * np.sqrt(1.7)) == 4 and np.ceil(3 * np.sqrt(1.7 + np.sqrt(0.1))) == 5
+    assert p["radius"] == 5
+    # rectangle from radius 5 around (64, 64): floor(59/16) = 3 .. floor((69+15)/16) = 5
+    assert p["rect"].tolist() == [3, 3, 5, 5]
