@@ -157,6 +157,13 @@ int gsr_render_states_vs_full(const gsr_scene* scene, const gsr_camera* cam, flo
  * receives the number of (tile, depth, record) keys the frame produced. */
 int gsr_workspace_status(const void* workspace, int64_t* keys_needed, void* cuda_stream);
 
+/* Index arrays given to the device-pointer helpers below (a send order, the pair lists of gsr_group_utility, the
+ * prefix pairs of gsr_prefix_monotonicity) are range-checked ON THE DEVICE: an entry out of range is skipped —
+ * an invalid group of a send order sends nothing and ends a frontier walk, an invalid pair belongs to no group
+ * and has zero difference — and latched in a per-device error word.  gsr_index_status synchronises
+ * `cuda_stream`, reads and clears that word: GSR_OK, or GSR_E_INVALID_ARG with the kind in gsr_last_error(). */
+int gsr_index_status(void* cuda_stream);
+
 /* ------------------------------------------------------------------------------------------------
  * gsr_distortion — north_star (5), DESIGN.md §3.6.  Per state b: MSE_b = sum((img_b - ref)^2)/(3HW)
  * accumulated in double with a fixed reduction tree; PSNR_b = -10 log10(max(MSE_b, 1e-10)).
@@ -171,10 +178,16 @@ int gsr_distortion(const float* imgs, const float* ref, int32_t B, int32_t H, in
  *   mse dev double [B], psnr_db dev fp32 [B]: distortions of a batch.
  *   idx_without[p], idx_with[p] (dev int32 [n_pairs]): the states m and m u g of pair p;
  *   group_id[p] in [0, G).  out dev gsr_utility [G].  delta_mse / delta_db: dev double [n_pairs] or NULL.
- * Asynchronous; one CTA per group, fixed summation order (deterministic). */
+ * Asynchronous; one CTA per group, fixed summation order (deterministic).
+ * Range errors (see gsr_index_status): a group id outside [0, G) or a negative state index.  The call has no
+ * B; gsr_group_utility_b is the same call with the number of states B behind mse / psnr_db, so that state
+ * indices >= B are refused too (the Python binding and gsr_utility_frame_host use it). */
 int gsr_group_utility(const double* mse, const float* psnr_db, const int32_t* idx_without,
                       const int32_t* idx_with, const int32_t* group_id, int32_t n_pairs, int32_t G,
                       gsr_utility* out, double* delta_mse, double* delta_db, void* cuda_stream);
+int gsr_group_utility_b(const double* mse, const float* psnr_db, int32_t B, const int32_t* idx_without,
+                        const int32_t* idx_with, const int32_t* group_id, int32_t n_pairs, int32_t G,
+                        gsr_utility* out, double* delta_mse, double* delta_db, void* cuda_stream);
 
 /* ------------------------------------------------------------------------------------------------
  * gsr_close_levels — dependency closure, PAPER.md:185 ("A cluster-layer is usable only when all
@@ -242,7 +255,9 @@ int gsr_best_state_under_budget(const float* psnr_db, const int64_t* state_bytes
  *   values: double [n] (dtype 0) or float [n] (dtype 1); out: gsr_risk [1].
  * gsr_prefix_monotonicity: "M penalizes quality regressions as a prefix grows" (reading G4):
  *   M = sum_p max(0, d[idx_next[p]] - d[idx_prev[p]]), violations = #{p : d[next] > d[prev]}.
- *   d double [.]; idx_prev, idx_next int32 [n_pairs]; m_out double [1]; violations int32 [1] (either may be NULL). */
+ *   d double [.]; idx_prev, idx_next int32 [n_pairs]; m_out double [1]; violations int32 [1] (either may be NULL).
+ *   gsr_prefix_monotonicity_n takes the length n of d and refuses indices >= n as well as negative ones
+ *   (gsr_index_status); a refused pair contributes nothing. */
 typedef struct {
   double mean, cvar, quantile, worst, count;
 } gsr_risk;
@@ -254,6 +269,8 @@ int gsr_risk_reduce(const void* values, int32_t dtype, int32_t n, double alpha, 
                     void* cuda_stream);
 int gsr_prefix_monotonicity(const double* d, const int32_t* idx_prev, const int32_t* idx_next, int32_t n_pairs,
                             double* m_out, int32_t* violations, void* cuda_stream);
+int gsr_prefix_monotonicity_n(const double* d, int32_t n, const int32_t* idx_prev, const int32_t* idx_next,
+                              int32_t n_pairs, double* m_out, int32_t* violations, void* cuda_stream);
 
 /* ------------------------------------------------------------------------------------------------
  * gsr_sample_delivery — the step before the hot path: "A training world samples capacity, RTT, display
@@ -270,7 +287,8 @@ int gsr_prefix_monotonicity(const double* d, const int32_t* idx_prev, const int3
  * IID drop, the GE transition, the GE drop and (packet 0) the initial state; an event of probability p happens
  * iff x < floor(p * 2^32).  The result for a world depends only on (seed, world0 + w): sampling a batch in
  * pieces gives the same masks.  Bit-exact against the oracle.
- *   raw_bytes dev int64 [4C]; order dev int32 [4C] (a permutation); model: host; packet_budget dev int32 [W] or
+ *   raw_bytes dev int64 [4C]; order dev int32 [4C] (a permutation of 0..4C-1; an entry outside that range sends
+ *   nothing and is reported by gsr_index_status); model: host; packet_budget dev int32 [W] or
  *   NULL; mask dev uint8 [W,C]; levels dev int8 [W,C] or NULL (feeds gsr_render_states directly);
  *   workspace dev >= gsr_delivery_workspace_bytes(C).  Asynchronous. */
 typedef struct {
@@ -286,7 +304,8 @@ int gsr_sample_delivery(const int64_t* raw_bytes, const int32_t* order, int32_t 
  * One-call convenience with HOST buffers (used for the end-to-end measurement): uploads `levels`
  * and the pair lists, renders the full state (all depths 3) as the reference, renders the batch with
  * fused distortion, aggregates utilities, and copies mse / psnr_db / util back.  Synchronous.
- *   levels host int8 [B,C]; idx_without, idx_with, group_id host int32 [n_pairs] (n_pairs may be 0);
+ *   levels host int8 [B,C]; idx_without, idx_with, group_id host int32 [n_pairs] (n_pairs may be 0; state
+ *   indices outside [0, B) or group ids outside [0, G) are refused on the host with GSR_E_INVALID_ARG);
  *   mse host double [B]; psnr_db host float [B]; util host gsr_utility [G] (may be NULL if G == 0);
  *   materialise_images != 0: the [B,H,W,3] images are written to device memory inside the workspace
  *   (as gsr_render_states does); out_host (host fp32 [B,H,W,3] or NULL) additionally copies them back.

@@ -7,6 +7,7 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <mutex>
 #include <vector>
 
 #include "gsr_internal.h"
@@ -152,6 +153,26 @@ static void activate_one(const float ls[3], const float q[4], float logit, float
     }
   *opac = (float)(1.0 / (1.0 + exp(-(double)logit)));
   *tau = (float)log(255.0 * (double)*opac);
+}
+
+}  // namespace gsr
+
+namespace gsr {
+// The per-device error word of the index checks (gsr_internal.h): allocated on first use, zeroed once.
+int* device_error_word() {
+  constexpr int kMaxDev = 64;
+  static std::mutex mu;
+  static int* words[kMaxDev] = {};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDev) return nullptr;
+  std::lock_guard<std::mutex> lock(mu);
+  if (!words[dev]) {
+    int* p = nullptr;
+    if (cudaMalloc(&p, sizeof(int)) != cudaSuccess) return nullptr;
+    if (cudaMemset(p, 0, sizeof(int)) != cudaSuccess) { cudaFree(p); return nullptr; }
+    words[dev] = p;
+  }
+  return words[dev];
 }
 
 }  // namespace gsr
@@ -530,18 +551,49 @@ int gsr_distortion(const float* imgs, const float* ref, int32_t B, int32_t H, in
   return GSR_OK;
 }
 
-int gsr_group_utility(const double* mse, const float* psnr_db, const int32_t* idx_without, const int32_t* idx_with,
-                      const int32_t* group_id, int32_t n_pairs, int32_t G, gsr_utility* out, double* delta_mse,
-                      double* delta_db, void* cuda_stream) {
+static int group_utility(const double* mse, const float* psnr_db, int32_t B, const int32_t* idx_without,
+                         const int32_t* idx_with, const int32_t* group_id, int32_t n_pairs, int32_t G, gsr_utility* out,
+                         double* delta_mse, double* delta_db, void* cuda_stream) {
   if (n_pairs < 0 || G < 0 || (n_pairs > 0 && (!mse || !psnr_db || !idx_without || !idx_with || !group_id)) ||
       (G > 0 && !out)) {
     set_error("gsr_group_utility: invalid argument");
     return GSR_E_INVALID_ARG;
   }
-  launch_group_utility(mse, psnr_db, idx_without, idx_with, group_id, n_pairs, G, out, delta_mse, delta_db,
+  launch_group_utility(mse, psnr_db, B, idx_without, idx_with, group_id, n_pairs, G, out, delta_mse, delta_db,
                        (cudaStream_t)cuda_stream);
   GSR_CUDA(cudaGetLastError());
   return GSR_OK;
+}
+
+int gsr_group_utility(const double* mse, const float* psnr_db, const int32_t* idx_without, const int32_t* idx_with,
+                      const int32_t* group_id, int32_t n_pairs, int32_t G, gsr_utility* out, double* delta_mse,
+                      double* delta_db, void* cuda_stream) {
+  return group_utility(mse, psnr_db, -1, idx_without, idx_with, group_id, n_pairs, G, out, delta_mse, delta_db,
+                       cuda_stream);
+}
+
+int gsr_group_utility_b(const double* mse, const float* psnr_db, int32_t B, const int32_t* idx_without,
+                        const int32_t* idx_with, const int32_t* group_id, int32_t n_pairs, int32_t G, gsr_utility* out,
+                        double* delta_mse, double* delta_db, void* cuda_stream) {
+  if (B < 0) { set_error("gsr_group_utility_b: B < 0"); return GSR_E_INVALID_ARG; }
+  return group_utility(mse, psnr_db, B, idx_without, idx_with, group_id, n_pairs, G, out, delta_mse, delta_db,
+                       cuda_stream);
+}
+
+int gsr_index_status(void* cuda_stream) {
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int* w = device_error_word();
+  if (!w) { set_error("gsr_index_status: no error word on this device"); return GSR_E_CUDA; }
+  int bits = 0;
+  GSR_CUDA(cudaMemcpyAsync(&bits, w, sizeof(int), cudaMemcpyDeviceToHost, st));
+  GSR_CUDA(cudaMemsetAsync(w, 0, sizeof(int), st));
+  GSR_CUDA(cudaStreamSynchronize(st));
+  if (bits == 0) return GSR_OK;
+  set_error("index out of range on the device:%s%s%s%s", (bits & kBadOrder) ? " send order entry outside [0, 4C)" : "",
+            (bits & kBadPairIndex) ? " pair state index outside [0, B)" : "",
+            (bits & kBadGroupId) ? " group id outside [0, G)" : "",
+            (bits & kBadPrefixIndex) ? " prefix pair index outside [0, n)" : "");
+  return GSR_E_INVALID_ARG;
 }
 
 int gsr_close_levels(const uint8_t* delivered_mask, int64_t n, int8_t* depth_out, uint8_t* closure_out,
@@ -655,15 +707,26 @@ int gsr_risk_reduce(const void* values, int32_t dtype, int32_t n, double alpha, 
   return GSR_OK;
 }
 
-int gsr_prefix_monotonicity(const double* d, const int32_t* idx_prev, const int32_t* idx_next, int32_t n_pairs,
-                            double* m_out, int32_t* violations, void* cuda_stream) {
+static int prefix_monotonicity(const double* d, int32_t n, const int32_t* idx_prev, const int32_t* idx_next,
+                               int32_t n_pairs, double* m_out, int32_t* violations, void* cuda_stream) {
   if (n_pairs < 0 || (n_pairs > 0 && (!d || !idx_prev || !idx_next)) || (!m_out && !violations)) {
     set_error("gsr_prefix_monotonicity: invalid argument");
     return GSR_E_INVALID_ARG;
   }
-  launch_prefix_monotonicity(d, idx_prev, idx_next, n_pairs, m_out, violations, (cudaStream_t)cuda_stream);
+  launch_prefix_monotonicity(d, n, idx_prev, idx_next, n_pairs, m_out, violations, (cudaStream_t)cuda_stream);
   GSR_CUDA(cudaGetLastError());
   return GSR_OK;
+}
+
+int gsr_prefix_monotonicity(const double* d, const int32_t* idx_prev, const int32_t* idx_next, int32_t n_pairs,
+                            double* m_out, int32_t* violations, void* cuda_stream) {
+  return prefix_monotonicity(d, -1, idx_prev, idx_next, n_pairs, m_out, violations, cuda_stream);
+}
+
+int gsr_prefix_monotonicity_n(const double* d, int32_t n, const int32_t* idx_prev, const int32_t* idx_next,
+                              int32_t n_pairs, double* m_out, int32_t* violations, void* cuda_stream) {
+  if (n < 0) { set_error("gsr_prefix_monotonicity_n: n < 0"); return GSR_E_INVALID_ARG; }
+  return prefix_monotonicity(d, n, idx_prev, idx_next, n_pairs, m_out, violations, cuda_stream);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -730,6 +793,16 @@ int gsr_utility_frame_host(const gsr_scene* scene, const gsr_camera* cam, float 
     set_error("gsr_utility_frame_host: invalid argument");
     return GSR_E_INVALID_ARG;
   }
+  for (int32_t p = 0; p < n_pairs; ++p) {  // the pair lists are on the host here: refuse bad entries before any work
+    if (idx_without[p] < 0 || idx_without[p] >= B || idx_with[p] < 0 || idx_with[p] >= B) {
+      set_error("gsr_utility_frame_host: pair %d has a state index outside [0, %d)", p, B);
+      return GSR_E_INVALID_ARG;
+    }
+    if (group_id[p] < 0 || group_id[p] >= G) {
+      set_error("gsr_utility_frame_host: pair %d has group id %d outside [0, %d)", p, group_id[p], G);
+      return GSR_E_INVALID_ARG;
+    }
+  }
   if (out_host) materialise_images = 1;
   const FrameCarve f = carve_frame(scene, cam, B, n_pairs, G, materialise_images);
   if (ws_bytes < f.total) { set_error("gsr_utility_frame_host: workspace too small"); return GSR_E_WORKSPACE_TOO_SMALL; }
@@ -757,8 +830,8 @@ int gsr_utility_frame_host(const gsr_scene* scene, const gsr_camera* cam, float 
   int rc = gsr_render_states_vs_full(scene, cam, t, d_levels, B, d_out, d_ref, d_mse, d_psnr, rws, rws_bytes, st);
   if (rc != GSR_OK) return rc;
   if (G > 0) {
-    rc = gsr_group_utility(d_mse, d_psnr, d_pairs, d_pairs + n_pairs, d_pairs + 2 * (size_t)n_pairs, n_pairs, G,
-                           d_util, nullptr, nullptr, st);
+    rc = gsr_group_utility_b(d_mse, d_psnr, B, d_pairs, d_pairs + n_pairs, d_pairs + 2 * (size_t)n_pairs, n_pairs, G,
+                             d_util, nullptr, nullptr, st);
     if (rc != GSR_OK) return rc;
   }
   GSR_CUDA(cudaMemcpyAsync(mse, d_mse, sizeof(double) * B, cudaMemcpyDeviceToHost, st));
@@ -825,11 +898,16 @@ int gsr_debug_keys(const gsr_scene* scene, const void* workspace, int32_t b, int
   if (rc != GSR_OK) return rc;
   if (b < 0 || b >= h.B || cap < 0 || !n_keys) { set_error("gsr_debug_keys: invalid argument"); return GSR_E_INVALID_ARG; }
   const size_t m = (size_t)(cap > 0 ? cap : 1);
-  uint32_t *d_tile = nullptr, *d_db = nullptr;
-  int32_t* d_gi = nullptr;
-  unsigned long long* d_n = nullptr;
-  GSR_CUDA(cudaMalloc(&d_tile, 4 * m)); GSR_CUDA(cudaMalloc(&d_db, 4 * m)); GSR_CUDA(cudaMalloc(&d_gi, 4 * m));
-  GSR_CUDA(cudaMalloc(&d_n, 8));
+  // one allocation for the counter and the three key columns, released on every exit path
+  struct DevBuf {
+    char* p = nullptr;
+    ~DevBuf() { if (p) cudaFree(p); }
+  } buf;
+  GSR_CUDA(cudaMalloc(&buf.p, 8 + 12 * m));
+  unsigned long long* d_n = (unsigned long long*)buf.p;
+  uint32_t* d_tile = (uint32_t*)(buf.p + 8);
+  uint32_t* d_db = d_tile + m;
+  int32_t* d_gi = (int32_t*)(d_db + m);
   launch_filter_keys(scene->impl.d, ws, b, d_tile, d_db, d_gi, d_n, cap, st);
   unsigned long long n = 0;
   GSR_CUDA(cudaMemcpyAsync(&n, d_n, 8, cudaMemcpyDeviceToHost, st));
@@ -840,7 +918,6 @@ int gsr_debug_keys(const gsr_scene* scene, const void* workspace, int32_t b, int
     if (depth_bits) GSR_CUDA(cudaMemcpy(depth_bits, d_db, 4 * ncopy, cudaMemcpyDeviceToHost));
     if (gaussian) GSR_CUDA(cudaMemcpy(gaussian, d_gi, 4 * ncopy, cudaMemcpyDeviceToHost));
   }
-  cudaFree(d_tile); cudaFree(d_db); cudaFree(d_gi); cudaFree(d_n);
   *n_keys = (int64_t)n;
   return GSR_OK;
 }

@@ -181,7 +181,8 @@ void launch_distortion(const float* imgs, const float* ref, int32_t B, int32_t H
                        double* mse, float* psnr, cudaStream_t st);
 void launch_distortion_finalize(const double* part, int32_t B, int32_t tiles, int64_t n_values, double* mse,
                                 float* psnr, cudaStream_t st);
-void launch_group_utility(const double* mse, const float* psnr, const int32_t* iwo, const int32_t* iw,
+// B = number of states behind mse / psnr (range of the pair indices), or < 0 if the caller did not say
+void launch_group_utility(const double* mse, const float* psnr, int32_t B, const int32_t* iwo, const int32_t* iw,
                           const int32_t* gid, int32_t n_pairs, int32_t G, gsr_utility* out, double* dmse,
                           double* ddb, cudaStream_t st);
 void launch_close_levels(const uint8_t* mask, int64_t n, int8_t* depth, uint8_t* closure, cudaStream_t st);
@@ -206,8 +207,9 @@ void launch_flicker(const float* a1, const float* a2, const float* r1, const flo
                     double* part, double* out, cudaStream_t st);
 void launch_risk_reduce(const void* values, int32_t is_f32, int32_t n, double alpha, int32_t upper, gsr_risk* out,
                         cudaStream_t st);
-void launch_prefix_monotonicity(const double* d, const int32_t* prev, const int32_t* next, int32_t n_pairs, double* m_out,
-                                int32_t* viol, cudaStream_t st);
+// n = length of d (range of the indices), or < 0 if the caller did not say
+void launch_prefix_monotonicity(const double* d, int32_t n, const int32_t* prev, const int32_t* next, int32_t n_pairs,
+                                double* m_out, int32_t* viol, cudaStream_t st);
 
 // delivery-mask sampler (k_delivery.cu)
 size_t delivery_workspace_bytes(int32_t C);
@@ -216,5 +218,11 @@ void launch_sample_delivery(const long long* raw, const int32_t* order, int32_t 
                             long long* pk_start, cudaStream_t st);
 
 void set_error(const char* fmt, ...);
+
+// Index arrays handed to the device-pointer calls (send orders, pair lists, prefix pairs) are checked IN the
+// kernels: an entry out of range is skipped and its bit is OR-ed into a per-device error word that
+// gsr_index_status reads and clears.  Returns nullptr if the word cannot be allocated.
+enum : int { kBadOrder = 1, kBadPairIndex = 2, kBadGroupId = 4, kBadPrefixIndex = 8 };
+int* device_error_word();
 
 }  // namespace gsr

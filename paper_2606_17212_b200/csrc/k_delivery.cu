@@ -38,12 +38,17 @@ constexpr int kDelWarps = 4;  // worlds per CTA
 
 // pk_start[k] = index of the first packet of the k-th group IN SEND ORDER, pk_start[4C] = total packets
 __global__ void k_packet_starts(const long long* __restrict__ raw, const int* __restrict__ order, int n_groups,
-                                long long* __restrict__ pk_start) {
+                                long long* __restrict__ pk_start, int* __restrict__ err) {
   if (blockIdx.x != 0 || threadIdx.x != 0) return;
   long long acc = 0;
   for (int k = 0; k < n_groups; ++k) {
     pk_start[k] = acc;
-    acc += (raw[order[k]] + 1199) / 1200;
+    const int g = order[k];
+    if ((unsigned)g >= (unsigned)n_groups) {  // not a group id: sends nothing, the caller is told
+      if (err) atomicOr(err, kBadOrder);
+      continue;
+    }
+    acc += (raw[g] + 1199) / 1200;
   }
   pk_start[n_groups] = acc;
 }
@@ -110,8 +115,9 @@ __global__ void __launch_bounds__(32 * kDelWarps) k_sample_delivery(const long l
         const int mid = (lo + hi + 1) >> 1;
         if (pk_start[mid] <= i) lo = mid; else hi = mid - 1;
       }
-      const int g = order[lo];
-      atomicAnd(&usable[g >> 5], ~(1u << (g & 31)));  // g = 4c + l: word c >> 3, bit 4 (c & 7) + l
+      const int g = order[lo];  // in range: k_packet_starts gives an invalid entry no packet
+      if ((unsigned)g < 4u * (unsigned)C)
+        atomicAnd(&usable[g >> 5], ~(1u << (g & 31)));  // g = 4c + l: word c >> 3, bit 4 (c & 7) + l
     }
   }
   __syncwarp();
@@ -144,7 +150,7 @@ void launch_sample_delivery(const long long* raw, const int32_t* order, int32_t 
   th.pi_bad = den > 0.0 ? loss_threshold(m.p_gb / den) : 0ull;
   th.key0 = (uint32_t)(m.seed & 0xFFFFFFFFull);
   th.key1 = (uint32_t)(m.seed >> 32);
-  k_packet_starts<<<1, 32, 0, st>>>(raw, order, 4 * C, pk_start);
+  k_packet_starts<<<1, 32, 0, st>>>(raw, order, 4 * C, pk_start, device_error_word());
   count_launches(1);
   if (W == 0) return;
   const size_t smem = sizeof(uint32_t) * kDelWarps * (size_t)((C + 7) >> 3);

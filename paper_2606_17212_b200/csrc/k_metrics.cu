@@ -215,16 +215,22 @@ __global__ void __launch_bounds__(kRiskThreads) k_risk_reduce(const void* __rest
 }
 
 // ---- prefix monotonicity (reading G4)
-__global__ void __launch_bounds__(kRiskThreads) k_prefix_monotonicity(const double* __restrict__ d,
+__global__ void __launch_bounds__(kRiskThreads) k_prefix_monotonicity(const double* __restrict__ d, int n,
                                                                       const int* __restrict__ prev,
                                                                       const int* __restrict__ next, int n_pairs,
-                                                                      double* __restrict__ m_out, int* __restrict__ viol) {
+                                                                      double* __restrict__ m_out, int* __restrict__ viol,
+                                                                      int* __restrict__ err) {
   __shared__ double sm_d[kRiskThreads];
   __shared__ unsigned long long sm_c[kRiskThreads];
   double s = 0.0;
   unsigned long long c = 0;
   for (int p = threadIdx.x; p < n_pairs; p += kRiskThreads) {
-    const double inc = d[next[p]] - d[prev[p]];
+    const int a = prev[p], b = next[p];
+    if (a < 0 || b < 0 || (n >= 0 && (a >= n || b >= n))) {  // refused pair: contributes nothing, the caller is told
+      if (err) atomicOr(err, kBadPrefixIndex);
+      continue;
+    }
+    const double inc = d[b] - d[a];
     if (inc > 0.0) { s += inc; ++c; }
   }
   s = risk_block_sum<double>(s, sm_d);
@@ -277,9 +283,9 @@ void launch_risk_reduce(const void* values, int32_t is_f32, int32_t n, double al
   count_launches(1);
 }
 
-void launch_prefix_monotonicity(const double* d, const int32_t* prev, const int32_t* next, int32_t n_pairs, double* m_out,
-                                int32_t* viol, cudaStream_t st) {
-  k_prefix_monotonicity<<<1, kRiskThreads, 0, st>>>(d, prev, next, n_pairs, m_out, viol);
+void launch_prefix_monotonicity(const double* d, int32_t n, const int32_t* prev, const int32_t* next, int32_t n_pairs,
+                                double* m_out, int32_t* viol, cudaStream_t st) {
+  k_prefix_monotonicity<<<1, kRiskThreads, 0, st>>>(d, n, prev, next, n_pairs, m_out, viol, device_error_word());
   count_launches(1);
 }
 

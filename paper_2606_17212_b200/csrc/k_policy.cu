@@ -96,7 +96,7 @@ __global__ void __launch_bounds__(kPolThreads) k_frontier_order(const double* __
 // ---- F3: thread j walks the order for budget j: longest prefix with cumulative wire bytes <= budget
 __global__ void k_frontier_states(const int* __restrict__ order, const long long* __restrict__ wire, int C,
                                   const long long* __restrict__ budgets, int nb, signed char* __restrict__ levels,
-                                  long long* __restrict__ used, int* __restrict__ n_groups) {
+                                  long long* __restrict__ used, int* __restrict__ n_groups, int* __restrict__ err) {
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= nb) return;
   signed char* row = levels + (size_t)j * C;
@@ -106,6 +106,10 @@ __global__ void k_frontier_states(const int* __restrict__ order, const long long
   int n = 0;
   for (int k = 0; k < 4 * C; ++k) {
     const int g = order[k];
+    if ((unsigned)g >= 4u * (unsigned)C) {  // not a group id: the walk stops here, the caller is told
+      if (err) atomicOr(err, kBadOrder);
+      break;
+    }
     const long long wg = wire[g];
     if (acc + wg > beta) break;
     acc += wg;
@@ -182,7 +186,8 @@ void launch_frontier_order(const double* score, const long long* wire, int32_t C
 void launch_frontier_states(const int32_t* order, const long long* wire, int32_t C, const long long* budgets,
                             int32_t nb, int8_t* levels, long long* used, int32_t* n_groups, cudaStream_t st) {
   if (nb == 0) return;
-  k_frontier_states<<<(nb + 63) / 64, 64, 0, st>>>(order, wire, C, budgets, nb, (signed char*)levels, used, n_groups);
+  k_frontier_states<<<(nb + 63) / 64, 64, 0, st>>>(order, wire, C, budgets, nb, (signed char*)levels, used, n_groups,
+                                                   device_error_word());
   count_launches(1);
 }
 

@@ -264,8 +264,7 @@ __global__ void __launch_bounds__(128) k_project(DeviceScene sc, FrameParams fp,
   float St[6];
   const float* Sp = S6;
   if (sc.affine_cov) { push_forward_cov(A, S6, St); Sp = St; }
-  Proj pa;
-  pa.count = 0;
+  Proj pa{};  // absent variant: all fields zero (gsr_debug_projection exports them), count = 0 = culled
   if (lvl == 0) pa = project_variant(fp, p, Sp, tau);
   Proj pb = project_variant(fp, muB, Sp, tau);
 
@@ -353,7 +352,7 @@ __global__ void __launch_bounds__(128) k_project4(DeviceScene sc, FrameParams fp
   bool any = false;
 #pragma unroll
   for (int v = 0; v < 4; ++v) {
-    pr[v].count = 0;
+    pr[v] = Proj{};  // absent variant: all fields zero, count = 0 = culled
     opv[v] = opac; tauv[v] = tau;
     if (v >= lvl) {
       if (sc.g1v) {  // scale / rotation / opacity refinements (reading I2): attributes of delivered depth v

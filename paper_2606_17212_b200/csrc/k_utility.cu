@@ -44,7 +44,15 @@ struct PairView {
   const float* psnr;
   const int32_t *iwo, *iw, *gid;
   int n_pairs;
+  int B;     // states behind mse / psnr; < 0: unknown (only negative indices can then be refused)
+  int* err;  // device error word (gsr_index_status) or nullptr
 };
+
+// both state indices of pair p usable?
+__device__ __forceinline__ bool pair_ok(const PairView& pv, int p) {
+  const int a = pv.iwo[p], b = pv.iw[p];
+  return a >= 0 && b >= 0 && (pv.B < 0 || (a < pv.B && b < pv.B));
+}
 
 __device__ __forceinline__ double pair_delta(const PairView& pv, int p, int metric) {
   return metric == 0 ? pv.mse[pv.iwo[p]] - pv.mse[pv.iw[p]]
@@ -62,7 +70,7 @@ __device__ double select_kth(const PairView& pv, int g, int metric, int n_g, con
       for (int i = threadIdx.x; i < n_g; i += kUtilThreads) c += ordered_key(cache[i]) < cand;
     } else {
       for (int p = threadIdx.x; p < pv.n_pairs; p += kUtilThreads)
-        if (pv.gid[p] == g) c += ordered_key(pair_delta(pv, p, metric)) < cand;
+        if (pv.gid[p] == g && pair_ok(pv, p)) c += ordered_key(pair_delta(pv, p, metric)) < cand;
     }
     c = block_sum<unsigned long long>(c, sm_cnt);
     if (c <= (unsigned long long)k) ans = cand;  // at most k keys below cand => the k-th key is >= cand
@@ -74,6 +82,12 @@ __global__ void __launch_bounds__(kUtilThreads) k_pair_delta(PairView pv, double
                                                              double* __restrict__ ddb) {
   int p = blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= pv.n_pairs) return;
+  if (!pair_ok(pv, p)) {  // refused pair: zero difference, the caller is told
+    if (pv.err) atomicOr(pv.err, kBadPairIndex);
+    if (dmse) dmse[p] = 0.0;
+    if (ddb) ddb[p] = 0.0;
+    return;
+  }
   if (dmse) dmse[p] = pair_delta(pv, p, 0);
   if (ddb) ddb[p] = pair_delta(pv, p, 1);
 }
@@ -88,13 +102,23 @@ __global__ void __launch_bounds__(kUtilThreads) k_group_utility(PairView pv, int
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   double res[2][4];
   int n_g = 0;
+  if (pv.err && g == 0) {  // one CTA reports group ids no group owns and pairs with unusable state indices
+    bool bad_g = false, bad_p = false;
+    for (int p = threadIdx.x; p < pv.n_pairs; p += kUtilThreads) {
+      const bool in = (unsigned)pv.gid[p] < (unsigned)G;
+      bad_g |= !in;
+      bad_p |= in && !pair_ok(pv, p);
+    }
+    if (bad_g) atomicOr(pv.err, kBadGroupId);
+    if (bad_p) atomicOr(pv.err, kBadPairIndex);
+  }
   for (int metric = 0; metric < 2; ++metric) {
     // ordered compaction of the group's deltas (pair order) into the cache; count members
     if (threadIdx.x == 0) run_s = 0;
     __syncthreads();
     for (int base = 0; base < pv.n_pairs; base += kUtilThreads) {
       const int p = base + threadIdx.x;
-      const bool mem = p < pv.n_pairs && pv.gid[p] == g;
+      const bool mem = p < pv.n_pairs && pv.gid[p] == g && pair_ok(pv, p);  // a refused pair belongs to no group
       const uint32_t bal = __ballot_sync(0xffffffffu, mem);
       if (lane == 0) wcnt[w] = __popc(bal);
       __syncthreads();
@@ -121,7 +145,7 @@ __global__ void __launch_bounds__(kUtilThreads) k_group_utility(PairView pv, int
       for (int i = threadIdx.x; i < n_g; i += kUtilThreads) s += cache[i];
     } else {
       for (int p = threadIdx.x; p < pv.n_pairs; p += kUtilThreads)
-        if (pv.gid[p] == g) s += pair_delta(pv, p, metric);
+        if (pv.gid[p] == g && pair_ok(pv, p)) s += pair_delta(pv, p, metric);
     }
     const double mean = block_sum<double>(s, sm_d) / (double)n_g;
     // population variance
@@ -130,7 +154,7 @@ __global__ void __launch_bounds__(kUtilThreads) k_group_utility(PairView pv, int
       for (int i = threadIdx.x; i < n_g; i += kUtilThreads) { const double d = cache[i] - mean; s += d * d; }
     } else {
       for (int p = threadIdx.x; p < pv.n_pairs; p += kUtilThreads)
-        if (pv.gid[p] == g) { const double d = pair_delta(pv, p, metric) - mean; s += d * d; }
+        if (pv.gid[p] == g && pair_ok(pv, p)) { const double d = pair_delta(pv, p, metric) - mean; s += d * d; }
     }
     const double sd = sqrt(block_sum<double>(s, sm_d) / (double)n_g);
     // Q_0.1 by linear interpolation at position 0.1 (n-1)
@@ -177,10 +201,10 @@ __global__ void __launch_bounds__(kUtilThreads) k_group_utility(PairView pv, int
   }
 }
 
-void launch_group_utility(const double* mse, const float* psnr, const int32_t* iwo, const int32_t* iw,
+void launch_group_utility(const double* mse, const float* psnr, int32_t B, const int32_t* iwo, const int32_t* iw,
                           const int32_t* gid, int32_t n_pairs, int32_t G, gsr_utility* out, double* dmse,
                           double* ddb, cudaStream_t st) {
-  PairView pv{mse, psnr, iwo, iw, gid, n_pairs};
+  PairView pv{mse, psnr, iwo, iw, gid, n_pairs, B, device_error_word()};
   if (n_pairs > 0 && (dmse || ddb))
   {
     k_pair_delta<<<(n_pairs + kUtilThreads - 1) / kUtilThreads, kUtilThreads, 0, st>>>(pv, dmse, ddb);

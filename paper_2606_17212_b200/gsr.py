@@ -75,6 +75,8 @@ def lib():
         L.gsr_distortion_workspace_bytes.restype = sz
         L.gsr_distortion.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp, sz, vp]
         L.gsr_group_utility.argtypes = [vp, vp, vp, vp, vp, i32, i32, vp, vp, vp, vp]
+        L.gsr_group_utility_b.argtypes = [vp, vp, i32, vp, vp, vp, i32, i32, vp, vp, vp, vp]
+        L.gsr_index_status.argtypes = [vp]
         L.gsr_close_levels.argtypes = [vp, i64, vp, vp, vp]
         L.gsr_frame_workspace_bytes.argtypes = [vp, C.POINTER(CameraC), i32, i32, i32, i32]
         L.gsr_frame_workspace_bytes.restype = sz
@@ -100,6 +102,7 @@ def lib():
         L.gsr_flicker.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp, sz, vp]
         L.gsr_risk_reduce.argtypes = [vp, i32, i32, C.c_double, i32, vp, vp]
         L.gsr_prefix_monotonicity.argtypes = [vp, vp, vp, i32, vp, vp, vp]
+        L.gsr_prefix_monotonicity_n.argtypes = [vp, i32, vp, vp, i32, vp, vp, vp]
         L.gsr_delivery_workspace_bytes.argtypes = [i32]
         L.gsr_delivery_workspace_bytes.restype = sz
         L.gsr_sample_delivery.argtypes = [vp, vp, i32, C.POINTER(LossModel), vp, i32, i32, vp, vp, vp, sz, vp]
@@ -348,16 +351,23 @@ def group_utility(mse, psnr, idx_without, idx_with, group_id, G: int, want_delta
     dd = torch.empty(max(n_pairs, 1), dtype=torch.float64, device="cuda") if want_deltas else None
     for t in (idx_without, idx_with, group_id):
         assert t.dtype == torch.int32 and t.is_cuda and t.is_contiguous()
-    _check(lib().gsr_group_utility(_dp(mse), _dp(psnr), _dp(idx_without), _dp(idx_with), _dp(group_id), n_pairs, G,
-                                   _dp(util), _dp(dm), _dp(dd), _stream()))
+    _check(lib().gsr_group_utility_b(_dp(mse), _dp(psnr), int(mse.numel()), _dp(idx_without), _dp(idx_with),
+                                     _dp(group_id), n_pairs, G, _dp(util), _dp(dm), _dp(dd), _stream()))
+    index_status()
     u = util[:G].cpu().numpy().view(UTILITY_DTYPE).reshape(G)
     return u, (dm[:n_pairs] if dm is not None else None), (dd[:n_pairs] if dd is not None else None)
 
 
 def group_utility_into(mse, psnr, idx_without, idx_with, group_id, G: int, util_out):
-    """gsr_group_utility with a caller-provided cuda float64 [G,9] output (no allocation, no sync)."""
-    _check(lib().gsr_group_utility(_dp(mse), _dp(psnr), _dp(idx_without), _dp(idx_with), _dp(group_id),
-                                   int(idx_without.numel()), G, _dp(util_out), None, None, _stream()))
+    """gsr_group_utility_b with a caller-provided cuda float64 [G,9] output (no allocation, no sync; range errors of
+    the pair lists stay latched until index_status() is called)."""
+    _check(lib().gsr_group_utility_b(_dp(mse), _dp(psnr), int(mse.numel()), _dp(idx_without), _dp(idx_with),
+                                     _dp(group_id), int(idx_without.numel()), G, _dp(util_out), None, None, _stream()))
+
+
+def index_status():
+    """gsr_index_status: synchronises the stream; raises if a device-side index check refused an entry."""
+    _check(lib().gsr_index_status(_stream()))
 
 
 def close_levels(mask):
@@ -485,8 +495,9 @@ def prefix_monotonicity(d, idx_prev, idx_next):
     assert d.dtype == torch.float64 and idx_prev.dtype == torch.int32 and idx_next.dtype == torch.int32
     m = torch.zeros(1, dtype=torch.float64, device="cuda")
     v = torch.zeros(1, dtype=torch.int32, device="cuda")
-    _check(lib().gsr_prefix_monotonicity(_dp(d), _dp(idx_prev), _dp(idx_next), idx_prev.numel(), _dp(m), _dp(v),
-                                         _stream()))
+    _check(lib().gsr_prefix_monotonicity_n(_dp(d), int(d.numel()), _dp(idx_prev), _dp(idx_next), idx_prev.numel(),
+                                           _dp(m), _dp(v), _stream()))
+    index_status()
     return float(m.item()), int(v.item())
 
 
