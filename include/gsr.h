@@ -358,11 +358,14 @@ int gsr_debug_closure(const gsr_scene* scene, const void* workspace, int8_t* dep
  *       (a lower bound of the oracle's E = sum_b E_b, whose lists are the unculled 3-sigma tile lists). */
 int gsr_debug_pair_counts(const gsr_scene* scene, const void* workspace, int64_t* counts3, void* cuda_stream);
 
-/* Options: "state_block" = states composited per CTA (1, 4, 8 or 16; default 8) and "dedup" = 0/1 (tile-level
- * state dedup, default 1) — results do not depend on either (bitwise); "profile" = 1 records CUDA events around
- * every compositing-kernel launch and around the projection and binning + sort phases of every frame (a
- * measurement aid: call the library from ONE host thread while it is on).  Everything else may be called from
- * several host threads at once, each with its own stream and workspace (tests/test_gpu_streams.py). */
+/* Options.  "state_block" = state slots per compositing warp (0 = default, 1, 4..8 or 16) and "dedup" = 0/1
+ * (tile-level state dedup, default 1): results do not depend on either (bitwise).  Both belong to the CALLING
+ * HOST THREAD — they steer the calls that thread makes afterwards and nothing another thread does.
+ * "profile" = 1 records CUDA events around every compositing launch and around the projection and binning +
+ * sort phases of every frame, for the calls of the thread that switched it on (other threads run unprofiled);
+ * it is refused with GSR_E_INVALID_ARG while any thread is inside a render call.
+ * Everything may be called from several host threads at once, each with its own stream and workspace
+ * (tests/test_gpu_streams.py). */
 int gsr_set_option(const char* name, int32_t value);
 
 /* Sum of the compositing kernel's durations (ms, CUDA events on its launch stream) and the number

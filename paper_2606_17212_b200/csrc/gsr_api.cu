@@ -7,7 +7,9 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <atomic>
 #include <mutex>
+#include <thread>
 #include <vector>
 
 #include "gsr_internal.h"
@@ -32,8 +34,17 @@ void set_error(const char* fmt, ...) {
     }                                                                                       \
   } while (0)
 
-extern int g_state_block, g_profile, g_dedup;
+extern thread_local int g_state_block, g_dedup;
+extern std::atomic<int> g_profile;
+extern std::thread::id g_profile_owner;
+bool profiling_here();
 void profile_reset();
+// calls that enqueue a frame, currently inside the library (any thread): "profile" may only be switched while 0
+static std::atomic<int> g_calls_in_flight{0};
+struct InFlight {
+  InFlight() { g_calls_in_flight.fetch_add(1, std::memory_order_acq_rel); }
+  ~InFlight() { g_calls_in_flight.fetch_sub(1, std::memory_order_acq_rel); }
+};
 int profile_read(double* ms, int* n);
 unsigned long long launches_total();
 int measure_ffma_peak(int num_sms, double* tflops, cudaStream_t st);
@@ -43,7 +54,7 @@ constexpr int kMaxPhaseFrames = 4096;
 static cudaEvent_t g_ph[kMaxPhaseFrames][3];
 static int g_ph_created = 0, g_ph_used = 0;
 static int phase_slot() {
-  if (!g_profile || g_ph_used >= kMaxPhaseFrames) return -1;
+  if (!profiling_here() || g_ph_used >= kMaxPhaseFrames) return -1;
   const int slot = g_ph_used++;
   while (g_ph_created <= slot) {
     for (int k = 0; k < 3; ++k) cudaEventCreate(&g_ph[g_ph_created][k]);
@@ -198,9 +209,17 @@ int gsr_set_option(const char* name, int value) {
     return GSR_OK;
   }
   if (name && strcmp(name, "profile") == 0) {
-    g_profile = value != 0;
+    if (g_calls_in_flight.load(std::memory_order_acquire) != 0) {
+      set_error("gsr_set_option: \"profile\" cannot be switched while another thread is inside a render call");
+      return GSR_E_INVALID_ARG;
+    }
+    g_profile.store(0, std::memory_order_release);
     profile_reset();
     g_ph_used = 0;
+    if (value != 0) {
+      g_profile_owner = std::this_thread::get_id();
+      g_profile.store(1, std::memory_order_release);
+    }
     return GSR_OK;
   }
   set_error("gsr_set_option: unknown option or value");
@@ -484,6 +503,7 @@ int gsr_render_states_ex(const gsr_scene* scene, const gsr_camera* cam, float t,
                          size_t ws_bytes, void* cuda_stream) {
   if (ref && !mse) { set_error("gsr_render_states: ref given without mse"); return GSR_E_INVALID_ARG; }
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  InFlight guard;
   Workspace ws;
   FrameParams fp;
   int rc = prepare_frame(scene, cam, t, levels, B, workspace, ws_bytes, st, &ws, &fp);
@@ -498,6 +518,7 @@ int gsr_render_states_vs_full(const gsr_scene* scene, const gsr_camera* cam, flo
                               size_t ws_bytes, void* cuda_stream) {
   if (!ref_out || !mse) { set_error("gsr_render_states_vs_full: ref_out and mse are required"); return GSR_E_INVALID_ARG; }
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  InFlight guard;
   Workspace ws;
   FrameParams fp;
   int rc = prepare_frame(scene, cam, t, levels, B, workspace, ws_bytes, st, &ws, &fp);

@@ -3,6 +3,7 @@
 // (same pixel -> thread mapping and the same reduction tree as the fused path: reduce.cuh), launch bookkeeping,
 // optional CUDA-event timing of the compositing launches and the FP32 peak measurement.
 #include <atomic>
+#include <thread>
 
 #include "composite_common.cuh"
 #include "gsr_internal.h"
@@ -76,9 +77,15 @@ static std::atomic<unsigned long long> g_launches{0};  // calls may come from se
 void count_launches(int n) { g_launches.fetch_add((unsigned long long)n, std::memory_order_relaxed); }
 unsigned long long launches_total() { return g_launches.load(std::memory_order_relaxed); }
 
-int g_state_block = 0;  // S; 0 = default (k_composite_q.cu); set through gsr_set_option for experiments (1, 4..8, 16)
-int g_dedup = 1;        // gsr_set_option("dedup", 0/1): tile-level state dedup
-int g_profile = 0;      // gsr_set_option("profile", 1): record events around every k_composite launch
+// Options (gsr_set_option).  The two that steer launches belong to the CALLING HOST THREAD: a thread that sets
+// them changes its own later calls only, never a launch another thread is preparing.
+thread_local int g_state_block = 0;  // S; 0 = default (k_composite_q.cu); experiments: 1, 4..8, 16
+thread_local int g_dedup = 1;        // tile-level state dedup on / off
+// "profile" is process-wide and owned by the thread that switched it on: only that thread's calls record events
+// (the event arrays below are not synchronised), calls of other threads run unprofiled.
+std::atomic<int> g_profile{0};
+std::thread::id g_profile_owner;
+bool profiling_here() { return g_profile.load(std::memory_order_acquire) != 0 && std::this_thread::get_id() == g_profile_owner; }
 constexpr int kMaxProfEvents = 8192;
 static cudaEvent_t g_ev[kMaxProfEvents][2];
 static int g_ev_created = 0, g_ev_used = 0;
@@ -101,7 +108,7 @@ int profile_read(double* ms, int* n) {
 // optional CUDA events around a compositing launch (gsr_set_option("profile", 1))
 static int profile_begin(cudaStream_t st) {
   int slot = -1;
-  if (g_profile && g_ev_used < kMaxProfEvents) {
+  if (profiling_here() && g_ev_used < kMaxProfEvents) {
     slot = g_ev_used++;
     while (g_ev_created <= slot) {
       cudaEventCreate(&g_ev[g_ev_created][0]);

@@ -309,11 +309,8 @@ bool launch_tile_dedup(const DeviceScene& sc, const FrameParams& fp, Workspace& 
   int Bp = 0;
   const size_t smem = dedup_smem_bytes(B, sc.C, &Bp);
   if (B < 2 || smem > 200 * 1024) return false;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaFuncSetAttribute(k_tile_dedup, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-    attr_set = true;
-  }
+  // the opt-in is per device and cheap: made whenever it is needed rather than once per process
+  if (smem > 48 * 1024) cudaFuncSetAttribute(k_tile_dedup, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
   k_tile_dedup<<<fp.TX * fp.TY, kDedupThreads, smem, st>>>(ws.render_range, ws.vals[1], ws.r1, depth_rows, B, sc.C, Bp,
                                                           ws.uorder, ws.upos, ws.n_unique);
   count_launches(1);

@@ -113,3 +113,71 @@ def test_host_call_from_threads_equals_serial_bitwise(gsr, torch_mod, workload):
                 assert np.array_equal(got[f][0], want[f][0]) and np.array_equal(got[f][1], want[f][1])
                 assert got[f][2].tobytes() == want[f][2].tobytes()
     scene.close()
+
+
+def test_options_belong_to_the_calling_thread(gsr, torch_mod, workload):
+    """include/gsr.h: "state_block" and "dedup" steer the calls of the thread that set them.  Three threads render the
+    same frames at the same time with different state blocks (one of them without dedup); every one of them gets
+    the bits of the serial default render, and the main thread's options are untouched.  "profile" is refused
+    while a call is in flight and never makes another thread's calls record events."""
+    import threading
+    torch = torch_mod
+    wl = workload
+    scene = gsr.Scene(wl.scene)
+    n = len(wl.frames)
+    dev = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a, dt)).cuda()
+    lv = [dev(l, np.int8) for l in wl.levels]
+    cams = [gsr.camera_struct(c) for c, _ in wl.frames]
+    ts = [float(t) for _, t in wl.frames]
+    cam0, _ = wl.frames[0]
+    B = wl.levels[0].shape[0]
+
+    def render_all(b):
+        res = []
+        for f in range(n):
+            scene.render_states_vs_full(cams[f], ts[f], lv[f], b["ws"], b["ref"], b["mse"], b["psnr"], out=b["out"])
+            torch.cuda.current_stream().synchronize()
+            res.append((b["out"].clone(), b["mse"].clone()))
+        return res
+
+    want = render_all(_bufs(torch, scene, cam0, B, 0))
+    settings = [(4, 1), (16, 1), (8, 0)]
+    got, errors = [None] * len(settings), []
+    start = threading.Barrier(len(settings))
+
+    def worker(k):
+        try:
+            torch.cuda.set_device(0)
+            S, dedup = settings[k]
+            gsr.set_option("state_block", S)
+            gsr.set_option("dedup", dedup)
+            b = _bufs(torch, scene, cam0, B, 0)
+            start.wait()
+            with torch.cuda.stream(torch.cuda.Stream()):
+                for _ in range(3):
+                    got[k] = render_all(b)
+        except Exception as e:  # noqa: BLE001
+            errors.append(repr(e))
+
+    threads = [threading.Thread(target=worker, args=(k,)) for k in range(len(settings))]
+    for th in threads:
+        th.start()
+    for th in threads:
+        th.join()
+    assert not errors, errors
+    for k in range(len(settings)):
+        for f in range(n):
+            assert torch.equal(got[k][f][0], want[f][0]) and torch.equal(got[k][f][1], want[f][1]), (settings[k], f)
+    # the main thread still renders with its own (default) options, and profiling stays with the thread that asked
+    gsr.set_option("profile", 1)
+    done = []
+    th = threading.Thread(target=lambda: done.append(render_all(_bufs(torch, scene, cam0, B, 0))))
+    th.start()
+    th.join()
+    ms, launches = gsr.profile_read()
+    assert launches == 0                                   # the other thread's calls recorded nothing
+    render_all(_bufs(torch, scene, cam0, B, 0))
+    ms, launches = gsr.profile_read()
+    assert launches == 2 * n                               # reference + batch per frame, this thread's calls
+    gsr.set_option("profile", 0)
+    scene.close()
