@@ -142,9 +142,10 @@ def oracle_sample(wl, frame: int, n_states: int):
     reference and the distortion).  Returns seconds."""
     from oracle import oracle as O
     cam, t = wl.frames[frame]
-    osc = oracle_sample.cache.get("scene")
+    osc = oracle_sample.cache.get(wl.name)
     if osc is None:
-        osc = oracle_sample.cache["scene"] = O.OracleScene(wl.scene)
+        oracle_sample.cache.clear()                       # one workload's scene at a time
+        osc = oracle_sample.cache[wl.name] = O.OracleScene(wl.scene)
     lv = np.ascontiguousarray(wl.levels[frame][:n_states])
     t0 = time.perf_counter()
     full = np.full((1, wl.scene.C), 3, np.int8)
@@ -186,7 +187,40 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------------ our arm
-def run_ours(args):
+KERNEL_SOURCE = ROOT / "paper_2606_17212_b200" / "csrc" / "k_composite_q.cu"
+
+
+def traffic_record(workload_name: str) -> dict:
+    """roofline.traffic = DRAM bytes per launch of the dominant kernel from an ncu --set full capture, recorded in
+    profiles/traffic.txt together with the SHA-256 of the kernel source it was taken on.  The number is only
+    reported while the kernel source still has that hash; otherwise traffic is null and the reason is given."""
+    import hashlib
+    tp = ROOT / "profiles" / "traffic.txt"
+    out = {"traffic": None, "traffic_source": None}
+    if not tp.exists():
+        return out
+    sha_now = hashlib.sha256(KERNEL_SOURCE.read_bytes()).hexdigest() if KERNEL_SOURCE.exists() else None
+    meta, val = {}, None
+    for ln in tp.read_text().splitlines():
+        f = ln.split()
+        if ln.startswith("# ") and len(f) >= 3 and f[1].endswith(":"):
+            meta[f[1][:-1]] = " ".join(f[2:])
+        elif len(f) == 2 and not ln.startswith("#") and f[0] == workload_name:
+            val = int(f[1])
+    src = {"file": "profiles/traffic.txt", "commit": meta.get("commit"), "command": meta.get("command"),
+           "kernel_source": str(KERNEL_SOURCE.relative_to(ROOT)), "kernel_source_sha256": meta.get("kernel_source_sha256"),
+           "matches_current_source": sha_now is not None and sha_now == meta.get("kernel_source_sha256")}
+    out["traffic_source"] = src
+    if val is not None and src["matches_current_source"]:
+        out["traffic"] = val
+    elif val is not None:
+        src["note"] = "the kernel source changed since the capture: traffic withheld"
+    return out
+
+
+def measure_ours(args, workload: str, steps: int, warmup: int, full: bool):
+    """One workload through the C ABI.  full = the N = 1 bench line (repetitions, sustained pass, end-to-end call,
+    the run without images); otherwise the compact sub-record of `workloads` (value, roofline, clocks, CPU sample)."""
     import torch
     from paper_2606_17212_b200 import build as gbuild
     gbuild.build()
@@ -202,9 +236,11 @@ def run_ours(args):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
-    total_steps = args.steps + args.warmup
-    n_frames = min(150, max(1, total_steps * world)) if args.workload in ("cfg1", "cfg1r") else min(8, max(1, total_steps))
-    wl = build_workload(args.workload, n_frames)
+    if args.gpus != world:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but {world} rank(s) are running (WORLD_SIZE)")
+    total_steps = steps + warmup
+    n_frames = min(150, max(1, total_steps * world)) if workload in ("cfg1", "cfg1r") else min(8, max(1, total_steps))
+    wl = build_workload(workload, n_frames)
     n_frames = len(wl.frames)
     scene = gsr.Scene(wl.scene)
     if args.state_block:
@@ -276,97 +312,126 @@ def run_ours(args):
         return shard.max_over_ranks(ms, device=dev)
 
     # ---- warm-up, then the timed region (device-resident inputs), clocks sampled during it
-    for k in range(args.warmup):
+    for k in range(warmup):
         step(k)
     torch.cuda.synchronize()
-    for b in bufs:
+    for b in bufs[:min(F, warmup)]:                  # the workspaces a warm-up step has written
         scene.status(b["ws"])
     l0 = gsr.launch_count()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
         sampler.mark()
-    ms = timed(step, args.warmup, args.steps, pipelined=True)
+    # protocol of PAPER.md:142 ("5 warm-ups, 3 repetitions, Student-t 95 % CI"): the timed region of exactly
+    # `steps` steps is repeated; `value` is the mean over the repetitions
+    n_rep = 3 if full else 1
+    ms_reps = []
+    for r in range(n_rep):
+        ms_reps.append(timed(step, warmup + r * steps, steps, pipelined=True))
+        if r == 0:
+            launches = gsr.launch_count() - l0
     clocks = sampler.stop() if rank == 0 else None
-    launches = gsr.launch_count() - l0
-    value = B * args.steps * world / (ms * 1e-3)
+    ms = float(np.mean(ms_reps))
+    value_reps = [B * steps * world / (m * 1e-3) for m in ms_reps]
+    value = float(np.mean(value_reps))
+    T975 = {1: 12.706, 2: 4.303, 3: 3.182, 4: 2.776}      # Student t, 97.5 %, n - 1 degrees of freedom
+    ci95 = (T975[n_rep - 1] * float(np.std(value_reps, ddof=1)) / np.sqrt(n_rep)) if n_rep > 1 else None
+
+    # ---- sustained pass: the same pipelined steps for >= 2 s, clocks and power sampled throughout, so that the
+    #      number is also on record at the power-steady clock
+    sustained = None
+    if full:
+        n_sus = int(np.ceil(2200.0 / max(ms / steps, 1e-3)))
+        sus = ClockSampler(local)
+        if rank == 0:
+            sus.start()
+            sus.mark()
+        ms_sus = timed(step, warmup, n_sus, pipelined=True)
+        sus_clocks = sus.stop() if rank == 0 else None
+        sustained = {"value": B * n_sus * world / (ms_sus * 1e-3), "unit": "states/s", "steps": n_sus,
+                     "seconds": ms_sus * 1e-3, "ms_per_step": ms_sus / n_sus, "clocks": sus_clocks}
 
     # ---- the same steps one frame at a time with CUDA events around every k_composite launch and around the
     #      memory-bound phases: what the roofline objects are computed from (events of overlapping streams
     #      would count co-running kernels twice)
     gsr.set_option("profile", 1)
-    ms_serial = timed(step_serial, args.warmup, args.steps)
+    ms_serial = timed(step_serial, warmup, steps)
     comp_ms, comp_n = gsr.profile_read()
     proj_ms, sort_ms, ph_n = gsr.profile_read_phases()
     gsr.set_option("profile", 0)
     keys = scene.status(ws)
 
     # ---- the same path without materialising the images (distortion/utility only), reported beside it
-    ms_noimg = timed(lambda k: step(k, images=False), args.warmup, args.steps, pipelined=True)
+    ms_noimg = timed(lambda k: step(k, images=False), warmup, steps, pipelined=True) if full else None
 
-    # ---- end to end through the host-buffer C-ABI call: pinned host inputs, H2D + D2H inside the timed region
-    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-    h_lv = [pin(l) for l in wl.levels]
-    h_iwo, h_iw, h_gid = [pin(a) for a in wl.idx_without], [pin(a) for a in wl.idx_with], [pin(a) for a in wl.group_id]
-    # F host threads, each with its own stream, workspace and pinned result buffers, call the (blocking) host
-    # API round-robin: the same frames-in-flight pipeline as above, driven through the public call
-    from concurrent.futures import ThreadPoolExecutor
-    lanes = []
-    for _ in range(F):
-        h_mse = torch.empty(B, dtype=torch.float64).pin_memory()
-        h_psnr = torch.empty(B, dtype=torch.float32).pin_memory()
-        h_util = torch.zeros((max(G, 1), 9), dtype=torch.float64).pin_memory()
-        lanes.append({"pins": (h_mse, h_psnr, h_util), "ws": None, "stream": torch.cuda.Stream(device=dev),
-                      "host": (h_mse.numpy(), h_psnr.numpy(), h_util.numpy().view(gsr.UTILITY_DTYPE).reshape(-1)),
-                      "pool": ThreadPoolExecutor(max_workers=1), "pending": []})
+    e2e = None
+    if full:
+        # ---- end to end through the host-buffer C-ABI call: pinned host inputs, H2D + D2H inside the timed region
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        h_lv = [pin(l) for l in wl.levels]
+        h_iwo, h_iw, h_gid = [pin(a) for a in wl.idx_without], [pin(a) for a in wl.idx_with], [pin(a) for a in wl.group_id]
+        # F host threads, each with its own stream, workspace and pinned result buffers, call the (blocking) host
+        # API round-robin: the same frames-in-flight pipeline as above, driven through the public call
+        from concurrent.futures import ThreadPoolExecutor
+        lanes = []
+        for _ in range(F):
+            h_mse = torch.empty(B, dtype=torch.float64).pin_memory()
+            h_psnr = torch.empty(B, dtype=torch.float32).pin_memory()
+            h_util = torch.zeros((max(G, 1), 9), dtype=torch.float64).pin_memory()
+            lanes.append({"pins": (h_mse, h_psnr, h_util), "ws": None, "stream": torch.cuda.Stream(device=dev),
+                          "host": (h_mse.numpy(), h_psnr.numpy(), h_util.numpy().view(gsr.UTILITY_DTYPE).reshape(-1)),
+                          "pool": ThreadPoolExecutor(max_workers=1), "pending": []})
 
-    def e2e_frame(lane, k):
-        f = frame_of(k)
-        torch.cuda.set_device(local)
-        with torch.cuda.stream(lane["stream"]):
-            r = scene.utility_frame_host(cams[f], ts[f], h_lv[f].numpy(), h_iwo[f].numpy(), h_iw[f].numpy(),
-                                         h_gid[f].numpy(), G, workspace=lane["ws"], materialise=True, bufs=lane["host"])
-        lane["ws"] = r[4]
+        def e2e_frame(lane, k):
+            f = frame_of(k)
+            torch.cuda.set_device(local)
+            with torch.cuda.stream(lane["stream"]):
+                r = scene.utility_frame_host(cams[f], ts[f], h_lv[f].numpy(), h_iwo[f].numpy(), h_iw[f].numpy(),
+                                             h_gid[f].numpy(), G, workspace=lane["ws"], materialise=True, bufs=lane["host"])
+            lane["ws"] = r[4]
 
-    def step_e2e(k):
-        lane = lanes[k % F]
-        lane["pending"].append(lane["pool"].submit(e2e_frame, lane, k))
+        def step_e2e(k):
+            lane = lanes[k % F]
+            lane["pending"].append(lane["pool"].submit(e2e_frame, lane, k))
 
-    def finish_e2e():
+        def finish_e2e():
+            for lane in lanes:
+                for fut in lane["pending"]:
+                    fut.result()
+                lane["pending"].clear()
+
+        for b in bufs:
+            b["out"] = None
+        torch.cuda.empty_cache()
+        for k in range(max(min(warmup, 3), F)):
+            step_e2e(k)
+        finish_e2e()
+        ms_e2e = timed(step_e2e, warmup, steps, finish=finish_e2e)
         for lane in lanes:
-            for fut in lane["pending"]:
-                fut.result()
-            lane["pending"].clear()
-
-    for b in bufs:
-        b["out"] = None
-    torch.cuda.empty_cache()
-    for k in range(max(min(args.warmup, 3), F)):
-        step_e2e(k)
-    finish_e2e()
-    ms_e2e = timed(step_e2e, args.warmup, args.steps, finish=finish_e2e)
-    for lane in lanes:
-        lane["pool"].shutdown()
-    n_pairs = int(wl.idx_without[0].size)
-    e2e = {"value": B * args.steps * world / (ms_e2e * 1e-3), "unit": "states/s",
-           "h2d_bytes_per_step": int(B * Cn + 3 * 4 * n_pairs), "d2h_bytes_per_step": int(B * 8 + B * 4 + G * 72),
-           "ms_per_step": ms_e2e / args.steps,
-           "host_threads": F,
-           "note": "gsr_utility_frame_host: pinned host levels/pairs in, mse/psnr/utilities out; images materialised on device; %d host threads, one stream + workspace each" % F}
+            lane["pool"].shutdown()
+        n_pairs = int(wl.idx_without[0].size)
+        e2e = {"value": B * steps * world / (ms_e2e * 1e-3), "unit": "states/s",
+               "h2d_bytes_per_step": int(B * Cn + 3 * 4 * n_pairs), "d2h_bytes_per_step": int(B * 8 + B * 4 + G * 72),
+               "ms_per_step": ms_e2e / steps,
+               "host_threads": F,
+               "note": "gsr_utility_frame_host: pinned host levels/pairs in, mse/psnr/utilities out; images materialised on device; %d host threads, one stream + workspace each" % F}
 
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
-        return
+        return None
+    for b in bufs:
+        b["out"] = None
+    torch.cuda.empty_cache()
 
     # ---- roofline of the dominant kernel (k_composite): counted work / CUDA-event time / FP32 peak
     bufs[0]["out"] = torch.empty((B, H, W, 3), dtype=torch.float32, device=dev)
-    n_cnt = min(args.steps, 6)
+    n_cnt = min(steps, 6)
     cnt = np.zeros(3, np.float64)
-    for k in range(args.warmup, args.warmup + n_cnt):
+    for k in range(warmup, warmup + n_cnt):
         step_serial(k)
         cnt += scene.debug_pair_counts(ws)
-    cnt *= args.steps / n_cnt                       # scaled to the timed region (frames are statistically alike)
+    cnt *= steps / n_cnt                       # scaled to the timed region (frames are statistically alike)
     comp_s = comp_ms * 1e-3
     flop_alg = cnt[0] * FLOP_SHARED + cnt[1] * FLOP_STATE
     peak_meas = gsr.measure_fp32_peak()
@@ -376,12 +441,12 @@ def run_ours(args):
                 "peak_kind": "measured here: FFMA-chain kernel (gsr_measure_fp32_peak); nominal %.1f" % NOMINAL_FP32_TFLOPS,
                 "kernel_ms_per_launch": comp_ms / max(comp_n, 1), "kernel_launches": comp_n,
                 "kernel_share_of_step": comp_ms / ms_serial,
-                "measured_on": "the same %d steps run one frame at a time (%.3f ms/step), CUDA events around every launch" % (args.steps, ms_serial / args.steps),
-                "alpha_evals_per_step": cnt[0] / args.steps, "state_updates_per_step": cnt[1] / args.steps,
-                "logical_pairs_per_step": cnt[2] / args.steps,
+                "measured_on": "the same %d steps run one frame at a time (%.3f ms/step), CUDA events around every launch" % (steps, ms_serial / steps),
+                "alpha_evals_per_step": cnt[0] / steps, "state_updates_per_step": cnt[1] / steps,
+                "logical_pairs_per_step": cnt[2] / steps,
                 "literal_equiv_tflops": cnt[2] * FLOP_LITERAL / comp_s / 1e12 if comp_s > 0 else 0.0,
                 "literal_equiv_frac": (cnt[2] * FLOP_LITERAL / comp_s / 1e12 / peak_meas) if comp_s > 0 and peak_meas else None,
-                "image_write_gbs": B * H * W * 12 * args.steps / comp_s / 1e9 if comp_s > 0 else None}
+                "image_write_gbs": B * H * W * 12 * steps / comp_s / 1e9 if comp_s > 0 else None}
     # ---- the memory-bound phases a1-a3 against the HBM roofline (algorithmic bytes per unit)
     K = (wl.scene.sh_degree + 1) ** 2
     n_rec = scene.V * wl.scene.N
@@ -410,18 +475,14 @@ def run_ours(args):
                                "frac": sg / hbm_peak, "radix_passes": passes, "launches_per_frame": 5 + 3 * passes,
                                "note": "latency-bound at this key count (%d keys): many small dependent launches" % keys},
                   "share_of_step": (proj_ms + sort_ms) / ms_serial}
-    tp = Path(ROOT / "profiles" / "traffic.txt")     # ncu DRAM bytes per launch of this kernel (see the file header)
-    if tp.exists():
-        for ln in tp.read_text().splitlines():
-            f = ln.split()
-            if len(f) == 2 and not ln.startswith("#") and f[0] == wl.name:
-                roofline["traffic"] = int(f[1])
+    roofline.update(traffic_record(wl.name))
 
     # ---- CPU oracle on this box's cores, bounded sample of the same workload
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        n_s = min(4 * args.ref_states, B)          # cfg1: all 256 states of two frames, ~15 s of CPU work
-        f0, f1 = frame_of(args.warmup), frame_of(args.warmup + 1)
+        # cfg1 (the bench line): all 256 states of two frames, ~15 s of CPU work; sub-records: 16 states of two frames
+        n_s = min(4 * args.ref_states, B) if full else min(16, B)
+        f0, f1 = frame_of(warmup), frame_of(warmup + 1)
         dt0, cores = oracle_sample(wl, f0, n_s)
         dt1, _ = oracle_sample(wl, f1, n_s)
         dt = dt0 + dt1
@@ -429,8 +490,8 @@ def run_ours(args):
                "sample": f"first {n_s} of {B} states of frames {f0} and {f1} (+ the full-state reference render and MSE/PSNR of each), {dt:.1f} s"}
 
     line = {"metric": "counterfactual_state_renders_per_s", "value": value, "unit": "states/s",
-            "mpix_states_per_s": value * W * H / 1e6, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms / args.steps, "ms_per_step_one_frame_in_flight": ms_serial / args.steps,
+            "mpix_states_per_s": value * W * H / 1e6, "n_gpus": world, "steps": steps, "warmup": warmup,
+            "ms_per_step": ms / steps, "ms_per_step_one_frame_in_flight": ms_serial / steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": wl.name, "states_per_frame": B, "resolution": [W, H], "gaussians": wl.scene.N,
@@ -438,18 +499,24 @@ def run_ours(args):
                        "images_materialised": True, "frames_in_flight": F, "state_block": args.state_block or "default", "keys_per_frame": keys,
                        "l2": "per-step working set (%.2f GB of images written) exceeds the 126 MB L2; every step is a different frame" % (B * H * W * 12 / 1e9),
                        "parallelism": "frames sharded over ranks, no collective" if world > 1 else "1 GPU"},
-            "value_without_images": B * args.steps * world / (ms_noimg * 1e-3),
-            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "memory_phases": phases,
-            "cpu_baseline": cpu,
-            "context": {"paper_h100_pcie_utility_states_per_s": 1889.7,
-                        "note": "PAPER.md:150, other hardware, unstated resolution/scene: context only"}}
-    print(json.dumps(line))
+            "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline, "memory_phases": phases,
+            "cpu_baseline": cpu}
+    if full:
+        line.update({"repetitions": n_rep, "value_reps": value_reps, "value_ci95": ci95,
+                     "ms_per_step_reps": [m / steps for m in ms_reps], "sustained": sustained,
+                     "value_without_images": B * steps * world / (ms_noimg * 1e-3), "e2e": e2e,
+                     "context": {"paper_h100_pcie_utility_states_per_s": 1889.7,
+                                 "note": "PAPER.md:150, other hardware, unstated resolution/scene: context only"}})
     if dist is not None:
         dist.destroy_process_group()
+    scene.close()
+    del bufs, lv_dev
+    torch.cuda.empty_cache()
+    return line
 
 
 # ------------------------------------------------------------------------------------------------ atlas workload
-def run_atlas(args):
+def measure_atlas(args, steps: int, warmup: int, full: bool):
     """--workload atlas.  A step = one view of the partial-state atlas:
     utility sweep (2 x 4C x n_ctx states, fused distortion) -> Eq. (3)-(4) -> three policy orders -> frontier
     states at 4 matched budgets -> 8197 sampled states + 12 frontier states rendered (fused distortion, no
@@ -463,7 +530,7 @@ def run_atlas(args):
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
     torch.cuda.set_device(0)
     dev = torch.device("cuda", 0)
-    n_views = max(1, min(args.steps + args.warmup, 4))
+    n_views = max(1, min(steps + warmup, 4))
     wl = synth.workload_atlas(n_views=n_views)
     scene = gsr.Scene(wl.scene)
     Cn, G = wl.scene.C, wl.G
@@ -513,7 +580,7 @@ def run_atlas(args):
         torch.cuda.synchronize()
         return e0.elapsed_time(e1)
 
-    for k in range(args.warmup):
+    for k in range(warmup):
         step(k)
     scene.status(ws)
     gsr.set_option("profile", 1)
@@ -521,14 +588,14 @@ def run_atlas(args):
     sampler = ClockSampler(0)
     sampler.start()
     sampler.mark()
-    ms = timed(step, args.warmup, args.steps)
+    ms = timed(step, warmup, steps)
     clocks = sampler.stop()
     launches = gsr.launch_count() - l0
     comp_ms, comp_n = gsr.profile_read()
     gsr.set_option("profile", 0)
     scene.status(ws)
     states_per_step = Bs + Bt
-    value = states_per_step * args.steps / (ms * 1e-3)
+    value = states_per_step * steps / (ms * 1e-3)
 
     # end to end: pinned host levels in, every result of the step back on the host
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
@@ -547,20 +614,22 @@ def run_atlas(args):
         h_out["util"].copy_(util, non_blocking=True)
         torch.cuda.current_stream().synchronize()
 
-    step_e2e(0)
-    ms_e2e = timed(step_e2e, args.warmup, args.steps)
-    e2e = {"value": states_per_step * args.steps / (ms_e2e * 1e-3), "unit": "states/s",
-           "h2d_bytes_per_step": int((Bs + Ba) * Cn), "d2h_bytes_per_step": int(Bt * 12 + nb * 4 + G * 72),
-           "ms_per_step": ms_e2e / args.steps}
+    e2e = None
+    if full:
+        step_e2e(0)
+        ms_e2e = timed(step_e2e, warmup, steps)
+        e2e = {"value": states_per_step * steps / (ms_e2e * 1e-3), "unit": "states/s",
+               "h2d_bytes_per_step": int((Bs + Ba) * Cn), "d2h_bytes_per_step": int(Bt * 12 + nb * 4 + G * 72),
+               "ms_per_step": ms_e2e / steps}
 
     # roofline of the dominant kernel, counted work of the two render calls of one step
     cnt = np.zeros(3, np.float64)
-    f = args.warmup % n_frames
+    f = warmup % n_frames
     scene.render_states_vs_full(cams[f], ts[f], sweep[f], ws, ref, mse_s, psnr_s, out=None)
     cnt += scene.debug_pair_counts(ws)
     scene.render_states_vs_full(cams[f], ts[f], batch[f], ws, ref, mse_a, psnr_a, out=None)
     cnt += scene.debug_pair_counts(ws)
-    comp_s = comp_ms * 1e-3 / args.steps
+    comp_s = comp_ms * 1e-3 / steps
     peak = gsr.measure_fp32_peak()
     achieved = (cnt[0] * FLOP_SHARED + cnt[1] * FLOP_STATE) / comp_s / 1e12
     roofline = {"kernel": "k_composite", "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
@@ -581,7 +650,7 @@ def run_atlas(args):
     if not args.no_cpu_baseline:
         from oracle import oracle as O
         osc = O.OracleScene(wl.scene)
-        n_s = min(args.ref_states, Ba)
+        n_s = min(args.ref_states if full else 16, Ba)
         cam, t = wl.frames[f]
         t0 = time.perf_counter()
         imgs, _ = osc.render_batch(cam, t, np.concatenate([wl.atlas_levels[f][:n_s], np.full((1, Cn), 3, np.int8)]))
@@ -590,8 +659,8 @@ def run_atlas(args):
         cpu = {"value": n_s / dt, "unit": "states/s", "cores": O.num_threads(), "kind": "oracle",
                "sample": f"first {n_s} of {Ba} atlas states of view {f} (+ full-state reference and MSE/PSNR), {dt:.1f} s"}
     line = {"metric": "counterfactual_state_renders_per_s", "value": value, "unit": "states/s",
-            "mpix_states_per_s": value * W * H / 1e6, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms / args.steps,
+            "mpix_states_per_s": value * W * H / 1e6, "n_gpus": 1, "steps": steps, "warmup": warmup,
+            "ms_per_step": ms / steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": wl.name, "states_per_step": states_per_step, "sweep_states": Bs, "atlas_states": Ba,
@@ -600,6 +669,41 @@ def run_atlas(args):
                        "l2": "each step projects, sorts and composites a different view; no output is re-read"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
             "atlas": result}
+    scene.close()
+    return line
+
+
+
+SUB_WORKLOADS = ("cfg2", "cfg3", "cfg4", "atlas")
+
+
+def run_ours(args):
+    """The N = 1 bench line: configs[1] in full (repetitions, CI, sustained pass, end-to-end, roofline, CPU sample) and
+    — SURVEY.md §8(d), BASELINE.md "what we will measure" — a compact sub-record for each other workload."""
+    if args.workload == "atlas":
+        line = measure_atlas(args, args.steps, args.warmup, full=True)
+    else:
+        line = measure_ours(args, args.workload, args.steps, args.warmup, full=True)
+    if line is None:                      # ranks other than 0
+        return
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.workload == "cfg1" and world == 1 and not args.no_sub_workloads:
+        subs = {}
+        for name in SUB_WORKLOADS:
+            t0 = time.perf_counter()
+            try:
+                sub = measure_atlas(args, 2, 2, full=False) if name == "atlas" else measure_ours(args, name, 3, 3, full=False)
+                keep = ("value", "unit", "mpix_states_per_s", "steps", "warmup", "ms_per_step", "config", "clocks",
+                        "gpu_launches", "cpu_baseline")
+                rec = {k: sub[k] for k in keep if k in sub}
+                r = sub["roofline"]
+                rec["roofline"] = {k: r[k] for k in ("kernel", "bound", "achieved", "peak", "unit", "frac",
+                                                     "kernel_share_of_step") if k in r}
+                rec["wall_s"] = time.perf_counter() - t0
+                subs[name] = rec
+            except Exception as e:  # noqa: BLE001  a sub-record must never cost the headline line
+                subs[name] = {"error": repr(e)}
+        line["workloads"] = subs
     print(json.dumps(line))
 
 
@@ -612,16 +716,28 @@ def main():
     ap.add_argument("--workload", default="cfg1", choices=["cfg0", "cfg1", "cfg1r", "cfg2", "cfg3", "cfg4", "atlas"])
     ap.add_argument("--ref-states", type=int, default=64, help="states per frame the CPU oracle renders")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sub-workloads", action="store_true",
+                    help="cfg1 only: skip the compact cfg2 / cfg3 / cfg4 / atlas sub-records")
     ap.add_argument("--state-block", type=int, default=0, help="states per compositing CTA (0 = library default)")
     ap.add_argument("--frames-in-flight", type=int, default=4,
                     help="frames pipelined on separate CUDA streams, each with its own workspace and outputs")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
-    elif args.workload == "atlas":
-        run_atlas(args)
-    else:
-        run_ours(args)
+        return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # started without torchrun: start the N ranks here (one process per GPU, NCCL only for the barrier and
+        # the max-over-ranks time); a box with fewer GPUs fails loudly instead of timing one GPU
+        import torch
+        n_dev = torch.cuda.device_count()
+        if n_dev < args.gpus:
+            raise SystemExit(f"bench.py: --gpus {args.gpus} but this box has {n_dev} CUDA device(s)")
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--standalone", "--nnodes=1",
+               f"--nproc-per-node={args.gpus}", "--local-addr", "127.0.0.1", str(Path(__file__).resolve()), *sys.argv[1:]]
+        os.environ.setdefault("NCCL_DEBUG", "INFO")      # the init log (on stderr) lets the driver count the ranks
+        os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")
+        raise SystemExit(subprocess.call(cmd))
+    run_ours(args)
 
 
 if __name__ == "__main__":
