@@ -452,11 +452,9 @@ def measure_ours(args, workload: str, steps: int, warmup: int, full: bool):
     n_rec = scene.V * wl.scene.N
     b_gauss = 48 + 2 * 16 * ((3 * K + 3) // 4) + 4 * ((3 * wl.scene.R + 3) // 4) + (24 if scene.V == 4 else 0)
     proj_bytes = wl.scene.N * b_gauss + n_rec * 88
-    tiles = ((W + 15) // 16) * ((H + 15) // 16)
-    tile_bits = max(1, int(np.ceil(np.log2(tiles))))
-    passes = (32 + tile_bits + 7) // 8
-    passes += passes & 1
-    sort_bytes = n_rec * 16 + keys * 12 + passes * keys * 32 + keys * 8
+    # a3 (k_sort.cu): count pass reads count + rect (12 B / record); the scatter reads them again with the depth
+    # bits (16 B / record) and writes 8 B / key; the per-tile sort reads 8 B and writes 12 B / key
+    sort_bytes = n_rec * 28 + keys * 28
     hbm_peak, hbm_kind = 6650.0, "fallback (B200_PROFILING.md)"
     mp = ROOT / "MEASURED_PEAKS.json"
     if mp.exists():
@@ -472,8 +470,8 @@ def measure_ours(args, workload: str, steps: int, warmup: int, full: bool):
                   "project": {"ms_per_frame": proj_ms / ph_n, "algorithmic_bytes": int(proj_bytes), "achieved": pg,
                               "frac": pg / hbm_peak},
                   "bin_sort": {"ms_per_frame": sort_ms / ph_n, "algorithmic_bytes": int(sort_bytes), "achieved": sg,
-                               "frac": sg / hbm_peak, "radix_passes": passes, "launches_per_frame": 5 + 3 * passes,
-                               "note": "latency-bound at this key count (%d keys): many small dependent launches" % keys},
+                               "frac": sg / hbm_peak, "launches_per_frame": 3,
+                               "note": "counting sort by tile + one bitonic sort per tile segment (%d keys)" % keys},
                   "share_of_step": (proj_ms + sort_ms) / ms_serial}
     roofline.update(traffic_record(wl.name))
 

@@ -88,13 +88,11 @@ size_t carve_workspace(Workspace* ws, void* base, int32_t N, int32_t C, int32_t 
   w.rect = (uint2*)take(sizeof(uint2) * n_rec);
   w.depth_bits = (uint32_t*)take(sizeof(uint32_t) * n_rec);
   w.count = (uint32_t*)take(sizeof(uint32_t) * n_rec);
-  w.offset = (uint32_t*)take(sizeof(uint32_t) * (n_rec + 1));
-  w.scan_blk = (uint32_t*)take(sizeof(uint32_t) * (n_rec / 2048 + 2));
   for (int k = 0; k < 2; ++k) {
     w.keys[k] = (unsigned long long*)take(sizeof(unsigned long long) * (size_t)cap);
     w.vals[k] = (uint32_t*)take(sizeof(uint32_t) * (size_t)cap);
   }
-  w.hist = (uint32_t*)take(sizeof(uint32_t) * 256 * ((size_t)cap / kSortTileKeys + 2));
+  w.tile_cursor = (uint32_t*)take(sizeof(uint32_t) * (size_t)tiles);
   w.tile_range = (uint2*)take(sizeof(uint2) * (size_t)tiles);
   w.render_range = (uint2*)take(sizeof(uint2) * (size_t)tiles);
   w.state_counts = (long long*)take(sizeof(long long) * (size_t)(B > 0 ? B : 1));

@@ -10,6 +10,7 @@
 namespace gsr {
 
 constexpr int kTile = GSR_TILE;
+
 constexpr int kTilePix = kTile * kTile;  // 256 threads per compositing CTA, one per pixel
 constexpr int kMaxC = 4096;              // clusters (mask table lives in shared memory)
 
@@ -69,11 +70,9 @@ struct Workspace {
   uint2* rect;            // [2N] 4 x u16: tx0,ty0,tx1,ty1
   uint32_t* depth_bits;   // [2N]
   uint32_t* count;        // [2N]
-  uint32_t* offset;       // [2N+1] exclusive scan of count
-  uint32_t* scan_blk;     // block sums of the scan
-  unsigned long long* keys[2];  // [cap] (tile<<32 | depth bits)
-  uint32_t* vals[2];            // [cap] record id
-  uint32_t* hist;         // [256 * n_sort_blocks]
+  unsigned long long* keys[2];  // [cap] [0]: sorted (tile<<32 | depth bits); [1]: per-tile segments of (depth bits<<32 | record id) before the sort
+  uint32_t* vals[2];            // [cap] [0]: record ids of the sorted list; [1]: the render list (k_tile_render_list)
+  uint32_t* tile_cursor;  // [tiles] keys per tile, then the write cursor of the tile's segment (k_sort.cu)
   uint2* tile_range;      // [tiles] start,end into the sorted list
   uint2* render_range;    // [tiles] start,end into the render list (vals[1]): the tile's records whose q <= tau
                           // box touches a pixel of the tile, in list order (k_tile_render_list)
@@ -145,9 +144,6 @@ __device__ __forceinline__ uint32_t record_block_mask_tight(float mx, float my, 
   return m;
 }
 
-constexpr int kSortThreads = 256;
-constexpr int kSortItems = 4;
-constexpr int kSortTileKeys = kSortThreads * kSortItems;  // keys per block per pass
 
 size_t carve_workspace(Workspace* ws, void* base, int32_t N, int32_t C, int32_t B, int32_t tiles, long long cap);
 long long default_key_capacity(int32_t N);

@@ -191,7 +191,9 @@ __device__ __forceinline__ void sh_dir(const FrameParams& fp, const float mu[3],
   sh_eval<K>(dx * inv, dy * inv, dz * inv, Y);
 }
 
-__device__ __forceinline__ void store_record(Workspace& ws, uint32_t rid, const Proj& p, float opac, float tau,
+// Also the first step of the binning (k_sort.cu): one increment per tile of the record's rectangle.  The
+// increments are fire-and-forget reductions that overlap the kernel's own memory latency.
+__device__ __forceinline__ void store_record(Workspace& ws, int TX, uint32_t rid, const Proj& p, float opac, float tau,
                                              uint32_t meta, const float* c0, const float* c1) {
   ws.r0[rid] = make_float4(p.mx, p.my, p.qa, p.qb);
   ws.r1[rid] = make_float4(p.qc, opac, tau, __uint_as_float(meta));
@@ -201,6 +203,9 @@ __device__ __forceinline__ void store_record(Workspace& ws, uint32_t rid, const 
   ws.rect[rid] = make_uint2((uint32_t)p.tx0 | ((uint32_t)p.ty0 << 16), (uint32_t)p.tx1 | ((uint32_t)p.ty1 << 16));
   ws.depth_bits[rid] = p.depth_bits;
   ws.count[rid] = p.count;
+  if (p.count != 0)
+    for (int ty = p.ty0; ty < p.ty1; ++ty)
+      for (int tx = p.tx0; tx < p.tx1; ++tx) atomicAdd(ws.tile_cursor + ty * TX + tx, 1u);
 }
 
 // reading I4 (optional): Sigma_t = L Sigma L^T, L = the 3x3 part of A_c(t); binary32 in the written order of
@@ -301,8 +306,8 @@ __global__ void __launch_bounds__(128) k_project(DeviceScene sc, FrameParams fp,
     }
   }
   // record class: 0 = variant A (depth == 0), 1 + lvl = variant B of a level-lvl Gaussian
-  store_record(ws, 2u * i + 0u, pa, opac, tau, (uint32_t)c | (0u << 16), cA, cA);
-  store_record(ws, 2u * i + 1u, pb, opac, tau, (uint32_t)c | ((uint32_t)(1 + lvl) << 16), cB0, cB1);
+  store_record(ws, fp.TX, 2u * i + 0u, pa, opac, tau, (uint32_t)c | (0u << 16), cA, cA);
+  store_record(ws, fp.TX, 2u * i + 1u, pb, opac, tau, (uint32_t)c | ((uint32_t)(1 + lvl) << 16), cB0, cB1);
 }
 
 // K1 with the position residual levels of Eq. (1) (reading I1): a Gaussian has one geometry per
@@ -407,10 +412,11 @@ __global__ void __launch_bounds__(128) k_project4(DeviceScene sc, FrameParams fp
   }
 #pragma unroll
   for (int v = 0; v < 4; ++v)
-    store_record(ws, 4u * i + (uint32_t)v, pr[v], opv[v], tauv[v], (uint32_t)c | ((uint32_t)(16 + v) << 16), col[v], col[v]);
+    store_record(ws, fp.TX, 4u * i + (uint32_t)v, pr[v], opv[v], tauv[v], (uint32_t)c | ((uint32_t)(16 + v) << 16), col[v], col[v]);
 }
 
 void launch_project(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, cudaStream_t st) {
+  cudaMemsetAsync(ws.tile_cursor, 0, sizeof(uint32_t) * (size_t)fp.TX * fp.TY, st);  // keys per tile, counted below
   if (sc.N == 0) return;
   dim3 grid((sc.N + 127) / 128), block(128);
   if (sc.V == 4) {

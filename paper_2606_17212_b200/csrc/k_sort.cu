@@ -1,28 +1,29 @@
 // k_sort.cu — stage a3 of the hot path: tile binning and the key sort.
 //
-//   K2a  exclusive scan of the per-record tile counts (warp-shuffle segmented scan, 3 phases)
-//   K2b  key emission: (tile << 32 | depth bits) with the record id as payload, written at
-//        scan offsets — i.e. in ascending record order, no atomics, so the emission is deterministic
-//   K3   stable LSD radix sort, 8-bit digits over the 32 + ceil(log2 tiles) significant key bits;
-//        ties in (tile, depth) keep emission order = ascending record id = ascending
-//        (Gaussian index, variant), which is exactly the (tile, depth, index) order of the spec
-//   K3b  per-tile [start, end) ranges
+// The spec's order inside a tile is (depth bits, Gaussian index, variant) = (depth bits, record id), and a
+// (depth bits, record id) pair is unique: the sorted list of a tile is a function of its SET of keys.  The sort
+// therefore does not have to be stable or to see the keys in any particular order, which allows a counting sort
+// by tile followed by an independent sort of every tile's segment — 3 kernels per frame (plus the counting inside k_project) instead of a 6-pass
+// global radix sort (23 launches, each pass re-reading and re-writing every key):
+//   K2a  (in k_project)  per record: one atomic increment per tile of its rectangle        -> tile_cursor
+//   K2b  k_tile_offsets  one CTA: exclusive scan over the tiles -> tile_range (start, end), the total number of
+//                        keys -> header (capacity check), cursors reset to the segment starts
+//   K2c  k_scatter_keys  per record: (depth bits << 32 | record id) into its tiles' segments (atomic cursor: the
+//                        order inside a segment is arbitrary at this point)
+//   K3   k_tile_sort     one CTA per tile: bitonic sort of the segment by the 64-bit key — in shared memory up to
+//                        4096 keys, in place in global memory beyond — then the canonical arrays
+//                        keys[0] = (tile << 32 | depth bits), vals[0] = record id that the parity exports read
 //
 // The state field of the spec's (state, tile, depth, index) key is factored out: the sorted list
 // of state b is the restriction of this per-frame superset list to the records present in b
 // (DESIGN.md §4.2).  k_filter_keys materialises it for the bit-exact parity check and
 // k_state_counts gives its length I_b for every state of the batch.
 //
-// All sizes that depend on the data (number of keys) stay on the device: grids are sized for the
-// key capacity and read the actual count from the workspace header, so the whole path is
-// asynchronous on the caller's stream.
+// All sizes that depend on the data (number of keys) stay on the device, so the whole path is asynchronous on
+// the caller's stream.
 #include "gsr_internal.h"
 
 namespace gsr {
-
-// ------------------------------------------------------------------------------------------------
-// K2a: exclusive scan over n uint32 (n <= 2^31), block = 256 threads x 8 items
-constexpr int kScanThreads = 256, kScanItems = 8, kScanTile = kScanThreads * kScanItems;
 
 __device__ __forceinline__ uint32_t warp_incl_scan(uint32_t v) {
 #pragma unroll
@@ -51,248 +52,135 @@ __device__ __forceinline__ uint32_t block_excl_scan_256(uint32_t v, uint32_t* sm
   return woff + inc - v;
 }
 
-__global__ void __launch_bounds__(kScanThreads) k_scan_block_sums(const uint32_t* __restrict__ in, int n,
-                                                                  uint32_t* __restrict__ blk) {
-  __shared__ uint32_t sm[8];
-  int base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
-  uint32_t s = 0;
-#pragma unroll
-  for (int k = 0; k < kScanItems; ++k)
-    if (base + k < n) s += in[base + k];
-  uint32_t tot;
-  block_excl_scan_256(s, sm, &tot);
-  if (threadIdx.x == 0) blk[blockIdx.x] = tot;
-}
-
-// single CTA: exclusive scan of the block sums in place; total (64-bit) -> header; capacity check
-__global__ void __launch_bounds__(kScanThreads) k_scan_top(uint32_t* __restrict__ blk, int nblk, WsHeader* hdr) {
+// ------------------------------------------------------------------------------------------------
+// K2b: one CTA.  tile_range[t] = [start, end) of tile t's segment, cursor[t] = start; total -> header.
+__global__ void __launch_bounds__(256) k_tile_offsets(uint32_t* __restrict__ tile_cursor, int tiles,
+                                                      uint2* __restrict__ tile_range, WsHeader* hdr) {
   __shared__ uint32_t sm[8];
   __shared__ unsigned long long carry_s;
   if (threadIdx.x == 0) carry_s = 0ull;
   __syncthreads();
-  for (int base = 0; base < nblk; base += kScanThreads) {
-    int i = base + threadIdx.x;
-    uint32_t v = i < nblk ? blk[i] : 0u;
-    uint32_t tot;
-    uint32_t ex = block_excl_scan_256(v, sm, &tot);
-    unsigned long long carry = carry_s;
-    if (i < nblk) blk[i] = (uint32_t)(carry + ex);  // meaningful only while the total fits the capacity (< 2^31)
-    __syncthreads();
-    if (threadIdx.x == 0) carry_s = carry + tot;
-    __syncthreads();
-  }
+  // first the total (64-bit) and the capacity check: beyond the capacity nothing is binned at all
+  unsigned long long part = 0;
+  for (int i = threadIdx.x; i < tiles; i += 256) part += tile_cursor[i];
+  for (int off = 16; off > 0; off >>= 1) part += __shfl_xor_sync(0xffffffffu, part, off);
+  __shared__ unsigned long long s_part[8];
+  if ((threadIdx.x & 31) == 0) s_part[threadIdx.x >> 5] = part;
+  __syncthreads();
+  unsigned long long total = 0;
+  for (int k = 0; k < 8; ++k) total += s_part[k];
+  const bool fits = (long long)total <= hdr->key_capacity;
   if (threadIdx.x == 0) {
-    unsigned long long total = carry_s;
     hdr->total_keys = total;
-    if ((long long)total > hdr->key_capacity) {
-      atomicMin(&hdr->status, GSR_E_WORKSPACE_TOO_SMALL);
-      hdr->n_keys = 0ull;  // render nothing rather than a truncated (wrong) list
-    } else {
-      hdr->n_keys = total;
+    if (!fits) atomicMin(&hdr->status, GSR_E_WORKSPACE_TOO_SMALL);
+    hdr->n_keys = fits ? total : 0ull;  // render nothing rather than a truncated (wrong) list
+  }
+  for (int base = 0; base < tiles; base += 256) {
+    const int i = base + threadIdx.x;
+    const uint32_t v = (i < tiles && fits) ? tile_cursor[i] : 0u;
+    uint32_t tot;
+    const uint32_t ex = block_excl_scan_256(v, sm, &tot);
+    const uint32_t start = (uint32_t)carry_s + ex;
+    if (i < tiles) {
+      tile_range[i] = make_uint2(start, start + v);
+      tile_cursor[i] = start;
     }
-  }
-}
-
-__global__ void __launch_bounds__(kScanThreads) k_scan_apply(const uint32_t* __restrict__ in, int n,
-                                                             const uint32_t* __restrict__ blk,
-                                                             uint32_t* __restrict__ out) {
-  __shared__ uint32_t sm[8];
-  int base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
-  uint32_t v[kScanItems], s = 0;
-#pragma unroll
-  for (int k = 0; k < kScanItems; ++k) {
-    v[k] = (base + k < n) ? in[base + k] : 0u;
-    s += v[k];
-  }
-  uint32_t tot;
-  uint32_t ex = block_excl_scan_256(s, sm, &tot) + blk[blockIdx.x];
-#pragma unroll
-  for (int k = 0; k < kScanItems; ++k) {
-    if (base + k < n) out[base + k] = ex;
-    ex += v[k];
-  }
-  if (blockIdx.x == gridDim.x - 1 && threadIdx.x == kScanThreads - 1) out[n] = ex;  // grand total (mod 2^32)
-}
-
-// ------------------------------------------------------------------------------------------------
-// K2b: one thread per record writes its count keys in (ty, tx) order at [offset, offset + count)
-__global__ void __launch_bounds__(256) k_emit_keys(int n_rec, const uint32_t* __restrict__ count,
-                                                   const uint32_t* __restrict__ offset,
-                                                   const uint2* __restrict__ rect,
-                                                   const uint32_t* __restrict__ depth_bits, int TX,
-                                                   const WsHeader* __restrict__ hdr,
-                                                   unsigned long long* __restrict__ keys,
-                                                   uint32_t* __restrict__ vals) {
-  int r = blockIdx.x * blockDim.x + threadIdx.x;
-  if (r >= n_rec) return;
-  if (hdr->n_keys == 0ull) return;
-  uint32_t cnt = count[r];
-  if (cnt == 0) return;
-  uint32_t o = offset[r];
-  uint2 rc = rect[r];
-  int tx0 = rc.x & 0xFFFF, ty0 = rc.x >> 16, tx1 = rc.y & 0xFFFF, ty1 = rc.y >> 16;
-  unsigned long long d = depth_bits[r];
-  for (int ty = ty0; ty < ty1; ++ty)
-    for (int tx = tx0; tx < tx1; ++tx) {
-      keys[o] = ((unsigned long long)(uint32_t)(ty * TX + tx) << 32) | d;
-      vals[o] = (uint32_t)r;
-      ++o;
-    }
-}
-
-// ------------------------------------------------------------------------------------------------
-// K3: stable LSD radix sort, one 8-bit digit per pass.
-//   hist    : per-block digit counts, layout [digit][block]
-//   scan    : exclusive scan over that array in (digit, block) order (single CTA)
-//   scatter : stable in-block ranking (warp match + per-warp counters), then write
-__global__ void __launch_bounds__(kSortThreads) k_radix_hist(const unsigned long long* __restrict__ keys,
-                                                            const WsHeader* __restrict__ hdr, int shift,
-                                                            uint32_t* __restrict__ hist) {
-  const unsigned long long n = hdr->n_keys;
-  const unsigned long long base = (unsigned long long)blockIdx.x * kSortTileKeys;
-  if (base >= n) return;
-  const uint32_t nblk = (uint32_t)((n + kSortTileKeys - 1) / kSortTileKeys);
-  __shared__ uint32_t h[256];
-  h[threadIdx.x] = 0;
-  __syncthreads();
-#pragma unroll 4
-  for (int k = 0; k < kSortItems; ++k) {
-    unsigned long long i = base + (unsigned long long)k * kSortThreads + threadIdx.x;
-    if (i < n) atomicAdd(&h[(uint32_t)(keys[i] >> shift) & 0xFFu], 1u);
-  }
-  __syncthreads();
-  hist[(size_t)threadIdx.x * nblk + blockIdx.x] = h[threadIdx.x];
-}
-
-// one warp per digit: exclusive prefix of that digit's per-block counts (in place) and the digit total,
-// stored behind the table at hist[256 * nblk + digit]; the scatter kernel scans the 256 totals itself
-__global__ void __launch_bounds__(256) k_radix_scan(uint32_t* __restrict__ hist, const WsHeader* __restrict__ hdr) {
-  const unsigned long long n = hdr->n_keys;
-  const uint32_t nblk = (uint32_t)((n + kSortTileKeys - 1) / kSortTileKeys);
-  const int lane = threadIdx.x & 31;
-  const uint32_t d = blockIdx.x * 8 + (threadIdx.x >> 5);
-  uint32_t* row = hist + (size_t)d * nblk;
-  uint32_t carry = 0;
-  for (uint32_t base = 0; base < nblk; base += 32) {
-    const uint32_t b = base + lane;
-    const uint32_t v = b < nblk ? row[b] : 0u;
-    const uint32_t inc = warp_incl_scan(v);
-    if (b < nblk) row[b] = carry + inc - v;
-    carry += __shfl_sync(0xffffffffu, inc, 31);
-  }
-  if (lane == 0) hist[(size_t)256 * nblk + d] = carry;
-}
-
-__global__ void __launch_bounds__(kSortThreads) k_radix_scatter(const unsigned long long* __restrict__ keys_in,
-                                                               const uint32_t* __restrict__ vals_in,
-                                                               unsigned long long* __restrict__ keys_out,
-                                                               uint32_t* __restrict__ vals_out,
-                                                               const WsHeader* __restrict__ hdr, int shift,
-                                                               const uint32_t* __restrict__ hist) {
-  const unsigned long long n = hdr->n_keys;
-  const unsigned long long base = (unsigned long long)blockIdx.x * kSortTileKeys;
-  if (base >= n) return;
-  const uint32_t nblk = (uint32_t)((n + kSortTileKeys - 1) / kSortTileKeys);
-  __shared__ uint32_t cnt[kSortThreads / 32][256];
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  for (int k = threadIdx.x; k < (kSortThreads / 32) * 256; k += kSortThreads) (&cnt[0][0])[k] = 0;
-  __syncthreads();
-  // warp w owns the contiguous chunk [base + w*512, base + (w+1)*512): stable order = (warp, round, lane)
-  unsigned long long key[kSortItems];
-  uint32_t val[kSortItems], rank[kSortItems];
-  const unsigned long long wbase = base + (unsigned long long)w * (32 * kSortItems);
-#pragma unroll
-  for (int k = 0; k < kSortItems; ++k) {
-    unsigned long long i = wbase + (unsigned long long)k * 32 + lane;
-    bool ok = i < n;
-    key[k] = ok ? keys_in[i] : ~0ull;
-    val[k] = ok ? vals_in[i] : 0u;
-  }
-#pragma unroll
-  for (int k = 0; k < kSortItems; ++k) {
-    unsigned long long i = wbase + (unsigned long long)k * 32 + lane;
-    bool ok = i < n;
-    uint32_t d = ok ? ((uint32_t)(key[k] >> shift) & 0xFFu) : 256u;  // 256 = "no key", never counted
-    uint32_t peers = __match_any_sync(0xffffffffu, d);
-    uint32_t lt = peers & ((1u << lane) - 1u);
-    uint32_t b = 0;
-    if (ok) b = cnt[w][d];
-    __syncwarp();
-    if (ok && lt == 0) cnt[w][d] = b + __popc(peers);
-    __syncwarp();
-    rank[k] = b + __popc(lt);
-  }
-  __syncthreads();
-  {  // per digit: exclusive prefix over warps + the block's global base
-    //   base(d) = sum of the totals of digits < d  +  this digit's count in earlier blocks
-    const int d = threadIdx.x;
-    __shared__ uint32_t s_w8[8];
-    const uint32_t tot = hist[(size_t)256 * nblk + d];
-    const uint32_t inc = warp_incl_scan(tot);
-    if (lane == 31) s_w8[w] = inc;
     __syncthreads();
-    uint32_t dbase = inc - tot;
-    for (int ww = 0; ww < w; ++ww) dbase += s_w8[ww];
-    uint32_t acc = hist[(size_t)d * nblk + blockIdx.x] + dbase;
-#pragma unroll
-    for (int ww = 0; ww < kSortThreads / 32; ++ww) {
-      uint32_t c = cnt[ww][d];
-      cnt[ww][d] = acc;
-      acc += c;
-    }
+    if (threadIdx.x == 0) carry_s += tot;
+    __syncthreads();
   }
-  __syncthreads();
-#pragma unroll
-  for (int k = 0; k < kSortItems; ++k) {
-    unsigned long long i = wbase + (unsigned long long)k * 32 + lane;
-    if (i < n) {
-      uint32_t d = (uint32_t)(key[k] >> shift) & 0xFFu;
-      uint32_t pos = cnt[w][d] + rank[k];
-      keys_out[pos] = key[k];
-      vals_out[pos] = val[k];
+}
+
+// K2c: every record writes (depth bits << 32 | record id) into the segment of each tile of its rectangle
+__global__ void __launch_bounds__(256) k_scatter_keys(int n_rec, const uint32_t* __restrict__ count,
+                                                      const uint2* __restrict__ rect,
+                                                      const uint32_t* __restrict__ depth_bits, int TX,
+                                                      const WsHeader* __restrict__ hdr,
+                                                      uint32_t* __restrict__ tile_cursor,
+                                                      unsigned long long* __restrict__ seg) {
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= n_rec || count[r] == 0 || hdr->n_keys == 0ull) return;
+  const uint2 rc = rect[r];
+  const int tx0 = rc.x & 0xFFFF, ty0 = rc.x >> 16, tx1 = rc.y & 0xFFFF, ty1 = rc.y >> 16;
+  const unsigned long long key = ((unsigned long long)depth_bits[r] << 32) | (uint32_t)r;
+  for (int ty = ty0; ty < ty1; ++ty)
+    for (int tx = tx0; tx < tx1; ++tx) seg[atomicAdd(tile_cursor + ty * TX + tx, 1u)] = key;
+}
+
+// ------------------------------------------------------------------------------------------------
+// K3: one CTA per tile sorts the tile's segment by (depth bits, record id) — keys are unique, so any correct sort
+// gives the one canonical order.  In shared memory when the segment fits (kSortSmemKeys), otherwise in place in
+// global memory (a tile with more than 4096 records: rare, and only slower; global writes of a step are visible to
+// the CTA's other threads after the barrier).  Writes the canonical arrays of the frame.
+constexpr int kSortThreads = 512;
+constexpr int kSortSmemKeys = 4096;
+
+// Bitonic sorting network in its all-ascending form (the first step of every merge compares mirrored partners,
+// the remaining steps are half-cleaners), over np2 = the next power of two >= n virtual elements of which those at
+// index >= n are +infinity.  Every compare-exchange puts the smaller key at the lower index, so a pair whose upper
+// index is >= n is a no-op and is skipped: the n real keys are sorted in place for any n.
+__device__ __forceinline__ void bitonic_sort(unsigned long long* a, uint32_t n, uint32_t np2) {
+  for (uint32_t size = 2; size <= np2; size <<= 1) {
+    for (uint32_t stride = size >> 1; stride > 0; stride >>= 1) {
+      const bool mirror = stride == (size >> 1);
+      for (uint32_t t = threadIdx.x; t < (np2 >> 1); t += kSortThreads) {
+        uint32_t lo, hi;
+        if (mirror) {
+          const uint32_t blk = t / stride, j = t - blk * stride;
+          lo = blk * size + j;
+          hi = blk * size + size - 1u - j;
+        } else {
+          lo = 2u * t - (t & (stride - 1u));
+          hi = lo + stride;
+        }
+        if (hi < n) {
+          const unsigned long long ka = a[lo], kb = a[hi];
+          if (ka > kb) { a[lo] = kb; a[hi] = ka; }
+        }
+      }
+      __syncthreads();
     }
   }
 }
 
-// K3b: tile ranges from the sorted keys
-__global__ void __launch_bounds__(256) k_tile_ranges(const unsigned long long* __restrict__ keys,
-                                                     const WsHeader* __restrict__ hdr, uint2* __restrict__ range) {
-  const unsigned long long n = hdr->n_keys;
-  for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
-       i += (unsigned long long)gridDim.x * blockDim.x) {
-    uint32_t t = (uint32_t)(keys[i] >> 32);
-    if (i == 0 || (uint32_t)(keys[i - 1] >> 32) != t) range[t].x = (uint32_t)i;
-    if (i + 1 == n || (uint32_t)(keys[i + 1] >> 32) != t) range[t].y = (uint32_t)(i + 1);
+__global__ void __launch_bounds__(kSortThreads) k_tile_sort(const uint2* __restrict__ tile_range,
+                                                           unsigned long long* __restrict__ seg,
+                                                           unsigned long long* __restrict__ keys_out,
+                                                           uint32_t* __restrict__ vals_out) {
+  __shared__ unsigned long long s_key[kSortSmemKeys];
+  const uint32_t tile = blockIdx.x;
+  const uint2 rg = tile_range[tile];
+  const uint32_t n = rg.y - rg.x;
+  if (n == 0) return;
+  uint32_t np2 = 1;
+  while (np2 < n) np2 <<= 1;
+  unsigned long long* a = seg + rg.x;
+  if (n <= kSortSmemKeys) {
+    for (uint32_t i = threadIdx.x; i < n; i += kSortThreads) s_key[i] = a[i];
+    a = s_key;
+    __syncthreads();
+  }
+  bitonic_sort(a, n, np2);
+  for (uint32_t i = threadIdx.x; i < n; i += kSortThreads) {
+    const unsigned long long k = a[i];
+    keys_out[rg.x + i] = ((unsigned long long)tile << 32) | (k >> 32);
+    vals_out[rg.x + i] = (uint32_t)k;
   }
 }
 
 void launch_bin_and_sort(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, long long cap,
                          cudaStream_t st) {
+  (void)cap;
   const int n_rec = sc.V * sc.N;
   const int tiles = fp.TX * fp.TY;
-  cudaMemsetAsync(ws.tile_range, 0, sizeof(uint2) * (size_t)tiles, st);
-  if (n_rec == 0) return;
-  const int nblk = (n_rec + kScanTile - 1) / kScanTile;
-  k_scan_block_sums<<<nblk, kScanThreads, 0, st>>>(ws.count, n_rec, ws.scan_blk);
-  k_scan_top<<<1, kScanThreads, 0, st>>>(ws.scan_blk, nblk, ws.hdr);
-  k_scan_apply<<<nblk, kScanThreads, 0, st>>>(ws.count, n_rec, ws.scan_blk, ws.offset);
-  k_emit_keys<<<(n_rec + 255) / 256, 256, 0, st>>>(n_rec, ws.count, ws.offset, ws.rect, ws.depth_bits, fp.TX,
-                                                   ws.hdr, ws.keys[0], ws.vals[0]);
-  // significant bits: 32 depth bits + tile bits, rounded up to whole 8-bit digits
-  int tile_bits = 1;
-  while ((1 << tile_bits) < tiles) ++tile_bits;
-  int passes = (32 + tile_bits + 7) / 8;
-  if (passes & 1) ++passes;  // an even number of passes leaves the result in buffer 0
-  const unsigned sort_blocks = (unsigned)((cap + kSortTileKeys - 1) / kSortTileKeys);
-  for (int p = 0; p < passes; ++p) {
-    const int in = p & 1, out = in ^ 1, shift = 8 * p;
-    k_radix_hist<<<sort_blocks, kSortThreads, 0, st>>>(ws.keys[in], ws.hdr, shift, ws.hist);
-    k_radix_scan<<<32, 256, 0, st>>>(ws.hist, ws.hdr);
-    k_radix_scatter<<<sort_blocks, kSortThreads, 0, st>>>(ws.keys[in], ws.vals[in], ws.keys[out], ws.vals[out],
-                                                          ws.hdr, shift, ws.hist);
+  const int grid = (n_rec + 255) / 256;
+  k_tile_offsets<<<1, 256, 0, st>>>(ws.tile_cursor, tiles, ws.tile_range, ws.hdr);
+  if (n_rec > 0) {
+    k_scatter_keys<<<grid, 256, 0, st>>>(n_rec, ws.count, ws.rect, ws.depth_bits, fp.TX, ws.hdr, ws.tile_cursor,
+                                         ws.keys[1]);
+    k_tile_sort<<<tiles, kSortThreads, 0, st>>>(ws.tile_range, ws.keys[1], ws.keys[0], ws.vals[0]);
   }
-  k_tile_ranges<<<148 * 8, 256, 0, st>>>(ws.keys[0], ws.hdr, ws.tile_range);
-  count_launches(4 + 3 * passes + 1);
+  count_launches(n_rec > 0 ? 3 : 1);
 }
 
 // ------------------------------------------------------------------------------------------------
