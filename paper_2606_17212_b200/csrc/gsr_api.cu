@@ -491,8 +491,6 @@ static int prepare_frame(const gsr_scene* scene, const gsr_camera* cam, float t,
   if (ph >= 0) cudaEventRecord(g_ph[ph][1], st);
   launch_bin_and_sort(s->d, *fp_out, *ws_out, cap, st);      // a3
   if (ph >= 0) cudaEventRecord(g_ph[ph][2], st);
-  launch_tile_render_list(*fp_out, *ws_out, st);             // a4 preparation: sub-tile culling, once per frame
-  launch_pack_records(s->d, *fp_out, *ws_out, st);
   return GSR_OK;
 }
 

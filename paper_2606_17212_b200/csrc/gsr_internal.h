@@ -78,7 +78,7 @@ struct Workspace {
                           // box touches a pixel of the tile, in list order (k_tile_render_list)
   long long* state_counts;  // [B]
   double* sse_blk;        // [B * tiles * 8] per-(state,tile,8x4 block) squared-error partials (fused distortion)
-  float4* rec;            // [4 * 2N] packed 64-byte records for the quadrant compositor (k_pack_records)
+  float4* rec;            // [4 * 2N] packed 64-byte records for the quadrant compositor (written by k_project)
   uint2* qlist;           // [4 * cap] per-(tile, quadrant) render lists of {record id, meta} (k_tile_render_list)
   uint2* qrange;          // [tiles * 4] start, end into qlist
   uint32_t* uorder;       // [tiles * B] states sorted by their tile-restricted signature (k_tile_dedup)
@@ -165,8 +165,6 @@ void launch_composite(const DeviceScene& sc, const FrameParams& fp, Workspace& w
 void launch_composite_count(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, const int8_t* depth_rows,
                             int32_t B, unsigned long long* counts, cudaStream_t st);
 void count_launches(int n);
-void launch_tile_render_list(const FrameParams& fp, Workspace& ws, cudaStream_t st);
-void launch_pack_records(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, cudaStream_t st);
 struct CompositeArgs;
 void launch_composite_q(const CompositeArgs& a, int S, bool count, cudaStream_t st);
 void launch_distortion_finalize_blk(const double* blk, int32_t B, int32_t tiles, int64_t n_values, double* mse,

@@ -14,7 +14,7 @@
 // Stop rule without a select: T keeps decaying after the stop and alpha >= 0 makes it non-increasing, so once
 // T < 1e-4 every later s is 0 and nothing is added any more (s is taken from the NEW T: "this Gaussian is not
 // added").  The frozen transmittance is not needed: pixel = C + T_stop bg with T_stop = 1 - sum of the accepted
-// w, hence pixel = bg + sum (s w)(c - bg); k_pack_records stores c - bg.  T, w and C are carried scaled by 2^40
+// w, hence pixel = bg + sum (s w)(c - bg); k_project stores c - bg in the packed records.  T, w and C are carried scaled by 2^40
 // (exact), which makes the step ONE saturating add with an immediate: s = sat(2^40 T - 2^40 pred(1e-4)):
 // neighbouring floats at 1e-4 are 2^-37 apart, so T >= 1e-4 gives >= 8 -> 1 and T <= pred(1e-4) gives <= 0 -> 0.
 //
@@ -99,29 +99,6 @@ __device__ __forceinline__ void cp_async_wait() {
 
 constexpr int kRecordUnroll = 2;
 constexpr int kChunk = 32;  // list entries staged per round: one per lane
-
-// Packed 64-byte records for the compositor, once per frame (every variant of every Gaussian):
-//   {m_x, m_y, A, B} {Cq, tau, o, meta} {rgb - bg, 0} {rgb with SH residual - bg, 0}
-__global__ void __launch_bounds__(256) k_pack_records(const float4* __restrict__ r0, const float4* __restrict__ r1,
-                                                      const float4* __restrict__ rc0, const float4* __restrict__ rc1,
-                                                      int n_rec, float bg0, float bg1, float bg2,
-                                                      float4* __restrict__ rec) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n_rec) return;
-  const float4 g1 = r1[i], c0 = rc0[i], c1 = rc1[i];
-  rec[4 * (size_t)i + 0] = r0[i];
-  rec[4 * (size_t)i + 1] = make_float4(g1.x, g1.z, g1.y, g1.w);
-  rec[4 * (size_t)i + 2] = make_float4(__fsub_rn(c0.x, bg0), __fsub_rn(c0.y, bg1), __fsub_rn(c0.z, bg2), 0.0f);
-  rec[4 * (size_t)i + 3] = make_float4(__fsub_rn(c1.x, bg0), __fsub_rn(c1.y, bg1), __fsub_rn(c1.z, bg2), 0.0f);
-}
-
-void launch_pack_records(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, cudaStream_t st) {
-  const int n_rec = sc.N * sc.V;
-  if (n_rec == 0) return;
-  k_pack_records<<<(n_rec + 255) / 256, 256, 0, st>>>(ws.r0, ws.r1, ws.rc0, ws.rc1, n_rec, fp.bg[0], fp.bg[1], fp.bg[2],
-                                                    ws.rec);
-  count_launches(1);
-}
 
 template <int S, bool COUNT>
 __global__ void __launch_bounds__(32, (S <= 5 ? 32 : (S <= 6 ? 28 : (S <= 8 ? 24 : 5)))) k_composite_q(const CompositeArgs a) {

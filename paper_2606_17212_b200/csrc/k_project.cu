@@ -193,8 +193,16 @@ __device__ __forceinline__ void sh_dir(const FrameParams& fp, const float mu[3],
 
 // Also the first step of the binning (k_sort.cu): one increment per tile of the record's rectangle.  The
 // increments are fire-and-forget reductions that overlap the kernel's own memory latency.
-__device__ __forceinline__ void store_record(Workspace& ws, int TX, uint32_t rid, const Proj& p, float opac, float tau,
-                                             uint32_t meta, const float* c0, const float* c1) {
+// And the packed 64-byte record the compositor stages (k_composite_q.cu):
+//   {m_x, m_y, A, B} {Cq, tau, o, meta} {rgb - bg, 0} {rgb with SH residual - bg, 0}
+__device__ __forceinline__ void store_record(Workspace& ws, const FrameParams& fp, uint32_t rid, const Proj& p,
+                                             float opac, float tau, uint32_t meta, const float* c0, const float* c1) {
+  const int TX = fp.TX;
+  float4* rec = ws.rec + 4 * (size_t)rid;
+  rec[0] = make_float4(p.mx, p.my, p.qa, p.qb);
+  rec[1] = make_float4(p.qc, tau, opac, __uint_as_float(meta));
+  rec[2] = make_float4(__fsub_rn(c0[0], fp.bg[0]), __fsub_rn(c0[1], fp.bg[1]), __fsub_rn(c0[2], fp.bg[2]), 0.0f);
+  rec[3] = make_float4(__fsub_rn(c1[0], fp.bg[0]), __fsub_rn(c1[1], fp.bg[1]), __fsub_rn(c1[2], fp.bg[2]), 0.0f);
   ws.r0[rid] = make_float4(p.mx, p.my, p.qa, p.qb);
   ws.r1[rid] = make_float4(p.qc, opac, tau, __uint_as_float(meta));
   ws.rc0[rid] = make_float4(c0[0], c0[1], c0[2], p.hx);
@@ -306,8 +314,8 @@ __global__ void __launch_bounds__(128) k_project(DeviceScene sc, FrameParams fp,
     }
   }
   // record class: 0 = variant A (depth == 0), 1 + lvl = variant B of a level-lvl Gaussian
-  store_record(ws, fp.TX, 2u * i + 0u, pa, opac, tau, (uint32_t)c | (0u << 16), cA, cA);
-  store_record(ws, fp.TX, 2u * i + 1u, pb, opac, tau, (uint32_t)c | ((uint32_t)(1 + lvl) << 16), cB0, cB1);
+  store_record(ws, fp, 2u * i + 0u, pa, opac, tau, (uint32_t)c | (0u << 16), cA, cA);
+  store_record(ws, fp, 2u * i + 1u, pb, opac, tau, (uint32_t)c | ((uint32_t)(1 + lvl) << 16), cB0, cB1);
 }
 
 // K1 with the position residual levels of Eq. (1) (reading I1): a Gaussian has one geometry per
@@ -412,7 +420,7 @@ __global__ void __launch_bounds__(128) k_project4(DeviceScene sc, FrameParams fp
   }
 #pragma unroll
   for (int v = 0; v < 4; ++v)
-    store_record(ws, fp.TX, 4u * i + (uint32_t)v, pr[v], opv[v], tauv[v], (uint32_t)c | ((uint32_t)(16 + v) << 16), col[v], col[v]);
+    store_record(ws, fp, 4u * i + (uint32_t)v, pr[v], opv[v], tauv[v], (uint32_t)c | ((uint32_t)(16 + v) << 16), col[v], col[v]);
 }
 
 void launch_project(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, cudaStream_t st) {

@@ -143,15 +143,105 @@ __device__ __forceinline__ void bitonic_sort(unsigned long long* a, uint32_t n, 
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Render list: the tile's sorted superset list without the records whose conservative q <= tau box touches
+// no pixel of the tile — they contribute to no pixel in any state, and every one of the
+// ~B/S CTAs that composite the tile would otherwise fetch and drop them again.  Order is kept (ballot
+// compaction); the canonical key lists (vals[0], tile_range) are untouched.  Run by the CTA that has just sorted the tile (k_tile_sort).
+// The same pass writes the four per-QUADRANT lists the quadrant compositor walks (k_composite_q.cu): quadrant
+// (qx, qy) of the tile = the 8x4 blocks qx + 4 qy and qx + 4 qy + 2; its list holds, in depth order, {record id,
+// meta} of the records whose block mask has one of the two bits.  The lists of tile t start at 4 * (start of
+// t's canonical list) — a tile with n entries owns 4 n slots, n per quadrant — so no allocation pass is needed.
+template <int THREADS>
+__device__ __forceinline__ void tile_render_lists(int tile, uint2 rg, const unsigned long long* sorted,
+                                                  const float4* __restrict__ r0, const float4* __restrict__ r1,
+                                                  const float4* __restrict__ rc0, const float4* __restrict__ rc1,
+                                                  int TX, uint32_t* __restrict__ rvals,
+                                                  uint2* __restrict__ render_range, uint2* __restrict__ qlist,
+                                                  uint2* __restrict__ qrange) {
+  __shared__ uint32_t s_cnt[THREADS / 32];
+  __shared__ uint32_t s_run;
+  __shared__ uint32_t s_qcnt[4][THREADS / 32];
+  __shared__ uint32_t s_qrun[4];
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  if (tid == 0) s_run = 0;
+  if (tid < 4) s_qrun[tid] = 0;
+  const uint32_t n_tile = rg.y - rg.x;
+  const size_t qbase = 4 * (size_t)rg.x;
+  __syncthreads();
+  for (uint32_t base = rg.x; base < rg.y; base += THREADS) {
+    const uint32_t i = base + tid;
+    uint32_t rid = 0, meta = 0;
+    uint32_t bm = 0;
+    if (i < rg.y) {
+      rid = (uint32_t)sorted[i - rg.x];  // low word of (depth bits << 32 | record id)
+      const float4 g0 = r0[rid], g1 = r1[rid];
+      meta = __float_as_uint(g1.w);
+      bm = record_block_mask_tight(g0.x, g0.y, g0.z, g0.w, g1.x, g1.z, rc0[rid].w, rc1[rid].w, tile % TX, tile / TX);
+    }
+    const bool keep = bm != 0u;
+    const uint32_t bal = __ballot_sync(0xffffffffu, keep);
+    if (lane == 0) s_cnt[w] = __popc(bal);
+    // quadrant q = (q & 1, q >> 1): blocks (q & 1) + 4 (q >> 1) and that + 2
+    const uint32_t qm = (bm | (bm >> 2)) & 0x33u;  // bits 0, 1, 4, 5 = quadrants 0, 1, 2, 3
+    uint32_t qbal[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      qbal[q] = __ballot_sync(0xffffffffu, (qm >> ((q & 1) + 4 * (q >> 1))) & 1u);
+      if (lane == 0) s_qcnt[q][w] = __popc(qbal[q]);
+    }
+    __syncthreads();
+    uint32_t woff = 0, tot = 0;
+    for (int q = 0; q < THREADS / 32; ++q) {
+      if (q < w) woff += s_cnt[q];
+      tot += s_cnt[q];
+    }
+    if (keep) {
+      const uint32_t pos = rg.x + s_run + woff + __popc(bal & ((1u << lane) - 1u));
+      rvals[pos] = rid;
+    }
+    uint32_t qtot[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      uint32_t qoff = 0;
+      qtot[q] = 0;
+      for (int k = 0; k < THREADS / 32; ++k) {
+        if (k < w) qoff += s_qcnt[q][k];
+        qtot[q] += s_qcnt[q][k];
+      }
+      if ((qm >> ((q & 1) + 4 * (q >> 1))) & 1u)
+        qlist[qbase + (size_t)q * n_tile + s_qrun[q] + qoff + __popc(qbal[q] & ((1u << lane) - 1u))] = make_uint2(rid, meta);
+    }
+    __syncthreads();
+    if (tid == 0) s_run += tot;
+    if (tid < 4) s_qrun[tid] += qtot[tid];
+    __syncthreads();
+  }
+  if (tid == 0) render_range[tile] = make_uint2(rg.x, rg.x + s_run);
+  if (tid < 4) {
+    const uint32_t st = (uint32_t)(qbase + (size_t)tid * n_tile);
+    qrange[4 * tile + tid] = make_uint2(st, st + s_qrun[tid]);
+  }
+}
+
 __global__ void __launch_bounds__(kSortThreads) k_tile_sort(const uint2* __restrict__ tile_range,
                                                            unsigned long long* __restrict__ seg,
                                                            unsigned long long* __restrict__ keys_out,
-                                                           uint32_t* __restrict__ vals_out) {
+                                                           uint32_t* __restrict__ vals_out,
+                                                           const float4* __restrict__ r0, const float4* __restrict__ r1,
+                                                           const float4* __restrict__ rc0, const float4* __restrict__ rc1,
+                                                           int TX, uint32_t* __restrict__ rvals,
+                                                           uint2* __restrict__ render_range, uint2* __restrict__ qlist,
+                                                           uint2* __restrict__ qrange) {
   __shared__ unsigned long long s_key[kSortSmemKeys];
   const uint32_t tile = blockIdx.x;
   const uint2 rg = tile_range[tile];
   const uint32_t n = rg.y - rg.x;
-  if (n == 0) return;
+  if (n == 0) {  // an empty tile still has (empty) render lists
+    if (threadIdx.x == 0) render_range[tile] = make_uint2(rg.x, rg.x);
+    if (threadIdx.x < 4) qrange[4 * tile + threadIdx.x] = make_uint2(4u * rg.x, 4u * rg.x);
+    return;
+  }
   uint32_t np2 = 1;
   while (np2 < n) np2 <<= 1;
   unsigned long long* a = seg + rg.x;
@@ -166,6 +256,8 @@ __global__ void __launch_bounds__(kSortThreads) k_tile_sort(const uint2* __restr
     keys_out[rg.x + i] = ((unsigned long long)tile << 32) | (k >> 32);
     vals_out[rg.x + i] = (uint32_t)k;
   }
+  // a4 preparation while the sorted segment is at hand: render list and the four quadrant lists of the tile
+  tile_render_lists<kSortThreads>((int)tile, rg, a, r0, r1, rc0, rc1, TX, rvals, render_range, qlist, qrange);
 }
 
 void launch_bin_and_sort(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, long long cap,
@@ -178,7 +270,11 @@ void launch_bin_and_sort(const DeviceScene& sc, const FrameParams& fp, Workspace
   if (n_rec > 0) {
     k_scatter_keys<<<grid, 256, 0, st>>>(n_rec, ws.count, ws.rect, ws.depth_bits, fp.TX, ws.hdr, ws.tile_cursor,
                                          ws.keys[1]);
-    k_tile_sort<<<tiles, kSortThreads, 0, st>>>(ws.tile_range, ws.keys[1], ws.keys[0], ws.vals[0]);
+    k_tile_sort<<<tiles, kSortThreads, 0, st>>>(ws.tile_range, ws.keys[1], ws.keys[0], ws.vals[0], ws.r0, ws.r1, ws.rc0,
+                                                ws.rc1, fp.TX, ws.vals[1], ws.render_range, ws.qlist, ws.qrange);
+  } else {
+    cudaMemsetAsync(ws.render_range, 0, sizeof(uint2) * (size_t)tiles, st);
+    cudaMemsetAsync(ws.qrange, 0, sizeof(uint2) * 4 * (size_t)tiles, st);
   }
   count_launches(n_rec > 0 ? 3 : 1);
 }
