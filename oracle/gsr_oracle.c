@@ -19,6 +19,10 @@
  *                                   front-to-back alpha compositing with early termination
  *   O-6 distortion ................ north_star (5): MSE / PSNR against the full-state render
  *   O-7 utility ................... PAPER.md:80-88, Eq. (3) and Eq. (4) (alpha=0.25, beta=0.05, Q_0.1)
+ *   O-8 backward of O-5 ........... PAPER.md:64-76 (the objective is a function of the rendered images): the
+ *                                   gradient of a linear functional of one state's image with respect to the
+ *                                   2-D quantities O-5 reads; the chain rule of O-5 written out, decisions fixed
+ *                                   (pins: tests/test_backward_pins.py — finite differences of O-5, closed form)
  *
  * Precision split.  Quantities that feed an INTEGER decision (deformed mean,
  * camera-space point, 2-D covariance, conic, radius, tile rectangle, depth bits, the quadratic
@@ -630,4 +634,95 @@ void orc_group_utility(const double* mse, const double* psnr_db, const int32_t* 
     util[9 * g + 8] = (double)n;
   }
   free(buf);
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* O-8  backward of O-5: gradients of a linear functional of one state's image                  */
+/* ------------------------------------------------------------------------------------------ */
+
+/* SURVEY.md §8(f)-4's follow-on (the training objective is a function of the rendered images, so
+ * its gradient enters through dL/d(image)).  Given g = dL/d(pixel) for every pixel and channel of ONE state's image
+ * (e.g. 2 (I - R) / (3 W H) for L = MSE), the gradient of L with respect to the 2-D quantities of every Gaussian of
+ * the state that O-5 reads: rgb[3], opacity, qa, qb, qc (= A, B, Cq), mx, my.
+ *
+ * Definition (the pixel of O-5 written out): with the accepted Gaussians i = 1..n of a pixel in O-4 order,
+ *   alpha_i = min(0.99, o_i exp(-q_i)),  T_1 = 1,  T_{i+1} = T_i (1 - alpha_i),  pixel = sum_i alpha_i T_i c_i + T_{n+1} bg.
+ * The discrete decisions — which Gaussians are evaluated (tile rectangles), the cut q > tau, the cap at 0.99 and the
+ * stop T' < t_stop — are constants of the differentiation (they are piecewise constant in the parameters).  Hence
+ *   dpixel/dc_i     = alpha_i T_i
+ *   dpixel/dalpha_i = T_i c_i - S_i / (1 - alpha_i),   S_i = sum_{j>i} alpha_j T_j c_j + T_{n+1} bg
+ *   dalpha_i/do_i   = exp(-q_i),  dalpha_i/dq_i = -alpha_i      (both 0 where the cap is active)
+ *   q = (A dx + B dy) dx + Cq dy^2 with dx = mx - px, dy = my - py:
+ *   dq/dA = dx^2, dq/dB = dx dy, dq/dCq = dy^2, dq/dmx = 2 A dx + B dy, dq/dmy = B dx + 2 Cq dy.
+ * Brute force per pixel like O1: a forward walk that records the accepted sequence, then the sums above in double
+ * from the same fp32 dx, dy, q the forward decisions use.
+ *   g_img  double [H,W,3];  grad double [N,9] = (drgb[3], dopacity, dqa, dqb, dqc, dmx, dmy), zeroed here. */
+void orc_backward_O1(const orc_scene* s, const orc_camera* cam, const orc_proj* p, double t_stop, const double* g_img,
+                     double* grad) {
+  order_key* ord = (order_key*)malloc(sizeof(order_key) * (size_t)(s->N > 0 ? s->N : 1));
+  int64_t n = build_order(p, s->N, ord);
+  for (int64_t k = 0; k < 9 * (int64_t)s->N; ++k) grad[k] = 0.0;
+  /* accepted sequence of one pixel */
+  int32_t* a_idx = (int32_t*)malloc(sizeof(int32_t) * (size_t)(n > 0 ? n : 1));
+  double* a_alpha = (double*)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+  double* a_T = (double*)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+  double* a_e = (double*)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+  float* a_dx = (float*)malloc(sizeof(float) * (size_t)(n > 0 ? n : 1));
+  float* a_dy = (float*)malloc(sizeof(float) * (size_t)(n > 0 ? n : 1));
+  int* a_cap = (int*)malloc(sizeof(int) * (size_t)(n > 0 ? n : 1));
+  for (int y = 0; y < cam->H; ++y)
+    for (int x = 0; x < cam->W; ++x) {
+      const int tx = x / TILE, ty = y / TILE;
+      const float px = (float)x + 0.5f, py = (float)y + 0.5f;
+      const double* g = g_img + 3 * ((int64_t)y * cam->W + x);
+      double T = 1.0;
+      int64_t m = 0;
+      for (int64_t k = 0; k < n; ++k) {
+        const orc_proj* gs = &p[ord[k].idx];
+        if (tx < gs->rect[0] || tx >= gs->rect[2] || ty < gs->rect[1] || ty >= gs->rect[3]) continue;
+        /* the forward step of O-5, decisions in fp32 */
+        float dx = gs->mx - px;
+        float dy = gs->my - py;
+        float u = gs->qa * dx;
+        float sacc = fmaf(gs->qb, dy, u);
+        float q = sacc * dx;
+        float v = gs->qc * dy;
+        q = fmaf(v, dy, q);
+        if (q > gs->tau) continue;
+        double e = exp(-(double)q);
+        double alpha = (double)gs->opacity * e;
+        int cap = 0;
+        if (alpha > 0.99) { alpha = 0.99; cap = 1; }
+        double Tn = T * (1.0 - alpha);
+        if (Tn < t_stop) break;
+        a_idx[m] = ord[k].idx; a_alpha[m] = alpha; a_T[m] = T; a_e[m] = e; a_dx[m] = dx; a_dy[m] = dy; a_cap[m] = cap;
+        ++m;
+        T = Tn;
+      }
+      /* suffix S_i, built from the back: starts as T_{n+1} bg */
+      double S[3] = {T * (double)s->background[0], T * (double)s->background[1], T * (double)s->background[2]};
+      for (int64_t i = m - 1; i >= 0; --i) {
+        const orc_proj* gs = &p[a_idx[i]];
+        double* gr = grad + 9 * (int64_t)a_idx[i];
+        const double w = a_alpha[i] * a_T[i];
+        double dL_dalpha = 0.0;
+        for (int ch = 0; ch < 3; ++ch) {
+          gr[ch] += w * g[ch];
+          dL_dalpha += g[ch] * (a_T[i] * gs->rgb[ch] - S[ch] / (1.0 - a_alpha[i]));
+        }
+        if (!a_cap[i]) {
+          const double dx = (double)a_dx[i], dy = (double)a_dy[i];
+          const double dL_dq = -a_alpha[i] * dL_dalpha;
+          gr[3] += a_e[i] * dL_dalpha;
+          gr[4] += dL_dq * dx * dx;
+          gr[5] += dL_dq * dx * dy;
+          gr[6] += dL_dq * dy * dy;
+          gr[7] += dL_dq * (2.0 * (double)gs->qa * dx + (double)gs->qb * dy);
+          gr[8] += dL_dq * ((double)gs->qb * dx + 2.0 * (double)gs->qc * dy);
+        }
+        for (int ch = 0; ch < 3; ++ch) S[ch] += w * gs->rgb[ch];
+      }
+    }
+  free(a_idx); free(a_alpha); free(a_T); free(a_e); free(a_dx); free(a_dy); free(a_cap);
+  free(ord);
 }
