@@ -152,6 +152,27 @@ int gsr_render_states_vs_full(const gsr_scene* scene, const gsr_camera* cam, flo
                               int32_t B, float* out, float* ref_out, double* mse, float* psnr_db,
                               void* workspace, size_t ws_bytes, void* cuda_stream);
 
+/* ------------------------------------------------------------------------------------------------
+ * gsr_render_backward — the backward of the compositing step (the training objective is a function
+ * of the rendered images; SURVEY.md §8(f)-4 follow-on).  To be called after gsr_render_states /
+ * _ex / _vs_full on the SAME workspace, batch and stream: it reuses the projected records, the sorted lists and the
+ * validated levels the forward call left there.
+ *   images      dev fp32 [B,H,W,3]  the forward output of that call
+ *   dL_dimages  dev fp32 [B,H,W,3]  the gradient of the objective with respect to every pixel of every state
+ *   grad        dev fp32 [gsr_num_records(scene), 12], overwritten: for record r (Gaussian i, variant v: r = 2 i + v,
+ *               v = 0 the geometry of cluster depth 0, v = 1 of depth >= 1; r = 4 i + v for scenes with position
+ *               residual levels), summed over the states and pixels that composite it,
+ *               d/d(rgb[3], rgb with the level-3 SH residual[3], opacity, A, B, Cq, m_x, m_y)
+ *               where pixel = sum_i alpha_i T_i rgb_i + T_end bg, alpha = min(0.99, opacity exp(-q)),
+ *               q = (A dx + B dy) dx + Cq dy^2, (dx, dy) = (m_x, m_y) - pixel centre; the cut, the
+ *               cap and the stop are constants of the differentiation.  States whose cluster depth is 3 use the
+ *               second colour, all others the first.
+ * Synchronises once at entry (reads the workspace header), then asynchronous.  Sums are formed with float
+ * atomics: the result is reproducible up to fp32 summation order.  B must be the forward call's B. */
+int64_t gsr_num_records(const gsr_scene* scene);
+int gsr_render_backward(const gsr_scene* scene, const void* workspace, const float* images, const float* dL_dimages,
+                        int32_t B, float* grad, void* cuda_stream);
+
 /* Synchronises `cuda_stream` and reads the status latched by the last render into `workspace`:
  * returns GSR_OK, GSR_E_INVALID_LEVEL or GSR_E_WORKSPACE_TOO_SMALL.  keys_needed (host, may be NULL)
  * receives the number of (tile, depth, record) keys the frame produced. */

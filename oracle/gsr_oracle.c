@@ -656,12 +656,18 @@ void orc_group_utility(const double* mse, const double* psnr_db, const int32_t* 
  *   dq/dA = dx^2, dq/dB = dx dy, dq/dCq = dy^2, dq/dmx = 2 A dx + B dy, dq/dmy = B dx + 2 Cq dy.
  * Brute force per pixel like O1: a forward walk that records the accepted sequence, then the sums above in double
  * from the same fp32 dx, dy, q the forward decisions use.
- *   g_img  double [H,W,3];  grad double [N,9] = (drgb[3], dopacity, dqa, dqb, dqc, dmx, dmy), zeroed here. */
+ *   g_img  double [H,W,3];  grad double [N,9] = (drgb[3], dopacity, dqa, dqb, dqc, dmx, dmy), zeroed here.
+ *   grad_abs (optional, [N,9]): a magnitude for every entry, against which a floating-point evaluation of these
+ *   strongly cancelling sums can be judged: the same sums with dL/dalpha replaced by
+ *   |g| (T |c| + 2 M / (1 - alpha)), M = sum_j alpha_j T_j |c_j| + T_end |bg| (everything a pixel is made of: an
+ *   implementation may form the suffix S_i as "final pixel minus prefix"), and absolute chain factors. */
 void orc_backward_O1(const orc_scene* s, const orc_camera* cam, const orc_proj* p, double t_stop, const double* g_img,
-                     double* grad) {
+                     double* grad, double* grad_abs) {
   order_key* ord = (order_key*)malloc(sizeof(order_key) * (size_t)(s->N > 0 ? s->N : 1));
   int64_t n = build_order(p, s->N, ord);
   for (int64_t k = 0; k < 9 * (int64_t)s->N; ++k) grad[k] = 0.0;
+  if (grad_abs)
+    for (int64_t k = 0; k < 9 * (int64_t)s->N; ++k) grad_abs[k] = 0.0;
   /* accepted sequence of one pixel */
   int32_t* a_idx = (int32_t*)malloc(sizeof(int32_t) * (size_t)(n > 0 ? n : 1));
   double* a_alpha = (double*)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
@@ -699,26 +705,44 @@ void orc_backward_O1(const orc_scene* s, const orc_camera* cam, const orc_proj* 
         ++m;
         T = Tn;
       }
+      double M[3]; /* magnitude of what the pixel is made of, per channel */
+      for (int ch = 0; ch < 3; ++ch) {
+        M[ch] = T * fabs((double)s->background[ch]);
+        for (int64_t i = 0; i < m; ++i) M[ch] += a_alpha[i] * a_T[i] * fabs(p[a_idx[i]].rgb[ch]);
+      }
       /* suffix S_i, built from the back: starts as T_{n+1} bg */
       double S[3] = {T * (double)s->background[0], T * (double)s->background[1], T * (double)s->background[2]};
       for (int64_t i = m - 1; i >= 0; --i) {
         const orc_proj* gs = &p[a_idx[i]];
         double* gr = grad + 9 * (int64_t)a_idx[i];
         const double w = a_alpha[i] * a_T[i];
-        double dL_dalpha = 0.0;
+        double dL_dalpha = 0.0, mag = 0.0, c9[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0}, m9[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
         for (int ch = 0; ch < 3; ++ch) {
-          gr[ch] += w * g[ch];
+          c9[ch] = w * g[ch];
+          m9[ch] = fabs(c9[ch]);
           dL_dalpha += g[ch] * (a_T[i] * gs->rgb[ch] - S[ch] / (1.0 - a_alpha[i]));
+          mag += fabs(g[ch]) * (a_T[i] * fabs(gs->rgb[ch]) + 2.0 * M[ch] / (1.0 - a_alpha[i]));
         }
         if (!a_cap[i]) {
           const double dx = (double)a_dx[i], dy = (double)a_dy[i];
           const double dL_dq = -a_alpha[i] * dL_dalpha;
-          gr[3] += a_e[i] * dL_dalpha;
-          gr[4] += dL_dq * dx * dx;
-          gr[5] += dL_dq * dx * dy;
-          gr[6] += dL_dq * dy * dy;
-          gr[7] += dL_dq * (2.0 * (double)gs->qa * dx + (double)gs->qb * dy);
-          gr[8] += dL_dq * ((double)gs->qb * dx + 2.0 * (double)gs->qc * dy);
+          c9[3] = a_e[i] * dL_dalpha;
+          c9[4] = dL_dq * dx * dx;
+          c9[5] = dL_dq * dx * dy;
+          c9[6] = dL_dq * dy * dy;
+          c9[7] = dL_dq * (2.0 * (double)gs->qa * dx + (double)gs->qb * dy);
+          c9[8] = dL_dq * ((double)gs->qb * dx + 2.0 * (double)gs->qc * dy);
+          const double mq = a_alpha[i] * mag;
+          m9[3] = a_e[i] * mag;
+          m9[4] = mq * dx * dx;
+          m9[5] = mq * fabs(dx * dy);
+          m9[6] = mq * dy * dy;
+          m9[7] = mq * (2.0 * fabs((double)gs->qa * dx) + fabs((double)gs->qb * dy));
+          m9[8] = mq * (fabs((double)gs->qb * dx) + 2.0 * fabs((double)gs->qc * dy));
+        }
+        for (int k = 0; k < 9; ++k) {
+          gr[k] += c9[k];
+          if (grad_abs) grad_abs[9 * (int64_t)a_idx[i] + k] += m9[k];
         }
         for (int ch = 0; ch < 3; ++ch) S[ch] += w * gs->rgb[ch];
       }

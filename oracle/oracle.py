@@ -204,16 +204,20 @@ class OracleScene:
            _p(Tf) if want_T else None)
         return (img, stats, Tf) if want_T else (img, stats)
 
-    def backward(self, cam, t: float, depth, g_img, t_stop: float = 1e-4, proj: np.ndarray | None = None):
+    def backward(self, cam, t: float, depth, g_img, t_stop: float = 1e-4, proj: np.ndarray | None = None,
+                 want_abs: bool = False):
         """orc_backward_O1: g_img = dL/d(image) double [H,W,3] of ONE state -> double [N,9] =
-        (drgb[3], dopacity, dqa, dqb, dqc, dmx, dmy) per Gaussian of that state."""
+        (drgb[3], dopacity, dqa, dqb, dqc, dmx, dmy) per Gaussian of that state; want_abs adds the same sums
+        with every per-pixel contribution in absolute value."""
         if proj is None:
             proj = self.project(cam, t, depth)
         g = _c(g_img, np.float64)
         assert g.shape == (cam.H, cam.W, 3)
         grad = np.zeros((self.N, 9), np.float64)
-        lib().orc_backward_O1(C.byref(self._s), C.byref(make_camera(cam)), _p(proj), C.c_double(t_stop), _p(g), _p(grad))
-        return grad
+        gabs = np.zeros((self.N, 9), np.float64) if want_abs else None
+        lib().orc_backward_O1(C.byref(self._s), C.byref(make_camera(cam)), _p(proj), C.c_double(t_stop), _p(g), _p(grad),
+                              _p(gabs) if want_abs else None)
+        return (grad, gabs) if want_abs else grad
 
     def trace_pixel(self, cam, t: float, depth, x: int, y: int, t_stop: float = 1e-4, cap: int = 4096):
         proj = self.project(cam, t, depth)

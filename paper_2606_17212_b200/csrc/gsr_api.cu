@@ -534,6 +534,33 @@ int gsr_render_states(const gsr_scene* scene, const gsr_camera* cam, float t, co
                               cuda_stream);
 }
 
+int64_t gsr_num_records(const gsr_scene* scene) {
+  return scene ? (int64_t)scene->impl.d.N * scene->impl.d.V : 0;
+}
+
+int gsr_render_backward(const gsr_scene* scene, const void* workspace, const float* images, const float* dL_dimages,
+                        int32_t B, float* grad, void* cuda_stream) {
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (!scene || !workspace || B < 0 || (B > 0 && (!images || !dL_dimages)) || !grad) {
+    set_error("gsr_render_backward: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  // the header is read on the host: the forward call that filled the workspace has to be complete on this stream
+  WsHeader h;
+  GSR_CUDA(cudaMemcpyAsync(&h, workspace, sizeof(h), cudaMemcpyDeviceToHost, st));
+  GSR_CUDA(cudaStreamSynchronize(st));
+  if (h.N != scene->impl.d.N || h.C != scene->impl.d.C || h.B != B) {
+    set_error("gsr_render_backward: the workspace does not hold a forward render of this scene with B = %d states", B);
+    return GSR_E_INVALID_ARG;
+  }
+  if (h.status != GSR_OK) { set_error("gsr_render_backward: the forward render failed (status %d)", h.status); return h.status; }
+  Workspace ws;
+  carve_workspace(&ws, const_cast<void*>(workspace), rec_half(scene->impl.d), h.C, h.B, h.TX * h.TY, h.key_capacity);
+  launch_backward(scene->impl.d, h, ws, images, dL_dimages, grad, st);
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
 int gsr_workspace_status(const void* workspace, int64_t* keys_needed, void* cuda_stream) {
   if (!workspace) { set_error("gsr_workspace_status: NULL workspace"); return GSR_E_INVALID_ARG; }
   WsHeader h;

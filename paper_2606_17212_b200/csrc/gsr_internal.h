@@ -167,6 +167,9 @@ void launch_composite_count(const DeviceScene& sc, const FrameParams& fp, Worksp
 void count_launches(int n);
 struct CompositeArgs;
 void launch_composite_q(const CompositeArgs& a, int S, bool count, cudaStream_t st);
+// backward of a4 (k_backward.cu): grad [records, 12], zeroed by the call
+void launch_backward(const DeviceScene& sc, const WsHeader& h, Workspace& ws, const float* images, const float* gimg,
+                     float* grad, cudaStream_t st);
 void launch_distortion_finalize_blk(const double* blk, int32_t B, int32_t tiles, int64_t n_values, double* mse,
                                     float* psnr, cudaStream_t st);
 bool launch_tile_dedup(const DeviceScene& sc, const FrameParams& fp, Workspace& ws, const int8_t* depth_rows,

@@ -1,0 +1,329 @@
+// k_backward.cu — backward of stage a4 (SURVEY.md §8(f)-4 follow-on; the objective
+// is a function of the rendered images, so its gradient enters through dL/d(image)).
+//
+// Given g[b] = dL/d(image of state b) for the B states of the frame a forward call has just rendered, the gradient
+// of L with respect to the 2-D quantities of every projected record that the compositor read, summed over the
+// states and pixels that use the record:
+//     grad[record][12] = d/d( rgb[3], rgb with SH residual[3], opacity, A, B, Cq, m_x, m_y )
+// Per pixel, with the accepted records i = 1..n in list order (cb = c - bg, w_i = alpha_i T_i):
+//     pixel - bg = sum_i w_i cb_i
+//     dL/dcb_i    = w_i g
+//     dL/dalpha_i = T_i (g . cb_i) - (Gf - G_i) / (1 - alpha_i),  G_i = sum_{j<=i} w_j (g . cb_j),  Gf = g . (pixel - bg)
+//     dalpha/do = exp(-q), dalpha/dq = -alpha  (both 0 where the cap 0.99 is active or the cut failed)
+//     dq/dA = dx^2, dq/dB = dx dy, dq/dCq = dy^2, dq/dm_x = 2 A dx + B dy, dq/dm_y = B dx + 2 Cq dy
+// The suffix of the pixel is taken as (final pixel) - (prefix), so the list is walked front to back exactly like the
+// forward pass — same quadrant lists, same staging, same decisions bit for bit (alpha, the cut, the stop rule are
+// the forward's operations on the same operands) — and the forward image is an input.
+//
+// Layout of the work: the forward's (k_composite_q.cu): one warp per 8x8 quadrant x S states, two pixels per lane on
+// packed FP32; per (pixel pair, state) T, G and the constants g[3], Gf live in registers (12 per slot, S = 4).
+// Per record the 12 partial sums of the lane's pixels and states are reduced over the warp with the
+// slot-splitting butterfly (16 shuffles instead of 60) and added to grad with one atomic per component.
+// Float atomics make the summation order, hence the last bits of grad, run-dependent; parity is by tolerance.
+#include "composite_common.cuh"
+#include "gsr_internal.h"
+
+namespace gsr {
+
+struct BackwardArgs {
+  const float4* rec;
+  const uint2* qlist;
+  const uint2* qrange;
+  const int8_t* depth;   // [B, C]
+  int32_t B, C, nsb;
+  int32_t W, H, TX, tiles;
+  float bg[3];
+  const float* images;   // [B,H,W,3] forward output
+  const float* gimg;     // [B,H,W,3] dL/d(image)
+  float* grad;           // [records, 12]
+};
+
+// The butterfly of reduce.cuh for 16 floats per lane: after the call the lane holds the warp total of component
+// `slot` (lanes with (lane & 1) == 0 are one representative per component).
+__device__ __forceinline__ float warp_sum_16(float (&v)[16], int lane, int& slot) {
+  int off = 16;
+  slot = 0;
+#pragma unroll
+  for (int n = 16; n > 1; n >>= 1) {
+    const int half = n >> 1;
+    const bool upper = (lane & off) != 0;
+#pragma unroll
+    for (int j = 0; j < half; ++j) {
+      const float send = upper ? v[j] : v[j + half];
+      const float keep = upper ? v[j + half] : v[j];
+      v[j] = keep + __shfl_xor_sync(0xffffffffu, send, off);
+    }
+    slot = 2 * slot + (upper ? 1 : 0);
+    off >>= 1;
+  }
+  v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
+  return v[0];
+}
+
+// One state slot, two pixels (header).  T, G, Gf are carried scaled by 2^40 like the forward's T.
+//   dal  += s (T u - (Gf - G') rinv)        accumulated dL/dalpha of the record over the slots
+//   dc*  += (s w) g                          accumulated colour gradient
+__device__ __forceinline__ void slot_backward(f32x2& T, f32x2& G, f32x2 gr, f32x2 gg, f32x2 gb, f32x2 Gf, f32x2 alpha2,
+                                              f32x2 rinv2, float cr, float cg, float cb, f32x2& dal, f32x2& dcr,
+                                              f32x2& dcg, f32x2& dcb) {
+  f32x2 u = mul2(gr, pack2(cr, cr));
+  u = fma2(gg, pack2(cg, cg), u);
+  u = fma2(gb, pack2(cb, cb), u);
+  const f32x2 w = mul2(alpha2, T);
+  f32x2 Tn;
+  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(Tn) : "l"(T), "l"(w));
+  float tl, th;
+  unpack2(Tn, tl, th);
+  asm("add.rn.sat.f32 %0, %0, 0fCCD1B716;" : "+f"(tl));  // the forward's stop rule: s = [T' >= 1e-4]
+  asm("add.rn.sat.f32 %0, %0, 0fCCD1B716;" : "+f"(th));
+  const f32x2 s = pack2(tl, th);
+  const f32x2 ws = mul2(w, s);
+  const f32x2 tu = mul2(T, u);
+  G = fma2(ws, u, G);
+  f32x2 d;
+  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(Gf), "l"(G));
+  const f32x2 dr = mul2(d, rinv2);
+  f32x2 t1;
+  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(t1) : "l"(tu), "l"(dr));  // T u - (Gf - G) / (1 - alpha)
+  dal = fma2(s, t1, dal);
+  dcr = fma2(ws, gr, dcr);
+  dcg = fma2(ws, gg, dcg);
+  dcb = fma2(ws, gb, dcb);
+  T = Tn;
+}
+
+template <int S>
+__global__ void __launch_bounds__(32) k_backward_q(const BackwardArgs a) {
+  extern __shared__ uint16_t s_tab[];  // [C][4]: slots (bit s) whose state has depth == 0, >= 1, >= 2, >= 3
+  __shared__ __align__(16) float4 s_rec[2][kChunk * 4];
+  __shared__ uint32_t s_tag[2][kChunk];  // act | res << 16
+  __shared__ uint32_t s_rid[2][kChunk];  // record id (row of grad)
+
+  const int lane = threadIdx.x;
+  const uint32_t tq = blockIdx.x / (uint32_t)a.nsb;  // 4 * tile + quadrant
+  const int sb = (int)(blockIdx.x - tq * (uint32_t)a.nsb);
+  const int tile = (int)(tq >> 2), quad = (int)(tq & 3u);
+  const int b0 = sb * S;  // slot s = state b0 + s (no tile-level dedup here: every state has its own g)
+
+  for (int c = lane; c < a.C; c += 32) {
+    uint32_t eq0 = 0, ge1 = 0, ge2 = 0, ge3 = 0;
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+      if (b0 + s < a.B) {
+        const int d = a.depth[(size_t)(b0 + s) * a.C + c];
+        eq0 |= (uint32_t)(d == 0) << s;
+        ge1 |= (uint32_t)(d >= 1) << s;
+        ge2 |= (uint32_t)(d >= 2) << s;
+        ge3 |= (uint32_t)(d >= 3) << s;
+      }
+    }
+    s_tab[4 * c + 0] = (uint16_t)eq0;
+    s_tab[4 * c + 1] = (uint16_t)ge1;
+    s_tab[4 * c + 2] = (uint16_t)ge2;
+    s_tab[4 * c + 3] = (uint16_t)ge3;
+  }
+  __syncwarp();
+
+  const int tx = tile % a.TX, ty = tile / a.TX;
+  const int x = tx * kTile + 8 * (quad & 1) + (lane & 7);
+  const int ya = ty * kTile + 8 * (quad >> 1) + (lane >> 3), yb = ya + 4;
+  const bool in_a = x < a.W && ya < a.H, in_b = x < a.W && yb < a.H;
+  float px = (float)x + 0.5f;
+  f32x2 npy2 = pack2(-((float)ya + 0.5f), -((float)yb + 0.5f));
+  asm volatile("" : "+f"(px), "+l"(npy2));
+  const uint32_t rec_base = (uint32_t)__cvta_generic_to_shared(&s_rec[0][0]);
+  const uint32_t tag_base = (uint32_t)__cvta_generic_to_shared(&s_tag[0][0]);
+  const uint32_t rid_base = (uint32_t)__cvta_generic_to_shared(&s_rid[0][0]);
+  const uint32_t lt = (1u << lane) - 1u;
+
+  // per (pixel pair, state): T (scaled by 2^40), the prefix G of w (g . cb), and the constants g[3], Gf (scaled)
+  f32x2 T2[S], G2[S], gr2[S], gg2[S], gb2[S], Gf2[S];
+  const size_t img = (size_t)a.H * a.W * 3;
+#pragma unroll
+  for (int s = 0; s < S; ++s) {
+    float g[2][3] = {{0.f, 0.f, 0.f}, {0.f, 0.f, 0.f}}, gf[2] = {0.f, 0.f};
+    const bool on = b0 + s < a.B;
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const int y = h ? yb : ya;
+      if (on && (h ? in_b : in_a)) {
+        const size_t o = (size_t)(b0 + s) * img + ((size_t)y * a.W + x) * 3;
+        float dot = 0.0f;
+#pragma unroll
+        for (int ch = 0; ch < 3; ++ch) {
+          g[h][ch] = __ldg(a.gimg + o + ch);
+          dot = __fmaf_rn(g[h][ch], __fsub_rn(__ldg(a.images + o + ch), a.bg[ch]), dot);
+        }
+        gf[h] = dot * kTScale;
+      }
+    }
+    T2[s] = pack2(on && in_a ? kTScale : 0.0f, on && in_b ? kTScale : 0.0f);
+    G2[s] = pack2(0.0f, 0.0f);
+    gr2[s] = pack2(g[0][0], g[1][0]); gg2[s] = pack2(g[0][1], g[1][1]); gb2[s] = pack2(g[0][2], g[1][2]);
+    Gf2[s] = pack2(gf[0], gf[1]);
+  }
+
+  const uint2 qr = a.qrange[tq];
+  const uint32_t n_ent = qr.y - qr.x;
+  const uint2* const list = a.qlist + qr.x;
+
+  auto stage = [&](uint2 e, bool have, int buf) -> uint32_t {
+    uint32_t act = 0, res = 0;
+    if (have) {
+      const uint32_t meta = e.y, cls = meta >> 16;
+      const uint16_t* t = s_tab + 4 * (meta & 0xFFFFu);
+      if (cls >= 16) {
+        const uint32_t v = cls - 16;
+        act = v == 0 ? t[0] : (v == 1 ? (t[1] & ~t[2]) : (v == 2 ? (t[2] & ~t[3]) : t[3]));
+      } else {
+        act = cls == 0 ? t[0] : (cls <= 2 ? t[1] : (cls == 3 ? t[2] : t[3]));
+        res = cls == 0 ? 0u : t[3];
+      }
+    }
+    const bool keep = act != 0;
+    const uint32_t bal = __ballot_sync(0xffffffffu, keep);
+    if (keep) {
+      const uint32_t pos = __popc(bal & lt);
+      const uint32_t dst = rec_base + (uint32_t)buf * (kChunk * 64u) + 64u * pos;
+      const float4* src = a.rec + 4 * (size_t)e.x;
+      cp_async16(dst, src);
+      cp_async16(dst + 16u, src + 1);
+      cp_async16(dst + 32u, src + 2);
+      cp_async16(dst + 48u, src + 3);
+      sts32(tag_base + (uint32_t)buf * (kChunk * 4u) + 4u * pos, act | (res << 16));
+      sts32(rid_base + (uint32_t)buf * (kChunk * 4u) + 4u * pos, e.x);
+    }
+    cp_async_commit();
+    return (uint32_t)__popc(bal);
+  };
+
+  uint32_t n_cur = 0;
+  uint2 e_next = make_uint2(0u, 0u);
+  if (n_ent > 0) {
+    const uint2 e0 = (uint32_t)lane < n_ent ? __ldg(list + lane) : make_uint2(0u, 0u);
+    n_cur = stage(e0, (uint32_t)lane < n_ent, 0);
+    if (kChunk + (uint32_t)lane < n_ent) e_next = __ldg(list + kChunk + lane);
+  }
+  for (uint32_t base = 0; base < n_ent; base += kChunk) {
+    const int buf = (int)((base / kChunk) & 1u);
+    uint32_t n_nxt = 0;
+    if (base + kChunk < n_ent) {
+      n_nxt = stage(e_next, base + kChunk + (uint32_t)lane < n_ent, buf ^ 1);
+      if (base + 2 * kChunk + (uint32_t)lane < n_ent) e_next = __ldg(list + base + 2 * kChunk + lane);
+      cp_async_wait<1>();
+    } else {
+      cp_async_wait<0>();
+    }
+    __syncwarp();
+    uint32_t walive = 0;
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+      float t0, t1;
+      unpack2(T2[s], t0, t1);
+      walive |= ((t0 >= kTStopScaled || t1 >= kTStopScaled) ? 1u : 0u) << s;
+    }
+    walive = __reduce_or_sync(0xffffffffu, walive);
+    if (walive == 0) {
+      cp_async_wait<0>();
+      break;
+    }
+    const uint32_t rb0 = rec_base + (uint32_t)buf * (kChunk * 64u), tb0 = tag_base + (uint32_t)buf * (kChunk * 4u);
+    const uint32_t ib0 = rid_base + (uint32_t)buf * (kChunk * 4u);
+#pragma unroll 1
+    for (uint32_t j = 0; j < n_cur; ++j) {
+      const uint32_t addr = rb0 + 64u * j;
+      const uint32_t tag = lds32(tb0 + 4u * j);
+      const uint32_t actl = tag & walive;
+      if (actl == 0) continue;
+      const float4 h0 = lds128(addr);        // {m_x, m_y, A, B}
+      const float4 hq = lds128(addr + 16u);  // {Cq, tau, o, -}
+      // the forward's alpha evaluation, operation for operation
+      const float dx = __fsub_rn(h0.x, px);
+      const f32x2 dy2 = add2(npy2, pack2(h0.y, h0.y));
+      const float u = __fmul_rn(h0.z, dx);
+      const f32x2 s2 = fma2(dy2, pack2(h0.w, h0.w), pack2(u, u));
+      f32x2 q2 = mul2(s2, pack2(dx, dx));
+      const f32x2 v2 = mul2(dy2, pack2(hq.x, hq.x));
+      q2 = fma2(v2, dy2, q2);
+      float qa, qb;
+      unpack2(q2, qa, qb);
+      const bool pass_a = !(qa > hq.y), pass_b = !(qb > hq.y);
+      const float e_a = ex2_approx_ftz(__fmul_rn(qa, -1.4426950408889634f));
+      const float e_b = ex2_approx_ftz(__fmul_rn(qb, -1.4426950408889634f));
+      const float raw_a = __fmul_rn(hq.z, e_a), raw_b = __fmul_rn(hq.z, e_b);
+      const float al_a = pass_a ? fminf(kAlphaCap, raw_a) : 0.0f, al_b = pass_b ? fminf(kAlphaCap, raw_b) : 0.0f;
+      // gradients flow through alpha only where the cut passed and the cap is not active
+      const float m_a = (pass_a && raw_a <= kAlphaCap) ? 1.0f : 0.0f, m_b = (pass_b && raw_b <= kAlphaCap) ? 1.0f : 0.0f;
+      const f32x2 alpha2 = pack2(al_a, al_b);
+      const f32x2 rinv2 = pack2(__frcp_rn(1.0f - al_a), __frcp_rn(1.0f - al_b));
+      f32x2 dal = pack2(0.f, 0.f);
+      f32x2 dc0[3] = {dal, dal, dal}, dc1[3] = {dal, dal, dal};
+      const uint32_t act1 = actl & (tag >> 16), act0 = actl ^ act1;
+      {
+        const float4 k0 = lds128(addr + 32u);  // {rgb - bg, -}
+#pragma unroll
+        for (int s = 0; s < S; ++s)
+          if ((act0 >> s) & 1u)
+            slot_backward(T2[s], G2[s], gr2[s], gg2[s], gb2[s], Gf2[s], alpha2, rinv2, k0.x, k0.y, k0.z, dal, dc0[0], dc0[1], dc0[2]);
+      }
+      if (act1 != 0) {
+        const float4 k1 = lds128(addr + 48u);  // {rgb with SH residual - bg, -}
+#pragma unroll
+        for (int s = 0; s < S; ++s)
+          if ((act1 >> s) & 1u)
+            slot_backward(T2[s], G2[s], gr2[s], gg2[s], gb2[s], Gf2[s], alpha2, rinv2, k1.x, k1.y, k1.z, dal, dc1[0], dc1[1], dc1[2]);
+      }
+      // per pixel: dL/do = exp(-q) dal, dL/dq = -alpha dal, then the chain through q; the two pixels added
+      float v[16];
+#pragma unroll
+      for (int ch = 0; ch < 3; ++ch) {
+        float lo, hi;
+        unpack2(dc0[ch], lo, hi); v[ch] = lo + hi;
+        unpack2(dc1[ch], lo, hi); v[3 + ch] = lo + hi;
+      }
+      float da_a, da_b, dya, dyb;
+      unpack2(dal, da_a, da_b);
+      unpack2(dy2, dya, dyb);
+      da_a *= m_a; da_b *= m_b;
+      const float dq_a = -al_a * da_a, dq_b = -al_b * da_b;
+      v[6] = e_a * da_a + e_b * da_b;
+      v[7] = (dq_a + dq_b) * dx * dx;
+      v[8] = (dq_a * dya + dq_b * dyb) * dx;
+      v[9] = dq_a * dya * dya + dq_b * dyb * dyb;
+      v[10] = dq_a * (2.0f * h0.z * dx + h0.w * dya) + dq_b * (2.0f * h0.z * dx + h0.w * dyb);
+      v[11] = dq_a * (h0.w * dx + 2.0f * hq.x * dya) + dq_b * (h0.w * dx + 2.0f * hq.x * dyb);
+      v[12] = v[13] = v[14] = v[15] = 0.0f;
+      int comp;
+      const float tot = warp_sum_16(v, lane, comp);
+      if ((lane & 1) == 0 && comp < 12 && tot != 0.0f)
+        atomicAdd(a.grad + 12 * (size_t)lds32(ib0 + 4u * j) + comp, tot * kInvTScale);
+    }
+    n_cur = n_nxt;
+    __syncwarp();
+  }
+}
+
+constexpr int kBackwardStateBlock = 4;
+
+void launch_backward(const DeviceScene& sc, const WsHeader& h, Workspace& ws, const float* images, const float* gimg,
+                     float* grad, cudaStream_t st) {
+  const int n_rec = sc.N * sc.V;
+  if (n_rec > 0) cudaMemsetAsync(grad, 0, sizeof(float) * 12 * (size_t)n_rec, st);
+  if (h.B == 0 || n_rec == 0) return;
+  BackwardArgs a;
+  a.rec = ws.rec; a.qlist = ws.qlist; a.qrange = ws.qrange; a.depth = ws.depth;
+  a.B = h.B; a.C = sc.C;
+  a.nsb = (h.B + kBackwardStateBlock - 1) / kBackwardStateBlock;
+  a.W = h.W; a.H = h.H; a.TX = h.TX; a.tiles = h.TX * h.TY;
+  a.bg[0] = sc.bg[0]; a.bg[1] = sc.bg[1]; a.bg[2] = sc.bg[2];
+  a.images = images; a.gimg = gimg; a.grad = grad;
+  const size_t smem = sizeof(uint16_t) * 4 * (size_t)sc.C;
+  if (smem > 40 * 1024)
+    cudaFuncSetAttribute(k_backward_q<kBackwardStateBlock>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                         (int)(sizeof(uint16_t) * 4 * kMaxC));
+  const long long grid = (long long)a.tiles * 4 * a.nsb;
+  k_backward_q<kBackwardStateBlock><<<(unsigned)grid, 32, smem, st>>>(a);
+  count_launches(1);
+}
+
+}  // namespace gsr

@@ -35,35 +35,6 @@
 
 namespace gsr {
 
-typedef unsigned long long f32x2;
-constexpr float kTScale = 1099511627776.0f;                       // 2^40
-constexpr float kTStopScaled = 109951160.0f;                      // 1e-4f * 2^40 (0x4CD1B717)
-constexpr float kInvTScale = 9.094947017729282379150390625e-13f;  // 2^-40
-
-__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
-  f32x2 r;
-  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-  return r;
-}
-__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) {
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
-  f32x2 r;
-  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
-  return r;
-}
-__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
-  f32x2 r;
-  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
-  return r;
-}
-__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
-  f32x2 r;
-  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
-  return r;
-}
-
 // One slot, two pixels: DESIGN.md §3.5 in the scaled form of the header.  8 instructions, all on the FMA pipe.
 __device__ __forceinline__ void slot_update(f32x2& T, f32x2& Cr, f32x2& Cg, f32x2& Cb, f32x2 alpha2, float cr,
                                             float cg, float cb) {
@@ -88,17 +59,7 @@ __device__ __forceinline__ void slot_update(f32x2& T, f32x2& Cr, f32x2& Cg, f32x
       : "l"(alpha2), "f"(cr), "f"(cg), "f"(cb));
 }
 
-__device__ __forceinline__ void cp_async16(uint32_t saddr, const void* gptr) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(saddr), "l"(gptr) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() {
-  asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
-}
-
 constexpr int kRecordUnroll = 2;
-constexpr int kChunk = 32;  // list entries staged per round: one per lane
 
 template <int S, bool COUNT>
 __global__ void __launch_bounds__(32, (S <= 5 ? 32 : (S <= 6 ? 28 : (S <= 8 ? 24 : 5)))) k_composite_q(const CompositeArgs a) {

@@ -77,6 +77,9 @@ def lib():
         L.gsr_group_utility.argtypes = [vp, vp, vp, vp, vp, i32, i32, vp, vp, vp, vp]
         L.gsr_group_utility_b.argtypes = [vp, vp, i32, vp, vp, vp, i32, i32, vp, vp, vp, vp]
         L.gsr_index_status.argtypes = [vp]
+        L.gsr_num_records.argtypes = [vp]
+        L.gsr_num_records.restype = i64
+        L.gsr_render_backward.argtypes = [vp, vp, vp, vp, i32, vp, vp]
         L.gsr_close_levels.argtypes = [vp, i64, vp, vp, vp]
         L.gsr_frame_workspace_bytes.argtypes = [vp, C.POINTER(CameraC), i32, i32, i32, i32]
         L.gsr_frame_workspace_bytes.restype = sz
@@ -255,6 +258,20 @@ class Scene:
         _check(lib().gsr_render_states_vs_full(self.handle, C.byref(camera_struct(cam)), C.c_float(t), _dp(levels),
                                                B, _dp(out), _dp(ref_out), _dp(mse), _dp(psnr), _dp(workspace),
                                                workspace.numel(), _stream()))
+
+    def num_records(self) -> int:
+        return int(lib().gsr_num_records(self.handle))
+
+    def render_backward(self, workspace, images, dL_dimages):
+        """gsr_render_backward after a forward call on `workspace`: images, dL_dimages cuda float32 [B,H,W,3] ->
+        cuda float32 [num_records, 12] (see include/gsr.h for the columns)."""
+        torch = _torch()
+        for t in (images, dL_dimages):
+            assert t.dtype == torch.float32 and t.is_cuda and t.is_contiguous() and t.shape == images.shape
+        grad = torch.empty((self.num_records(), 12), dtype=torch.float32, device="cuda")
+        _check(lib().gsr_render_backward(self.handle, _dp(workspace), _dp(images), _dp(dL_dimages),
+                                         int(images.shape[0]), _dp(grad), _stream()))
+        return grad
 
     def debug_pair_counts(self, workspace) -> np.ndarray:
         c = np.zeros(3, np.int64)

@@ -136,6 +136,10 @@ def test_b4_linearity_in_the_image_gradient_and_mse_chain(oracle_mod):
     a, b = sc.backward(cam, 0.0, depth, g1, proj=p0), sc.backward(cam, 0.0, depth, g2, proj=p0)
     c = sc.backward(cam, 0.0, depth, 2.0 * g1 - 3.0 * g2, proj=p0)
     assert np.allclose(c, 2.0 * a - 3.0 * b, rtol=1e-10, atol=1e-12)
+    # the magnitude the GPU parity bar uses dominates the gradient entry by entry and does not depend on signs
+    a2, mag = sc.backward(cam, 0.0, depth, g1, proj=p0, want_abs=True)
+    assert np.array_equal(a2, a) and np.all(mag >= np.abs(a))
+    assert np.allclose(sc.backward(cam, 0.0, depth, -g1, proj=p0, want_abs=True)[1], mag, rtol=1e-12)
     R = rng.uniform(0, 1, (cam.H, cam.W, 3))
     img = sc.render(cam, 0.0, depth, brute_force=True, proj=p0)[0]
     grad = sc.backward(cam, 0.0, depth, 2.0 * (img - R) / img.size, proj=p0)

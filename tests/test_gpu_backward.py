@@ -1,0 +1,131 @@
+"""GPU parity of gsr_render_backward (include/gsr.h) against the backward oracle (oracle O-8) through
+the C ABI: for a batch of states with random dL/d(image), the per-record gradients summed over the states.
+Floating point with atomics: by tolerance (stated per test), never bitwise."""
+import numpy as np
+import pytest
+
+from paper_2606_17212_b200 import synth
+from tests.test_backward_pins import smooth_scene
+from tests.helpers import axis_camera, tiny_scene
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_mod():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+@pytest.fixture(scope="module")
+def gsr(torch_mod):
+    from paper_2606_17212_b200 import gsr as G
+    G.lib()
+    return G
+
+
+def oracle_record_grads(oracle_mod, scn, cam, t, lv, g, V=2):
+    """The oracle's per-state [N, 9] gradients mapped onto the records the GPU composites and summed over states:
+    record = V i + variant (V = 2: variant 0 at cluster depth 0, else 1; V = 4: variant = depth); columns
+    (rgb[3], rgb with SH residual[3], opacity, A, B, Cq, mx, my) — depth 3 uses the second colour (V = 2)."""
+    osc = oracle_mod.OracleScene(scn)
+    N = scn.N
+    cl = scn.cluster_of()
+    out, out_abs = np.zeros((V * N, 12)), np.zeros((V * N, 12))
+    for b in range(lv.shape[0]):
+        gr, ga = osc.backward(cam, t, lv[b], g[b].astype(np.float64), want_abs=True)
+        d = lv[b][cl].astype(np.int64)
+        variant = np.where(d == 0, 0, 1) if V == 2 else np.clip(d, 0, 3)
+        rid = V * np.arange(N) + variant
+        live = np.any(gr != 0.0, axis=1)
+        col = np.where((d == 3) & (V == 2), 3, 0)
+        for i in np.nonzero(live)[0]:
+            out[rid[i], col[i]:col[i] + 3] += gr[i, :3]
+            out[rid[i], 6:] += gr[i, 3:]
+            out_abs[rid[i], col[i]:col[i] + 3] += ga[i, :3]
+            out_abs[rid[i], 6:] += ga[i, 3:]
+    return out, out_abs
+
+
+def _run(gsr, torch, scn, cam, t, lv, seed):
+    scene = gsr.Scene(scn)
+    ws = scene.new_workspace(cam, lv.shape[0])
+    dlv = torch.from_numpy(np.ascontiguousarray(lv, np.int8)).cuda()
+    out, _, _ = scene.render_states(cam, t, dlv, workspace=ws)
+    scene.status(ws)
+    rng = np.random.default_rng(seed)
+    g = rng.standard_normal(tuple(out.shape)).astype(np.float32)
+    grad = scene.render_backward(ws, out, torch.from_numpy(g).cuda()).cpu().numpy().astype(np.float64)
+    V = scene.num_records() // scn.N
+    scene.close()
+    return grad, g, V
+
+
+def _compare(got, want_and_abs, k_eps=64.0):
+    """Every entry is a sum of many signed fp32 terms (per pixel and state; atomics order on the GPU, double in the
+    oracle), often strongly cancelling (dB on a symmetric footprint).  The bar is the floating-point one:
+    |got - want| <= k_eps * 2^-24 * (the entry's magnitude: every product in absolute value, the suffix of a pixel
+    counted as everything the pixel is made of — the kernel forms it as final pixel minus prefix), from the oracle
+    (grad_abs).  The GPU's factors carry ~1e-6 relative error each (fp32 alpha, ex2.approx, rcp, the fp32 forward
+    pixel), hence k_eps = 64."""
+    want, wabs = want_and_abs
+    err = np.abs(got - want)
+    bound = k_eps * 2.0 ** -24 * wabs
+    bad = err > bound + 1e-30
+    assert not bad.any(), (np.argwhere(bad)[:5], err[bad][:5], bound[bad][:5])
+    # and in relative terms wherever the sum is not dominated by cancellation
+    solid = np.abs(want) > 0.05 * wabs
+    assert np.all(err[solid] <= 2e-4 * np.abs(want[solid]))
+    # records no state composites have exactly zero gradient on both sides
+    dead = ~np.any(wabs != 0.0, axis=1)
+    assert np.all(got[dead] == 0.0)
+
+
+def test_backward_smooth_three_gaussians(gsr, torch_mod, oracle_mod):
+    scn, cam = smooth_scene()
+    lv = np.zeros((1, 1), np.int8)
+    got, g, V = _run(gsr, torch_mod, scn, cam, 0.0, lv, 1)
+    want = oracle_record_grads(oracle_mod, scn, cam, 0.0, lv, g, V)
+    _compare(got, want)
+
+
+def test_backward_cap_and_stop(gsr, torch_mod, oracle_mod):
+    cam = axis_camera(32, 32, 100.0, 4.0, cx=16.5, cy=16.5)
+    lv = np.zeros((1, 1), np.int8)
+    scn, _ = tiny_scene([[0, 0, 0]], 20.0, logits=12.0, colors=(0.5, 0.5, 0.5))          # capped everywhere
+    got, g, V = _run(gsr, torch_mod, scn, cam, 0.0, lv, 2)
+    want = oracle_record_grads(oracle_mod, scn, cam, 0.0, lv, g, V)
+    _compare(got, want)
+    assert np.all(got[:, 6:] == 0.0)
+    scn, _ = tiny_scene([[0, 0, 0.01 * k] for k in range(20)], 5.0, logits=0.0, colors=(0.7, 0.7, 0.7))   # stop after 13
+    got, g, V = _run(gsr, torch_mod, scn, cam, 0.0, lv, 3)
+    want = oracle_record_grads(oracle_mod, scn, cam, 0.0, lv, g, V)
+    _compare(got, want)
+    assert (np.any(got != 0.0, axis=1)).sum() == 13
+
+
+@pytest.mark.parametrize("bg", [(0.0, 0.0, 0.0), (1.0, 1.0, 1.0)])
+def test_backward_batch_of_states_scaled_scene(gsr, torch_mod, oracle_mod, bg):
+    wl = synth.scaled_object_workload(23, C=5, per_cluster=260.0, W=120, H=88, fov=40.0, n_frames=1, B=14)
+    wl.scene.background = np.asarray(bg, np.float32)
+    cam, t = wl.frames[0]
+    lv = wl.levels[0].copy()
+    lv[0] = 3
+    lv[1] = -1
+    lv[2] = 0                                               # all-full, all-absent and all-base states among them
+    got, g, V = _run(gsr, torch_mod, wl.scene, cam, t, lv, 4)
+    want = oracle_record_grads(oracle_mod, wl.scene, cam, t, lv, g, V)
+    assert np.any(want[0][:, 3:6] != 0.0) and np.any(want[0][0::2] != 0.0)   # both colours and both variants occur
+    _compare(got, want)
+
+
+def test_backward_refuses_a_workspace_of_another_batch(gsr, torch_mod):
+    scn, cam = smooth_scene()
+    scene = gsr.Scene(scn)
+    ws = scene.new_workspace(cam, 2)
+    lv = torch_mod.zeros((2, 1), dtype=torch_mod.int8, device="cuda")
+    out, _, _ = scene.render_states(cam, 0.0, lv, workspace=ws)
+    with pytest.raises(gsr.GsrError):
+        scene.render_backward(ws, out[:1].contiguous(), out[:1].contiguous())
+    scene.close()
