@@ -475,6 +475,30 @@ def measure_ours(args, workload: str, steps: int, warmup: int, full: bool):
                   "share_of_step": (proj_ms + sort_ms) / ms_serial}
     roofline.update(traffic_record(wl.name))
 
+    # ---- backward of the compositor (gsr_render_backward; SURVEY.md §8(f)-4 follow-on): forward + backward of the
+    #      same frames, one frame in flight, dL/d(image) resident (a fixed random tensor: the kernel's work does not
+    #      depend on its values)
+    backward = None
+    if full and not args.no_backward:
+        n_b = min(steps, 6)
+        gimg = torch.randn((B, H, W, 3), dtype=torch.float32, device=dev) * (2.0 / (3.0 * W * H))
+        b0 = bufs[0]
+
+        def fwd_bwd(k, with_bwd=True):
+            frame_into(b0, k, True)
+            if with_bwd:
+                scene.render_backward(b0["ws"], b0["out"], gimg)
+
+        for k in range(2):
+            fwd_bwd(warmup + k)
+        ms_fb = timed(fwd_bwd, warmup, n_b)
+        ms_f = timed(lambda k: fwd_bwd(k, False), warmup, n_b)
+        backward = {"value": B * n_b * world / (ms_fb * 1e-3), "unit": "states/s (forward + backward)",
+                    "ms_per_step_forward_backward": ms_fb / n_b, "ms_per_step_forward": ms_f / n_b,
+                    "ms_per_step_backward": (ms_fb - ms_f) / n_b, "steps": n_b,
+                    "note": "gsr_render_states_vs_full + gsr_render_backward, one frame in flight; grad [records, 12] summed over the %d states" % B}
+        del gimg
+
     # ---- CPU oracle on this box's cores, bounded sample of the same workload
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
@@ -502,7 +526,7 @@ def measure_ours(args, workload: str, steps: int, warmup: int, full: bool):
     if full:
         line.update({"repetitions": n_rep, "value_reps": value_reps, "value_ci95": ci95,
                      "ms_per_step_reps": [m / steps for m in ms_reps], "sustained": sustained,
-                     "value_without_images": B * steps * world / (ms_noimg * 1e-3), "e2e": e2e,
+                     "value_without_images": B * steps * world / (ms_noimg * 1e-3), "e2e": e2e, "backward": backward,
                      "context": {"paper_h100_pcie_utility_states_per_s": 1889.7,
                                  "note": "PAPER.md:150, other hardware, unstated resolution/scene: context only"}})
     if dist is not None:
@@ -714,6 +738,7 @@ def main():
     ap.add_argument("--workload", default="cfg1", choices=["cfg0", "cfg1", "cfg1r", "cfg2", "cfg3", "cfg4", "atlas"])
     ap.add_argument("--ref-states", type=int, default=64, help="states per frame the CPU oracle renders")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-backward", action="store_true", help="skip the forward + backward timing")
     ap.add_argument("--no-sub-workloads", action="store_true",
                     help="cfg1 only: skip the compact cfg2 / cfg3 / cfg4 / atlas sub-records")
     ap.add_argument("--state-block", type=int, default=0, help="states per compositing CTA (0 = library default)")

@@ -16,7 +16,7 @@
 // the forward's operations on the same operands) — and the forward image is an input.
 //
 // Layout of the work: the forward's (k_composite_q.cu): one warp per 8x8 quadrant x S states, two pixels per lane on
-// packed FP32; per (pixel pair, state) T, G and the constants g[3], Gf live in registers (12 per slot, S = 4).
+// packed FP32; per (pixel pair, state) T, G and the constants g[3], Gf live in registers (12 per slot, S = 8).
 // Per record the 12 partial sums of the lane's pixels and states are reduced over the warp with the
 // slot-splitting butterfly (16 shuffles instead of 60) and added to grad with one atomic per component.
 // Float atomics make the summation order, hence the last bits of grad, run-dependent; parity is by tolerance.
@@ -303,7 +303,7 @@ __global__ void __launch_bounds__(32) k_backward_q(const BackwardArgs a) {
   }
 }
 
-constexpr int kBackwardStateBlock = 4;
+constexpr int kBackwardStateBlock = 8;  // measured on cfg1 (ms per 256-state frame): S = 2: 25.4, 4: 20.2, 8: 17.5
 
 void launch_backward(const DeviceScene& sc, const WsHeader& h, Workspace& ws, const float* images, const float* gimg,
                      float* grad, cudaStream_t st) {
