@@ -13,6 +13,8 @@ struct CompositeArgs {
   const int8_t* depth;   // [B, C] validated delivered depths
   int32_t B, C, nsb;
   int32_t W, H, TX, tiles;
+  uint32_t n_items;        // work items of the launch = tiles * 4 * nsb
+  uint32_t* work_counter;  // next work item (zeroed before the launch)
   float bg[3];
   float* out;          // [B,H,W,3] or nullptr
   const float* ref;    // [H,W,3] or nullptr

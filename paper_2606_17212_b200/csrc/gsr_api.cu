@@ -103,6 +103,7 @@ size_t carve_workspace(Workspace* ws, void* base, int32_t N, int32_t C, int32_t 
   w.uorder = (uint32_t*)take(sizeof(uint32_t) * (size_t)(B > 0 ? B : 1) * tiles);
   w.upos = (uint32_t*)take(sizeof(uint32_t) * (size_t)(B > 0 ? B : 1) * tiles);
   w.n_unique = (uint32_t*)take(sizeof(uint32_t) * (size_t)tiles);
+  w.work_counter = (uint32_t*)take(sizeof(uint32_t));
   w.bytes = off;
   if (ws) *ws = w;
   return off;

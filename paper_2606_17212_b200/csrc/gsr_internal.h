@@ -84,6 +84,7 @@ struct Workspace {
   uint32_t* uorder;       // [tiles * B] states sorted by their tile-restricted signature (k_tile_dedup)
   uint32_t* upos;         // [tiles * B] upos[tile*B + u] = index in uorder of the first member of class u
   uint32_t* n_unique;     // [tiles] number of distinct signatures
+  uint32_t* work_counter; // next work item of the persistent compositing warps
   size_t bytes;           // total
 };
 

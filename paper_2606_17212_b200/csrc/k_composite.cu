@@ -133,6 +133,7 @@ static CompositeArgs make_args(const DeviceScene& sc, const FrameParams& fp, Wor
   a.out = nullptr; a.ref = nullptr; a.counts = nullptr;
   a.uorder = nullptr; a.upos = nullptr; a.n_unique = nullptr;
   a.rec = ws.rec; a.qlist = ws.qlist; a.qrange = ws.qrange; a.sse_blk = ws.sse_blk;
+  a.work_counter = ws.work_counter; a.n_items = 0;
   return a;
 }
 

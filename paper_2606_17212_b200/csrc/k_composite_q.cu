@@ -70,15 +70,23 @@ __global__ void __launch_bounds__(32, (S <= 5 ? 32 : (S <= 6 ? 28 : (S <= 8 ? 24
   __shared__ uint32_t s_mlo[S], s_mhi[S];  // members of the class: uorder[tile*B + [mlo, mhi))
 
   const int lane = threadIdx.x;
-  const uint32_t tq = blockIdx.x / (uint32_t)a.nsb;  // 4 * tile + quadrant
-  const int sb = (int)(blockIdx.x - tq * (uint32_t)a.nsb);
+  // Persistent warps: the grid is one wave of one-warp CTAs and every warp takes work items — (tile, quadrant,
+  // state block) in launch order — from a counter until none is left, so that a register slot is never empty
+  // between two CTAs (one-warp CTAs live ~30 us; the launch gap showed as 5.5 of 7 warps resident).
+  for (;;) {
+  uint32_t item = 0;
+  if (lane == 0) item = atomicAdd(a.work_counter, 1u);
+  item = __shfl_sync(0xffffffffu, item, 0);
+  if (item >= a.n_items) break;
+  const uint32_t tq = item / (uint32_t)a.nsb;  // 4 * tile + quadrant
+  const int sb = (int)(item - tq * (uint32_t)a.nsb);
   const int tile = (int)(tq >> 2), quad = (int)(tq & 3u);
   const int b0 = sb * S;  // first slot of this block: a state index, or a class index when dedup is on
 
   // ---- which states this warp composites.  With tile-level dedup (k_tile_dedup) slot s is the s-th distinct
   //      signature class of this tile from b0 on; its first member stands for the class.
   const int n_slots = a.n_unique ? (int)a.n_unique[tile] : a.B;
-  if (b0 >= n_slots) return;
+  if (b0 >= n_slots) continue;
   if (lane < S) {
     const int u = b0 + lane;
     int rep = -1;
@@ -279,7 +287,7 @@ __global__ void __launch_bounds__(32, (S <= 5 ? 32 : (S <= 6 ? 28 : (S <= 8 ? 24
       atomicAdd(a.counts + 1, n_state);
       atomicAdd(a.counts + 2, n_logical);
     }
-    return;
+    continue;
   }
 
   // ---- pixel = bg + 2^-40 C (C accumulated relative to the background, scaled); optional fused squared error
@@ -342,6 +350,8 @@ __global__ void __launch_bounds__(32, (S <= 5 ? 32 : (S <= 6 ? 28 : (S <= 8 ? 24
       }
     }
   }
+  __syncwarp();  // the shared tables and buffers are rewritten by the next item
+  }
 }
 
 // One CTA per state.  The tree is the one of reduce.cuh — per tile the eight block partials in index order, tiles
@@ -389,11 +399,21 @@ void launch_distortion_finalize_blk(const double* blk, int32_t B, int32_t tiles,
 template <int S, bool COUNT>
 static void launch_q_S(const CompositeArgs& a, cudaStream_t st) {
   const size_t smem = sizeof(uint16_t) * 4 * (size_t)a.C;
-  const long long grid = (long long)a.tiles * 4 * a.nsb;
+  const long long items = (long long)a.tiles * 4 * a.nsb;
   if (smem > 40 * 1024)  // static + dynamic shared memory passes 48 KB for very large C
     cudaFuncSetAttribute(k_composite_q<S, COUNT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                          (int)(sizeof(uint16_t) * 4 * kMaxC));
-  k_composite_q<S, COUNT><<<(unsigned)grid, 32, smem, st>>>(a);
+  // one wave: as many one-warp CTAs as fit the device at this kernel's register and shared-memory use
+  int dev = 0, sms = 1, per_sm = 1;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_composite_q<S, COUNT>, 32, smem);
+  const long long wave = (long long)sms * (per_sm > 0 ? per_sm : 1);
+  CompositeArgs b = a;
+  b.n_items = (uint32_t)items;
+  cudaMemsetAsync(b.work_counter, 0, sizeof(uint32_t), st);
+  const long long grid = items < wave ? items : wave;
+  k_composite_q<S, COUNT><<<(unsigned)grid, 32, smem, st>>>(b);
 }
 
 // States per warp.  Measured on cfg1 (states/s, 4 frames in flight): S = 4: 78.5 k, 5: 83.7 k, 6: 86.0 k, 7: 78.4 k,
