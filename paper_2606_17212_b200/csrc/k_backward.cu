@@ -36,6 +36,8 @@ struct BackwardArgs {
   const float* images;   // [B,H,W,3] forward output
   const float* gimg;     // [B,H,W,3] dL/d(image)
   float* grad;           // [records, 12]
+  uint32_t n_items;        // tiles * 4 * nsb
+  uint32_t* work_counter;  // zeroed before the launch
 };
 
 // The butterfly of reduce.cuh for 16 floats per lane: after the call the lane holds the warp total of component
@@ -100,8 +102,13 @@ __global__ void __launch_bounds__(32) k_backward_q(const BackwardArgs a) {
   __shared__ uint32_t s_rid[2][kChunk];  // record id (row of grad)
 
   const int lane = threadIdx.x;
-  const uint32_t tq = blockIdx.x / (uint32_t)a.nsb;  // 4 * tile + quadrant
-  const int sb = (int)(blockIdx.x - tq * (uint32_t)a.nsb);
+  for (;;) {  // persistent warps: work items (tile, quadrant, state block) from a counter, as in k_composite_q
+  uint32_t item = 0;
+  if (lane == 0) item = atomicAdd(a.work_counter, 1u);
+  item = __shfl_sync(0xffffffffu, item, 0);
+  if (item >= a.n_items) break;
+  const uint32_t tq = item / (uint32_t)a.nsb;  // 4 * tile + quadrant
+  const int sb = (int)(item - tq * (uint32_t)a.nsb);
   const int tile = (int)(tq >> 2), quad = (int)(tq & 3u);
   const int b0 = sb * S;  // slot s = state b0 + s (no tile-level dedup here: every state has its own g)
 
@@ -301,6 +308,8 @@ __global__ void __launch_bounds__(32) k_backward_q(const BackwardArgs a) {
     n_cur = n_nxt;
     __syncwarp();
   }
+  __syncwarp();  // the shared tables and buffers are rewritten by the next item
+  }
 }
 
 constexpr int kBackwardStateBlock = 8;  // measured on cfg1 (ms per 256-state frame): S = 2: 25.4, 4: 20.2, 8: 17.5
@@ -321,8 +330,16 @@ void launch_backward(const DeviceScene& sc, const WsHeader& h, Workspace& ws, co
   if (smem > 40 * 1024)
     cudaFuncSetAttribute(k_backward_q<kBackwardStateBlock>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                          (int)(sizeof(uint16_t) * 4 * kMaxC));
-  const long long grid = (long long)a.tiles * 4 * a.nsb;
-  k_backward_q<kBackwardStateBlock><<<(unsigned)grid, 32, smem, st>>>(a);
+  const long long items = (long long)a.tiles * 4 * a.nsb;
+  int dev = 0, sms = 1, per_sm = 1;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_backward_q<kBackwardStateBlock>, 32, smem);
+  const long long wave = (long long)sms * (per_sm > 0 ? per_sm : 1);
+  a.n_items = (uint32_t)items;
+  a.work_counter = ws.work_counter;
+  cudaMemsetAsync(ws.work_counter, 0, sizeof(uint32_t), st);
+  k_backward_q<kBackwardStateBlock><<<(unsigned)(items < wave ? items : wave), 32, smem, st>>>(a);
   count_launches(1);
 }
 
