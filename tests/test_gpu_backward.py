@@ -129,3 +129,61 @@ def test_backward_refuses_a_workspace_of_another_batch(gsr, torch_mod):
     with pytest.raises(gsr.GsrError):
         scene.render_backward(ws, out[:1].contiguous(), out[:1].contiguous())
     scene.close()
+
+
+def test_backward_four_variant_scene(gsr, torch_mod, oracle_mod):
+    """Scenes with position residual levels / attribute refinements project FOUR records per Gaussian (record =
+    4 i + cluster depth, one colour each): the gradients land on the variant the state composites."""
+    wl = synth.scaled_object_workload(29, C=4, per_cluster=220.0, W=104, H=72, fov=40.0, n_frames=1, B=10)
+    scn = synth.with_attribute_refinements(synth.with_position_residuals(wl.scene))
+    cam, t = wl.frames[0]
+    lv = wl.levels[0].copy()
+    lv[0], lv[1], lv[2], lv[3] = 3, 2, 1, 0
+    got, g, V = _run(gsr, torch_mod, scn, cam, t, lv, 6)
+    assert V == 4
+    want = oracle_record_grads(oracle_mod, scn, cam, t, lv, g, V)
+    assert all(np.any(want[0][v::4] != 0.0) for v in range(4))           # every variant receives gradient
+    assert np.all(got[:, 3:6] == 0.0)                                    # one colour per record: the second triple is unused
+    _compare(got, want)
+
+
+def test_backward_full_size_cfg1_identities(gsr, torch_mod):
+    """configs[1] at full size (800x800, B = 256, the batch bench.py times): two properties that hold at any size.
+    (1) Colour identity: pixel - bg = sum_i w_i (c_i - bg) and dL/dc_i = sum w_i g, hence
+        sum_records (c - bg) . dL/dc = sum_{state, pixel} g . (image - bg)   (both colour triples, fp32 sums).
+    (2) Batch consistency: the gradient of a batch whose dL/d(image) is non-zero for ONE state equals the gradient
+        of that state rendered alone with the same dL/d(image) (other state block, other presence tables)."""
+    torch = torch_mod
+    wl = synth.workload_cfg1(n_frames=2)
+    cam, t = wl.frames[1]
+    lv = wl.levels[1]
+    B = lv.shape[0]
+    scene = gsr.Scene(wl.scene)
+    ws = scene.new_workspace(cam, B)
+    dlv = torch.from_numpy(np.ascontiguousarray(lv)).cuda()
+    out, _, _ = scene.render_states(cam, t, dlv, workspace=ws)
+    scene.status(ws)
+    gen = torch.Generator(device="cuda").manual_seed(11)
+    g = torch.randn(out.shape, generator=gen, device="cuda", dtype=torch.float32)
+    grad = scene.render_backward(ws, out, g).double()
+    P = scene.debug_projection(ws)
+    bg = torch.from_numpy(np.asarray(wl.scene.background, np.float64)).cuda()
+    c0 = torch.from_numpy(P["rgb_base"].astype(np.float64)).cuda() - bg
+    c1 = torch.from_numpy(P["rgb_res"].astype(np.float64)).cuda() - bg
+    lhs = float((c0 * grad[:, 0:3]).sum() + (c1 * grad[:, 3:6]).sum())
+    rhs = float((g.double() * (out.double() - bg)).sum())
+    mag = float((c0.abs() * grad[:, 0:3].abs()).sum() + (c1.abs() * grad[:, 3:6].abs()).sum())
+    assert abs(lhs - rhs) <= 2e-5 * mag, (lhs, rhs, mag)
+    # (2) one state of the batch alone
+    b = 137
+    g1 = torch.zeros_like(g)
+    g1[b] = g[b]
+    grad_b = scene.render_backward(ws, out, g1)
+    ws1 = scene.new_workspace(cam, 1)
+    out1, _, _ = scene.render_states(cam, t, dlv[b:b + 1].contiguous(), workspace=ws1)
+    assert torch.equal(out1[0], out[b])
+    grad_1 = scene.render_backward(ws1, out1, g[b:b + 1].contiguous())
+    scale = grad_1.abs().amax(dim=0).clamp_min(1e-20)
+    assert float(((grad_b - grad_1).abs() / scale).max()) <= 2e-4
+    assert bool((grad_b != 0).any())
+    scene.close()
