@@ -351,7 +351,7 @@ def measure_ours(args, workload: str, steps: int, warmup: int, full: bool):
         sustained = {"value": B * n_sus * world / (ms_sus * 1e-3), "unit": "states/s", "steps": n_sus,
                      "seconds": ms_sus * 1e-3, "ms_per_step": ms_sus / n_sus, "clocks": sus_clocks}
 
-    # ---- the same steps one frame at a time with CUDA events around every k_composite launch and around the
+    # ---- the same steps one frame at a time with CUDA events around every k_composite_q launch and around the
     #      memory-bound phases: what the roofline objects are computed from (events of overlapping streams
     #      would count co-running kernels twice)
     gsr.set_option("profile", 1)
@@ -424,7 +424,7 @@ def measure_ours(args, workload: str, steps: int, warmup: int, full: bool):
         b["out"] = None
     torch.cuda.empty_cache()
 
-    # ---- roofline of the dominant kernel (k_composite): counted work / CUDA-event time / FP32 peak
+    # ---- roofline of the dominant kernel (k_composite_q): counted work / CUDA-event time / FP32 peak
     bufs[0]["out"] = torch.empty((B, H, W, 3), dtype=torch.float32, device=dev)
     n_cnt = min(steps, 6)
     cnt = np.zeros(3, np.float64)
@@ -436,7 +436,7 @@ def measure_ours(args, workload: str, steps: int, warmup: int, full: bool):
     flop_alg = cnt[0] * FLOP_SHARED + cnt[1] * FLOP_STATE
     peak_meas = gsr.measure_fp32_peak()
     achieved = flop_alg / comp_s / 1e12 if comp_s > 0 else 0.0
-    roofline = {"kernel": "k_composite", "bound": "alu", "achieved": achieved, "peak": peak_meas, "unit": "TFLOP/s",
+    roofline = {"kernel": "k_composite_q", "bound": "alu", "achieved": achieved, "peak": peak_meas, "unit": "TFLOP/s",
                 "frac": achieved / peak_meas if peak_meas else None, "traffic": None,
                 "peak_kind": "measured here: FFMA-chain kernel (gsr_measure_fp32_peak); nominal %.1f" % NOMINAL_FP32_TFLOPS,
                 "kernel_ms_per_launch": comp_ms / max(comp_n, 1), "kernel_launches": comp_n,
@@ -654,7 +654,7 @@ def measure_atlas(args, steps: int, warmup: int, full: bool):
     comp_s = comp_ms * 1e-3 / steps
     peak = gsr.measure_fp32_peak()
     achieved = (cnt[0] * FLOP_SHARED + cnt[1] * FLOP_STATE) / comp_s / 1e12
-    roofline = {"kernel": "k_composite", "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+    roofline = {"kernel": "k_composite_q", "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                 "frac": achieved / peak, "traffic": None,
                 "peak_kind": "measured here: FFMA-chain kernel (gsr_measure_fp32_peak); nominal %.1f" % NOMINAL_FP32_TFLOPS,
                 "kernel_ms_per_launch": comp_ms / max(comp_n, 1), "kernel_launches": comp_n,

@@ -8,7 +8,7 @@ namespace gsr {
 
 struct CompositeArgs {
   const float4* rec;     // [4 * records] packed 64-byte records (k_project)
-  const uint2* qlist;    // per (tile, 8x8 quadrant) render lists of {record id, meta} (k_tile_render_list)
+  const uint2* qlist;    // per (tile, 8x8 quadrant) render lists of {record id, meta} (tile_render_lists in k_tile_sort)
   const uint2* qrange;   // [tiles * 4] start, end into qlist
   const int8_t* depth;   // [B, C] validated delivered depths
   int32_t B, C, nsb;

@@ -71,15 +71,15 @@ struct Workspace {
   uint32_t* depth_bits;   // [2N]
   uint32_t* count;        // [2N]
   unsigned long long* keys[2];  // [cap] [0]: sorted (tile<<32 | depth bits); [1]: per-tile segments of (depth bits<<32 | record id) before the sort
-  uint32_t* vals[2];            // [cap] [0]: record ids of the sorted list; [1]: the render list (k_tile_render_list)
+  uint32_t* vals[2];            // [cap] [0]: record ids of the sorted list; [1]: the render list (tile_render_lists in k_tile_sort)
   uint32_t* tile_cursor;  // [tiles] keys per tile, then the write cursor of the tile's segment (k_sort.cu)
   uint2* tile_range;      // [tiles] start,end into the sorted list
   uint2* render_range;    // [tiles] start,end into the render list (vals[1]): the tile's records whose q <= tau
-                          // box touches a pixel of the tile, in list order (k_tile_render_list)
+                          // box touches a pixel of the tile, in list order (tile_render_lists in k_tile_sort)
   long long* state_counts;  // [B]
   double* sse_blk;        // [B * tiles * 8] per-(state,tile,8x4 block) squared-error partials (fused distortion)
   float4* rec;            // [4 * 2N] packed 64-byte records for the quadrant compositor (written by k_project)
-  uint2* qlist;           // [4 * cap] per-(tile, quadrant) render lists of {record id, meta} (k_tile_render_list)
+  uint2* qlist;           // [4 * cap] per-(tile, quadrant) render lists of {record id, meta} (tile_render_lists in k_tile_sort)
   uint2* qrange;          // [tiles * 4] start, end into qlist
   uint32_t* uorder;       // [tiles * B] states sorted by their tile-restricted signature (k_tile_dedup)
   uint32_t* upos;         // [tiles * B] upos[tile*B + u] = index in uorder of the first member of class u
@@ -105,7 +105,7 @@ __device__ __forceinline__ uint32_t record_block_mask(float mx, float my, float 
   return m;
 }
 
-// Tighter version, evaluated once per frame per (tile, record) by k_tile_render_list: a block that passes the
+// Tighter version, evaluated once per frame per (tile, record) by tile_render_lists (k_sort.cu): a block that passes the
 // box test is kept only if the MINIMUM of the quadratic form q over the block's rectangle of pixel centres can
 // pass the cut.  q is convex, so when the centre lies outside the rectangle the minimum sits on one of the four
 // edges, where q is a 1-D quadratic (closed-form minimiser, clamped to the edge).  The block is dropped iff

@@ -18,7 +18,7 @@
 // (exact), which makes the step ONE saturating add with an immediate: s = sat(2^40 T - 2^40 pred(1e-4)):
 // neighbouring floats at 1e-4 are 2^-37 apart, so T >= 1e-4 gives >= 8 -> 1 and T <= pred(1e-4) gives <= 0 -> 0.
 //
-// No barrier anywhere: the warp walks the quadrant's own render list (k_tile_render_list, once per frame: the
+// No barrier anywhere: the warp walks the quadrant's own render list (k_tile_sort, once per frame: the
 // tile's depth-sorted list restricted to the records whose q <= tau region can reach the quadrant), 32 entries
 // at a time: each lane takes one entry {record id, meta}, derives from the presence table which of the S slots
 // contain the record, and the records present in at least one slot are copied global -> shared with cp.async

@@ -71,7 +71,7 @@ __global__ void __launch_bounds__(kDedupThreads) k_tile_dedup(const uint2* __res
   for (int k = tid; k < C; k += kDedupThreads) ccnt[k] = 0;
   __syncthreads();
   for (uint32_t i = rg.x + tid; i < rg.y; i += kDedupThreads) {
-    const uint32_t rid = vals[i];  // render list: sub-tile-culled records are already gone (k_tile_render_list)
+    const uint32_t rid = vals[i];  // render list: sub-tile-culled records are already gone (tile_render_lists in k_sort.cu)
     const uint32_t meta = __float_as_uint(r1[rid].w);
     const uint32_t c = meta & 0xFFFFu, cls = meta >> 16;
     const uint32_t bit = cls >= 16 ? (16u << (cls - 16)) : (cls == 0 ? 1u : (cls <= 2 ? 2u : (cls == 3 ? 4u : 8u)));

@@ -563,7 +563,7 @@ def test_subtile_culling_never_drops_a_contribution(gsr, torch_mod, oracle_mod):
 
 @pytest.mark.parametrize("aspect", [1.5, 6.0, 40.0])
 def test_block_culling_by_minimum_of_q_keeps_every_contribution(gsr, torch_mod, oracle_mod, aspect):
-    """The once-per-frame per-block culling (minimum of q over the 8x4 block, k_tile_render_list) on its own
+    """The once-per-frame per-block culling (minimum of q over the 8x4 block, tile_render_lists in k_sort.cu) on its own
     ground: moderately elongated, randomly rotated Gaussians (conditioning 2 .. ~2000, below the kappa cut-off of
     the tight test) a few pixels wide, so that most footprints clip block corners and edges; strong and faint
     opacities.  The oracle culls nothing: a wrongly dropped block would show as a >= 1/255 pixel error."""
