@@ -156,7 +156,9 @@ int gsr_render_states_vs_full(const gsr_scene* scene, const gsr_camera* cam, flo
  * gsr_render_backward — the backward of the compositing step (the training objective is a function
  * of the rendered images; SURVEY.md §8(f)-4 follow-on).  To be called after gsr_render_states /
  * _ex / _vs_full on the SAME workspace, batch and stream: it reuses the projected records, the sorted lists and the
- * validated levels the forward call left there.
+ * validated levels the forward call left there, and uses the workspace's scratch tables (so one backward call per
+ * workspace at a time, like a render).  States whose pixels in a tile are identical are walked once
+ * per tile with the sum of their dL_dimages — the gradient is linear in it (option "dedup", default on).
  *   images      dev fp32 [B,H,W,3]  the forward output of that call
  *   dL_dimages  dev fp32 [B,H,W,3]  the gradient of the objective with respect to every pixel of every state
  *   grad        dev fp32 [gsr_num_records(scene), 12], overwritten: for record r (Gaussian i, variant v: r = 2 i + v,
@@ -170,7 +172,7 @@ int gsr_render_states_vs_full(const gsr_scene* scene, const gsr_camera* cam, flo
  * Synchronises once at entry (reads the workspace header), then asynchronous.  Sums are formed with float
  * atomics: the result is reproducible up to fp32 summation order.  B must be the forward call's B. */
 int64_t gsr_num_records(const gsr_scene* scene);
-int gsr_render_backward(const gsr_scene* scene, const void* workspace, const float* images, const float* dL_dimages,
+int gsr_render_backward(const gsr_scene* scene, void* workspace, const float* images, const float* dL_dimages,
                         int32_t B, float* grad, void* cuda_stream);
 
 /* Synchronises `cuda_stream` and reads the status latched by the last render into `workspace`:

@@ -539,7 +539,7 @@ int64_t gsr_num_records(const gsr_scene* scene) {
   return scene ? (int64_t)scene->impl.d.N * scene->impl.d.V : 0;
 }
 
-int gsr_render_backward(const gsr_scene* scene, const void* workspace, const float* images, const float* dL_dimages,
+int gsr_render_backward(const gsr_scene* scene, void* workspace, const float* images, const float* dL_dimages,
                         int32_t B, float* grad, void* cuda_stream) {
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (!scene || !workspace || B < 0 || (B > 0 && (!images || !dL_dimages)) || !grad) {
@@ -556,7 +556,7 @@ int gsr_render_backward(const gsr_scene* scene, const void* workspace, const flo
   }
   if (h.status != GSR_OK) { set_error("gsr_render_backward: the forward render failed (status %d)", h.status); return h.status; }
   Workspace ws;
-  carve_workspace(&ws, const_cast<void*>(workspace), rec_half(scene->impl.d), h.C, h.B, h.TX * h.TY, h.key_capacity);
+  carve_workspace(&ws, workspace, rec_half(scene->impl.d), h.C, h.B, h.TX * h.TY, h.key_capacity);
   launch_backward(scene->impl.d, h, ws, images, dL_dimages, grad, st);
   GSR_CUDA(cudaGetLastError());
   return GSR_OK;

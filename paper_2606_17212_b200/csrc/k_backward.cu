@@ -38,6 +38,8 @@ struct BackwardArgs {
   float* grad;           // [records, 12]
   uint32_t n_items;        // tiles * 4 * nsb
   uint32_t* work_counter;  // zeroed before the launch
+  // tile-level state dedup (k_tile_dedup), or all nullptr: slot = signature class of the tile
+  const uint32_t *uorder, *upos, *n_unique;
 };
 
 // The butterfly of reduce.cuh for 16 floats per lane: after the call the lane holds the warp total of component
@@ -100,6 +102,8 @@ __global__ void __launch_bounds__(32) k_backward_q(const BackwardArgs a) {
   __shared__ __align__(16) float4 s_rec[2][kChunk * 4];
   __shared__ uint32_t s_tag[2][kChunk];  // act | res << 16
   __shared__ uint32_t s_rid[2][kChunk];  // record id (row of grad)
+  __shared__ int s_rep[S];                 // representative state of slot s, -1 = empty slot
+  __shared__ uint32_t s_mlo[S], s_mhi[S];  // members of the class: uorder[tile*B + [mlo, mhi))
 
   const int lane = threadIdx.x;
   for (;;) {  // persistent warps: work items (tile, quadrant, state block) from a counter, as in k_composite_q
@@ -110,14 +114,36 @@ __global__ void __launch_bounds__(32) k_backward_q(const BackwardArgs a) {
   const uint32_t tq = item / (uint32_t)a.nsb;  // 4 * tile + quadrant
   const int sb = (int)(item - tq * (uint32_t)a.nsb);
   const int tile = (int)(tq >> 2), quad = (int)(tq & 3u);
-  const int b0 = sb * S;  // slot s = state b0 + s (no tile-level dedup here: every state has its own g)
+  const int b0 = sb * S;  // first slot of this block: a state index, or a class index when dedup is on
+
+  // With tile-level dedup slot s is the s-th signature class of this tile from b0 on.  The members of a class
+  // have bitwise identical tile pixels, hence identical T, alpha, w along the list, and the gradient is linear in
+  // g: the sum over the members of their gradients is the gradient for the SUM of their g.  One walk per class.
+  const int n_slots = a.n_unique ? (int)a.n_unique[tile] : a.B;
+  if (b0 >= n_slots) continue;
+  if (lane < S) {
+    const int u = b0 + lane;
+    int rep = -1;
+    uint32_t lo = 0, hi = 0;
+    if (u < n_slots) {
+      if (a.n_unique) {
+        lo = a.upos[(size_t)tile * a.B + u];
+        hi = u + 1 < n_slots ? a.upos[(size_t)tile * a.B + u + 1] : (uint32_t)a.B;
+        rep = (int)a.uorder[(size_t)tile * a.B + lo];
+      } else {
+        rep = u;
+      }
+    }
+    s_rep[lane] = rep; s_mlo[lane] = lo; s_mhi[lane] = hi;
+  }
+  __syncwarp();
 
   for (int c = lane; c < a.C; c += 32) {
     uint32_t eq0 = 0, ge1 = 0, ge2 = 0, ge3 = 0;
 #pragma unroll
     for (int s = 0; s < S; ++s) {
-      if (b0 + s < a.B) {
-        const int d = a.depth[(size_t)(b0 + s) * a.C + c];
+      if (s_rep[s] >= 0) {
+        const int d = a.depth[(size_t)s_rep[s] * a.C + c];
         eq0 |= (uint32_t)(d == 0) << s;
         ge1 |= (uint32_t)(d >= 1) << s;
         ge2 |= (uint32_t)(d >= 2) << s;
@@ -146,21 +172,27 @@ __global__ void __launch_bounds__(32) k_backward_q(const BackwardArgs a) {
   // per (pixel pair, state): T (scaled by 2^40), the prefix G of w (g . cb), and the constants g[3], Gf (scaled)
   f32x2 T2[S], G2[S], gr2[S], gg2[S], gb2[S], Gf2[S];
   const size_t img = (size_t)a.H * a.W * 3;
+  const uint32_t* const mem = a.n_unique ? a.uorder + (size_t)tile * a.B : nullptr;
 #pragma unroll
   for (int s = 0; s < S; ++s) {
     float g[2][3] = {{0.f, 0.f, 0.f}, {0.f, 0.f, 0.f}}, gf[2] = {0.f, 0.f};
-    const bool on = b0 + s < a.B;
+    const int rep = s_rep[s];
+    const bool on = rep >= 0;
+    const uint32_t lo = mem ? s_mlo[s] : (uint32_t)rep, hi = mem ? s_mhi[s] : lo + 1u;
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
       const int y = h ? yb : ya;
       if (on && (h ? in_b : in_a)) {
-        const size_t o = (size_t)(b0 + s) * img + ((size_t)y * a.W + x) * 3;
+        const size_t po = ((size_t)y * a.W + x) * 3;
+        for (uint32_t i = lo; i < hi; ++i) {  // g of the class = sum of its members' g, in uorder order
+          const float* gp = a.gimg + (size_t)(mem ? mem[i] : i) * img + po;
+#pragma unroll
+          for (int ch = 0; ch < 3; ++ch) g[h][ch] += __ldg(gp + ch);
+        }
+        const float* ip = a.images + (size_t)rep * img + po;
         float dot = 0.0f;
 #pragma unroll
-        for (int ch = 0; ch < 3; ++ch) {
-          g[h][ch] = __ldg(a.gimg + o + ch);
-          dot = __fmaf_rn(g[h][ch], __fsub_rn(__ldg(a.images + o + ch), a.bg[ch]), dot);
-        }
+        for (int ch = 0; ch < 3; ++ch) dot = __fmaf_rn(g[h][ch], __fsub_rn(__ldg(ip + ch), a.bg[ch]), dot);
         gf[h] = dot * kTScale;
       }
     }
@@ -314,11 +346,18 @@ __global__ void __launch_bounds__(32) k_backward_q(const BackwardArgs a) {
 
 constexpr int kBackwardStateBlock = 8;  // measured on cfg1 (ms per 256-state frame): S = 2: 25.4, 4: 20.2, 8: 17.5
 
+extern thread_local int g_dedup;  // k_composite.cu: option "dedup" of the calling thread
+
 void launch_backward(const DeviceScene& sc, const WsHeader& h, Workspace& ws, const float* images, const float* gimg,
                      float* grad, cudaStream_t st) {
   const int n_rec = sc.N * sc.V;
   if (n_rec > 0) cudaMemsetAsync(grad, 0, sizeof(float) * 12 * (size_t)n_rec, st);
   if (h.B == 0 || n_rec == 0) return;
+  // The signature classes are rebuilt here (k_tile_dedup, ~1 % of the pass) rather than taken from the forward
+  // call: that call may have run with the option off, or over chunks of a larger batch.
+  FrameParams fp{};
+  fp.W = h.W; fp.H = h.H; fp.TX = h.TX; fp.TY = h.TY;
+  const bool dedup = g_dedup && launch_tile_dedup(sc, fp, ws, ws.depth, h.B, st);
   BackwardArgs a;
   a.rec = ws.rec; a.qlist = ws.qlist; a.qrange = ws.qrange; a.depth = ws.depth;
   a.B = h.B; a.C = sc.C;
@@ -326,6 +365,7 @@ void launch_backward(const DeviceScene& sc, const WsHeader& h, Workspace& ws, co
   a.W = h.W; a.H = h.H; a.TX = h.TX; a.tiles = h.TX * h.TY;
   a.bg[0] = sc.bg[0]; a.bg[1] = sc.bg[1]; a.bg[2] = sc.bg[2];
   a.images = images; a.gimg = gimg; a.grad = grad;
+  a.uorder = dedup ? ws.uorder : nullptr; a.upos = dedup ? ws.upos : nullptr; a.n_unique = dedup ? ws.n_unique : nullptr;
   const size_t smem = sizeof(uint16_t) * 4 * (size_t)sc.C;
   if (smem > 40 * 1024)
     cudaFuncSetAttribute(k_backward_q<kBackwardStateBlock>, cudaFuncAttributeMaxDynamicSharedMemorySize,

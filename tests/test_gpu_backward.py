@@ -187,3 +187,47 @@ def test_backward_full_size_cfg1_identities(gsr, torch_mod):
     assert float(((grad_b - grad_1).abs() / scale).max()) <= 2e-4
     assert bool((grad_b != 0).any())
     scene.close()
+
+
+def test_backward_shared_tile_classes_against_the_oracle(gsr, torch_mod, oracle_mod):
+    """States with identical pixels in a tile are walked once with the SUM of their dL/d(image):
+    a batch made of utility pairs (m, m u g: they differ in one cluster) plus exact duplicates, each state with its
+    own random g — against the oracle, which differentiates every state on its own."""
+    wl = synth.scaled_object_workload(31, C=6, per_cluster=240.0, W=112, H=80, fov=40.0, n_frames=1, B=6)
+    cam, t = wl.frames[0]
+    base = wl.levels[0]
+    rows = []
+    for b in range(base.shape[0]):
+        rows.append(base[b].copy())
+        up = base[b].copy()
+        up[b % up.shape[0]] = min(3, up[b % up.shape[0]] + 1)     # the pair state: one cluster one level further
+        rows.append(up)
+        rows.append(base[b].copy())                               # an exact duplicate
+    lv = np.stack(rows).astype(np.int8)
+    got, g, V = _run(gsr, torch_mod, wl.scene, cam, t, lv, 8)
+    want = oracle_record_grads(oracle_mod, wl.scene, cam, t, lv, g, V)
+    _compare(got, want)
+
+
+def test_backward_dedup_option_off_gives_the_same_gradient(gsr, torch_mod):
+    """configs[1], full size: the class-summed walk (default) against one walk per state (option dedup = 0)."""
+    torch = torch_mod
+    wl = synth.workload_cfg1(n_frames=1)
+    cam, t = wl.frames[0]
+    dlv = torch.from_numpy(np.ascontiguousarray(wl.levels[0])).cuda()
+    scene = gsr.Scene(wl.scene)
+    ws = scene.new_workspace(cam, dlv.shape[0])
+    out, _, _ = scene.render_states(cam, t, dlv, workspace=ws)
+    scene.status(ws)
+    gen = torch.Generator(device="cuda").manual_seed(12)
+    g = torch.randn(out.shape, generator=gen, device="cuda", dtype=torch.float32)
+    grad_on = scene.render_backward(ws, out, g).clone()
+    gsr.set_option("dedup", 0)
+    try:
+        grad_off = scene.render_backward(ws, out, g).clone()
+    finally:
+        gsr.set_option("dedup", 1)
+    scale = grad_off.abs().amax(dim=0).clamp_min(1e-20)
+    assert float(((grad_on - grad_off).abs() / scale).max()) <= 2e-4
+    assert bool((grad_on != 0).any())
+    scene.close()
