@@ -17,8 +17,8 @@
 //
 // Layout of the work: the forward's (k_composite_q.cu): one warp per 8x8 quadrant x S states, two pixels per lane on
 // packed FP32; per (pixel pair, state) T, G and the constants g[3], Gf live in registers (12 per slot, S = 8).
-// Per record the 12 partial sums of the lane's pixels and states are reduced over the warp with the
-// slot-splitting butterfly (16 shuffles instead of 60) and added to grad with one atomic per component.
+// Per record the 12 partial sums of the lane's pixels and states are reduced over the warp through shared memory,
+// eight records at a time, and added to grad with three vector atomics per record (below).
 // Float atomics make the summation order, hence the last bits of grad, run-dependent; parity is by tolerance.
 #include "composite_common.cuh"
 #include "gsr_internal.h"
@@ -42,26 +42,25 @@ struct BackwardArgs {
   const uint32_t *uorder, *upos, *n_unique;
 };
 
-// The butterfly of reduce.cuh for 16 floats per lane: after the call the lane holds the warp total of component
-// `slot` (lanes with (lane & 1) == 0 are one representative per component).
-__device__ __forceinline__ float warp_sum_16(float (&v)[16], int lane, int& slot) {
-  int off = 16;
-  slot = 0;
-#pragma unroll
-  for (int n = 16; n > 1; n >>= 1) {
-    const int half = n >> 1;
-    const bool upper = (lane & off) != 0;
-#pragma unroll
-    for (int j = 0; j < half; ++j) {
-      const float send = upper ? v[j] : v[j + half];
-      const float keep = upper ? v[j + half] : v[j];
-      v[j] = keep + __shfl_xor_sync(0xffffffffu, send, off);
-    }
-    slot = 2 * slot + (upper ? 1 : 0);
-    off >>= 1;
-  }
-  v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
-  return v[0];
+// Reduction of the per-lane partial sums over the warp, through shared memory and kGroup records at a time: every
+// lane stores its 12 partials of a record as three float4 (row of 12 floats per lane, record stride kPartStride:
+// conflict-free stores and loads); when kGroup records are pending, lane (r = lane % kGroup, h = lane / kGroup < 3)
+// adds the h-th float4 of record r over the 32 source lanes and issues ONE vector reduction to grad
+// (red.global.add.v4.f32).  Per record: 3 STS.128 + 4 LDS.128-and-add steps per lane instead of a 5-deep shuffle
+// butterfly of 16 SHFL + ~45 FSEL / FADD, and 3 vector atomics instead of 12 scalar ones.
+constexpr int kGroup = 8;
+constexpr int kPartStride = 32 * 12 + 4;  // floats; + 4: the kGroup rows of a quarter-warp load fall in distinct banks
+
+__device__ __forceinline__ void sts128f(uint32_t addr, float x, float y, float z, float w) {
+  asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(x), "f"(y), "f"(z), "f"(w) : "memory");
+}
+__device__ __forceinline__ void red_add_v4(float* p, float x, float y, float z, float w) {
+  asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(x), "f"(y), "f"(z), "f"(w) : "memory");
+}
+__device__ __forceinline__ float rcp_approx_ftz(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
 }
 
 // One state slot, two pixels (header).  T, G, Gf are carried scaled by 2^40 like the forward's T.
@@ -102,6 +101,8 @@ __global__ void __launch_bounds__(32) k_backward_q(const BackwardArgs a) {
   __shared__ __align__(16) float4 s_rec[2][kChunk * 4];
   __shared__ uint32_t s_tag[2][kChunk];  // act | res << 16
   __shared__ uint32_t s_rid[2][kChunk];  // record id (row of grad)
+  __shared__ __align__(16) float s_part[kGroup * kPartStride];  // pending per-lane partials: [record][lane][12]
+  __shared__ uint32_t s_grid[kGroup];                           // their record ids
   __shared__ int s_rep[S];                 // representative state of slot s, -1 = empty slot
   __shared__ uint32_t s_mlo[S], s_mhi[S];  // members of the class: uorder[tile*B + [mlo, mhi))
 
@@ -168,6 +169,28 @@ __global__ void __launch_bounds__(32) k_backward_q(const BackwardArgs a) {
   const uint32_t tag_base = (uint32_t)__cvta_generic_to_shared(&s_tag[0][0]);
   const uint32_t rid_base = (uint32_t)__cvta_generic_to_shared(&s_rid[0][0]);
   const uint32_t lt = (1u << lane) - 1u;
+  const uint32_t part_base = (uint32_t)__cvta_generic_to_shared(&s_part[0]);
+  const uint32_t grid_base = (uint32_t)__cvta_generic_to_shared(&s_grid[0]);
+  uint32_t n_pend = 0;  // records waiting in s_part (warp-uniform)
+  auto flush = [&](uint32_t n) {
+    __syncwarp();
+    const uint32_t r = (uint32_t)lane % kGroup, h = (uint32_t)lane / kGroup;
+    if (h < 3 && r < n) {
+      const uint32_t src = part_base + 4u * (r * kPartStride + 4u * h);
+      float4 acc0 = lds128(src), acc1 = lds128(src + 48u);
+#pragma unroll
+      for (int l = 2; l < 32; l += 2) {
+        const float4 t0 = lds128(src + 48u * l), t1 = lds128(src + 48u * (l + 1));
+        acc0.x += t0.x; acc0.y += t0.y; acc0.z += t0.z; acc0.w += t0.w;
+        acc1.x += t1.x; acc1.y += t1.y; acc1.z += t1.z; acc1.w += t1.w;
+      }
+      acc0.x += acc1.x; acc0.y += acc1.y; acc0.z += acc1.z; acc0.w += acc1.w;
+      if (acc0.x != 0.0f || acc0.y != 0.0f || acc0.z != 0.0f || acc0.w != 0.0f)
+        red_add_v4(a.grad + 12 * (size_t)lds32(grid_base + 4u * r) + 4 * h, acc0.x * kInvTScale, acc0.y * kInvTScale,
+                   acc0.z * kInvTScale, acc0.w * kInvTScale);
+    }
+    __syncwarp();
+  };
 
   // per (pixel pair, state): T (scaled by 2^40), the prefix G of w (g . cb), and the constants g[3], Gf (scaled)
   f32x2 T2[S], G2[S], gr2[S], gg2[S], gb2[S], Gf2[S];
@@ -294,7 +317,7 @@ __global__ void __launch_bounds__(32) k_backward_q(const BackwardArgs a) {
       // gradients flow through alpha only where the cut passed and the cap is not active
       const float m_a = (pass_a && raw_a <= kAlphaCap) ? 1.0f : 0.0f, m_b = (pass_b && raw_b <= kAlphaCap) ? 1.0f : 0.0f;
       const f32x2 alpha2 = pack2(al_a, al_b);
-      const f32x2 rinv2 = pack2(__frcp_rn(1.0f - al_a), __frcp_rn(1.0f - al_b));
+      const f32x2 rinv2 = pack2(rcp_approx_ftz(1.0f - al_a), rcp_approx_ftz(1.0f - al_b));  // 1 - alpha in [0.01, 1]
       f32x2 dal = pack2(0.f, 0.f);
       f32x2 dc0[3] = {dal, dal, dal}, dc1[3] = {dal, dal, dal};
       const uint32_t act1 = actl & (tag >> 16), act0 = actl ^ act1;
@@ -313,7 +336,7 @@ __global__ void __launch_bounds__(32) k_backward_q(const BackwardArgs a) {
             slot_backward(T2[s], G2[s], gr2[s], gg2[s], gb2[s], Gf2[s], alpha2, rinv2, k1.x, k1.y, k1.z, dal, dc1[0], dc1[1], dc1[2]);
       }
       // per pixel: dL/do = exp(-q) dal, dL/dq = -alpha dal, then the chain through q; the two pixels added
-      float v[16];
+      float v[12];
 #pragma unroll
       for (int ch = 0; ch < 3; ++ch) {
         float lo, hi;
@@ -331,15 +354,20 @@ __global__ void __launch_bounds__(32) k_backward_q(const BackwardArgs a) {
       v[9] = dq_a * dya * dya + dq_b * dyb * dyb;
       v[10] = dq_a * (2.0f * h0.z * dx + h0.w * dya) + dq_b * (2.0f * h0.z * dx + h0.w * dyb);
       v[11] = dq_a * (h0.w * dx + 2.0f * hq.x * dya) + dq_b * (h0.w * dx + 2.0f * hq.x * dyb);
-      v[12] = v[13] = v[14] = v[15] = 0.0f;
-      int comp;
-      const float tot = warp_sum_16(v, lane, comp);
-      if ((lane & 1) == 0 && comp < 12 && tot != 0.0f)
-        atomicAdd(a.grad + 12 * (size_t)lds32(ib0 + 4u * j) + comp, tot * kInvTScale);
+      const uint32_t dst = part_base + 4u * (n_pend * kPartStride + 12u * (uint32_t)lane);
+      sts128f(dst, v[0], v[1], v[2], v[3]);
+      sts128f(dst + 16u, v[4], v[5], v[6], v[7]);
+      sts128f(dst + 32u, v[8], v[9], v[10], v[11]);
+      if (lane == 0) sts32(grid_base + 4u * n_pend, lds32(ib0 + 4u * j));
+      if (++n_pend == kGroup) {
+        flush(kGroup);
+        n_pend = 0;
+      }
     }
     n_cur = n_nxt;
     __syncwarp();
   }
+  if (n_pend) flush(n_pend);
   __syncwarp();  // the shared tables and buffers are rewritten by the next item
   }
 }
