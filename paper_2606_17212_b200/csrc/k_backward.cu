@@ -16,7 +16,7 @@
 // the forward's operations on the same operands) — and the forward image is an input.
 //
 // Layout of the work: the forward's (k_composite_q.cu): one warp per 8x8 quadrant x S states, two pixels per lane on
-// packed FP32; per (pixel pair, state) T, G and the constants g[3], Gf live in registers (12 per slot, S = 8).
+// packed FP32; per (pixel pair, state) T, E = G - Gf and the constants g[3] live in registers (10 per slot).
 // Per record the 12 partial sums of the lane's pixels and states are reduced over the warp through shared memory,
 // eight records at a time, and added to grad with three vector atomics per record (below).
 // Float atomics make the summation order, hence the last bits of grad, run-dependent; parity is by tolerance.
@@ -48,7 +48,10 @@ struct BackwardArgs {
 // adds the h-th float4 of record r over the 32 source lanes and issues ONE vector reduction to grad
 // (red.global.add.v4.f32).  Per record: 3 STS.128 + 4 LDS.128-and-add steps per lane instead of a 5-deep shuffle
 // butterfly of 16 SHFL + ~45 FSEL / FADD, and 3 vector atomics instead of 12 scalar ones.
-constexpr int kGroup = 8;
+#ifndef GSR_BW_GROUP
+#define GSR_BW_GROUP 8
+#endif
+constexpr int kGroup = GSR_BW_GROUP;
 constexpr int kPartStride = 32 * 12 + 4;  // floats; + 4: the kGroup rows of a quarter-warp load fall in distinct banks
 
 __device__ __forceinline__ void sts128f(uint32_t addr, float x, float y, float z, float w) {
@@ -63,10 +66,11 @@ __device__ __forceinline__ float rcp_approx_ftz(float x) {
   return y;
 }
 
-// One state slot, two pixels (header).  T, G, Gf are carried scaled by 2^40 like the forward's T.
-//   dal  += s (T u - (Gf - G') rinv)        accumulated dL/dalpha of the record over the slots
+// One state slot, two pixels (header).  T and E = G - Gf (the prefix minus the whole pixel: minus the suffix) are
+// carried scaled by 2^40 like the forward's T.
+//   dal  += s (T u + E' rinv)               accumulated dL/dalpha of the record over the slots
 //   dc*  += (s w) g                          accumulated colour gradient
-__device__ __forceinline__ void slot_backward(f32x2& T, f32x2& G, f32x2 gr, f32x2 gg, f32x2 gb, f32x2 Gf, f32x2 alpha2,
+__device__ __forceinline__ void slot_backward(f32x2& T, f32x2& E, f32x2 gr, f32x2 gg, f32x2 gb, f32x2 alpha2,
                                               f32x2 rinv2, float cr, float cg, float cb, f32x2& dal, f32x2& dcr,
                                               f32x2& dcg, f32x2& dcb) {
   f32x2 u = mul2(gr, pack2(cr, cr));
@@ -82,12 +86,8 @@ __device__ __forceinline__ void slot_backward(f32x2& T, f32x2& G, f32x2 gr, f32x
   const f32x2 s = pack2(tl, th);
   const f32x2 ws = mul2(w, s);
   const f32x2 tu = mul2(T, u);
-  G = fma2(ws, u, G);
-  f32x2 d;
-  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(Gf), "l"(G));
-  const f32x2 dr = mul2(d, rinv2);
-  f32x2 t1;
-  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(t1) : "l"(tu), "l"(dr));  // T u - (Gf - G) / (1 - alpha)
+  E = fma2(ws, u, E);
+  const f32x2 t1 = fma2(E, rinv2, tu);  // T u - (Gf - G) / (1 - alpha)
   dal = fma2(s, t1, dal);
   dcr = fma2(ws, gr, dcr);
   dcg = fma2(ws, gg, dcg);
@@ -95,8 +95,11 @@ __device__ __forceinline__ void slot_backward(f32x2& T, f32x2& G, f32x2 gr, f32x
   T = Tn;
 }
 
+#ifndef GSR_BW_MINB
+#define GSR_BW_MINB 12
+#endif
 template <int S>
-__global__ void __launch_bounds__(32) k_backward_q(const BackwardArgs a) {
+__global__ void __launch_bounds__(32, GSR_BW_MINB) k_backward_q(const BackwardArgs a) {
   extern __shared__ uint16_t s_tab[];  // [C][4]: slots (bit s) whose state has depth == 0, >= 1, >= 2, >= 3
   __shared__ __align__(16) float4 s_rec[2][kChunk * 4];
   __shared__ uint32_t s_tag[2][kChunk];  // act | res << 16
@@ -192,8 +195,8 @@ __global__ void __launch_bounds__(32) k_backward_q(const BackwardArgs a) {
     __syncwarp();
   };
 
-  // per (pixel pair, state): T (scaled by 2^40), the prefix G of w (g . cb), and the constants g[3], Gf (scaled)
-  f32x2 T2[S], G2[S], gr2[S], gg2[S], gb2[S], Gf2[S];
+  // per (pixel pair, state): T (scaled by 2^40), E = (prefix of w (g . cb)) - Gf (scaled), and the constants g[3]
+  f32x2 T2[S], E2[S], gr2[S], gg2[S], gb2[S];
   const size_t img = (size_t)a.H * a.W * 3;
   const uint32_t* const mem = a.n_unique ? a.uorder + (size_t)tile * a.B : nullptr;
 #pragma unroll
@@ -220,9 +223,8 @@ __global__ void __launch_bounds__(32) k_backward_q(const BackwardArgs a) {
       }
     }
     T2[s] = pack2(on && in_a ? kTScale : 0.0f, on && in_b ? kTScale : 0.0f);
-    G2[s] = pack2(0.0f, 0.0f);
+    E2[s] = pack2(-gf[0], -gf[1]);
     gr2[s] = pack2(g[0][0], g[1][0]); gg2[s] = pack2(g[0][1], g[1][1]); gb2[s] = pack2(g[0][2], g[1][2]);
-    Gf2[s] = pack2(gf[0], gf[1]);
   }
 
   const uint2 qr = a.qrange[tq];
@@ -326,14 +328,14 @@ __global__ void __launch_bounds__(32) k_backward_q(const BackwardArgs a) {
 #pragma unroll
         for (int s = 0; s < S; ++s)
           if ((act0 >> s) & 1u)
-            slot_backward(T2[s], G2[s], gr2[s], gg2[s], gb2[s], Gf2[s], alpha2, rinv2, k0.x, k0.y, k0.z, dal, dc0[0], dc0[1], dc0[2]);
+            slot_backward(T2[s], E2[s], gr2[s], gg2[s], gb2[s], alpha2, rinv2, k0.x, k0.y, k0.z, dal, dc0[0], dc0[1], dc0[2]);
       }
       if (act1 != 0) {
         const float4 k1 = lds128(addr + 48u);  // {rgb with SH residual - bg, -}
 #pragma unroll
         for (int s = 0; s < S; ++s)
           if ((act1 >> s) & 1u)
-            slot_backward(T2[s], G2[s], gr2[s], gg2[s], gb2[s], Gf2[s], alpha2, rinv2, k1.x, k1.y, k1.z, dal, dc1[0], dc1[1], dc1[2]);
+            slot_backward(T2[s], E2[s], gr2[s], gg2[s], gb2[s], alpha2, rinv2, k1.x, k1.y, k1.z, dal, dc1[0], dc1[1], dc1[2]);
       }
       // per pixel: dL/do = exp(-q) dal, dL/dq = -alpha dal, then the chain through q; the two pixels added
       float v[12];
@@ -372,7 +374,10 @@ __global__ void __launch_bounds__(32) k_backward_q(const BackwardArgs a) {
   }
 }
 
-constexpr int kBackwardStateBlock = 8;  // measured on cfg1 (ms per 256-state frame): S = 2: 25.4, 4: 20.2, 8: 17.5
+#ifndef GSR_BW_S
+#define GSR_BW_S 10
+#endif
+constexpr int kBackwardStateBlock = GSR_BW_S;  // measured on cfg1 (ms per 256-state frame): S = 2: 25.4, 4: 20.2, 8: 17.5
 
 extern thread_local int g_dedup;  // k_composite.cu: option "dedup" of the calling thread
 
