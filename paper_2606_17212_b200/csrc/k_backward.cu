@@ -199,32 +199,83 @@ __global__ void __launch_bounds__(32, GSR_BW_MINB) k_backward_q(const BackwardAr
   f32x2 T2[S], E2[S], gr2[S], gg2[S], gb2[S];
   const size_t img = (size_t)a.H * a.W * 3;
   const uint32_t* const mem = a.n_unique ? a.uorder + (size_t)tile * a.B : nullptr;
+  const size_t po_a = ((size_t)ya * a.W + x) * 3, po_b = ((size_t)yb * a.W + x) * 3;
+  {
+    // g of a class = the sum of its members' g, in uorder order.  The classes of this block are consecutive in
+    // uorder, so the members of all S slots are ONE range [f_lo, f_hi): walked kGBatch members at a time with all
+    // their loads in flight together (6 per member and lane; the member indices one batch ahead), the running sum
+    // parked in shared memory (s_part, idle until the first record) whenever the walk crosses into the next class.
+    static_assert(S * 6 * 32 <= kGroup * kPartStride, "the class sums are parked in s_part");
+    constexpr int kGBatch = 8;
+    const int n_valid = n_slots - b0 < S ? n_slots - b0 : S;
+    const uint32_t f_lo = mem ? s_mlo[0] : (uint32_t)b0, f_hi = mem ? s_mhi[n_valid - 1] : (uint32_t)(b0 + n_valid);
+    float acc[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    int cur = 0;
+    uint32_t bound = mem ? s_mhi[0] : f_lo + 1u;
+    auto park = [&](int slot) {
 #pragma unroll
-  for (int s = 0; s < S; ++s) {
-    float g[2][3] = {{0.f, 0.f, 0.f}, {0.f, 0.f, 0.f}}, gf[2] = {0.f, 0.f};
-    const int rep = s_rep[s];
-    const bool on = rep >= 0;
-    const uint32_t lo = mem ? s_mlo[s] : (uint32_t)rep, hi = mem ? s_mhi[s] : lo + 1u;
+      for (int c = 0; c < 6; ++c) {
+        sts32(part_base + 4u * (uint32_t)((slot * 6 + c) * 32 + lane), __float_as_uint(acc[c]));
+        acc[c] = 0.0f;
+      }
+    };
+    uint32_t idx_nxt = 0;
+    if (mem && f_lo + (uint32_t)lane < f_hi && lane < kGBatch) idx_nxt = __ldg(mem + f_lo + lane);
+    for (uint32_t base = f_lo; base < f_hi; base += kGBatch) {
+      const uint32_t idx_cur = idx_nxt;
+      if (mem && base + kGBatch + (uint32_t)lane < f_hi && lane < kGBatch) idx_nxt = __ldg(mem + base + kGBatch + lane);
+      float v[kGBatch][6];
 #pragma unroll
-    for (int h = 0; h < 2; ++h) {
-      const int y = h ? yb : ya;
-      if (on && (h ? in_b : in_a)) {
-        const size_t po = ((size_t)y * a.W + x) * 3;
-        for (uint32_t i = lo; i < hi; ++i) {  // g of the class = sum of its members' g, in uorder order
-          const float* gp = a.gimg + (size_t)(mem ? mem[i] : i) * img + po;
+      for (int k = 0; k < kGBatch; ++k) {
+        const uint32_t sid = mem ? __shfl_sync(0xffffffffu, idx_cur, k) : base + k;
+        const bool have = base + k < f_hi;
+        const float* gp = a.gimg + (size_t)sid * img;
 #pragma unroll
-          for (int ch = 0; ch < 3; ++ch) g[h][ch] += __ldg(gp + ch);
+        for (int ch = 0; ch < 3; ++ch) {
+          v[k][ch] = have && in_a ? __ldg(gp + po_a + ch) : 0.0f;
+          v[k][3 + ch] = have && in_b ? __ldg(gp + po_b + ch) : 0.0f;
         }
-        const float* ip = a.images + (size_t)rep * img + po;
-        float dot = 0.0f;
+      }
 #pragma unroll
-        for (int ch = 0; ch < 3; ++ch) dot = __fmaf_rn(g[h][ch], __fsub_rn(__ldg(ip + ch), a.bg[ch]), dot);
-        gf[h] = dot * kTScale;
+      for (int k = 0; k < kGBatch; ++k) {
+        if (base + k < f_hi) {
+          if (base + k == bound) {  // warp-uniform: classes are non-empty, so one step at most
+            park(cur);
+            ++cur;
+            bound = mem ? s_mhi[cur] : bound + 1u;
+          }
+#pragma unroll
+          for (int c = 0; c < 6; ++c) acc[c] += v[k][c];
+        }
       }
     }
-    T2[s] = pack2(on && in_a ? kTScale : 0.0f, on && in_b ? kTScale : 0.0f);
-    E2[s] = pack2(-gf[0], -gf[1]);
-    gr2[s] = pack2(g[0][0], g[1][0]); gg2[s] = pack2(g[0][1], g[1][1]); gb2[s] = pack2(g[0][2], g[1][2]);
+    park(cur);
+    __syncwarp();
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+      const int rep = s_rep[s];
+      const bool on = rep >= 0;
+      float g[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, gf[2] = {0.f, 0.f};
+      if (on) {
+#pragma unroll
+        for (int c = 0; c < 6; ++c) g[c] = __uint_as_float(lds32(part_base + 4u * (uint32_t)((s * 6 + c) * 32 + lane)));
+        const float* ip = a.images + (size_t)rep * img;
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          if (h ? in_b : in_a) {
+            float dot = 0.0f;
+#pragma unroll
+            for (int ch = 0; ch < 3; ++ch)
+              dot = __fmaf_rn(g[3 * h + ch], __fsub_rn(__ldg(ip + (h ? po_b : po_a) + ch), a.bg[ch]), dot);
+            gf[h] = dot * kTScale;
+          }
+        }
+      }
+      T2[s] = pack2(on && in_a ? kTScale : 0.0f, on && in_b ? kTScale : 0.0f);
+      E2[s] = pack2(-gf[0], -gf[1]);
+      gr2[s] = pack2(g[0], g[3]); gg2[s] = pack2(g[1], g[4]); gb2[s] = pack2(g[2], g[5]);
+    }
+    __syncwarp();  // s_part is free again
   }
 
   const uint2 qr = a.qrange[tq];
