@@ -426,9 +426,9 @@ __global__ void __launch_bounds__(32, GSR_BW_MINB) k_backward_q(const BackwardAr
 }
 
 #ifndef GSR_BW_S
-#define GSR_BW_S 10
+#define GSR_BW_S 12
 #endif
-constexpr int kBackwardStateBlock = GSR_BW_S;  // measured on cfg1 (ms per 256-state frame): S = 2: 25.4, 4: 20.2, 8: 17.5
+constexpr int kBackwardStateBlock = GSR_BW_S;  // measured on cfg1 (ms per 256-state frame): S = 8: 7.6, 9: 7.2, 10: 6.8, 12: 6.67, 14: 11.6
 
 extern thread_local int g_dedup;  // k_composite.cu: option "dedup" of the calling thread
 
