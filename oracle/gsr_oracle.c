@@ -23,6 +23,13 @@
  *                                   gradient of a linear functional of one state's image with respect to the
  *                                   2-D quantities O-5 reads; the chain rule of O-5 written out, decisions fixed
  *                                   (pins: tests/test_backward_pins.py — finite differences of O-5, closed form)
+ *   O-9 backward of O-0/O-2/O-3 ... the same chain one step further back: from the gradient with respect to the
+ *                                   2-D quantities of a Gaussian in one state (O-8's output) to the gradient with
+ *                                   respect to the scene's own parameters (mean, motion residual, log-scale,
+ *                                   quaternion, opacity logit, SH coefficients, cluster affine, s_c); the chain
+ *                                   rule of DESIGN.md §3.0-§3.3 written out in double, decisions fixed
+ *                                   (pins: tests/test_projection_backward_pins.py — finite differences of
+ *                                   O-0/O-2/O-3, closed forms, invariants)
  *
  * Precision split.  Quantities that feed an INTEGER decision (deformed mean,
  * camera-space point, 2-D covariance, conic, radius, tile rectangle, depth bits, the quadratic
@@ -749,4 +756,274 @@ void orc_backward_O1(const orc_scene* s, const orc_camera* cam, const orc_proj* 
     }
   free(a_idx); free(a_alpha); free(a_T); free(a_e); free(a_dx); free(a_dy); free(a_cap);
   free(ord);
+}
+
+
+/* ------------------------------------------------------------------------------------------ */
+/* O-9  backward of activation, deformation, EWA projection and SH colour       */
+/* ------------------------------------------------------------------------------------------ */
+
+/* partial derivatives of the SH basis of sh_basis() with respect to x, y, z taken as three independent variables
+ * (the polynomial of each basis function differentiated term by term) */
+static void sh_basis_grad(int K, double x, double y, double z, double* Yx, double* Yy, double* Yz) {
+  const double pi = M_PI;
+  for (int j = 0; j < K; ++j) Yx[j] = Yy[j] = Yz[j] = 0.0;
+  if (K <= 1) return;
+  double c1 = sqrt(3.0 / (4.0 * pi));
+  Yy[1] = c1;
+  Yz[2] = c1;
+  Yx[3] = c1;
+  if (K <= 4) return;
+  double k4 = 0.5 * sqrt(15.0 / pi), k6 = 0.25 * sqrt(5.0 / pi), k8 = 0.25 * sqrt(15.0 / pi);
+  Yx[4] = k4 * y;       Yy[4] = k4 * x;                            /* k4 x y           */
+  Yy[5] = k4 * z;       Yz[5] = k4 * y;                            /* k4 y z           */
+  Yz[6] = k6 * 6.0 * z;                                            /* k6 (3 z^2 - 1)   */
+  Yx[7] = k4 * z;       Yz[7] = k4 * x;                            /* k4 x z           */
+  Yx[8] = k8 * 2.0 * x; Yy[8] = -k8 * 2.0 * y;                     /* k8 (x^2 - y^2)   */
+  if (K <= 9) return;
+  double k9 = 0.25 * sqrt(35.0 / (2.0 * pi)), k10 = 0.5 * sqrt(105.0 / pi), k11 = 0.25 * sqrt(21.0 / (2.0 * pi));
+  double k12 = 0.25 * sqrt(7.0 / pi), k14 = 0.25 * sqrt(105.0 / pi);
+  Yx[9] = k9 * 6.0 * x * y;              Yy[9] = k9 * (3.0 * x * x - 3.0 * y * y);             /* k9 y (3x^2 - y^2) */
+  Yx[10] = k10 * y * z;  Yy[10] = k10 * x * z;  Yz[10] = k10 * x * y;                           /* k10 x y z         */
+  Yy[11] = k11 * (5.0 * z * z - 1.0);    Yz[11] = k11 * 10.0 * y * z;                           /* k11 y (5z^2 - 1)  */
+  Yz[12] = k12 * (15.0 * z * z - 3.0);                                                           /* k12 (5z^3 - 3z)   */
+  Yx[13] = k11 * (5.0 * z * z - 1.0);    Yz[13] = k11 * 10.0 * x * z;                           /* k11 x (5z^2 - 1)  */
+  Yx[14] = k14 * 2.0 * x * z;  Yy[14] = -k14 * 2.0 * y * z;  Yz[14] = k14 * (x * x - y * y);    /* k14 (x^2 - y^2) z */
+  Yx[15] = k9 * (3.0 * x * x - 3.0 * y * y);  Yy[15] = -k9 * 6.0 * x * y;                       /* k9 x (x^2 - 3y^2) */
+}
+
+/* exported for its pin (finite differences of orc_sh_basis) */
+void orc_sh_basis_grad(int32_t K, double x, double y, double z, double* Yx, double* Yy, double* Yz) {
+  sh_basis_grad(K, x, y, z, Yx, Yy, Yz);
+}
+
+/* One state.  For every Gaussian i present in the state (cluster depth d = depth[c] >= level(i)) and not culled by
+ * z > znear / det > 0, g9[i] = dL/d(rgb[3], opacity, A, B, Cq, m_x, m_y) (O-8's layout) is carried back through
+ *   colour      rgb_ch = max(0, S_ch), S_ch = 0.5 + sum_j Y_j(dir) coef_j,ch, coef = sh_base (+ sh_res iff d = 3),
+ *               dir = (mu - camera centre) / |.|
+ *   projection  DESIGN.md §3.3 in its written order (pc, rz, txz, the clamp, J, M = J R, Sigma' = M Sigma M^T + 0.3 I,
+ *               conic = Sigma'^-1, A = conic_a / 2, B = conic_b, Cq = conic_c / 2, m = f txz + c)
+ *   deformation mu = p + [d >= 1] rho, p = A_c(t) [mu_bar; 1], rho = s_c sum_r b_r q_r          (Eq. (1))
+ *   activation  Sigma = M M^T, M = Rm(quat / |quat|) diag(exp(log_scale)); opacity = sigmoid(logit)  (§3.0)
+ * all in double from the raw parameters.  Fixed decisions (constants of the differentiation, reading K1): presence,
+ * the culls, the clamp of x/z, y/z at +-1.3 lim (a clamped coordinate passes no gradient through x~), rgb = max(0, .)
+ * (no gradient where S_ch <= 0), tau, the radius and the rectangle.
+ * Outputs are ACCUMULATED (+=), so that the caller sums states:
+ *   g_mean [N,3], g_rho [N,3] (rho = the motion residual vector; dL/d(s_c q_{i,r,k}) = b_r g_rho[i,k]),
+ *   g_ls [N,3], g_quat [N,4] (raw quaternion), g_logit [N], g_shb / g_shr [N,K,3], g_A [C,12] (A_c(t), row-major 3x4;
+ *   dL/dA0 = g_A, dL/dA1 = t g_A), g_sc [C].
+ * margin [N] (overwritten where the Gaussian is present): the smallest relative distance of a decision from its
+ * threshold — a caller comparing against an fp32 implementation skips Gaussians whose margin is tiny.
+ * Returns 0, or -1 for scenes this oracle does not cover (position residual levels, per-level attribute
+ * refinements, affine on the covariance). */
+int32_t orc_project_backward_O9(const orc_scene* s, const float* log_scale, const float* quat, const float* logit,
+                                const orc_camera* cam, float t, const int8_t* depth, const double* g9,
+                                double* g_mean, double* g_rho, double* g_ls, double* g_quat, double* g_logit,
+                                double* g_shb, double* g_shr, double* g_A, double* g_sc, double* margin) {
+  if (s->delta2 || s->delta3 || s->cov3d_lv || s->d_sh || s->affine_cov) return -1;
+  float basis_f[64];
+  orc_basis(t, s->R, basis_f);
+  double Rw[9], tw[3];
+  for (int k = 0; k < 9; ++k) Rw[k] = (double)cam->R[k];
+  for (int k = 0; k < 3; ++k) tw[k] = (double)cam->t[k];
+  const double fx = cam->fx, fy = cam->fy;
+  double cc3[3]; /* camera centre = -R^T t */
+  for (int k = 0; k < 3; ++k) cc3[k] = -(Rw[0 + k] * tw[0] + Rw[3 + k] * tw[1] + Rw[6 + k] * tw[2]);
+  const double limx = ((0.5 * (double)cam->W) / fx) * 1.3, limy = ((0.5 * (double)cam->H) / fy) * 1.3;
+
+  for (int c = 0; c < s->C; ++c)
+    for (int i = s->group_off[4 * c]; i < s->group_off[4 * c + 4]; ++i) {
+      const int d = (int)depth[c];
+      if (d < level_of(s, c, i)) continue;
+      const double* g = g9 + 9 * (int64_t)i;
+      double mg = 1e300;
+
+      /* ================= forward, in double ================= */
+      /* O-0 */
+      double sc3[3];
+      for (int k = 0; k < 3; ++k) sc3[k] = exp((double)log_scale[3 * (int64_t)i + k]);
+      const double qw = quat[4 * (int64_t)i + 0], qx = quat[4 * (int64_t)i + 1], qy = quat[4 * (int64_t)i + 2],
+                   qz = quat[4 * (int64_t)i + 3];
+      const double qn = sqrt(qw * qw + qx * qx + qy * qy + qz * qz);
+      const double w = qw / qn, x = qx / qn, y = qy / qn, z = qz / qn;
+      const double Rm[9] = {1.0 - 2.0 * (y * y + z * z), 2.0 * (x * y - w * z),       2.0 * (x * z + w * y),
+                            2.0 * (x * y + w * z),       1.0 - 2.0 * (x * x + z * z), 2.0 * (y * z - w * x),
+                            2.0 * (x * z - w * y),       2.0 * (y * z + w * x),       1.0 - 2.0 * (x * x + y * y)};
+      double Mm[9], Sg[9]; /* Mm = Rm diag(s); Sigma = Mm Mm^T (full 3x3) */
+      for (int a = 0; a < 3; ++a)
+        for (int k = 0; k < 3; ++k) Mm[3 * a + k] = Rm[3 * a + k] * sc3[k];
+      for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b)
+          Sg[3 * a + b] = Mm[3 * a + 0] * Mm[3 * b + 0] + Mm[3 * a + 1] * Mm[3 * b + 1] + Mm[3 * a + 2] * Mm[3 * b + 2];
+      const double opac = 1.0 / (1.0 + exp(-(double)logit[i]));
+      /* O-2 */
+      double A[12];
+      for (int k = 0; k < 12; ++k) A[k] = (double)s->A0[12 * c + k] + (double)t * (double)s->A1[12 * c + k];
+      const double mb[3] = {s->mean[3 * (int64_t)i + 0], s->mean[3 * (int64_t)i + 1], s->mean[3 * (int64_t)i + 2]};
+      double acc[3], mu[3];
+      for (int k = 0; k < 3; ++k) {
+        const double p = A[4 * k + 0] * mb[0] + A[4 * k + 1] * mb[1] + A[4 * k + 2] * mb[2] + A[4 * k + 3];
+        acc[k] = 0.0;
+        for (int r = 0; r < s->R; ++r) acc[k] += (double)basis_f[r] * (double)s->motion_q[((int64_t)i * s->R + r) * 3 + k];
+        mu[k] = d >= 1 ? p + (double)s->motion_scale[c] * acc[k] : p;
+      }
+      /* O-3 */
+      double pc[3];
+      for (int k = 0; k < 3; ++k) pc[k] = Rw[3 * k + 0] * mu[0] + Rw[3 * k + 1] * mu[1] + Rw[3 * k + 2] * mu[2] + tw[k];
+      const double zc = pc[2];
+      mg = fmin(mg, fabs(zc - (double)cam->znear) / fmax(fabs(zc), 1e-30));
+      if (!(zc > (double)cam->znear)) { margin[i] = mg; continue; }
+      const double rz = 1.0 / zc, txz = pc[0] * rz, tyz = pc[1] * rz;
+      const int in_x = txz >= -limx && txz <= limx, in_y = tyz >= -limy && tyz <= limy;
+      mg = fmin(mg, fabs(fabs(txz) - limx) / limx);
+      mg = fmin(mg, fabs(fabs(tyz) - limy) / limy);
+      const double cxz = in_x ? txz : (txz < 0.0 ? -limx : limx), cyz = in_y ? tyz : (tyz < 0.0 ? -limy : limy);
+      const double xt = cxz * zc, yt = cyz * zc;
+      const double J00 = fx * rz, J02 = -(fx * xt) * rz * rz, J11 = fy * rz, J12 = -(fy * yt) * rz * rz;
+      double M0[3], M1[3], v0[3], v1[3];
+      for (int k = 0; k < 3; ++k) {
+        M0[k] = J00 * Rw[0 + k] + J02 * Rw[6 + k];
+        M1[k] = J11 * Rw[3 + k] + J12 * Rw[6 + k];
+      }
+      for (int a = 0; a < 3; ++a) {
+        v0[a] = Sg[3 * a + 0] * M0[0] + Sg[3 * a + 1] * M0[1] + Sg[3 * a + 2] * M0[2];
+        v1[a] = Sg[3 * a + 0] * M1[0] + Sg[3 * a + 1] * M1[1] + Sg[3 * a + 2] * M1[2];
+      }
+      const double s00 = M0[0] * v0[0] + M0[1] * v0[1] + M0[2] * v0[2];
+      const double s01 = M0[0] * v1[0] + M0[1] * v1[1] + M0[2] * v1[2];
+      const double s11 = M1[0] * v1[0] + M1[1] * v1[1] + M1[2] * v1[2];
+      const double a2 = s00 + 0.3, b2 = s01, c2 = s11 + 0.3;
+      const double det = a2 * c2 - b2 * b2;
+      mg = fmin(mg, fabs(det) / fmax(a2 * c2, 1e-300));
+      if (!(det > 0.0)) { margin[i] = mg; continue; }
+      /* colour */
+      double dv[3] = {mu[0] - cc3[0], mu[1] - cc3[1], mu[2] - cc3[2]};
+      const double nrm = sqrt(dv[0] * dv[0] + dv[1] * dv[1] + dv[2] * dv[2]);
+      const double dir[3] = {dv[0] / nrm, dv[1] / nrm, dv[2] / nrm};
+      double Y[16], Yx[16], Yy[16], Yz[16], Sch[3];
+      sh_basis(s->K, dir[0], dir[1], dir[2], Y);
+      sh_basis_grad(s->K, dir[0], dir[1], dir[2], Yx, Yy, Yz);
+      for (int ch = 0; ch < 3; ++ch) {
+        Sch[ch] = 0.5;
+        for (int j = 0; j < s->K; ++j) {
+          double coef = (double)s->sh_base[((int64_t)i * s->K + j) * 3 + ch];
+          if (d >= 3) coef += (double)s->sh_res[((int64_t)i * s->K + j) * 3 + ch];
+          Sch[ch] += Y[j] * coef;
+        }
+        mg = fmin(mg, fabs(Sch[ch]));
+      }
+      margin[i] = mg;
+
+      /* ================= backward ================= */
+      double dmu[3] = {0.0, 0.0, 0.0};
+      /* colour: rgb_ch = max(0, S_ch) */
+      {
+        double dS[3], dY[16];
+        for (int ch = 0; ch < 3; ++ch) dS[ch] = Sch[ch] > 0.0 ? g[ch] : 0.0;
+        for (int j = 0; j < s->K; ++j) {
+          dY[j] = 0.0;
+          for (int ch = 0; ch < 3; ++ch) {
+            double coef = (double)s->sh_base[((int64_t)i * s->K + j) * 3 + ch];
+            if (d >= 3) coef += (double)s->sh_res[((int64_t)i * s->K + j) * 3 + ch];
+            dY[j] += dS[ch] * coef;
+            g_shb[((int64_t)i * s->K + j) * 3 + ch] += Y[j] * dS[ch];
+            if (d >= 3) g_shr[((int64_t)i * s->K + j) * 3 + ch] += Y[j] * dS[ch];
+          }
+        }
+        double gdir[3] = {0.0, 0.0, 0.0};
+        for (int j = 0; j < s->K; ++j) {
+          gdir[0] += dY[j] * Yx[j];
+          gdir[1] += dY[j] * Yy[j];
+          gdir[2] += dY[j] * Yz[j];
+        }
+        /* dir = v / |v|: d dir_a / d v_b = (delta_ab - dir_a dir_b) / |v| */
+        const double dot = dir[0] * gdir[0] + dir[1] * gdir[1] + dir[2] * gdir[2];
+        for (int k = 0; k < 3; ++k) dmu[k] += (gdir[k] - dir[k] * dot) / nrm;
+      }
+      /* opacity = sigmoid(logit) */
+      g_logit[i] += g[3] * opac * (1.0 - opac);
+      /* A = conic_a / 2, B = conic_b, Cq = conic_c / 2; conic = (c, -b, a) / det, det = a c - b^2 */
+      const double gca = 0.5 * g[4], gcb = g[5], gcc = 0.5 * g[6];
+      const double det2 = det * det;
+      const double da = gca * (-c2 * c2 / det2) + gcb * (b2 * c2 / det2) + gcc * (1.0 / det - a2 * c2 / det2);
+      const double db = gca * (2.0 * b2 * c2 / det2) + gcb * (-1.0 / det - 2.0 * b2 * b2 / det2) + gcc * (2.0 * a2 * b2 / det2);
+      const double dc = gca * (1.0 / det - c2 * a2 / det2) + gcb * (b2 * a2 / det2) + gcc * (-a2 * a2 / det2);
+      /* a = s00 + 0.3, b = s01, c = s11 + 0.3; s00 = M0.Sigma M0, s01 = M0.Sigma M1, s11 = M1.Sigma M1 */
+      double G[9], dM0[3], dM1[3]; /* G_ab = dL/dSigma_ab, the nine entries taken as independent */
+      for (int a = 0; a < 3; ++a) {
+        for (int b = 0; b < 3; ++b) G[3 * a + b] = da * M0[a] * M0[b] + db * M0[a] * M1[b] + dc * M1[a] * M1[b];
+        dM0[a] = 2.0 * da * v0[a] + db * v1[a];
+        dM1[a] = 2.0 * dc * v1[a] + db * v0[a];
+      }
+      /* M0 = J00 R_0 + J02 R_2, M1 = J11 R_1 + J12 R_2 */
+      double dJ00 = 0.0, dJ02 = 0.0, dJ11 = 0.0, dJ12 = 0.0;
+      for (int k = 0; k < 3; ++k) {
+        dJ00 += dM0[k] * Rw[0 + k];
+        dJ02 += dM0[k] * Rw[6 + k];
+        dJ11 += dM1[k] * Rw[3 + k];
+        dJ12 += dM1[k] * Rw[6 + k];
+      }
+      /* J00 = fx rz, J02 = -fx xt rz^2, J11 = fy rz, J12 = -fy yt rz^2 */
+      double drz = fx * dJ00 + fy * dJ11 - 2.0 * fx * xt * rz * dJ02 - 2.0 * fy * yt * rz * dJ12;
+      const double dxt = -fx * rz * rz * dJ02, dyt = -fy * rz * rz * dJ12;
+      /* xt = clamp(txz) zc, yt = clamp(tyz) zc; m_x = fx txz + cx, m_y = fy tyz + cy */
+      double dzc = cxz * dxt + cyz * dyt;
+      double dtxz = fx * g[7], dtyz = fy * g[8];
+      if (in_x) dtxz += zc * dxt;
+      if (in_y) dtyz += zc * dyt;
+      /* txz = pc0 rz, tyz = pc1 rz, rz = 1 / zc */
+      double dpc[3];
+      dpc[0] = rz * dtxz;
+      dpc[1] = rz * dtyz;
+      drz += pc[0] * dtxz + pc[1] * dtyz;
+      dzc += -rz * rz * drz;
+      dpc[2] = dzc;
+      /* pc = R mu + t */
+      for (int k = 0; k < 3; ++k) dmu[k] += Rw[0 + k] * dpc[0] + Rw[3 + k] * dpc[1] + Rw[6 + k] * dpc[2];
+      /* Eq. (1): mu = p + [d >= 1] s_c acc, p = A [mu_bar; 1] */
+      if (d >= 1) {
+        for (int k = 0; k < 3; ++k) {
+          g_rho[3 * (int64_t)i + k] += dmu[k];
+          g_sc[c] += dmu[k] * acc[k];
+        }
+      }
+      for (int k = 0; k < 3; ++k) {
+        for (int j = 0; j < 3; ++j) {
+          g_mean[3 * (int64_t)i + j] += A[4 * k + j] * dmu[k];
+          g_A[12 * c + 4 * k + j] += dmu[k] * mb[j];
+        }
+        g_A[12 * c + 4 * k + 3] += dmu[k];
+      }
+      /* Sigma = Mm Mm^T, Mm = Rm diag(s), s = exp(log_scale) */
+      double dMm[9], dRm[9];
+      for (int a = 0; a < 3; ++a)
+        for (int k = 0; k < 3; ++k) {
+          dMm[3 * a + k] = 0.0;
+          for (int b = 0; b < 3; ++b) dMm[3 * a + k] += (G[3 * a + b] + G[3 * b + a]) * Mm[3 * b + k];
+        }
+      for (int k = 0; k < 3; ++k) {
+        double ds = 0.0;
+        for (int a = 0; a < 3; ++a) {
+          ds += dMm[3 * a + k] * Rm[3 * a + k];
+          dRm[3 * a + k] = dMm[3 * a + k] * sc3[k];
+        }
+        g_ls[3 * (int64_t)i + k] += ds * sc3[k];
+      }
+      /* Rm(w, x, y, z) entry by entry (the matrix written in O-0) */
+      const double dw = dRm[1] * (-2.0 * z) + dRm[2] * (2.0 * y) + dRm[3] * (2.0 * z) + dRm[5] * (-2.0 * x) +
+                        dRm[6] * (-2.0 * y) + dRm[7] * (2.0 * x);
+      const double dx_ = dRm[1] * (2.0 * y) + dRm[2] * (2.0 * z) + dRm[3] * (2.0 * y) + dRm[4] * (-4.0 * x) +
+                         dRm[5] * (-2.0 * w) + dRm[6] * (2.0 * z) + dRm[7] * (2.0 * w) + dRm[8] * (-4.0 * x);
+      const double dy_ = dRm[0] * (-4.0 * y) + dRm[1] * (2.0 * x) + dRm[2] * (2.0 * w) + dRm[3] * (2.0 * x) +
+                         dRm[5] * (2.0 * z) + dRm[6] * (-2.0 * w) + dRm[7] * (2.0 * z) + dRm[8] * (-4.0 * y);
+      const double dz_ = dRm[0] * (-4.0 * z) + dRm[1] * (-2.0 * w) + dRm[2] * (2.0 * x) + dRm[3] * (2.0 * w) +
+                         dRm[4] * (-4.0 * z) + dRm[5] * (2.0 * y) + dRm[6] * (2.0 * x) + dRm[7] * (2.0 * y);
+      /* (w, x, y, z) = quat / |quat| */
+      const double qd = w * dw + x * dx_ + y * dy_ + z * dz_;
+      g_quat[4 * (int64_t)i + 0] += (dw - w * qd) / qn;
+      g_quat[4 * (int64_t)i + 1] += (dx_ - x * qd) / qn;
+      g_quat[4 * (int64_t)i + 2] += (dy_ - y * qd) / qn;
+      g_quat[4 * (int64_t)i + 3] += (dz_ - z * qd) / qn;
+    }
+  return 0;
 }

@@ -71,6 +71,7 @@ def lib():
         _lib.orc_trace_pixel.restype = C.c_int64
         _lib.orc_sizeof_proj.restype = C.c_int32
         _lib.orc_num_threads.restype = C.c_int32
+        _lib.orc_project_backward_O9.restype = C.c_int32
         assert _lib.orc_sizeof_proj() == PROJ_DTYPE.itemsize, (_lib.orc_sizeof_proj(), PROJ_DTYPE.itemsize)
     return _lib
 
@@ -105,6 +106,14 @@ def sh_basis(K: int, d) -> np.ndarray:
     return Y[:K]
 
 
+def sh_basis_grad(K: int, d) -> np.ndarray:
+    """[3, K]: partial derivatives of the SH basis with respect to x, y, z taken as independent variables."""
+    g = np.zeros((3, 16), np.float64)
+    lib().orc_sh_basis_grad(C.c_int32(K), C.c_double(d[0]), C.c_double(d[1]), C.c_double(d[2]), _p(g[0]), _p(g[1]),
+                            _p(g[2]))
+    return g[:, :K]
+
+
 def make_camera(cam) -> _Camera:
     c = _Camera()
     c.R[:] = [float(v) for v in np.asarray(cam.R_wc, np.float32).reshape(9)]
@@ -133,6 +142,7 @@ class OracleScene:
         self.opacity = np.empty(self.N, np.float32)
         self.tau = np.empty(self.N, np.float32)
         ls, qt, lg = _c(sc.log_scale, np.float32), _c(sc.quat, np.float32), _c(sc.opacity_logit, np.float32)
+        self.log_scale, self.quat, self.opacity_logit = ls, qt, lg   # raw parameters (O-9 differentiates them)
         L.orc_activate(C.c_int64(self.N), _p(ls), _p(qt), _p(lg), _p(self.cov3d), _p(self.opacity),
                        _p(self.tau))
         s = _Scene()
@@ -218,6 +228,32 @@ class OracleScene:
         lib().orc_backward_O1(C.byref(self._s), C.byref(make_camera(cam)), _p(proj), C.c_double(t_stop), _p(g), _p(grad),
                               _p(gabs) if want_abs else None)
         return (grad, gabs) if want_abs else grad
+
+    PARAM_GRADS = ("mean", "rho", "log_scale", "quat", "opacity_logit", "sh_base", "sh_res", "A", "motion_scale")
+
+    def project_backward(self, cam, t: float, depth, g9, into: dict | None = None):
+        """orc_project_backward_O9: g9 = dL/d(rgb[3], opacity, A, B, Cq, m_x, m_y) double [N,9] of ONE state (the
+        output of `backward`) -> dict of double gradients with respect to the scene's parameters (PARAM_GRADS:
+        mean [N,3], rho [N,3] (motion residual vector), log_scale [N,3], quat [N,4], opacity_logit [N],
+        sh_base / sh_res [N,K,3], A [C,3,4] (A_c(t)), motion_scale [C]) plus "margin" [N].  `into` accumulates."""
+        d = _c(depth, np.int8)
+        g = _c(g9, np.float64)
+        assert d.shape == (self.C,) and g.shape == (self.N, 9)
+        out = into if into is not None else {
+            "mean": np.zeros((self.N, 3)), "rho": np.zeros((self.N, 3)), "log_scale": np.zeros((self.N, 3)),
+            "quat": np.zeros((self.N, 4)), "opacity_logit": np.zeros(self.N),
+            "sh_base": np.zeros((self.N, self.K, 3)), "sh_res": np.zeros((self.N, self.K, 3)),
+            "A": np.zeros((self.C, 3, 4)), "motion_scale": np.zeros(self.C), "margin": np.full(self.N, np.inf)}
+        margin = np.full(self.N, np.inf)
+        rc = lib().orc_project_backward_O9(
+            C.byref(self._s), _p(self.log_scale), _p(self.quat), _p(self.opacity_logit), C.byref(make_camera(cam)),
+            C.c_float(t), _p(d), _p(g), _p(out["mean"]), _p(out["rho"]), _p(out["log_scale"]), _p(out["quat"]),
+            _p(out["opacity_logit"]), _p(out["sh_base"]), _p(out["sh_res"]), _p(out["A"]), _p(out["motion_scale"]),
+            _p(margin))
+        if rc != 0:
+            raise ValueError("orc_project_backward_O9 does not cover this scene (residual levels / refinements)")
+        out["margin"] = np.minimum(out["margin"], margin)
+        return out
 
     def trace_pixel(self, cam, t: float, depth, x: int, y: int, t_stop: float = 1e-4, cap: int = 4096):
         proj = self.project(cam, t, depth)
