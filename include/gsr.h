@@ -175,6 +175,26 @@ int64_t gsr_num_records(const gsr_scene* scene);
 int gsr_render_backward(const gsr_scene* scene, void* workspace, const float* images, const float* dL_dimages,
                         int32_t B, float* grad, void* cuda_stream);
 
+/* ------------------------------------------------------------------------------------------------
+ * gsr_project_backward — the backward of the steps in front of the compositor: activation,
+ * deformation Eq. (1), EWA projection and SH colour; DESIGN.md §17.  Takes the
+ * per-record gradient gsr_render_backward produced for a frame (same scene, camera and t) to the gradient with
+ * respect to the scene's own parameters.  Needs no workspace: the projection is recomputed.
+ *   grad_records dev fp32 [gsr_num_records(scene), 12]   (16-byte aligned)
+ *   g_gauss      dev fp32 [N, 14], overwritten: d/d(mean[3], rho[3], log_scale[3], quat[4], opacity_logit) with rho
+ *                the motion residual vector s_c sum_r b_r(t) q_{i,r} of Eq. (1): the gradient with respect to the
+ *                real-valued coefficient s_c q_{i,r,k} is b_r(t) * d/drho_k, b_r(t) = cos(pi r t); quat is the raw
+ *                (unnormalised) quaternion
+ *   g_sh_base    dev fp32 [N, K, 3], overwritten: d/d(sh_base); g_sh_res likewise for the level-3 payload
+ *   g_cluster    dev fp32 [C, 13], overwritten: d/dA_c(t) [3,4] row-major (d/dA0 = it, d/dA1 = t * it), d/ds_c
+ * The discrete decisions are constants of the differentiation: presence, the culls, the clamp of x/z and y/z at
+ * 1.3 lim (a clamped coordinate passes no gradient through the Jacobian), rgb = max(0, .), tau, radius, rectangle.
+ * Asynchronous on `cuda_stream`; the per-cluster sums use float atomics (reproducible up to fp32 summation
+ * order).  Scenes with position residual levels, per-level attribute refinements or affine_on_covariance are
+ * refused (GSR_E_INVALID_ARG). */
+int gsr_project_backward(const gsr_scene* scene, const gsr_camera* cam, float t, const float* grad_records,
+                         float* g_gauss, float* g_sh_base, float* g_sh_res, float* g_cluster, void* cuda_stream);
+
 /* Synchronises `cuda_stream` and reads the status latched by the last render into `workspace`:
  * returns GSR_OK, GSR_E_INVALID_LEVEL or GSR_E_WORKSPACE_TOO_SMALL.  keys_needed (host, may be NULL)
  * receives the number of (tile, depth, record) keys the frame produced. */

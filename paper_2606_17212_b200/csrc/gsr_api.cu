@@ -293,6 +293,7 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
   // ---- host staging in the device layout
   std::vector<float4> g0(Np), g1(Np), g2(Np), shb((size_t)n_sh4 * Np), shr((size_t)n_sh4 * Np);
   std::vector<uint32_t> qw((size_t)n_qw * Np, 0u);
+  std::vector<float4> rawq(Np), rawl(Np);
   for (int c = 0; c < C; ++c)
     for (int l = 0; l < 4; ++l)
       for (int i = d->group_off[4 * c + l]; i < d->group_off[4 * c + l + 1]; ++i) {
@@ -304,6 +305,8 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
         g0[i] = make_float4(d->mean[3 * (size_t)i], d->mean[3 * (size_t)i + 1], d->mean[3 * (size_t)i + 2], opac);
         g1[i] = make_float4(cov[0], cov[1], cov[2], tau);
         g2[i] = make_float4(cov[3], cov[4], cov[5], bitsf);
+        rawq[i] = make_float4(d->quat[4 * (size_t)i], d->quat[4 * (size_t)i + 1], d->quat[4 * (size_t)i + 2], d->quat[4 * (size_t)i + 3]);
+        rawl[i] = make_float4(d->log_scale[3 * (size_t)i], d->log_scale[3 * (size_t)i + 1], d->log_scale[3 * (size_t)i + 2], d->opacity_logit[i]);
         for (int w4 = 0; w4 < n_sh4; ++w4) {
           float vb[4] = {0, 0, 0, 0}, vr[4] = {0, 0, 0, 0};
           for (int e = 0; e < 4; ++e) {
@@ -341,6 +344,7 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
                o_shr = reserve(sizeof(float4) * n_sh4 * Np), o_qw = reserve(sizeof(uint32_t) * n_qw * Np),
                o_A0 = reserve(sizeof(float) * 12 * C), o_A1 = reserve(sizeof(float) * 12 * C),
                o_ms = reserve(sizeof(float) * C), o_go = reserve(sizeof(int32_t) * (4 * C + 1)),
+               o_rq = reserve(sizeof(float4) * Np), o_rl = reserve(sizeof(float4) * Np),
                o_dl = reserve(has_delta ? sizeof(float) * 6 * Np : 0),
                o_g1v = reserve(has_attr ? sizeof(float4) * 4 * Np : 0), o_g2v = reserve(has_attr ? sizeof(float4) * 4 * Np : 0),
                o_opv = reserve(has_attr ? sizeof(float) * 4 * Np : 0),
@@ -356,6 +360,7 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
   D.sh_base = (float4*)(base + o_shb); D.sh_res = (float4*)(base + o_shr); D.qw = (uint32_t*)(base + o_qw);
   D.A0 = (float*)(base + o_A0); D.A1 = (float*)(base + o_A1); D.mscale = (float*)(base + o_ms);
   D.group_off = (int32_t*)(base + o_go);
+  D.raw_quat = (float4*)(base + o_rq); D.raw_ls = (float4*)(base + o_rl);
   if (has_delta) D.delta = (float*)(base + o_dl);
   if (has_dsh) D.d_sh = (float4*)(base + o_dsh);
   if (has_attr) { D.g1v = (float4*)(base + o_g1v); D.g2v = (float4*)(base + o_g2v); D.opv = (float*)(base + o_opv); }
@@ -367,6 +372,7 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
   up(D.g2, g2.data(), sizeof(float4) * Np);
   up(D.sh_base, shb.data(), sizeof(float4) * n_sh4 * Np); up(D.sh_res, shr.data(), sizeof(float4) * n_sh4 * Np);
   up(D.qw, qw.data(), sizeof(uint32_t) * n_qw * Np);
+  up(D.raw_quat, rawq.data(), sizeof(float4) * Np); up(D.raw_ls, rawl.data(), sizeof(float4) * Np);
   up(D.A0, d->A0, sizeof(float) * 12 * C); up(D.A1, d->A1, sizeof(float) * 12 * C);
   up(D.mscale, d->motion_scale, sizeof(float) * C); up(D.group_off, d->group_off, sizeof(int32_t) * (4 * C + 1));
   if (has_delta) {  // SoA [6][N]: delta2.xyz, delta3.xyz; a missing array is zero (reading I1)
@@ -558,6 +564,25 @@ int gsr_render_backward(const gsr_scene* scene, void* workspace, const float* im
   Workspace ws;
   carve_workspace(&ws, workspace, rec_half(scene->impl.d), h.C, h.B, h.TX * h.TY, h.key_capacity);
   launch_backward(scene->impl.d, h, ws, images, dL_dimages, grad, st);
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
+int gsr_project_backward(const gsr_scene* scene, const gsr_camera* cam, float t, const float* grad_records,
+                         float* g_gauss, float* g_sh_base, float* g_sh_res, float* g_cluster, void* cuda_stream) {
+  if (!scene || !camera_ok(cam) || !g_cluster || (scene->impl.d.N > 0 && (!grad_records || !g_gauss || !g_sh_base || !g_sh_res))) {
+    set_error("gsr_project_backward: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  const DeviceScene& D = scene->impl.d;
+  if (D.V != 2 || D.affine_cov) {
+    set_error("gsr_project_backward: scenes with position residual levels, per-level attribute refinements or the "
+              "affine on the covariance are not covered");
+    return GSR_E_INVALID_ARG;
+  }
+  FrameParams fp;
+  make_frame(&scene->impl, cam, t, &fp);
+  launch_project_backward(D, fp, grad_records, g_gauss, g_sh_base, g_sh_res, g_cluster, (cudaStream_t)cuda_stream);
   GSR_CUDA(cudaGetLastError());
   return GSR_OK;
 }

@@ -36,6 +36,8 @@ struct DeviceScene {
   float* opv;       // [4][N] per-depth opacity
   float4* d_sh;     // [3][n_sh4][N] per-level colour residuals (layout of sh_base), else nullptr
   int32_t* group_off;  // [4C+1]
+  float4* raw_quat;    // [N] the quaternion as given (w, x, y, z): the backward of the activation (k_project_backward.cu)
+  float4* raw_ls;      // [N] log_scale.xyz, opacity_logit
   float bg[3];
 };
 
@@ -169,6 +171,8 @@ void count_launches(int n);
 struct CompositeArgs;
 void launch_composite_q(const CompositeArgs& a, int S, bool count, cudaStream_t st);
 // backward of a4 (k_backward.cu): grad [records, 12], zeroed by the call
+void launch_project_backward(const DeviceScene& sc, const FrameParams& fp, const float* grad_rec, float* g_gauss,
+                             float* g_shb, float* g_shr, float* g_cluster, cudaStream_t st);
 void launch_backward(const DeviceScene& sc, const WsHeader& h, Workspace& ws, const float* images, const float* gimg,
                      float* grad, cudaStream_t st);
 void launch_distortion_finalize_blk(const double* blk, int32_t B, int32_t tiles, int64_t n_values, double* mse,

@@ -80,6 +80,7 @@ def lib():
         L.gsr_num_records.argtypes = [vp]
         L.gsr_num_records.restype = i64
         L.gsr_render_backward.argtypes = [vp, vp, vp, vp, i32, vp, vp]
+        L.gsr_project_backward.argtypes = [vp, C.POINTER(CameraC), f32, vp, vp, vp, vp, vp, vp]
         L.gsr_close_levels.argtypes = [vp, i64, vp, vp, vp]
         L.gsr_frame_workspace_bytes.argtypes = [vp, C.POINTER(CameraC), i32, i32, i32, i32]
         L.gsr_frame_workspace_bytes.restype = sz
@@ -272,6 +273,23 @@ class Scene:
         _check(lib().gsr_render_backward(self.handle, _dp(workspace), _dp(images), _dp(dL_dimages),
                                          int(images.shape[0]), _dp(grad), _stream()))
         return grad
+
+    def project_backward(self, cam, t: float, grad_records):
+        """gsr_project_backward: grad_records cuda float32 [num_records, 12] (from render_backward, same cam and t)
+        -> dict of cuda float32 gradients: gauss [N,14] (mean 3, rho 3, log_scale 3, quat 4, opacity_logit),
+        sh_base / sh_res [N,K,3], cluster [C,13] (A_c(t) 3x4, s_c)."""
+        torch = _torch()
+        assert grad_records.dtype == torch.float32 and grad_records.is_cuda and grad_records.is_contiguous()
+        assert tuple(grad_records.shape) == (self.num_records(), 12)
+        K = (self.sh_degree + 1) ** 2
+        out = {"gauss": torch.empty((self.N, 14), dtype=torch.float32, device="cuda"),
+               "sh_base": torch.empty((self.N, K, 3), dtype=torch.float32, device="cuda"),
+               "sh_res": torch.empty((self.N, K, 3), dtype=torch.float32, device="cuda"),
+               "cluster": torch.empty((self.C, 13), dtype=torch.float32, device="cuda")}
+        _check(lib().gsr_project_backward(self.handle, C.byref(camera_struct(cam)), float(t), _dp(grad_records),
+                                          _dp(out["gauss"]), _dp(out["sh_base"]), _dp(out["sh_res"]),
+                                          _dp(out["cluster"]), _stream()))
+        return out
 
     def debug_pair_counts(self, workspace) -> np.ndarray:
         c = np.zeros(3, np.int64)
