@@ -475,29 +475,38 @@ def measure_ours(args, workload: str, steps: int, warmup: int, full: bool):
                   "share_of_step": (proj_ms + sort_ms) / ms_serial}
     roofline.update(traffic_record(wl.name))
 
-    # ---- backward of the compositor (gsr_render_backward; SURVEY.md §8(f)-4 follow-on): forward + backward of the
-    #      same frames, one frame in flight, dL/d(image) resident (a fixed random tensor: the kernel's work does not
-    #      depend on its values)
+    # ---- backward (gsr_render_backward: the compositor; gsr_project_backward: projection, SH colour, Eq. (1) and the
+    #      activation; SURVEY.md §8(f)-4 follow-on): forward + backward of the same frames, one frame in flight,
+    #      dL/d(image) resident (a fixed random tensor: the kernels' work does not depend on its values)
     backward = None
     if full and not args.no_backward:
         n_b = min(steps, 6)
         gimg = torch.randn((B, H, W, 3), dtype=torch.float32, device=dev) * (2.0 / (3.0 * W * H))
         b0 = bufs[0]
+        grec = torch.empty((scene.num_records(), 12), dtype=torch.float32, device=dev)
+        chain = scene.V == 2                      # gsr_project_backward covers the 2-record scenes (all configs)
+        gpar = [None]
 
-        def fwd_bwd(k, with_bwd=True):
+        def fwd_bwd(k, mode=2):
             frame_into(b0, k, True)
-            if with_bwd:
-                scene.render_backward(b0["ws"], b0["out"], gimg)
+            if mode >= 1:
+                scene.render_backward(b0["ws"], b0["out"], gimg, grad=grec)
+            if mode >= 2 and chain:
+                f = frame_of(k)
+                gpar[0] = scene.project_backward(cams[f], ts[f], grec, out=gpar[0])
 
         for k in range(2):
             fwd_bwd(warmup + k)
-        ms_fb = timed(fwd_bwd, warmup, n_b)
-        ms_f = timed(lambda k: fwd_bwd(k, False), warmup, n_b)
-        backward = {"value": B * n_b * world / (ms_fb * 1e-3), "unit": "states/s (forward + backward)",
-                    "ms_per_step_forward_backward": ms_fb / n_b, "ms_per_step_forward": ms_f / n_b,
-                    "ms_per_step_backward": (ms_fb - ms_f) / n_b, "steps": n_b,
-                    "note": "gsr_render_states_vs_full + gsr_render_backward, one frame in flight; grad [records, 12] summed over the %d states" % B}
-        del gimg
+        ms_fbp = timed(fwd_bwd, warmup, n_b)
+        ms_fb = timed(lambda k: fwd_bwd(k, 1), warmup, n_b)
+        ms_f = timed(lambda k: fwd_bwd(k, 0), warmup, n_b)
+        backward = {"value": B * n_b * world / (ms_fbp * 1e-3), "unit": "states/s (forward + backward)",
+                    "ms_per_step_forward_backward": ms_fbp / n_b, "ms_per_step_forward": ms_f / n_b,
+                    "ms_per_step_backward": (ms_fb - ms_f) / n_b,
+                    "ms_per_step_project_backward": (ms_fbp - ms_fb) / n_b if chain else None, "steps": n_b,
+                    "note": "gsr_render_states_vs_full + gsr_render_backward (grad [records, 12] summed over the %d "
+                            "states) + gsr_project_backward (gradients of the scene's parameters), one frame in flight" % B}
+        del gimg, grec
 
     # ---- CPU oracle on this box's cores, bounded sample of the same workload
     cpu = None

@@ -263,29 +263,36 @@ class Scene:
     def num_records(self) -> int:
         return int(lib().gsr_num_records(self.handle))
 
-    def render_backward(self, workspace, images, dL_dimages):
+    def render_backward(self, workspace, images, dL_dimages, grad=None):
         """gsr_render_backward after a forward call on `workspace`: images, dL_dimages cuda float32 [B,H,W,3] ->
-        cuda float32 [num_records, 12] (see include/gsr.h for the columns)."""
+        cuda float32 [num_records, 12] (see include/gsr.h for the columns); `grad` reuses a buffer."""
         torch = _torch()
         for t in (images, dL_dimages):
             assert t.dtype == torch.float32 and t.is_cuda and t.is_contiguous() and t.shape == images.shape
-        grad = torch.empty((self.num_records(), 12), dtype=torch.float32, device="cuda")
+        if grad is None:
+            grad = torch.empty((self.num_records(), 12), dtype=torch.float32, device="cuda")
+        assert grad.dtype == torch.float32 and grad.is_cuda and grad.is_contiguous() and tuple(grad.shape) == (self.num_records(), 12)
         _check(lib().gsr_render_backward(self.handle, _dp(workspace), _dp(images), _dp(dL_dimages),
                                          int(images.shape[0]), _dp(grad), _stream()))
         return grad
 
-    def project_backward(self, cam, t: float, grad_records):
+    def project_backward(self, cam, t: float, grad_records, out=None):
         """gsr_project_backward: grad_records cuda float32 [num_records, 12] (from render_backward, same cam and t)
         -> dict of cuda float32 gradients: gauss [N,14] (mean 3, rho 3, log_scale 3, quat 4, opacity_logit),
-        sh_base / sh_res [N,K,3], cluster [C,13] (A_c(t) 3x4, s_c)."""
+        sh_base / sh_res [N,K,3], cluster [C,13] (A_c(t) 3x4, s_c); `out` reuses the dict of a previous call."""
         torch = _torch()
         assert grad_records.dtype == torch.float32 and grad_records.is_cuda and grad_records.is_contiguous()
         assert tuple(grad_records.shape) == (self.num_records(), 12)
         K = (self.sh_degree + 1) ** 2
-        out = {"gauss": torch.empty((self.N, 14), dtype=torch.float32, device="cuda"),
-               "sh_base": torch.empty((self.N, K, 3), dtype=torch.float32, device="cuda"),
-               "sh_res": torch.empty((self.N, K, 3), dtype=torch.float32, device="cuda"),
-               "cluster": torch.empty((self.C, 13), dtype=torch.float32, device="cuda")}
+        if out is None:
+            out = {"gauss": torch.empty((self.N, 14), dtype=torch.float32, device="cuda"),
+                   "sh_base": torch.empty((self.N, K, 3), dtype=torch.float32, device="cuda"),
+                   "sh_res": torch.empty((self.N, K, 3), dtype=torch.float32, device="cuda"),
+                   "cluster": torch.empty((self.C, 13), dtype=torch.float32, device="cuda")}
+        for name, shape in (("gauss", (self.N, 14)), ("sh_base", (self.N, K, 3)), ("sh_res", (self.N, K, 3)),
+                            ("cluster", (self.C, 13))):
+            v = out[name]
+            assert v.dtype == torch.float32 and v.is_cuda and v.is_contiguous() and tuple(v.shape) == shape
         _check(lib().gsr_project_backward(self.handle, C.byref(camera_struct(cam)), float(t), _dp(grad_records),
                                           _dp(out["gauss"]), _dp(out["sh_base"]), _dp(out["sh_res"]),
                                           _dp(out["cluster"]), _stream()))
