@@ -451,7 +451,11 @@ void launch_backward(const DeviceScene& sc, const WsHeader& h, Workspace& ws, co
   a.images = images; a.gimg = gimg; a.grad = grad;
   a.uorder = dedup ? ws.uorder : nullptr; a.upos = dedup ? ws.upos : nullptr; a.n_unique = dedup ? ws.n_unique : nullptr;
   const size_t smem = sizeof(uint16_t) * 4 * (size_t)sc.C;
-  if (smem > 40 * 1024)
+  // static (staging + the pending partials, ~17 KB) + dynamic (the presence table, 8 bytes per cluster) passes the
+  // default 48 KB from C ~ 3900 on: opt in whenever the sum does
+  cudaFuncAttributes fa;
+  cudaFuncGetAttributes(&fa, k_backward_q<kBackwardStateBlock>);
+  if (smem + fa.sharedSizeBytes > 48 * 1024)
     cudaFuncSetAttribute(k_backward_q<kBackwardStateBlock>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                          (int)(sizeof(uint16_t) * 4 * kMaxC));
   const long long items = (long long)a.tiles * 4 * a.nsb;

@@ -231,3 +231,23 @@ def test_backward_dedup_option_off_gives_the_same_gradient(gsr, torch_mod):
     assert float(((grad_on - grad_off).abs() / scale).max()) <= 2e-4
     assert bool((grad_on != 0).any())
     scene.close()
+
+
+def test_backward_maximum_cluster_count(gsr, torch_mod, oracle_mod):
+    """C = 4096, the documented maximum: the presence table (8 bytes per cluster) plus the kernel's static shared
+    memory pass the default 48 KB, so the launch needs the opt-in; against the oracle, with and without dedup."""
+    rng = np.random.default_rng(4097)
+    Cn, n = 4096, 6000
+    scn, _ = tiny_scene(rng.uniform(-0.8, 0.8, (n, 3)), rng.uniform(0.03, 0.08, (n, 3)), logits=rng.uniform(-1, 3, n),
+                        colors=rng.uniform(0.1, 0.9, (n, 3)), levels=rng.integers(0, 4, n), clusters=np.arange(n) % Cn,
+                        C=Cn, background=(0.1, 0.1, 0.1))
+    cam = axis_camera(W=64, H=48, f=60.0, z0=3.0)
+    lv = synth.sample_levels(rng, 5, Cn)
+    for dedup in (1, 0):
+        gsr.set_option("dedup", dedup)
+        try:
+            got, g, V = _run(gsr, torch_mod, scn, cam, 0.0, lv, 9)
+        finally:
+            gsr.set_option("dedup", 1)
+        want = oracle_record_grads(oracle_mod, scn, cam, 0.0, lv, g, V)
+        _compare(got, want)
