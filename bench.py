@@ -705,7 +705,90 @@ def measure_atlas(args, steps: int, warmup: int, full: bool):
 
 
 
-SUB_WORKLOADS = ("cfg2", "cfg3", "cfg4", "atlas")
+def measure_train(args, steps: int, warmup: int, full: bool):
+    """--workload train: the forward-plus-backward render step at the size of the paper's Table 2 ("2.7M primitives",
+    128 worlds).  A step = one frame: B states rendered (images materialised),
+    gsr_render_backward with a resident dL/d(image), gsr_project_backward -> the gradients of the scene's parameters.
+    Reports world-frames/s (a world-frame = one rendered receiver-state image, the paper's unit) with three
+    repetitions and a Student-t 95 % interval, and the split of the step.  The paper's scene, resolution and masks are
+    not given: context for BASELINE.md row 2, not a comparison."""
+    import torch
+    from paper_2606_17212_b200 import build as gbuild
+    gbuild.build()
+    from paper_2606_17212_b200 import gsr
+
+    assert int(os.environ.get("WORLD_SIZE", "1")) == 1, "the train workload is a 1-GPU bench line"
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    n_frames = max(1, min(steps + warmup, 3))
+    wl = synth.workload_train(n_frames=n_frames, B=args.train_worlds, n_gaussians=args.train_gaussians)
+    scene = gsr.Scene(wl.scene)
+    cam0, _ = wl.frames[0]
+    W, H, B = cam0.W, cam0.H, wl.levels[0].shape[0]
+    cams = [gsr.camera_struct(c) for c, _ in wl.frames]
+    ts = [float(t) for _, t in wl.frames]
+    lv = [torch.from_numpy(np.ascontiguousarray(l)).to(dev) for l in wl.levels]
+    ws = scene.new_workspace(cam0, B)
+    out = torch.empty((B, H, W, 3), dtype=torch.float32, device=dev)
+    gimg = torch.randn((B, H, W, 3), dtype=torch.float32, device=dev) * (2.0 / (3.0 * W * H))
+    grec = torch.empty((scene.num_records(), 12), dtype=torch.float32, device=dev)
+    gpar = [None]
+
+    def step(k, mode=2):
+        f = k % n_frames
+        scene.render_states(cams[f], ts[f], lv[f], workspace=ws, out=out)
+        if mode >= 1:
+            scene.render_backward(ws, out, gimg, grad=grec)
+        if mode >= 2:
+            gpar[0] = scene.project_backward(cams[f], ts[f], grec, out=gpar[0])
+
+    def timed(fn, k0, K):
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for k in range(k0, k0 + K):
+            fn(k)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1)
+
+    for k in range(warmup):
+        step(k)
+    keys = scene.status(ws)
+    l0 = gsr.launch_count()
+    sampler = ClockSampler(0)
+    sampler.start()
+    sampler.mark()
+    reps = [timed(step, warmup + r * steps, steps) for r in range(3 if full else 1)]
+    clocks = sampler.stop()
+    launches = (gsr.launch_count() - l0) // len(reps)
+    ms_fb = timed(lambda k: step(k, 1), warmup, steps)
+    ms_f = timed(lambda k: step(k, 0), warmup, steps)
+    vals = [B * steps / (m * 1e-3) for m in reps]
+    value = float(np.mean(vals))
+    T975 = {1: 12.706, 2: 4.303, 3: 3.182, 4: 2.776}      # Student t, 97.5 %, n - 1 degrees of freedom
+    ci = float(T975[len(vals) - 1] * np.std(vals, ddof=1) / np.sqrt(len(vals))) if len(vals) > 1 else None
+    ms = float(np.mean(reps))
+    line = {"metric": "training_render_world_frames_per_s", "value": value, "unit": "world-frames/s (forward + backward)",
+            "value_reps": vals, "value_ci95": ci, "n_gpus": 1, "steps": steps, "warmup": warmup, "ms_per_step": ms / steps,
+            "ms_per_step_forward": ms_f / steps, "ms_per_step_backward": (ms_fb - ms_f) / steps,
+            "ms_per_step_project_backward": (ms - ms_fb) / steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": wl.name, "worlds": B, "resolution": [W, H], "gaussians": wl.scene.N,
+                       "clusters": wl.scene.C, "sh_degree": wl.scene.sh_degree, "R": wl.scene.R, "frames": n_frames,
+                       "keys_per_frame": int(keys), "images_materialised": True,
+                       "l2": "per-step working set (%.2f GB of images written, %.2f GB of dL/d(image) read) exceeds the "
+                             "126 MB L2; every step is a different frame" % (B * H * W * 12 / 1e9, B * H * W * 12 / 1e9)},
+            "clocks": clocks, "gpu_launches": int(launches),
+            "paper": {"value": 360.46, "unit": "world-frames/s", "where": "PAPER.md:238-249, Table 2, 128 worlds, H100 PCIe, "
+                      "2.7M primitives, scene replicated per world; scene / resolution / masks not given: context only"}}
+    scene.close()
+    del out, gimg, grec
+    return line
+
+
+SUB_WORKLOADS = ("cfg2", "cfg3", "cfg4", "atlas", "train")
 
 
 def run_ours(args):
@@ -713,6 +796,8 @@ def run_ours(args):
     — SURVEY.md §8(d), BASELINE.md "what we will measure" — a compact sub-record for each other workload."""
     if args.workload == "atlas":
         line = measure_atlas(args, args.steps, args.warmup, full=True)
+    elif args.workload == "train":
+        line = measure_train(args, max(1, min(args.steps, 6)), args.warmup, full=True)
     else:
         line = measure_ours(args, args.workload, args.steps, args.warmup, full=True)
     if line is None:                      # ranks other than 0
@@ -723,13 +808,18 @@ def run_ours(args):
         for name in SUB_WORKLOADS:
             t0 = time.perf_counter()
             try:
-                sub = measure_atlas(args, 2, 2, full=False) if name == "atlas" else measure_ours(args, name, 3, 3, full=False)
-                keep = ("value", "unit", "mpix_states_per_s", "steps", "warmup", "ms_per_step", "config", "clocks",
-                        "gpu_launches", "cpu_baseline")
+                if name == "train":
+                    sub = measure_train(args, 2, 3, full=False)
+                else:
+                    sub = measure_atlas(args, 2, 2, full=False) if name == "atlas" else measure_ours(args, name, 3, 3, full=False)
+                keep = ("metric", "value", "unit", "mpix_states_per_s", "steps", "warmup", "ms_per_step", "ms_per_step_forward",
+                        "ms_per_step_backward", "ms_per_step_project_backward", "config", "clocks", "gpu_launches",
+                        "cpu_baseline", "paper")
                 rec = {k: sub[k] for k in keep if k in sub}
-                r = sub["roofline"]
-                rec["roofline"] = {k: r[k] for k in ("kernel", "bound", "achieved", "peak", "unit", "frac",
-                                                     "kernel_share_of_step") if k in r}
+                r = sub.get("roofline")
+                if r:
+                    rec["roofline"] = {k: r[k] for k in ("kernel", "bound", "achieved", "peak", "unit", "frac",
+                                                         "kernel_share_of_step") if k in r}
                 rec["wall_s"] = time.perf_counter() - t0
                 subs[name] = rec
             except Exception as e:  # noqa: BLE001  a sub-record must never cost the headline line
@@ -744,7 +834,9 @@ def main():
     ap.add_argument("--steps", type=int, default=60)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg1", choices=["cfg0", "cfg1", "cfg1r", "cfg2", "cfg3", "cfg4", "atlas"])
+    ap.add_argument("--workload", default="cfg1", choices=["cfg0", "cfg1", "cfg1r", "cfg2", "cfg3", "cfg4", "atlas", "train"])
+    ap.add_argument("--train-worlds", type=int, default=128, help="--workload train: states per frame (the paper's worlds)")
+    ap.add_argument("--train-gaussians", type=float, default=2.7e6, help="--workload train: primitives")
     ap.add_argument("--ref-states", type=int, default=64, help="states per frame the CPU oracle renders")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-backward", action="store_true", help="skip the forward + backward timing")

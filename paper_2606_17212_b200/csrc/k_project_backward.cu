@@ -68,12 +68,13 @@ struct PbArgs {
 
 // One variant: geometry mean `mu`; gc0 / gc1 = dL/d(first / second colour) (gc1 only for the variant with the
 // residual), gq = dL/d(opacity, A, B, Cq, m_x, m_y).  Adds to dmu, dS6 (dL/dSigma, the 9 entries folded onto the 6
-// stored ones), dopac and the SH gradients of Gaussian i.  Returns false if the variant is culled.
+// stored ones), dopac and the SH gradients of Gaussian i (its rows of the CTA's shared tile).  Returns false if the
+// variant is culled.
 template <int K>
 __device__ __forceinline__ bool variant_backward(const DeviceScene& sc, const FrameParams& fp, int i, const float* mu,
                                                  const float* S6, bool with_res, const float* gc0, const float* gc1,
                                                  const float* gq, float* dmu, float* dS6, float& dopac,
-                                                 const PbArgs& a) {
+                                                 float* shb_row, float* shr_row) {
   const float* Rw = fp.R;
   float pc[3];
 #pragma unroll
@@ -159,9 +160,8 @@ __device__ __forceinline__ bool variant_backward(const DeviceScene& sc, const Fr
           if (flat < 3 * K) {
             const int j = flat / 3, ch = flat % 3;
             dY[j] += d0[ch] * vb[e] + d1[ch] * (vb[e] + vr[e]);
-            float* pb = a.g_shb + (size_t)i * 3 * K + flat;
-            *pb += Y[j] * (d0[ch] + d1[ch]);
-            if (with_res) a.g_shr[(size_t)i * 3 * K + flat] += Y[j] * d1[ch];
+            shb_row[flat] += Y[j] * (d0[ch] + d1[ch]);
+            if (with_res) shr_row[flat] += Y[j] * d1[ch];
           }
         }
       }
@@ -209,11 +209,20 @@ __device__ __forceinline__ bool variant_backward(const DeviceScene& sc, const Fr
   return true;
 }
 
+constexpr int kPbThreads = 64;
+
 template <int K>
-__global__ void __launch_bounds__(128) k_project_backward(DeviceScene sc, FrameParams fp, PbArgs a) {
+__global__ void __launch_bounds__(kPbThreads) k_project_backward(DeviceScene sc, FrameParams fp, PbArgs a) {
+  // the SH gradients of the CTA's Gaussians: [thread][3K (+1: conflict-free rows)], written out coalesced at the end
+  constexpr int kRow = 3 * K + 1;
+  __shared__ float s_shb[kPbThreads * kRow], s_shr[kPbThreads * kRow];
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int lane = threadIdx.x & 31;
   const bool live = i < sc.N;
+  float* const shb_row = s_shb + threadIdx.x * kRow;
+  float* const shr_row = s_shr + threadIdx.x * kRow;
+#pragma unroll
+  for (int f = 0; f < 3 * K; ++f) { shb_row[f] = 0.0f; shr_row[f] = 0.0f; }
   int c = -1;
   float cl13[13];
 #pragma unroll
@@ -253,14 +262,14 @@ __global__ void __launch_bounds__(128) k_project_backward(DeviceScene sc, FrameP
       const float4* gp = reinterpret_cast<const float4*>(a.grad_rec + 12 * (size_t)(2 * i));
 #pragma unroll
       for (int q = 0; q < 3; ++q) { const float4 v = __ldg(gp + q); g[4 * q] = v.x; g[4 * q + 1] = v.y; g[4 * q + 2] = v.z; g[4 * q + 3] = v.w; }
-      variant_backward<K>(sc, fp, i, p, S6, false, g, zero3, g + 6, dp, dS6, dopac, a);
+      variant_backward<K>(sc, fp, i, p, S6, false, g, zero3, g + 6, dp, dS6, dopac, shb_row, shr_row);
     }
     {  // variant B: record 2 i + 1, colours without / with the SH residual
       float g[12];
       const float4* gp = reinterpret_cast<const float4*>(a.grad_rec + 12 * (size_t)(2 * i + 1));
 #pragma unroll
       for (int q = 0; q < 3; ++q) { const float4 v = __ldg(gp + q); g[4 * q] = v.x; g[4 * q + 1] = v.y; g[4 * q + 2] = v.z; g[4 * q + 3] = v.w; }
-      variant_backward<K>(sc, fp, i, muB, S6, true, g, g + 3, g + 6, drho, dS6, dopac, a);
+      variant_backward<K>(sc, fp, i, muB, S6, true, g, g + 3, g + 6, drho, dS6, dopac, shb_row, shr_row);
     }
     // ---- deformation: mu_A = p, mu_B = p + rho
 #pragma unroll
@@ -308,6 +317,17 @@ __global__ void __launch_bounds__(128) k_project_backward(DeviceScene sc, FrameP
     out[12] = (dz - z * qd) * rqn;
     out[13] = dopac * g0.w * (1.0f - g0.w);
   }
+  // ---- the CTA's SH gradients: rows i0 .. i0 + 63 are contiguous in g_sh_base / g_sh_res
+  __syncthreads();
+  {
+    const size_t i0 = (size_t)blockIdx.x * kPbThreads;
+    const int rows = sc.N - (int)i0 < kPbThreads ? sc.N - (int)i0 : kPbThreads;
+    for (int f = threadIdx.x; f < rows * 3 * K; f += kPbThreads) {
+      const int r = f / (3 * K), col = f - r * (3 * K);
+      a.g_shb[i0 * 3 * K + f] = s_shb[r * kRow + col];
+      a.g_shr[i0 * 3 * K + f] = s_shr[r * kRow + col];
+    }
+  }
   // ---- per-cluster sums: over the warp when it holds one cluster, else lane by lane
   const int c0 = __shfl_sync(0xffffffffu, c, 0);
   if (__all_sync(0xffffffffu, c == c0)) {
@@ -328,15 +348,10 @@ __global__ void __launch_bounds__(128) k_project_backward(DeviceScene sc, FrameP
 
 void launch_project_backward(const DeviceScene& sc, const FrameParams& fp, const float* grad_rec, float* g_gauss,
                              float* g_shb, float* g_shr, float* g_cluster, cudaStream_t st) {
-  const size_t nsh = sizeof(float) * 3 * (size_t)sc.K * (size_t)sc.N;
-  if (sc.N > 0) {
-    cudaMemsetAsync(g_shb, 0, nsh, st);
-    cudaMemsetAsync(g_shr, 0, nsh, st);
-  }
   cudaMemsetAsync(g_cluster, 0, sizeof(float) * 13 * (size_t)sc.C, st);
   if (sc.N == 0) return;
   PbArgs a{grad_rec, g_gauss, g_shb, g_shr, g_cluster};
-  dim3 grid((sc.N + 127) / 128), block(128);
+  dim3 grid((sc.N + kPbThreads - 1) / kPbThreads), block(kPbThreads);
   switch (sc.K) {
     case 1: k_project_backward<1><<<grid, block, 0, st>>>(sc, fp, a); break;
     case 4: k_project_backward<4><<<grid, block, 0, st>>>(sc, fp, a); break;

@@ -213,7 +213,7 @@ def scene_cfg0() -> Scene:
                  np.zeros(3, np.float32))
 
 
-def _object_scene(cfg: int, C: int, per_cluster: float, f: float, background) -> Scene:
+def _object_scene(cfg: int, C: int, per_cluster: float, f: float, background, size_mul: float = 1.0) -> Scene:
     rng = _rng(cfg)
     R, deg = 8, 3
     n_c = np.rint(per_cluster * rng.uniform(0.8, 1.2, C)).astype(np.int64)
@@ -223,7 +223,7 @@ def _object_scene(cfg: int, C: int, per_cluster: float, f: float, background) ->
     centres = rng.uniform(-0.8, 0.8, (C, 3))
     cl = np.repeat(np.arange(C), counts.sum(axis=1))
     mean = np.clip(centres[cl] + 0.2 * rng.standard_normal((N, 3)), -1.0, 1.0).astype(np.float32)
-    log_scale = (np.log(2.5 * 4.0 / f) + 0.3 * rng.standard_normal((N, 3))).astype(np.float32)
+    log_scale = (np.log(size_mul * 2.5 * 4.0 / f) + 0.3 * rng.standard_normal((N, 3))).astype(np.float32)
     quat, logit, sh_base, sh_res, q = _common_attributes(rng, N, deg, R)
     A0, A1, s = _motion(rng, C, R)
     return Scene(C, N, deg, R, off, mean, log_scale, quat, logit, sh_base, sh_res, q, A0, A1, s,
@@ -335,6 +335,20 @@ def workload_cfg1(n_frames: int = 150, B: int = 256, scene: Scene | None = None)
     frames = [(cams[n], float(np.float32((n + 0.5) / 150.0))) for n in range(n_frames)]
     levels, iw, iwith, gid = _paired_frame_batches(1, sc, n_frames, B)
     return Workload("cfg1_object_centric_800x800_B256", sc, frames, levels, iw, iwith, gid, 4 * sc.C)
+
+
+def workload_train(n_frames: int = 3, B: int = 128, n_gaussians: float = 2.7e6, scene: Scene | None = None) -> Workload:
+    """The size of the paper's forward-plus-backward benchmark ("2.7M primitives", up to 128 worlds, PAPER.md:148,
+    238-249; its scene, resolution and masks are not given): the cfg1 recipe at 32 clusters x 84 k Gaussians, 800 x
+    800, B = 128 sampled states per frame, the Gaussians' extents scaled by sqrt(N_cfg1 / N) so that the summed
+    footprint — hence the depth complexity of a pixel — stays that of cfg1."""
+    C = 32
+    sc = scene if scene is not None else _object_scene(7, C, n_gaussians / C, focal_from_fov(800, 40.0), (1.0, 1.0, 1.0),
+                                                       size_mul=float(np.sqrt(1.0e5 / n_gaussians)))
+    cams = sphere_cameras(7, n_frames, 800, 800, 40.0)
+    frames = [(cams[n], float(np.float32((n + 0.5) / max(n_frames, 1)))) for n in range(n_frames)]
+    levels, iw, iwith, gid = _paired_frame_batches(7, sc, n_frames, B)
+    return Workload("train_object_centric_800x800_B%d_N%d" % (B, sc.N), sc, frames, levels, iw, iwith, gid, 4 * sc.C)
 
 
 def workload_cfg2(n_frames: int = 4, B: int = 512, scene: Scene | None = None) -> Workload:
