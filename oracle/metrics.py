@@ -24,6 +24,11 @@ What it follows (PAPER.md = /root/reference/PAPER.md; DESIGN.md §12 = the writt
                       (prev, next) of states where next is a larger prefix: M = sum max(0, D[next] - D[prev]);
                       violations = number of pairs with D[next] > D[prev].
 
+  gradient of D ..... d/d(image) of sum_b weight_b D_b, D = MSE + lambda (1 - SSIM) (the term E_w[D_w] of Eq. (2),
+                      PAPER.md:66-72): the chain rule of the definitions above written out (distortion_backward);
+                      pins: tests/test_distortion_backward_pins.py (central differences of D itself, the zero
+                      at image = reference, the MSE-only closed form)
+
 Pins: tests/test_metrics_pins.py (SSIM(x,x) = 1, constant-image closed form, scipy.ndimage Gaussian filtering
 as an independent library route, hand-worked CVaR / quantile, constant-shift flicker closed form, the paper's
 four monotone prefix points PAPER.md:94).
@@ -78,6 +83,48 @@ def ssim_map(img: np.ndarray, ref: np.ndarray) -> np.ndarray:
 def ssim(imgs: np.ndarray, ref: np.ndarray) -> np.ndarray:
     """[B, H, W, 3] vs [H, W, 3] -> SSIM per state, float64 [B]."""
     return np.array([ssim_map(im, ref).mean() for im in np.asarray(imgs)])
+
+
+def ssim_backward_map(img: np.ndarray, ref: np.ndarray) -> np.ndarray:
+    """d(mean of the SSIM map)/d(img) for one state, [H, W, 3].  With m1 = w*x, m2 = w*(x x), m12 = w*(x y) (the
+    three blurred planes that depend on x) and
+        N1 = 2 mu_x mu_y + C1, N2 = 2 s_xy + C2, D1 = mu_x^2 + mu_y^2 + C1, D2 = s_xx + s_yy + C2, ssim = N1 N2 / (D1 D2),
+        mu_x = m1, s_xx = m2 - m1^2, s_xy = m12 - m1 mu_y:
+        d ssim/d s_xx = -N1 N2 / (D1 D2^2)                      (= d ssim/d m2)
+        d ssim/d s_xy = 2 N1 / (D1 D2)                          (= d ssim/d m12)
+        d ssim/d m1   = 2 mu_y N2 / (D1 D2) - 2 mu_x N1 N2 / (D1^2 D2) - 2 mu_x d ssim/d s_xx - mu_y d ssim/d s_xy
+    A blurred plane is linear in x with the symmetric window (zero padding keeps the operator symmetric), so
+        d mean/dx = ( w*(d ssim/d m1) + 2 x w*(d ssim/d m2) + y w*(d ssim/d m12) ) / (3 H W)."""
+    x, y = np.asarray(img, np.float64), np.asarray(ref, np.float64)
+    out = np.zeros(x.shape)
+    n = float(x.size)
+    for ch in range(x.shape[2]):
+        xc, yc = x[:, :, ch], y[:, :, ch]
+        mx, my = _blur(xc), _blur(yc)
+        sxx = _blur(xc * xc) - mx * mx
+        syy = _blur(yc * yc) - my * my
+        sxy = _blur(xc * yc) - mx * my
+        N1, N2 = 2 * mx * my + SSIM_C1, 2 * sxy + SSIM_C2
+        D1, D2 = mx * mx + my * my + SSIM_C1, sxx + syy + SSIM_C2
+        d_sxx = -N1 * N2 / (D1 * D2 * D2)
+        d_sxy = 2 * N1 / (D1 * D2)
+        d_m1 = 2 * my * N2 / (D1 * D2) - 2 * mx * N1 * N2 / (D1 * D1 * D2) - 2 * mx * d_sxx - my * d_sxy
+        out[:, :, ch] = (_blur(d_m1) + 2 * xc * _blur(d_sxx) + yc * _blur(d_sxy)) / n
+    return out
+
+
+def distortion_backward(imgs: np.ndarray, ref: np.ndarray, weight, lam: float = MIX_WEIGHT) -> np.ndarray:
+    """d/d(imgs) of sum_b weight[b] (MSE_b + lam (1 - SSIM_b)): [B, H, W, 3] float64.
+    MSE_b = mean((img_b - ref)^2) over H x W x 3, so d MSE/d img = 2 (img - ref) / (3 H W)."""
+    im, rf = np.asarray(imgs, np.float64), np.asarray(ref, np.float64)
+    w = np.asarray(weight, np.float64).reshape(-1)
+    out = np.zeros(im.shape)
+    for b in range(im.shape[0]):
+        g = 2.0 * (im[b] - rf) / float(rf.size)
+        if lam != 0.0:
+            g = g - lam * ssim_backward_map(im[b], rf)
+        out[b] = w[b] * g
+    return out
 
 
 def mixed_distortion(mse: np.ndarray, ssim_v: np.ndarray) -> np.ndarray:
