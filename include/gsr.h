@@ -176,6 +176,16 @@ int gsr_render_backward(const gsr_scene* scene, void* workspace, const float* im
                         int32_t B, float* grad, void* cuda_stream);
 
 /* ------------------------------------------------------------------------------------------------
+ * gsr_distortion_backward — d/d(imgs) of L = sum_b weight[b] D_b with D_b = MSE_b + lambda_ssim (1 - SSIM_b)
+ * (the term E_w[D_w] of Eq. (2), "D = MSE + 0.20(1 - SSIM)"; SSIM per reading G1 as in
+ * gsr_distortion_ssim): the dL_dimages input of gsr_render_backward for that objective.
+ *   imgs fp32 dev [B,H,W,3]; ref fp32 dev [H,W,3]; weight double dev [B] or NULL (= 1 for every state; pass 1/B for
+ *   the mean over states); lambda_ssim >= 0 (0.20 in the paper; 0 = the MSE term alone);
+ *   dL_dimgs fp32 dev [B,H,W,3], overwritten.  Window moments in double (as the forward).  Asynchronous. */
+int gsr_distortion_backward(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, const double* weight,
+                            double lambda_ssim, float* dL_dimgs, void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------------------
  * gsr_project_backward — the backward of the steps in front of the compositor: activation,
  * deformation Eq. (1), EWA projection and SH colour; DESIGN.md §17.  Takes the
  * per-record gradient gsr_render_backward produced for a frame (same scene, camera and t) to the gradient with

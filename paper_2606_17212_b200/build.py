@@ -16,7 +16,7 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libgsr.so"
-SOURCES = ["gsr_api.cu", "k_project.cu", "k_sort.cu", "k_composite.cu", "k_composite_q.cu", "k_backward.cu", "k_project_backward.cu", "k_dedup.cu", "k_utility.cu", "k_policy.cu", "k_metrics.cu", "k_delivery.cu"]
+SOURCES = ["gsr_api.cu", "k_project.cu", "k_sort.cu", "k_composite.cu", "k_composite_q.cu", "k_backward.cu", "k_project_backward.cu", "k_distortion_backward.cu", "k_dedup.cu", "k_utility.cu", "k_policy.cu", "k_metrics.cu", "k_delivery.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC,-O2,-ffp-contract=off",

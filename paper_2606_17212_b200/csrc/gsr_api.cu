@@ -568,6 +568,21 @@ int gsr_render_backward(const gsr_scene* scene, void* workspace, const float* im
   return GSR_OK;
 }
 
+int gsr_distortion_backward(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, const double* weight,
+                            double lambda_ssim, float* dL_dimgs, void* cuda_stream) {
+  if (B < 0 || H <= 0 || W <= 0 || (B > 0 && (!imgs || !ref || !dL_dimgs)) || !(lambda_ssim >= 0.0) ||
+      3ull * (unsigned long long)W * (unsigned long long)H >= (1ull << 32)) {
+    set_error("gsr_distortion_backward: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  if (launch_distortion_backward(imgs, ref, B, H, W, weight, lambda_ssim, dL_dimgs, (cudaStream_t)cuda_stream) != 0) {
+    set_error("gsr_distortion_backward: shared-memory opt-in failed: %s", cudaGetErrorString(cudaGetLastError()));
+    return GSR_E_CUDA;
+  }
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
 int gsr_project_backward(const gsr_scene* scene, const gsr_camera* cam, float t, const float* grad_records,
                          float* g_gauss, float* g_sh_base, float* g_sh_res, float* g_cluster, void* cuda_stream) {
   if (!scene || !camera_ok(cam) || !g_cluster || (scene->impl.d.N > 0 && (!grad_records || !g_gauss || !g_sh_base || !g_sh_res))) {

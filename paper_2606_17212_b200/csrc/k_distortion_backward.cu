@@ -1,0 +1,170 @@
+// k_distortion_backward.cu — d/d(image) of sum_b weight_b D_b, D = MSE + lambda (1 - SSIM) (the term
+// E_w[D_w] of Eq. (2) with "D = MSE + 0.20(1 - SSIM)"; SSIM per reading G1 of DESIGN.md §12).
+//
+// Per channel, with the 11 x 11 Gaussian window w (zero padding) and m1 = w*x, m2 = w*(x x), m12 = w*(x y):
+//   ssim = N1 N2 / (D1 D2), N1 = 2 mu_x mu_y + C1, N2 = 2 s_xy + C2, D1 = mu_x^2 + mu_y^2 + C1, D2 = s_xx + s_yy + C2
+//   b = d ssim/d m2  = -N1 N2 / (D1 D2^2)
+//   c = d ssim/d m12 = 2 N1 / (D1 D2)
+//   a = d ssim/d m1  = 2 mu_y N2 / (D1 D2) - 2 mu_x N1 N2 / (D1^2 D2) - 2 mu_x b - mu_y c
+//   d mean(ssim)/dx = ( w*a + 2 x w*b + y w*c ) / (3 H W)          (the window is symmetric)
+//   dL/dx = weight_b ( 2 (x - y) / (3 H W) - lambda d mean(ssim)/dx )
+// One CTA per (16 x 16 tile, state): the tile with a halo of 10 pixels is staged, the five moments are blurred on the
+// 26 x 26 tile-plus-5 region, a, b, c are formed there (zero outside the image: no SSIM value exists there) and
+// blurred back onto the tile.  Moments and maps in double, like the forward SSIM (k_metrics.cu): the variance terms
+// cancel against C2 = 9e-4.
+#include "gsr_internal.h"
+
+namespace gsr {
+
+constexpr int kDbR = 5;                    // window radius
+constexpr int kDbIn = kTile + 4 * kDbR;    // 36: staged pixels per side
+constexpr int kDbMid = kTile + 2 * kDbR;   // 26: positions where the SSIM map is needed
+constexpr double kDbC1 = 0.01 * 0.01, kDbC2 = 0.03 * 0.03;
+
+struct DbWindow { double g[2 * kDbR + 1]; };
+
+struct DbSmem {
+  float x[kDbIn][kDbIn + 1], y[kDbIn][kDbIn + 1];
+  double h[5][kDbIn][kDbMid + 1];   // moments blurred along x; reused for the maps blurred along x: [3][kDbMid][kTile + 1]
+  double m[3][kDbMid][kDbMid + 1];  // a, b, c
+};
+
+__global__ void __launch_bounds__(kTilePix) k_distortion_backward(const float* __restrict__ imgs,
+                                                                  const float* __restrict__ ref, int W, int H, int TX,
+                                                                  const double* __restrict__ weight, double lambda,
+                                                                  DbWindow win, float* __restrict__ out) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  DbSmem& s = *reinterpret_cast<DbSmem*>(smem_raw);
+  double(*gx)[kDbMid][kTile + 1] = reinterpret_cast<double(*)[kDbMid][kTile + 1]>(&s.h[0][0][0]);
+  const int tid = threadIdx.x, tile = blockIdx.x, b = blockIdx.y;
+  const int x0 = (tile % TX) * kTile, y0 = (tile / TX) * kTile;
+  const size_t img = (size_t)H * W * 3;
+  const float* im = imgs + (size_t)b * img;
+  const double wb = weight ? weight[b] : 1.0;
+  const double inv_n = 1.0 / (3.0 * (double)W * (double)H);
+  const int ty = tid / kTile, tx = tid % kTile;
+  const int px = x0 + tx, py = y0 + ty;
+  for (int ch = 0; ch < 3; ++ch) {
+    // A. stage the tile and its halo of 10 (zero outside the image)
+    for (int i = tid; i < kDbIn * kDbIn; i += kTilePix) {
+      const int hy = i / kDbIn, hx = i - hy * kDbIn;
+      const int qx = x0 + hx - 2 * kDbR, qy = y0 + hy - 2 * kDbR;
+      float vx = 0.0f, vy = 0.0f;
+      if (qx >= 0 && qx < W && qy >= 0 && qy < H) {
+        const size_t o = ((size_t)qy * W + qx) * 3 + ch;
+        vx = __ldg(im + o);
+        vy = __ldg(ref + o);
+      }
+      s.x[hy][hx] = vx;
+      s.y[hy][hx] = vy;
+    }
+    __syncthreads();
+    // B. the five moments blurred along x: rows 0..35, columns 0..25 (column c is staged column c + 5)
+    for (int i = tid; i < kDbIn * kDbMid; i += kTilePix) {
+      const int r = i / kDbMid, c = i - r * kDbMid;
+      double a0 = 0, a1 = 0, a2 = 0, a3 = 0, a4 = 0;
+#pragma unroll
+      for (int k = 0; k <= 2 * kDbR; ++k) {
+        const double xv = (double)s.x[r][c + k], yv = (double)s.y[r][c + k], g = win.g[k];
+        a0 += g * xv; a1 += g * yv; a2 += g * (xv * xv); a3 += g * (yv * yv); a4 += g * (xv * yv);
+      }
+      s.h[0][r][c] = a0; s.h[1][r][c] = a1; s.h[2][r][c] = a2; s.h[3][r][c] = a3; s.h[4][r][c] = a4;
+    }
+    __syncthreads();
+    // C. along y, then a, b, c at the 26 x 26 positions (row r is staged row r + 5)
+    for (int i = tid; i < kDbMid * kDbMid; i += kTilePix) {
+      const int r = i / kDbMid, c = i - r * kDbMid;
+      const int qx = x0 + c - kDbR, qy = y0 + r - kDbR;
+      double va = 0.0, vb = 0.0, vc = 0.0;
+      if (qx >= 0 && qx < W && qy >= 0 && qy < H) {
+        double m0 = 0, m1 = 0, m2 = 0, m3 = 0, m4 = 0;
+#pragma unroll
+        for (int k = 0; k <= 2 * kDbR; ++k) {
+          const double g = win.g[k];
+          m0 += g * s.h[0][r + k][c]; m1 += g * s.h[1][r + k][c]; m2 += g * s.h[2][r + k][c];
+          m3 += g * s.h[3][r + k][c]; m4 += g * s.h[4][r + k][c];
+        }
+        const double mx = m0, my = m1, sxx = m2 - mx * mx, syy = m3 - my * my, sxy = m4 - mx * my;
+        const double N1 = 2.0 * mx * my + kDbC1, N2 = 2.0 * sxy + kDbC2;
+        const double D1 = mx * mx + my * my + kDbC1, D2 = sxx + syy + kDbC2;
+        const double r12 = 1.0 / (D1 * D2);
+        vb = -N1 * N2 * r12 / D2;
+        vc = 2.0 * N1 * r12;
+        va = 2.0 * my * N2 * r12 - 2.0 * mx * N1 * N2 * r12 / D1 - 2.0 * mx * vb - my * vc;
+      }
+      s.m[0][r][c] = va; s.m[1][r][c] = vb; s.m[2][r][c] = vc;
+    }
+    __syncthreads();
+    // D. the maps blurred along x: rows 0..25, tile columns 0..15 (tile column c is map column c + 5)
+    for (int i = tid; i < kDbMid * kTile; i += kTilePix) {
+      const int r = i / kTile, c = i - r * kTile;
+      double a0 = 0, a1 = 0, a2 = 0;
+#pragma unroll
+      for (int k = 0; k <= 2 * kDbR; ++k) {
+        const double g = win.g[k];
+        a0 += g * s.m[0][r][c + k]; a1 += g * s.m[1][r][c + k]; a2 += g * s.m[2][r][c + k];
+      }
+      gx[0][r][c] = a0; gx[1][r][c] = a1; gx[2][r][c] = a2;
+    }
+    __syncthreads();
+    // E. along y and the pixel's gradient
+    if (px < W && py < H) {
+      double a0 = 0, a1 = 0, a2 = 0;
+#pragma unroll
+      for (int k = 0; k <= 2 * kDbR; ++k) {
+        const double g = win.g[k];
+        a0 += g * gx[0][ty + k][tx]; a1 += g * gx[1][ty + k][tx]; a2 += g * gx[2][ty + k][tx];
+      }
+      const double xv = (double)s.x[ty + 2 * kDbR][tx + 2 * kDbR], yv = (double)s.y[ty + 2 * kDbR][tx + 2 * kDbR];
+      const double dssim = (a0 + 2.0 * xv * a1 + yv * a2) * inv_n;
+      out[(size_t)b * img + ((size_t)py * W + px) * 3 + ch] = (float)(wb * (2.0 * (xv - yv) * inv_n - lambda * dssim));
+    }
+    __syncthreads();  // the staging buffers are rewritten for the next channel
+  }
+}
+
+// lambda == 0: the MSE term alone, no window
+__global__ void k_mse_backward(const float* __restrict__ imgs, const float* __restrict__ ref, size_t img, int B,
+                               const double* __restrict__ weight, float* __restrict__ out) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int b = blockIdx.y;
+  if (i >= img) return;
+  const double wb = weight ? weight[b] : 1.0;
+  out[(size_t)b * img + i] = (float)(wb * 2.0 * ((double)imgs[(size_t)b * img + i] - (double)ref[i]) / (double)img);
+}
+
+int launch_distortion_backward(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W,
+                               const double* weight, double lambda, float* out, cudaStream_t st) {
+  if (B == 0) return 0;
+  const size_t img = (size_t)H * W * 3;
+  if (lambda == 0.0) {
+    for (int b0 = 0; b0 < B; b0 += 65535) {
+      const int nb = B - b0 < 65535 ? B - b0 : 65535;
+      k_mse_backward<<<dim3((unsigned)((img + 255) / 256), nb), 256, 0, st>>>(imgs + (size_t)b0 * img, ref, img, nb,
+                                                                             weight ? weight + b0 : nullptr,
+                                                                             out + (size_t)b0 * img);
+      count_launches(1);
+    }
+    return 0;
+  }
+  DbWindow win;
+  double g[2 * kDbR + 1], sum = 0.0;
+  for (int k = 0; k <= 2 * kDbR; ++k) {  // exp(-(k-5)^2 / (2 * 1.5^2)), normalised
+    g[k] = exp(-(double)((k - kDbR) * (k - kDbR)) / (2.0 * 1.5 * 1.5));
+    sum += g[k];
+  }
+  for (int k = 0; k <= 2 * kDbR; ++k) win.g[k] = g[k] / sum;
+  const int TX = (W + kTile - 1) / kTile, TY = (H + kTile - 1) / kTile;
+  if (cudaFuncSetAttribute(k_distortion_backward, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(DbSmem)) !=
+      cudaSuccess)
+    return -1;
+  for (int b0 = 0; b0 < B; b0 += 65535) {
+    const int nb = B - b0 < 65535 ? B - b0 : 65535;
+    k_distortion_backward<<<dim3(TX * TY, nb), kTilePix, sizeof(DbSmem), st>>>(
+        imgs + (size_t)b0 * img, ref, W, H, TX, weight ? weight + b0 : nullptr, lambda, win, out + (size_t)b0 * img);
+    count_launches(1);
+  }
+  return 0;
+}
+
+}  // namespace gsr

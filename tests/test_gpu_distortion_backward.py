@@ -1,0 +1,155 @@
+"""GPU parity of gsr_distortion_backward (include/gsr.h) against oracle/metrics.py distortion_backward,
+and the whole gradient chain objective -> images -> records -> scene parameters against central differences of the
+GPU's own forward objective."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+from oracle import metrics as M
+from paper_2606_17212_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_mod():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+@pytest.fixture(scope="module")
+def gsr(torch_mod):
+    from paper_2606_17212_b200 import gsr as G
+    G.lib()
+    return G
+
+
+def _images(seed, B, H, W):
+    rng = np.random.default_rng(seed)
+    yy, xx = np.mgrid[0:H, 0:W]
+    ref = np.stack([0.5 + 0.4 * np.sin(0.3 * xx + 0.2 * yy + k) for k in range(3)], -1).astype(np.float32)
+    imgs = np.clip(ref[None] + 0.08 * rng.standard_normal((B, H, W, 3)), 0.0, 1.0).astype(np.float32)
+    return imgs, ref
+
+
+@pytest.mark.parametrize("H,W", [(37, 53), (16, 16), (4, 7), (64, 33)])
+def test_against_the_oracle(gsr, torch_mod, H, W):
+    """Sizes with ragged tiles, one exact tile, an image smaller than the window; weights incl. 0; lambda 0.2, 1, 0.
+    Double moments on both sides, fp32 output: 2e-6 of the largest entry."""
+    torch = torch_mod
+    imgs, ref = _images(H * 100 + W, 3, H, W)
+    w = np.array([0.7, 0.0, 1.9])
+    di, dr, dw = torch.from_numpy(imgs).cuda(), torch.from_numpy(ref).cuda(), torch.from_numpy(w).cuda()
+    for lam in (0.20, 1.0, 0.0):
+        got = gsr.distortion_backward(di, dr, dw, lam).cpu().numpy().astype(np.float64)
+        want = M.distortion_backward(imgs, ref, w, lam)
+        assert np.abs(got - want).max() <= 2e-6 * np.abs(want).max(), (lam, np.abs(got - want).max(), np.abs(want).max())
+        assert np.all(got[1] == 0.0)
+    got = gsr.distortion_backward(di, dr, None, 0.20).cpu().numpy().astype(np.float64)
+    want = M.distortion_backward(imgs, ref, np.ones(3), 0.20)
+    assert np.abs(got - want).max() <= 2e-6 * np.abs(want).max()
+    # at the reference itself the gradient vanishes
+    z = gsr.distortion_backward(dr[None].contiguous(), dr, None, 0.20)
+    assert float(z.abs().max()) <= 1e-9
+
+
+def test_full_size_sampled_pixels_and_directional_derivative(gsr, torch_mod):
+    """800 x 800, 8 states (the resolution bench.py times): (1) the directional derivative of the GPU's own forward
+    D = MSE + 0.2 (1 - SSIM) (gsr_distortion / gsr_distortion_ssim, double sums) along a random direction equals
+    <gradient, direction>; (2) a 64 x 64 crop far from the border is an image of its own for the 21 x 21 support of the
+    gradient at its centre: the centre pixels against the oracle on the crop, rescaled by the pixel counts."""
+    torch = torch_mod
+    H = W = 800
+    B = 8
+    gen = torch.Generator(device="cuda").manual_seed(5)
+    yy, xx = torch.meshgrid(torch.arange(H, device="cuda"), torch.arange(W, device="cuda"), indexing="ij")
+    ref = torch.stack([0.5 + 0.4 * torch.sin(0.03 * xx + 0.02 * yy + k) for k in range(3)], -1).float().contiguous()
+    imgs = (ref[None] + 0.05 * torch.randn((B, H, W, 3), generator=gen, device="cuda")).clamp(0, 1).float().contiguous()
+    w = torch.full((B,), 1.0 / B, dtype=torch.float64, device="cuda")
+    g = gsr.distortion_backward(imgs, ref, w, 0.20)
+
+    def D(im):
+        mse, _ = gsr.distortion(im, ref)
+        _, dmix = gsr.distortion_ssim(im, ref, mse=mse)
+        return float((w * dmix).sum())
+
+    # along the gradient itself (plus noise): a random direction in 15 M dimensions gives a derivative that is a
+    # cancelling sum, below the differences' own noise
+    u = g / g.abs().max() + 0.1 * torch.randn(imgs.shape, generator=gen, device="cuda")
+    h = 1e-3                                                   # fp32 images: the step must survive their rounding
+    ip, im_ = (imgs + h * u).float(), (imgs - h * u).float()
+    fd = D(ip) - D(im_)
+    pred = float((g.double() * (ip.double() - im_.double())).sum())
+    assert abs(fd - pred) <= 2e-4 * abs(pred) + 1e-12, (fd, pred)
+    # (2)
+    y0, x0 = 300, 420
+    crop = imgs[2:3, y0:y0 + 64, x0:x0 + 64].cpu().numpy()
+    want = M.distortion_backward(crop, ref[y0:y0 + 64, x0:x0 + 64].cpu().numpy(), np.ones(1), 0.20)[0]
+    got = g[2, y0:y0 + 64, x0:x0 + 64].double().cpu().numpy() * B * (H * W) / (64 * 64)
+    c = slice(22, 42)                                          # 10 + 10 pixels from the crop's border and more
+    assert np.abs(got[c, c] - want[c, c]).max() <= 5e-6 * np.abs(want[c, c]).max()
+
+
+def test_objective_to_parameters_against_differences_of_the_gpu_forward(gsr, torch_mod):
+    """L = mean_b D_b, D = MSE + 0.2 (1 - SSIM) against the full-state render: gsr_distortion_backward ->
+    gsr_render_backward -> gsr_project_backward, compared with (L(theta + h u) - L(theta - h u)) where L is evaluated
+    by the FORWARD calls alone (render, gsr_distortion, gsr_distortion_ssim) on perturbed scenes.  The reference
+    image is held fixed (it is a target, not a function of the parameters)."""
+    torch = torch_mod
+    wl = synth.scaled_object_workload(61, C=3, per_cluster=150.0, W=96, H=80, fov=40.0, n_frames=1, B=6)
+    cam, t = wl.frames[0]
+    scn = wl.scene
+    lv = wl.levels[0].copy()
+    lv[0] = 3
+    dlv = torch.from_numpy(np.ascontiguousarray(lv, np.int8)).cuda()
+    B = lv.shape[0]
+    w = torch.full((B,), 1.0 / B, dtype=torch.float64, device="cuda")
+    rng = np.random.default_rng(61)
+    # the target: the full-state render of a scene with perturbed colours and positions (so that D > 0 at full state)
+    tgt_scn = dataclasses.replace(scn, mean=(scn.mean + 0.01 * rng.standard_normal(scn.mean.shape)).astype(np.float32),
+                                  sh_base=(scn.sh_base + 0.05 * rng.standard_normal(scn.sh_base.shape)).astype(np.float32))
+    s0 = gsr.Scene(tgt_scn)
+    full = torch.full((1, scn.C), 3, dtype=torch.int8, device="cuda")
+    ref = s0.render_states(cam, t, full)[0][0].contiguous()
+    s0.close()
+
+    def objective(sc_np):
+        s = gsr.Scene(sc_np)
+        ws = s.new_workspace(cam, B)
+        out, _, _ = s.render_states(cam, t, dlv, workspace=ws)
+        mse, _ = gsr.distortion(out, ref)
+        _, dmix = gsr.distortion_ssim(out, ref, mse=mse)
+        return float((w * dmix).sum()), s, ws, out
+
+    L0, scene, ws, out = objective(scn)
+    gimg = gsr.distortion_backward(out, ref, w, 0.20)
+    grec = scene.render_backward(ws, out, gimg)
+    gp = scene.project_backward(cam, t, grec)
+    gg = gp["gauss"].double().cpu().numpy()
+    grads = {"mean": gg[:, 0:3], "log_scale": gg[:, 6:9], "quat": gg[:, 9:13], "opacity_logit": gg[:, 13],
+             "sh_base": gp["sh_base"].double().cpu().numpy(), "sh_res": gp["sh_res"].double().cpu().numpy()}
+    scene.close()
+    for field, h in (("mean", 2e-3), ("log_scale", 1e-2), ("quat", 1e-2), ("opacity_logit", 2e-2), ("sh_base", 1e-2),
+                     ("sh_res", 2e-2)):
+        theta = np.asarray(getattr(scn, field), np.float32)
+        u = rng.standard_normal(theta.shape)
+        if field == "mean":
+            # parallel to the image plane: a step along the viewing axis swaps the depth order of neighbouring
+            # Gaussians (their depths are ~4e-3 apart), at which the composite jumps — the sort is a constant of the
+            # differentiation, so that direction is not one along which differences test the gradient
+            Rw = np.asarray(cam.R_wc, np.float64).reshape(3, 3)
+            u = rng.standard_normal((scn.N, 1)) * Rw[0] + rng.standard_normal((scn.N, 1)) * Rw[1]
+        tp = (theta.astype(np.float64) + h * u).astype(np.float32)
+        tm = (theta.astype(np.float64) - h * u).astype(np.float32)
+        Lp, s1, _, _ = objective(dataclasses.replace(scn, **{field: tp}))
+        s1.close()
+        Lm, s2, _, _ = objective(dataclasses.replace(scn, **{field: tm}))
+        s2.close()
+        delta = tp.astype(np.float64) - tm.astype(np.float64)
+        pred = float((grads[field].reshape(theta.shape) * delta).sum())
+        mag = float(np.abs(grads[field].reshape(theta.shape) * delta).sum())
+        # the image is piecewise smooth in the parameters (tile rectangles, cut, cap, stop, depth order are discrete):
+        # finite steps cross a few of those, hence a percent-level bar; a wrong chain is off by O(1)
+        assert abs((Lp - Lm) - pred) <= 3e-2 * mag + 2e-2 * abs(pred), (field, Lp - Lm, pred, mag)
