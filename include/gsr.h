@@ -181,9 +181,12 @@ int gsr_render_backward(const gsr_scene* scene, void* workspace, const float* im
  * gsr_distortion_ssim): the dL_dimages input of gsr_render_backward for that objective.
  *   imgs fp32 dev [B,H,W,3]; ref fp32 dev [H,W,3]; weight double dev [B] or NULL (= 1 for every state; pass 1/B for
  *   the mean over states); lambda_ssim >= 0 (0.20 in the paper; 0 = the MSE term alone);
- *   dL_dimgs fp32 dev [B,H,W,3], overwritten.  Window moments in double (as the forward).  Asynchronous. */
+ *   dL_dimgs fp32 dev [B,H,W,3], overwritten.  workspace dev, >= gsr_distortion_backward_workspace_bytes(H, W), 256-byte
+ *   aligned (the window moments of the reference, computed once per call; may be NULL when lambda_ssim == 0; else
+ *   GSR_E_WORKSPACE_TOO_SMALL).  Window moments in double (as the forward).  Asynchronous. */
+size_t gsr_distortion_backward_workspace_bytes(int32_t H, int32_t W);
 int gsr_distortion_backward(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, const double* weight,
-                            double lambda_ssim, float* dL_dimgs, void* cuda_stream);
+                            double lambda_ssim, float* dL_dimgs, void* workspace, size_t ws_bytes, void* cuda_stream);
 
 /* ------------------------------------------------------------------------------------------------
  * gsr_project_backward — the backward of the steps in front of the compositor: activation,

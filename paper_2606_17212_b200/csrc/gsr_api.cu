@@ -568,14 +568,24 @@ int gsr_render_backward(const gsr_scene* scene, void* workspace, const float* im
   return GSR_OK;
 }
 
+size_t gsr_distortion_backward_workspace_bytes(int32_t H, int32_t W) {
+  if (H <= 0 || W <= 0) return 0;
+  return align_up(sizeof(double) * 2 * 3 * (size_t)H * (size_t)W);
+}
+
 int gsr_distortion_backward(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, const double* weight,
-                            double lambda_ssim, float* dL_dimgs, void* cuda_stream) {
+                            double lambda_ssim, float* dL_dimgs, void* workspace, size_t ws_bytes, void* cuda_stream) {
   if (B < 0 || H <= 0 || W <= 0 || (B > 0 && (!imgs || !ref || !dL_dimgs)) || !(lambda_ssim >= 0.0) ||
       3ull * (unsigned long long)W * (unsigned long long)H >= (1ull << 32)) {
     set_error("gsr_distortion_backward: invalid argument");
     return GSR_E_INVALID_ARG;
   }
-  if (launch_distortion_backward(imgs, ref, B, H, W, weight, lambda_ssim, dL_dimgs, (cudaStream_t)cuda_stream) != 0) {
+  if (lambda_ssim > 0.0 && B > 0 && (!workspace || ws_bytes < gsr_distortion_backward_workspace_bytes(H, W))) {
+    set_error("gsr_distortion_backward: workspace too small (needs %zu bytes)", gsr_distortion_backward_workspace_bytes(H, W));
+    return GSR_E_WORKSPACE_TOO_SMALL;
+  }
+  if (launch_distortion_backward(imgs, ref, B, H, W, weight, lambda_ssim, dL_dimgs, (double*)workspace,
+                                 (cudaStream_t)cuda_stream) != 0) {
     set_error("gsr_distortion_backward: shared-memory opt-in failed: %s", cudaGetErrorString(cudaGetLastError()));
     return GSR_E_CUDA;
   }

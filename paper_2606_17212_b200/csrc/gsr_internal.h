@@ -172,7 +172,7 @@ struct CompositeArgs;
 void launch_composite_q(const CompositeArgs& a, int S, bool count, cudaStream_t st);
 // backward of a4 (k_backward.cu): grad [records, 12], zeroed by the call
 int launch_distortion_backward(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W,
-                               const double* weight, double lambda, float* out, cudaStream_t st);
+                               const double* weight, double lambda, float* out, double* ref_planes, cudaStream_t st);
 void launch_project_backward(const DeviceScene& sc, const FrameParams& fp, const float* grad_rec, float* g_gauss,
                              float* g_shb, float* g_shr, float* g_cluster, cudaStream_t st);
 void launch_backward(const DeviceScene& sc, const WsHeader& h, Workspace& ws, const float* images, const float* gimg,

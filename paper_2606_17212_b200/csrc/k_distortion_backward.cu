@@ -8,45 +8,90 @@
 //   a = d ssim/d m1  = 2 mu_y N2 / (D1 D2) - 2 mu_x N1 N2 / (D1^2 D2) - 2 mu_x b - mu_y c
 //   d mean(ssim)/dx = ( w*a + 2 x w*b + y w*c ) / (3 H W)          (the window is symmetric)
 //   dL/dx = weight_b ( 2 (x - y) / (3 H W) - lambda d mean(ssim)/dx )
-// One CTA per (16 x 16 tile, state): the tile with a halo of 10 pixels is staged, the five moments are blurred on the
-// 26 x 26 tile-plus-5 region, a, b, c are formed there (zero outside the image: no SSIM value exists there) and
-// blurred back onto the tile.  Moments and maps in double, like the forward SSIM (k_metrics.cu): the variance terms
-// cancel against C2 = 9e-4.
+// One CTA per (32 x 32 block of pixels, state): the block with a halo of 10 pixels is staged, the three moments that
+// depend on the image are blurred on the block-plus-5 region (42 x 42), a, b, c are formed there (zero outside the
+// image: no SSIM value exists there) and blurred back onto the block.  The two moments of the reference alone
+// (mu_y, w*(y y)) do not depend on the state: k_ref_moments computes them once per call into the workspace.
+// Moments and maps in double, like the forward SSIM (k_metrics.cu): the variance terms cancel against C2 = 9e-4.
 #include "gsr_internal.h"
 
 namespace gsr {
 
 constexpr int kDbR = 5;                    // window radius
-constexpr int kDbIn = kTile + 4 * kDbR;    // 36: staged pixels per side
-constexpr int kDbMid = kTile + 2 * kDbR;   // 26: positions where the SSIM map is needed
+constexpr int kDbT = 32;                   // block edge
+constexpr int kDbIn = kDbT + 4 * kDbR;     // 52: staged pixels per side
+constexpr int kDbMid = kDbT + 2 * kDbR;    // 42: positions where the SSIM map is needed
+constexpr int kDbThreads = 512;
 constexpr double kDbC1 = 0.01 * 0.01, kDbC2 = 0.03 * 0.03;
 
 struct DbWindow { double g[2 * kDbR + 1]; };
 
 struct DbSmem {
   float x[kDbIn][kDbIn + 1], y[kDbIn][kDbIn + 1];
-  double h[5][kDbIn][kDbMid + 1];   // moments blurred along x; reused for the maps blurred along x: [3][kDbMid][kTile + 1]
+  double h[3][kDbIn][kDbMid + 1];   // x, x x, x y blurred along x; reused for the maps blurred along x: [3][kDbMid][kDbT + 1]
   double m[3][kDbMid][kDbMid + 1];  // a, b, c
 };
 
-__global__ void __launch_bounds__(kTilePix) k_distortion_backward(const float* __restrict__ imgs,
-                                                                  const float* __restrict__ ref, int W, int H, int TX,
-                                                                  const double* __restrict__ weight, double lambda,
-                                                                  DbWindow win, float* __restrict__ out) {
+// mu_y = w*y and w*(y y) of the reference, double [H, W, 3] each (the image layout), zero padding
+__global__ void __launch_bounds__(kTilePix) k_ref_moments(const float* __restrict__ ref, int W, int H, int TX,
+                                                          DbWindow win, double* __restrict__ my,
+                                                          double* __restrict__ eyy) {
+  constexpr int kHalo = kTile + 2 * kDbR;  // 26
+  __shared__ float s_y[kHalo][kHalo + 1];
+  __shared__ double s_h[2][kHalo][kTile + 1];
+  const int tid = threadIdx.x, tile = blockIdx.x;
+  const int x0 = (tile % TX) * kTile, y0 = (tile / TX) * kTile;
+  const int ty = tid / kTile, tx = tid % kTile;
+  for (int ch = 0; ch < 3; ++ch) {
+    for (int i = tid; i < kHalo * kHalo; i += kTilePix) {
+      const int hy = i / kHalo, hx = i - hy * kHalo;
+      const int qx = x0 + hx - kDbR, qy = y0 + hy - kDbR;
+      s_y[hy][hx] = (qx >= 0 && qx < W && qy >= 0 && qy < H) ? __ldg(ref + ((size_t)qy * W + qx) * 3 + ch) : 0.0f;
+    }
+    __syncthreads();
+    for (int i = tid; i < kHalo * kTile; i += kTilePix) {
+      const int r = i / kTile, c = i - r * kTile;
+      double a0 = 0, a1 = 0;
+#pragma unroll
+      for (int k = 0; k <= 2 * kDbR; ++k) {
+        const double yv = (double)s_y[r][c + k], g = win.g[k];
+        a0 += g * yv; a1 += g * (yv * yv);
+      }
+      s_h[0][r][c] = a0; s_h[1][r][c] = a1;
+    }
+    __syncthreads();
+    if (x0 + tx < W && y0 + ty < H) {
+      double a0 = 0, a1 = 0;
+#pragma unroll
+      for (int k = 0; k <= 2 * kDbR; ++k) {
+        a0 += win.g[k] * s_h[0][ty + k][tx]; a1 += win.g[k] * s_h[1][ty + k][tx];
+      }
+      const size_t o = ((size_t)(y0 + ty) * W + (x0 + tx)) * 3 + ch;
+      my[o] = a0;
+      eyy[o] = a1;
+    }
+    __syncthreads();
+  }
+}
+
+__global__ void __launch_bounds__(kDbThreads) k_distortion_backward(const float* __restrict__ imgs,
+                                                                    const float* __restrict__ ref, int W, int H, int TX,
+                                                                    const double* __restrict__ ref_my,
+                                                                    const double* __restrict__ ref_eyy,
+                                                                    const double* __restrict__ weight, double lambda,
+                                                                    DbWindow win, float* __restrict__ out) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   DbSmem& s = *reinterpret_cast<DbSmem*>(smem_raw);
-  double(*gx)[kDbMid][kTile + 1] = reinterpret_cast<double(*)[kDbMid][kTile + 1]>(&s.h[0][0][0]);
+  double(*gx)[kDbMid][kDbT + 1] = reinterpret_cast<double(*)[kDbMid][kDbT + 1]>(&s.h[0][0][0]);
   const int tid = threadIdx.x, tile = blockIdx.x, b = blockIdx.y;
-  const int x0 = (tile % TX) * kTile, y0 = (tile / TX) * kTile;
+  const int x0 = (tile % TX) * kDbT, y0 = (tile / TX) * kDbT;
   const size_t img = (size_t)H * W * 3;
   const float* im = imgs + (size_t)b * img;
   const double wb = weight ? weight[b] : 1.0;
   const double inv_n = 1.0 / (3.0 * (double)W * (double)H);
-  const int ty = tid / kTile, tx = tid % kTile;
-  const int px = x0 + tx, py = y0 + ty;
   for (int ch = 0; ch < 3; ++ch) {
-    // A. stage the tile and its halo of 10 (zero outside the image)
-    for (int i = tid; i < kDbIn * kDbIn; i += kTilePix) {
+    // A. stage the block and its halo of 10 (zero outside the image)
+    for (int i = tid; i < kDbIn * kDbIn; i += kDbThreads) {
       const int hy = i / kDbIn, hx = i - hy * kDbIn;
       const int qx = x0 + hx - 2 * kDbR, qy = y0 + hy - 2 * kDbR;
       float vx = 0.0f, vy = 0.0f;
@@ -59,32 +104,32 @@ __global__ void __launch_bounds__(kTilePix) k_distortion_backward(const float* _
       s.y[hy][hx] = vy;
     }
     __syncthreads();
-    // B. the five moments blurred along x: rows 0..35, columns 0..25 (column c is staged column c + 5)
-    for (int i = tid; i < kDbIn * kDbMid; i += kTilePix) {
+    // B. x, x x, x y blurred along x: rows 0..51, columns 0..41 (column c is staged column c + 5)
+    for (int i = tid; i < kDbIn * kDbMid; i += kDbThreads) {
       const int r = i / kDbMid, c = i - r * kDbMid;
-      double a0 = 0, a1 = 0, a2 = 0, a3 = 0, a4 = 0;
+      double a0 = 0, a2 = 0, a4 = 0;
 #pragma unroll
       for (int k = 0; k <= 2 * kDbR; ++k) {
         const double xv = (double)s.x[r][c + k], yv = (double)s.y[r][c + k], g = win.g[k];
-        a0 += g * xv; a1 += g * yv; a2 += g * (xv * xv); a3 += g * (yv * yv); a4 += g * (xv * yv);
+        a0 += g * xv; a2 += g * (xv * xv); a4 += g * (xv * yv);
       }
-      s.h[0][r][c] = a0; s.h[1][r][c] = a1; s.h[2][r][c] = a2; s.h[3][r][c] = a3; s.h[4][r][c] = a4;
+      s.h[0][r][c] = a0; s.h[1][r][c] = a2; s.h[2][r][c] = a4;
     }
     __syncthreads();
-    // C. along y, then a, b, c at the 26 x 26 positions (row r is staged row r + 5)
-    for (int i = tid; i < kDbMid * kDbMid; i += kTilePix) {
+    // C. along y, then a, b, c at the 42 x 42 positions (row r is staged row r + 5)
+    for (int i = tid; i < kDbMid * kDbMid; i += kDbThreads) {
       const int r = i / kDbMid, c = i - r * kDbMid;
       const int qx = x0 + c - kDbR, qy = y0 + r - kDbR;
       double va = 0.0, vb = 0.0, vc = 0.0;
       if (qx >= 0 && qx < W && qy >= 0 && qy < H) {
-        double m0 = 0, m1 = 0, m2 = 0, m3 = 0, m4 = 0;
+        double m0 = 0, m2 = 0, m4 = 0;
 #pragma unroll
         for (int k = 0; k <= 2 * kDbR; ++k) {
           const double g = win.g[k];
-          m0 += g * s.h[0][r + k][c]; m1 += g * s.h[1][r + k][c]; m2 += g * s.h[2][r + k][c];
-          m3 += g * s.h[3][r + k][c]; m4 += g * s.h[4][r + k][c];
+          m0 += g * s.h[0][r + k][c]; m2 += g * s.h[1][r + k][c]; m4 += g * s.h[2][r + k][c];
         }
-        const double mx = m0, my = m1, sxx = m2 - mx * mx, syy = m3 - my * my, sxy = m4 - mx * my;
+        const size_t o = ((size_t)qy * W + qx) * 3 + ch;
+        const double mx = m0, my = ref_my[o], sxx = m2 - mx * mx, syy = ref_eyy[o] - my * my, sxy = m4 - mx * my;
         const double N1 = 2.0 * mx * my + kDbC1, N2 = 2.0 * sxy + kDbC2;
         const double D1 = mx * mx + my * my + kDbC1, D2 = sxx + syy + kDbC2;
         const double r12 = 1.0 / (D1 * D2);
@@ -95,9 +140,9 @@ __global__ void __launch_bounds__(kTilePix) k_distortion_backward(const float* _
       s.m[0][r][c] = va; s.m[1][r][c] = vb; s.m[2][r][c] = vc;
     }
     __syncthreads();
-    // D. the maps blurred along x: rows 0..25, tile columns 0..15 (tile column c is map column c + 5)
-    for (int i = tid; i < kDbMid * kTile; i += kTilePix) {
-      const int r = i / kTile, c = i - r * kTile;
+    // D. the maps blurred along x: rows 0..41, block columns 0..31 (block column c is map column c + 5)
+    for (int i = tid; i < kDbMid * kDbT; i += kDbThreads) {
+      const int r = i / kDbT, c = i - r * kDbT;
       double a0 = 0, a1 = 0, a2 = 0;
 #pragma unroll
       for (int k = 0; k <= 2 * kDbR; ++k) {
@@ -108,16 +153,20 @@ __global__ void __launch_bounds__(kTilePix) k_distortion_backward(const float* _
     }
     __syncthreads();
     // E. along y and the pixel's gradient
-    if (px < W && py < H) {
-      double a0 = 0, a1 = 0, a2 = 0;
+    for (int i = tid; i < kDbT * kDbT; i += kDbThreads) {
+      const int ty = i / kDbT, tx = i - ty * kDbT;
+      const int px = x0 + tx, py = y0 + ty;
+      if (px < W && py < H) {
+        double a0 = 0, a1 = 0, a2 = 0;
 #pragma unroll
-      for (int k = 0; k <= 2 * kDbR; ++k) {
-        const double g = win.g[k];
-        a0 += g * gx[0][ty + k][tx]; a1 += g * gx[1][ty + k][tx]; a2 += g * gx[2][ty + k][tx];
+        for (int k = 0; k <= 2 * kDbR; ++k) {
+          const double g = win.g[k];
+          a0 += g * gx[0][ty + k][tx]; a1 += g * gx[1][ty + k][tx]; a2 += g * gx[2][ty + k][tx];
+        }
+        const double xv = (double)s.x[ty + 2 * kDbR][tx + 2 * kDbR], yv = (double)s.y[ty + 2 * kDbR][tx + 2 * kDbR];
+        const double dssim = (a0 + 2.0 * xv * a1 + yv * a2) * inv_n;
+        out[(size_t)b * img + ((size_t)py * W + px) * 3 + ch] = (float)(wb * (2.0 * (xv - yv) * inv_n - lambda * dssim));
       }
-      const double xv = (double)s.x[ty + 2 * kDbR][tx + 2 * kDbR], yv = (double)s.y[ty + 2 * kDbR][tx + 2 * kDbR];
-      const double dssim = (a0 + 2.0 * xv * a1 + yv * a2) * inv_n;
-      out[(size_t)b * img + ((size_t)py * W + px) * 3 + ch] = (float)(wb * (2.0 * (xv - yv) * inv_n - lambda * dssim));
     }
     __syncthreads();  // the staging buffers are rewritten for the next channel
   }
@@ -134,7 +183,7 @@ __global__ void k_mse_backward(const float* __restrict__ imgs, const float* __re
 }
 
 int launch_distortion_backward(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W,
-                               const double* weight, double lambda, float* out, cudaStream_t st) {
+                               const double* weight, double lambda, float* out, double* ref_planes, cudaStream_t st) {
   if (B == 0) return 0;
   const size_t img = (size_t)H * W * 3;
   if (lambda == 0.0) {
@@ -154,14 +203,20 @@ int launch_distortion_backward(const float* imgs, const float* ref, int32_t B, i
     sum += g[k];
   }
   for (int k = 0; k <= 2 * kDbR; ++k) win.g[k] = g[k] / sum;
-  const int TX = (W + kTile - 1) / kTile, TY = (H + kTile - 1) / kTile;
   if (cudaFuncSetAttribute(k_distortion_backward, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(DbSmem)) !=
       cudaSuccess)
     return -1;
+  double* my = ref_planes;
+  double* eyy = ref_planes + img;
+  const int TX16 = (W + kTile - 1) / kTile, TY16 = (H + kTile - 1) / kTile;
+  k_ref_moments<<<TX16 * TY16, kTilePix, 0, st>>>(ref, W, H, TX16, win, my, eyy);
+  count_launches(1);
+  const int TX = (W + kDbT - 1) / kDbT, TY = (H + kDbT - 1) / kDbT;
   for (int b0 = 0; b0 < B; b0 += 65535) {
     const int nb = B - b0 < 65535 ? B - b0 : 65535;
-    k_distortion_backward<<<dim3(TX * TY, nb), kTilePix, sizeof(DbSmem), st>>>(
-        imgs + (size_t)b0 * img, ref, W, H, TX, weight ? weight + b0 : nullptr, lambda, win, out + (size_t)b0 * img);
+    k_distortion_backward<<<dim3(TX * TY, nb), kDbThreads, sizeof(DbSmem), st>>>(
+        imgs + (size_t)b0 * img, ref, W, H, TX, my, eyy, weight ? weight + b0 : nullptr, lambda, win,
+        out + (size_t)b0 * img);
     count_launches(1);
   }
   return 0;

@@ -80,7 +80,9 @@ def lib():
         L.gsr_num_records.argtypes = [vp]
         L.gsr_num_records.restype = i64
         L.gsr_render_backward.argtypes = [vp, vp, vp, vp, i32, vp, vp]
-        L.gsr_distortion_backward.argtypes = [vp, vp, i32, i32, i32, vp, C.c_double, vp, vp]
+        L.gsr_distortion_backward.argtypes = [vp, vp, i32, i32, i32, vp, C.c_double, vp, vp, sz, vp]
+        L.gsr_distortion_backward_workspace_bytes.argtypes = [i32, i32]
+        L.gsr_distortion_backward_workspace_bytes.restype = sz
         L.gsr_project_backward.argtypes = [vp, C.POINTER(CameraC), f32, vp, vp, vp, vp, vp, vp]
         L.gsr_close_levels.argtypes = [vp, i64, vp, vp, vp]
         L.gsr_frame_workspace_bytes.argtypes = [vp, C.POINTER(CameraC), i32, i32, i32, i32]
@@ -509,9 +511,10 @@ def distortion_ssim(imgs, ref, mse=None, workspace=None):
     return ssim, dmix
 
 
-def distortion_backward(imgs, ref, weight=None, lambda_ssim: float = 0.20, out=None):
+def distortion_backward(imgs, ref, weight=None, lambda_ssim: float = 0.20, out=None, workspace=None):
     """gsr_distortion_backward: d/d(imgs) of sum_b weight[b] (MSE_b + lambda_ssim (1 - SSIM_b)) -> cuda float32
-    [B,H,W,3].  weight: cuda float64 [B] or None (= 1 per state)."""
+    [B,H,W,3].  weight: cuda float64 [B] or None (= 1 per state); workspace: cuda uint8 of
+    gsr_distortion_backward_workspace_bytes(H, W) bytes (allocated here if None)."""
     torch = _torch()
     B, H, W = int(imgs.shape[0]), int(imgs.shape[1]), int(imgs.shape[2])
     assert imgs.dtype == torch.float32 and imgs.is_cuda and imgs.is_contiguous()
@@ -521,8 +524,10 @@ def distortion_backward(imgs, ref, weight=None, lambda_ssim: float = 0.20, out=N
     if out is None:
         out = torch.empty_like(imgs)
     assert out.dtype == torch.float32 and out.is_cuda and out.is_contiguous() and out.shape == imgs.shape
+    if workspace is None:
+        workspace = torch.empty(int(lib().gsr_distortion_backward_workspace_bytes(H, W)), dtype=torch.uint8, device="cuda")
     _check(lib().gsr_distortion_backward(_dp(imgs), _dp(ref), B, H, W, _dp(weight), float(lambda_ssim), _dp(out),
-                                         _stream()))
+                                         _dp(workspace), workspace.numel(), _stream()))
     return out
 
 
