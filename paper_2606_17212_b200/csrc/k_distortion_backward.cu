@@ -27,10 +27,15 @@ constexpr double kDbC1 = 0.01 * 0.01, kDbC2 = 0.03 * 0.03;
 struct DbWindow { double g[2 * kDbR + 1]; };
 
 struct DbSmem {
-  float x[kDbIn][kDbIn + 1], y[kDbIn][kDbIn + 1];
+  double x[kDbIn][kDbIn + 1], y[kDbIn][kDbIn + 1];  // converted once at staging (F2F runs at a fraction of the DFMA rate)
   double h[3][kDbIn][kDbMid + 1];   // x, x x, x y blurred along x; reused for the maps blurred along x: [3][kDbMid][kDbT + 1]
   double m[3][kDbMid][kDbMid + 1];  // a, b, c
 };
+
+// Every blur step gives a thread a run of kRun consecutive outputs along the blur direction: the kRun + 10 inputs
+// are read once into registers (a sliding window), instead of 11 loads per output — the first version of this
+// kernel was bound by the shared-memory instruction queue (mio_throttle 3.5 per issue), not by the DFMAs.
+constexpr int kRunB = 6, kRunD = 4;  // 42 = 7 * 6 positions per row / column of the middle region; 32 = 8 * 4 of the block
 
 // mu_y = w*y and w*(y y) of the reference, double [H, W, 3] each (the image layout), zero padding
 __global__ void __launch_bounds__(kTilePix) k_ref_moments(const float* __restrict__ ref, int W, int H, int TX,
@@ -100,72 +105,116 @@ __global__ void __launch_bounds__(kDbThreads) k_distortion_backward(const float*
         vx = __ldg(im + o);
         vy = __ldg(ref + o);
       }
-      s.x[hy][hx] = vx;
-      s.y[hy][hx] = vy;
+      s.x[hy][hx] = (double)vx;
+      s.y[hy][hx] = (double)vy;
     }
     __syncthreads();
-    // B. x, x x, x y blurred along x: rows 0..51, columns 0..41 (column c is staged column c + 5)
-    for (int i = tid; i < kDbIn * kDbMid; i += kDbThreads) {
-      const int r = i / kDbMid, c = i - r * kDbMid;
-      double a0 = 0, a2 = 0, a4 = 0;
+    // B. x, x x, x y blurred along x: rows 0..51, columns 0..41 (column c is staged column c + 5); lanes run over
+    //    rows (pitch 53 doubles: 16 distinct bank pairs per half-warp)
+    for (int i = tid; i < kDbIn * (kDbMid / kRunB); i += kDbThreads) {
+      const int grp = i / kDbIn, r = i - grp * kDbIn, c0 = grp * kRunB;
+      double xv[kRunB + 2 * kDbR], xx[kRunB + 2 * kDbR], xy[kRunB + 2 * kDbR];
 #pragma unroll
-      for (int k = 0; k <= 2 * kDbR; ++k) {
-        const double xv = (double)s.x[r][c + k], yv = (double)s.y[r][c + k], g = win.g[k];
-        a0 += g * xv; a2 += g * (xv * xv); a4 += g * (xv * yv);
+      for (int j = 0; j < kRunB + 2 * kDbR; ++j) {
+        const double yv = s.y[r][c0 + j];
+        xv[j] = s.x[r][c0 + j];
+        xx[j] = xv[j] * xv[j];
+        xy[j] = xv[j] * yv;
       }
-      s.h[0][r][c] = a0; s.h[1][r][c] = a2; s.h[2][r][c] = a4;
-    }
-    __syncthreads();
-    // C. along y, then a, b, c at the 42 x 42 positions (row r is staged row r + 5)
-    for (int i = tid; i < kDbMid * kDbMid; i += kDbThreads) {
-      const int r = i / kDbMid, c = i - r * kDbMid;
-      const int qx = x0 + c - kDbR, qy = y0 + r - kDbR;
-      double va = 0.0, vb = 0.0, vc = 0.0;
-      if (qx >= 0 && qx < W && qy >= 0 && qy < H) {
-        double m0 = 0, m2 = 0, m4 = 0;
+#pragma unroll
+      for (int o = 0; o < kRunB; ++o) {
+        double a0 = 0, a2 = 0, a4 = 0;
 #pragma unroll
         for (int k = 0; k <= 2 * kDbR; ++k) {
           const double g = win.g[k];
-          m0 += g * s.h[0][r + k][c]; m2 += g * s.h[1][r + k][c]; m4 += g * s.h[2][r + k][c];
+          a0 += g * xv[o + k]; a2 += g * xx[o + k]; a4 += g * xy[o + k];
         }
-        const size_t o = ((size_t)qy * W + qx) * 3 + ch;
-        const double mx = m0, my = ref_my[o], sxx = m2 - mx * mx, syy = ref_eyy[o] - my * my, sxy = m4 - mx * my;
-        const double N1 = 2.0 * mx * my + kDbC1, N2 = 2.0 * sxy + kDbC2;
-        const double D1 = mx * mx + my * my + kDbC1, D2 = sxx + syy + kDbC2;
-        const double r12 = 1.0 / (D1 * D2);
-        vb = -N1 * N2 * r12 / D2;
-        vc = 2.0 * N1 * r12;
-        va = 2.0 * my * N2 * r12 - 2.0 * mx * N1 * N2 * r12 / D1 - 2.0 * mx * vb - my * vc;
+        s.h[0][r][c0 + o] = a0; s.h[1][r][c0 + o] = a2; s.h[2][r][c0 + o] = a4;
       }
-      s.m[0][r][c] = va; s.m[1][r][c] = vb; s.m[2][r][c] = vc;
     }
     __syncthreads();
-    // D. the maps blurred along x: rows 0..41, block columns 0..31 (block column c is map column c + 5)
-    for (int i = tid; i < kDbMid * kDbT; i += kDbThreads) {
-      const int r = i / kDbT, c = i - r * kDbT;
-      double a0 = 0, a1 = 0, a2 = 0;
+    // C. along y, then a, b, c at the 42 x 42 positions (row r is staged row r + 5); lanes run over columns
+    for (int i = tid; i < kDbMid * (kDbMid / kRunB); i += kDbThreads) {
+      const int grp = i / kDbMid, c = i - grp * kDbMid, r0 = grp * kRunB;
+      double mo[3][kRunB];
 #pragma unroll
-      for (int k = 0; k <= 2 * kDbR; ++k) {
-        const double g = win.g[k];
-        a0 += g * s.m[0][r][c + k]; a1 += g * s.m[1][r][c + k]; a2 += g * s.m[2][r][c + k];
+      for (int j3 = 0; j3 < 3; ++j3) {
+        double v[kRunB + 2 * kDbR];
+#pragma unroll
+        for (int j = 0; j < kRunB + 2 * kDbR; ++j) v[j] = s.h[j3][r0 + j][c];
+#pragma unroll
+        for (int o = 0; o < kRunB; ++o) {
+          double acc = 0;
+#pragma unroll
+          for (int k = 0; k <= 2 * kDbR; ++k) acc += win.g[k] * v[o + k];
+          mo[j3][o] = acc;
+        }
       }
-      gx[0][r][c] = a0; gx[1][r][c] = a1; gx[2][r][c] = a2;
+      const int qx = x0 + c - kDbR;
+#pragma unroll
+      for (int o = 0; o < kRunB; ++o) {
+        const int r = r0 + o, qy = y0 + r - kDbR;
+        double va = 0.0, vb = 0.0, vc = 0.0;
+        if (qx >= 0 && qx < W && qy >= 0 && qy < H) {
+          const size_t oo = ((size_t)qy * W + qx) * 3 + ch;
+          const double mx = mo[0][o], my = ref_my[oo], sxx = mo[1][o] - mx * mx, syy = ref_eyy[oo] - my * my,
+                       sxy = mo[2][o] - mx * my;
+          const double N1 = 2.0 * mx * my + kDbC1, N2 = 2.0 * sxy + kDbC2;
+          const double D1 = mx * mx + my * my + kDbC1, D2 = sxx + syy + kDbC2;
+          const double r12 = 1.0 / (D1 * D2);
+          vb = -N1 * N2 * r12 / D2;
+          vc = 2.0 * N1 * r12;
+          va = 2.0 * my * N2 * r12 - 2.0 * mx * N1 * N2 * r12 / D1 - 2.0 * mx * vb - my * vc;
+        }
+        s.m[0][r][c] = va; s.m[1][r][c] = vb; s.m[2][r][c] = vc;
+      }
     }
     __syncthreads();
-    // E. along y and the pixel's gradient
-    for (int i = tid; i < kDbT * kDbT; i += kDbThreads) {
-      const int ty = i / kDbT, tx = i - ty * kDbT;
-      const int px = x0 + tx, py = y0 + ty;
-      if (px < W && py < H) {
-        double a0 = 0, a1 = 0, a2 = 0;
+    // D. the maps blurred along x: rows 0..41, block columns 0..31 (block column c is map column c + 5); lanes run
+    //    over rows (pitch 43 doubles)
+    for (int i = tid; i < kDbMid * (kDbT / kRunD); i += kDbThreads) {
+      const int grp = i / kDbMid, r = i - grp * kDbMid, c0 = grp * kRunD;
 #pragma unroll
-        for (int k = 0; k <= 2 * kDbR; ++k) {
-          const double g = win.g[k];
-          a0 += g * gx[0][ty + k][tx]; a1 += g * gx[1][ty + k][tx]; a2 += g * gx[2][ty + k][tx];
+      for (int j3 = 0; j3 < 3; ++j3) {
+        double v[kRunD + 2 * kDbR];
+#pragma unroll
+        for (int j = 0; j < kRunD + 2 * kDbR; ++j) v[j] = s.m[j3][r][c0 + j];
+#pragma unroll
+        for (int o = 0; o < kRunD; ++o) {
+          double acc = 0;
+#pragma unroll
+          for (int k = 0; k <= 2 * kDbR; ++k) acc += win.g[k] * v[o + k];
+          gx[j3][r][c0 + o] = acc;
         }
-        const double xv = (double)s.x[ty + 2 * kDbR][tx + 2 * kDbR], yv = (double)s.y[ty + 2 * kDbR][tx + 2 * kDbR];
-        const double dssim = (a0 + 2.0 * xv * a1 + yv * a2) * inv_n;
-        out[(size_t)b * img + ((size_t)py * W + px) * 3 + ch] = (float)(wb * (2.0 * (xv - yv) * inv_n - lambda * dssim));
+      }
+    }
+    __syncthreads();
+    // E. along y and the pixels' gradient; lanes run over columns
+    for (int i = tid; i < kDbT * (kDbT / kRunD); i += kDbThreads) {
+      const int grp = i / kDbT, tx = i - grp * kDbT, ty0 = grp * kRunD;
+      double bl[3][kRunD];
+#pragma unroll
+      for (int j3 = 0; j3 < 3; ++j3) {
+        double v[kRunD + 2 * kDbR];
+#pragma unroll
+        for (int j = 0; j < kRunD + 2 * kDbR; ++j) v[j] = gx[j3][ty0 + j][tx];
+#pragma unroll
+        for (int o = 0; o < kRunD; ++o) {
+          double acc = 0;
+#pragma unroll
+          for (int k = 0; k <= 2 * kDbR; ++k) acc += win.g[k] * v[o + k];
+          bl[j3][o] = acc;
+        }
+      }
+      const int px = x0 + tx;
+#pragma unroll
+      for (int o = 0; o < kRunD; ++o) {
+        const int ty = ty0 + o, py = y0 + ty;
+        if (px < W && py < H) {
+          const double xv = s.x[ty + 2 * kDbR][tx + 2 * kDbR], yv = s.y[ty + 2 * kDbR][tx + 2 * kDbR];
+          const double dssim = (bl[0][o] + 2.0 * xv * bl[1][o] + yv * bl[2][o]) * inv_n;
+          out[(size_t)b * img + ((size_t)py * W + px) * 3 + ch] = (float)(wb * (2.0 * (xv - yv) * inv_n - lambda * dssim));
+        }
       }
     }
     __syncthreads();  // the staging buffers are rewritten for the next channel
