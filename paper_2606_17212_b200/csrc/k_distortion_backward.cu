@@ -21,16 +21,20 @@ constexpr int kDbR = 5;                    // window radius
 constexpr int kDbT = 32;                   // block edge
 constexpr int kDbIn = kDbT + 4 * kDbR;     // 52: staged pixels per side
 constexpr int kDbMid = kDbT + 2 * kDbR;    // 42: positions where the SSIM map is needed
-constexpr int kDbThreads = 512;
+constexpr int kDbThreads = 384;
 constexpr double kDbC1 = 0.01 * 0.01, kDbC2 = 0.03 * 0.03;
 
 struct DbWindow { double g[2 * kDbR + 1]; };
 
 struct DbSmem {
-  double x[kDbIn][kDbIn + 1], y[kDbIn][kDbIn + 1];  // converted once at staging (F2F runs at a fraction of the DFMA rate)
+  // staging, converted once (F2F runs at a fraction of the DFMA rate); dead after step B, when a, b, c
+  // ([3][kDbMid][kDbMid + 1] doubles) take its place — 106 KB in all, so that two CTAs share an SM and one computes
+  // while the other waits at a barrier
+  double x[kDbIn][kDbIn + 1], y[kDbIn][kDbIn + 1];
   double h[3][kDbIn][kDbMid + 1];   // x, x x, x y blurred along x; reused for the maps blurred along x: [3][kDbMid][kDbT + 1]
-  double m[3][kDbMid][kDbMid + 1];  // a, b, c
+  float cx[kDbT][kDbT + 1], cy[kDbT][kDbT + 1];  // the block's own pixels, for step E
 };
+static_assert(sizeof(double) * 3 * kDbMid * (kDbMid + 1) <= sizeof(double) * 2 * kDbIn * (kDbIn + 1), "a, b, c alias the staging");
 
 // Every blur step gives a thread a run of kRun consecutive outputs along the blur direction: the kRun + 10 inputs
 // are read once into registers (a sliding window), instead of 11 loads per output — the first version of this
@@ -79,7 +83,7 @@ __global__ void __launch_bounds__(kTilePix) k_ref_moments(const float* __restric
   }
 }
 
-__global__ void __launch_bounds__(kDbThreads) k_distortion_backward(const float* __restrict__ imgs,
+__global__ void __launch_bounds__(kDbThreads, 2) k_distortion_backward(const float* __restrict__ imgs,
                                                                     const float* __restrict__ ref, int W, int H, int TX,
                                                                     const double* __restrict__ ref_my,
                                                                     const double* __restrict__ ref_eyy,
@@ -88,6 +92,7 @@ __global__ void __launch_bounds__(kDbThreads) k_distortion_backward(const float*
   extern __shared__ __align__(16) unsigned char smem_raw[];
   DbSmem& s = *reinterpret_cast<DbSmem*>(smem_raw);
   double(*gx)[kDbMid][kDbT + 1] = reinterpret_cast<double(*)[kDbMid][kDbT + 1]>(&s.h[0][0][0]);
+  double(*sm)[kDbMid][kDbMid + 1] = reinterpret_cast<double(*)[kDbMid][kDbMid + 1]>(&s.x[0][0]);
   const int tid = threadIdx.x, tile = blockIdx.x, b = blockIdx.y;
   const int x0 = (tile % TX) * kDbT, y0 = (tile / TX) * kDbT;
   const size_t img = (size_t)H * W * 3;
@@ -107,6 +112,8 @@ __global__ void __launch_bounds__(kDbThreads) k_distortion_backward(const float*
       }
       s.x[hy][hx] = (double)vx;
       s.y[hy][hx] = (double)vy;
+      const int bx = hx - 2 * kDbR, by = hy - 2 * kDbR;
+      if (bx >= 0 && bx < kDbT && by >= 0 && by < kDbT) { s.cx[by][bx] = vx; s.cy[by][bx] = vy; }
     }
     __syncthreads();
     // B. x, x x, x y blurred along x: rows 0..51, columns 0..41 (column c is staged column c + 5); lanes run over
@@ -166,7 +173,7 @@ __global__ void __launch_bounds__(kDbThreads) k_distortion_backward(const float*
           vc = 2.0 * N1 * r12;
           va = 2.0 * my * N2 * r12 - 2.0 * mx * N1 * N2 * r12 / D1 - 2.0 * mx * vb - my * vc;
         }
-        s.m[0][r][c] = va; s.m[1][r][c] = vb; s.m[2][r][c] = vc;
+        sm[0][r][c] = va; sm[1][r][c] = vb; sm[2][r][c] = vc;
       }
     }
     __syncthreads();
@@ -178,7 +185,7 @@ __global__ void __launch_bounds__(kDbThreads) k_distortion_backward(const float*
       for (int j3 = 0; j3 < 3; ++j3) {
         double v[kRunD + 2 * kDbR];
 #pragma unroll
-        for (int j = 0; j < kRunD + 2 * kDbR; ++j) v[j] = s.m[j3][r][c0 + j];
+        for (int j = 0; j < kRunD + 2 * kDbR; ++j) v[j] = sm[j3][r][c0 + j];
 #pragma unroll
         for (int o = 0; o < kRunD; ++o) {
           double acc = 0;
@@ -211,7 +218,7 @@ __global__ void __launch_bounds__(kDbThreads) k_distortion_backward(const float*
       for (int o = 0; o < kRunD; ++o) {
         const int ty = ty0 + o, py = y0 + ty;
         if (px < W && py < H) {
-          const double xv = s.x[ty + 2 * kDbR][tx + 2 * kDbR], yv = s.y[ty + 2 * kDbR][tx + 2 * kDbR];
+          const double xv = (double)s.cx[ty][tx], yv = (double)s.cy[ty][tx];
           const double dssim = (bl[0][o] + 2.0 * xv * bl[1][o] + yv * bl[2][o]) * inv_n;
           out[(size_t)b * img + ((size_t)py * W + px) * 3 + ch] = (float)(wb * (2.0 * (xv - yv) * inv_n - lambda * dssim));
         }
