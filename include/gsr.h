@@ -161,8 +161,8 @@ int gsr_render_states_vs_full(const gsr_scene* scene, const gsr_camera* cam, flo
  * per tile with the sum of their dL_dimages — the gradient is linear in it (option "dedup", default on).
  *   images      dev fp32 [B,H,W,3]  the forward output of that call
  *   dL_dimages  dev fp32 [B,H,W,3]  the gradient of the objective with respect to every pixel of every state
- *   grad        dev fp32 [gsr_num_records(scene), 12], overwritten: for record r (Gaussian i, variant v: r = 2 i + v,
- *               v = 0 the geometry of cluster depth 0, v = 1 of depth >= 1; r = 4 i + v for scenes with position
+ *   grad        dev fp32 [gsr_num_records(scene), 12], 16-byte aligned, overwritten: for record r (Gaussian i,
+ *               variant v: r = 2 i + v, v = 0 the geometry of cluster depth 0, v = 1 of depth >= 1; r = 4 i + v for scenes with position
  *               residual levels), summed over the states and pixels that composite it,
  *               d/d(rgb[3], rgb with the level-3 SH residual[3], opacity, A, B, Cq, m_x, m_y)
  *               where pixel = sum_i alpha_i T_i rgb_i + T_end bg, alpha = min(0.99, opacity exp(-q)),

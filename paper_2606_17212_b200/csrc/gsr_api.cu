@@ -552,6 +552,10 @@ int gsr_render_backward(const gsr_scene* scene, void* workspace, const float* im
     set_error("gsr_render_backward: invalid argument");
     return GSR_E_INVALID_ARG;
   }
+  if (((uintptr_t)grad & 15u) != 0) {  // rows of 12 floats are added with 16-byte vector reductions
+    set_error("gsr_render_backward: grad must be 16-byte aligned");
+    return GSR_E_INVALID_ARG;
+  }
   // the header is read on the host: the forward call that filled the workspace has to be complete on this stream
   WsHeader h;
   GSR_CUDA(cudaMemcpyAsync(&h, workspace, sizeof(h), cudaMemcpyDeviceToHost, st));
@@ -597,6 +601,10 @@ int gsr_project_backward(const gsr_scene* scene, const gsr_camera* cam, float t,
                          float* g_gauss, float* g_sh_base, float* g_sh_res, float* g_cluster, void* cuda_stream) {
   if (!scene || !camera_ok(cam) || !g_cluster || (scene->impl.d.N > 0 && (!grad_records || !g_gauss || !g_sh_base || !g_sh_res))) {
     set_error("gsr_project_backward: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  if (((uintptr_t)grad_records & 15u) != 0) {  // rows of 12 floats are read as three 16-byte words
+    set_error("gsr_project_backward: grad_records must be 16-byte aligned");
     return GSR_E_INVALID_ARG;
   }
   const DeviceScene& D = scene->impl.d;

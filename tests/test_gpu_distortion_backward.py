@@ -153,3 +153,32 @@ def test_objective_to_parameters_against_differences_of_the_gpu_forward(gsr, tor
         # the image is piecewise smooth in the parameters (tile rectangles, cut, cap, stop, depth order are discrete):
         # finite steps cross a few of those, hence a percent-level bar; a wrong chain is off by O(1)
         assert abs((Lp - Lm) - pred) <= 3e-2 * mag + 2e-2 * abs(pred), (field, Lp - Lm, pred, mag)
+
+
+def test_argument_checks(gsr, torch_mod):
+    """Workspace too small -> GSR_E_WORKSPACE_TOO_SMALL (not needed when lambda = 0); misaligned gradient rows of
+    gsr_render_backward / gsr_project_backward -> GSR_E_INVALID_ARG."""
+    torch = torch_mod
+    imgs, ref = _images(9, 2, 20, 24)
+    di, dr = torch.from_numpy(imgs).cuda(), torch.from_numpy(ref).cuda()
+    small = torch.empty(64, dtype=torch.uint8, device="cuda")
+    with pytest.raises(gsr.GsrError):
+        gsr.distortion_backward(di, dr, None, 0.20, workspace=small)
+    g = gsr.distortion_backward(di, dr, None, 0.0, workspace=small)            # the MSE term alone needs none
+    assert np.allclose(g.cpu().numpy(), 2.0 * (imgs - ref[None]) / ref.size, rtol=1e-6, atol=1e-12)
+    wl = synth.scaled_object_workload(29, C=2, per_cluster=40.0, W=64, H=48, fov=40.0, n_frames=1, B=2)
+    cam, t = wl.frames[0]
+    scene = gsr.Scene(wl.scene)
+    ws = scene.new_workspace(cam, 2)
+    lv = torch.from_numpy(np.ascontiguousarray(wl.levels[0])).cuda()
+    out, _, _ = scene.render_states(cam, t, lv, workspace=ws)
+    buf = torch.zeros(scene.num_records() * 12 + 1, dtype=torch.float32, device="cuda")
+    off = buf[1:]                                                               # 4 bytes past a 16-byte boundary
+    assert off.data_ptr() % 16 != 0
+    C = gsr.C
+    rc = gsr.lib().gsr_render_backward(scene.handle, ws.data_ptr(), out.data_ptr(), out.data_ptr(), 2, off.data_ptr(), None)
+    assert rc == -1
+    rc = gsr.lib().gsr_project_backward(scene.handle, C.byref(gsr.camera_struct(cam)), float(t), off.data_ptr(),
+                                        buf.data_ptr(), buf.data_ptr(), buf.data_ptr(), buf.data_ptr(), None)
+    assert rc == -1
+    scene.close()
