@@ -29,6 +29,14 @@ What it follows (PAPER.md = /root/reference/PAPER.md; DESIGN.md §12 = the writt
                       pins: tests/test_distortion_backward_pins.py (central differences of D itself, the zero
                       at image = reference, the MSE-only closed form)
 
+  objective weights . d/dD_b of  w_mean mean(D) + w_cvar CVaR_alpha(D) + w_mono M(D)  (Eq. (2): the terms
+                      of the objective that are functions of the per-state distortions; lambda_c = 0.30,
+                      lambda_m = 2.0 in PAPER.md:72): mean -> 1/n each; CVaR (upper tail) -> 1/k for every value
+                      strictly above the threshold, and the remaining (k - #above)/k shared equally by the values
+                      equal to it (a subgradient; reading L1); M -> +1 on next and -1 on prev of every violated pair
+                      (objective_weights); flicker_backward: d F_b/d out_b(t2) = 2 e / (3 H W) = - d F_b/d out_b(t1)
+                      pins: tests/test_distortion_backward_pins.py d4, d5 (differences of the forward reductions)
+
 Pins: tests/test_metrics_pins.py (SSIM(x,x) = 1, constant-image closed form, scipy.ndimage Gaussian filtering
 as an independent library route, hand-worked CVaR / quantile, constant-shift flicker closed form, the paper's
 four monotone prefix points PAPER.md:94).
@@ -177,3 +185,40 @@ def prefix_monotonicity(d, idx_prev, idx_next):
             M += inc
             viol += 1
     return M, viol
+
+
+def objective_weights(d, w_mean: float, w_cvar: float, alpha: float, idx_prev=(), idx_next=(), w_mono: float = 0.0) -> np.ndarray:
+    """dL/dD_b for L = w_mean mean(D) + w_cvar CVaR_alpha(D) (upper tail, reading G2) + w_mono M(D) (reading G4)."""
+    v = [float(x) for x in np.asarray(d, np.float64).reshape(-1)]
+    n = len(v)
+    w = [0.0] * n
+    if n == 0:
+        return np.zeros(0)
+    for i in range(n):
+        w[i] += w_mean / n
+    k = min(max(1, int(math.ceil(alpha * n))), n)
+    thr = sorted(v)[n - k]                      # the mildest of the k worst (largest) values
+    above = sum(1 for x in v if x > thr)
+    ties = sum(1 for x in v if x == thr)
+    for i in range(n):
+        if v[i] > thr:
+            w[i] += w_cvar / k
+        elif v[i] == thr:
+            w[i] += w_cvar * (k - above) / (ties * k)
+    for p, q in zip(np.asarray(idx_prev).tolist(), np.asarray(idx_next).tolist()):
+        if v[q] - v[p] > 0.0:
+            w[q] += w_mono
+            w[p] -= w_mono
+    return np.array(w)
+
+
+def flicker_backward(imgs_t1, imgs_t2, ref_t1, ref_t2, weight):
+    """d/d(imgs_t1), d/d(imgs_t2) of sum_b weight[b] F_b (reading G3): ([B,H,W,3], [B,H,W,3]) float64."""
+    a, b = np.asarray(imgs_t1, np.float64), np.asarray(imgs_t2, np.float64)
+    r1, r2 = np.asarray(ref_t1, np.float64), np.asarray(ref_t2, np.float64)
+    w = np.asarray(weight, np.float64).reshape(-1)
+    g2 = np.zeros(a.shape)
+    for s_ in range(a.shape[0]):
+        e = (b[s_] - a[s_]) - (r2 - r1)
+        g2[s_] = w[s_] * 2.0 * e / e.size
+    return -g2, g2
