@@ -188,6 +188,23 @@ size_t gsr_distortion_backward_workspace_bytes(int32_t H, int32_t W);
 int gsr_distortion_backward(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, const double* weight,
                             double lambda_ssim, float* dL_dimgs, void* workspace, size_t ws_bytes, void* cuda_stream);
 
+/* The other image-space terms of Eq. (2) (L = E_w[D_w] + lambda_c CVaR_0.05(D) + lambda_r R +
+ * lambda_t F + lambda_m M; lambda_c = 0.30, lambda_t = 0.10, lambda_m = 2.0 in PAPER.md:72):
+ * gsr_objective_weights: weights[b] = dL/dD_b of w_mean mean(D) + w_cvar CVaR_alpha(D) + w_mono M(D) — the `weight`
+ *   input of gsr_distortion_backward.  1/n each; 1/k (k = max(1, ceil(alpha n))) for every D strictly above the CVaR
+ *   threshold, the remaining (k - #above)/k shared equally by the values equal to it (a subgradient); + w_mono on
+ *   idx_next[p] and - w_mono on idx_prev[p] of every pair with D[next] > D[prev] (indices outside [0, n) are refused:
+ *   gsr_index_status).  d, weights double dev [n]; idx_* int32 dev [n_pairs] (may be NULL when n_pairs = 0);
+ *   0 < alpha <= 1.
+ * gsr_flicker_backward: d/d(imgs_t1), d/d(imgs_t2) of sum_b weight[b] F_b (F of gsr_flicker): g_t2 = weight[b] 2 e /
+ *   (3 H W), g_t1 = - g_t2, e = (imgs_t2 - imgs_t1) - (ref_t2 - ref_t1); weight double dev [B] or NULL (= 1);
+ *   g_t1, g_t2 fp32 dev [B,H,W,3], overwritten (either may be NULL).  Both asynchronous. */
+int gsr_objective_weights(const double* d, int32_t n, double w_mean, double w_cvar, double alpha,
+                          const int32_t* idx_prev, const int32_t* idx_next, int32_t n_pairs, double w_mono,
+                          double* weights, void* cuda_stream);
+int gsr_flicker_backward(const float* imgs_t1, const float* imgs_t2, const float* ref_t1, const float* ref_t2, int32_t B,
+                         int32_t H, int32_t W, const double* weight, float* g_t1, float* g_t2, void* cuda_stream);
+
 /* ------------------------------------------------------------------------------------------------
  * gsr_project_backward — the backward of the steps in front of the compositor: activation,
  * deformation Eq. (1), EWA projection and SH colour; DESIGN.md §17.  Takes the

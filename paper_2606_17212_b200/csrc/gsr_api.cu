@@ -572,6 +572,31 @@ int gsr_render_backward(const gsr_scene* scene, void* workspace, const float* im
   return GSR_OK;
 }
 
+int gsr_objective_weights(const double* d, int32_t n, double w_mean, double w_cvar, double alpha,
+                          const int32_t* idx_prev, const int32_t* idx_next, int32_t n_pairs, double w_mono,
+                          double* weights, void* cuda_stream) {
+  if (n < 0 || n_pairs < 0 || (n > 0 && (!d || !weights)) || (n_pairs > 0 && (!idx_prev || !idx_next)) ||
+      !(alpha > 0.0 && alpha <= 1.0)) {
+    set_error("gsr_objective_weights: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  launch_objective_weights(d, n, w_mean, w_cvar, alpha, idx_prev, idx_next, n_pairs, w_mono, weights,
+                           (cudaStream_t)cuda_stream);
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
+int gsr_flicker_backward(const float* imgs_t1, const float* imgs_t2, const float* ref_t1, const float* ref_t2, int32_t B,
+                         int32_t H, int32_t W, const double* weight, float* g_t1, float* g_t2, void* cuda_stream) {
+  if (B < 0 || H <= 0 || W <= 0 || (B > 0 && (!imgs_t1 || !imgs_t2 || !ref_t1 || !ref_t2 || (!g_t1 && !g_t2)))) {
+    set_error("gsr_flicker_backward: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  launch_flicker_backward(imgs_t1, imgs_t2, ref_t1, ref_t2, B, H, W, weight, g_t1, g_t2, (cudaStream_t)cuda_stream);
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
 size_t gsr_distortion_backward_workspace_bytes(int32_t H, int32_t W) {
   if (H <= 0 || W <= 0) return 0;
   return align_up(sizeof(double) * 2 * 3 * (size_t)H * (size_t)W);

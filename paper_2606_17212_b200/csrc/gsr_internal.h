@@ -171,6 +171,11 @@ void count_launches(int n);
 struct CompositeArgs;
 void launch_composite_q(const CompositeArgs& a, int S, bool count, cudaStream_t st);
 // backward of a4 (k_backward.cu): grad [records, 12], zeroed by the call
+void launch_objective_weights(const double* d, int32_t n, double w_mean, double w_cvar, double alpha,
+                              const int32_t* prev, const int32_t* next, int32_t n_pairs, double w_mono, double* w,
+                              cudaStream_t st);
+void launch_flicker_backward(const float* a1, const float* a2, const float* r1, const float* r2, int32_t B, int32_t H,
+                             int32_t W, const double* weight, float* g1, float* g2, cudaStream_t st);
 int launch_distortion_backward(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W,
                                const double* weight, double lambda, float* out, double* ref_planes, cudaStream_t st);
 void launch_project_backward(const DeviceScene& sc, const FrameParams& fp, const float* grad_rec, float* g_gauss,

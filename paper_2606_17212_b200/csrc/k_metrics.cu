@@ -241,6 +241,59 @@ __global__ void __launch_bounds__(kRiskThreads) k_prefix_monotonicity(const doub
   }
 }
 
+// ---- dL/dD_b of L = w_mean mean(D) + w_cvar CVaR_alpha(D) + w_mono M(D) (Eq. (2)):
+//      1/n each; 1/k for every value strictly above the CVaR threshold and the remaining (k - #above)/k shared
+//      equally by the values equal to it (a subgradient, reading L1); +w_mono on next, -w_mono on prev of every
+//      violated pair.  One CTA.
+__global__ void __launch_bounds__(kRiskThreads) k_objective_weights(const double* __restrict__ d, int n, double w_mean,
+                                                                    double w_cvar, double alpha,
+                                                                    const int* __restrict__ prev,
+                                                                    const int* __restrict__ next, int n_pairs,
+                                                                    double w_mono, double* __restrict__ w,
+                                                                    int* __restrict__ err) {
+  __shared__ unsigned long long sm_c[kRiskThreads];
+  if (n <= 0) return;
+  int k = (int)ceil(alpha * (double)n);
+  k = k < 1 ? 1 : (k > n ? n : k);
+  const double thr = risk_select(d, 0, n, n - k, sm_c);
+  unsigned long long above = 0, ties = 0;
+  for (int i = threadIdx.x; i < n; i += kRiskThreads) {
+    above += d[i] > thr;
+    ties += d[i] == thr;
+  }
+  above = risk_block_sum<unsigned long long>(above, sm_c);
+  ties = risk_block_sum<unsigned long long>(ties, sm_c);
+  const double share = ties ? w_cvar * (double)(k - (int)above) / ((double)ties * (double)k) : 0.0;
+  for (int i = threadIdx.x; i < n; i += kRiskThreads)
+    w[i] = w_mean / (double)n + (d[i] > thr ? w_cvar / (double)k : (d[i] == thr ? share : 0.0));
+  __syncthreads();
+  for (int p = threadIdx.x; p < n_pairs; p += kRiskThreads) {
+    const int a = prev[p], b = next[p];
+    if (a < 0 || b < 0 || a >= n || b >= n) {
+      if (err) atomicOr(err, kBadPrefixIndex);
+      continue;
+    }
+    if (d[b] - d[a] > 0.0) {
+      atomicAdd(w + b, w_mono);
+      atomicAdd(w + a, -w_mono);
+    }
+  }
+}
+
+// ---- d/d(imgs_t1), d/d(imgs_t2) of sum_b weight_b F_b (reading G3): the forward's fp32 differences, then 2 e / (3 H W)
+__global__ void k_flicker_backward(const float* __restrict__ a1, const float* __restrict__ a2, const float* __restrict__ r1,
+                                   const float* __restrict__ r2, size_t img, const double* __restrict__ weight,
+                                   float* __restrict__ g1, float* __restrict__ g2) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int b = blockIdx.y;
+  if (i >= img) return;
+  const size_t o = (size_t)b * img + i;
+  const float e = __fsub_rn(__fsub_rn(a2[o], a1[o]), __fsub_rn(__ldg(r2 + i), __ldg(r1 + i)));
+  const double g = (weight ? weight[b] : 1.0) * 2.0 * (double)e / (double)img;
+  if (g2) g2[o] = (float)g;
+  if (g1) g1[o] = (float)(-g);
+}
+
 // ------------------------------------------------------------------------------------------------ launchers
 void launch_ssim(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, const double* mse, double* part,
                  double* ssim, double* dmix, cudaStream_t st) {
@@ -287,6 +340,28 @@ void launch_prefix_monotonicity(const double* d, int32_t n, const int32_t* prev,
                                 double* m_out, int32_t* viol, cudaStream_t st) {
   k_prefix_monotonicity<<<1, kRiskThreads, 0, st>>>(d, n, prev, next, n_pairs, m_out, viol, device_error_word());
   count_launches(1);
+}
+
+void launch_objective_weights(const double* d, int32_t n, double w_mean, double w_cvar, double alpha,
+                              const int32_t* prev, const int32_t* next, int32_t n_pairs, double w_mono, double* w,
+                              cudaStream_t st) {
+  if (n <= 0) return;
+  k_objective_weights<<<1, kRiskThreads, 0, st>>>(d, n, w_mean, w_cvar, alpha, prev, next, n_pairs, w_mono, w,
+                                                  device_error_word());
+  count_launches(1);
+}
+
+void launch_flicker_backward(const float* a1, const float* a2, const float* r1, const float* r2, int32_t B, int32_t H,
+                             int32_t W, const double* weight, float* g1, float* g2, cudaStream_t st) {
+  if (B == 0) return;
+  const size_t img = (size_t)H * W * 3;
+  for (int b0 = 0; b0 < B; b0 += 65535) {
+    const int nb = B - b0 < 65535 ? B - b0 : 65535;
+    k_flicker_backward<<<dim3((unsigned)((img + 255) / 256), nb), 256, 0, st>>>(
+        a1 + (size_t)b0 * img, a2 + (size_t)b0 * img, r1, r2, img, weight ? weight + b0 : nullptr,
+        g1 ? g1 + (size_t)b0 * img : nullptr, g2 ? g2 + (size_t)b0 * img : nullptr);
+    count_launches(1);
+  }
 }
 
 }  // namespace gsr

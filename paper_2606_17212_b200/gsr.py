@@ -83,6 +83,8 @@ def lib():
         L.gsr_distortion_backward.argtypes = [vp, vp, i32, i32, i32, vp, C.c_double, vp, vp, sz, vp]
         L.gsr_distortion_backward_workspace_bytes.argtypes = [i32, i32]
         L.gsr_distortion_backward_workspace_bytes.restype = sz
+        L.gsr_objective_weights.argtypes = [vp, i32, C.c_double, C.c_double, C.c_double, vp, vp, i32, C.c_double, vp, vp]
+        L.gsr_flicker_backward.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp, vp, vp]
         L.gsr_project_backward.argtypes = [vp, C.POINTER(CameraC), f32, vp, vp, vp, vp, vp, vp]
         L.gsr_close_levels.argtypes = [vp, i64, vp, vp, vp]
         L.gsr_frame_workspace_bytes.argtypes = [vp, C.POINTER(CameraC), i32, i32, i32, i32]
@@ -529,6 +531,35 @@ def distortion_backward(imgs, ref, weight=None, lambda_ssim: float = 0.20, out=N
     _check(lib().gsr_distortion_backward(_dp(imgs), _dp(ref), B, H, W, _dp(weight), float(lambda_ssim), _dp(out),
                                          _dp(workspace), workspace.numel(), _stream()))
     return out
+
+
+def objective_weights(d, w_mean: float = 1.0, w_cvar: float = 0.30, alpha: float = 0.05, idx_prev=None, idx_next=None,
+                      w_mono: float = 0.0, out=None):
+    """gsr_objective_weights: d cuda float64 [n] -> dL/dD_b of w_mean mean + w_cvar CVaR_alpha + w_mono M, cuda float64 [n]."""
+    torch = _torch()
+    assert d.dtype == torch.float64 and d.is_cuda and d.is_contiguous()
+    n = int(d.numel())
+    n_pairs = 0 if idx_prev is None else int(idx_prev.numel())
+    if n_pairs:
+        for t in (idx_prev, idx_next):
+            assert t.dtype == torch.int32 and t.is_cuda and t.is_contiguous() and t.numel() == n_pairs
+    if out is None:
+        out = torch.empty(n, dtype=torch.float64, device="cuda")
+    _check(lib().gsr_objective_weights(_dp(d), n, float(w_mean), float(w_cvar), float(alpha), _dp(idx_prev) if n_pairs else None,
+                                       _dp(idx_next) if n_pairs else None, n_pairs, float(w_mono), _dp(out), _stream()))
+    return out
+
+
+def flicker_backward(imgs_t1, imgs_t2, ref_t1, ref_t2, weight=None):
+    """gsr_flicker_backward -> (g_t1, g_t2) cuda float32 [B,H,W,3]."""
+    torch = _torch()
+    B, H, W = int(imgs_t1.shape[0]), int(imgs_t1.shape[1]), int(imgs_t1.shape[2])
+    for t in (imgs_t1, imgs_t2, ref_t1, ref_t2):
+        assert t.dtype == torch.float32 and t.is_cuda and t.is_contiguous()
+    g1, g2 = torch.empty_like(imgs_t1), torch.empty_like(imgs_t2)
+    _check(lib().gsr_flicker_backward(_dp(imgs_t1), _dp(imgs_t2), _dp(ref_t1), _dp(ref_t2), B, H, W, _dp(weight),
+                                      _dp(g1), _dp(g2), _stream()))
+    return g1, g2
 
 
 def flicker(imgs_t1, imgs_t2, ref_t1, ref_t2, workspace=None):

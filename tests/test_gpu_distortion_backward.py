@@ -182,3 +182,34 @@ def test_argument_checks(gsr, torch_mod):
                                         buf.data_ptr(), buf.data_ptr(), buf.data_ptr(), buf.data_ptr(), None)
     assert rc == -1
     scene.close()
+
+
+def test_objective_weights_and_flicker_gradient_against_the_oracle(gsr, torch_mod):
+    """gsr_objective_weights (double, exact selection: 1e-15) incl. ties at the CVaR threshold, n = 1, the paper's
+    weights (1, 0.30 at alpha 0.05, lambda_m = 2.0); refused pair indices; gsr_flicker_backward (fp32 differences)."""
+    torch = torch_mod
+    rng = np.random.default_rng(21)
+    for n, alpha in ((96, 0.05), (40, 0.05), (7, 0.2), (1, 0.05), (300, 0.5), (8197, 0.05)):
+        d = rng.uniform(0.01, 0.2, n)
+        if n >= 7:
+            d[3] = d[5] = np.sort(d)[-max(1, int(np.ceil(alpha * n)))]           # ties exactly at the threshold
+        prev = rng.integers(0, n, 16).astype(np.int32)
+        nxt = rng.integers(0, n, 16).astype(np.int32)
+        want = M.objective_weights(d, 1.0, 0.30, alpha, prev, nxt, 2.0)
+        got = gsr.objective_weights(torch.from_numpy(d).cuda(), 1.0, 0.30, alpha, torch.from_numpy(prev).cuda(),
+                                    torch.from_numpy(nxt).cuda(), 2.0).cpu().numpy()
+        assert np.abs(got - want).max() <= 1e-15 * max(1.0, np.abs(want).max()), (n, alpha)
+        assert abs(got.sum() - 1.30) <= 1e-12                                    # mean and CVaR weights sum to 1 each; M's cancel
+    got = gsr.objective_weights(torch.from_numpy(np.array([0.3, 0.2])).cuda(), 1.0, 0.0, 0.05,
+                                torch.tensor([0, 5], dtype=torch.int32, device="cuda"),
+                                torch.tensor([1, 1], dtype=torch.int32, device="cuda"), 2.0).cpu().numpy()
+    assert np.array_equal(got, [0.5, 0.5])                                        # no violation; the pair (5, 1) is refused
+    with pytest.raises(gsr.GsrError):
+        gsr.index_status()                                                       # the refusal is latched and reported
+    a, b = rng.uniform(0, 1, (2, 3, 21, 17, 3)).astype(np.float32)
+    r1, r2 = rng.uniform(0, 1, (2, 21, 17, 3)).astype(np.float32)
+    wgt = np.array([0.3, 0.0, 1.7])
+    g1, g2 = gsr.flicker_backward(*(torch.from_numpy(x).cuda() for x in (a, b, r1, r2)), torch.from_numpy(wgt).cuda())
+    w1, w2 = M.flicker_backward(a, b, r1, r2, wgt)
+    assert np.abs(g2.cpu().numpy() - w2).max() <= 2e-7 * np.abs(w2).max()
+    assert torch.equal(g1, -g2)
