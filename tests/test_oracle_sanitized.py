@@ -1,5 +1,6 @@
 """The oracle under AddressSanitizer + UndefinedBehaviorSanitizer: the tiny scene of configs[0] is
-projected, key-listed and rendered (brute force and Gaussian-major) in a child process that preloads libasan; any
+projected, key-listed, rendered (brute force and Gaussian-major) and differentiated (O-8, O-9) in a child process
+that preloads libasan; any
 out-of-bounds access, use of uninitialised stack, signed overflow or misaligned access aborts the child."""
 import os
 import subprocess
@@ -26,6 +27,13 @@ assert len(tile) == p["count"][p["valid"] == 1].sum()
 ref, _ = sc.render(cam, t, np.full(4, 3, np.int8))
 mse, psnr = O.distortion(a, ref)
 assert mse.shape == (lv.shape[0],)
+# the backward oracles (O-8, O-9): one state, random dL/d(image)
+d3 = np.array([3, 1, -1, 0], np.int8)
+g = np.random.default_rng(0).standard_normal((cam.H, cam.W, 3))
+g9, gabs = sc.backward(cam, t, d3, g, want_abs=True)
+gp = sc.project_backward(cam, t, d3, g9)
+assert np.isfinite(gp["mean"]).all() and np.isfinite(gp["sh_base"]).all() and np.any(gp["quat"] != 0.0)
+assert O.sh_basis_grad(16, (0.1, 0.2, 0.97)).shape == (3, 16)
 print("sanitized oracle ok", len(tile))
 """
 
