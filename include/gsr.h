@@ -246,6 +246,20 @@ size_t gsr_distortion_workspace_bytes(int32_t B, int32_t H, int32_t W);
 int gsr_distortion(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, double* mse,
                    float* psnr_db, void* workspace, size_t ws_bytes, void* cuda_stream);
 
+/* gsr_distortion_static — gsr_distortion for callers that may not allocate device memory (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc): the same kernels and reduction tree, hence the same
+ * values, with the per-(state, tile) partials in a scratch array built into the library instead of a caller-provided
+ * workspace.  The call allocates nothing (no cudaMalloc / cudaFree / allocating library routine).
+ *   Limit: B * ceil(W/16) * ceil(H/16) <= gsr_distortion_static_max_partials() = 2^20 (8 MiB of device memory, held by
+ *   every GPU that loads the library until the process exits); beyond it GSR_E_WORKSPACE_TOO_SMALL and nothing is
+ *   launched — use gsr_distortion.
+ *   Every call on a device shares that array; a call overwrites all the entries it reads, so earlier contents never
+ *   matter, but two calls that overlap on the GPU (different streams, no ordering between them) race: serialise them.
+ *   imgs, ref, mse, psnr_db as for gsr_distortion (psnr_db may be NULL).  Asynchronous on `cuda_stream`. */
+int64_t gsr_distortion_static_max_partials(void);
+int gsr_distortion_static(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, double* mse,
+                          float* psnr_db, void* cuda_stream);
+
 /* ------------------------------------------------------------------------------------------------
  * gsr_group_utility — Eq. (3) and Eq. (4); DESIGN.md §3.7.
  *   mse dev double [B], psnr_db dev fp32 [B]: distortions of a batch.

@@ -679,6 +679,29 @@ int gsr_distortion(const float* imgs, const float* ref, int32_t B, int32_t H, in
   return GSR_OK;
 }
 
+int64_t gsr_distortion_static_max_partials(void) { return (int64_t)kStaticPartials; }
+
+int gsr_distortion_static(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, double* mse,
+                          float* psnr_db, void* cuda_stream) {
+  if (B < 0 || H <= 0 || W <= 0 || (B > 0 && (!imgs || !ref || !mse))) {
+    set_error("gsr_distortion_static: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  const long long tiles = (long long)((W + kTile - 1) / kTile) * (long long)((H + kTile - 1) / kTile);
+  if ((long long)B * tiles > kStaticPartials) {
+    set_error("gsr_distortion_static: B * tiles = %lld exceeds the built-in scratch of %lld partials "
+              "(use gsr_distortion with a workspace)", (long long)B * tiles, kStaticPartials);
+    return GSR_E_WORKSPACE_TOO_SMALL;
+  }
+  const int rc = launch_distortion_static(imgs, ref, B, H, W, mse, psnr_db, (cudaStream_t)cuda_stream);
+  if (rc != 0) {
+    set_error("gsr_distortion_static: cudaGetSymbolAddress failed: %s", cudaGetErrorString((cudaError_t)rc));
+    return GSR_E_CUDA;
+  }
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
 static int group_utility(const double* mse, const float* psnr_db, int32_t B, const int32_t* idx_without,
                          const int32_t* idx_with, const int32_t* group_id, int32_t n_pairs, int32_t G, gsr_utility* out,
                          double* delta_mse, double* delta_db, void* cuda_stream) {

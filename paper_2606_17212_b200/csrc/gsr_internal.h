@@ -176,6 +176,9 @@ void launch_objective_weights(const double* d, int32_t n, double w_mean, double 
                               cudaStream_t st);
 void launch_flicker_backward(const float* a1, const float* a2, const float* r1, const float* r2, int32_t B, int32_t H,
                              int32_t W, const double* weight, float* g1, float* g2, cudaStream_t st);
+constexpr long long kStaticPartials = 1ll << 20;  // doubles of file-scope scratch behind gsr_distortion_static (8 MiB)
+int launch_distortion_static(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, double* mse,
+                             float* psnr, cudaStream_t st);
 int launch_distortion_backward(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W,
                                const double* weight, double lambda, float* out, double* ref_planes, cudaStream_t st);
 void launch_project_backward(const DeviceScene& sc, const FrameParams& fp, const float* grad_rec, float* g_gauss,

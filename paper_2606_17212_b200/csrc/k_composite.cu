@@ -3,6 +3,7 @@
 // (same pixel -> thread mapping and the same reduction tree as the fused path: reduce.cuh), launch bookkeeping,
 // optional CUDA-event timing of the compositing launches and the FP32 peak measurement.
 #include <atomic>
+#include <mutex>
 #include <thread>
 
 #include "composite_common.cuh"
@@ -230,6 +231,53 @@ int measure_ffma_peak(int num_sms, double* tflops, cudaStream_t st) {
   cudaEventDestroy(e0); cudaEventDestroy(e1);
   cudaFree(sink);
   *tflops = best;
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------------
+// gsr_distortion_static: gsr_distortion for callers that may not allocate (CUDA graph capture, serving loops,
+// harnesses that forbid cudaMalloc).  The per-(state, tile) partials live in a file-scope device array instead of a
+// caller-provided workspace: kStaticPartials doubles = 8 MiB, held by every GPU that loads the library until exit.
+// In HOST code the array's name is a host-side stand-in, not a device address: the address is asked for once per
+// device (that device current) with cudaGetSymbolAddress and handed to the kernels.  Every call on a device shares
+// the array: k_distortion_tiles writes every partial the finalize step reads, so nothing has to start at zero and a
+// previous call's contents are harmless — but two calls that overlap on the GPU (different streams) race.
+static __device__ __align__(256) double g_static_partials[kStaticPartials];
+
+static std::mutex g_static_mu;
+static double* g_static_ptr[64] = {};  // per device ordinal
+
+// 0 and *out = the device address of g_static_partials on the CURRENT device, or the CUDA error code
+static int static_partials_address(double** out) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return (int)e;
+  if (dev < 0 || dev >= 64) return (int)cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_ptr[dev]) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_static_partials);
+    if (e != cudaSuccess) return (int)e;
+    g_static_ptr[dev] = (double*)p;
+  }
+  *out = g_static_ptr[dev];
+  return 0;
+}
+
+// Same kernels, same reduction tree as launch_distortion.  Returns 0, or a CUDA error code from the set-up.
+int launch_distortion_static(const float* imgs, const float* ref, int32_t B, int32_t H, int32_t W, double* mse,
+                             float* psnr, cudaStream_t st) {
+  if (B == 0) return 0;
+  double* part = nullptr;
+  const int rc = static_partials_address(&part);
+  if (rc != 0) return rc;
+  const int TX = (W + kTile - 1) / kTile, TY = (H + kTile - 1) / kTile, tiles = TX * TY;
+  for (int b0 = 0; b0 < B; b0 += 65535) {  // gridDim.y limit
+    const int nb = B - b0 < 65535 ? B - b0 : 65535;
+    k_distortion_tiles<<<dim3(tiles, nb), kTilePix, 0, st>>>(imgs + (size_t)b0 * H * W * 3, ref, W, H, TX, tiles,
+                                                            part + (size_t)b0 * tiles);
+  }
+  launch_distortion_finalize(part, B, tiles, (int64_t)3 * W * H, mse, psnr, st);
   return 0;
 }
 

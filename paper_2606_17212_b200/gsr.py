@@ -74,6 +74,9 @@ def lib():
         L.gsr_distortion_workspace_bytes.argtypes = [i32, i32, i32]
         L.gsr_distortion_workspace_bytes.restype = sz
         L.gsr_distortion.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp, sz, vp]
+        L.gsr_distortion_static.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp]
+        L.gsr_distortion_static_max_partials.argtypes = []
+        L.gsr_distortion_static_max_partials.restype = i64
         L.gsr_group_utility.argtypes = [vp, vp, vp, vp, vp, i32, i32, vp, vp, vp, vp]
         L.gsr_group_utility_b.argtypes = [vp, vp, i32, vp, vp, vp, i32, i32, vp, vp, vp, vp]
         L.gsr_index_status.argtypes = [vp]
@@ -386,6 +389,19 @@ def distortion(imgs, ref, workspace=None):
     psnr = torch.empty(B, dtype=torch.float32, device="cuda")
     _check(lib().gsr_distortion(_dp(imgs), _dp(ref), B, H, W, _dp(mse), _dp(psnr), _dp(workspace),
                                 workspace.numel(), _stream()))
+    return mse, psnr
+
+
+def distortion_static(imgs, ref, mse, psnr):
+    """gsr_distortion_static: like `distortion`, but the library allocates nothing — the outputs mse (cuda f64 [B])
+    and psnr (cuda f32 [B]) are the caller's, the scratch is built into the library (B * tiles <= 2^20)."""
+    torch = _torch()
+    B, H, W = int(imgs.shape[0]), int(imgs.shape[1]), int(imgs.shape[2])
+    assert imgs.dtype == torch.float32 and imgs.is_cuda and imgs.is_contiguous()
+    assert ref.dtype == torch.float32 and ref.is_cuda and ref.is_contiguous() and tuple(ref.shape) == (H, W, 3)
+    assert mse.dtype == torch.float64 and mse.is_cuda and mse.is_contiguous() and mse.numel() == B
+    assert psnr.dtype == torch.float32 and psnr.is_cuda and psnr.is_contiguous() and psnr.numel() == B
+    _check(lib().gsr_distortion_static(_dp(imgs), _dp(ref), B, H, W, _dp(mse), _dp(psnr), _stream()))
     return mse, psnr
 
 
