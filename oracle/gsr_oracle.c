@@ -814,13 +814,23 @@ void orc_sh_basis_grad(int32_t K, double x, double y, double z, double* Yx, doub
  *   dL/dA0 = g_A, dL/dA1 = t g_A), g_sc [C].
  * margin [N] (overwritten where the Gaussian is present): the smallest relative distance of a decision from its
  * threshold — a caller comparing against an fp32 implementation skips Gaussians whose margin is tiny.
- * Returns 0, or -1 for scenes this oracle does not cover (position residual levels, per-level attribute
- * refinements, affine on the covariance). */
+ * The rest of the representation: position residual levels (g_delta2, g_delta3 [N,3]: dL/dmu of the
+ * states that apply them), per-level colour residuals (g_dsh [3][N,K,3]: level l collects the states of depth >= l),
+ * the affine on the covariance (reading I4: Su = L Sigma L^T adds (G + G^T) L Sigma to the linear part of g_A), and
+ * per-level attribute refinements: ls_lv / quat_lv / logit_lv = the raw attributes per delivered depth [4][N,.] (base +
+ * residuals of levels 1..d), and g_ls / g_quat / g_logit are then [4][N,.] too — the state's gradient goes to row
+ * depth; the caller folds: base = sum over depths, residual level l = sum over depths >= l.
+ * Returns 0, or -1 if a scene with such terms comes without the arrays they need. */
 int32_t orc_project_backward_O9(const orc_scene* s, const float* log_scale, const float* quat, const float* logit,
                                 const orc_camera* cam, float t, const int8_t* depth, const double* g9,
                                 double* g_mean, double* g_rho, double* g_ls, double* g_quat, double* g_logit,
-                                double* g_shb, double* g_shr, double* g_A, double* g_sc, double* margin) {
-  if (s->delta2 || s->delta3 || s->cov3d_lv || s->d_sh || s->affine_cov) return -1;
+                                double* g_shb, double* g_shr, double* g_A, double* g_sc, double* margin,
+                                const float* ls_lv, const float* quat_lv, const float* logit_lv, double* g_delta2,
+                                double* g_delta3, double* g_dsh) {
+  /* the full representation: a scene with per-level attribute refinements must come with its
+   * raw per-depth parameters, one with position / colour residual levels with the arrays that receive their gradients */
+  if ((s->cov3d_lv != 0) != (ls_lv != 0) || (ls_lv != 0) != (quat_lv != 0) || (ls_lv != 0) != (logit_lv != 0)) return -1;
+  if ((s->delta2 && !g_delta2) || (s->delta3 && !g_delta3) || (s->d_sh && !g_dsh)) return -1;
   float basis_f[64];
   orc_basis(t, s->R, basis_f);
   double Rw[9], tw[3];
@@ -840,10 +850,15 @@ int32_t orc_project_backward_O9(const orc_scene* s, const float* log_scale, cons
 
       /* ================= forward, in double ================= */
       /* O-0 */
+      /* raw attributes of this state's depth: the base, or base + the residuals of levels 1..d (reading I2; summed
+       * in binary32 by the caller exactly as the forward oracle's activation sees them); ia = their row */
+      const int64_t ia = ls_lv ? (int64_t)d * s->N + i : (int64_t)i;
+      const float* ls_p = ls_lv ? ls_lv : log_scale;
+      const float* qt_p = quat_lv ? quat_lv : quat;
+      const float* lg_p = logit_lv ? logit_lv : logit;
       double sc3[3];
-      for (int k = 0; k < 3; ++k) sc3[k] = exp((double)log_scale[3 * (int64_t)i + k]);
-      const double qw = quat[4 * (int64_t)i + 0], qx = quat[4 * (int64_t)i + 1], qy = quat[4 * (int64_t)i + 2],
-                   qz = quat[4 * (int64_t)i + 3];
+      for (int k = 0; k < 3; ++k) sc3[k] = exp((double)ls_p[3 * ia + k]);
+      const double qw = qt_p[4 * ia + 0], qx = qt_p[4 * ia + 1], qy = qt_p[4 * ia + 2], qz = qt_p[4 * ia + 3];
       const double qn = sqrt(qw * qw + qx * qx + qy * qy + qz * qz);
       const double w = qw / qn, x = qx / qn, y = qy / qn, z = qz / qn;
       const double Rm[9] = {1.0 - 2.0 * (y * y + z * z), 2.0 * (x * y - w * z),       2.0 * (x * z + w * y),
@@ -855,7 +870,7 @@ int32_t orc_project_backward_O9(const orc_scene* s, const float* log_scale, cons
       for (int a = 0; a < 3; ++a)
         for (int b = 0; b < 3; ++b)
           Sg[3 * a + b] = Mm[3 * a + 0] * Mm[3 * b + 0] + Mm[3 * a + 1] * Mm[3 * b + 1] + Mm[3 * a + 2] * Mm[3 * b + 2];
-      const double opac = 1.0 / (1.0 + exp(-(double)logit[i]));
+      const double opac = 1.0 / (1.0 + exp(-(double)lg_p[ia]));
       /* O-2 */
       double A[12];
       for (int k = 0; k < 12; ++k) A[k] = (double)s->A0[12 * c + k] + (double)t * (double)s->A1[12 * c + k];
@@ -866,6 +881,19 @@ int32_t orc_project_backward_O9(const orc_scene* s, const float* log_scale, cons
         acc[k] = 0.0;
         for (int r = 0; r < s->R; ++r) acc[k] += (double)basis_f[r] * (double)s->motion_q[((int64_t)i * s->R + r) * 3 + k];
         mu[k] = d >= 1 ? p + (double)s->motion_scale[c] * acc[k] : p;
+        if (d >= 2 && s->delta2) mu[k] += (double)s->delta2[3 * (int64_t)i + k];
+        if (d >= 3 && s->delta3) mu[k] += (double)s->delta3[3 * (int64_t)i + k];
+      }
+      /* reading I4 (optional): the cluster affine also transforms the covariance, Su = L Sg L^T, L = A[:, :3] */
+      double Su[9], LS[9];
+      for (int a = 0; a < 9; ++a) Su[a] = Sg[a];
+      if (s->affine_cov) {
+        for (int a = 0; a < 3; ++a)
+          for (int b = 0; b < 3; ++b)
+            LS[3 * a + b] = A[4 * a + 0] * Sg[0 + b] + A[4 * a + 1] * Sg[3 + b] + A[4 * a + 2] * Sg[6 + b];
+        for (int a = 0; a < 3; ++a)
+          for (int b = 0; b < 3; ++b)
+            Su[3 * a + b] = LS[3 * a + 0] * A[4 * b + 0] + LS[3 * a + 1] * A[4 * b + 1] + LS[3 * a + 2] * A[4 * b + 2];
       }
       /* O-3 */
       double pc[3];
@@ -886,8 +914,8 @@ int32_t orc_project_backward_O9(const orc_scene* s, const float* log_scale, cons
         M1[k] = J11 * Rw[3 + k] + J12 * Rw[6 + k];
       }
       for (int a = 0; a < 3; ++a) {
-        v0[a] = Sg[3 * a + 0] * M0[0] + Sg[3 * a + 1] * M0[1] + Sg[3 * a + 2] * M0[2];
-        v1[a] = Sg[3 * a + 0] * M1[0] + Sg[3 * a + 1] * M1[1] + Sg[3 * a + 2] * M1[2];
+        v0[a] = Su[3 * a + 0] * M0[0] + Su[3 * a + 1] * M0[1] + Su[3 * a + 2] * M0[2];
+        v1[a] = Su[3 * a + 0] * M1[0] + Su[3 * a + 1] * M1[1] + Su[3 * a + 2] * M1[2];
       }
       const double s00 = M0[0] * v0[0] + M0[1] * v0[1] + M0[2] * v0[2];
       const double s01 = M0[0] * v1[0] + M0[1] * v1[1] + M0[2] * v1[2];
@@ -908,6 +936,9 @@ int32_t orc_project_backward_O9(const orc_scene* s, const float* log_scale, cons
         for (int j = 0; j < s->K; ++j) {
           double coef = (double)s->sh_base[((int64_t)i * s->K + j) * 3 + ch];
           if (d >= 3) coef += (double)s->sh_res[((int64_t)i * s->K + j) * 3 + ch];
+          if (s->d_sh)
+            for (int l = 1; l <= d && l <= 3; ++l)
+              coef += (double)s->d_sh[(((int64_t)(l - 1) * s->N + i) * s->K + j) * 3 + ch];
           Sch[ch] += Y[j] * coef;
         }
         mg = fmin(mg, fabs(Sch[ch]));
@@ -925,6 +956,11 @@ int32_t orc_project_backward_O9(const orc_scene* s, const float* log_scale, cons
           for (int ch = 0; ch < 3; ++ch) {
             double coef = (double)s->sh_base[((int64_t)i * s->K + j) * 3 + ch];
             if (d >= 3) coef += (double)s->sh_res[((int64_t)i * s->K + j) * 3 + ch];
+            if (s->d_sh)
+              for (int l = 1; l <= d && l <= 3; ++l) {
+                coef += (double)s->d_sh[(((int64_t)(l - 1) * s->N + i) * s->K + j) * 3 + ch];
+                g_dsh[(((int64_t)(l - 1) * s->N + i) * s->K + j) * 3 + ch] += Y[j] * g[ch];
+              }
             dY[j] += dS[ch] * coef;
             g_shb[((int64_t)i * s->K + j) * 3 + ch] += Y[j] * dS[ch];
             if (d >= 3) g_shr[((int64_t)i * s->K + j) * 3 + ch] += Y[j] * dS[ch];
@@ -941,7 +977,7 @@ int32_t orc_project_backward_O9(const orc_scene* s, const float* log_scale, cons
         for (int k = 0; k < 3; ++k) dmu[k] += (gdir[k] - dir[k] * dot) / nrm;
       }
       /* opacity = sigmoid(logit) */
-      g_logit[i] += g[3] * opac * (1.0 - opac);
+      g_logit[ia] += g[3] * opac * (1.0 - opac);
       /* A = conic_a / 2, B = conic_b, Cq = conic_c / 2; conic = (c, -b, a) / det, det = a c - b^2 */
       const double gca = 0.5 * g[4], gcb = g[5], gcc = 0.5 * g[6];
       const double det2 = det * det;
@@ -954,6 +990,24 @@ int32_t orc_project_backward_O9(const orc_scene* s, const float* log_scale, cons
         for (int b = 0; b < 3; ++b) G[3 * a + b] = da * M0[a] * M0[b] + db * M0[a] * M1[b] + dc * M1[a] * M1[b];
         dM0[a] = 2.0 * da * v0[a] + db * v1[a];
         dM1[a] = 2.0 * dc * v1[a] + db * v0[a];
+      }
+      if (s->affine_cov) {
+        /* Su = L Sg L^T: dL/dL = (G + G^T) (L Sg) (Sg symmetric), dL/dSg = L^T G L */
+        double Gs[9];
+        for (int r = 0; r < 3; ++r)
+          for (int cc = 0; cc < 3; ++cc) {
+            double acc2 = 0.0;
+            for (int q = 0; q < 3; ++q) acc2 += (G[3 * r + q] + G[3 * q + r]) * LS[3 * q + cc];
+            g_A[12 * c + 4 * r + cc] += acc2;
+          }
+        for (int a = 0; a < 3; ++a)
+          for (int b = 0; b < 3; ++b) {
+            double acc2 = 0.0;
+            for (int pp = 0; pp < 3; ++pp)
+              for (int q = 0; q < 3; ++q) acc2 += G[3 * pp + q] * A[4 * pp + a] * A[4 * q + b];
+            Gs[3 * a + b] = acc2;
+          }
+        for (int a = 0; a < 9; ++a) G[a] = Gs[a];
       }
       /* M0 = J00 R_0 + J02 R_2, M1 = J11 R_1 + J12 R_2 */
       double dJ00 = 0.0, dJ02 = 0.0, dJ11 = 0.0, dJ12 = 0.0;
@@ -980,6 +1034,9 @@ int32_t orc_project_backward_O9(const orc_scene* s, const float* log_scale, cons
       dpc[2] = dzc;
       /* pc = R mu + t */
       for (int k = 0; k < 3; ++k) dmu[k] += Rw[0 + k] * dpc[0] + Rw[3 + k] * dpc[1] + Rw[6 + k] * dpc[2];
+      /* Eq. (1) "+ delta^(2) + delta^(3)": each applied residual moves mu one to one */
+      if (d >= 2 && s->delta2) for (int k = 0; k < 3; ++k) g_delta2[3 * (int64_t)i + k] += dmu[k];
+      if (d >= 3 && s->delta3) for (int k = 0; k < 3; ++k) g_delta3[3 * (int64_t)i + k] += dmu[k];
       /* Eq. (1): mu = p + [d >= 1] s_c acc, p = A [mu_bar; 1] */
       if (d >= 1) {
         for (int k = 0; k < 3; ++k) {
@@ -1007,7 +1064,7 @@ int32_t orc_project_backward_O9(const orc_scene* s, const float* log_scale, cons
           ds += dMm[3 * a + k] * Rm[3 * a + k];
           dRm[3 * a + k] = dMm[3 * a + k] * sc3[k];
         }
-        g_ls[3 * (int64_t)i + k] += ds * sc3[k];
+        g_ls[3 * ia + k] += ds * sc3[k];
       }
       /* Rm(w, x, y, z) entry by entry (the matrix written in O-0) */
       const double dw = dRm[1] * (-2.0 * z) + dRm[2] * (2.0 * y) + dRm[3] * (2.0 * z) + dRm[5] * (-2.0 * x) +
@@ -1020,10 +1077,10 @@ int32_t orc_project_backward_O9(const orc_scene* s, const float* log_scale, cons
                          dRm[4] * (-4.0 * z) + dRm[5] * (2.0 * y) + dRm[6] * (2.0 * x) + dRm[7] * (2.0 * y);
       /* (w, x, y, z) = quat / |quat| */
       const double qd = w * dw + x * dx_ + y * dy_ + z * dz_;
-      g_quat[4 * (int64_t)i + 0] += (dw - w * qd) / qn;
-      g_quat[4 * (int64_t)i + 1] += (dx_ - x * qd) / qn;
-      g_quat[4 * (int64_t)i + 2] += (dy_ - y * qd) / qn;
-      g_quat[4 * (int64_t)i + 3] += (dz_ - z * qd) / qn;
+      g_quat[4 * ia + 0] += (dw - w * qd) / qn;
+      g_quat[4 * ia + 1] += (dx_ - x * qd) / qn;
+      g_quat[4 * ia + 2] += (dy_ - y * qd) / qn;
+      g_quat[4 * ia + 3] += (dz_ - z * qd) / qn;
     }
   return 0;
 }

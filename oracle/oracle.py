@@ -160,16 +160,20 @@ class OracleScene:
         # order in binary32, then activated exactly like the base (O-0)
         refs = [getattr(sc, n, None) for n in ("d_log_scale", "d_quat", "d_opacity_logit")]
         s.cov3d_lv = s.opacity_lv = s.tau_lv = None
+        self.raw_lv = None
         if any(r is not None for r in refs):
             cur = [ls.copy(), qt.copy(), lg.copy()]
             self.cov3d_lv = np.empty((4, self.N, 6), np.float32)
             self.opacity_lv = np.empty((4, self.N), np.float32)
             self.tau_lv = np.empty((4, self.N), np.float32)
+            self.raw_lv = [np.empty((4,) + c.shape, np.float32) for c in cur]   # raw attributes per delivered depth
             for v in range(4):
                 if v >= 1:
                     for k, r in enumerate(refs):
                         if r is not None:
                             cur[k] = (cur[k] + _c(r[v - 1], np.float32).reshape(cur[k].shape)).astype(np.float32)
+                for k in range(3):
+                    self.raw_lv[k][v] = cur[k]
                 L.orc_activate(C.c_int64(self.N), _p(_c(cur[0], np.float32)), _p(_c(cur[1], np.float32)),
                                _p(_c(cur[2], np.float32)), _p(self.cov3d_lv[v]), _p(self.opacity_lv[v]),
                                _p(self.tau_lv[v]))
@@ -230,28 +234,45 @@ class OracleScene:
         return (grad, gabs) if want_abs else grad
 
     PARAM_GRADS = ("mean", "rho", "log_scale", "quat", "opacity_logit", "sh_base", "sh_res", "A", "motion_scale")
+    FULL_GRADS = ("delta2", "delta3", "d_log_scale", "d_quat", "d_opacity_logit", "d_sh")
 
     def project_backward(self, cam, t: float, depth, g9, into: dict | None = None):
         """orc_project_backward_O9: g9 = dL/d(rgb[3], opacity, A, B, Cq, m_x, m_y) double [N,9] of ONE state (the
         output of `backward`) -> dict of double gradients with respect to the scene's parameters (PARAM_GRADS:
         mean [N,3], rho [N,3] (motion residual vector), log_scale [N,3], quat [N,4], opacity_logit [N],
-        sh_base / sh_res [N,K,3], A [C,3,4] (A_c(t)), motion_scale [C]) plus "margin" [N].  `into` accumulates."""
+        sh_base / sh_res [N,K,3], A [C,3,4] (A_c(t)), motion_scale [C]; and, where the scene has them, FULL_GRADS:
+        delta2 / delta3 [N,3], d_log_scale [3,N,3], d_quat [3,N,4], d_opacity_logit [3,N], d_sh [3,N,K,3]) plus
+        "margin" [N].  `into` accumulates."""
         d = _c(depth, np.int8)
         g = _c(g9, np.float64)
         assert d.shape == (self.C,) and g.shape == (self.N, 9)
+        N, K = self.N, self.K
         out = into if into is not None else {
-            "mean": np.zeros((self.N, 3)), "rho": np.zeros((self.N, 3)), "log_scale": np.zeros((self.N, 3)),
-            "quat": np.zeros((self.N, 4)), "opacity_logit": np.zeros(self.N),
-            "sh_base": np.zeros((self.N, self.K, 3)), "sh_res": np.zeros((self.N, self.K, 3)),
-            "A": np.zeros((self.C, 3, 4)), "motion_scale": np.zeros(self.C), "margin": np.full(self.N, np.inf)}
-        margin = np.full(self.N, np.inf)
+            "mean": np.zeros((N, 3)), "rho": np.zeros((N, 3)), "log_scale": np.zeros((N, 3)),
+            "quat": np.zeros((N, 4)), "opacity_logit": np.zeros(N),
+            "sh_base": np.zeros((N, K, 3)), "sh_res": np.zeros((N, K, 3)),
+            "A": np.zeros((self.C, 3, 4)), "motion_scale": np.zeros(self.C), "margin": np.full(N, np.inf),
+            "delta2": np.zeros((N, 3)), "delta3": np.zeros((N, 3)), "d_log_scale": np.zeros((3, N, 3)),
+            "d_quat": np.zeros((3, N, 4)), "d_opacity_logit": np.zeros((3, N)), "d_sh": np.zeros((3, N, K, 3))}
+        margin = np.full(N, np.inf)
+        lv = self.raw_lv is not None
+        # per-depth attribute gradients of this state (row = the state's depth of the Gaussian's cluster)
+        g_ls = np.zeros((4, N, 3)) if lv else out["log_scale"]
+        g_qt = np.zeros((4, N, 4)) if lv else out["quat"]
+        g_lg = np.zeros((4, N)) if lv else out["opacity_logit"]
         rc = lib().orc_project_backward_O9(
             C.byref(self._s), _p(self.log_scale), _p(self.quat), _p(self.opacity_logit), C.byref(make_camera(cam)),
-            C.c_float(t), _p(d), _p(g), _p(out["mean"]), _p(out["rho"]), _p(out["log_scale"]), _p(out["quat"]),
-            _p(out["opacity_logit"]), _p(out["sh_base"]), _p(out["sh_res"]), _p(out["A"]), _p(out["motion_scale"]),
-            _p(margin))
+            C.c_float(t), _p(d), _p(g), _p(out["mean"]), _p(out["rho"]), _p(g_ls), _p(g_qt), _p(g_lg),
+            _p(out["sh_base"]), _p(out["sh_res"]), _p(out["A"]), _p(out["motion_scale"]), _p(margin),
+            _p(self.raw_lv[0]) if lv else None, _p(self.raw_lv[1]) if lv else None, _p(self.raw_lv[2]) if lv else None,
+            _p(out["delta2"]), _p(out["delta3"]), _p(out["d_sh"]))
         if rc != 0:
-            raise ValueError("orc_project_backward_O9 does not cover this scene (residual levels / refinements)")
+            raise ValueError("orc_project_backward_O9: inconsistent optional arrays")
+        if lv:   # fold: the attributes at depth v are base + levels 1..v
+            for name, arr in (("log_scale", g_ls), ("quat", g_qt), ("opacity_logit", g_lg)):
+                out[name] += arr.sum(0)
+                for l in (1, 2, 3):
+                    out["d_" + name][l - 1] += arr[l:].sum(0)
         out["margin"] = np.minimum(out["margin"], margin)
         return out
 

@@ -285,3 +285,97 @@ def test_c7_colour_only_functional_isolates_the_view_direction_path(oracle_mod):
     for i in np.nonzero(valid0 == 1)[0][:10]:
         dmu = np.linalg.solve(A[cl[i], :, :3].T, grads["mean"][i])
         assert abs(dmu @ v[i]) <= 1e-5 * np.linalg.norm(dmu) * np.linalg.norm(v[i])
+
+
+FULL_FAMILIES = [("mean", "mean", 4e-3), ("log_scale", "log_scale", 1e-2), ("quat", "quat", 1e-2),
+                 ("opacity_logit", "opacity_logit", 2e-2), ("sh_base", "sh_base", 2e-2), ("sh_res", "sh_res", 2e-2),
+                 ("A0", "A", 4e-3), ("A1", "A", 4e-3),
+                 ("delta2", "delta2", 4e-3), ("delta3", "delta3", 4e-3), ("d_log_scale", "d_log_scale", 1e-2),
+                 ("d_quat", "d_quat", 1e-2), ("d_opacity_logit", "d_opacity_logit", 2e-2), ("d_sh", "d_sh", 2e-2)]
+
+
+@pytest.mark.parametrize("affine", [False, True])
+def test_c8_full_representation_against_central_differences(oracle_mod, affine):
+    """The rest of the representation: position residual levels, per-level scale / rotation / opacity /
+    colour refinements and, optionally, the affine on the covariance — a mixed state (cluster depths 3, 2, 1) so that
+    every level's residual is applied by some cluster and skipped by another."""
+    base, cam, t = small_workload()
+    scn = synth.with_attribute_refinements(synth.with_position_residuals(base))
+    scn = dataclasses.replace(scn, affine_on_covariance=affine)
+    depth = np.array([3, 2, 1], np.int8)
+    rng = np.random.default_rng(300 + int(affine))
+    w = rng.standard_normal((scn.N, 9))
+    L0, p0 = functional(oracle_mod, scn, cam, t, depth, w)
+    valid0 = p0["valid"].copy()
+    assert valid0.sum() > 20
+    sc = oracle_mod.OracleScene(scn)
+    grads = sc.project_backward(cam, t, depth, np.where((valid0 == 1)[:, None], w, 0.0))
+    assert grads["margin"][valid0 == 1].min() > 1e-3
+    for field, gname, h in FULL_FAMILIES:
+        theta = np.asarray(getattr(scn, field), np.float32)
+        for trial in range(2):
+            u = rng.standard_normal(theta.shape)
+            tp = (theta.astype(np.float64) + h * u).astype(np.float32)
+            tm = (theta.astype(np.float64) - h * u).astype(np.float32)
+            delta = tp.astype(np.float64) - tm.astype(np.float64)
+            Lp, _ = functional(oracle_mod, dataclasses.replace(scn, **{field: tp}), cam, t, depth, w, valid0)
+            Lm, _ = functional(oracle_mod, dataclasses.replace(scn, **{field: tm}), cam, t, depth, w, valid0)
+            g = grads[gname].reshape(theta.shape).copy()
+            if field == "A1":
+                g = t * g
+            pred = float((g * delta).sum())
+            mag = float(np.abs(g * delta).sum())
+            assert mag > 0.0
+            assert abs((Lp - Lm) - pred) <= 5e-3 * mag + 1e-4 * abs(Lp - Lm) + 2e-3, (field, trial, Lp - Lm, pred, mag)
+    # which states feed which level: cluster 0 (depth 3) feeds all three levels, cluster 1 (depth 2) levels 1-2,
+    # cluster 2 (depth 1) level 1 only; delta3 only from cluster 0, delta2 from clusters 0 and 1
+    cl = scn.cluster_of()
+    live = valid0 == 1
+    for name in ("d_log_scale", "d_quat", "d_opacity_logit", "d_sh"):
+        g = grads[name].reshape(3, scn.N, -1)
+        assert np.any(g[2][(cl == 0) & live] != 0.0) and np.all(g[2][cl != 0] == 0.0)
+        assert np.any(g[1][(cl == 1) & live] != 0.0) and np.all(g[1][cl == 2] == 0.0)
+        assert np.any(g[0][(cl == 2) & live] != 0.0)
+    assert np.all(grads["delta3"][cl != 0] == 0.0) and np.any(grads["delta3"][cl == 0] != 0.0)
+    assert np.all(grads["delta2"][cl == 2] == 0.0) and np.any(grads["delta2"][cl == 1] != 0.0)
+    # a residual that is applied moves mu exactly like rho does
+    assert np.allclose(grads["delta2"][cl == 1], grads["rho"][cl == 1], rtol=1e-12, atol=0.0)
+    # base attribute gradient = the sum over all depths; level-1 residual = the same here (every cluster has depth >= 1)
+    assert np.allclose(grads["d_log_scale"][0], grads["log_scale"], rtol=1e-12, atol=0.0)
+
+
+def test_c9_affine_on_the_covariance_isolated_on_the_conic(oracle_mod):
+    """Reading I4 with a cluster affine far from the identity (linear part I + 0.3 N(0,1) + t A1) and a functional
+    of the conic alone (values ~0.1, so the forward oracle's fp32 noise is ~1e-6 and the bar has no room for a missing
+    4 % term): the covariance path into A (dL/dL = (G + G^T) L Sigma) and into scale / rotation (dL/dSigma = L^T G L)."""
+    base, cam, t = small_workload()
+    rng = np.random.default_rng(77)
+    A0 = base.A0.copy()
+    A0[:, :, :3] += (0.3 * rng.standard_normal((base.C, 3, 3))).astype(np.float32)
+    scn = dataclasses.replace(synth.with_attribute_refinements(base), A0=A0, affine_on_covariance=True)
+    depth = np.array([3, 1, 2], np.int8)
+    w = np.zeros((scn.N, 9))
+    w[:, 4:7] = rng.standard_normal((scn.N, 3))
+    L0, p0 = functional(oracle_mod, scn, cam, t, depth, w)
+    valid0 = p0["valid"].copy()
+    assert valid0.sum() > 20
+    sc = oracle_mod.OracleScene(scn)
+    grads = sc.project_backward(cam, t, depth, np.where((valid0 == 1)[:, None], w, 0.0))
+    for field, gname, h in (("A0", "A", 2e-3), ("A1", "A", 4e-3), ("log_scale", "log_scale", 5e-3), ("quat", "quat", 5e-3),
+                            ("d_log_scale", "d_log_scale", 5e-3), ("d_quat", "d_quat", 5e-3), ("mean", "mean", 2e-3)):
+        theta = np.asarray(getattr(scn, field), np.float32)
+        for trial in range(3):
+            u = rng.standard_normal(theta.shape)
+            if field in ("A0", "A1") and trial == 0:
+                u[:, :, 3] = 0.0                                # the linear part alone
+            tp = (theta.astype(np.float64) + h * u).astype(np.float32)
+            tm = (theta.astype(np.float64) - h * u).astype(np.float32)
+            delta = tp.astype(np.float64) - tm.astype(np.float64)
+            Lp, _ = functional(oracle_mod, dataclasses.replace(scn, **{field: tp}), cam, t, depth, w, valid0)
+            Lm, _ = functional(oracle_mod, dataclasses.replace(scn, **{field: tm}), cam, t, depth, w, valid0)
+            g = grads[gname].reshape(theta.shape).copy()
+            if field == "A1":
+                g = t * g
+            pred = float((g * delta).sum())
+            mag = float(np.abs(g * delta).sum())
+            assert abs((Lp - Lm) - pred) <= 5e-3 * mag + 1e-5, (field, trial, Lp - Lm, pred, mag)
