@@ -959,7 +959,7 @@ int32_t orc_project_backward_O9(const orc_scene* s, const float* log_scale, cons
             if (s->d_sh)
               for (int l = 1; l <= d && l <= 3; ++l) {
                 coef += (double)s->d_sh[(((int64_t)(l - 1) * s->N + i) * s->K + j) * 3 + ch];
-                g_dsh[(((int64_t)(l - 1) * s->N + i) * s->K + j) * 3 + ch] += Y[j] * g[ch];
+                g_dsh[(((int64_t)(l - 1) * s->N + i) * s->K + j) * 3 + ch] += Y[j] * dS[ch];
               }
             dY[j] += dS[ch] * coef;
             g_shb[((int64_t)i * s->K + j) * 3 + ch] += Y[j] * dS[ch];

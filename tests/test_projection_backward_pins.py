@@ -379,3 +379,33 @@ def test_c9_affine_on_the_covariance_isolated_on_the_conic(oracle_mod):
             pred = float((g * delta).sum())
             mag = float(np.abs(g * delta).sum())
             assert abs((Lp - Lm) - pred) <= 5e-3 * mag + 1e-5, (field, trial, Lp - Lm, pred, mag)
+
+
+def test_c10_colour_refinement_levels_respect_the_clamp_and_the_depth(oracle_mod):
+    """One Gaussian with a channel below zero (rgb = max(0, .) = 0) and per-level colour residuals, at depth 2: the
+    clamped channel passes nothing to any level; the live channel passes the same row Y_j to sh_base and to the
+    residuals of levels 1 and 2 — and nothing to level 3, which this state does not contain, nor to sh_res."""
+    cam = axis_camera(64, 64, 100.0, 4.0)
+    scn, _ = tiny_scene([[0.1, 0.07, 0.0]], 0.3, logits=0.5, sh_degree=1,
+                        sh_base=np.array([[[0.3 / Y0, -0.7 / Y0, 0.1 / Y0], [0.1, 0.2, 0.3], [0.2, 0.1, 0.1], [0.3, 0.3, 0.2]]]))
+    dsh = np.zeros((3, 1, 4, 3), np.float32)
+    dsh[:, 0, :, :] = 0.002 * np.arange(1, 37, dtype=np.float32).reshape(3, 4, 3)
+    scn = dataclasses.replace(scn, d_sh=dsh)
+    sc = oracle_mod.OracleScene(scn)
+    depth = np.full(1, 2, np.int8)
+    p = sc.project(cam, 0.0, depth)
+    assert p["rgb"][0][1] == 0.0 and p["rgb"][0][0] > 0.0
+    g9 = np.zeros((1, 9))
+    g9[0, 1] = 1.0                                              # the clamped channel only
+    gr = sc.project_backward(cam, 0.0, depth, g9)
+    assert np.all(gr["d_sh"] == 0.0) and np.all(gr["sh_base"] == 0.0) and np.all(gr["mean"] == 0.0)
+    g9[0, 0] = 1.0
+    gr = sc.project_backward(cam, 0.0, depth, g9)
+    assert np.all(gr["sh_base"][0, :, 0] != 0.0) and np.all(gr["sh_base"][0, :, 1] == 0.0)
+    assert np.array_equal(gr["d_sh"][0][0], gr["sh_base"][0]) and np.array_equal(gr["d_sh"][1][0], gr["sh_base"][0])
+    assert np.all(gr["d_sh"][2] == 0.0) and np.all(gr["sh_res"] == 0.0)
+    # the rows are Y_j(dir) g: against the exported basis at the Gaussian's view direction
+    centre = -(cam.R_wc.astype(np.float64).T @ cam.t_wc.astype(np.float64))
+    v = p["mu"][0].astype(np.float64) - centre
+    Y = oracle_mod.sh_basis(4, v / np.linalg.norm(v))
+    assert np.allclose(gr["sh_base"][0, :, 0], Y, rtol=1e-12, atol=0.0)
