@@ -225,6 +225,22 @@ int gsr_flicker_backward(const float* imgs_t1, const float* imgs_t2, const float
 int gsr_project_backward(const gsr_scene* scene, const gsr_camera* cam, float t, const float* grad_records,
                          float* g_gauss, float* g_sh_base, float* g_sh_res, float* g_cluster, void* cuda_stream);
 
+/* gsr_project_backward_full — gsr_project_backward for every scene, including the full representation of
+ * position residual levels delta2 / delta3, per-level refinements of scale,
+ * rotation, opacity and colour, affine_on_covariance; four records per Gaussian (record 4 i + delivered depth).
+ * grad_records, g_gauss, g_sh_base, g_sh_res, g_cluster as for gsr_project_backward; the log_scale / quat /
+ * opacity_logit / sh_base columns are the gradients of the BASE arrays (every depth contains the base).  In addition
+ * (each may be NULL = not wanted; overwritten; zero where the scene has no such term):
+ *   g_delta dev fp32 [N, 6]        d/d(delta2[3], delta3[3]): dL/dmu of the depths that apply the residual
+ *   g_attr  dev fp32 [3, N, 8]     per refinement level l = 1..3: d/d(d_log_scale[l][3], d_quat[l][4],
+ *                                  d_opacity_logit[l]) = the sum over the depths >= l
+ *   g_d_sh  dev fp32 [3, N, K, 3]  per level: d/d(d_sh[l])
+ * With affine_on_covariance the covariance path (Sigma_t = L Sigma L^T) adds to the linear part of g_cluster.
+ * Scenes with two records per Gaussian are served by the kernel of gsr_project_backward. */
+int gsr_project_backward_full(const gsr_scene* scene, const gsr_camera* cam, float t, const float* grad_records,
+                              float* g_gauss, float* g_sh_base, float* g_sh_res, float* g_cluster, float* g_delta,
+                              float* g_attr, float* g_d_sh, void* cuda_stream);
+
 /* Synchronises `cuda_stream` and reads the status latched by the last render into `workspace`:
  * returns GSR_OK, GSR_E_INVALID_LEVEL or GSR_E_WORKSPACE_TOO_SMALL.  keys_needed (host, may be NULL)
  * receives the number of (tile, depth, record) keys the frame produced. */

@@ -336,6 +336,8 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
   D.V = has_delta ? 4 : 2;
   D.affine_cov = d->affine_on_covariance != 0;
   D.delta = nullptr; D.g1v = nullptr; D.g2v = nullptr; D.opv = nullptr; D.d_sh = nullptr;
+  D.raw_quat_v = nullptr; D.raw_ls_v = nullptr;
+  D.has_delta2 = d->delta2 != nullptr; D.has_delta3 = d->delta3 != nullptr;
   for (int k = 0; k < 3; ++k) D.bg[k] = d->background[k];
   size_t off = 0;
   auto reserve = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
@@ -348,6 +350,7 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
                o_dl = reserve(has_delta ? sizeof(float) * 6 * Np : 0),
                o_g1v = reserve(has_attr ? sizeof(float4) * 4 * Np : 0), o_g2v = reserve(has_attr ? sizeof(float4) * 4 * Np : 0),
                o_opv = reserve(has_attr ? sizeof(float) * 4 * Np : 0),
+               o_rqv = reserve(has_attr ? sizeof(float4) * 4 * Np : 0), o_rlv = reserve(has_attr ? sizeof(float4) * 4 * Np : 0),
                o_dsh = reserve(has_dsh ? sizeof(float4) * 3 * n_sh4 * Np : 0);
   cudaError_t e = cudaMalloc(&sc->impl.blob, off);
   if (e != cudaSuccess) {
@@ -363,7 +366,10 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
   D.raw_quat = (float4*)(base + o_rq); D.raw_ls = (float4*)(base + o_rl);
   if (has_delta) D.delta = (float*)(base + o_dl);
   if (has_dsh) D.d_sh = (float4*)(base + o_dsh);
-  if (has_attr) { D.g1v = (float4*)(base + o_g1v); D.g2v = (float4*)(base + o_g2v); D.opv = (float*)(base + o_opv); }
+  if (has_attr) {
+    D.g1v = (float4*)(base + o_g1v); D.g2v = (float4*)(base + o_g2v); D.opv = (float*)(base + o_opv);
+    D.raw_quat_v = (float4*)(base + o_rqv); D.raw_ls_v = (float4*)(base + o_rlv);
+  }
   bool ok = true;
   auto up = [&](void* dst, const void* src, size_t bytes) {
     if (bytes && cudaMemcpy(dst, src, bytes, cudaMemcpyHostToDevice) != cudaSuccess) ok = false;
@@ -399,7 +405,7 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
     up(D.d_sh, ds.data(), sizeof(float4) * 3 * n_sh4 * Np);
   }
   if (has_attr) {  // per-depth attributes: base + levels 1..v in binary32 (level order), then §3.0 (reading I2)
-    std::vector<float4> a1(4 * Np), a2(4 * Np);
+    std::vector<float4> a1(4 * Np), a2(4 * Np), rqv(4 * Np), rlv(4 * Np);
     std::vector<float> ao(4 * Np);
     for (int i = 0; i < N; ++i) {
       float ls[3] = {d->log_scale[3 * (size_t)i], d->log_scale[3 * (size_t)i + 1], d->log_scale[3 * (size_t)i + 2]};
@@ -414,12 +420,15 @@ int gsr_load_scene(const gsr_scene_desc* d, gsr_scene** out) {
         }
         float cov[6], opac, tau;
         activate_one(ls, q, lg, cov, &opac, &tau);
+        rqv[(size_t)v * Np + i] = make_float4(q[0], q[1], q[2], q[3]);   // raw, for the backward of the activation
+        rlv[(size_t)v * Np + i] = make_float4(ls[0], ls[1], ls[2], lg);
         a1[(size_t)v * Np + i] = make_float4(cov[0], cov[1], cov[2], tau);
         a2[(size_t)v * Np + i] = make_float4(cov[3], cov[4], cov[5], 0.0f);
         ao[(size_t)v * Np + i] = opac;
       }
     }
     up(D.g1v, a1.data(), sizeof(float4) * 4 * Np); up(D.g2v, a2.data(), sizeof(float4) * 4 * Np);
+    up(D.raw_quat_v, rqv.data(), sizeof(float4) * 4 * Np); up(D.raw_ls_v, rlv.data(), sizeof(float4) * 4 * Np);
     up(D.opv, ao.data(), sizeof(float) * 4 * Np);
   }
   if (!ok) {
@@ -641,6 +650,38 @@ int gsr_project_backward(const gsr_scene* scene, const gsr_camera* cam, float t,
   FrameParams fp;
   make_frame(&scene->impl, cam, t, &fp);
   launch_project_backward(D, fp, grad_records, g_gauss, g_sh_base, g_sh_res, g_cluster, (cudaStream_t)cuda_stream);
+  GSR_CUDA(cudaGetLastError());
+  return GSR_OK;
+}
+
+int gsr_project_backward_full(const gsr_scene* scene, const gsr_camera* cam, float t, const float* grad_records,
+                              float* g_gauss, float* g_sh_base, float* g_sh_res, float* g_cluster, float* g_delta,
+                              float* g_attr, float* g_d_sh, void* cuda_stream) {
+  if (!scene || !camera_ok(cam) || !g_cluster || (scene->impl.d.N > 0 && (!grad_records || !g_gauss || !g_sh_base || !g_sh_res))) {
+    set_error("gsr_project_backward_full: invalid argument");
+    return GSR_E_INVALID_ARG;
+  }
+  if (((uintptr_t)grad_records & 15u) != 0) {
+    set_error("gsr_project_backward_full: grad_records must be 16-byte aligned");
+    return GSR_E_INVALID_ARG;
+  }
+  const DeviceScene& D = scene->impl.d;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  FrameParams fp;
+  make_frame(&scene->impl, cam, t, &fp);
+  if (D.V == 2) {  // two records per Gaussian: the kernel of gsr_project_backward; no refinement has any gradient
+    if (D.affine_cov) {
+      set_error("gsr_project_backward_full: affine_on_covariance needs a scene with four records per Gaussian");
+      return GSR_E_INVALID_ARG;
+    }
+    launch_project_backward(D, fp, grad_records, g_gauss, g_sh_base, g_sh_res, g_cluster, st);
+    const size_t N = (size_t)D.N;
+    if (g_delta && N) GSR_CUDA(cudaMemsetAsync(g_delta, 0, sizeof(float) * 6 * N, st));
+    if (g_attr && N) GSR_CUDA(cudaMemsetAsync(g_attr, 0, sizeof(float) * 24 * N, st));
+    if (g_d_sh && N) GSR_CUDA(cudaMemsetAsync(g_d_sh, 0, sizeof(float) * 9 * (size_t)D.K * N, st));
+  } else {
+    launch_project_backward4(D, fp, grad_records, g_gauss, g_sh_base, g_sh_res, g_cluster, g_delta, g_attr, g_d_sh, st);
+  }
   GSR_CUDA(cudaGetLastError());
   return GSR_OK;
 }

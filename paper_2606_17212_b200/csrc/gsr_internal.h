@@ -21,6 +21,7 @@ struct DeviceScene {
   int32_t V;      // projected records per Gaussian: 2 (no position residual levels) or 4 (delta2 / delta3 given)
   int32_t n_sh4;  // float4 words of SH coefficients per Gaussian = ceil(3K/4)
   int32_t n_qw;   // 32-bit words of int8 motion coefficients per Gaussian = ceil(3R/4)
+  int32_t has_delta2, has_delta3;  // the scene was given delta2 / delta3 (a missing one is stored as zeros)
   float4* g0;     // [N] mean.xyz, opacity
   float4* g1;     // [N] Sxx Sxy Sxz, tau
   float4* g2;     // [N] Syy Syz Szz, bits(cluster<<2 | level)
@@ -38,6 +39,8 @@ struct DeviceScene {
   int32_t* group_off;  // [4C+1]
   float4* raw_quat;    // [N] the quaternion as given (w, x, y, z): the backward of the activation (k_project_backward.cu)
   float4* raw_ls;      // [N] log_scale.xyz, opacity_logit
+  float4* raw_quat_v;  // [4][N] the raw quaternion per delivered depth (base + residuals of levels 1..v), else nullptr
+  float4* raw_ls_v;    // [4][N] log_scale.xyz, opacity_logit per delivered depth, else nullptr
   float bg[3];
 };
 
@@ -183,6 +186,9 @@ int launch_distortion_backward(const float* imgs, const float* ref, int32_t B, i
                                const double* weight, double lambda, float* out, double* ref_planes, cudaStream_t st);
 void launch_project_backward(const DeviceScene& sc, const FrameParams& fp, const float* grad_rec, float* g_gauss,
                              float* g_shb, float* g_shr, float* g_cluster, cudaStream_t st);
+void launch_project_backward4(const DeviceScene& sc, const FrameParams& fp, const float* grad_rec, float* g_gauss,
+                              float* g_shb, float* g_shr, float* g_cluster, float* g_delta, float* g_attr, float* g_dsh,
+                              cudaStream_t st);
 void launch_backward(const DeviceScene& sc, const WsHeader& h, Workspace& ws, const float* images, const float* gimg,
                      float* grad, cudaStream_t st);
 void launch_distortion_finalize_blk(const double* blk, int32_t B, int32_t tiles, int64_t n_values, double* mse,

@@ -74,7 +74,8 @@ template <int K>
 __device__ __forceinline__ bool variant_backward(const DeviceScene& sc, const FrameParams& fp, int i, const float* mu,
                                                  const float* S6, bool with_res, const float* gc0, const float* gc1,
                                                  const float* gq, float* dmu, float* dS6, float& dopac,
-                                                 float* shb_row, float* shr_row) {
+                                                 float* shb_row, float* shr_row, int n_dsh = 0,
+                                                 float* const* dsh_rows = nullptr) {
   const float* Rw = fp.R;
   float pc[3];
 #pragma unroll
@@ -118,7 +119,11 @@ __device__ __forceinline__ bool variant_backward(const DeviceScene& sc, const Fr
 #pragma unroll
     for (int w4 = 0; w4 < n4; ++w4) {
       const float4 b4 = __ldg(sc.sh_base + (size_t)w4 * sc.N + i);
-      const float vb[4] = {b4.x, b4.y, b4.z, b4.w};
+      float vb[4] = {b4.x, b4.y, b4.z, b4.w};
+      for (int l = 0; l < n_dsh; ++l) {  // colour refinements of the delivered levels 1..n_dsh (reading I3)
+        const float4 dl = __ldg(sc.d_sh + ((size_t)l * n4 + w4) * sc.N + i);
+        vb[0] += dl.x; vb[1] += dl.y; vb[2] += dl.z; vb[3] += dl.w;
+      }
       float vr[4] = {0.f, 0.f, 0.f, 0.f};
       if (with_res) {
         const float4 r4 = __ldg(sc.sh_res + (size_t)w4 * sc.N + i);
@@ -148,7 +153,11 @@ __device__ __forceinline__ bool variant_backward(const DeviceScene& sc, const Fr
 #pragma unroll
       for (int w4 = 0; w4 < n4; ++w4) {
         const float4 b4 = __ldg(sc.sh_base + (size_t)w4 * sc.N + i);
-        const float vb[4] = {b4.x, b4.y, b4.z, b4.w};
+        float vb[4] = {b4.x, b4.y, b4.z, b4.w};
+        for (int l = 0; l < n_dsh; ++l) {
+          const float4 dl = __ldg(sc.d_sh + ((size_t)l * n4 + w4) * sc.N + i);
+          vb[0] += dl.x; vb[1] += dl.y; vb[2] += dl.z; vb[3] += dl.w;
+        }
         float vr[4] = {0.f, 0.f, 0.f, 0.f};
         if (with_res) {
           const float4 r4 = __ldg(sc.sh_res + (size_t)w4 * sc.N + i);
@@ -162,6 +171,7 @@ __device__ __forceinline__ bool variant_backward(const DeviceScene& sc, const Fr
             dY[j] += d0[ch] * vb[e] + d1[ch] * (vb[e] + vr[e]);
             shb_row[flat] += Y[j] * (d0[ch] + d1[ch]);
             if (with_res) shr_row[flat] += Y[j] * d1[ch];
+            for (int l = 0; l < n_dsh; ++l) dsh_rows[l][flat] += Y[j] * (d0[ch] + d1[ch]);
           }
         }
       }
@@ -345,6 +355,292 @@ __global__ void __launch_bounds__(kPbThreads) k_project_backward(DeviceScene sc,
       if (cl13[k] != 0.0f) atomicAdd(a.g_cluster + 13 * (size_t)c + k, cl13[k]);
   }
 }
+
+// ------------------------------------------------------------------------------------------------
+// The full representation: four records per Gaussian, one per delivered depth v = 0..3
+// (record 4 i + v, one colour each), with position residual levels, per-level attribute and colour refinements and,
+// optionally, the affine on the covariance.
+
+// Backward of the activation for one set of raw attributes: dS6 = dL/dSigma folded onto the 6
+// stored entries, dopac = dL/d(opacity), opac = the activated opacity -> out8 = d/d(log_scale[3], quat[4], logit)
+__device__ __forceinline__ void activation_backward(const float4 rq, const float4 rl, const float* dS6, float dopac,
+                                                    float opac, float* out8) {
+  const float qn = sqrtf(rq.x * rq.x + rq.y * rq.y + rq.z * rq.z + rq.w * rq.w), rqn = 1.0f / qn;
+  const float w = rq.x * rqn, x = rq.y * rqn, y = rq.z * rqn, z = rq.w * rqn;
+  const float Rm[9] = {1.f - 2.f * (y * y + z * z), 2.f * (x * y - w * z), 2.f * (x * z + w * y),
+                       2.f * (x * y + w * z), 1.f - 2.f * (x * x + z * z), 2.f * (y * z - w * x),
+                       2.f * (x * z - w * y), 2.f * (y * z + w * x), 1.f - 2.f * (x * x + y * y)};
+  const float s3[3] = {expf(rl.x), expf(rl.y), expf(rl.z)};
+  const float Gs[9] = {2.f * dS6[0], dS6[1], dS6[2], dS6[1], 2.f * dS6[3], dS6[4], dS6[2], dS6[4], 2.f * dS6[5]};
+  float dRm[9];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    float ds = 0.0f;
+#pragma unroll
+    for (int r = 0; r < 3; ++r) {
+      const float dMm = (Gs[3 * r] * Rm[k] + Gs[3 * r + 1] * Rm[3 + k] + Gs[3 * r + 2] * Rm[6 + k]) * s3[k];
+      ds += dMm * Rm[3 * r + k];
+      dRm[3 * r + k] = dMm * s3[k];
+    }
+    out8[k] = ds * s3[k];
+  }
+  const float dw = 2.f * (-z * dRm[1] + y * dRm[2] + z * dRm[3] - x * dRm[5] - y * dRm[6] + x * dRm[7]);
+  const float dx = 2.f * (y * dRm[1] + z * dRm[2] + y * dRm[3] - 2.f * x * dRm[4] - w * dRm[5] + z * dRm[6] + w * dRm[7] - 2.f * x * dRm[8]);
+  const float dy = 2.f * (-2.f * y * dRm[0] + x * dRm[1] + w * dRm[2] + x * dRm[3] + z * dRm[5] - w * dRm[6] + z * dRm[7] - 2.f * y * dRm[8]);
+  const float dz = 2.f * (-2.f * z * dRm[0] - w * dRm[1] + x * dRm[2] + w * dRm[3] - 2.f * z * dRm[4] + y * dRm[5] + x * dRm[6] + y * dRm[7]);
+  const float qd = w * dw + x * dx + y * dy + z * dz;
+  out8[3] = (dw - w * qd) * rqn;
+  out8[4] = (dx - x * qd) * rqn;
+  out8[5] = (dy - y * qd) * rqn;
+  out8[6] = (dz - z * qd) * rqn;
+  out8[7] = dopac * opac * (1.0f - opac);
+}
+
+// Reading I4: Su = L Sg L^T, L = the 3x3 part of A (row-major 3x4).  Forward.
+__device__ __forceinline__ void affine_cov_forward(const float* A, const float* S6, float* Su6) {
+  const float Sf[9] = {S6[0], S6[1], S6[2], S6[1], S6[3], S6[4], S6[2], S6[4], S6[5]};
+  float LS[9];
+#pragma unroll
+  for (int a = 0; a < 3; ++a)
+#pragma unroll
+    for (int b = 0; b < 3; ++b) LS[3 * a + b] = A[4 * a] * Sf[b] + A[4 * a + 1] * Sf[3 + b] + A[4 * a + 2] * Sf[6 + b];
+  int o = 0;
+#pragma unroll
+  for (int a = 0; a < 3; ++a)
+#pragma unroll
+    for (int b = a; b < 3; ++b) Su6[o++] = LS[3 * a] * A[4 * b] + LS[3 * a + 1] * A[4 * b + 1] + LS[3 * a + 2] * A[4 * b + 2];
+}
+
+// ... and backward: dSu6 (folded) -> dSg6 (folded) = L^T G L, and dL/dL = (G + G^T) L Sg added to dA (3x4 row-major)
+__device__ __forceinline__ void affine_cov_backward(const float* A, const float* S6, const float* dSu6, float* dSg6,
+                                                    float* dA) {
+  const float Sf[9] = {S6[0], S6[1], S6[2], S6[1], S6[3], S6[4], S6[2], S6[4], S6[5]};
+  // the symmetric part of G: diagonal entries as they are, off-diagonal ones halved
+  const float G[9] = {dSu6[0], 0.5f * dSu6[1], 0.5f * dSu6[2], 0.5f * dSu6[1], dSu6[3], 0.5f * dSu6[4],
+                      0.5f * dSu6[2], 0.5f * dSu6[4], dSu6[5]};
+  float LS[9], GL[9];
+#pragma unroll
+  for (int a = 0; a < 3; ++a)
+#pragma unroll
+    for (int b = 0; b < 3; ++b) {
+      LS[3 * a + b] = A[4 * a] * Sf[b] + A[4 * a + 1] * Sf[3 + b] + A[4 * a + 2] * Sf[6 + b];
+      GL[3 * a + b] = G[3 * a] * A[b] + G[3 * a + 1] * A[4 + b] + G[3 * a + 2] * A[8 + b];  // (G L)_ab
+    }
+#pragma unroll
+  for (int r = 0; r < 3; ++r)
+#pragma unroll
+    for (int c = 0; c < 3; ++c) dA[4 * r + c] += 2.0f * (G[3 * r] * LS[c] + G[3 * r + 1] * LS[3 + c] + G[3 * r + 2] * LS[6 + c]);
+  float T[9];  // L^T (G L)
+#pragma unroll
+  for (int a = 0; a < 3; ++a)
+#pragma unroll
+    for (int b = 0; b < 3; ++b) T[3 * a + b] = A[a] * GL[b] + A[4 + a] * GL[3 + b] + A[8 + a] * GL[6 + b];
+  dSg6[0] = T[0]; dSg6[1] = 2.0f * T[1]; dSg6[2] = 2.0f * T[2]; dSg6[3] = T[4]; dSg6[4] = 2.0f * T[5]; dSg6[5] = T[8];
+}
+
+struct Pb4Args {
+  const float* grad_rec;  // [4N, 12]
+  float* g_gauss;         // [N, 14]
+  float* g_shb;           // [N, K, 3]
+  float* g_shr;           // [N, K, 3]
+  float* g_cluster;       // [C, 13]
+  float* g_delta;         // [N, 6] delta2.xyz, delta3.xyz, or nullptr
+  float* g_attr;          // [3][N, 8] per refinement level: log_scale[3], quat[4], logit, or nullptr
+  float* g_dsh;           // [3][N, K, 3], or nullptr
+};
+
+constexpr int kPb4Threads = 32;
+
+template <int K>
+__global__ void __launch_bounds__(kPb4Threads) k_project_backward4(DeviceScene sc, FrameParams fp, Pb4Args a) {
+  constexpr int kRow = 3 * K + 1;
+  constexpr int n4 = (3 * K + 3) / 4;
+  // rows of the CTA's Gaussians: sh_base, sh_res, and the three colour refinement levels
+  __shared__ float s_rows[5][kPb4Threads * kRow];
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int lane = threadIdx.x & 31;
+  const bool live = i < sc.N;
+  float* const shb_row = s_rows[0] + threadIdx.x * kRow;
+  float* const shr_row = s_rows[1] + threadIdx.x * kRow;
+  float* const dsh_rows[3] = {s_rows[2] + threadIdx.x * kRow, s_rows[3] + threadIdx.x * kRow, s_rows[4] + threadIdx.x * kRow};
+#pragma unroll
+  for (int r = 0; r < 5; ++r)
+    for (int f = 0; f < 3 * K; ++f) s_rows[r][threadIdx.x * kRow + f] = 0.0f;
+  int c = -1;
+  float cl13[13];
+#pragma unroll
+  for (int k = 0; k < 13; ++k) cl13[k] = 0.0f;
+  if (live) {
+    const float4 g0 = __ldg(sc.g0 + i), g1 = __ldg(sc.g1 + i), g2 = __ldg(sc.g2 + i);
+    const uint32_t bits = __float_as_uint(g2.w);
+    c = (int)(bits >> 2);
+    const int lvl = (int)(bits & 3u);
+    // ---- Eq. (1) with the position residual levels: mu_0 = p, mu_1 = p + rho, mu_2 = mu_1 + delta2, mu_3 = mu_2 + delta3
+    float A[12];
+#pragma unroll
+    for (int k = 0; k < 12; ++k) A[k] = fmaf(fp.time, __ldg(sc.A1 + 12 * c + k), __ldg(sc.A0 + 12 * c + k));
+    float mu[4][3], acc[3] = {0.f, 0.f, 0.f};
+#pragma unroll
+    for (int k = 0; k < 3; ++k) mu[0][k] = A[4 * k] * g0.x + A[4 * k + 1] * g0.y + A[4 * k + 2] * g0.z + A[4 * k + 3];
+    {
+      uint32_t w = 0;
+      for (int r = 0; r < sc.R; ++r) {
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+          const int byte = r * 3 + k;
+          if ((byte & 3) == 0) w = __ldg(sc.qw + (size_t)(byte >> 2) * sc.N + i);
+          acc[k] = fmaf(fp.basis[r], (float)(int)(int8_t)((w >> ((byte & 3) * 8)) & 0xFFu), acc[k]);
+        }
+      }
+    }
+    const float s_c = __ldg(sc.mscale + c);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      mu[1][k] = fmaf(s_c, acc[k], mu[0][k]);
+      mu[2][k] = mu[1][k] + __ldg(sc.delta + (size_t)k * sc.N + i);
+      mu[3][k] = mu[2][k] + __ldg(sc.delta + (size_t)(3 + k) * sc.N + i);
+    }
+    const bool attr = sc.g1v != nullptr;
+    float dmu_all[3] = {0.f, 0.f, 0.f}, drho[3] = {0.f, 0.f, 0.f}, dd2[3] = {0.f, 0.f, 0.f}, dd3[3] = {0.f, 0.f, 0.f};
+    float dA[12];
+#pragma unroll
+    for (int k = 0; k < 12; ++k) dA[k] = 0.0f;
+    float base8[8], lev[3][8], dS6sum[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, dopac_sum = 0.0f;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { base8[k] = 0.0f; lev[0][k] = 0.0f; lev[1][k] = 0.0f; lev[2][k] = 0.0f; }
+    const float zero3[3] = {0.f, 0.f, 0.f};
+#pragma unroll
+    for (int v = 0; v < 4; ++v) {
+      if (v < lvl) continue;  // a level-l Gaussian has the variants v >= l only
+      float S6[6] = {g1.x, g1.y, g1.z, g2.x, g2.y, g2.z}, opac = g0.w;
+      if (attr) {  // the attributes of delivered depth v (reading I2)
+        const float4 h1 = __ldg(sc.g1v + (size_t)v * sc.N + i), h2 = __ldg(sc.g2v + (size_t)v * sc.N + i);
+        S6[0] = h1.x; S6[1] = h1.y; S6[2] = h1.z; S6[3] = h2.x; S6[4] = h2.y; S6[5] = h2.z;
+        opac = __ldg(sc.opv + (size_t)v * sc.N + i);
+      }
+      float Su[6];
+      if (sc.affine_cov) affine_cov_forward(A, S6, Su);
+      else {
+#pragma unroll
+        for (int k = 0; k < 6; ++k) Su[k] = S6[k];
+      }
+      float g[12];
+      const float4* gp = reinterpret_cast<const float4*>(a.grad_rec + 12 * (size_t)(4 * i + v));
+#pragma unroll
+      for (int q = 0; q < 3; ++q) { const float4 t4 = __ldg(gp + q); g[4 * q] = t4.x; g[4 * q + 1] = t4.y; g[4 * q + 2] = t4.z; g[4 * q + 3] = t4.w; }
+      float dmu[3] = {0.f, 0.f, 0.f}, dSu[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, dop = 0.0f;
+      // one colour per record (columns 0..2): at depth 3 it includes the SH residual
+      const bool ok = variant_backward<K>(sc, fp, i, mu[v], Su, v == 3, v == 3 ? zero3 : g, v == 3 ? g : zero3, g + 6, dmu,
+                                          dSu, dop, shb_row, shr_row, sc.d_sh ? v : 0, dsh_rows);
+      if (!ok) continue;
+      float dSg[6];
+      if (sc.affine_cov) affine_cov_backward(A, S6, dSu, dSg, dA);
+      else {
+#pragma unroll
+        for (int k = 0; k < 6; ++k) dSg[k] = dSu[k];
+      }
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        dmu_all[k] += dmu[k];
+        if (v >= 1) drho[k] += dmu[k];
+        if (v >= 2) dd2[k] += dmu[k];
+        if (v >= 3) dd3[k] += dmu[k];
+      }
+      if (attr) {
+        float gv[8];
+        activation_backward(__ldg(sc.raw_quat_v + (size_t)v * sc.N + i), __ldg(sc.raw_ls_v + (size_t)v * sc.N + i), dSg, dop,
+                            opac, gv);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          base8[k] += gv[k];
+#pragma unroll
+          for (int l = 0; l < 3; ++l)
+            if (l < v) lev[l][k] += gv[k];  // the residual of level l + 1 is part of every depth >= l + 1
+        }
+      } else {
+#pragma unroll
+        for (int k = 0; k < 6; ++k) dS6sum[k] += dSg[k];
+        dopac_sum += dop;
+      }
+    }
+    if (!attr) activation_backward(__ldg(sc.raw_quat + i), __ldg(sc.raw_ls + i), dS6sum, dopac_sum, g0.w, base8);
+    float* out = a.g_gauss + 14 * (size_t)i;
+#pragma unroll
+    for (int j = 0; j < 3; ++j) out[j] = A[j] * dmu_all[0] + A[4 + j] * dmu_all[1] + A[8 + j] * dmu_all[2];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) out[3 + k] = drho[k];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) out[6 + k] = base8[k];
+    if (a.g_delta) {
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {  // zero where the scene has no such residual
+        a.g_delta[6 * (size_t)i + k] = sc.has_delta2 ? dd2[k] : 0.0f;
+        a.g_delta[6 * (size_t)i + 3 + k] = sc.has_delta3 ? dd3[k] : 0.0f;
+      }
+    }
+    if (a.g_attr) {
+#pragma unroll
+      for (int l = 0; l < 3; ++l)
+#pragma unroll
+        for (int k = 0; k < 8; ++k) a.g_attr[((size_t)l * sc.N + i) * 8 + k] = lev[l][k];
+    }
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      cl13[4 * k] = dmu_all[k] * g0.x + dA[4 * k]; cl13[4 * k + 1] = dmu_all[k] * g0.y + dA[4 * k + 1];
+      cl13[4 * k + 2] = dmu_all[k] * g0.z + dA[4 * k + 2]; cl13[4 * k + 3] = dmu_all[k];
+    }
+    cl13[12] = drho[0] * acc[0] + drho[1] * acc[1] + drho[2] * acc[2];
+  }
+  __syncthreads();
+  {
+    const size_t i0 = (size_t)blockIdx.x * kPb4Threads;
+    const int rows = sc.N - (int)i0 < kPb4Threads ? sc.N - (int)i0 : kPb4Threads;
+    for (int f = threadIdx.x; f < rows * 3 * K; f += kPb4Threads) {
+      const int r = f / (3 * K), col = f - r * (3 * K);
+      a.g_shb[i0 * 3 * K + f] = s_rows[0][r * kRow + col];
+      a.g_shr[i0 * 3 * K + f] = s_rows[1][r * kRow + col];
+      if (a.g_dsh) {
+#pragma unroll
+        for (int l = 0; l < 3; ++l) a.g_dsh[((size_t)l * sc.N + i0) * 3 * K + f] = s_rows[2 + l][r * kRow + col];
+      }
+    }
+  }
+  const int c0 = __shfl_sync(0xffffffffu, c, 0);
+  if (__all_sync(0xffffffffu, c == c0)) {
+    if (c0 < 0) return;
+#pragma unroll
+    for (int k = 0; k < 13; ++k) {
+      float v = cl13[k];
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+      if (lane == 0 && v != 0.0f) atomicAdd(a.g_cluster + 13 * (size_t)c0 + k, v);
+    }
+  } else if (live) {
+#pragma unroll
+    for (int k = 0; k < 13; ++k)
+      if (cl13[k] != 0.0f) atomicAdd(a.g_cluster + 13 * (size_t)c + k, cl13[k]);
+  }
+}
+
+void launch_project_backward4(const DeviceScene& sc, const FrameParams& fp, const float* grad_rec, float* g_gauss,
+                              float* g_shb, float* g_shr, float* g_cluster, float* g_delta, float* g_attr, float* g_dsh,
+                              cudaStream_t st) {
+  cudaMemsetAsync(g_cluster, 0, sizeof(float) * 13 * (size_t)sc.C, st);
+  if (sc.N == 0) return;
+  // a scene without that kind of refinement has zero gradient for it
+  if (g_attr && !sc.g1v) { cudaMemsetAsync(g_attr, 0, sizeof(float) * 24 * (size_t)sc.N, st); g_attr = nullptr; }
+  if (g_dsh && !sc.d_sh) { cudaMemsetAsync(g_dsh, 0, sizeof(float) * 9 * (size_t)sc.K * (size_t)sc.N, st); g_dsh = nullptr; }
+  Pb4Args a{grad_rec, g_gauss, g_shb, g_shr, g_cluster, g_delta, g_attr, g_dsh};
+  dim3 grid((sc.N + kPb4Threads - 1) / kPb4Threads), block(kPb4Threads);
+  switch (sc.K) {
+    case 1: k_project_backward4<1><<<grid, block, 0, st>>>(sc, fp, a); break;
+    case 4: k_project_backward4<4><<<grid, block, 0, st>>>(sc, fp, a); break;
+    case 9: k_project_backward4<9><<<grid, block, 0, st>>>(sc, fp, a); break;
+    default: k_project_backward4<16><<<grid, block, 0, st>>>(sc, fp, a); break;
+  }
+  count_launches(1);
+}
+
 
 void launch_project_backward(const DeviceScene& sc, const FrameParams& fp, const float* grad_rec, float* g_gauss,
                              float* g_shb, float* g_shr, float* g_cluster, cudaStream_t st) {

@@ -88,6 +88,7 @@ def lib():
         L.gsr_distortion_backward_workspace_bytes.restype = sz
         L.gsr_objective_weights.argtypes = [vp, i32, C.c_double, C.c_double, C.c_double, vp, vp, i32, C.c_double, vp, vp]
         L.gsr_flicker_backward.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp, vp, vp]
+        L.gsr_project_backward_full.argtypes = [vp, C.POINTER(CameraC), f32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.gsr_project_backward.argtypes = [vp, C.POINTER(CameraC), f32, vp, vp, vp, vp, vp, vp]
         L.gsr_close_levels.argtypes = [vp, i64, vp, vp, vp]
         L.gsr_frame_workspace_bytes.argtypes = [vp, C.POINTER(CameraC), i32, i32, i32, i32]
@@ -304,6 +305,22 @@ class Scene:
         _check(lib().gsr_project_backward(self.handle, C.byref(camera_struct(cam)), float(t), _dp(grad_records),
                                           _dp(out["gauss"]), _dp(out["sh_base"]), _dp(out["sh_res"]),
                                           _dp(out["cluster"]), _stream()))
+        return out
+
+    def project_backward_full(self, cam, t: float, grad_records):
+        """gsr_project_backward_full: like project_backward, for every scene; adds "delta" [N,6], "attr" [3,N,8]
+        (log_scale 3, quat 4, opacity_logit per refinement level) and "d_sh" [3,N,K,3]."""
+        torch = _torch()
+        assert grad_records.dtype == torch.float32 and grad_records.is_cuda and grad_records.is_contiguous()
+        assert tuple(grad_records.shape) == (self.num_records(), 12)
+        K = (self.sh_degree + 1) ** 2
+        e = lambda *shape: torch.empty(shape, dtype=torch.float32, device="cuda")
+        out = {"gauss": e(self.N, 14), "sh_base": e(self.N, K, 3), "sh_res": e(self.N, K, 3), "cluster": e(self.C, 13),
+               "delta": e(self.N, 6), "attr": e(3, self.N, 8), "d_sh": e(3, self.N, K, 3)}
+        _check(lib().gsr_project_backward_full(self.handle, C.byref(camera_struct(cam)), float(t), _dp(grad_records),
+                                               _dp(out["gauss"]), _dp(out["sh_base"]), _dp(out["sh_res"]),
+                                               _dp(out["cluster"]), _dp(out["delta"]), _dp(out["attr"]), _dp(out["d_sh"]),
+                                               _stream()))
         return out
 
     def debug_pair_counts(self, workspace) -> np.ndarray:

@@ -211,3 +211,120 @@ def test_refuses_scenes_it_does_not_cover(gsr, torch_mod):
     with pytest.raises(gsr.GsrError):
         scene.project_backward(wl.frames[0][0], 0.5, gr)
     scene.close()
+
+
+def oracle_from_records4(oracle_mod, scn, cam, t, grad_rec):
+    """grad_rec double [4N, 12] of a scene with four records per Gaussian (record 4 i + delivered depth v, one colour in
+    columns 0..2) -> the oracle's parameter gradients: pseudo-state v = every cluster at depth v, with the rows of
+    record v (the oracle skips the Gaussians whose level is above v, as the GPU skips the records that do not exist)."""
+    osc = oracle_mod.OracleScene(scn)
+    out = None
+    for v in range(4):
+        r = grad_rec[v::4]
+        g9 = np.ascontiguousarray(np.concatenate([r[:, 0:3], r[:, 6:12]], 1))
+        out = osc.project_backward(cam, t, np.full(scn.C, v, np.int8), g9, into=out)
+    return out
+
+
+def compare_full(scn, got, want, tol=2e-4):
+    compare(scn, got, want, tol)
+    ok = want["margin"] > 1e-4
+
+    def block(name, g, w):
+        g, w = g.reshape(scn.N, -1), w.reshape(scn.N, -1)
+        bmax = np.abs(w).max(1, keepdims=True)
+        bad = (np.abs(g - w) > tol * bmax + 1e-12) & ok[:, None]
+        assert not bad.any(), (name, np.argwhere(bad)[:4], g[bad][:4], w[bad][:4])
+
+    d = got["delta"].double().cpu().numpy()
+    block("delta2", d[:, 0:3], want["delta2"])
+    block("delta3", d[:, 3:6], want["delta3"])
+    at = got["attr"].double().cpu().numpy()
+    dsh = got["d_sh"].double().cpu().numpy()
+    for l in range(3):
+        block(f"d_log_scale[{l}]", at[l][:, 0:3], want["d_log_scale"][l])
+        block(f"d_quat[{l}]", at[l][:, 3:7], want["d_quat"][l])
+        block(f"d_opacity_logit[{l}]", at[l][:, 7:8], want["d_opacity_logit"][l])
+        block(f"d_sh[{l}]", dsh[l], want["d_sh"][l])
+
+
+@pytest.mark.parametrize("what", ["all", "all+affine", "delta_only", "attr_only"])
+def test_full_representation_against_the_oracle(gsr, torch_mod, oracle_mod, what):
+    """Four records per Gaussian: position residual levels, per-level attribute and colour refinements, optionally the
+    affine on the covariance (with a cluster affine far from the identity) — random record gradients against O-9."""
+    import dataclasses
+    torch = torch_mod
+    wl = synth.scaled_object_workload(57, C=4, per_cluster=150.0, W=120, H=88, fov=40.0, n_frames=2, B=2)
+    cam, t = wl.frames[1]
+    scn = wl.scene
+    rng = np.random.default_rng(57)
+    if what in ("all", "all+affine"):
+        scn = synth.with_attribute_refinements(synth.with_position_residuals(scn))
+    elif what == "delta_only":
+        scn = synth.with_position_residuals(scn)
+    else:
+        scn = synth.with_attribute_refinements(scn)
+    if what == "all+affine":
+        A0 = scn.A0.copy()
+        A0[:, :, :3] += (0.2 * rng.standard_normal((scn.C, 3, 3))).astype(np.float32)
+        scn = dataclasses.replace(scn, A0=A0, affine_on_covariance=True)
+    lvl = scn.level_of()
+    grad_rec = rng.standard_normal((4 * scn.N, 12)).astype(np.float32).astype(np.float64)
+    grad_rec[:, 3:6] = 0.0                                  # one colour per record
+    for v in range(4):
+        grad_rec[v::4][lvl > v] = 0.0                       # a level-l Gaussian has the records v >= l only
+    scene = gsr.Scene(scn)
+    assert scene.num_records() == 4 * scn.N
+    got = scene.project_backward_full(cam, t, torch.from_numpy(grad_rec.astype(np.float32)).cuda())
+    torch.cuda.synchronize()
+    scene.close()
+    want = oracle_from_records4(oracle_mod, scn, cam, t, grad_rec)
+    compare_full(scn, got, want)
+    if what == "delta_only":
+        assert float(got["attr"].abs().max()) == 0.0 and float(got["d_sh"].abs().max()) == 0.0
+    if what in ("all", "all+affine"):
+        assert np.any(want["d_quat"][2] != 0.0) and np.any(want["delta3"] != 0.0) and np.any(want["d_sh"][2] != 0.0)
+
+
+def test_full_entry_serves_two_record_scenes_and_the_chain(gsr, torch_mod, oracle_mod):
+    """(1) A scene with two records per Gaussian through gsr_project_backward_full: the same numbers as
+    gsr_project_backward, zeros for the refinement outputs.  (2) The whole chain on the full representation:
+    render -> gsr_render_backward -> gsr_project_backward_full against O-5 -> O-8 -> O-9 state by state."""
+    torch = torch_mod
+    wl = synth.scaled_object_workload(58, C=4, per_cluster=110.0, W=96, H=72, fov=40.0, n_frames=1, B=6)
+    cam, t = wl.frames[0]
+    scene = gsr.Scene(wl.scene)
+    gen = torch.Generator(device="cuda").manual_seed(4)
+    gr = torch.randn((scene.num_records(), 12), generator=gen, device="cuda", dtype=torch.float32)
+    a, b = scene.project_backward(cam, t, gr), scene.project_backward_full(cam, t, gr)
+    for k in ("gauss", "sh_base", "sh_res"):
+        assert torch.equal(a[k], b[k])
+    assert torch.allclose(a["cluster"], b["cluster"], rtol=1e-4, atol=1e-6)
+    assert float(b["delta"].abs().max()) == 0.0 and float(b["attr"].abs().max()) == 0.0 and float(b["d_sh"].abs().max()) == 0.0
+    scene.close()
+    # (2)
+    scn = synth.with_attribute_refinements(synth.with_position_residuals(wl.scene))
+    lv = wl.levels[0].copy()
+    lv[0], lv[1], lv[2] = 3, 2, 1
+    scene = gsr.Scene(scn)
+    ws = scene.new_workspace(cam, lv.shape[0])
+    dlv = torch.from_numpy(np.ascontiguousarray(lv, np.int8)).cuda()
+    out, _, _ = scene.render_states(cam, t, dlv, workspace=ws)
+    scene.status(ws)
+    rng = np.random.default_rng(58)
+    g = rng.standard_normal(tuple(out.shape)).astype(np.float32)
+    grad_rec = scene.render_backward(ws, out, torch.from_numpy(g).cuda())
+    got = scene.project_backward_full(cam, t, grad_rec)
+    torch.cuda.synchronize()
+    scene.close()
+    osc = oracle_mod.OracleScene(scn)
+    want = None
+    for s_ in range(lv.shape[0]):
+        g9 = osc.backward(cam, t, lv[s_], g[s_].astype(np.float64))
+        want = osc.project_backward(cam, t, lv[s_], g9, into=want)
+    compare(scn, got, want, tol=2e-3, floor=2e-3)
+    at = got["attr"].double().cpu().numpy()
+    for l in range(3):
+        w = want["d_log_scale"][l]
+        scale = np.median(np.abs(w).max(1)[np.abs(w).max(1) > 0])
+        assert np.all(np.abs(at[l][:, 0:3] - w) <= 2e-3 * np.abs(w).max(1, keepdims=True) + 2e-3 * scale + 1e-12)
