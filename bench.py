@@ -484,7 +484,7 @@ def measure_ours(args, workload: str, steps: int, warmup: int, full: bool):
         gimg = torch.randn((B, H, W, 3), dtype=torch.float32, device=dev) * (2.0 / (3.0 * W * H))
         b0 = bufs[0]
         grec = torch.empty((scene.num_records(), 12), dtype=torch.float32, device=dev)
-        chain = scene.V == 2                      # gsr_project_backward covers the 2-record scenes (all configs)
+        chain = True                              # 2-record scenes: gsr_project_backward; cfg1r: gsr_project_backward_full
         gpar = [None]
 
         def fwd_bwd(k, mode=2):
@@ -493,7 +493,8 @@ def measure_ours(args, workload: str, steps: int, warmup: int, full: bool):
                 scene.render_backward(b0["ws"], b0["out"], gimg, grad=grec)
             if mode >= 2 and chain:
                 f = frame_of(k)
-                gpar[0] = scene.project_backward(cams[f], ts[f], grec, out=gpar[0])
+                pb = scene.project_backward if scene.V == 2 else scene.project_backward_full
+                gpar[0] = pb(cams[f], ts[f], grec, out=gpar[0])
 
         for k in range(2):
             fwd_bwd(warmup + k)

@@ -307,7 +307,7 @@ class Scene:
                                           _dp(out["cluster"]), _stream()))
         return out
 
-    def project_backward_full(self, cam, t: float, grad_records):
+    def project_backward_full(self, cam, t: float, grad_records, out=None):
         """gsr_project_backward_full: like project_backward, for every scene; adds "delta" [N,6], "attr" [3,N,8]
         (log_scale 3, quat 4, opacity_logit per refinement level) and "d_sh" [3,N,K,3]."""
         torch = _torch()
@@ -315,8 +315,9 @@ class Scene:
         assert tuple(grad_records.shape) == (self.num_records(), 12)
         K = (self.sh_degree + 1) ** 2
         e = lambda *shape: torch.empty(shape, dtype=torch.float32, device="cuda")
-        out = {"gauss": e(self.N, 14), "sh_base": e(self.N, K, 3), "sh_res": e(self.N, K, 3), "cluster": e(self.C, 13),
-               "delta": e(self.N, 6), "attr": e(3, self.N, 8), "d_sh": e(3, self.N, K, 3)}
+        if out is None:                                      # `out` reuses the dict of a previous call
+            out = {"gauss": e(self.N, 14), "sh_base": e(self.N, K, 3), "sh_res": e(self.N, K, 3), "cluster": e(self.C, 13),
+                   "delta": e(self.N, 6), "attr": e(3, self.N, 8), "d_sh": e(3, self.N, K, 3)}
         _check(lib().gsr_project_backward_full(self.handle, C.byref(camera_struct(cam)), float(t), _dp(grad_records),
                                                _dp(out["gauss"]), _dp(out["sh_base"]), _dp(out["sh_res"]),
                                                _dp(out["cluster"]), _dp(out["delta"]), _dp(out["attr"]), _dp(out["d_sh"]),
