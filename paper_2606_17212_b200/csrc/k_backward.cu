@@ -52,6 +52,7 @@ struct BackwardArgs {
 #define GSR_BW_GROUP 8
 #endif
 constexpr int kGroup = GSR_BW_GROUP;
+constexpr int kSlotGroup = 4;  // slots tested together before the per-slot tests (k_backward_q)
 constexpr int kPartStride = 32 * 12 + 4;  // floats; + 4: the kGroup rows of a quarter-warp load fall in distinct banks
 
 __device__ __forceinline__ void sts128f(uint32_t addr, float x, float y, float z, float w) {
@@ -376,17 +377,27 @@ __global__ void __launch_bounds__(32, GSR_BW_MINB) k_backward_q(const BackwardAr
       const uint32_t act1 = actl & (tag >> 16), act0 = actl ^ act1;
       {
         const float4 k0 = lds128(addr + 32u);  // {rgb - bg, -}
+        // the slots are tested four at a time first: a record is present in ~2 of the 12 classes of a block, so most
+        // groups are skipped with one test instead of four (measured: 6.67 -> 6.43 ms with both passes grouped)
 #pragma unroll
-        for (int s = 0; s < S; ++s)
-          if ((act0 >> s) & 1u)
-            slot_backward(T2[s], E2[s], gr2[s], gg2[s], gb2[s], alpha2, rinv2, k0.x, k0.y, k0.z, dal, dc0[0], dc0[1], dc0[2]);
+        for (int g4 = 0; g4 < S; g4 += kSlotGroup)
+          if (act0 & (((1u << kSlotGroup) - 1u) << g4)) {
+#pragma unroll
+            for (int s = g4; s < g4 + kSlotGroup && s < S; ++s)
+              if ((act0 >> s) & 1u)
+                slot_backward(T2[s], E2[s], gr2[s], gg2[s], gb2[s], alpha2, rinv2, k0.x, k0.y, k0.z, dal, dc0[0], dc0[1], dc0[2]);
+          }
       }
       if (act1 != 0) {
         const float4 k1 = lds128(addr + 48u);  // {rgb with SH residual - bg, -}
 #pragma unroll
-        for (int s = 0; s < S; ++s)
-          if ((act1 >> s) & 1u)
-            slot_backward(T2[s], E2[s], gr2[s], gg2[s], gb2[s], alpha2, rinv2, k1.x, k1.y, k1.z, dal, dc1[0], dc1[1], dc1[2]);
+        for (int g4 = 0; g4 < S; g4 += kSlotGroup)
+          if (act1 & (((1u << kSlotGroup) - 1u) << g4)) {
+#pragma unroll
+            for (int s = g4; s < g4 + kSlotGroup && s < S; ++s)
+              if ((act1 >> s) & 1u)
+                slot_backward(T2[s], E2[s], gr2[s], gg2[s], gb2[s], alpha2, rinv2, k1.x, k1.y, k1.z, dal, dc1[0], dc1[1], dc1[2]);
+          }
       }
       // per pixel: dL/do = exp(-q) dal, dL/dq = -alpha dal, then the chain through q; the two pixels added
       float v[12];
