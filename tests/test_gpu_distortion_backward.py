@@ -213,3 +213,59 @@ def test_objective_weights_and_flicker_gradient_against_the_oracle(gsr, torch_mo
     w1, w2 = M.flicker_backward(a, b, r1, r2, wgt)
     assert np.abs(g2.cpu().numpy() - w2).max() <= 2e-7 * np.abs(w2).max()
     assert torch.equal(g1, -g2)
+
+
+def test_image_space_objective_of_eq2_end_to_end(gsr, torch_mod):
+    """L = mean_b D_b + 0.30 CVaR_0.05(D) + 2.0 M(D), D = MSE + 0.20 (1 - SSIM) (Eq. (2) with the paper's weights,
+    PAPER.md:68-72; lambda_r R has no image gradient, lambda_t F is a separate call): forward by gsr_distortion,
+    gsr_distortion_ssim, gsr_risk_reduce, gsr_prefix_monotonicity; gradient by gsr_objective_weights ->
+    gsr_distortion_backward -> gsr_render_backward -> gsr_project_backward; against central differences of the forward
+    along the SH coefficients of both colour payloads."""
+    torch = torch_mod
+    wl = synth.scaled_object_workload(62, C=4, per_cluster=120.0, W=96, H=80, fov=40.0, n_frames=1, B=12)
+    cam, t = wl.frames[0]
+    scn = wl.scene
+    lv = wl.levels[0].copy()
+    dlv = torch.from_numpy(np.ascontiguousarray(lv, np.int8)).cuda()
+    B = lv.shape[0]
+    rng = np.random.default_rng(62)
+    prev = torch.from_numpy(np.arange(0, B - 1, dtype=np.int32)).cuda()
+    nxt = torch.from_numpy(np.arange(1, B, dtype=np.int32)).cuda()
+    tgt = dataclasses.replace(scn, sh_base=(scn.sh_base + 0.05 * rng.standard_normal(scn.sh_base.shape)).astype(np.float32))
+    s0 = gsr.Scene(tgt)
+    ref = s0.render_states(cam, t, torch.full((1, scn.C), 3, dtype=torch.int8, device="cuda"))[0][0].contiguous()
+    s0.close()
+
+    def forward(sc_np):
+        s = gsr.Scene(sc_np)
+        ws = s.new_workspace(cam, B)
+        out, _, _ = s.render_states(cam, t, dlv, workspace=ws)
+        mse, _ = gsr.distortion(out, ref)
+        _, D = gsr.distortion_ssim(out, ref, mse=mse)
+        r = gsr.risk_reduce(D, 0.05, True)
+        M_, viol = gsr.prefix_monotonicity(D, prev, nxt)
+        return float(r["mean"]) + 0.30 * float(r["cvar"]) + 2.0 * M_, s, ws, out, D, viol
+
+    L0, scene, ws, out, D, viol = forward(scn)
+    assert viol >= 2                                           # the monotonicity term is active
+    w = gsr.objective_weights(D, 1.0, 0.30, 0.05, prev, nxt, 2.0)
+    gimg = gsr.distortion_backward(out, ref, w, 0.20)
+    gp = scene.project_backward(cam, t, scene.render_backward(ws, out, gimg))
+    grads = {"sh_base": gp["sh_base"].double().cpu().numpy(), "sh_res": gp["sh_res"].double().cpu().numpy()}
+    scene.close()
+    # colour coefficients: the image is exactly smooth in them (opacity and scale also move the cut q <= tau and the
+    # footprint, which are constants of the differentiation: reading K1)
+    for field, h in (("sh_base", 5e-3), ("sh_res", 1e-2)):
+        theta = np.asarray(getattr(scn, field), np.float32)
+        u = rng.standard_normal(theta.shape)
+        tp = (theta.astype(np.float64) + h * u).astype(np.float32)
+        tm = (theta.astype(np.float64) - h * u).astype(np.float32)
+        Lp, s1, _, _, _, vp = forward(dataclasses.replace(scn, **{field: tp}))
+        s1.close()
+        Lm, s2, _, _, _, vm = forward(dataclasses.replace(scn, **{field: tm}))
+        s2.close()
+        assert vp == viol and vm == viol                       # no pair changed sides: L is smooth along the step
+        delta = tp.astype(np.float64) - tm.astype(np.float64)
+        pred = float((grads[field].reshape(theta.shape) * delta).sum())
+        mag = float(np.abs(grads[field].reshape(theta.shape) * delta).sum())
+        assert abs((Lp - Lm) - pred) <= 3e-2 * mag + 2e-2 * abs(pred), (field, Lp - Lm, pred, mag)
