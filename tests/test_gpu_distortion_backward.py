@@ -269,3 +269,35 @@ def test_image_space_objective_of_eq2_end_to_end(gsr, torch_mod):
         pred = float((grads[field].reshape(theta.shape) * delta).sum())
         mag = float(np.abs(grads[field].reshape(theta.shape) * delta).sum())
         assert abs((Lp - Lm) - pred) <= 3e-2 * mag + 2e-2 * abs(pred), (field, Lp - Lm, pred, mag)
+
+
+def test_degenerate_sizes_of_the_backward_calls(gsr, torch_mod):
+    """Empty batches and a one-pixel image through the calls added for the backward: nothing launched or all-zero
+    results, never an error from the device."""
+    torch = torch_mod
+    L, C = gsr.lib(), gsr.C
+    ref = torch.rand((5, 7, 3), device="cuda")
+    e = torch.empty((0, 5, 7, 3), device="cuda")
+    assert gsr.distortion_backward(e, ref, None, 0.20).shape == (0, 5, 7, 3)
+    assert gsr.objective_weights(torch.empty(0, dtype=torch.float64, device="cuda")).numel() == 0
+    one = torch.rand((2, 1, 1, 3), device="cuda")
+    r1 = torch.rand((1, 1, 3), device="cuda")
+    g = gsr.distortion_backward(one, r1, None, 0.20)
+    want = M.distortion_backward(one.cpu().numpy(), r1.cpu().numpy(), np.ones(2), 0.20)
+    assert np.abs(g.cpu().numpy() - want).max() <= 2e-6 * np.abs(want).max()
+    # a batch of zero states through render_backward: the gradient is defined (all zero)
+    wl = synth.scaled_object_workload(29, C=2, per_cluster=30.0, W=48, H=32, fov=40.0, n_frames=1, B=2)
+    cam, t = wl.frames[0]
+    scene = gsr.Scene(wl.scene)
+    ws = scene.new_workspace(cam, 0)
+    lv = torch.empty((0, wl.scene.C), dtype=torch.int8, device="cuda")
+    out, _, _ = scene.render_states(cam, t, lv, workspace=ws)
+    assert out.shape[0] == 0
+    grad = scene.render_backward(ws, out, out)
+    assert float(grad.abs().max()) == 0.0
+    gp = scene.project_backward(cam, t, grad)
+    assert float(gp["gauss"].abs().max()) == 0.0 and float(gp["cluster"].abs().max()) == 0.0
+    gp = scene.project_backward_full(cam, t, grad)
+    assert float(gp["gauss"].abs().max()) == 0.0 and float(gp["delta"].abs().max()) == 0.0
+    scene.close()
+    torch.cuda.synchronize()
